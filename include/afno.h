@@ -1,0 +1,133 @@
+/*
+ * afno.h -- C ABI of the B200-native AFNO spectral token-mixing layer.
+ *
+ * The layer (FourCastNet, arXiv 2208.05419; citations are /root/reference/PAPER.md lines):
+ *   step 1  PAPER.md:114  "An FFT spatially mixes the ... grid of tokens"      (rfft2, ortho)
+ *   step 2  PAPER.md:115-121  "the channels are mixed using a block-diagonal MLP in the
+ *           Fourier space ... MLP weights are shared across tokens"
+ *   step 3  PAPER.md:122  "An inverse FFT demixes the tokens"                  (irfft2, ortho)
+ *   PAPER.md:136  real-to-complex / complex-to-real FFTs batched over batch and features
+ *   PAPER.md:138  weights are real tensors with (re, im) as the fastest index; activations
+ *                 act on real and imaginary parts independently
+ * Bias, ReLU, softshrink(lambda), hard mode truncation by a kept fraction, ortho
+ * normalisation and the residual add are fixed by BASELINE.json:north_star and the
+ * readings A1-A20 in DESIGN.md S3.  In formulas (h,r rows; w columns; c column frequency;
+ * Wh = W/2+1; channel ch = j*bs + i):
+ *
+ *   Xh[b,r,c,ch] = (HW)^-1/2 sum_{h,w} x[b,h,w,ch] exp(-2 pi i (r h/H + c w/W))
+ *   kept (r,c)  <=>  |kappa(r)| < Kh and c < Kw,  kappa(r) = r if r <= H/2 else r-H,
+ *                    Kh = clamp(floor(f (H/2+1)), 1, H/2+1), Kw likewise from W
+ *   P1[o] = sum_i Xh[j*bs+i] W1[j,i,o] + b1[j,o];  O1 = relu(Re P1) + i relu(Im P1)
+ *   P2[o] = sum_i O1[i] W2[j,i,o] + b2[j,o];       Z = S_l(Re P2) + i S_l(Im P2), 0 if not kept
+ *   s[b,h,w,ch] = (HW)^-1/2 sum_{r,c} alpha_c Re(Z[b,r,c,ch] exp(+2 pi i (r h/H + c w/W)))
+ *   y = x + s
+ *
+ * Everything runs on the device in this library's own kernels; there is no CPU fallback.
+ * All entry points are plain C: integers, floats, raw pointers.  Unless a parameter says
+ * "host", every data pointer is a DEVICE pointer on the current CUDA device, 16-byte
+ * aligned, owned by the caller, and must stay valid until the work queued on `cuda_stream`
+ * has completed.  fwd/bwd allocate no device memory, never synchronise the host and are
+ * CUDA-graph capturable once afno_plan_warmup() has run for the descriptor's (H, W).
+ *
+ * Errors: every call returns an afno_status_t; nothing aborts or throws.  A human-readable
+ * reason for the calling thread's last failure is available from afno_last_error().
+ */
+#ifndef AFNO_H
+#define AFNO_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  AFNO_OK = 0,
+  AFNO_ERR_INVALID_ARG = 1, /* null/misaligned/aliased pointer, bad dims, bad lambda/fraction */
+  AFNO_ERR_UNSUPPORTED = 2, /* odd W, H or W with a prime factor > 5, size beyond smem limits */
+  AFNO_ERR_WORKSPACE = 3,   /* workspace smaller than afno_spectral_workspace_bytes()         */
+  AFNO_ERR_CUDA = 4         /* a CUDA runtime call or kernel launch failed                    */
+} afno_status_t;
+
+typedef enum { AFNO_F32 = 0, AFNO_BF16 = 1 } afno_dtype_t; /* dtype of x, y, dy, dx */
+
+enum {
+  AFNO_FLAG_NO_RESIDUAL = 1,     /* test aid: y = s, dx = branch only (no "+ x", no "+ dy")   */
+  AFNO_FLAG_ACCUM_GRADS = 2,     /* dw1, db1, dw2, db2 += instead of =                        */
+  AFNO_FLAG_FORCE_FP32_MATH = 4, /* bf16 I/O but fp32 FFT + fp32 FFMA MLP (generic path)      */
+  AFNO_FLAG_EXPORT_MASKS = 8     /* bwd only: write ReLU / softshrink masks, see below        */
+};
+
+typedef struct {
+  int32_t B, H, W, C;     /* x is [B][H][W][C], channel-last, C fastest                      */
+  int32_t num_blocks;     /* C % num_blocks == 0; bs = C / num_blocks                        */
+  int32_t hidden_factor;  /* hid = bs * hidden_factor, >= 1                                  */
+  float lambda;           /* softshrink threshold, >= 0                                      */
+  float kept_fraction;    /* f in (0,1]; products with it are evaluated in double            */
+  int32_t dtype;          /* afno_dtype_t                                                    */
+  uint32_t flags;         /* AFNO_FLAG_*                                                     */
+} afno_desc_t;
+
+int afno_version(void);
+const char* afno_status_string(int status);
+const char* afno_last_error(void); /* thread-local, valid until the thread's next call */
+
+/* Name of the kernel family the descriptor dispatches to: "generic-fp32" or "tcgen05-bf16".
+ * Returns NULL for an invalid / unsupported descriptor. */
+const char* afno_spectral_path(const afno_desc_t* d);
+
+/* Pure host arithmetic; 0 for an invalid descriptor. */
+size_t afno_spectral_workspace_bytes(const afno_desc_t* d, int for_backward);
+
+/* Sizes in bytes of the two mask arrays written by AFNO_FLAG_EXPORT_MASKS:
+ *   mask1 [B][H][Wh][num_blocks*hid][2] uint8 : 1 where Re/Im P1 > 0      (ReLU passes)
+ *   mask2 [B][H][Wh][C][2]              uint8 : 1 where |Re/Im P2| > lambda and (r,c) kept
+ * They are written at workspace + 0 and workspace + mask1_bytes (rounded up to 256) and
+ * remain valid after afno_spectral_bwd returns (stream order). */
+int afno_spectral_mask_bytes(const afno_desc_t* d, size_t* mask1_bytes, size_t* mask2_offset,
+                             size_t* mask2_bytes);
+
+/* Builds the per-(device, H, W) constant tables (twiddles, digit permutations, DFT
+ * matrices).  Allocates and synchronises: call it outside stream capture.  fwd/bwd call it
+ * implicitly on first use when the stream is not capturing. */
+int afno_plan_warmup(const afno_desc_t* d);
+
+/* Forward.  x, y: [B][H][W][C] of d->dtype; y must not alias x.
+ * w1 [nb][bs][hid][2], b1 [nb][hid][2], w2 [nb][hid][bs][2], b2 [nb][bs][2]: fp32,
+ * out[o] = sum_i in[i] * w[j][i][o] (row vector times matrix), (re, im) fastest. */
+int afno_spectral_fwd(const afno_desc_t* d, const void* x, const float* w1, const float* b1,
+                      const float* w2, const float* b2, void* y, void* workspace,
+                      size_t workspace_bytes, void* cuda_stream);
+
+/* Backward (stateless: recomputes the forward spectrum from x).  dy, dx like x; dx must not
+ * alias dy or x.  dw1, db1, dw2, db2: fp32, shapes of the parameters, gradients with respect
+ * to the real storage (dW = dL/dRe W + i dL/dIm W = sum conj(in) * g).  Sums over samples
+ * and modes are evaluated in a fixed order: two calls give bit-identical results. */
+int afno_spectral_bwd(const afno_desc_t* d, const void* x, const void* dy, const float* w1,
+                      const float* b1, const float* w2, const float* b2, void* dx, float* dw1,
+                      float* db1, float* dw2, float* db2, void* workspace,
+                      size_t workspace_bytes, void* cuda_stream);
+
+/* End-to-end variants with HOST buffers (pinned memory recommended).  `arena` is a device
+ * scratch buffer of at least afno_spectral_host_arena_bytes(); the calls copy the inputs
+ * host->device, run the device path above, copy the results device->host on `cuda_stream`
+ * and synchronise that stream before returning.  Every *_host pointer is a host pointer. */
+size_t afno_spectral_host_arena_bytes(const afno_desc_t* d, int for_backward);
+int afno_spectral_fwd_host(const afno_desc_t* d, const void* x_host, const float* w1_host,
+                           const float* b1_host, const float* w2_host, const float* b2_host,
+                           void* y_host, void* arena, size_t arena_bytes, void* cuda_stream);
+int afno_spectral_bwd_host(const afno_desc_t* d, const void* x_host, const void* dy_host,
+                           const float* w1_host, const float* b1_host, const float* w2_host,
+                           const float* b2_host, void* dx_host, float* dw1_host,
+                           float* db1_host, float* dw2_host, float* db2_host, void* arena,
+                           size_t arena_bytes, void* cuda_stream);
+
+/* Number of kernel launches the last fwd / bwd call of this thread enqueued (bench.py's
+ * "gpu_launches" is counted from this, not guessed). */
+int afno_last_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AFNO_H */

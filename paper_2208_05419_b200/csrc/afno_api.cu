@@ -1,0 +1,405 @@
+// C ABI of libafno_b200.so (include/afno.h): descriptor validation, plan cache, dispatch.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "afno_internal.h"
+
+namespace afno {
+
+namespace {
+
+thread_local std::string t_error;
+thread_local int t_launches = 0;
+
+int fail(int status, const std::string& msg) {
+  t_error = msg;
+  return status;
+}
+
+bool smooth235(int n, std::vector<int>* radices) {
+  if (n < 1) return false;
+  std::vector<int> r;
+  while (n % 4 == 0) { r.push_back(4); n /= 4; }
+  while (n % 2 == 0) { r.push_back(2); n /= 2; }
+  while (n % 3 == 0) { r.push_back(3); n /= 3; }
+  while (n % 5 == 0) { r.push_back(5); n /= 5; }
+  if (n != 1) return false;
+  if (radices) *radices = r;
+  return true;
+}
+
+// Validates d and fills g.  Returns AFNO_OK or an error status (message set).
+int resolve(const afno_desc_t* d, Geometry* g) {
+  if (!d) return fail(AFNO_ERR_INVALID_ARG, "descriptor is NULL");
+  if (d->B <= 0 || d->H <= 0 || d->W <= 0 || d->C <= 0)
+    return fail(AFNO_ERR_INVALID_ARG, "B, H, W, C must be positive");
+  if (d->num_blocks <= 0 || d->C % d->num_blocks != 0)
+    return fail(AFNO_ERR_INVALID_ARG, "num_blocks must be positive and divide C");
+  if (d->hidden_factor < 1) return fail(AFNO_ERR_INVALID_ARG, "hidden_factor must be >= 1");
+  if (!(d->lambda >= 0.f) || isinf(d->lambda)) return fail(AFNO_ERR_INVALID_ARG, "lambda must be finite and >= 0");
+  if (!(d->kept_fraction > 0.f && d->kept_fraction <= 1.f))
+    return fail(AFNO_ERR_INVALID_ARG, "kept_fraction must be in (0, 1]");
+  if (d->dtype != AFNO_F32 && d->dtype != AFNO_BF16) return fail(AFNO_ERR_INVALID_ARG, "unknown dtype");
+  if (d->flags & ~(uint32_t)(AFNO_FLAG_NO_RESIDUAL | AFNO_FLAG_ACCUM_GRADS | AFNO_FLAG_FORCE_FP32_MATH |
+                             AFNO_FLAG_EXPORT_MASKS))
+    return fail(AFNO_ERR_INVALID_ARG, "unknown flag bits");
+  if ((long long)d->B * d->H * d->W >= (1LL << 31) / 4)
+    return fail(AFNO_ERR_UNSUPPORTED, "B*H*W too large for 32-bit token indexing");
+  if (d->W % 2 != 0) return fail(AFNO_ERR_UNSUPPORTED, "odd W is not supported on the GPU path");
+  if (!smooth235(d->H, nullptr) || !smooth235(d->W, nullptr))
+    return fail(AFNO_ERR_UNSUPPORTED, "H and W must have no prime factor larger than 5");
+  g->B = d->B; g->H = d->H; g->W = d->W; g->C = d->C;
+  g->nb = d->num_blocks;
+  g->bs = d->C / d->num_blocks;
+  g->hid = g->bs * d->hidden_factor;
+  g->CH = g->nb * g->hid;
+  g->Wh = d->W / 2 + 1;
+  // readings A7/A8: box of low |wavenumber|, floor, clamped to >= 1; product in double
+  const double f = (double)d->kept_fraction;
+  const int nh = d->H / 2 + 1;
+  int kh = (int)floor(f * (double)nh), kw = (int)floor(f * (double)g->Wh);
+  g->Kh = kh < 1 ? 1 : (kh > nh ? nh : kh);
+  g->Kw = kw < 1 ? 1 : (kw > g->Wh ? g->Wh : kw);
+  g->lambda = d->lambda;
+  g->scale = (float)(1.0 / sqrt((double)d->H * (double)d->W));
+  g->bf16 = d->dtype == AFNO_BF16;
+  g->no_residual = (d->flags & AFNO_FLAG_NO_RESIDUAL) != 0;
+  g->accum = (d->flags & AFNO_FLAG_ACCUM_GRADS) != 0;
+  g->export_masks = (d->flags & AFNO_FLAG_EXPORT_MASKS) != 0;
+  const char* why = nullptr;
+  if (!generic_supported(*g, &why)) return fail(AFNO_ERR_UNSUPPORTED, why);
+  return AFNO_OK;
+}
+
+// ---- plan cache ------------------------------------------------------------------------
+std::mutex g_plan_mutex;
+std::vector<Plan*> g_plans;
+
+cudaError_t build_fft_plan(int n, FftPlan* out) {
+  std::vector<int> radices;
+  smooth235(n, &radices);
+  if ((int)radices.size() > kMaxStages) return cudaErrorInvalidValue;
+  memset(out, 0, sizeof(*out));
+  out->n = n;
+  out->nstages = (int)radices.size();
+  for (size_t i = 0; i < radices.size(); ++i) out->radix[i] = radices[i];
+  std::vector<float2> tw(n);
+  const double two_pi = 6.283185307179586476925286766559;
+  for (int k = 0; k < n; ++k) {
+    const double a = -two_pi * (double)k / (double)n;
+    tw[k] = make_float2((float)cos(a), (float)sin(a));
+  }
+  // DIF output order: bin k sits at sum_s (k_s * n / (r_1 ... r_s)), k = k_1 + r_1 (k_2 + r_2 (...))
+  std::vector<int16_t> perm(n);
+  for (int k = 0; k < n; ++k) {
+    int kk = k, L = n, pos = 0;
+    for (int r : radices) {
+      const int m = L / r;
+      pos += (kk % r) * m;
+      kk /= r;
+      L = m;
+    }
+    perm[k] = (int16_t)pos;
+  }
+  float2* dtw = nullptr;
+  int16_t* dperm = nullptr;
+  cudaError_t e = cudaMalloc(&dtw, sizeof(float2) * n);
+  if (e != cudaSuccess) return e;
+  e = cudaMalloc(&dperm, sizeof(int16_t) * n);
+  if (e != cudaSuccess) return e;
+  e = cudaMemcpy(dtw, tw.data(), sizeof(float2) * n, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) return e;
+  e = cudaMemcpy(dperm, perm.data(), sizeof(int16_t) * n, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) return e;
+  out->tw = dtw;
+  out->perm = dperm;
+  return cudaSuccess;
+}
+
+// Returns the plan for (current device, H, W); builds it when allowed.
+int get_plan(const Geometry& g, bool may_build, const Plan** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail(AFNO_ERR_CUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e));
+  std::lock_guard<std::mutex> lock(g_plan_mutex);
+  for (Plan* p : g_plans)
+    if (p->device == dev && p->H == g.H && p->W == g.W) {
+      *out = p;
+      return AFNO_OK;
+    }
+  if (!may_build)
+    return fail(AFNO_ERR_INVALID_ARG, "stream is capturing and no plan exists: call afno_plan_warmup first");
+  Plan* p = new Plan();
+  p->device = dev;
+  p->H = g.H;
+  p->W = g.W;
+  e = build_fft_plan(g.H, &p->fh);
+  if (e == cudaSuccess) e = build_fft_plan(g.W, &p->fw);
+  if (e != cudaSuccess) {
+    delete p;
+    return fail(AFNO_ERR_CUDA, std::string("plan creation: ") + cudaGetErrorString(e));
+  }
+  g_plans.push_back(p);
+  *out = p;
+  return AFNO_OK;
+}
+
+bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
+
+bool overlaps(const void* a, const void* b, size_t bytes) {
+  const char* pa = (const char*)a;
+  const char* pb = (const char*)b;
+  return pa < pb + bytes && pb < pa + bytes;
+}
+
+int stream_may_build(cudaStream_t st, bool* may_build) {
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  cudaError_t e = cudaStreamIsCapturing(st, &cs);
+  if (e != cudaSuccess) return fail(AFNO_ERR_CUDA, std::string("cudaStreamIsCapturing: ") + cudaGetErrorString(e));
+  *may_build = cs == cudaStreamCaptureStatusNone;
+  return AFNO_OK;
+}
+
+size_t act_bytes(const Geometry& g) {
+  return (size_t)g.B * g.H * g.W * g.C * (g.bf16 ? 2 : 4);
+}
+
+} // namespace
+
+void count_launch(int n) { t_launches += n; }
+
+} // namespace afno
+
+using namespace afno;
+
+extern "C" {
+
+int afno_version(void) { return 100; }
+
+const char* afno_status_string(int status) {
+  switch (status) {
+    case AFNO_OK: return "ok";
+    case AFNO_ERR_INVALID_ARG: return "invalid argument";
+    case AFNO_ERR_UNSUPPORTED: return "unsupported configuration";
+    case AFNO_ERR_WORKSPACE: return "workspace too small";
+    case AFNO_ERR_CUDA: return "CUDA error";
+    default: return "unknown status";
+  }
+}
+
+const char* afno_last_error(void) { return t_error.c_str(); }
+
+int afno_last_launch_count(void) { return t_launches; }
+
+const char* afno_spectral_path(const afno_desc_t* d) {
+  Geometry g;
+  if (resolve(d, &g) != AFNO_OK) return nullptr;
+  return "generic-fp32";
+}
+
+size_t afno_spectral_workspace_bytes(const afno_desc_t* d, int for_backward) {
+  Geometry g;
+  if (resolve(d, &g) != AFNO_OK) return 0;
+  return generic_workspace_bytes(g, for_backward != 0);
+}
+
+int afno_spectral_mask_bytes(const afno_desc_t* d, size_t* mask1_bytes, size_t* mask2_offset,
+                             size_t* mask2_bytes) {
+  Geometry g;
+  int rc = resolve(d, &g);
+  if (rc != AFNO_OK) return rc;
+  const size_t b1 = (size_t)g.modes_all() * g.CH * 2, b2 = (size_t)g.modes_all() * g.C * 2;
+  if (mask1_bytes) *mask1_bytes = b1;
+  if (mask2_offset) *mask2_offset = align_up(b1, 256);
+  if (mask2_bytes) *mask2_bytes = b2;
+  return AFNO_OK;
+}
+
+int afno_plan_warmup(const afno_desc_t* d) {
+  Geometry g;
+  int rc = resolve(d, &g);
+  if (rc != AFNO_OK) return rc;
+  const Plan* p = nullptr;
+  return get_plan(g, true, &p);
+}
+
+int afno_spectral_fwd(const afno_desc_t* d, const void* x, const float* w1, const float* b1,
+                      const float* w2, const float* b2, void* y, void* workspace,
+                      size_t workspace_bytes, void* cuda_stream) {
+  t_launches = 0;
+  Geometry g;
+  int rc = resolve(d, &g);
+  if (rc != AFNO_OK) return rc;
+  if (!x || !w1 || !b1 || !w2 || !b2 || !y || !workspace) return fail(AFNO_ERR_INVALID_ARG, "NULL pointer argument");
+  const void* ptrs[] = {x, w1, b1, w2, b2, y, workspace};
+  for (const void* p : ptrs)
+    if (!aligned16(p)) return fail(AFNO_ERR_INVALID_ARG, "pointers must be 16-byte aligned");
+  if (overlaps(x, y, act_bytes(g))) return fail(AFNO_ERR_INVALID_ARG, "y must not alias x");
+  if (workspace_bytes < generic_workspace_bytes(g, false))
+    return fail(AFNO_ERR_WORKSPACE, "workspace smaller than afno_spectral_workspace_bytes(d, 0)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  bool may_build = false;
+  rc = stream_may_build(st, &may_build);
+  if (rc != AFNO_OK) return rc;
+  const Plan* p = nullptr;
+  rc = get_plan(g, may_build, &p);
+  if (rc != AFNO_OK) return rc;
+  cudaError_t e = generic_forward(g, *p, x, w1, b1, w2, b2, y, workspace, st);
+  if (e != cudaSuccess) return fail(AFNO_ERR_CUDA, std::string("forward launch: ") + cudaGetErrorString(e));
+  return AFNO_OK;
+}
+
+int afno_spectral_bwd(const afno_desc_t* d, const void* x, const void* dy, const float* w1,
+                      const float* b1, const float* w2, const float* b2, void* dx, float* dw1,
+                      float* db1, float* dw2, float* db2, void* workspace,
+                      size_t workspace_bytes, void* cuda_stream) {
+  t_launches = 0;
+  Geometry g;
+  int rc = resolve(d, &g);
+  if (rc != AFNO_OK) return rc;
+  if (!x || !dy || !w1 || !b1 || !w2 || !b2 || !dx || !dw1 || !db1 || !dw2 || !db2 || !workspace)
+    return fail(AFNO_ERR_INVALID_ARG, "NULL pointer argument");
+  const void* ptrs[] = {x, dy, w1, b1, w2, b2, dx, dw1, db1, dw2, db2, workspace};
+  for (const void* p : ptrs)
+    if (!aligned16(p)) return fail(AFNO_ERR_INVALID_ARG, "pointers must be 16-byte aligned");
+  if (overlaps(dx, dy, act_bytes(g)) || overlaps(dx, x, act_bytes(g)))
+    return fail(AFNO_ERR_INVALID_ARG, "dx must not alias dy or x");
+  if (workspace_bytes < generic_workspace_bytes(g, true))
+    return fail(AFNO_ERR_WORKSPACE, "workspace smaller than afno_spectral_workspace_bytes(d, 1)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  bool may_build = false;
+  rc = stream_may_build(st, &may_build);
+  if (rc != AFNO_OK) return rc;
+  const Plan* p = nullptr;
+  rc = get_plan(g, may_build, &p);
+  if (rc != AFNO_OK) return rc;
+  size_t m1 = 0, m2off = 0, m2 = 0;
+  afno_spectral_mask_bytes(d, &m1, &m2off, &m2);
+  cudaError_t e = generic_backward(g, *p, x, dy, w1, b1, w2, b2, dx, dw1, db1, dw2, db2, workspace, m1, m2off, st);
+  if (e != cudaSuccess) return fail(AFNO_ERR_CUDA, std::string("backward launch: ") + cudaGetErrorString(e));
+  return AFNO_OK;
+}
+
+// ---- host-buffer (end-to-end) variants ---------------------------------------------------
+namespace {
+struct Arena {
+  char* base;
+  size_t off = 0;
+  void* take(size_t bytes) {
+    void* p = base ? base + off : nullptr;
+    off = align_up(off + bytes, 256);
+    return p;
+  }
+};
+struct HostLayout {
+  void *x, *dy, *y, *dx;
+  float *w1, *b1, *w2, *b2, *dw1, *db1, *dw2, *db2;
+  void* ws;
+  size_t ws_bytes, total, act, nw, nb1, nb2;
+};
+HostLayout host_layout(const afno_desc_t* d, const Geometry& g, bool backward, char* base) {
+  HostLayout h{};
+  Arena a{base};
+  h.act = act_bytes(g);
+  h.nw = (size_t)g.nb * g.bs * g.hid * 2 * sizeof(float);
+  h.nb1 = (size_t)g.nb * g.hid * 2 * sizeof(float);
+  h.nb2 = (size_t)g.nb * g.bs * 2 * sizeof(float);
+  h.x = a.take(h.act);
+  h.w1 = (float*)a.take(h.nw);
+  h.b1 = (float*)a.take(h.nb1);
+  h.w2 = (float*)a.take(h.nw);
+  h.b2 = (float*)a.take(h.nb2);
+  if (backward) {
+    h.dy = a.take(h.act);
+    h.dx = a.take(h.act);
+    h.dw1 = (float*)a.take(h.nw);
+    h.db1 = (float*)a.take(h.nb1);
+    h.dw2 = (float*)a.take(h.nw);
+    h.db2 = (float*)a.take(h.nb2);
+  } else {
+    h.y = a.take(h.act);
+  }
+  h.ws_bytes = afno_spectral_workspace_bytes(d, backward ? 1 : 0);
+  h.ws = a.take(h.ws_bytes);
+  h.total = a.off;
+  return h;
+}
+} // namespace
+
+size_t afno_spectral_host_arena_bytes(const afno_desc_t* d, int for_backward) {
+  Geometry g;
+  if (resolve(d, &g) != AFNO_OK) return 0;
+  return host_layout(d, g, for_backward != 0, nullptr).total;
+}
+
+#define AFNO_CUDA_TRY(expr)                                                                     \
+  do {                                                                                          \
+    cudaError_t e_ = (expr);                                                                    \
+    if (e_ != cudaSuccess) return fail(AFNO_ERR_CUDA, std::string(#expr ": ") + cudaGetErrorString(e_)); \
+  } while (0)
+
+int afno_spectral_fwd_host(const afno_desc_t* d, const void* x_host, const float* w1_host,
+                           const float* b1_host, const float* w2_host, const float* b2_host,
+                           void* y_host, void* arena, size_t arena_bytes, void* cuda_stream) {
+  Geometry g;
+  int rc = resolve(d, &g);
+  if (rc != AFNO_OK) return rc;
+  if (!x_host || !w1_host || !b1_host || !w2_host || !b2_host || !y_host || !arena)
+    return fail(AFNO_ERR_INVALID_ARG, "NULL pointer argument");
+  if (!aligned16(arena)) return fail(AFNO_ERR_INVALID_ARG, "arena must be 16-byte aligned");
+  HostLayout h = host_layout(d, g, false, (char*)arena);
+  if (arena_bytes < h.total) return fail(AFNO_ERR_WORKSPACE, "arena smaller than afno_spectral_host_arena_bytes(d, 0)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.x, x_host, h.act, cudaMemcpyHostToDevice, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w1, w1_host, h.nw, cudaMemcpyHostToDevice, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b1, b1_host, h.nb1, cudaMemcpyHostToDevice, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w2, w2_host, h.nw, cudaMemcpyHostToDevice, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b2, b2_host, h.nb2, cudaMemcpyHostToDevice, st));
+  rc = afno_spectral_fwd(d, h.x, h.w1, h.b1, h.w2, h.b2, h.y, h.ws, h.ws_bytes, cuda_stream);
+  if (rc != AFNO_OK) return rc;
+  AFNO_CUDA_TRY(cudaMemcpyAsync(y_host, h.y, h.act, cudaMemcpyDeviceToHost, st));
+  AFNO_CUDA_TRY(cudaStreamSynchronize(st));
+  return AFNO_OK;
+}
+
+int afno_spectral_bwd_host(const afno_desc_t* d, const void* x_host, const void* dy_host,
+                           const float* w1_host, const float* b1_host, const float* w2_host,
+                           const float* b2_host, void* dx_host, float* dw1_host,
+                           float* db1_host, float* dw2_host, float* db2_host, void* arena,
+                           size_t arena_bytes, void* cuda_stream) {
+  Geometry g;
+  int rc = resolve(d, &g);
+  if (rc != AFNO_OK) return rc;
+  if (!x_host || !dy_host || !w1_host || !b1_host || !w2_host || !b2_host || !dx_host || !dw1_host ||
+      !db1_host || !dw2_host || !db2_host || !arena)
+    return fail(AFNO_ERR_INVALID_ARG, "NULL pointer argument");
+  if (d->flags & AFNO_FLAG_ACCUM_GRADS)
+    return fail(AFNO_ERR_INVALID_ARG, "AFNO_FLAG_ACCUM_GRADS is not meaningful for the host variant");
+  if (!aligned16(arena)) return fail(AFNO_ERR_INVALID_ARG, "arena must be 16-byte aligned");
+  HostLayout h = host_layout(d, g, true, (char*)arena);
+  if (arena_bytes < h.total) return fail(AFNO_ERR_WORKSPACE, "arena smaller than afno_spectral_host_arena_bytes(d, 1)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.x, x_host, h.act, cudaMemcpyHostToDevice, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.dy, dy_host, h.act, cudaMemcpyHostToDevice, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w1, w1_host, h.nw, cudaMemcpyHostToDevice, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b1, b1_host, h.nb1, cudaMemcpyHostToDevice, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w2, w2_host, h.nw, cudaMemcpyHostToDevice, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b2, b2_host, h.nb2, cudaMemcpyHostToDevice, st));
+  rc = afno_spectral_bwd(d, h.x, h.dy, h.w1, h.b1, h.w2, h.b2, h.dx, h.dw1, h.db1, h.dw2, h.db2, h.ws,
+                         h.ws_bytes, cuda_stream);
+  if (rc != AFNO_OK) return rc;
+  AFNO_CUDA_TRY(cudaMemcpyAsync(dx_host, h.dx, h.act, cudaMemcpyDeviceToHost, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(dw1_host, h.dw1, h.nw, cudaMemcpyDeviceToHost, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(db1_host, h.db1, h.nb1, cudaMemcpyDeviceToHost, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(dw2_host, h.dw2, h.nw, cudaMemcpyDeviceToHost, st));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(db2_host, h.db2, h.nb2, cudaMemcpyDeviceToHost, st));
+  AFNO_CUDA_TRY(cudaStreamSynchronize(st));
+  return AFNO_OK;
+}
+
+} // extern "C"

@@ -1,0 +1,55 @@
+// Internal declarations shared by the translation units of libafno_b200.so.
+// Nothing here is part of the C ABI (include/afno.h) and nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/afno.h"
+
+namespace afno {
+
+constexpr int kMaxStages = 16;
+
+// One 1-D FFT plan: in-place decimation-in-frequency, output bin k lands at perm[k].
+struct FftPlan {
+  int n;
+  int nstages;
+  int radix[kMaxStages];
+  const float2* tw;    // device: tw[k] = exp(-2 pi i k / n), rounded from fp64
+  const int16_t* perm; // device: position of output bin k after the last stage
+};
+
+// Resolved problem geometry (host side), derived once per call from afno_desc_t.
+struct Geometry {
+  int B, H, W, C, nb, bs, hid, CH; // CH = nb * hid
+  int Wh, Kh, Kw;
+  float lambda;
+  float scale; // 1/sqrt(H*W)
+  bool bf16, no_residual, accum, export_masks;
+  long long modes_all() const { return (long long)B * H * Wh; }
+  long long rows() const { return (long long)B * H * Kw; } // rows of the stored spectra
+};
+
+struct Plan {
+  int device, H, W;
+  FftPlan fh, fw;
+};
+
+// launch accounting (thread-local, reported through afno_last_launch_count)
+void count_launch(int n = 1);
+
+// ---- generic fp32-math path (generic.cu) -------------------------------------------
+size_t generic_workspace_bytes(const Geometry& g, bool backward);
+cudaError_t generic_forward(const Geometry& g, const Plan& p, const void* x, const float* w1,
+                            const float* b1, const float* w2, const float* b2, void* y,
+                            void* ws, cudaStream_t st);
+cudaError_t generic_backward(const Geometry& g, const Plan& p, const void* x, const void* dy,
+                             const float* w1, const float* b1, const float* w2, const float* b2,
+                             void* dx, float* dw1, float* db1, float* dw2, float* db2, void* ws,
+                             size_t mask1_bytes, size_t mask2_offset, cudaStream_t st);
+bool generic_supported(const Geometry& g, const char** why);
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+} // namespace afno

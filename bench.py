@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""bench.py -- AFNO spectral layer fwd+bwd samples/s at 90x180x768 bf16 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (afno_spectral_fwd then afno_spectral_bwd, i.e.
+every row F1-F9 and B1-B8 of DESIGN.md S1) over one batch of synthetic FourCastNet-shaped
+activations.  Workload: BASELINE.json configs[4] (B=4, 90x180x768, 8 blocks of 96, bf16,
+lambda 0.01, kept fraction 1.0).  Prints ONE JSON line (contract in the task prompt).
+
+N > 1: the path does not shard ("replicas only", S6): every rank runs an
+independent replica on its own GPU, no data-path collective; value = all ranks' samples /
+max-over-ranks device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "afno_spectral_fwd_bwd_samples_per_s_90x180x768_bf16"
+UNIT = "samples/s"
+WL_NAME = "fcn_b4_bwd"
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(hbm_gbs=float(p["hbm_gbs"]), tensor_tflops=float(p["bf16_tflops"]),
+                    tensor_tflops_sustained=float(p.get("bf16_tflops_sustained", p["bf16_tflops"])),
+                    sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, tensor_tflops=1590.0, tensor_tflops_sustained=1400.0, sm_max_mhz=1965.0,
+                source="fallback")
+
+
+def layer_work(B, H, W, C, nb, kept_modes):
+    """Algorithmic work of one fwd+bwd step (S5): compulsory HBM bytes and model MLP FLOPs."""
+    act = B * H * W * C * 2                                  # one bf16 activation tensor
+    params = 2 * (nb * (C // nb) ** 2 * 2 + C * 2) * 4       # w1,b1,w2,b2 fp32
+    bytes_fwd = 2 * act + params                             # x in, y out
+    bytes_bwd = 3 * act + 2 * params                         # x, dy in, dx out; params in, grads out
+    bs = C // nb
+    gemm = 2 * (2 * bs) * (2 * bs) * nb * kept_modes * B     # one complex block GEMM over all modes
+    flops_fwd = 2 * gemm                                     # F3, F5
+    flops_bwd_model = 4 * gemm                               # B4, B5, B6, B7
+    flops_bwd_exec = 6 * gemm                                # + recompute of F3, F5
+    return dict(bytes=bytes_fwd + bytes_bwd, flops_model=flops_fwd + flops_bwd_model,
+                flops_exec=flops_fwd + flops_bwd_exec)
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.02)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons)}
+
+
+def oracle_time(n_samples: int):
+    """Times the fp64 CPU oracle (as it stands) fwd+bwd on n_samples samples of the workload."""
+    from oracle import afno_oracle
+    from paper_2208_05419_b200 import inputs
+    wl = inputs.WORKLOADS[WL_NAME]
+    d = inputs.make_inputs(wl, B=n_samples)
+    cfg = afno_oracle.Config(n_samples, wl.H, wl.W, wl.C, wl.num_blocks, lam=float(np.float32(wl.lam)),
+                             kept_fraction=wl.kept_fraction)
+    afno_oracle.lib()
+    t0 = time.perf_counter()
+    afno_oracle.forward(cfg, d["x"], d["w1"], d["b1"], d["w2"], d["b2"])
+    afno_oracle.backward(cfg, d["x"], d["dy"], d["w1"], d["b1"], d["w2"], d["b2"])
+    dt = time.perf_counter() - t0
+    return n_samples / dt, dt, afno_oracle.num_threads()
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric/config, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2208_05419_b200 import inputs
+    wl = inputs.WORKLOADS[WL_NAME]
+    steps = max(1, args.steps)
+    for _ in range(min(args.warmup, 1)):
+        oracle_time(1)
+    tot_s, tot_t, cores = 0, 0.0, 0
+    for _ in range(steps):
+        v, dt, cores = oracle_time(1)
+        tot_s += 1
+        tot_t += dt
+    value = tot_s / tot_t
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * tot_t / steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[4]: {wl.name}; one sample per step (bounded sample)",
+                   "H": wl.H, "W": wl.W, "C": wl.C, "num_blocks": wl.num_blocks, "lambda": wl.lam,
+                   "kept_fraction": wl.kept_fraction},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"{steps} x (1 sample fwd+bwd at 90x180x768, fp64, mixed-radix FFT mode)"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+
+    from paper_2208_05419_b200 import binding, inputs
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the AFNO path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    wl = inputs.WORKLOADS[WL_NAME]
+    B = wl.B
+    desc = binding.Desc(B, wl.H, wl.W, wl.C, wl.num_blocks, wl.hidden_factor, wl.lam, wl.kept_fraction,
+                        binding.AFNO_BF16, 0)
+    binding.afno_plan_warmup(desc)
+    path = binding.afno_spectral_path(desc)
+    peaks = _peaks()
+
+    # --- inputs resident in HBM; rotate NSETS disjoint buffer sets so reads are cold -------
+    data = inputs.make_inputs(wl)
+    NSETS = 3
+    dev = torch.device("cuda", local_rank)
+    to_bf16 = lambda a: torch.from_numpy(a).to(dev).to(torch.bfloat16)
+    x0, dy0 = to_bf16(data["x"]), to_bf16(data["dy"])
+    sets = []
+    for s in range(NSETS):
+        # distinct data per set (a roll along the batch axis keeps the statistics)
+        sets.append(dict(x=torch.roll(x0, s, 0).contiguous(), dy=torch.roll(dy0, s, 0).contiguous(),
+                         y=torch.empty_like(x0), dx=torch.empty_like(x0)))
+    params = [torch.from_numpy(data[k]).to(dev) for k in ("w1", "b1", "w2", "b2")]
+    grads = [torch.empty_like(p) for p in params]
+    ws_f = torch.empty(binding.afno_spectral_workspace_bytes(desc, False), dtype=torch.uint8, device=dev)
+    ws_b = torch.empty(binding.afno_spectral_workspace_bytes(desc, True), dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    launches = [0]
+
+    def step(i):
+        s = sets[i % NSETS]
+        binding.afno_spectral_fwd(desc, s["x"], *params, s["y"], ws_f, stream)
+        n = binding.afno_last_launch_count()
+        binding.afno_spectral_bwd(desc, s["x"], s["dy"], *params, s["dx"], *grads, ws_b, stream)
+        launches[0] = n + binding.afno_last_launch_count()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for i in range(args.warmup):
+        step(i)
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        ev0.record(stream)
+        for i in range(args.steps):
+            step(i)
+        ev1.record(stream)
+        barrier()
+    ms = ev0.elapsed_time(ev1)
+    if dist is not None:
+        t = torch.tensor([ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_per_step = ms / args.steps
+    value = world * B * args.steps / (ms * 1e-3)
+
+    # --- per-kernel durations, measured live with CUDA events around every launch -----------
+    binding.afno_profile_start()
+    PROF_STEPS = max(2, min(args.steps, 5))
+    for i in range(PROF_STEPS):
+        step(i)
+    prof = binding.afno_profile_stop()
+    total_prof_ms = sum(v[1] for v in prof.values())
+    dom = max(prof, key=lambda k: prof[k][1])
+    dom_n, dom_ms = prof[dom]
+    kept_modes = None
+    Kh = max(1, min(wl.H // 2 + 1, int(np.floor(float(np.float32(wl.kept_fraction)) * (wl.H // 2 + 1)))))
+    Kw = max(1, min(wl.W // 2 + 1, int(np.floor(float(np.float32(wl.kept_fraction)) * (wl.W // 2 + 1)))))
+    kept_modes = (2 * Kh - 1 if Kh <= wl.H // 2 else wl.H) * Kw
+    work = layer_work(B, wl.H, wl.W, wl.C, wl.num_blocks, kept_modes)
+    roofline = kernel_roofline(dom, dom_n, dom_ms, PROF_STEPS, work, peaks, clocks.summary(), B, wl, kept_modes)
+    roofline["share_of_step"] = dom_ms / total_prof_ms if total_prof_ms > 0 else None
+    roofline["kernels_ms_per_step"] = {k: round(v[1] / PROF_STEPS, 4) for k, v in sorted(prof.items())}
+
+    # --- whole-layer 2-term roofline of BASELINE.json's metric ---------------------------------
+    t_hbm = work["bytes"] / (peaks["hbm_gbs"] * 1e9)
+    t_tensor = work["flops_model"] / (peaks["tensor_tflops"] * 1e12)
+    t_roof = max(t_hbm, t_tensor)
+    layer = {"bound": "hbm" if t_hbm >= t_tensor else "tensor", "t_roof_us_per_step": 1e6 * t_roof,
+             "frac": t_roof / (ms_per_step * 1e-3), "bytes_per_step": work["bytes"],
+             "mlp_flops_model_per_step": work["flops_model"], "mlp_flops_executed_per_step": work["flops_exec"],
+             "achieved_tbs": work["bytes"] / (ms_per_step * 1e-3) / 1e12,
+             "achieved_tflops_model": work["flops_model"] / (ms_per_step * 1e-3) / 1e12,
+             "peaks": f"{peaks['hbm_gbs']} GB/s, {peaks['tensor_tflops']} TFLOP/s bf16 burst ({peaks['source']})"}
+
+    # --- end to end through the C ABI with HOST buffers -----------------------------------------
+    e2e = None
+    if rank == 0 or world > 1:
+        pin = lambda t: t.cpu().pin_memory()
+        hx, hdy = pin(x0), pin(dy0)
+        hp = [pin(p) for p in params]
+        hy, hdx = torch.empty_like(hx).pin_memory(), torch.empty_like(hx).pin_memory()
+        hg = [torch.empty_like(p).pin_memory() for p in hp]
+        arena = torch.empty(max(binding.afno_spectral_host_arena_bytes(desc, False),
+                                binding.afno_spectral_host_arena_bytes(desc, True)), dtype=torch.uint8, device=dev)
+        act = hx.numel() * 2
+        pbytes = sum(p.numel() * 4 for p in hp)
+        E2E_STEPS = max(1, min(args.steps, 5))
+
+        def host_step():
+            binding.afno_spectral_fwd_host(desc, hx, *hp, hy, arena, stream)
+            binding.afno_spectral_bwd_host(desc, hx, hdy, *hp, hdx, *hg, arena, stream)
+
+        host_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(E2E_STEPS):
+            host_step()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * B * E2E_STEPS / dt, "unit": UNIT,
+               "h2d_bytes_per_step": 3 * act + 2 * pbytes, "d2h_bytes_per_step": 2 * act + pbytes,
+               "steps": E2E_STEPS, "note": "afno_spectral_fwd_host + afno_spectral_bwd_host, pinned host buffers"}
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, dt, cores = oracle_time(2)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                        "sample": f"2 samples fwd+bwd at 90x180x768 (fp64 oracle, mixed-radix FFT mode), {dt:.1f} s"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[4]: {wl.name}", "B_per_gpu": B, "H": wl.H, "W": wl.W,
+                       "C": wl.C, "num_blocks": wl.num_blocks, "lambda": wl.lam, "kept_fraction": wl.kept_fraction,
+                       "path": path, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": f"{NSETS} rotating input/output buffer sets of {4 * x0.numel() * 2 / 1e6:.0f} MB "
+                             "each (> 126 MB L2), no explicit flush"},
+            "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches[0] * args.steps,
+            "roofline": roofline, "layer_roofline": layer, "cpu_baseline": cpu_baseline,
+        }
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def kernel_roofline(name, n_launch, total_ms, steps, work, peaks, clocks, B, wl, kept_modes):
+    """roofline object for the dominant kernel (S5 states the per-launch figures)."""
+    per_launch_s = total_ms * 1e-3 / n_launch
+    bs = wl.C // wl.num_blocks
+    rows = B * kept_modes
+    if name in ("k_block_gemm", "k_block_wgrad"):
+        # fp32 FFMA complex block GEMM: 8 real FLOPs per complex MAC, rows x nb x bs x bs complex MACs
+        flops = 8.0 * rows * wl.num_blocks * bs * bs
+        sm_mhz = clocks.get("sm_mhz") or peaks["sm_max_mhz"]
+        peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12   # fp32 FMA peak at max clock, TFLOP/s
+        ach = flops / per_launch_s / 1e12
+        return {"kernel": name, "bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                "frac": ach / peak, "traffic": None,
+                "note": f"fp32 FFMA peak = 148 SM x 128 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz "
+                        f"(DESIGN.md S5); sm clock under load {sm_mhz}"}
+    # streaming FFT kernels: activation tensor in + spectrum out (or the reverse)
+    act = B * wl.H * wl.W * wl.C * 2
+    spec = B * wl.H * (wl.W // 2 + 1) * wl.C * 8
+    nbytes = act + spec
+    ach = nbytes / per_launch_s / 1e9
+    return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+            "frac": ach / peaks["hbm_gbs"], "traffic": None}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -127,6 +127,13 @@ int afno_spectral_bwd_host(const afno_desc_t* d, const void* x_host, const void*
  * "gpu_launches" is counted from this, not guessed). */
 int afno_last_launch_count(void);
 
+/* Measurement aid: between start and stop every kernel this thread launches through the
+ * library is bracketed by CUDA events on its stream (do not use during stream capture).
+ * stop synchronises the device and writes one line per kernel name into `out` (host
+ * buffer of `cap` bytes): "<kernel> <launches> <total_ms>\n". */
+int afno_profile_start(void);
+int afno_profile_stop(char* out, size_t cap);
+
 #ifdef __cplusplus
 }
 #endif

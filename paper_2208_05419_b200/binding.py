@@ -23,6 +23,7 @@ EXPORTS = [
     "afno_spectral_workspace_bytes", "afno_spectral_mask_bytes", "afno_plan_warmup",
     "afno_spectral_fwd", "afno_spectral_bwd", "afno_spectral_host_arena_bytes",
     "afno_spectral_fwd_host", "afno_spectral_bwd_host", "afno_last_launch_count",
+    "afno_profile_start", "afno_profile_stop",
 ]
 
 
@@ -77,6 +78,9 @@ def lib():
         L.afno_spectral_bwd_host.restype = ctypes.c_int
         L.afno_spectral_bwd_host.argtypes = [dp] + [vp] * 12 + [sz, vp]
         L.afno_last_launch_count.restype = ctypes.c_int
+        L.afno_profile_start.restype = ctypes.c_int
+        L.afno_profile_stop.restype = ctypes.c_int
+        L.afno_profile_stop.argtypes = [ctypes.c_char_p, sz]
         _lib = L
     return _lib
 
@@ -170,6 +174,21 @@ def afno_plan_warmup(d: Desc):
 
 def afno_last_launch_count() -> int:
     return int(lib().afno_last_launch_count())
+
+
+def afno_profile_start():
+    _check(lib().afno_profile_start())
+
+
+def afno_profile_stop() -> dict:
+    """{kernel name: (launches, total_ms)} for the launches since afno_profile_start()."""
+    buf = ctypes.create_string_buffer(1 << 16)
+    _check(lib().afno_profile_stop(buf, len(buf)))
+    out = {}
+    for line in buf.value.decode().splitlines():
+        name, n, ms = line.split()
+        out[name] = (int(n), float(ms))
+    return out
 
 
 def _ws_bytes(ws):

@@ -173,6 +173,28 @@ size_t act_bytes(const Geometry& g) {
 
 void count_launch(int n) { t_launches += n; }
 
+// ---- optional per-kernel profiler (CUDA events around every launch) -----------------------
+namespace {
+struct ProfRec {
+  const char* name;
+  cudaEvent_t a, b;
+};
+thread_local bool t_prof_on = false;
+thread_local std::vector<ProfRec> t_prof;
+} // namespace
+
+void prof_begin(const char* name, cudaStream_t st) {
+  if (!t_prof_on) return;
+  ProfRec r{name, nullptr, nullptr};
+  if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) return;
+  cudaEventRecord(r.a, st);
+  t_prof.push_back(r);
+}
+void prof_end(cudaStream_t st) {
+  if (!t_prof_on || t_prof.empty()) return;
+  cudaEventRecord(t_prof.back().b, st);
+}
+
 } // namespace afno
 
 using namespace afno;
@@ -195,6 +217,47 @@ const char* afno_status_string(int status) {
 const char* afno_last_error(void) { return t_error.c_str(); }
 
 int afno_last_launch_count(void) { return t_launches; }
+
+int afno_profile_start(void) {
+  for (auto& r : t_prof) {
+    cudaEventDestroy(r.a);
+    cudaEventDestroy(r.b);
+  }
+  t_prof.clear();
+  t_prof_on = true;
+  return AFNO_OK;
+}
+
+int afno_profile_stop(char* out, size_t cap) {
+  t_prof_on = false;
+  cudaError_t e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) return fail(AFNO_ERR_CUDA, std::string("profile sync: ") + cudaGetErrorString(e));
+  struct Agg { const char* name; int n; double ms; };
+  std::vector<Agg> agg;
+  for (auto& r : t_prof) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, r.a, r.b) != cudaSuccess) ms = 0.f;
+    bool found = false;
+    for (auto& a : agg)
+      if (strcmp(a.name, r.name) == 0) { a.n++; a.ms += ms; found = true; break; }
+    if (!found) agg.push_back({r.name, 1, (double)ms});
+    cudaEventDestroy(r.a);
+    cudaEventDestroy(r.b);
+  }
+  t_prof.clear();
+  std::string text;
+  char line[256];
+  for (auto& a : agg) {
+    snprintf(line, sizeof(line), "%s %d %.6f\n", a.name, a.n, a.ms);
+    text += line;
+  }
+  if (out && cap > 0) {
+    const size_t n = text.size() < cap - 1 ? text.size() : cap - 1;
+    memcpy(out, text.data(), n);
+    out[n] = 0;
+  }
+  return AFNO_OK;
+}
 
 const char* afno_spectral_path(const afno_desc_t* d) {
   Geometry g;

@@ -36,8 +36,11 @@ struct Plan {
   FftPlan fh, fw;
 };
 
-// launch accounting (thread-local, reported through afno_last_launch_count)
+// launch accounting (thread-local, reported through afno_last_launch_count) and the optional
+// per-kernel CUDA-event profiler behind afno_profile_start / afno_profile_stop
 void count_launch(int n = 1);
+void prof_begin(const char* kernel_name, cudaStream_t st);
+void prof_end(cudaStream_t st);
 
 // ---- generic fp32-math path (generic.cu) -------------------------------------------
 size_t generic_workspace_bytes(const Geometry& g, bool backward);

@@ -473,8 +473,10 @@ __global__ void k_reduce_parts(const float2* __restrict__ part, float2* __restri
 struct Launcher {
   cudaStream_t st;
   cudaError_t err = cudaSuccess;
+  void begin(const char* name) { prof_begin(name, st); }
   void check() {
     if (err == cudaSuccess) err = cudaGetLastError();
+    prof_end(st);
     count_launch();
   }
 };
@@ -492,6 +494,7 @@ void launch_wfft_fwd(Launcher& L, const Geometry& g, const Plan& p, const T* x, 
   L.err = set_smem(k_wfft_fwd<T>, smem);
   if (L.err != cudaSuccess) return;
   dim3 grid((g.C + 63) / 64, g.H, g.B), block(kLanes, kFftWarps);
+  L.begin("k_wfft_fwd");
   k_wfft_fwd<T><<<grid, block, smem, L.st>>>(x, S, p.fw, g.H, g.W, g.C, g.Kw, g.scale, alpha ? 1 : 0);
   L.check();
 }
@@ -502,6 +505,7 @@ void launch_hfft(Launcher& L, const Geometry& g, const Plan& p, float2* S, int C
   L.err = set_smem(k_hfft, smem);
   if (L.err != cudaSuccess) return;
   dim3 grid((C + kLanes - 1) / kLanes, g.Kw, g.B), block(kLanes, kFftWarps);
+  L.begin("k_hfft");
   k_hfft<<<grid, block, smem, L.st>>>(S, p.fh, g.H, g.Kw, C, inverse ? +1.f : -1.f);
   L.check();
 }
@@ -514,6 +518,7 @@ void launch_wfft_inv(Launcher& L, const Geometry& g, const Plan& p, const float2
   L.err = set_smem(k_wfft_inv<T>, smem);
   if (L.err != cudaSuccess) return;
   dim3 grid((g.C + 63) / 64, g.H, g.B), block(kLanes, kFftWarps);
+  L.begin("k_wfft_inv");
   k_wfft_inv<T><<<grid, block, smem, L.st>>>(S, res, out, p.fw, g.H, g.W, g.C, g.Kw, g.scale,
                                            half_interior ? 1 : 0);
   L.check();
@@ -528,6 +533,7 @@ void launch_gemm(Launcher& L, const Geometry& g, const float2* in, int ldin, con
   L.err = set_smem(k_block_gemm<EPI>, smem);
   if (L.err != cudaSuccess) return;
   dim3 grid((unsigned)((M + kGemmTM - 1) / kGemmTM), g.nb);
+  L.begin("k_block_gemm");
   k_block_gemm<EPI><<<grid, kGemmThreads, smem, L.st>>>(in, ldin, Wm, bias, out, ldout, aux, ldaux, M, K, N,
                                                        g.H, g.Kw, g.Kh, g.lambda);
   L.check();
@@ -553,12 +559,15 @@ void launch_wgrad(Launcher& L, const Geometry& g, const float2* A, int lda, cons
   float2* partW = part;
   float2* partB = part + (size_t)S * g.nb * K * N;
   dim3 grid(S, g.nb, ntK * ntN);
+  L.begin("k_block_wgrad");
   k_block_wgrad<<<grid, 256, 0, L.st>>>(A, lda, G, ldg, partW, partB, M, K, N, rps, ntN);
   L.check();
   if (L.err != cudaSuccess) return;
   const size_t nW = (size_t)g.nb * K * N, nB = (size_t)g.nb * N;
+  L.begin("k_reduce_parts");
   k_reduce_parts<<<(unsigned)((nW + 255) / 256), 256, 0, L.st>>>(partW, (float2*)dW, nW, S, g.accum ? 1 : 0);
   L.check();
+  L.begin("k_reduce_parts");
   k_reduce_parts<<<(unsigned)((nB + 255) / 256), 256, 0, L.st>>>(partB, (float2*)dB, nB, S, g.accum ? 1 : 0);
   L.check();
 }
@@ -640,21 +649,26 @@ cudaError_t backward_t(const Geometry& g, const Plan& p, const T* x, const T* dy
   launch_hfft(L, g, p, w.G, g.C, false);
   if (L.err != cudaSuccess) return L.err;
   // B3: G2 = G (.) mask2
+  L.begin("k_mask_nonzero");
   k_mask_nonzero<<<148 * 8, 256, 0, st>>>(w.G, w.Z, rows * g.C);
   L.check();
   if (g.export_masks) {
     if (L.err == cudaSuccess) L.err = cudaMemsetAsync(ws, 0, mask_region, st);
     if (L.err != cudaSuccess) return L.err;
+    L.begin("k_export_masks");
     k_export_masks<<<148 * 8, 256, 0, st>>>(w.O1, (uint8_t*)ws, g.H, g.Kw, g.Wh, g.CH, rows * g.CH, 1);
     L.check();
+    L.begin("k_export_masks");
     k_export_masks<<<148 * 8, 256, 0, st>>>(w.Z, (uint8_t*)ws + m2off, g.H, g.Kw, g.Wh, g.C, rows * g.C, 0);
     L.check();
   }
   // conjugate-transposed weights for the input-gradient GEMMs
   {
     const size_t n = (size_t)g.nb * g.bs * g.hid;
+    L.begin("k_transpose_conj");
     k_transpose_conj<<<(unsigned)((n + 255) / 256), 256, 0, st>>>((const float2*)w1, w.Wt1, g.nb, g.bs, g.hid);
     L.check();
+    L.begin("k_transpose_conj");
     k_transpose_conj<<<(unsigned)((n + 255) / 256), 256, 0, st>>>((const float2*)w2, w.Wt2, g.nb, g.hid, g.bs);
     L.check();
   }

@@ -71,9 +71,18 @@ int resolve(const afno_desc_t* d, Geometry* g) {
   g->no_residual = (d->flags & AFNO_FLAG_NO_RESIDUAL) != 0;
   g->accum = (d->flags & AFNO_FLAG_ACCUM_GRADS) != 0;
   g->export_masks = (d->flags & AFNO_FLAG_EXPORT_MASKS) != 0;
+  g->force_fp32 = (d->flags & AFNO_FLAG_FORCE_FP32_MATH) != 0;
   const char* why = nullptr;
   if (!generic_supported(*g, &why)) return fail(AFNO_ERR_UNSUPPORTED, why);
   return AFNO_OK;
+}
+
+// which kernel family serves the descriptor (the backward still runs on the generic path)
+bool use_tc_fwd(const Geometry& g) { return !g.force_fp32 && tc_supported(g); }
+bool use_tc_bwd(const Geometry&) { return false; }
+size_t workspace_bytes(const Geometry& g, bool backward) {
+  if (backward) return use_tc_bwd(g) ? tc_workspace_bytes(g, true) : generic_workspace_bytes(g, true);
+  return use_tc_fwd(g) ? tc_workspace_bytes(g, false) : generic_workspace_bytes(g, false);
 }
 
 // ---- plan cache ------------------------------------------------------------------------
@@ -140,6 +149,7 @@ int get_plan(const Geometry& g, bool may_build, const Plan** out) {
   p->W = g.W;
   e = build_fft_plan(g.H, &p->fh);
   if (e == cudaSuccess) e = build_fft_plan(g.W, &p->fw);
+  if (e == cudaSuccess && g.H <= 96 && g.W <= 192) e = tc_build_plan(g.H, g.W, &p->tc);
   if (e != cudaSuccess) {
     delete p;
     return fail(AFNO_ERR_CUDA, std::string("plan creation: ") + cudaGetErrorString(e));
@@ -262,13 +272,13 @@ int afno_profile_stop(char* out, size_t cap) {
 const char* afno_spectral_path(const afno_desc_t* d) {
   Geometry g;
   if (resolve(d, &g) != AFNO_OK) return nullptr;
-  return "generic-fp32";
+  return use_tc_fwd(g) ? "tcgen05-bf16" : "generic-fp32";
 }
 
 size_t afno_spectral_workspace_bytes(const afno_desc_t* d, int for_backward) {
   Geometry g;
   if (resolve(d, &g) != AFNO_OK) return 0;
-  return generic_workspace_bytes(g, for_backward != 0);
+  return workspace_bytes(g, for_backward != 0);
 }
 
 int afno_spectral_mask_bytes(const afno_desc_t* d, size_t* mask1_bytes, size_t* mask2_offset,
@@ -303,7 +313,7 @@ int afno_spectral_fwd(const afno_desc_t* d, const void* x, const float* w1, cons
   for (const void* p : ptrs)
     if (!aligned16(p)) return fail(AFNO_ERR_INVALID_ARG, "pointers must be 16-byte aligned");
   if (overlaps(x, y, act_bytes(g))) return fail(AFNO_ERR_INVALID_ARG, "y must not alias x");
-  if (workspace_bytes < generic_workspace_bytes(g, false))
+  if (workspace_bytes < afno::workspace_bytes(g, false))
     return fail(AFNO_ERR_WORKSPACE, "workspace smaller than afno_spectral_workspace_bytes(d, 0)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   bool may_build = false;
@@ -312,7 +322,8 @@ int afno_spectral_fwd(const afno_desc_t* d, const void* x, const float* w1, cons
   const Plan* p = nullptr;
   rc = get_plan(g, may_build, &p);
   if (rc != AFNO_OK) return rc;
-  cudaError_t e = generic_forward(g, *p, x, w1, b1, w2, b2, y, workspace, st);
+  cudaError_t e = (use_tc_fwd(g) && p->tc.valid) ? tc_forward(g, *p, x, w1, b1, w2, b2, y, workspace, st)
+                                                 : generic_forward(g, *p, x, w1, b1, w2, b2, y, workspace, st);
   if (e != cudaSuccess) return fail(AFNO_ERR_CUDA, std::string("forward launch: ") + cudaGetErrorString(e));
   return AFNO_OK;
 }
@@ -332,7 +343,7 @@ int afno_spectral_bwd(const afno_desc_t* d, const void* x, const void* dy, const
     if (!aligned16(p)) return fail(AFNO_ERR_INVALID_ARG, "pointers must be 16-byte aligned");
   if (overlaps(dx, dy, act_bytes(g)) || overlaps(dx, x, act_bytes(g)))
     return fail(AFNO_ERR_INVALID_ARG, "dx must not alias dy or x");
-  if (workspace_bytes < generic_workspace_bytes(g, true))
+  if (workspace_bytes < afno::workspace_bytes(g, true))
     return fail(AFNO_ERR_WORKSPACE, "workspace smaller than afno_spectral_workspace_bytes(d, 1)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   bool may_build = false;

@@ -26,14 +26,22 @@ struct Geometry {
   int Wh, Kh, Kw;
   float lambda;
   float scale; // 1/sqrt(H*W)
-  bool bf16, no_residual, accum, export_masks;
+  bool bf16, no_residual, accum, export_masks, force_fp32;
   long long modes_all() const { return (long long)B * H * Wh; }
   long long rows() const { return (long long)B * H * Kw; } // rows of the stored spectra
+};
+
+// constant operand images of the tcgen05 path (device pointers, shared-memory layout order)
+struct TcPlan {
+  bool valid = false;
+  int num_sms = 148;
+  uint8_t *dft = nullptr, *fw = nullptr, *fw_alpha = nullptr, *gw = nullptr, *gw_noalpha = nullptr;
 };
 
 struct Plan {
   int device, H, W;
   FftPlan fh, fw;
+  TcPlan tc;
 };
 
 // launch accounting (thread-local, reported through afno_last_launch_count) and the optional
@@ -52,6 +60,13 @@ cudaError_t generic_backward(const Geometry& g, const Plan& p, const void* x, co
                              void* dx, float* dw1, float* db1, float* dw2, float* db2, void* ws,
                              size_t mask1_bytes, size_t mask2_offset, cudaStream_t st);
 bool generic_supported(const Geometry& g, const char** why);
+
+// ---- tcgen05 bf16 path (tc_path.cu) --------------------------------------------------
+bool tc_supported(const Geometry& g);
+cudaError_t tc_build_plan(int H, int W, TcPlan* out);
+size_t tc_workspace_bytes(const Geometry& g, bool backward);
+cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const float* w1, const float* b1,
+                       const float* w2, const float* b2, void* y, void* ws, cudaStream_t st);
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 

@@ -1,0 +1,590 @@
+// tcgen05 (5th-generation tensor core) path of the AFNO spectral layer for bf16 activations,
+// 96-wide channel blocks, H <= 96 (90 in FourCastNet's 8x8 patch grid) and W <= 192.
+//
+// On B200 the tensor pipe is ~30x the fp32 ALU pipe, while a dense DFT of length 90 / 180 costs
+// only ~20x the FLOPs of an FFT, so every transform of the layer is computed as a bf16 GEMM
+// with fp32 accumulation against constant DFT matrices (S5 gives the arithmetic and
+// the measured error).  The layer becomes three GEMM-chain kernels:
+//
+//   tc_wdft_fwd  [F1, B2]   per (b, h, 128 channels):  A1[c, (ri,kw)] = x^T[c, w] * Fw[w, (ri,kw)]
+//   tc_mix_fwd   [F2-F7]    per (b, kw, block j), everything on chip in tensor memory:
+//                            Xh = Fh * A1  ->  relu(Xh W1 + b1)  ->  shrink(. W2 + b2)  ->  Fh^H * Z
+//   tc_wdft_inv  [F8, F9, B8] per (b, h, 128 channels): y[c, w] = x + A2^T[c, (ri,kw)] * Gw[(ri,kw), w]
+//
+// Complex arithmetic runs as real GEMMs on separate (re | im) column halves using the
+// instruction descriptor's negate bit for the minus signs, so only W_re and W_im (not the 2x2
+// real block form) live in shared memory.
+#include <math.h>
+#include <string.h>
+
+#include <vector>
+
+#include "afno_internal.h"
+#include "tc_common.cuh"
+
+namespace afno {
+
+namespace {
+
+using namespace tc;
+
+constexpr int BS = 96;    // channel block size handled by this path
+constexpr int NT = 192;   // (re | im) columns of one block
+constexpr int HP = 96;    // H padded to the K extent of the H-direction GEMMs
+constexpr int WP = 192;   // W padded to the K / N extent of the W-direction GEMMs
+constexpr int CGRP = 128; // channels per W-direction tile (= UMMA M)
+
+// shared-memory operand geometry (bytes), see tc_common.cuh for the layout formulas
+constexpr uint32_t kDftLbo = 2048, kDftSbo = 128;   // Ch / Sh: K-major A [128 x 96], order [k/8][m/8]
+constexpr uint32_t kDftBytes = 128 * HP * 2;         // 24576
+constexpr uint32_t kWLbo = 1536, kWSbo = 128;       // weights: K-major B [96 x 96], order [k/8][n/8]
+constexpr uint32_t kWBytes = BS * BS * 2;            // 18432
+constexpr uint32_t kTileLbo = 128, kTileSbo = 1536; // mode tile: MN-major B [K=96 rows][N=192]
+constexpr uint32_t kTileBytes = HP * NT * 2;         // 36864
+constexpr uint32_t kFwLbo = 3072, kFwSbo = 128;     // Fw^T / Gw^T: K-major B [192 x 192]
+constexpr uint32_t kFwBytes = WP * NT * 2;           // 73728
+constexpr uint32_t kRowLbo = 128, kRowSbo = 3072;   // W-direction data tile: MN-major A [K=192][M=128]
+constexpr uint32_t kRowBytes = WP * CGRP * 2;        // 49152
+
+constexpr uint32_t kMixSmem = 2 * kDftBytes + 4 * kWBytes + kTileBytes + 2 * NT * 4; // 161280
+constexpr uint32_t kRowSmem = kFwBytes + kRowBytes;                                  // 122880
+
+// ---- weight preparation: fp32 [nb][96][96][2] -> bf16 K-major interleaved operands --------------
+// per block, 8 matrices of kWBytes: fwd {W1r, W1i, W2r, W2i} with element (n=o, k=i) = W[i][o];
+// bwd {W1r, W1i, W2r, W2i} with element (n=i, k=o) = W[i][o].
+__global__ void k_tc_prep_weights(const float* __restrict__ w1, const float* __restrict__ w2,
+                                  __nv_bfloat16* __restrict__ out, int nb) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= nb * BS * BS) return;
+  const int o = idx % BS, i = (idx / BS) % BS, j = idx / (BS * BS);
+  const float2 a = ((const float2*)w1)[idx], b = ((const float2*)w2)[idx];
+  __nv_bfloat16* base = out + (size_t)j * 8 * (kWBytes / 2);
+  const uint32_t f = ((i / 8) * kWLbo + (o / 8) * kWSbo + (o % 8) * 16 + (i % 8) * 2) / 2; // n=o, k=i
+  const uint32_t t = ((o / 8) * kWLbo + (i / 8) * kWSbo + (i % 8) * 16 + (o % 8) * 2) / 2; // n=i, k=o
+  const uint32_t m = kWBytes / 2;
+  base[0 * m + f] = __float2bfloat16_rn(a.x);
+  base[1 * m + f] = __float2bfloat16_rn(a.y);
+  base[2 * m + f] = __float2bfloat16_rn(b.x);
+  base[3 * m + f] = __float2bfloat16_rn(b.y);
+  base[4 * m + t] = __float2bfloat16_rn(a.x);
+  base[5 * m + t] = __float2bfloat16_rn(a.y);
+  base[6 * m + t] = __float2bfloat16_rn(b.x);
+  base[7 * m + t] = __float2bfloat16_rn(b.y);
+}
+
+// ---- F1 / B2: W-direction forward DFT as a GEMM ------------------------------------------------
+// A1 layout: [b][kw < Kw][j][h][ri][96] bf16 (one (b,kw,j) tile = H x 192 contiguous).
+__global__ void __launch_bounds__(128, 1)
+tc_wdft_fwd(const __nv_bfloat16* __restrict__ x, __nv_bfloat16* __restrict__ A1,
+            const uint8_t* __restrict__ FwT, int B, int H, int W, int C, int Kw, int nb) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t mbar;
+  __shared__ uint32_t tmem_slot;
+  uint8_t* sF = smem;
+  uint8_t* sA = smem + kFwBytes;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  for (uint32_t i = tid; i < kRowBytes / 16; i += 128) ((uint4*)sA)[i] = make_uint4(0, 0, 0, 0);
+  for (uint32_t i = tid; i < kFwBytes / 16; i += 128) cp_async16(smem_u32(sF) + i * 16, FwT + (size_t)i * 16);
+  if (tid == 0) {
+    mbar_init(&mbar, 1);
+    mbar_init_fence();
+  }
+  if (warp == 0) tmem_alloc<256>(&tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+  const int ncg = (C + CGRP - 1) / CGRP;
+  const int ntiles = B * H * ncg;
+  uint32_t phase = 0;
+  const uint32_t idesc = idesc_bf16(128, NT, kIdescAMn);
+  const int hl = lane & 7, cl4 = lane >> 3;
+  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    const int cg = t % ncg, bh = t / ncg;
+    const __nv_bfloat16* xrow = x + (size_t)bh * W * C;
+    // x[b,h,:,cg*128 .. +128) becomes the MN-major A operand (K = w, M = channel)
+    const int nunits = ((W + 7) / 8) * 4;
+    for (int u = warp; u < nunits; u += 4) {
+      const int w = (u >> 2) * 8 + hl;
+      const int mc = (u & 3) * 4 + cl4;
+      const int c0 = cg * CGRP + mc * 8;
+      if (w < W && c0 < C) cp_async16(smem_u32(sA) + mc * kRowSbo + w * 16, xrow + (size_t)w * C + c0);
+    }
+    cp_async_wait_all();
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (tid == 0) {
+      tc_fence_after();
+      for (int ks = 0; ks < WP / 16; ++ks)
+        mma_ss(tmem, smem_desc(smem_u32(sA) + ks * 2 * kRowLbo, kRowLbo, kRowSbo),
+               smem_desc(smem_u32(sF) + ks * 2 * kFwLbo, kFwLbo, kFwSbo), idesc, ks > 0);
+      mma_commit(&mbar);
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+    const int c = cg * CGRP + tid;
+    const int b = bh / H, h = bh - b * H;
+    const int j = c / BS, cl = c - j * BS;
+#pragma unroll 1
+    for (int c0 = 0; c0 < NT; c0 += 32) {
+      uint32_t v[32];
+      tmem_ld32(tmem + lane_base + c0, v);
+      tmem_wait_ld();
+      if (c < C) {
+#pragma unroll
+        for (int q = 0; q < 32; ++q) {
+          const int n = c0 + q;
+          const int ri = n >= BS ? 1 : 0, kw = n - ri * BS;
+          if (kw < Kw)
+            A1[((((size_t)b * Kw + kw) * nb + j) * H + h) * NT + ri * BS + cl] =
+                __float2bfloat16_rn(__uint_as_float(v[q]));
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<256>(tmem);
+}
+
+// ---- F8 + F9 / B8: W-direction inverse DFT as a GEMM, residual add, store -----------------------
+__global__ void __launch_bounds__(128, 1)
+tc_wdft_inv(const __nv_bfloat16* __restrict__ A2, const __nv_bfloat16* __restrict__ res,
+            __nv_bfloat16* __restrict__ y, const uint8_t* __restrict__ GwT, int B, int H, int W, int C,
+            int Kw, int nb) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t mbar;
+  __shared__ uint32_t tmem_slot;
+  uint8_t* sG = smem;
+  uint8_t* sA = smem + kFwBytes;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  for (uint32_t i = tid; i < kRowBytes / 16; i += 128) ((uint4*)sA)[i] = make_uint4(0, 0, 0, 0);
+  for (uint32_t i = tid; i < kFwBytes / 16; i += 128) cp_async16(smem_u32(sG) + i * 16, GwT + (size_t)i * 16);
+  if (tid == 0) {
+    mbar_init(&mbar, 1);
+    mbar_init_fence();
+  }
+  if (warp == 0) tmem_alloc<256>(&tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+  const int ncg = (C + CGRP - 1) / CGRP;
+  const int ntiles = B * H * ncg;
+  uint32_t phase = 0;
+  const uint32_t idesc = idesc_bf16(128, NT, kIdescAMn);
+  const int hl = lane & 7, cl4 = lane >> 3;
+  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    const int cg = t % ncg, bh = t / ncg;
+    const int b = bh / H, h = bh - b * H;
+    // A2[b][kw][j][h][ri][cl] gathered into the MN-major A operand (K = (ri,kw), M = channel)
+    const int kwg = (Kw + 7) / 8;
+    const int nunits = 2 * kwg * 4;
+    for (int u = warp; u < nunits; u += 4) {
+      const int rg = u >> 2;                 // (ri, kw group)
+      const int ri = rg / kwg, kw = (rg - ri * kwg) * 8 + hl;
+      const int mc = (u & 3) * 4 + cl4;
+      const int c0 = cg * CGRP + mc * 8;
+      if (kw < Kw && c0 < C) {
+        const int j = c0 / BS, cl = c0 - j * BS;
+        const __nv_bfloat16* src = A2 + ((((size_t)b * Kw + kw) * nb + j) * H + h) * NT + ri * BS + cl;
+        cp_async16(smem_u32(sA) + mc * kRowSbo + (ri * BS + kw) * 16, src);
+      }
+    }
+    cp_async_wait_all();
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (tid == 0) {
+      tc_fence_after();
+      for (int ks = 0; ks < NT / 16; ++ks)
+        mma_ss(tmem, smem_desc(smem_u32(sA) + ks * 2 * kRowLbo, kRowLbo, kRowSbo),
+               smem_desc(smem_u32(sG) + ks * 2 * kFwLbo, kFwLbo, kFwSbo), idesc, ks > 0);
+      mma_commit(&mbar);
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+    const int c = cg * CGRP + tid;
+    const size_t rowoff = (size_t)bh * W * C + c;
+#pragma unroll 1
+    for (int c0 = 0; c0 < WP; c0 += 32) {
+      uint32_t v[32];
+      tmem_ld32(tmem + lane_base + c0, v);
+      tmem_wait_ld();
+      if (c < C) {
+#pragma unroll
+        for (int q = 0; q < 32; ++q) {
+          const int w = c0 + q;
+          if (w < W) {
+            float val = __uint_as_float(v[q]);
+            if (res) val += __bfloat162float(res[rowoff + (size_t)w * C]);
+            y[rowoff + (size_t)w * C] = __float2bfloat16_rn(val);
+          }
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<256>(tmem);
+}
+
+// ---- F2-F7: per (b, kw, block) chain  H-DFT -> layer 1 -> layer 2 -> inverse H-DFT ---------------
+// Accumulators in tensor memory: region R0 = columns [0,192), R1 = [256,448); a layer's bf16
+// input (A operand) is written in place over the fp32 accumulator it was computed from.
+struct MixParams {
+  const __nv_bfloat16* A1;
+  __nv_bfloat16* A2;
+  const uint8_t* dft;      // Ch then Sh, kDftBytes each, smem image
+  const uint8_t* wprep;    // per block 8 x kWBytes
+  const float* b1;         // [nb][96][2]
+  const float* b2;
+  int B, H, Kw, nb, Kh;
+  float lambda;
+};
+
+// D[:, dcol .. dcol+96) (+)= A_smem(K-major [128 x 96]) * tile half (MN-major, 96 columns)
+__device__ __forceinline__ void issue_dft(uint32_t d, uint32_t a_base, uint32_t b_base, uint32_t idesc, bool fresh) {
+#pragma unroll
+  for (int ks = 0; ks < HP / 16; ++ks)
+    mma_ss(d, smem_desc(a_base + ks * 2 * kDftLbo, kDftLbo, kDftSbo),
+           smem_desc(b_base + ks * 2 * kTileLbo, kTileLbo, kTileSbo), idesc, !(fresh && ks == 0));
+}
+// D[:, dcol .. dcol+96) (+)= A_tmem(packed bf16, 48 columns = K 96) * W_smem(K-major [96 x 96])
+__device__ __forceinline__ void issue_mlp(uint32_t d, uint32_t a_tmem, uint32_t w_base, uint32_t idesc, bool fresh) {
+#pragma unroll
+  for (int ks = 0; ks < BS / 16; ++ks)
+    mma_ts(d, a_tmem + ks * 8, smem_desc(w_base + ks * 2 * kWLbo, kWLbo, kWSbo), idesc, !(fresh && ks == 0));
+}
+
+__global__ void __launch_bounds__(128, 1) tc_mix_fwd(MixParams p) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t mbar;
+  __shared__ uint32_t tmem_slot;
+  uint8_t* sCh = smem;
+  uint8_t* sSh = smem + kDftBytes;
+  uint8_t* sW = smem + 2 * kDftBytes;
+  uint8_t* sTile = sW + 4 * kWBytes;
+  float* sBias = (float*)(sTile + kTileBytes); // b1 (re 96 | im 96), b2 (re 96 | im 96)
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  for (uint32_t i = tid; i < kTileBytes / 16; i += 128) ((uint4*)sTile)[i] = make_uint4(0, 0, 0, 0);
+  for (uint32_t i = tid; i < 2 * kDftBytes / 16; i += 128) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
+  if (tid == 0) {
+    mbar_init(&mbar, 1);
+    mbar_init_fence();
+  }
+  if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+  const uint32_t R0 = tmem, R1 = tmem + 256;
+  const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW), aTile = smem_u32(sTile);
+  const uint32_t tile_re = aTile, tile_im = aTile + (BS / 8) * kTileSbo;
+  const uint32_t id_dft = idesc_bf16(128, BS, kIdescBMn);
+  const uint32_t id_mlp = idesc_bf16(128, BS);
+
+  const int ntiles = p.nb * p.B * p.Kw;
+  const int per = (ntiles + gridDim.x - 1) / gridDim.x;
+  const int t_begin = blockIdx.x * per, t_end = min(ntiles, t_begin + per);
+  uint32_t phase = 0;
+  int cur_j = -1;
+  const int r = tid; // this thread's accumulator row (mode row kh, or output row h)
+  const int kappa = (r <= p.H / 2) ? r : p.H - r;
+  const bool row_kept = (r < p.H) && (kappa < p.Kh);
+  const int hl = lane & 7, cl4 = lane >> 3;
+
+  for (int t = t_begin; t < t_end; ++t) {
+    const int j = t / (p.B * p.Kw);
+    const int rem = t - j * (p.B * p.Kw);
+    if (j != cur_j) {
+      cur_j = j;
+      const uint8_t* wsrc = p.wprep + (size_t)j * 8 * kWBytes;
+      for (uint32_t i = tid; i < 4 * kWBytes / 16; i += 128) cp_async16(aW + i * 16, wsrc + (size_t)i * 16);
+      for (int i = tid; i < 2 * NT; i += 128) {
+        const int which = i / NT, n = i % NT, ri = n / BS, o = n % BS;
+        sBias[i] = (which == 0 ? p.b1 : p.b2)[((size_t)j * BS + o) * 2 + ri];
+      }
+    }
+    // tile (b, kw, j) of A1: H rows of 192 bf16 -> MN-major B operand (K = h, N = (ri, c))
+    const __nv_bfloat16* src = p.A1 + ((size_t)rem * p.nb + j) * p.H * NT;
+    {
+      const int nunits = ((p.H + 7) / 8) * 6;
+      for (int u = warp; u < nunits; u += 4) {
+        const int h = (u / 6) * 8 + hl;
+        const int nc = (u % 6) * 4 + cl4;
+        if (h < p.H) cp_async16(aTile + nc * kTileSbo + h * 16, src + (size_t)h * NT + nc * 8);
+      }
+    }
+    cp_async_wait_all();
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    // F2: Xr = Ch Ar + Sh Ai ; Xi = Ch Ai - Sh Ar      (forward kernel exp(-i theta))
+    if (tid == 0) {
+      tc_fence_after();
+      issue_dft(R0, aCh, tile_re, id_dft, true);
+      issue_dft(R0, aSh, tile_im, id_dft, false);
+      issue_dft(R0 + BS, aCh, tile_im, id_dft, true);
+      issue_dft(R0 + BS, aSh, tile_re, id_dft | kIdescNegA, false);
+      mma_commit(&mbar);
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+    // fp32 spectrum -> bf16 A operand, in place
+#pragma unroll 1
+    for (int c0 = 0; c0 < NT; c0 += 32) {
+      uint32_t v[32], pk[16];
+      tmem_ld32(R0 + lane_base + c0, v);
+      tmem_wait_ld();
+#pragma unroll
+      for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
+      tmem_st16(R0 + lane_base + c0 / 2, pk);
+    }
+    tmem_wait_st();
+    tc_fence_before();
+    __syncthreads();
+    // F3: P1 = Xh W1 + b1
+    if (tid == 0) {
+      tc_fence_after();
+      issue_mlp(R1, R0, aW + 0 * kWBytes, id_mlp, true);                         // Xr W1r
+      issue_mlp(R1, R0 + BS / 2, aW + 1 * kWBytes, id_mlp | kIdescNegB, false);  // - Xi W1i
+      issue_mlp(R1 + BS, R0, aW + 1 * kWBytes, id_mlp, true);                    // Xr W1i
+      issue_mlp(R1 + BS, R0 + BS / 2, aW + 0 * kWBytes, id_mlp, false);          // + Xi W1r
+      mma_commit(&mbar);
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+    // F4: bias + split ReLU -> bf16 A operand, in place
+#pragma unroll 1
+    for (int c0 = 0; c0 < NT; c0 += 32) {
+      uint32_t v[32], pk[16];
+      tmem_ld32(R1 + lane_base + c0, v);
+      tmem_wait_ld();
+#pragma unroll
+      for (int q = 0; q < 16; ++q) {
+        const float a = fmaxf(__uint_as_float(v[2 * q]) + sBias[c0 + 2 * q], 0.f);
+        const float b = fmaxf(__uint_as_float(v[2 * q + 1]) + sBias[c0 + 2 * q + 1], 0.f);
+        pk[q] = pack_bf16(a, b);
+      }
+      tmem_st16(R1 + lane_base + c0 / 2, pk);
+    }
+    tmem_wait_st();
+    tc_fence_before();
+    __syncthreads();
+    // F5: P2 = O1 W2 + b2
+    if (tid == 0) {
+      tc_fence_after();
+      issue_mlp(R0, R1, aW + 2 * kWBytes, id_mlp, true);
+      issue_mlp(R0, R1 + BS / 2, aW + 3 * kWBytes, id_mlp | kIdescNegB, false);
+      issue_mlp(R0 + BS, R1, aW + 3 * kWBytes, id_mlp, true);
+      issue_mlp(R0 + BS, R1 + BS / 2, aW + 2 * kWBytes, id_mlp, false);
+      mma_commit(&mbar);
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+    // F6: bias + softshrink + truncation -> bf16 Z written as the MN-major B operand (K = row r)
+#pragma unroll 1
+    for (int c0 = 0; c0 < NT; c0 += 32) {
+      uint32_t v[32];
+      tmem_ld32(R0 + lane_base + c0, v);
+      tmem_wait_ld();
+      if (r < HP) {
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+          uint32_t pk[4];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const int n = c0 + g * 8 + 2 * q;
+            float a = __uint_as_float(v[g * 8 + 2 * q]) + sBias[NT + n];
+            float b = __uint_as_float(v[g * 8 + 2 * q + 1]) + sBias[NT + n + 1];
+            float ma = fabsf(a) - p.lambda, mb = fabsf(b) - p.lambda;
+            a = (row_kept && ma > 0.f) ? copysignf(ma, a) : 0.f;
+            b = (row_kept && mb > 0.f) ? copysignf(mb, b) : 0.f;
+            pk[q] = pack_bf16(a, b);
+          }
+          *(uint4*)(sTile + ((c0 >> 3) + g) * kTileSbo + r * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        }
+      }
+    }
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    // F7: Tr = Ch Zr - Sh Zi ; Ti = Ch Zi + Sh Zr      (inverse kernel exp(+i theta))
+    if (tid == 0) {
+      tc_fence_after();
+      issue_dft(R1, aCh, tile_re, id_dft, true);
+      issue_dft(R1, aSh, tile_im, id_dft | kIdescNegA, false);
+      issue_dft(R1 + BS, aCh, tile_im, id_dft, true);
+      issue_dft(R1 + BS, aSh, tile_re, id_dft, false);
+      mma_commit(&mbar);
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+    __nv_bfloat16* dst = p.A2 + (((size_t)rem * p.nb + j) * p.H + r) * NT;
+#pragma unroll 1
+    for (int c0 = 0; c0 < NT; c0 += 32) {
+      uint32_t v[32];
+      tmem_ld32(R1 + lane_base + c0, v);
+      tmem_wait_ld();
+      if (r < p.H) {
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+          uint4 o;
+          o.x = pack_bf16(__uint_as_float(v[g * 8 + 0]), __uint_as_float(v[g * 8 + 1]));
+          o.y = pack_bf16(__uint_as_float(v[g * 8 + 2]), __uint_as_float(v[g * 8 + 3]));
+          o.z = pack_bf16(__uint_as_float(v[g * 8 + 4]), __uint_as_float(v[g * 8 + 5]));
+          o.w = pack_bf16(__uint_as_float(v[g * 8 + 6]), __uint_as_float(v[g * 8 + 7]));
+          *(uint4*)(dst + c0 + g * 8) = o;
+        }
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<512>(tmem);
+}
+
+// ---- host side: constant operand images ------------------------------------------------------------
+uint16_t host_bf16(double v) {
+  float f = (float)v;
+  uint32_t u;
+  memcpy(&u, &f, 4);
+  u += 0x7FFFu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+
+cudaError_t upload(const std::vector<uint16_t>& h, uint8_t** d) {
+  cudaError_t e = cudaMalloc((void**)d, h.size() * 2);
+  if (e != cudaSuccess) return e;
+  return cudaMemcpy(*d, h.data(), h.size() * 2, cudaMemcpyHostToDevice);
+}
+
+template <typename K>
+cudaError_t set_smem(K kernel, size_t bytes) {
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+struct TcWs {
+  __nv_bfloat16 *A1, *A2, *wprep;
+  size_t total;
+};
+TcWs tc_carve(const Geometry& g, char* base) {
+  TcWs w{};
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    char* p = base + off;
+    off = align_up(off + bytes, 256);
+    return p;
+  };
+  const size_t spec = (size_t)g.B * g.Kw * g.nb * g.H * NT * 2;
+  w.A1 = (__nv_bfloat16*)take(spec);
+  w.A2 = (__nv_bfloat16*)take(spec);
+  w.wprep = (__nv_bfloat16*)take((size_t)g.nb * 8 * kWBytes);
+  w.total = off;
+  return w;
+}
+
+} // namespace
+
+bool tc_supported(const Geometry& g) {
+  return g.bf16 && g.bs == BS && g.hid == BS && g.H <= HP && g.W <= WP && g.Wh <= BS && g.C % 8 == 0;
+}
+
+cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
+  const double two_pi = 6.283185307179586476925286766559;
+  const int Wh = W / 2 + 1;
+  // Ch, Sh: element (r, h) = cos / sin (2 pi r h / H) / sqrt(H); K-major [k/8][m/8]
+  std::vector<uint16_t> dft(2 * kDftBytes / 2, 0);
+  for (int r = 0; r < H; ++r)
+    for (int h = 0; h < H; ++h) {
+      const double a = two_pi * (double)((long)r * h % H) / (double)H, s = 1.0 / sqrt((double)H);
+      const uint32_t off = ((h / 8) * kDftLbo + (r / 8) * kDftSbo + (r % 8) * 16 + (h % 8) * 2) / 2;
+      dft[off] = host_bf16(cos(a) * s);
+      dft[kDftBytes / 2 + off] = host_bf16(sin(a) * s);
+    }
+  // Fw^T: element (n = ri*96 + kw, k = w) = {cos, -sin}(2 pi kw w / W) / sqrt(W)  [x alpha_kw]
+  // Gw^T: element (n = w, k = ri*96 + kw) = alpha_kw {cos, -sin}(2 pi kw w / W) / sqrt(W)  [or alpha = 1]
+  std::vector<uint16_t> fw(kFwBytes / 2, 0), fwa(kFwBytes / 2, 0), gw(kFwBytes / 2, 0), gw1(kFwBytes / 2, 0);
+  for (int kw = 0; kw < Wh; ++kw)
+    for (int w = 0; w < W; ++w) {
+      const double a = two_pi * (double)((long)kw * w % W) / (double)W, s = 1.0 / sqrt((double)W);
+      const double alpha = (kw == 0 || 2 * kw == W) ? 1.0 : 2.0;
+      for (int ri = 0; ri < 2; ++ri) {
+        const double v = (ri == 0 ? cos(a) : -sin(a)) * s;
+        const int n = ri * BS + kw;
+        const uint32_t of = ((w / 8) * kFwLbo + (n / 8) * kFwSbo + (n % 8) * 16 + (w % 8) * 2) / 2;
+        const uint32_t og = ((n / 8) * kFwLbo + (w / 8) * kFwSbo + (w % 8) * 16 + (n % 8) * 2) / 2;
+        fw[of] = host_bf16(v);
+        fwa[of] = host_bf16(v * alpha);
+        gw[og] = host_bf16(v * alpha);
+        gw1[og] = host_bf16(v);
+      }
+    }
+  cudaError_t e = upload(dft, &out->dft);
+  if (e == cudaSuccess) e = upload(fw, &out->fw);
+  if (e == cudaSuccess) e = upload(fwa, &out->fw_alpha);
+  if (e == cudaSuccess) e = upload(gw, &out->gw);
+  if (e == cudaSuccess) e = upload(gw1, &out->gw_noalpha);
+  if (e == cudaSuccess) e = set_smem(tc_wdft_fwd, kRowSmem);
+  if (e == cudaSuccess) e = set_smem(tc_wdft_inv, kRowSmem);
+  if (e == cudaSuccess) e = set_smem(tc_mix_fwd, kMixSmem);
+  int dev = 0, sms = 148;
+  if (e == cudaSuccess) e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  out->num_sms = sms;
+  out->valid = (e == cudaSuccess);
+  return e;
+}
+
+size_t tc_workspace_bytes(const Geometry& g, bool backward) {
+  (void)backward;
+  return tc_carve(g, nullptr).total;
+}
+
+cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const float* w1, const float* b1,
+                       const float* w2, const float* b2, void* y, void* ws, cudaStream_t st) {
+  TcWs w = tc_carve(g, (char*)ws);
+  const TcPlan& tp = p.tc;
+  cudaError_t e;
+  const int nW = g.nb * BS * BS;
+  prof_begin("k_tc_prep_weights", st);
+  k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, w2, w.wprep, g.nb);
+  prof_end(st);
+  count_launch();
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  const int ncg = (g.C + CGRP - 1) / CGRP;
+  const int row_tiles = g.B * g.H * ncg;
+  const int grid_row = row_tiles < tp.num_sms ? row_tiles : tp.num_sms;
+  prof_begin("tc_wdft_fwd", st);
+  tc_wdft_fwd<<<grid_row, 128, kRowSmem, st>>>((const __nv_bfloat16*)x, w.A1, tp.fw, g.B, g.H, g.W, g.C, g.Kw, g.nb);
+  prof_end(st);
+  count_launch();
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  MixParams mp{w.A1, w.A2, tp.dft, (const uint8_t*)w.wprep, b1, b2, g.B, g.H, g.Kw, g.nb, g.Kh, g.lambda};
+  const int mix_tiles = g.nb * g.B * g.Kw;
+  const int grid_mix = mix_tiles < tp.num_sms ? mix_tiles : tp.num_sms;
+  prof_begin("tc_mix_fwd", st);
+  tc_mix_fwd<<<grid_mix, 128, kMixSmem, st>>>(mp);
+  prof_end(st);
+  count_launch();
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  prof_begin("tc_wdft_inv", st);
+  tc_wdft_inv<<<grid_row, 128, kRowSmem, st>>>(w.A2, g.no_residual ? nullptr : (const __nv_bfloat16*)x,
+                                              (__nv_bfloat16*)y, tp.gw, g.B, g.H, g.W, g.C, g.Kw, g.nb);
+  prof_end(st);
+  count_launch();
+  return cudaGetLastError();
+}
+
+} // namespace afno

@@ -47,7 +47,27 @@ constexpr uint32_t kRowLbo = 128, kRowSbo = 3072;   // W-direction data tile: MN
 constexpr uint32_t kRowBytes = WP * CGRP * 2;        // 49152
 
 constexpr uint32_t kMixSmem = 2 * kDftBytes + 4 * kWBytes + kTileBytes + 2 * NT * 4; // 161280
-constexpr uint32_t kRowSmem = kFwBytes + kRowBytes;                                  // 122880
+constexpr int kTrPitch = 132;                        // fp32 words per row of the epilogue transpose buffer
+constexpr uint32_t kTrBytes = 32 * kTrPitch * 4;     // 16896
+constexpr uint32_t kRowSmem = kFwBytes + kRowBytes + kTrBytes;                       // 139776
+
+// Epilogue transpose of the W-direction kernels: every thread holds 32 consecutive accumulator
+// columns of ITS channel (TMEM lane).  The chunk goes through shared memory so that thread
+// (q, c4) = (tid/32 + 4*pass, tid%32) then owns 4 consecutive channels of column q and global
+// accesses become 8-byte vectors, 256 contiguous bytes per warp.
+template <typename F>
+__device__ __forceinline__ void transposed_chunk(float* sT, const uint32_t (&v)[32], int tid, F&& consume) {
+#pragma unroll
+  for (int q = 0; q < 32; ++q) sT[q * kTrPitch + tid] = __uint_as_float(v[q]);
+  __syncthreads();
+  const int c4 = (tid & 31) * 4;
+#pragma unroll
+  for (int pass = 0; pass < 8; ++pass) {
+    const int q = pass * 4 + (tid >> 5);
+    consume(pass, q, c4, *(const float4*)&sT[q * kTrPitch + c4]);
+  }
+  __syncthreads();
+}
 
 // ---- weight preparation: fp32 [nb][96][96][2] -> bf16 K-major interleaved operands --------------
 // per block, 8 matrices of kWBytes: fwd {W1r, W1i, W2r, W2i} with element (n=o, k=i) = W[i][o];
@@ -82,6 +102,7 @@ tc_wdft_fwd(const __nv_bfloat16* __restrict__ x, __nv_bfloat16* __restrict__ A1,
   __shared__ uint32_t tmem_slot;
   uint8_t* sF = smem;
   uint8_t* sA = smem + kFwBytes;
+  float* sT = (float*)(smem + kFwBytes + kRowBytes);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   for (uint32_t i = tid; i < kRowBytes / 16; i += 128) ((uint4*)sA)[i] = make_uint4(0, 0, 0, 0);
   for (uint32_t i = tid; i < kFwBytes / 16; i += 128) cp_async16(smem_u32(sF) + i * 16, FwT + (size_t)i * 16);
@@ -125,24 +146,22 @@ tc_wdft_fwd(const __nv_bfloat16* __restrict__ x, __nv_bfloat16* __restrict__ A1,
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-    const int c = cg * CGRP + tid;
     const int b = bh / H, h = bh - b * H;
-    const int j = c / BS, cl = c - j * BS;
 #pragma unroll 1
     for (int c0 = 0; c0 < NT; c0 += 32) {
       uint32_t v[32];
       tmem_ld32(tmem + lane_base + c0, v);
       tmem_wait_ld();
-      if (c < C) {
-#pragma unroll
-        for (int q = 0; q < 32; ++q) {
-          const int n = c0 + q;
-          const int ri = n >= BS ? 1 : 0, kw = n - ri * BS;
-          if (kw < Kw)
-            A1[((((size_t)b * Kw + kw) * nb + j) * H + h) * NT + ri * BS + cl] =
-                __float2bfloat16_rn(__uint_as_float(v[q]));
+      transposed_chunk(sT, v, tid, [&](int, int q, int c4, float4 f) {
+        const int n = c0 + q;
+        const int ri = n >= BS ? 1 : 0, kw = n - ri * BS;
+        const int c = cg * CGRP + c4;
+        if (kw < Kw && c < C) {
+          const int j = c / BS, cl = c - j * BS;
+          uint2 o = make_uint2(pack_bf16(f.x, f.y), pack_bf16(f.z, f.w));
+          *(uint2*)(A1 + ((((size_t)b * Kw + kw) * nb + j) * H + h) * NT + ri * BS + cl) = o;
         }
-      }
+      });
     }
   }
   tc_fence_before();
@@ -160,6 +179,7 @@ tc_wdft_inv(const __nv_bfloat16* __restrict__ A2, const __nv_bfloat16* __restric
   __shared__ uint32_t tmem_slot;
   uint8_t* sG = smem;
   uint8_t* sA = smem + kFwBytes;
+  float* sT = (float*)(smem + kFwBytes + kRowBytes);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   for (uint32_t i = tid; i < kRowBytes / 16; i += 128) ((uint4*)sA)[i] = make_uint4(0, 0, 0, 0);
   for (uint32_t i = tid; i < kFwBytes / 16; i += 128) cp_async16(smem_u32(sG) + i * 16, GwT + (size_t)i * 16);
@@ -209,24 +229,31 @@ tc_wdft_inv(const __nv_bfloat16* __restrict__ A2, const __nv_bfloat16* __restric
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-    const int c = cg * CGRP + tid;
-    const size_t rowoff = (size_t)bh * W * C + c;
+    const int cbase = cg * CGRP + (tid & 31) * 4;
+    const size_t rowoff = (size_t)bh * W * C + cbase;
 #pragma unroll 1
     for (int c0 = 0; c0 < WP; c0 += 32) {
       uint32_t v[32];
       tmem_ld32(tmem + lane_base + c0, v);
       tmem_wait_ld();
-      if (c < C) {
+      // residual rows of this chunk first (8 independent 8-byte loads in flight per thread)
+      uint2 rr[8];
 #pragma unroll
-        for (int q = 0; q < 32; ++q) {
-          const int w = c0 + q;
-          if (w < W) {
-            float val = __uint_as_float(v[q]);
-            if (res) val += __bfloat162float(res[rowoff + (size_t)w * C]);
-            y[rowoff + (size_t)w * C] = __float2bfloat16_rn(val);
-          }
-        }
+      for (int pass = 0; pass < 8; ++pass) {
+        const int w = c0 + pass * 4 + (tid >> 5);
+        rr[pass] = make_uint2(0u, 0u);
+        if (res && w < W && cbase < C) rr[pass] = __ldg((const uint2*)(res + rowoff + (size_t)w * C));
       }
+      transposed_chunk(sT, v, tid, [&](int pass, int q, int c4, float4 f) {
+        const int w = c0 + q;
+        if (w < W && cbase < C) {
+          const uint2 r2 = rr[pass];
+          const float2 ra = __bfloat1622float2(*(const __nv_bfloat162*)&r2.x);
+          const float2 rb = __bfloat1622float2(*(const __nv_bfloat162*)&r2.y);
+          uint2 o = make_uint2(pack_bf16(f.x + ra.x, f.y + ra.y), pack_bf16(f.z + rb.x, f.w + rb.y));
+          *(uint2*)(y + rowoff + (size_t)w * C) = o;
+        }
+      });
     }
   }
   tc_fence_before();

@@ -77,9 +77,9 @@ int resolve(const afno_desc_t* d, Geometry* g) {
   return AFNO_OK;
 }
 
-// which kernel family serves the descriptor (the backward still runs on the generic path)
+// which kernel family serves the descriptor
 bool use_tc_fwd(const Geometry& g) { return !g.force_fp32 && tc_supported(g); }
-bool use_tc_bwd(const Geometry&) { return false; }
+bool use_tc_bwd(const Geometry& g) { return use_tc_fwd(g); }
 size_t workspace_bytes(const Geometry& g, bool backward) {
   if (backward) return use_tc_bwd(g) ? tc_workspace_bytes(g, true) : generic_workspace_bytes(g, true);
   return use_tc_fwd(g) ? tc_workspace_bytes(g, false) : generic_workspace_bytes(g, false);
@@ -354,7 +354,9 @@ int afno_spectral_bwd(const afno_desc_t* d, const void* x, const void* dy, const
   if (rc != AFNO_OK) return rc;
   size_t m1 = 0, m2off = 0, m2 = 0;
   afno_spectral_mask_bytes(d, &m1, &m2off, &m2);
-  cudaError_t e = generic_backward(g, *p, x, dy, w1, b1, w2, b2, dx, dw1, db1, dw2, db2, workspace, m1, m2off, st);
+  cudaError_t e = (use_tc_bwd(g) && p->tc.valid)
+                      ? tc_backward(g, *p, x, dy, w1, b1, w2, b2, dx, dw1, db1, dw2, db2, workspace, st)
+                      : generic_backward(g, *p, x, dy, w1, b1, w2, b2, dx, dw1, db1, dw2, db2, workspace, m1, m2off, st);
   if (e != cudaSuccess) return fail(AFNO_ERR_CUDA, std::string("backward launch: ") + cudaGetErrorString(e));
   return AFNO_OK;
 }

@@ -68,6 +68,10 @@ size_t tc_workspace_bytes(const Geometry& g, bool backward);
 cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const float* w1, const float* b1,
                        const float* w2, const float* b2, void* y, void* ws, cudaStream_t st);
 
+cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const void* dy, const float* w1,
+                        const float* b1, const float* w2, const float* b2, void* dx, float* dw1, float* db1,
+                        float* dw2, float* db2, void* ws, cudaStream_t st);
+
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 } // namespace afno

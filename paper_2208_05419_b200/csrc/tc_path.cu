@@ -482,6 +482,482 @@ __global__ void __launch_bounds__(128, 1) tc_mix_fwd(MixParams p) {
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
+// ---- B1-B7 (except the parameter sums): per (b, kw, block) backward chain ------------------------
+//   recompute  Xh = Fh A1x -> P1 -> O1 -> P2 (masks kept as bit sets in registers)
+//   G = Fh A1g ; G2 = G (.) mask2 ; G1 = mask1 (.) (G2 W2^H) ; GX = G1 W1^H ; A2 = Fh^H GX
+// Xh, O1, G2, G1 are also written (bf16, tile layout [b*Kw+kw][j][r][192]) for tc_wgrad.
+struct MixBwdParams {
+  const __nv_bfloat16* A1x;
+  const __nv_bfloat16* A1g;
+  __nv_bfloat16* A2;
+  __nv_bfloat16 *Xh, *O1, *G2, *G1;
+  const uint8_t* dft;
+  const uint8_t* wprep;
+  const float* b1;
+  const float* b2;
+  uint8_t* mask1; // optional export, [B][H][Wh][C][2]
+  uint8_t* mask2;
+  int B, H, Kw, Wh, nb, Kh;
+  float lambda;
+};
+
+// D[:, dcol .. dcol+96) (+)= A_tmem(packed, K = 96 output features o) * W^H part: the forward
+// weight image (n=o, k=i, K-major) read as an MN-major B operand with (k=o, n=i)
+__device__ __forceinline__ void issue_mlp_t(uint32_t d, uint32_t a_tmem, uint32_t w_base, uint32_t idesc, bool fresh) {
+#pragma unroll
+  for (int ks = 0; ks < BS / 16; ++ks)
+    mma_ts(d, a_tmem + ks * 8, smem_desc(w_base + ks * 2 * kWSbo, kWSbo, kWLbo), idesc, !(fresh && ks == 0));
+}
+
+__device__ __forceinline__ void store_row_chunk(__nv_bfloat16* dst, const uint32_t (&pk)[16]) {
+#pragma unroll
+  for (int g = 0; g < 4; ++g) *(uint4*)(dst + g * 8) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
+}
+
+constexpr uint32_t kMixBwdSmem = kMixSmem + kTileBytes; // second tile buffer for the gradient spectrum
+
+__global__ void __launch_bounds__(128, 1) tc_mix_bwd(MixBwdParams p) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t mbar;
+  __shared__ uint32_t tmem_slot;
+  uint8_t* sCh = smem;
+  uint8_t* sSh = smem + kDftBytes;
+  uint8_t* sW = smem + 2 * kDftBytes;
+  uint8_t* sTile = sW + 4 * kWBytes;
+  float* sBias = (float*)(sTile + kTileBytes);
+  uint8_t* sTileG = sTile + kTileBytes + 2 * NT * 4;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  for (uint32_t i = tid; i < kTileBytes / 16; i += 128) {
+    ((uint4*)sTile)[i] = make_uint4(0, 0, 0, 0);
+    ((uint4*)sTileG)[i] = make_uint4(0, 0, 0, 0);
+  }
+  for (uint32_t i = tid; i < 2 * kDftBytes / 16; i += 128) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
+  if (tid == 0) {
+    mbar_init(&mbar, 1);
+    mbar_init_fence();
+  }
+  if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+  const uint32_t R0 = tmem, R1 = tmem + 256;
+  const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW);
+  const uint32_t aTile = smem_u32(sTile), aTileG = smem_u32(sTileG);
+  const uint32_t half = (BS / 8) * kTileSbo;
+  const uint32_t id_dft = idesc_bf16(128, BS, kIdescBMn);
+  const uint32_t id_mlp = idesc_bf16(128, BS);
+  const uint32_t id_mlp_t = idesc_bf16(128, BS, kIdescBMn);
+
+  const int ntiles = p.nb * p.B * p.Kw;
+  const int per = (ntiles + gridDim.x - 1) / gridDim.x;
+  const int t_begin = blockIdx.x * per, t_end = min(ntiles, t_begin + per);
+  uint32_t phase = 0;
+  int cur_j = -1;
+  const int r = tid;
+  const int kappa = (r <= p.H / 2) ? r : p.H - r;
+  const bool row_valid = r < p.H;
+  const bool row_kept = row_valid && (kappa < p.Kh);
+  const int hl = lane & 7, cl4 = lane >> 3;
+
+  for (int t = t_begin; t < t_end; ++t) {
+    const int j = t / (p.B * p.Kw);
+    const int rem = t - j * (p.B * p.Kw);
+    if (j != cur_j) {
+      cur_j = j;
+      const uint8_t* wsrc = p.wprep + (size_t)j * 8 * kWBytes;
+      for (uint32_t i = tid; i < 4 * kWBytes / 16; i += 128) cp_async16(aW + i * 16, wsrc + (size_t)i * 16);
+      for (int i = tid; i < 2 * NT; i += 128) {
+        const int which = i / NT, n = i % NT, ri = n / BS, o = n % BS;
+        sBias[i] = (which == 0 ? p.b1 : p.b2)[((size_t)j * BS + o) * 2 + ri];
+      }
+    }
+    const size_t tile_off = ((size_t)rem * p.nb + j) * p.H * NT;
+    {
+      const __nv_bfloat16* srcx = p.A1x + tile_off;
+      const __nv_bfloat16* srcg = p.A1g + tile_off;
+      const int nunits = ((p.H + 7) / 8) * 6;
+      for (int u = warp; u < nunits; u += 4) {
+        const int h = (u / 6) * 8 + hl;
+        const int nc = (u % 6) * 4 + cl4;
+        if (h < p.H) {
+          cp_async16(aTile + nc * kTileSbo + h * 16, srcx + (size_t)h * NT + nc * 8);
+          cp_async16(aTileG + nc * kTileSbo + h * 16, srcg + (size_t)h * NT + nc * 8);
+        }
+      }
+    }
+    const size_t row_off = tile_off + (size_t)r * NT;
+    cp_async_wait_all();
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    // ---- Xh = Fh A1x -----------------------------------------------------------------------
+    if (tid == 0) {
+      tc_fence_after();
+      issue_dft(R0, aCh, aTile, id_dft, true);
+      issue_dft(R0, aSh, aTile + half, id_dft, false);
+      issue_dft(R0 + BS, aCh, aTile + half, id_dft, true);
+      issue_dft(R0 + BS, aSh, aTile, id_dft | kIdescNegA, false);
+      mma_commit(&mbar);
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+#pragma unroll 1
+    for (int c0 = 0; c0 < NT; c0 += 32) {
+      uint32_t v[32], pk[16];
+      tmem_ld32(R0 + lane_base + c0, v);
+      tmem_wait_ld();
+#pragma unroll
+      for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
+      tmem_st16(R0 + lane_base + c0 / 2, pk);
+      if (row_valid) store_row_chunk(p.Xh + row_off + c0, pk);
+    }
+    tmem_wait_st();
+    tc_fence_before();
+    __syncthreads();
+    // ---- P1 = Xh W1 + b1 ; O1 = relu ; mask1 -------------------------------------------------
+    if (tid == 0) {
+      tc_fence_after();
+      issue_mlp(R1, R0, aW + 0 * kWBytes, id_mlp, true);
+      issue_mlp(R1, R0 + BS / 2, aW + 1 * kWBytes, id_mlp | kIdescNegB, false);
+      issue_mlp(R1 + BS, R0, aW + 1 * kWBytes, id_mlp, true);
+      issue_mlp(R1 + BS, R0 + BS / 2, aW + 0 * kWBytes, id_mlp, false);
+      mma_commit(&mbar);
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+    uint32_t m1[6], m2[6];
+#pragma unroll 1
+    for (int ch = 0; ch < 6; ++ch) {
+      const int c0 = ch * 32;
+      uint32_t v[32], pk[16];
+      tmem_ld32(R1 + lane_base + c0, v);
+      tmem_wait_ld();
+      uint32_t bits = 0;
+#pragma unroll
+      for (int q = 0; q < 16; ++q) {
+        const float a = __uint_as_float(v[2 * q]) + sBias[c0 + 2 * q];
+        const float b = __uint_as_float(v[2 * q + 1]) + sBias[c0 + 2 * q + 1];
+        bits |= (a > 0.f ? 1u : 0u) << (2 * q);
+        bits |= (b > 0.f ? 1u : 0u) << (2 * q + 1);
+        pk[q] = pack_bf16(fmaxf(a, 0.f), fmaxf(b, 0.f));
+      }
+      m1[ch] = bits;
+      tmem_st16(R1 + lane_base + c0 / 2, pk);
+      if (row_valid) store_row_chunk(p.O1 + row_off + c0, pk);
+    }
+    tmem_wait_st();
+    tc_fence_before();
+    __syncthreads();
+    // ---- P2 = O1 W2 + b2 ; mask2 ----------------------------------------------------------------
+    if (tid == 0) {
+      tc_fence_after();
+      issue_mlp(R0, R1, aW + 2 * kWBytes, id_mlp, true);
+      issue_mlp(R0, R1 + BS / 2, aW + 3 * kWBytes, id_mlp | kIdescNegB, false);
+      issue_mlp(R0 + BS, R1, aW + 3 * kWBytes, id_mlp, true);
+      issue_mlp(R0 + BS, R1 + BS / 2, aW + 2 * kWBytes, id_mlp, false);
+      mma_commit(&mbar);
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+#pragma unroll 1
+    for (int ch = 0; ch < 6; ++ch) {
+      const int c0 = ch * 32;
+      uint32_t v[32];
+      tmem_ld32(R0 + lane_base + c0, v);
+      tmem_wait_ld();
+      uint32_t bits = 0;
+#pragma unroll
+      for (int q = 0; q < 32; ++q)
+        bits |= (fabsf(__uint_as_float(v[q]) + sBias[NT + c0 + q]) > p.lambda ? 1u : 0u) << q;
+      m2[ch] = row_kept ? bits : 0u;
+    }
+    tc_fence_before();
+    __syncthreads();
+    // ---- G = Fh A1g ; G2 = G (.) mask2 -----------------------------------------------------------
+    if (tid == 0) {
+      tc_fence_after();
+      issue_dft(R1, aCh, aTileG, id_dft, true);
+      issue_dft(R1, aSh, aTileG + half, id_dft, false);
+      issue_dft(R1 + BS, aCh, aTileG + half, id_dft, true);
+      issue_dft(R1 + BS, aSh, aTileG, id_dft | kIdescNegA, false);
+      mma_commit(&mbar);
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+#pragma unroll 1
+    for (int ch = 0; ch < 6; ++ch) {
+      const int c0 = ch * 32;
+      uint32_t v[32], pk[16];
+      tmem_ld32(R1 + lane_base + c0, v);
+      tmem_wait_ld();
+      const uint32_t bits = m2[ch];
+#pragma unroll
+      for (int q = 0; q < 16; ++q) {
+        const float a = (bits >> (2 * q)) & 1u ? __uint_as_float(v[2 * q]) : 0.f;
+        const float b = (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[2 * q + 1]) : 0.f;
+        pk[q] = pack_bf16(a, b);
+      }
+      tmem_st16(R1 + lane_base + c0 / 2, pk);
+      if (row_valid) store_row_chunk(p.G2 + row_off + c0, pk);
+    }
+    tmem_wait_st();
+    tc_fence_before();
+    __syncthreads();
+    // ---- G1 = mask1 (.) (G2 W2^H):  re = G2r W2r^T + G2i W2i^T ; im = G2i W2r^T - G2r W2i^T ----
+    if (tid == 0) {
+      tc_fence_after();
+      issue_mlp_t(R0, R1, aW + 2 * kWBytes, id_mlp_t, true);
+      issue_mlp_t(R0, R1 + BS / 2, aW + 3 * kWBytes, id_mlp_t, false);
+      issue_mlp_t(R0 + BS, R1 + BS / 2, aW + 2 * kWBytes, id_mlp_t, true);
+      issue_mlp_t(R0 + BS, R1, aW + 3 * kWBytes, id_mlp_t | kIdescNegB, false);
+      mma_commit(&mbar);
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+#pragma unroll 1
+    for (int ch = 0; ch < 6; ++ch) {
+      const int c0 = ch * 32;
+      uint32_t v[32], pk[16];
+      tmem_ld32(R0 + lane_base + c0, v);
+      tmem_wait_ld();
+      const uint32_t bits = m1[ch];
+#pragma unroll
+      for (int q = 0; q < 16; ++q) {
+        const float a = (bits >> (2 * q)) & 1u ? __uint_as_float(v[2 * q]) : 0.f;
+        const float b = (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[2 * q + 1]) : 0.f;
+        pk[q] = pack_bf16(a, b);
+      }
+      tmem_st16(R0 + lane_base + c0 / 2, pk);
+      if (row_valid) store_row_chunk(p.G1 + row_off + c0, pk);
+    }
+    tmem_wait_st();
+    tc_fence_before();
+    __syncthreads();
+    // ---- GX = G1 W1^H ----------------------------------------------------------------------------
+    if (tid == 0) {
+      tc_fence_after();
+      issue_mlp_t(R1, R0, aW + 0 * kWBytes, id_mlp_t, true);
+      issue_mlp_t(R1, R0 + BS / 2, aW + 1 * kWBytes, id_mlp_t, false);
+      issue_mlp_t(R1 + BS, R0 + BS / 2, aW + 0 * kWBytes, id_mlp_t, true);
+      issue_mlp_t(R1 + BS, R0, aW + 1 * kWBytes, id_mlp_t | kIdescNegB, false);
+      mma_commit(&mbar);
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+#pragma unroll 1
+    for (int c0 = 0; c0 < NT; c0 += 32) {
+      uint32_t v[32];
+      tmem_ld32(R1 + lane_base + c0, v);
+      tmem_wait_ld();
+      if (r < HP) {
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {
+          uint4 o;
+          o.x = row_valid ? pack_bf16(__uint_as_float(v[g * 8 + 0]), __uint_as_float(v[g * 8 + 1])) : 0u;
+          o.y = row_valid ? pack_bf16(__uint_as_float(v[g * 8 + 2]), __uint_as_float(v[g * 8 + 3])) : 0u;
+          o.z = row_valid ? pack_bf16(__uint_as_float(v[g * 8 + 4]), __uint_as_float(v[g * 8 + 5])) : 0u;
+          o.w = row_valid ? pack_bf16(__uint_as_float(v[g * 8 + 6]), __uint_as_float(v[g * 8 + 7])) : 0u;
+          *(uint4*)(sTile + ((c0 >> 3) + g) * kTileSbo + r * 16) = o;
+        }
+      }
+    }
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    // ---- A2 = Fh^H GX (inverse kernel) ---------------------------------------------------------
+    if (tid == 0) {
+      tc_fence_after();
+      issue_dft(R0, aCh, aTile, id_dft, true);
+      issue_dft(R0, aSh, aTile + half, id_dft | kIdescNegA, false);
+      issue_dft(R0 + BS, aCh, aTile + half, id_dft, true);
+      issue_dft(R0 + BS, aSh, aTile, id_dft, false);
+      mma_commit(&mbar);
+    }
+    // optional mask export while the tensor core works
+    if (p.mask1 != nullptr && row_valid) {
+      const int b = rem / p.Kw, kw = rem - b * p.Kw;
+      const size_t base = ((((size_t)b * p.H + r) * p.Wh + kw) * (size_t)(p.nb * BS) + (size_t)j * BS) * 2;
+#pragma unroll 1
+      for (int o8 = 0; o8 < BS; o8 += 8) {
+        uint32_t w1[4], w2[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          uint32_t a = 0, b2v = 0;
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int o = o8 + 2 * q + e;
+            const int nre = o, nim = BS + o;
+            const uint32_t r1 = (m1[nre >> 5] >> (nre & 31)) & 1u, i1 = (m1[nim >> 5] >> (nim & 31)) & 1u;
+            const uint32_t r2 = (m2[nre >> 5] >> (nre & 31)) & 1u, i2 = (m2[nim >> 5] >> (nim & 31)) & 1u;
+            a |= (r1 | (i1 << 8)) << (16 * e);
+            b2v |= (r2 | (i2 << 8)) << (16 * e);
+          }
+          w1[q] = a;
+          w2[q] = b2v;
+        }
+        *(uint4*)(p.mask1 + base + o8 * 2) = make_uint4(w1[0], w1[1], w1[2], w1[3]);
+        *(uint4*)(p.mask2 + base + o8 * 2) = make_uint4(w2[0], w2[1], w2[2], w2[3]);
+      }
+    }
+    mbar_wait(&mbar, phase);
+    phase ^= 1;
+    tc_fence_after();
+#pragma unroll 1
+    for (int c0 = 0; c0 < NT; c0 += 32) {
+      uint32_t v[32], pk[16];
+      tmem_ld32(R0 + lane_base + c0, v);
+      tmem_wait_ld();
+#pragma unroll
+      for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
+      if (row_valid) store_row_chunk(p.A2 + row_off + c0, pk);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<512>(tmem);
+}
+
+// ---- B4 / B6: parameter gradients as a split-K tensor-core GEMM ------------------------------------
+// For block j:  R[(ri_a,i), (ri_g,o)] = sum_rows A[row,(ri_a,i)] * G[row,(ri_g,o)] with K = mode rows.
+// Two M=128 accumulators: D_re rows = (re, i) plus a constant-one row 96 (gives sum_rows G = db),
+// D_im rows = (im, i).  CTA (j, s) sums tiles rem = s, s+S, ... and writes its partial sums.
+constexpr uint32_t kWgABytes = HP * 128 * 2;                           // 24576: MN-major A [K=96][M=128]
+constexpr uint32_t kWgStage = 2 * kWgABytes + kTileBytes;              // 86016
+constexpr uint32_t kWgSmem = 2 * kWgStage;                             // 172032
+constexpr uint32_t kWgALbo = 128, kWgASbo = 1536;
+
+__global__ void __launch_bounds__(128, 1)
+tc_wgrad(const __nv_bfloat16* __restrict__ Aws, const __nv_bfloat16* __restrict__ Gws, float* __restrict__ part,
+         int BKw, int H, int nb, int S) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t mbar[2];
+  __shared__ uint32_t tmem_slot;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int j = blockIdx.x / S, s = blockIdx.x - j * S;
+  for (uint32_t i = tid; i < kWgSmem / 16; i += 128) ((uint4*)smem)[i] = make_uint4(0, 0, 0, 0);
+  __syncthreads();
+  // constant-one column m = 96 of the "re" A operand, rows r < H, both stages
+  for (int i = tid; i < 2 * H; i += 128) {
+    const int st = i / H, rr = i - st * H;
+    *(uint16_t*)(smem + st * kWgStage + 12 * kWgASbo + rr * 16) = 0x3F80; // bf16 1.0
+  }
+  if (tid == 0) {
+    mbar_init(&mbar[0], 1);
+    mbar_init(&mbar[1], 1);
+    mbar_init_fence();
+  }
+  if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+  const uint32_t Dre = tmem, Dim = tmem + 256;
+  const uint32_t idesc = idesc_bf16(128, NT, kIdescAMn | kIdescBMn);
+  const int nt = (BKw - s + S - 1) / S; // tiles of this CTA
+  const int hl = lane & 7, cl4 = lane >> 3;
+  auto prefetch = [&](int it) {
+    const int rem = s + it * S;
+    const uint32_t stage = smem_u32(smem) + (it & 1) * kWgStage;
+    const size_t off = ((size_t)rem * nb + j) * H * NT;
+    const int nunits = ((H + 7) / 8) * 6;
+    for (int u = warp; u < nunits; u += 4) {
+      const int h = (u / 6) * 8 + hl;
+      const int nc = (u % 6) * 4 + cl4;
+      if (h < H) {
+        const uint32_t adst = stage + (nc < 12 ? 0u : kWgABytes) + (nc % 12) * kWgASbo + h * 16;
+        cp_async16(adst, Aws + off + (size_t)h * NT + nc * 8);
+        cp_async16(stage + 2 * kWgABytes + nc * kTileSbo + h * 16, Gws + off + (size_t)h * NT + nc * 8);
+      }
+    }
+  };
+  if (nt > 0) prefetch(0);
+  cp_async_commit();
+  for (int it = 0; it < nt; ++it) {
+    if (it + 1 < nt) {
+      if (it >= 1) mbar_wait(&mbar[(it + 1) & 1], (uint32_t)(((it - 1) >> 1) & 1));
+      prefetch(it + 1);
+    }
+    cp_async_commit();
+    cp_async_wait_group<1>();
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (tid == 0) {
+      tc_fence_after();
+      const uint32_t stage = smem_u32(smem) + (it & 1) * kWgStage;
+      const uint32_t g = stage + 2 * kWgABytes;
+#pragma unroll
+      for (int ks = 0; ks < HP / 16; ++ks) {
+        const uint64_t bd = smem_desc(g + ks * 2 * kTileLbo, kTileLbo, kTileSbo);
+        mma_ss(Dre, smem_desc(stage + ks * 2 * kWgALbo, kWgALbo, kWgASbo), bd, idesc, (it | ks) != 0);
+        mma_ss(Dim, smem_desc(stage + kWgABytes + ks * 2 * kWgALbo, kWgALbo, kWgASbo), bd, idesc, (it | ks) != 0);
+      }
+      mma_commit(&mbar[it & 1]);
+    }
+  }
+  float* dst = part + ((size_t)blockIdx.x * 2) * 128 * NT + (size_t)tid * NT;
+  if (nt > 0) {
+    mbar_wait(&mbar[(nt - 1) & 1], (uint32_t)(((nt - 1) >> 1) & 1));
+    tc_fence_after();
+#pragma unroll 1
+    for (int acc = 0; acc < 2; ++acc)
+#pragma unroll 1
+      for (int c0 = 0; c0 < NT; c0 += 32) {
+        uint32_t v[32];
+        tmem_ld32((acc ? Dim : Dre) + lane_base + c0, v);
+        tmem_wait_ld();
+#pragma unroll
+        for (int q = 0; q < 32; q += 4)
+          *(float4*)(dst + (size_t)acc * 128 * NT + c0 + q) =
+              make_float4(__uint_as_float(v[q]), __uint_as_float(v[q + 1]), __uint_as_float(v[q + 2]),
+                          __uint_as_float(v[q + 3]));
+      }
+  } else {
+    for (int acc = 0; acc < 2; ++acc)
+      for (int c0 = 0; c0 < NT; c0 += 4) *(float4*)(dst + (size_t)acc * 128 * NT + c0) = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<512>(tmem);
+}
+
+// dW[j][i][o] = sum_s ( Dre[i][o] + Dim[i][96+o] ,  Dre[i][96+o] - Dim[i][o] ) ;  db[j][o] = sum_s Dre[96][(ri,o)]
+__global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __restrict__ dW, float2* __restrict__ dB,
+                                  int nb, int S, int accumulate) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int nW = nb * BS * BS;
+  if (idx < nW) {
+    const int o = idx % BS, i = (idx / BS) % BS, j = idx / (BS * BS);
+    float2 acc = accumulate ? dW[idx] : make_float2(0.f, 0.f);
+    for (int s = 0; s < S; ++s) {
+      const float* P = part + ((size_t)(j * S + s) * 2) * 128 * NT;
+      const float* Pre = P + (size_t)i * NT;
+      const float* Pim = P + (size_t)128 * NT + (size_t)i * NT;
+      acc.x += Pre[o] + Pim[BS + o];
+      acc.y += Pre[BS + o] - Pim[o];
+    }
+    dW[idx] = acc;
+  } else if (idx < nW + nb * BS) {
+    const int k = idx - nW, o = k % BS, j = k / BS;
+    float2 acc = accumulate ? dB[k] : make_float2(0.f, 0.f);
+    for (int s = 0; s < S; ++s) {
+      const float* P = part + ((size_t)(j * S + s) * 2) * 128 * NT + (size_t)96 * NT;
+      acc.x += P[o];
+      acc.y += P[BS + o];
+    }
+    dB[k] = acc;
+  }
+}
+
 // ---- host side: constant operand images ------------------------------------------------------------
 uint16_t host_bf16(double v) {
   float f = (float)v;
@@ -504,9 +980,14 @@ cudaError_t set_smem(K kernel, size_t bytes) {
 
 struct TcWs {
   __nv_bfloat16 *A1, *A2, *wprep;
+  __nv_bfloat16 *A1g, *Xh, *O1, *G2, *G1; // backward only
+  float* part;
+  uint8_t *mask1, *mask2;
+  size_t mask_region;
+  int S;
   size_t total;
 };
-TcWs tc_carve(const Geometry& g, char* base) {
+TcWs tc_carve(const Geometry& g, bool backward, char* base) {
   TcWs w{};
   size_t off = 0;
   auto take = [&](size_t bytes) {
@@ -514,10 +995,28 @@ TcWs tc_carve(const Geometry& g, char* base) {
     off = align_up(off + bytes, 256);
     return p;
   };
+  if (backward && g.export_masks) {
+    const size_t b1 = (size_t)g.modes_all() * g.CH * 2, b2 = (size_t)g.modes_all() * g.C * 2;
+    w.mask1 = (uint8_t*)take(b1);
+    w.mask2 = (uint8_t*)take(b2);
+    w.mask_region = off;
+  }
   const size_t spec = (size_t)g.B * g.Kw * g.nb * g.H * NT * 2;
   w.A1 = (__nv_bfloat16*)take(spec);
   w.A2 = (__nv_bfloat16*)take(spec);
   w.wprep = (__nv_bfloat16*)take((size_t)g.nb * 8 * kWBytes);
+  if (backward) {
+    w.A1g = (__nv_bfloat16*)take(spec);
+    w.Xh = (__nv_bfloat16*)take(spec);
+    w.O1 = (__nv_bfloat16*)take(spec);
+    w.G2 = (__nv_bfloat16*)take(spec);
+    w.G1 = (__nv_bfloat16*)take(spec);
+    int S = 148 / g.nb;
+    if (S < 1) S = 1;
+    if (S > g.B * g.Kw) S = g.B * g.Kw;
+    w.S = S;
+    w.part = (float*)take((size_t)g.nb * S * 2 * 128 * NT * sizeof(float));
+  }
   w.total = off;
   return w;
 }
@@ -566,6 +1065,8 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
   if (e == cudaSuccess) e = set_smem(tc_wdft_fwd, kRowSmem);
   if (e == cudaSuccess) e = set_smem(tc_wdft_inv, kRowSmem);
   if (e == cudaSuccess) e = set_smem(tc_mix_fwd, kMixSmem);
+  if (e == cudaSuccess) e = set_smem(tc_mix_bwd, kMixBwdSmem);
+  if (e == cudaSuccess) e = set_smem(tc_wgrad, kWgSmem);
   int dev = 0, sms = 148;
   if (e == cudaSuccess) e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -575,13 +1076,12 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
 }
 
 size_t tc_workspace_bytes(const Geometry& g, bool backward) {
-  (void)backward;
-  return tc_carve(g, nullptr).total;
+  return tc_carve(g, backward, nullptr).total;
 }
 
 cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const float* w1, const float* b1,
                        const float* w2, const float* b2, void* y, void* ws, cudaStream_t st) {
-  TcWs w = tc_carve(g, (char*)ws);
+  TcWs w = tc_carve(g, false, (char*)ws);
   const TcPlan& tp = p.tc;
   cudaError_t e;
   const int nW = g.nb * BS * BS;
@@ -612,6 +1112,57 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   prof_end(st);
   count_launch();
   return cudaGetLastError();
+}
+
+cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const void* dy, const float* w1,
+                        const float* b1, const float* w2, const float* b2, void* dx, float* dw1, float* db1,
+                        float* dw2, float* db2, void* ws, cudaStream_t st) {
+  TcWs w = tc_carve(g, true, (char*)ws);
+  const TcPlan& tp = p.tc;
+  cudaError_t e;
+#define TC_LAUNCH(name, ...)                                  \
+  prof_begin(name, st);                                       \
+  __VA_ARGS__;                                                \
+  prof_end(st);                                               \
+  count_launch();                                             \
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  const int nW = g.nb * BS * BS;
+  if (g.export_masks) {
+    if ((e = cudaMemsetAsync(ws, 0, w.mask_region, st)) != cudaSuccess) return e;
+  }
+  TC_LAUNCH("k_tc_prep_weights", k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, w2, w.wprep, g.nb));
+  const int ncg = (g.C + CGRP - 1) / CGRP;
+  const int row_tiles = g.B * g.H * ncg;
+  const int grid_row = row_tiles < tp.num_sms ? row_tiles : tp.num_sms;
+  // B1 (first half) and B2: W-direction spectra of x and of dy (alpha-weighted)
+  TC_LAUNCH("tc_wdft_fwd", tc_wdft_fwd<<<grid_row, 128, kRowSmem, st>>>((const __nv_bfloat16*)x, w.A1, tp.fw, g.B,
+                                                                       g.H, g.W, g.C, g.Kw, g.nb));
+  TC_LAUNCH("tc_wdft_fwd", tc_wdft_fwd<<<grid_row, 128, kRowSmem, st>>>((const __nv_bfloat16*)dy, w.A1g, tp.fw_alpha,
+                                                                       g.B, g.H, g.W, g.C, g.Kw, g.nb));
+  MixBwdParams mp{};
+  mp.A1x = w.A1; mp.A1g = w.A1g; mp.A2 = w.A2;
+  mp.Xh = w.Xh; mp.O1 = w.O1; mp.G2 = w.G2; mp.G1 = w.G1;
+  mp.dft = tp.dft; mp.wprep = (const uint8_t*)w.wprep; mp.b1 = b1; mp.b2 = b2;
+  mp.mask1 = g.export_masks ? w.mask1 : nullptr;
+  mp.mask2 = g.export_masks ? w.mask2 : nullptr;
+  mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
+  const int mix_tiles = g.nb * g.B * g.Kw;
+  const int grid_mix = mix_tiles < tp.num_sms ? mix_tiles : tp.num_sms;
+  TC_LAUNCH("tc_mix_bwd", tc_mix_bwd<<<grid_mix, 128, kMixBwdSmem, st>>>(mp));
+  // B4 / B6: parameter gradients
+  const int nred = nW + g.nb * BS;
+  TC_LAUNCH("tc_wgrad", tc_wgrad<<<g.nb * w.S, 128, kWgSmem, st>>>(w.O1, w.G2, w.part, g.B * g.Kw, g.H, g.nb, w.S));
+  TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce<<<(nred + 255) / 256, 256, 0, st>>>(
+                                     w.part, (float2*)dw2, (float2*)db2, g.nb, w.S, g.accum ? 1 : 0));
+  TC_LAUNCH("tc_wgrad", tc_wgrad<<<g.nb * w.S, 128, kWgSmem, st>>>(w.Xh, w.G1, w.part, g.B * g.Kw, g.H, g.nb, w.S));
+  TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce<<<(nred + 255) / 256, 256, 0, st>>>(
+                                     w.part, (float2*)dw1, (float2*)db1, g.nb, w.S, g.accum ? 1 : 0));
+  // B8: dx = dy + irfft2(GX / alpha)
+  TC_LAUNCH("tc_wdft_inv", tc_wdft_inv<<<grid_row, 128, kRowSmem, st>>>(
+                               w.A2, g.no_residual ? nullptr : (const __nv_bfloat16*)dy, (__nv_bfloat16*)dx,
+                               tp.gw_noalpha, g.B, g.H, g.W, g.C, g.Kw, g.nb));
+#undef TC_LAUNCH
+  return cudaSuccess;
 }
 
 } // namespace afno

@@ -262,8 +262,10 @@ tc_wdft_inv(const __nv_bfloat16* __restrict__ A2, const __nv_bfloat16* __restric
 }
 
 // ---- F2-F7: per (b, kw, block) chain  H-DFT -> layer 1 -> layer 2 -> inverse H-DFT ---------------
-// Accumulators in tensor memory: region R0 = columns [0,192), R1 = [256,448); a layer's bf16
-// input (A operand) is written in place over the fp32 accumulator it was computed from.
+// 256 threads: warp w owns TMEM lanes 32*(w&3).. (accumulator rows) and the column half w>>2
+// (re | im), so every epilogue is split two ways.  Accumulators in tensor memory: region R0 =
+// columns [0,192), R1 = [256,448); a layer's bf16 input (A operand) is packed in place over
+// the fp32 accumulator it was computed from (all loads, block barrier, then the stores).
 struct MixParams {
   const __nv_bfloat16* A1;
   __nv_bfloat16* A2;
@@ -274,6 +276,8 @@ struct MixParams {
   int B, H, Kw, nb, Kh;
   float lambda;
 };
+
+constexpr int kMixThreads = 256;
 
 // D[:, dcol .. dcol+96) (+)= A_smem(K-major [128 x 96]) * tile half (MN-major, 96 columns)
 __device__ __forceinline__ void issue_dft(uint32_t d, uint32_t a_base, uint32_t b_base, uint32_t idesc, bool fresh) {
@@ -288,19 +292,81 @@ __device__ __forceinline__ void issue_mlp(uint32_t d, uint32_t a_tmem, uint32_t 
   for (int ks = 0; ks < BS / 16; ++ks)
     mma_ts(d, a_tmem + ks * 8, smem_desc(w_base + ks * 2 * kWLbo, kWLbo, kWSbo), idesc, !(fresh && ks == 0));
 }
+// same with W^H: the forward weight image (n=o, k=i, K-major) read as an MN-major B operand (k=o, n=i)
+__device__ __forceinline__ void issue_mlp_t(uint32_t d, uint32_t a_tmem, uint32_t w_base, uint32_t idesc, bool fresh) {
+#pragma unroll
+  for (int ks = 0; ks < BS / 16; ++ks)
+    mma_ts(d, a_tmem + ks * 8, smem_desc(w_base + ks * 2 * kWSbo, kWSbo, kWLbo), idesc, !(fresh && ks == 0));
+}
 
-__global__ void __launch_bounds__(128, 1) tc_mix_fwd(MixParams p) {
+struct MixThread {
+  uint32_t lane_base; // TMEM lane offset of this warp's 32 rows
+  int colh;           // 0: re columns [0,96), 1: im columns [96,192)
+  int r;              // accumulator row of this thread
+};
+
+// this thread's 96 accumulator columns of a region -> registers
+__device__ __forceinline__ void ld_half(uint32_t region, const MixThread& t, uint32_t (&v)[3][32]) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k) tmem_ld32(region + t.lane_base + t.colh * BS + 32 * k, v[k]);
+  tmem_wait_ld();
+}
+// packed bf16 A operand of the next GEMM: K index = column, re half -> columns [0,48), im -> [48,96)
+__device__ __forceinline__ void st_half_packed(uint32_t region, const MixThread& t, const uint32_t (&pk)[3][16]) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k) tmem_st16(region + t.lane_base + t.colh * (BS / 2) + 16 * k, pk[k]);
+}
+__device__ __forceinline__ void store_row_half(__nv_bfloat16* dst, const uint32_t (&pk)[3][16]) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+#pragma unroll
+    for (int g = 0; g < 4; ++g)
+      *(uint4*)(dst + k * 32 + g * 8) = make_uint4(pk[k][4 * g], pk[k][4 * g + 1], pk[k][4 * g + 2], pk[k][4 * g + 3]);
+}
+// bf16 rows written as the MN-major B operand of the inverse H-DFT (K = row r)
+__device__ __forceinline__ void store_tile_half(uint8_t* tile, const MixThread& t, const uint32_t (&pk)[3][16]) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+#pragma unroll
+    for (int g = 0; g < 4; ++g)
+      *(uint4*)(tile + (t.colh * 12 + k * 4 + g) * kTileSbo + t.r * 16) =
+          make_uint4(pk[k][4 * g], pk[k][4 * g + 1], pk[k][4 * g + 2], pk[k][4 * g + 3]);
+}
+// rows of a (b,kw,j) tile [H][192] -> MN-major B operand (K = h, N = (ri, c)); 8 warps
+__device__ __forceinline__ void load_tile(uint32_t tile_saddr, const __nv_bfloat16* src, int H, int warp, int lane) {
+  const int hl = lane & 7, cl4 = lane >> 3;
+  const int nunits = ((H + 7) / 8) * 6;
+  for (int u = warp; u < nunits; u += kMixThreads / 32) {
+    const int h = (u / 6) * 8 + hl;
+    const int nc = (u % 6) * 4 + cl4;
+    if (h < H) cp_async16(tile_saddr + nc * kTileSbo + h * 16, src + (size_t)h * NT + nc * 8);
+  }
+}
+__device__ __forceinline__ void block_tmem_sync() {
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+}
+
+constexpr uint32_t kMixFwdSmem = kMixSmem + kTileBytes; // two tile buffers (prefetch of the next tile)
+
+__global__ void __launch_bounds__(kMixThreads, 1) tc_mix_fwd(MixParams p) {
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ __align__(8) uint64_t mbar;
   __shared__ uint32_t tmem_slot;
   uint8_t* sCh = smem;
   uint8_t* sSh = smem + kDftBytes;
   uint8_t* sW = smem + 2 * kDftBytes;
-  uint8_t* sTile = sW + 4 * kWBytes;
-  float* sBias = (float*)(sTile + kTileBytes); // b1 (re 96 | im 96), b2 (re 96 | im 96)
+  uint8_t* sTile0 = sW + 4 * kWBytes;
+  float* sBias = (float*)(sTile0 + kTileBytes); // b1 (re 96 | im 96), b2 (re 96 | im 96)
+  uint8_t* sTile1 = sTile0 + kTileBytes + 2 * NT * 4;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (uint32_t i = tid; i < kTileBytes / 16; i += 128) ((uint4*)sTile)[i] = make_uint4(0, 0, 0, 0);
-  for (uint32_t i = tid; i < 2 * kDftBytes / 16; i += 128) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
+  for (uint32_t i = tid; i < kTileBytes / 16; i += kMixThreads) {
+    ((uint4*)sTile0)[i] = make_uint4(0, 0, 0, 0);
+    ((uint4*)sTile1)[i] = make_uint4(0, 0, 0, 0);
+  }
+  for (uint32_t i = tid; i < 2 * kDftBytes / 16; i += kMixThreads)
+    cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
   if (tid == 0) {
     mbar_init(&mbar, 1);
     mbar_init_fence();
@@ -310,10 +376,13 @@ __global__ void __launch_bounds__(128, 1) tc_mix_fwd(MixParams p) {
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
-  const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+  MixThread th;
+  th.lane_base = (uint32_t)((warp & 3) * 32) << 16;
+  th.colh = warp >> 2;
+  th.r = (warp & 3) * 32 + lane;
   const uint32_t R0 = tmem, R1 = tmem + 256;
-  const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW), aTile = smem_u32(sTile);
-  const uint32_t tile_re = aTile, tile_im = aTile + (BS / 8) * kTileSbo;
+  const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW);
+  const uint32_t half = (BS / 8) * kTileSbo;
   const uint32_t id_dft = idesc_bf16(128, BS, kIdescBMn);
   const uint32_t id_mlp = idesc_bf16(128, BS);
 
@@ -322,65 +391,67 @@ __global__ void __launch_bounds__(128, 1) tc_mix_fwd(MixParams p) {
   const int t_begin = blockIdx.x * per, t_end = min(ntiles, t_begin + per);
   uint32_t phase = 0;
   int cur_j = -1;
-  const int r = tid; // this thread's accumulator row (mode row kh, or output row h)
+  const int r = th.r;
   const int kappa = (r <= p.H / 2) ? r : p.H - r;
   const bool row_kept = (r < p.H) && (kappa < p.Kh);
-  const int hl = lane & 7, cl4 = lane >> 3;
+  const float* bias1 = sBias + th.colh * BS;
+  const float* bias2 = sBias + NT + th.colh * BS;
+
+  auto tile_src = [&](int t) {
+    const int j = t / (p.B * p.Kw);
+    const int rem = t - j * (p.B * p.Kw);
+    return p.A1 + ((size_t)rem * p.nb + j) * p.H * NT;
+  };
+  if (t_begin < t_end) load_tile(smem_u32(sTile0), tile_src(t_begin), p.H, warp, lane);
+  cp_async_commit();
 
   for (int t = t_begin; t < t_end; ++t) {
     const int j = t / (p.B * p.Kw);
     const int rem = t - j * (p.B * p.Kw);
-    if (j != cur_j) {
+    uint8_t* sTile = ((t - t_begin) & 1) ? sTile1 : sTile0;
+    const uint32_t aTile = smem_u32(sTile);
+    const bool new_block = j != cur_j;
+    if (new_block) {
       cur_j = j;
       const uint8_t* wsrc = p.wprep + (size_t)j * 8 * kWBytes;
-      for (uint32_t i = tid; i < 4 * kWBytes / 16; i += 128) cp_async16(aW + i * 16, wsrc + (size_t)i * 16);
-      for (int i = tid; i < 2 * NT; i += 128) {
+      for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMixThreads) cp_async16(aW + i * 16, wsrc + (size_t)i * 16);
+      for (int i = tid; i < 2 * NT; i += kMixThreads) {
         const int which = i / NT, n = i % NT, ri = n / BS, o = n % BS;
         sBias[i] = (which == 0 ? p.b1 : p.b2)[((size_t)j * BS + o) * 2 + ri];
       }
     }
-    // tile (b, kw, j) of A1: H rows of 192 bf16 -> MN-major B operand (K = h, N = (ri, c))
-    const __nv_bfloat16* src = p.A1 + ((size_t)rem * p.nb + j) * p.H * NT;
-    {
-      const int nunits = ((p.H + 7) / 8) * 6;
-      for (int u = warp; u < nunits; u += 4) {
-        const int h = (u / 6) * 8 + hl;
-        const int nc = (u % 6) * 4 + cl4;
-        if (h < p.H) cp_async16(aTile + nc * kTileSbo + h * 16, src + (size_t)h * NT + nc * 8);
-      }
-    }
-    cp_async_wait_all();
+    // prefetch the next tile into the other buffer (its last reader, the previous inverse DFT, is complete)
+    if (t + 1 < t_end) load_tile(smem_u32(((t - t_begin) & 1) ? sTile0 : sTile1), tile_src(t + 1), p.H, warp, lane);
+    cp_async_commit();
+    if (new_block) cp_async_wait_group<0>();
+    else cp_async_wait_group<1>();
     fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
+    block_tmem_sync();
     // F2: Xr = Ch Ar + Sh Ai ; Xi = Ch Ai - Sh Ar      (forward kernel exp(-i theta))
     if (tid == 0) {
-      tc_fence_after();
-      issue_dft(R0, aCh, tile_re, id_dft, true);
-      issue_dft(R0, aSh, tile_im, id_dft, false);
-      issue_dft(R0 + BS, aCh, tile_im, id_dft, true);
-      issue_dft(R0 + BS, aSh, tile_re, id_dft | kIdescNegA, false);
+      issue_dft(R0, aCh, aTile, id_dft, true);
+      issue_dft(R0, aSh, aTile + half, id_dft, false);
+      issue_dft(R0 + BS, aCh, aTile + half, id_dft, true);
+      issue_dft(R0 + BS, aSh, aTile, id_dft | kIdescNegA, false);
       mma_commit(&mbar);
     }
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-    // fp32 spectrum -> bf16 A operand, in place
-#pragma unroll 1
-    for (int c0 = 0; c0 < NT; c0 += 32) {
-      uint32_t v[32], pk[16];
-      tmem_ld32(R0 + lane_base + c0, v);
-      tmem_wait_ld();
+    {
+      uint32_t v[3][32], pk[3][16];
+      ld_half(R0, th, v);
+      block_tmem_sync();
 #pragma unroll
-      for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
-      tmem_st16(R0 + lane_base + c0 / 2, pk);
+      for (int k = 0; k < 3; ++k)
+#pragma unroll
+        for (int q = 0; q < 16; ++q) pk[k][q] = pack_bf16(__uint_as_float(v[k][2 * q]), __uint_as_float(v[k][2 * q + 1]));
+      st_half_packed(R0, th, pk);
+      tmem_wait_st();
     }
-    tmem_wait_st();
-    tc_fence_before();
-    __syncthreads();
+    block_tmem_sync();
     // F3: P1 = Xh W1 + b1
     if (tid == 0) {
-      tc_fence_after();
       issue_mlp(R1, R0, aW + 0 * kWBytes, id_mlp, true);                         // Xr W1r
       issue_mlp(R1, R0 + BS / 2, aW + 1 * kWBytes, id_mlp | kIdescNegB, false);  // - Xi W1i
       issue_mlp(R1 + BS, R0, aW + 1 * kWBytes, id_mlp, true);                    // Xr W1i
@@ -390,26 +461,25 @@ __global__ void __launch_bounds__(128, 1) tc_mix_fwd(MixParams p) {
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-    // F4: bias + split ReLU -> bf16 A operand, in place
-#pragma unroll 1
-    for (int c0 = 0; c0 < NT; c0 += 32) {
-      uint32_t v[32], pk[16];
-      tmem_ld32(R1 + lane_base + c0, v);
-      tmem_wait_ld();
+    {
+      // F4: bias + split ReLU
+      uint32_t v[3][32], pk[3][16];
+      ld_half(R1, th, v);
+      block_tmem_sync();
 #pragma unroll
-      for (int q = 0; q < 16; ++q) {
-        const float a = fmaxf(__uint_as_float(v[2 * q]) + sBias[c0 + 2 * q], 0.f);
-        const float b = fmaxf(__uint_as_float(v[2 * q + 1]) + sBias[c0 + 2 * q + 1], 0.f);
-        pk[q] = pack_bf16(a, b);
-      }
-      tmem_st16(R1 + lane_base + c0 / 2, pk);
+      for (int k = 0; k < 3; ++k)
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+          const float a = fmaxf(__uint_as_float(v[k][2 * q]) + bias1[32 * k + 2 * q], 0.f);
+          const float b = fmaxf(__uint_as_float(v[k][2 * q + 1]) + bias1[32 * k + 2 * q + 1], 0.f);
+          pk[k][q] = pack_bf16(a, b);
+        }
+      st_half_packed(R1, th, pk);
+      tmem_wait_st();
     }
-    tmem_wait_st();
-    tc_fence_before();
-    __syncthreads();
+    block_tmem_sync();
     // F5: P2 = O1 W2 + b2
     if (tid == 0) {
-      tc_fence_after();
       issue_mlp(R0, R1, aW + 2 * kWBytes, id_mlp, true);
       issue_mlp(R0, R1 + BS / 2, aW + 3 * kWBytes, id_mlp | kIdescNegB, false);
       issue_mlp(R0 + BS, R1, aW + 3 * kWBytes, id_mlp, true);
@@ -419,62 +489,44 @@ __global__ void __launch_bounds__(128, 1) tc_mix_fwd(MixParams p) {
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-    // F6: bias + softshrink + truncation -> bf16 Z written as the MN-major B operand (K = row r)
-#pragma unroll 1
-    for (int c0 = 0; c0 < NT; c0 += 32) {
-      uint32_t v[32];
-      tmem_ld32(R0 + lane_base + c0, v);
-      tmem_wait_ld();
-      if (r < HP) {
+    {
+      // F6: bias + softshrink + truncation -> bf16 Z as the B operand of the inverse transform
+      uint32_t v[3][32], pk[3][16];
+      ld_half(R0, th, v);
 #pragma unroll
-        for (int g = 0; g < 4; ++g) {
-          uint32_t pk[4];
+      for (int k = 0; k < 3; ++k)
 #pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const int n = c0 + g * 8 + 2 * q;
-            float a = __uint_as_float(v[g * 8 + 2 * q]) + sBias[NT + n];
-            float b = __uint_as_float(v[g * 8 + 2 * q + 1]) + sBias[NT + n + 1];
-            float ma = fabsf(a) - p.lambda, mb = fabsf(b) - p.lambda;
-            a = (row_kept && ma > 0.f) ? copysignf(ma, a) : 0.f;
-            b = (row_kept && mb > 0.f) ? copysignf(mb, b) : 0.f;
-            pk[q] = pack_bf16(a, b);
-          }
-          *(uint4*)(sTile + ((c0 >> 3) + g) * kTileSbo + r * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        for (int q = 0; q < 16; ++q) {
+          float a = __uint_as_float(v[k][2 * q]) + bias2[32 * k + 2 * q];
+          float b = __uint_as_float(v[k][2 * q + 1]) + bias2[32 * k + 2 * q + 1];
+          const float ma = fabsf(a) - p.lambda, mb = fabsf(b) - p.lambda;
+          a = (row_kept && ma > 0.f) ? copysignf(ma, a) : 0.f;
+          b = (row_kept && mb > 0.f) ? copysignf(mb, b) : 0.f;
+          pk[k][q] = pack_bf16(a, b);
         }
-      }
+      if (r < HP) store_tile_half(sTile, th, pk);
     }
     fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
+    block_tmem_sync();
     // F7: Tr = Ch Zr - Sh Zi ; Ti = Ch Zi + Sh Zr      (inverse kernel exp(+i theta))
     if (tid == 0) {
-      tc_fence_after();
-      issue_dft(R1, aCh, tile_re, id_dft, true);
-      issue_dft(R1, aSh, tile_im, id_dft | kIdescNegA, false);
-      issue_dft(R1 + BS, aCh, tile_im, id_dft, true);
-      issue_dft(R1 + BS, aSh, tile_re, id_dft, false);
+      issue_dft(R1, aCh, aTile, id_dft, true);
+      issue_dft(R1, aSh, aTile + half, id_dft | kIdescNegA, false);
+      issue_dft(R1 + BS, aCh, aTile + half, id_dft, true);
+      issue_dft(R1 + BS, aSh, aTile, id_dft, false);
       mma_commit(&mbar);
     }
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-    __nv_bfloat16* dst = p.A2 + (((size_t)rem * p.nb + j) * p.H + r) * NT;
-#pragma unroll 1
-    for (int c0 = 0; c0 < NT; c0 += 32) {
-      uint32_t v[32];
-      tmem_ld32(R1 + lane_base + c0, v);
-      tmem_wait_ld();
-      if (r < p.H) {
+    {
+      uint32_t v[3][32], pk[3][16];
+      ld_half(R1, th, v);
 #pragma unroll
-        for (int g = 0; g < 4; ++g) {
-          uint4 o;
-          o.x = pack_bf16(__uint_as_float(v[g * 8 + 0]), __uint_as_float(v[g * 8 + 1]));
-          o.y = pack_bf16(__uint_as_float(v[g * 8 + 2]), __uint_as_float(v[g * 8 + 3]));
-          o.z = pack_bf16(__uint_as_float(v[g * 8 + 4]), __uint_as_float(v[g * 8 + 5]));
-          o.w = pack_bf16(__uint_as_float(v[g * 8 + 6]), __uint_as_float(v[g * 8 + 7]));
-          *(uint4*)(dst + c0 + g * 8) = o;
-        }
-      }
+      for (int k = 0; k < 3; ++k)
+#pragma unroll
+        for (int q = 0; q < 16; ++q) pk[k][q] = pack_bf16(__uint_as_float(v[k][2 * q]), __uint_as_float(v[k][2 * q + 1]));
+      if (r < p.H) store_row_half(p.A2 + (((size_t)rem * p.nb + j) * p.H + r) * NT + th.colh * BS, pk);
     }
   }
   tc_fence_before();
@@ -501,22 +553,9 @@ struct MixBwdParams {
   float lambda;
 };
 
-// D[:, dcol .. dcol+96) (+)= A_tmem(packed, K = 96 output features o) * W^H part: the forward
-// weight image (n=o, k=i, K-major) read as an MN-major B operand with (k=o, n=i)
-__device__ __forceinline__ void issue_mlp_t(uint32_t d, uint32_t a_tmem, uint32_t w_base, uint32_t idesc, bool fresh) {
-#pragma unroll
-  for (int ks = 0; ks < BS / 16; ++ks)
-    mma_ts(d, a_tmem + ks * 8, smem_desc(w_base + ks * 2 * kWSbo, kWSbo, kWLbo), idesc, !(fresh && ks == 0));
-}
-
-__device__ __forceinline__ void store_row_chunk(__nv_bfloat16* dst, const uint32_t (&pk)[16]) {
-#pragma unroll
-  for (int g = 0; g < 4; ++g) *(uint4*)(dst + g * 8) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
-}
-
 constexpr uint32_t kMixBwdSmem = kMixSmem + kTileBytes; // second tile buffer for the gradient spectrum
 
-__global__ void __launch_bounds__(128, 1) tc_mix_bwd(MixBwdParams p) {
+__global__ void __launch_bounds__(kMixThreads, 1) tc_mix_bwd(MixBwdParams p) {
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ __align__(8) uint64_t mbar;
   __shared__ uint32_t tmem_slot;
@@ -527,11 +566,12 @@ __global__ void __launch_bounds__(128, 1) tc_mix_bwd(MixBwdParams p) {
   float* sBias = (float*)(sTile + kTileBytes);
   uint8_t* sTileG = sTile + kTileBytes + 2 * NT * 4;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (uint32_t i = tid; i < kTileBytes / 16; i += 128) {
+  for (uint32_t i = tid; i < kTileBytes / 16; i += kMixThreads) {
     ((uint4*)sTile)[i] = make_uint4(0, 0, 0, 0);
     ((uint4*)sTileG)[i] = make_uint4(0, 0, 0, 0);
   }
-  for (uint32_t i = tid; i < 2 * kDftBytes / 16; i += 128) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
+  for (uint32_t i = tid; i < 2 * kDftBytes / 16; i += kMixThreads)
+    cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
   if (tid == 0) {
     mbar_init(&mbar, 1);
     mbar_init_fence();
@@ -541,7 +581,10 @@ __global__ void __launch_bounds__(128, 1) tc_mix_bwd(MixBwdParams p) {
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
-  const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+  MixThread th;
+  th.lane_base = (uint32_t)((warp & 3) * 32) << 16;
+  th.colh = warp >> 2;
+  th.r = (warp & 3) * 32 + lane;
   const uint32_t R0 = tmem, R1 = tmem + 256;
   const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW);
   const uint32_t aTile = smem_u32(sTile), aTileG = smem_u32(sTileG);
@@ -555,11 +598,12 @@ __global__ void __launch_bounds__(128, 1) tc_mix_bwd(MixBwdParams p) {
   const int t_begin = blockIdx.x * per, t_end = min(ntiles, t_begin + per);
   uint32_t phase = 0;
   int cur_j = -1;
-  const int r = tid;
+  const int r = th.r;
   const int kappa = (r <= p.H / 2) ? r : p.H - r;
   const bool row_valid = r < p.H;
   const bool row_kept = row_valid && (kappa < p.Kh);
-  const int hl = lane & 7, cl4 = lane >> 3;
+  const float* bias1 = sBias + th.colh * BS;
+  const float* bias2 = sBias + NT + th.colh * BS;
 
   for (int t = t_begin; t < t_end; ++t) {
     const int j = t / (p.B * p.Kw);
@@ -567,34 +611,21 @@ __global__ void __launch_bounds__(128, 1) tc_mix_bwd(MixBwdParams p) {
     if (j != cur_j) {
       cur_j = j;
       const uint8_t* wsrc = p.wprep + (size_t)j * 8 * kWBytes;
-      for (uint32_t i = tid; i < 4 * kWBytes / 16; i += 128) cp_async16(aW + i * 16, wsrc + (size_t)i * 16);
-      for (int i = tid; i < 2 * NT; i += 128) {
+      for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMixThreads) cp_async16(aW + i * 16, wsrc + (size_t)i * 16);
+      for (int i = tid; i < 2 * NT; i += kMixThreads) {
         const int which = i / NT, n = i % NT, ri = n / BS, o = n % BS;
         sBias[i] = (which == 0 ? p.b1 : p.b2)[((size_t)j * BS + o) * 2 + ri];
       }
     }
     const size_t tile_off = ((size_t)rem * p.nb + j) * p.H * NT;
-    {
-      const __nv_bfloat16* srcx = p.A1x + tile_off;
-      const __nv_bfloat16* srcg = p.A1g + tile_off;
-      const int nunits = ((p.H + 7) / 8) * 6;
-      for (int u = warp; u < nunits; u += 4) {
-        const int h = (u / 6) * 8 + hl;
-        const int nc = (u % 6) * 4 + cl4;
-        if (h < p.H) {
-          cp_async16(aTile + nc * kTileSbo + h * 16, srcx + (size_t)h * NT + nc * 8);
-          cp_async16(aTileG + nc * kTileSbo + h * 16, srcg + (size_t)h * NT + nc * 8);
-        }
-      }
-    }
-    const size_t row_off = tile_off + (size_t)r * NT;
+    load_tile(aTile, p.A1x + tile_off, p.H, warp, lane);
+    load_tile(aTileG, p.A1g + tile_off, p.H, warp, lane);
+    const size_t row_off = tile_off + (size_t)r * NT + th.colh * BS;
     cp_async_wait_all();
     fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
+    block_tmem_sync();
     // ---- Xh = Fh A1x -----------------------------------------------------------------------
     if (tid == 0) {
-      tc_fence_after();
       issue_dft(R0, aCh, aTile, id_dft, true);
       issue_dft(R0, aSh, aTile + half, id_dft, false);
       issue_dft(R0 + BS, aCh, aTile + half, id_dft, true);
@@ -604,22 +635,21 @@ __global__ void __launch_bounds__(128, 1) tc_mix_bwd(MixBwdParams p) {
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-#pragma unroll 1
-    for (int c0 = 0; c0 < NT; c0 += 32) {
-      uint32_t v[32], pk[16];
-      tmem_ld32(R0 + lane_base + c0, v);
-      tmem_wait_ld();
+    {
+      uint32_t v[3][32], pk[3][16];
+      ld_half(R0, th, v);
+      block_tmem_sync();
 #pragma unroll
-      for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
-      tmem_st16(R0 + lane_base + c0 / 2, pk);
-      if (row_valid) store_row_chunk(p.Xh + row_off + c0, pk);
+      for (int k = 0; k < 3; ++k)
+#pragma unroll
+        for (int q = 0; q < 16; ++q) pk[k][q] = pack_bf16(__uint_as_float(v[k][2 * q]), __uint_as_float(v[k][2 * q + 1]));
+      st_half_packed(R0, th, pk);
+      if (row_valid) store_row_half(p.Xh + row_off, pk);
+      tmem_wait_st();
     }
-    tmem_wait_st();
-    tc_fence_before();
-    __syncthreads();
+    block_tmem_sync();
     // ---- P1 = Xh W1 + b1 ; O1 = relu ; mask1 -------------------------------------------------
     if (tid == 0) {
-      tc_fence_after();
       issue_mlp(R1, R0, aW + 0 * kWBytes, id_mlp, true);
       issue_mlp(R1, R0 + BS / 2, aW + 1 * kWBytes, id_mlp | kIdescNegB, false);
       issue_mlp(R1 + BS, R0, aW + 1 * kWBytes, id_mlp, true);
@@ -629,32 +659,31 @@ __global__ void __launch_bounds__(128, 1) tc_mix_bwd(MixBwdParams p) {
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-    uint32_t m1[6], m2[6];
-#pragma unroll 1
-    for (int ch = 0; ch < 6; ++ch) {
-      const int c0 = ch * 32;
-      uint32_t v[32], pk[16];
-      tmem_ld32(R1 + lane_base + c0, v);
-      tmem_wait_ld();
-      uint32_t bits = 0;
+    uint32_t m1[3], m2[3];
+    {
+      uint32_t v[3][32], pk[3][16];
+      ld_half(R1, th, v);
+      block_tmem_sync();
 #pragma unroll
-      for (int q = 0; q < 16; ++q) {
-        const float a = __uint_as_float(v[2 * q]) + sBias[c0 + 2 * q];
-        const float b = __uint_as_float(v[2 * q + 1]) + sBias[c0 + 2 * q + 1];
-        bits |= (a > 0.f ? 1u : 0u) << (2 * q);
-        bits |= (b > 0.f ? 1u : 0u) << (2 * q + 1);
-        pk[q] = pack_bf16(fmaxf(a, 0.f), fmaxf(b, 0.f));
+      for (int k = 0; k < 3; ++k) {
+        uint32_t bits = 0;
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+          const float a = __uint_as_float(v[k][2 * q]) + bias1[32 * k + 2 * q];
+          const float b = __uint_as_float(v[k][2 * q + 1]) + bias1[32 * k + 2 * q + 1];
+          bits |= (a > 0.f ? 1u : 0u) << (2 * q);
+          bits |= (b > 0.f ? 1u : 0u) << (2 * q + 1);
+          pk[k][q] = pack_bf16(fmaxf(a, 0.f), fmaxf(b, 0.f));
+        }
+        m1[k] = bits;
       }
-      m1[ch] = bits;
-      tmem_st16(R1 + lane_base + c0 / 2, pk);
-      if (row_valid) store_row_chunk(p.O1 + row_off + c0, pk);
+      st_half_packed(R1, th, pk);
+      if (row_valid) store_row_half(p.O1 + row_off, pk);
+      tmem_wait_st();
     }
-    tmem_wait_st();
-    tc_fence_before();
-    __syncthreads();
+    block_tmem_sync();
     // ---- P2 = O1 W2 + b2 ; mask2 ----------------------------------------------------------------
     if (tid == 0) {
-      tc_fence_after();
       issue_mlp(R0, R1, aW + 2 * kWBytes, id_mlp, true);
       issue_mlp(R0, R1 + BS / 2, aW + 3 * kWBytes, id_mlp | kIdescNegB, false);
       issue_mlp(R0 + BS, R1, aW + 3 * kWBytes, id_mlp, true);
@@ -664,23 +693,21 @@ __global__ void __launch_bounds__(128, 1) tc_mix_bwd(MixBwdParams p) {
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-#pragma unroll 1
-    for (int ch = 0; ch < 6; ++ch) {
-      const int c0 = ch * 32;
-      uint32_t v[32];
-      tmem_ld32(R0 + lane_base + c0, v);
-      tmem_wait_ld();
-      uint32_t bits = 0;
+    {
+      uint32_t v[3][32];
+      ld_half(R0, th, v);
 #pragma unroll
-      for (int q = 0; q < 32; ++q)
-        bits |= (fabsf(__uint_as_float(v[q]) + sBias[NT + c0 + q]) > p.lambda ? 1u : 0u) << q;
-      m2[ch] = row_kept ? bits : 0u;
+      for (int k = 0; k < 3; ++k) {
+        uint32_t bits = 0;
+#pragma unroll
+        for (int q = 0; q < 32; ++q)
+          bits |= (fabsf(__uint_as_float(v[k][q]) + bias2[32 * k + q]) > p.lambda ? 1u : 0u) << q;
+        m2[k] = row_kept ? bits : 0u;
+      }
     }
-    tc_fence_before();
-    __syncthreads();
+    block_tmem_sync();
     // ---- G = Fh A1g ; G2 = G (.) mask2 -----------------------------------------------------------
     if (tid == 0) {
-      tc_fence_after();
       issue_dft(R1, aCh, aTileG, id_dft, true);
       issue_dft(R1, aSh, aTileG + half, id_dft, false);
       issue_dft(R1 + BS, aCh, aTileG + half, id_dft, true);
@@ -690,28 +717,27 @@ __global__ void __launch_bounds__(128, 1) tc_mix_bwd(MixBwdParams p) {
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-#pragma unroll 1
-    for (int ch = 0; ch < 6; ++ch) {
-      const int c0 = ch * 32;
-      uint32_t v[32], pk[16];
-      tmem_ld32(R1 + lane_base + c0, v);
-      tmem_wait_ld();
-      const uint32_t bits = m2[ch];
+    {
+      uint32_t v[3][32], pk[3][16];
+      ld_half(R1, th, v);
+      block_tmem_sync();
 #pragma unroll
-      for (int q = 0; q < 16; ++q) {
-        const float a = (bits >> (2 * q)) & 1u ? __uint_as_float(v[2 * q]) : 0.f;
-        const float b = (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[2 * q + 1]) : 0.f;
-        pk[q] = pack_bf16(a, b);
+      for (int k = 0; k < 3; ++k) {
+        const uint32_t bits = m2[k];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+          const float a = (bits >> (2 * q)) & 1u ? __uint_as_float(v[k][2 * q]) : 0.f;
+          const float b = (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[k][2 * q + 1]) : 0.f;
+          pk[k][q] = pack_bf16(a, b);
+        }
       }
-      tmem_st16(R1 + lane_base + c0 / 2, pk);
-      if (row_valid) store_row_chunk(p.G2 + row_off + c0, pk);
+      st_half_packed(R1, th, pk);
+      if (row_valid) store_row_half(p.G2 + row_off, pk);
+      tmem_wait_st();
     }
-    tmem_wait_st();
-    tc_fence_before();
-    __syncthreads();
+    block_tmem_sync();
     // ---- G1 = mask1 (.) (G2 W2^H):  re = G2r W2r^T + G2i W2i^T ; im = G2i W2r^T - G2r W2i^T ----
     if (tid == 0) {
-      tc_fence_after();
       issue_mlp_t(R0, R1, aW + 2 * kWBytes, id_mlp_t, true);
       issue_mlp_t(R0, R1 + BS / 2, aW + 3 * kWBytes, id_mlp_t, false);
       issue_mlp_t(R0 + BS, R1 + BS / 2, aW + 2 * kWBytes, id_mlp_t, true);
@@ -721,28 +747,27 @@ __global__ void __launch_bounds__(128, 1) tc_mix_bwd(MixBwdParams p) {
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-#pragma unroll 1
-    for (int ch = 0; ch < 6; ++ch) {
-      const int c0 = ch * 32;
-      uint32_t v[32], pk[16];
-      tmem_ld32(R0 + lane_base + c0, v);
-      tmem_wait_ld();
-      const uint32_t bits = m1[ch];
+    {
+      uint32_t v[3][32], pk[3][16];
+      ld_half(R0, th, v);
+      block_tmem_sync();
 #pragma unroll
-      for (int q = 0; q < 16; ++q) {
-        const float a = (bits >> (2 * q)) & 1u ? __uint_as_float(v[2 * q]) : 0.f;
-        const float b = (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[2 * q + 1]) : 0.f;
-        pk[q] = pack_bf16(a, b);
+      for (int k = 0; k < 3; ++k) {
+        const uint32_t bits = m1[k];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+          const float a = (bits >> (2 * q)) & 1u ? __uint_as_float(v[k][2 * q]) : 0.f;
+          const float b = (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[k][2 * q + 1]) : 0.f;
+          pk[k][q] = pack_bf16(a, b);
+        }
       }
-      tmem_st16(R0 + lane_base + c0 / 2, pk);
-      if (row_valid) store_row_chunk(p.G1 + row_off + c0, pk);
+      st_half_packed(R0, th, pk);
+      if (row_valid) store_row_half(p.G1 + row_off, pk);
+      tmem_wait_st();
     }
-    tmem_wait_st();
-    tc_fence_before();
-    __syncthreads();
+    block_tmem_sync();
     // ---- GX = G1 W1^H ----------------------------------------------------------------------------
     if (tid == 0) {
-      tc_fence_after();
       issue_mlp_t(R1, R0, aW + 0 * kWBytes, id_mlp_t, true);
       issue_mlp_t(R1, R0 + BS / 2, aW + 1 * kWBytes, id_mlp_t, false);
       issue_mlp_t(R1 + BS, R0 + BS / 2, aW + 0 * kWBytes, id_mlp_t, true);
@@ -752,78 +777,56 @@ __global__ void __launch_bounds__(128, 1) tc_mix_bwd(MixBwdParams p) {
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-#pragma unroll 1
-    for (int c0 = 0; c0 < NT; c0 += 32) {
-      uint32_t v[32];
-      tmem_ld32(R1 + lane_base + c0, v);
-      tmem_wait_ld();
-      if (r < HP) {
+    {
+      uint32_t v[3][32], pk[3][16];
+      ld_half(R1, th, v);
 #pragma unroll
-        for (int g = 0; g < 4; ++g) {
-          uint4 o;
-          o.x = row_valid ? pack_bf16(__uint_as_float(v[g * 8 + 0]), __uint_as_float(v[g * 8 + 1])) : 0u;
-          o.y = row_valid ? pack_bf16(__uint_as_float(v[g * 8 + 2]), __uint_as_float(v[g * 8 + 3])) : 0u;
-          o.z = row_valid ? pack_bf16(__uint_as_float(v[g * 8 + 4]), __uint_as_float(v[g * 8 + 5])) : 0u;
-          o.w = row_valid ? pack_bf16(__uint_as_float(v[g * 8 + 6]), __uint_as_float(v[g * 8 + 7])) : 0u;
-          *(uint4*)(sTile + ((c0 >> 3) + g) * kTileSbo + r * 16) = o;
-        }
-      }
+      for (int k = 0; k < 3; ++k)
+#pragma unroll
+        for (int q = 0; q < 16; ++q)
+          pk[k][q] = row_valid ? pack_bf16(__uint_as_float(v[k][2 * q]), __uint_as_float(v[k][2 * q + 1])) : 0u;
+      if (r < HP) store_tile_half(sTile, th, pk);
     }
     fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
+    block_tmem_sync();
     // ---- A2 = Fh^H GX (inverse kernel) ---------------------------------------------------------
     if (tid == 0) {
-      tc_fence_after();
       issue_dft(R0, aCh, aTile, id_dft, true);
       issue_dft(R0, aSh, aTile + half, id_dft | kIdescNegA, false);
       issue_dft(R0 + BS, aCh, aTile + half, id_dft, true);
       issue_dft(R0 + BS, aSh, aTile, id_dft, false);
       mma_commit(&mbar);
     }
-    // optional mask export while the tensor core works
+    // optional mask export (test aid) while the tensor core works: bytes (re, im) interleaved per channel
     if (p.mask1 != nullptr && row_valid) {
       const int b = rem / p.Kw, kw = rem - b * p.Kw;
-      const size_t base = ((((size_t)b * p.H + r) * p.Wh + kw) * (size_t)(p.nb * BS) + (size_t)j * BS) * 2;
-#pragma unroll 1
-      for (int o8 = 0; o8 < BS; o8 += 8) {
-        uint32_t w1[4], w2[4];
+      const size_t base = ((((size_t)b * p.H + r) * p.Wh + kw) * (size_t)(p.nb * BS) + (size_t)j * BS) * 2 + th.colh;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          uint32_t a = 0, b2v = 0;
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            const int o = o8 + 2 * q + e;
-            const int nre = o, nim = BS + o;
-            const uint32_t r1 = (m1[nre >> 5] >> (nre & 31)) & 1u, i1 = (m1[nim >> 5] >> (nim & 31)) & 1u;
-            const uint32_t r2 = (m2[nre >> 5] >> (nre & 31)) & 1u, i2 = (m2[nim >> 5] >> (nim & 31)) & 1u;
-            a |= (r1 | (i1 << 8)) << (16 * e);
-            b2v |= (r2 | (i2 << 8)) << (16 * e);
-          }
-          w1[q] = a;
-          w2[q] = b2v;
+      for (int k = 0; k < 3; ++k)
+#pragma unroll 4
+        for (int q = 0; q < 32; ++q) {
+          p.mask1[base + (size_t)(32 * k + q) * 2] = (uint8_t)((m1[k] >> q) & 1u);
+          p.mask2[base + (size_t)(32 * k + q) * 2] = (uint8_t)((m2[k] >> q) & 1u);
         }
-        *(uint4*)(p.mask1 + base + o8 * 2) = make_uint4(w1[0], w1[1], w1[2], w1[3]);
-        *(uint4*)(p.mask2 + base + o8 * 2) = make_uint4(w2[0], w2[1], w2[2], w2[3]);
-      }
     }
     mbar_wait(&mbar, phase);
     phase ^= 1;
     tc_fence_after();
-#pragma unroll 1
-    for (int c0 = 0; c0 < NT; c0 += 32) {
-      uint32_t v[32], pk[16];
-      tmem_ld32(R0 + lane_base + c0, v);
-      tmem_wait_ld();
+    {
+      uint32_t v[3][32], pk[3][16];
+      ld_half(R0, th, v);
 #pragma unroll
-      for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
-      if (row_valid) store_row_chunk(p.A2 + row_off + c0, pk);
+      for (int k = 0; k < 3; ++k)
+#pragma unroll
+        for (int q = 0; q < 16; ++q) pk[k][q] = pack_bf16(__uint_as_float(v[k][2 * q]), __uint_as_float(v[k][2 * q + 1]));
+      if (row_valid) store_row_half(p.A2 + row_off, pk);
     }
   }
   tc_fence_before();
   __syncthreads();
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
+
 
 // ---- B4 / B6: parameter gradients as a split-K tensor-core GEMM ------------------------------------
 // For block j:  R[(ri_a,i), (ri_g,o)] = sum_rows A[row,(ri_a,i)] * G[row,(ri_g,o)] with K = mode rows.
@@ -1064,7 +1067,7 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
   if (e == cudaSuccess) e = upload(gw1, &out->gw_noalpha);
   if (e == cudaSuccess) e = set_smem(tc_wdft_fwd, kRowSmem);
   if (e == cudaSuccess) e = set_smem(tc_wdft_inv, kRowSmem);
-  if (e == cudaSuccess) e = set_smem(tc_mix_fwd, kMixSmem);
+  if (e == cudaSuccess) e = set_smem(tc_mix_fwd, kMixFwdSmem);
   if (e == cudaSuccess) e = set_smem(tc_mix_bwd, kMixBwdSmem);
   if (e == cudaSuccess) e = set_smem(tc_wgrad, kWgSmem);
   int dev = 0, sms = 148;
@@ -1102,7 +1105,7 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   const int mix_tiles = g.nb * g.B * g.Kw;
   const int grid_mix = mix_tiles < tp.num_sms ? mix_tiles : tp.num_sms;
   prof_begin("tc_mix_fwd", st);
-  tc_mix_fwd<<<grid_mix, 128, kMixSmem, st>>>(mp);
+  tc_mix_fwd<<<grid_mix, kMixThreads, kMixFwdSmem, st>>>(mp);
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -1148,7 +1151,7 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
   const int mix_tiles = g.nb * g.B * g.Kw;
   const int grid_mix = mix_tiles < tp.num_sms ? mix_tiles : tp.num_sms;
-  TC_LAUNCH("tc_mix_bwd", tc_mix_bwd<<<grid_mix, 128, kMixBwdSmem, st>>>(mp));
+  TC_LAUNCH("tc_mix_bwd", tc_mix_bwd<<<grid_mix, kMixThreads, kMixBwdSmem, st>>>(mp));
   // B4 / B6: parameter gradients
   const int nred = nW + g.nb * BS;
   TC_LAUNCH("tc_wgrad", tc_wgrad<<<g.nb * w.S, 128, kWgSmem, st>>>(w.O1, w.G2, w.part, g.B * g.Kw, g.H, g.nb, w.S));

@@ -101,18 +101,46 @@ def oracle_cfg(oracle, d: binding.Desc, no_residual=False, naive=False):
                          no_residual=no_residual, naive_dft=naive)
 
 
+def preactivation_scales(cfg, dump, w1, b1, w2, b2):
+    """Per-(mode, block) magnitude scale of the two pre-activations (S3, P-bwd (ii)).
+
+    |P1[m,j,o] - b1| <= ||Xh[m,j,:]||_2 * ||W1[j,:,o]||_2 (Cauchy-Schwarz), so a kernel whose
+    operands carry a relative error eps perturbs P1 by at most ~eps * that product.  A DFT is
+    only NORMWISE accurate (||dXh|| <= eps ||x|| over the plane, not component by component),
+    so the row norm gets the plane's rms row norm added as an absolute floor; the same holds
+    for P2 with O1 and W2.  Returned arrays broadcast over the features of a block."""
+    nb, bs, hid = cfg.num_blocks, cfg.bs, cfg.hid
+    cw1 = w1[..., 0] + 1j * w1[..., 1]
+    cw2 = w2[..., 0] + 1j * w2[..., 1]
+    w1n = np.sqrt((np.abs(cw1) ** 2).sum(axis=1)).max(axis=1)          # [nb]
+    w2n = np.sqrt((np.abs(cw2) ** 2).sum(axis=1)).max(axis=1)
+    b1n = np.abs(b1[..., 0] + 1j * b1[..., 1]).max(axis=1)
+    b2n = np.abs(b2[..., 0] + 1j * b2[..., 1]).max(axis=1)
+    xh = dump["xhat"]
+    xn = np.sqrt((np.abs(xh.reshape(xh.shape[:3] + (nb, bs))) ** 2).sum(-1))       # [B,H,Wh,nb]
+    p1 = dump["p1"]
+    o1 = np.maximum(p1.real, 0) + 1j * np.maximum(p1.imag, 0)
+    on = np.sqrt((np.abs(o1.reshape(o1.shape[:3] + (nb, hid))) ** 2).sum(-1))
+    xfloor = np.sqrt((xn ** 2).mean(axis=(1, 2), keepdims=True))                    # [B,1,1,nb]
+    ofloor = np.sqrt((on ** 2).mean(axis=(1, 2), keepdims=True))
+    s1 = np.repeat((xn + xfloor) * w1n + b1n, hid, axis=-1)                         # [B,H,Wh,nb*hid]
+    s2 = np.repeat((on + ofloor) * w2n + b2n, bs, axis=-1)                          # [B,H,Wh,C]
+    return s1, s2
+
+
 def mask_flip_report(oracle_dump, gpu_mask1, gpu_mask2, lam, tau1, tau2):
     """Fraction of flipped masks and whether every flip is justified: the oracle's fp64
-    pre-activation lies within tau of the threshold (S3 P-bwd (ii))."""
+    pre-activation lies within tau of the threshold (S3 P-bwd (ii)).  tau1 / tau2 are
+    arrays broadcastable to the masks' shapes without the trailing (re, im) axis."""
     p1, p2 = oracle_dump["p1"], oracle_dump["p2"]
     z = oracle_dump["z"]
     o1 = np.stack([p1.real > 0, p1.imag > 0], -1)
     o2 = np.stack([z.real != 0, z.imag != 0], -1)
     f1 = o1 != gpu_mask1.astype(bool)
     f2 = o2 != gpu_mask2.astype(bool)
-    d1 = np.abs(np.stack([p1.real, p1.imag], -1))
-    d2 = np.abs(np.abs(np.stack([p2.real, p2.imag], -1)) - lam)
+    d1 = np.abs(np.stack([p1.real, p1.imag], -1)) / np.asarray(tau1)[..., None]
+    d2 = np.abs(np.abs(np.stack([p2.real, p2.imag], -1)) - lam) / np.asarray(tau2)[..., None]
     worst1 = float(d1[f1].max()) if f1.any() else 0.0
     worst2 = float(d2[f2].max()) if f2.any() else 0.0
     return dict(flip1=float(f1.mean()), flip2=float(f2.mean()), worst1=worst1, worst2=worst2,
-                justified=(worst1 <= tau1 and worst2 <= tau2))
+                justified=(worst1 <= 1.0 and worst2 <= 1.0))

@@ -4,7 +4,8 @@ Tolerances (BASELINE.json:north_star): relative L2 <= 1e-5 on the fp32 path, <= 
 bf16 path; gated on y AND on the spectral branch s (AFNO_FLAG_NO_RESIDUAL), because the
 branch is only ~5 % of y (SURVEY.md S0 finding 1).  Backward is compared mask-consistently
 (S3 P-bwd): the oracle is evaluated with the GPU's exported masks, every flipped
-mask must sit within tau of its threshold, and the raw comparison is printed, not gated.
+mask must sit within tau of its threshold (tau = tolerance x the Cauchy-Schwarz scale of that
+mode's pre-activation), and the raw comparison is printed, not gated.
 """
 import numpy as np
 import pytest
@@ -48,11 +49,11 @@ def _check_backward(oracle, desc, data, label=""):
     ref = oracle.backward(cfg, *args, mask1=g["mask1"], mask2=g["mask2"])
     raw = oracle.backward(cfg, *args, dump=True)
     tol = _tol(desc)
-    rms1 = float(np.sqrt(np.mean(np.abs(raw["dump"]["p1"]) ** 2) / 2))
-    rms2 = float(np.sqrt(np.mean(np.abs(raw["dump"]["p2"]) ** 2) / 2))
-    rep = parity.mask_flip_report(raw["dump"], g["mask1"], g["mask2"], cfg.lam, tol * rms1, tol * rms2)
-    print(f"[bwd {label}] mask flips: relu {rep['flip1']:.2e} shrink {rep['flip2']:.2e} "
-          f"worst distance {rep['worst1']:.2e}/{rep['worst2']:.2e} (tau {tol * rms1:.2e}/{tol * rms2:.2e})")
+    s1, s2 = parity.preactivation_scales(cfg, raw["dump"], data["w1"].astype(np.float64), data["b1"].astype(np.float64),
+                                         data["w2"].astype(np.float64), data["b2"].astype(np.float64))
+    rep = parity.mask_flip_report(raw["dump"], g["mask1"], g["mask2"], cfg.lam, tol * s1, tol * s2)
+    print(f"[bwd {label}] mask flips: relu {rep['flip1']:.2e} shrink {rep['flip2']:.2e}; worst flipped "
+          f"|pre-activation - threshold| / (tol * row scale) = {rep['worst1']:.2f} / {rep['worst2']:.2f} (must be <= 1)")
     for k in ("dx", "dw1", "db1", "dw2", "db2"):
         e, eraw = parity.rel_l2(g[k], ref[k]), parity.rel_l2(g[k], raw[k])
         print(f"[bwd {label}] {k}: rel_l2 mask-consistent {e:.3e}  raw {eraw:.3e}  max_abs {parity.max_abs(g[k], ref[k]):.3e}")

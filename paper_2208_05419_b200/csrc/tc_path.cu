@@ -49,24 +49,26 @@ constexpr uint32_t kRowBytes = WP * CGRP * 2;        // 49152
 constexpr uint32_t kMixSmem = 2 * kDftBytes + 4 * kWBytes + kTileBytes + 2 * NT * 4; // 161280
 constexpr int kTrPitch = 132;                        // fp32 words per row of the epilogue transpose buffer
 constexpr uint32_t kTrBytes = 32 * kTrPitch * 4;     // 16896
-constexpr uint32_t kRowSmem = kFwBytes + kRowBytes + kTrBytes;                       // 139776
+constexpr int kRowThreads = 256;
+constexpr uint32_t kRowSmem = kFwBytes + 2 * kRowBytes + 2 * kTrBytes;               // 205824
 
 // Epilogue transpose of the W-direction kernels: every thread holds 32 consecutive accumulator
 // columns of ITS channel (TMEM lane).  The chunk goes through shared memory so that thread
-// (q, c4) = (tid/32 + 4*pass, tid%32) then owns 4 consecutive channels of column q and global
-// accesses become 8-byte vectors, 256 contiguous bytes per warp.
+// (q, c4) = (t/32 + 4*pass, t%32) then owns 4 consecutive channels of column q and global
+// accesses become 8-byte vectors, 256 contiguous bytes per warp.  t = thread index inside a
+// 128-thread warp group; the two groups (column halves) use their own buffer and named barrier.
 template <typename F>
-__device__ __forceinline__ void transposed_chunk(float* sT, const uint32_t (&v)[32], int tid, F&& consume) {
+__device__ __forceinline__ void transposed_chunk(float* sT, const uint32_t (&v)[32], int t, int bar_id, F&& consume) {
 #pragma unroll
-  for (int q = 0; q < 32; ++q) sT[q * kTrPitch + tid] = __uint_as_float(v[q]);
-  __syncthreads();
-  const int c4 = (tid & 31) * 4;
+  for (int q = 0; q < 32; ++q) sT[q * kTrPitch + t] = __uint_as_float(v[q]);
+  asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
+  const int c4 = (t & 31) * 4;
 #pragma unroll
   for (int pass = 0; pass < 8; ++pass) {
-    const int q = pass * 4 + (tid >> 5);
+    const int q = pass * 4 + (t >> 5);
     consume(pass, q, c4, *(const float4*)&sT[q * kTrPitch + c4]);
   }
-  __syncthreads();
+  asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
 }
 
 // ---- weight preparation: fp32 [nb][96][96][2] -> bf16 K-major interleaved operands --------------
@@ -92,174 +94,168 @@ __global__ void k_tc_prep_weights(const float* __restrict__ w1, const float* __r
   base[7 * m + t] = __float2bfloat16_rn(b.y);
 }
 
-// ---- F1 / B2: W-direction forward DFT as a GEMM ------------------------------------------------
-// A1 layout: [b][kw < Kw][j][h][ri][96] bf16 (one (b,kw,j) tile = H x 192 contiguous).
-__global__ void __launch_bounds__(128, 1)
-tc_wdft_fwd(const __nv_bfloat16* __restrict__ x, __nv_bfloat16* __restrict__ A1,
-            const uint8_t* __restrict__ FwT, int B, int H, int W, int C, int Kw, int nb) {
+// ---- F1 / B2 and F8 + F9 / B8: the W-direction transforms as GEMMs -------------------------------
+// One tile = (b, h, 128 channels): D[c, n] = sum_k A[k, c] * Bconst[k, n], 12 UMMAs of 128x192x16.
+//   forward (INVERSE = false): k = w, A = x^T slab, n = (ri, kw); D -> A1[b][kw][j][h][ri][96]
+//   inverse (INVERSE = true) : k = (ri, kw), A gathered from A2, n = w; D + residual -> y
+// Software pipeline per CTA (persistent over tiles): the operand tile of iteration i+2 is copied
+// (cp.async) while the tensor core works on tile i+1 (second TMEM accumulator) and all 8 warps
+// run the epilogue of tile i.
+template <bool INVERSE>
+__global__ void __launch_bounds__(kRowThreads, 1)
+tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ res, __nv_bfloat16* __restrict__ out,
+        const uint8_t* __restrict__ Bconst, int B, int H, int W, int C, int Kw, int nb) {
   extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) uint64_t mbar;
+  __shared__ __align__(8) uint64_t mbar[2];
   __shared__ uint32_t tmem_slot;
   uint8_t* sF = smem;
-  uint8_t* sA = smem + kFwBytes;
-  float* sT = (float*)(smem + kFwBytes + kRowBytes);
+  uint8_t* sA0 = smem + kFwBytes;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (uint32_t i = tid; i < kRowBytes / 16; i += 128) ((uint4*)sA)[i] = make_uint4(0, 0, 0, 0);
-  for (uint32_t i = tid; i < kFwBytes / 16; i += 128) cp_async16(smem_u32(sF) + i * 16, FwT + (size_t)i * 16);
+  const int grp = warp >> 2, tg = tid & 127;          // column half / thread index inside the warp group
+  float* sT = (float*)(smem + kFwBytes + 2 * kRowBytes + grp * kTrBytes);
+  for (uint32_t i = tid; i < 2 * kRowBytes / 16; i += kRowThreads) ((uint4*)sA0)[i] = make_uint4(0, 0, 0, 0);
+  for (uint32_t i = tid; i < kFwBytes / 16; i += kRowThreads) cp_async16(smem_u32(sF) + i * 16, Bconst + (size_t)i * 16);
   if (tid == 0) {
-    mbar_init(&mbar, 1);
+    mbar_init(&mbar[0], 1);
+    mbar_init(&mbar[1], 1);
     mbar_init_fence();
   }
-  if (warp == 0) tmem_alloc<256>(&tmem_slot);
+  if (warp == 0) tmem_alloc<512>(&tmem_slot);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
-  const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
+  const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
   const int ncg = (C + CGRP - 1) / CGRP;
   const int ntiles = B * H * ncg;
-  uint32_t phase = 0;
+  const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
   const uint32_t idesc = idesc_bf16(128, NT, kIdescAMn);
   const int hl = lane & 7, cl4 = lane >> 3;
-  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+
+  auto load_tile = [&](int it) {
+    const int t = blockIdx.x + it * gridDim.x;
     const int cg = t % ncg, bh = t / ncg;
-    const __nv_bfloat16* xrow = x + (size_t)bh * W * C;
-    // x[b,h,:,cg*128 .. +128) becomes the MN-major A operand (K = w, M = channel)
-    const int nunits = ((W + 7) / 8) * 4;
-    for (int u = warp; u < nunits; u += 4) {
-      const int w = (u >> 2) * 8 + hl;
-      const int mc = (u & 3) * 4 + cl4;
-      const int c0 = cg * CGRP + mc * 8;
-      if (w < W && c0 < C) cp_async16(smem_u32(sA) + mc * kRowSbo + w * 16, xrow + (size_t)w * C + c0);
+    const uint32_t dst = smem_u32(sA0) + (it & 1) * kRowBytes;
+    if (!INVERSE) {
+      // x[b,h,:,cg*128 .. +128) -> MN-major A operand (K = w, M = channel)
+      const __nv_bfloat16* xrow = in + (size_t)bh * W * C;
+      const int nunits = ((W + 7) / 8) * 4;
+      for (int u = warp; u < nunits; u += kRowThreads / 32) {
+        const int w = (u >> 2) * 8 + hl;
+        const int mc = (u & 3) * 4 + cl4;
+        const int c0 = cg * CGRP + mc * 8;
+        if (w < W && c0 < C) cp_async16(dst + mc * kRowSbo + w * 16, xrow + (size_t)w * C + c0);
+      }
+    } else {
+      // A2[b][kw][j][h][ri][cl] gathered into the MN-major A operand (K = (ri,kw), M = channel)
+      const int b = bh / H, h = bh - b * H;
+      const int kwg = (Kw + 7) / 8;
+      const int nunits = 2 * kwg * 4;
+      for (int u = warp; u < nunits; u += kRowThreads / 32) {
+        const int rg = u >> 2;
+        const int ri = rg / kwg, kw = (rg - ri * kwg) * 8 + hl;
+        const int mc = (u & 3) * 4 + cl4;
+        const int c0 = cg * CGRP + mc * 8;
+        if (kw < Kw && c0 < C) {
+          const int j = c0 / BS, cl = c0 - j * BS;
+          cp_async16(dst + mc * kRowSbo + (ri * BS + kw) * 16,
+                     in + ((((size_t)b * Kw + kw) * nb + j) * H + h) * NT + ri * BS + cl);
+        }
+      }
     }
-    cp_async_wait_all();
+  };
+  auto issue_mma = [&](int it) {
+    const uint32_t a = smem_u32(sA0) + (it & 1) * kRowBytes;
+    const uint32_t d = tmem + (it & 1) * 256;
+#pragma unroll
+    for (int ks = 0; ks < WP / 16; ++ks)
+      mma_ss(d, smem_desc(a + ks * 2 * kRowLbo, kRowLbo, kRowSbo), smem_desc(smem_u32(sF) + ks * 2 * kFwLbo, kFwLbo, kFwSbo),
+             idesc, ks > 0);
+    mma_commit(&mbar[it & 1]);
+  };
+
+  if (nmine > 0) load_tile(0);
+  cp_async_commit();
+  if (nmine > 1) load_tile(1);
+  cp_async_commit();
+  cp_async_wait_group<1>();
+  fence_async_smem();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  if (tid == 0 && nmine > 0) issue_mma(0);
+
+  for (int it = 0; it < nmine; ++it) {
+    const int t = blockIdx.x + it * gridDim.x;
+    const int cg = t % ncg, bh = t / ncg;
+    // tile it+1 has landed -> start its MMA into the other accumulator (drained by the epilogue of it-1)
+    cp_async_wait_group<0>();
     fence_async_smem();
     tc_fence_before();
     __syncthreads();
-    if (tid == 0) {
-      tc_fence_after();
-      for (int ks = 0; ks < WP / 16; ++ks)
-        mma_ss(tmem, smem_desc(smem_u32(sA) + ks * 2 * kRowLbo, kRowLbo, kRowSbo),
-               smem_desc(smem_u32(sF) + ks * 2 * kFwLbo, kFwLbo, kFwSbo), idesc, ks > 0);
-      mma_commit(&mbar);
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
     tc_fence_after();
-    const int b = bh / H, h = bh - b * H;
+    if (tid == 0 && it + 1 < nmine) issue_mma(it + 1);
+    // accumulator of tile `it`
+    mbar_wait(&mbar[it & 1], (uint32_t)((it >> 1) & 1));
+    tc_fence_after();
+    // its operand buffer is free again: prefetch tile it+2 into it
+    if (it + 2 < nmine) load_tile(it + 2);
+    cp_async_commit();
+
+    const uint32_t acc = tmem + (it & 1) * 256 + lane_base + grp * BS;
+    if (!INVERSE) {
+      const int b = bh / H, h = bh - b * H;
 #pragma unroll 1
-    for (int c0 = 0; c0 < NT; c0 += 32) {
-      uint32_t v[32];
-      tmem_ld32(tmem + lane_base + c0, v);
-      tmem_wait_ld();
-      transposed_chunk(sT, v, tid, [&](int, int q, int c4, float4 f) {
-        const int n = c0 + q;
-        const int ri = n >= BS ? 1 : 0, kw = n - ri * BS;
-        const int c = cg * CGRP + c4;
-        if (kw < Kw && c < C) {
-          const int j = c / BS, cl = c - j * BS;
-          uint2 o = make_uint2(pack_bf16(f.x, f.y), pack_bf16(f.z, f.w));
-          *(uint2*)(A1 + ((((size_t)b * Kw + kw) * nb + j) * H + h) * NT + ri * BS + cl) = o;
+      for (int k = 0; k < 3; ++k) {
+        uint32_t v[32];
+        tmem_ld32(acc + 32 * k, v);
+        tmem_wait_ld();
+        transposed_chunk(sT, v, tg, 1 + grp, [&](int, int q, int c4, float4 f) {
+          const int kw = 32 * k + q;      // column n = grp*96 + kw  (ri = grp)
+          const int c = cg * CGRP + c4;
+          if (kw < Kw && c < C) {
+            const int j = c / BS, cl = c - j * BS;
+            uint2 o = make_uint2(pack_bf16(f.x, f.y), pack_bf16(f.z, f.w));
+            *(uint2*)(out + ((((size_t)b * Kw + kw) * nb + j) * H + h) * NT + grp * BS + cl) = o;
+          }
+        });
+      }
+    } else {
+      const int cbase = cg * CGRP + (tg & 31) * 4;
+      const size_t rowoff = (size_t)bh * W * C + cbase;
+#pragma unroll 1
+      for (int k = 0; k < 3; ++k) {
+        const int w0 = grp * BS + 32 * k;
+        uint32_t v[32];
+        tmem_ld32(acc + 32 * k, v);
+        // residual rows of this chunk (8 independent 8-byte loads in flight per thread)
+        uint2 rr[8];
+#pragma unroll
+        for (int pass = 0; pass < 8; ++pass) {
+          const int w = w0 + pass * 4 + (tg >> 5);
+          rr[pass] = make_uint2(0u, 0u);
+          if (res && w < W && cbase < C) rr[pass] = __ldg((const uint2*)(res + rowoff + (size_t)w * C));
         }
-      });
+        tmem_wait_ld();
+        transposed_chunk(sT, v, tg, 1 + grp, [&](int pass, int q, int c4, float4 f) {
+          const int w = w0 + q;
+          if (w < W && cbase < C) {
+            const uint2 r2 = rr[pass];
+            const float2 ra = __bfloat1622float2(*(const __nv_bfloat162*)&r2.x);
+            const float2 rb = __bfloat1622float2(*(const __nv_bfloat162*)&r2.y);
+            uint2 o = make_uint2(pack_bf16(f.x + ra.x, f.y + ra.y), pack_bf16(f.z + rb.x, f.w + rb.y));
+            *(uint2*)(out + rowoff + (size_t)w * C) = o;
+          }
+        });
+      }
     }
   }
+  cp_async_wait_all();
   tc_fence_before();
   __syncthreads();
-  if (warp == 0) tmem_dealloc<256>(tmem);
+  if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
-// ---- F8 + F9 / B8: W-direction inverse DFT as a GEMM, residual add, store -----------------------
-__global__ void __launch_bounds__(128, 1)
-tc_wdft_inv(const __nv_bfloat16* __restrict__ A2, const __nv_bfloat16* __restrict__ res,
-            __nv_bfloat16* __restrict__ y, const uint8_t* __restrict__ GwT, int B, int H, int W, int C,
-            int Kw, int nb) {
-  extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) uint64_t mbar;
-  __shared__ uint32_t tmem_slot;
-  uint8_t* sG = smem;
-  uint8_t* sA = smem + kFwBytes;
-  float* sT = (float*)(smem + kFwBytes + kRowBytes);
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (uint32_t i = tid; i < kRowBytes / 16; i += 128) ((uint4*)sA)[i] = make_uint4(0, 0, 0, 0);
-  for (uint32_t i = tid; i < kFwBytes / 16; i += 128) cp_async16(smem_u32(sG) + i * 16, GwT + (size_t)i * 16);
-  if (tid == 0) {
-    mbar_init(&mbar, 1);
-    mbar_init_fence();
-  }
-  if (warp == 0) tmem_alloc<256>(&tmem_slot);
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = tmem_slot;
-  const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
-  const int ncg = (C + CGRP - 1) / CGRP;
-  const int ntiles = B * H * ncg;
-  uint32_t phase = 0;
-  const uint32_t idesc = idesc_bf16(128, NT, kIdescAMn);
-  const int hl = lane & 7, cl4 = lane >> 3;
-  for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-    const int cg = t % ncg, bh = t / ncg;
-    const int b = bh / H, h = bh - b * H;
-    // A2[b][kw][j][h][ri][cl] gathered into the MN-major A operand (K = (ri,kw), M = channel)
-    const int kwg = (Kw + 7) / 8;
-    const int nunits = 2 * kwg * 4;
-    for (int u = warp; u < nunits; u += 4) {
-      const int rg = u >> 2;                 // (ri, kw group)
-      const int ri = rg / kwg, kw = (rg - ri * kwg) * 8 + hl;
-      const int mc = (u & 3) * 4 + cl4;
-      const int c0 = cg * CGRP + mc * 8;
-      if (kw < Kw && c0 < C) {
-        const int j = c0 / BS, cl = c0 - j * BS;
-        const __nv_bfloat16* src = A2 + ((((size_t)b * Kw + kw) * nb + j) * H + h) * NT + ri * BS + cl;
-        cp_async16(smem_u32(sA) + mc * kRowSbo + (ri * BS + kw) * 16, src);
-      }
-    }
-    cp_async_wait_all();
-    fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
-    if (tid == 0) {
-      tc_fence_after();
-      for (int ks = 0; ks < NT / 16; ++ks)
-        mma_ss(tmem, smem_desc(smem_u32(sA) + ks * 2 * kRowLbo, kRowLbo, kRowSbo),
-               smem_desc(smem_u32(sG) + ks * 2 * kFwLbo, kFwLbo, kFwSbo), idesc, ks > 0);
-      mma_commit(&mbar);
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
-    tc_fence_after();
-    const int cbase = cg * CGRP + (tid & 31) * 4;
-    const size_t rowoff = (size_t)bh * W * C + cbase;
-#pragma unroll 1
-    for (int c0 = 0; c0 < WP; c0 += 32) {
-      uint32_t v[32];
-      tmem_ld32(tmem + lane_base + c0, v);
-      tmem_wait_ld();
-      // residual rows of this chunk first (8 independent 8-byte loads in flight per thread)
-      uint2 rr[8];
-#pragma unroll
-      for (int pass = 0; pass < 8; ++pass) {
-        const int w = c0 + pass * 4 + (tid >> 5);
-        rr[pass] = make_uint2(0u, 0u);
-        if (res && w < W && cbase < C) rr[pass] = __ldg((const uint2*)(res + rowoff + (size_t)w * C));
-      }
-      transposed_chunk(sT, v, tid, [&](int pass, int q, int c4, float4 f) {
-        const int w = c0 + q;
-        if (w < W && cbase < C) {
-          const uint2 r2 = rr[pass];
-          const float2 ra = __bfloat1622float2(*(const __nv_bfloat162*)&r2.x);
-          const float2 rb = __bfloat1622float2(*(const __nv_bfloat162*)&r2.y);
-          uint2 o = make_uint2(pack_bf16(f.x + ra.x, f.y + ra.y), pack_bf16(f.z + rb.x, f.w + rb.y));
-          *(uint2*)(y + rowoff + (size_t)w * C) = o;
-        }
-      });
-    }
-  }
-  tc_fence_before();
-  __syncthreads();
-  if (warp == 0) tmem_dealloc<256>(tmem);
-}
 
 // ---- F2-F7: per (b, kw, block) chain  H-DFT -> layer 1 -> layer 2 -> inverse H-DFT ---------------
 // 256 threads: warp w owns TMEM lanes 32*(w&3).. (accumulator rows) and the column half w>>2
@@ -1065,8 +1061,8 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
   if (e == cudaSuccess) e = upload(fwa, &out->fw_alpha);
   if (e == cudaSuccess) e = upload(gw, &out->gw);
   if (e == cudaSuccess) e = upload(gw1, &out->gw_noalpha);
-  if (e == cudaSuccess) e = set_smem(tc_wdft_fwd, kRowSmem);
-  if (e == cudaSuccess) e = set_smem(tc_wdft_inv, kRowSmem);
+  if (e == cudaSuccess) e = set_smem(tc_wdft<false>, kRowSmem);
+  if (e == cudaSuccess) e = set_smem(tc_wdft<true>, kRowSmem);
   if (e == cudaSuccess) e = set_smem(tc_mix_fwd, kMixFwdSmem);
   if (e == cudaSuccess) e = set_smem(tc_mix_bwd, kMixBwdSmem);
   if (e == cudaSuccess) e = set_smem(tc_wgrad, kWgSmem);
@@ -1097,7 +1093,8 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   const int row_tiles = g.B * g.H * ncg;
   const int grid_row = row_tiles < tp.num_sms ? row_tiles : tp.num_sms;
   prof_begin("tc_wdft_fwd", st);
-  tc_wdft_fwd<<<grid_row, 128, kRowSmem, st>>>((const __nv_bfloat16*)x, w.A1, tp.fw, g.B, g.H, g.W, g.C, g.Kw, g.nb);
+  tc_wdft<false><<<grid_row, kRowThreads, kRowSmem, st>>>((const __nv_bfloat16*)x, nullptr, w.A1, tp.fw, g.B, g.H, g.W,
+                                                          g.C, g.Kw, g.nb);
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -1110,8 +1107,8 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   prof_begin("tc_wdft_inv", st);
-  tc_wdft_inv<<<grid_row, 128, kRowSmem, st>>>(w.A2, g.no_residual ? nullptr : (const __nv_bfloat16*)x,
-                                              (__nv_bfloat16*)y, tp.gw, g.B, g.H, g.W, g.C, g.Kw, g.nb);
+  tc_wdft<true><<<grid_row, kRowThreads, kRowSmem, st>>>(w.A2, g.no_residual ? nullptr : (const __nv_bfloat16*)x,
+                                                         (__nv_bfloat16*)y, tp.gw, g.B, g.H, g.W, g.C, g.Kw, g.nb);
   prof_end(st);
   count_launch();
   return cudaGetLastError();
@@ -1138,10 +1135,10 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   const int row_tiles = g.B * g.H * ncg;
   const int grid_row = row_tiles < tp.num_sms ? row_tiles : tp.num_sms;
   // B1 (first half) and B2: W-direction spectra of x and of dy (alpha-weighted)
-  TC_LAUNCH("tc_wdft_fwd", tc_wdft_fwd<<<grid_row, 128, kRowSmem, st>>>((const __nv_bfloat16*)x, w.A1, tp.fw, g.B,
-                                                                       g.H, g.W, g.C, g.Kw, g.nb));
-  TC_LAUNCH("tc_wdft_fwd", tc_wdft_fwd<<<grid_row, 128, kRowSmem, st>>>((const __nv_bfloat16*)dy, w.A1g, tp.fw_alpha,
-                                                                       g.B, g.H, g.W, g.C, g.Kw, g.nb));
+  TC_LAUNCH("tc_wdft_fwd", tc_wdft<false><<<grid_row, kRowThreads, kRowSmem, st>>>((const __nv_bfloat16*)x, nullptr, w.A1,
+                                                                                  tp.fw, g.B, g.H, g.W, g.C, g.Kw, g.nb));
+  TC_LAUNCH("tc_wdft_fwd", tc_wdft<false><<<grid_row, kRowThreads, kRowSmem, st>>>((const __nv_bfloat16*)dy, nullptr, w.A1g,
+                                                                                  tp.fw_alpha, g.B, g.H, g.W, g.C, g.Kw, g.nb));
   MixBwdParams mp{};
   mp.A1x = w.A1; mp.A1g = w.A1g; mp.A2 = w.A2;
   mp.Xh = w.Xh; mp.O1 = w.O1; mp.G2 = w.G2; mp.G1 = w.G1;
@@ -1161,7 +1158,7 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce<<<(nred + 255) / 256, 256, 0, st>>>(
                                      w.part, (float2*)dw1, (float2*)db1, g.nb, w.S, g.accum ? 1 : 0));
   // B8: dx = dy + irfft2(GX / alpha)
-  TC_LAUNCH("tc_wdft_inv", tc_wdft_inv<<<grid_row, 128, kRowSmem, st>>>(
+  TC_LAUNCH("tc_wdft_inv", tc_wdft<true><<<grid_row, kRowThreads, kRowSmem, st>>>(
                                w.A2, g.no_residual ? nullptr : (const __nv_bfloat16*)dy, (__nv_bfloat16*)dx,
                                tp.gw_noalpha, g.B, g.H, g.W, g.C, g.Kw, g.nb));
 #undef TC_LAUNCH

@@ -49,49 +49,37 @@ constexpr uint32_t kRowBytes = WP * CGRP * 2;        // 49152
 constexpr uint32_t kMixSmem = 2 * kDftBytes + 4 * kWBytes + kTileBytes + 2 * NT * 4; // 161280
 constexpr int kTrPitch = 132;                        // fp32 words per row of the epilogue transpose buffer
 constexpr uint32_t kTrBytes = 32 * kTrPitch * 4;     // 16896
-constexpr int kRowThreads = 256;
+constexpr int kRowEpiThreads = 256;                 // 8 epilogue warps
+constexpr int kRowThreads = kRowEpiThreads + 64;     // + 2 producer / MMA warps
 constexpr uint32_t kRowSmem = kFwBytes + 2 * kRowBytes + 2 * kTrBytes;               // 205824
 
-// Epilogue transpose of the W-direction kernels: every thread holds 32 consecutive accumulator
-// columns of ITS channel (TMEM lane).  The chunk goes through shared memory so that thread
-// (q, c4) = (t/32 + 4*pass, t%32) then owns 4 consecutive channels of column q and global
-// accesses become 8-byte vectors, 256 contiguous bytes per warp.  t = thread index inside a
-// 128-thread warp group; the two groups (column halves) use their own buffer and named barrier.
-template <typename F>
-__device__ __forceinline__ void transposed_chunk(float* sT, const uint32_t (&v)[32], int t, int bar_id, F&& consume) {
-#pragma unroll
-  for (int q = 0; q < 32; ++q) sT[q * kTrPitch + t] = __uint_as_float(v[q]);
-  asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
-  const int c4 = (t & 31) * 4;
-#pragma unroll
-  for (int pass = 0; pass < 8; ++pass) {
-    const int q = pass * 4 + (t >> 5);
-    consume(pass, q, c4, *(const float4*)&sT[q * kTrPitch + c4]);
-  }
-  asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
-}
-
 // ---- weight preparation: fp32 [nb][96][96][2] -> bf16 K-major interleaved operands --------------
-// per block, 8 matrices of kWBytes: fwd {W1r, W1i, W2r, W2i} with element (n=o, k=i) = W[i][o];
-// bwd {W1r, W1i, W2r, W2i} with element (n=i, k=o) = W[i][o].
-__global__ void k_tc_prep_weights(const float* __restrict__ w1, const float* __restrict__ w2,
-                                  __nv_bfloat16* __restrict__ out, int nb) {
+// per block 4 matrices of kWBytes {W1r, W1i, W2r, W2i} with element (n=o, k=i) = W[i][o] (the
+// backward pass reads the same images as MN-major operands), and the biases regrouped as
+// [block][layer][re 96 | im 96] fp32.
+__global__ void k_tc_prep_weights(const float* __restrict__ w1, const float* __restrict__ b1,
+                                  const float* __restrict__ w2, const float* __restrict__ b2,
+                                  __nv_bfloat16* __restrict__ out, float* __restrict__ bout, int nb) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx < nb * BS) {
+    const int o = idx % BS, j = idx / BS;
+    const float2 a = ((const float2*)b1)[idx], b = ((const float2*)b2)[idx];
+    float* bb = bout + (size_t)j * 2 * NT;
+    bb[o] = a.x;
+    bb[BS + o] = a.y;
+    bb[NT + o] = b.x;
+    bb[NT + BS + o] = b.y;
+  }
   if (idx >= nb * BS * BS) return;
   const int o = idx % BS, i = (idx / BS) % BS, j = idx / (BS * BS);
   const float2 a = ((const float2*)w1)[idx], b = ((const float2*)w2)[idx];
-  __nv_bfloat16* base = out + (size_t)j * 8 * (kWBytes / 2);
+  __nv_bfloat16* base = out + (size_t)j * 4 * (kWBytes / 2);
   const uint32_t f = ((i / 8) * kWLbo + (o / 8) * kWSbo + (o % 8) * 16 + (i % 8) * 2) / 2; // n=o, k=i
-  const uint32_t t = ((o / 8) * kWLbo + (i / 8) * kWSbo + (i % 8) * 16 + (o % 8) * 2) / 2; // n=i, k=o
   const uint32_t m = kWBytes / 2;
   base[0 * m + f] = __float2bfloat16_rn(a.x);
   base[1 * m + f] = __float2bfloat16_rn(a.y);
   base[2 * m + f] = __float2bfloat16_rn(b.x);
   base[3 * m + f] = __float2bfloat16_rn(b.y);
-  base[4 * m + t] = __float2bfloat16_rn(a.x);
-  base[5 * m + t] = __float2bfloat16_rn(a.y);
-  base[6 * m + t] = __float2bfloat16_rn(b.x);
-  base[7 * m + t] = __float2bfloat16_rn(b.y);
 }
 
 // ---- F1 / B2 and F8 + F9 / B8: the W-direction transforms as GEMMs -------------------------------
@@ -106,723 +94,632 @@ __global__ void __launch_bounds__(kRowThreads, 1)
 tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ res, __nv_bfloat16* __restrict__ out,
         const uint8_t* __restrict__ Bconst, int B, int H, int W, int C, int Kw, int nb) {
   extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) uint64_t mbar[2];
+  __shared__ __align__(8) uint64_t full[2], empty[2];
   __shared__ uint32_t tmem_slot;
   uint8_t* sF = smem;
   uint8_t* sA0 = smem + kFwBytes;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int grp = warp >> 2, tg = tid & 127;          // column half / thread index inside the warp group
-  float* sT = (float*)(smem + kFwBytes + 2 * kRowBytes + grp * kTrBytes);
   for (uint32_t i = tid; i < 2 * kRowBytes / 16; i += kRowThreads) ((uint4*)sA0)[i] = make_uint4(0, 0, 0, 0);
   for (uint32_t i = tid; i < kFwBytes / 16; i += kRowThreads) cp_async16(smem_u32(sF) + i * 16, Bconst + (size_t)i * 16);
   if (tid == 0) {
-    mbar_init(&mbar[0], 1);
-    mbar_init(&mbar[1], 1);
+    mbar_init(&full[0], 1);
+    mbar_init(&full[1], 1);
+    mbar_init(&empty[0], kRowEpiThreads);
+    mbar_init(&empty[1], kRowEpiThreads);
     mbar_init_fence();
   }
   if (warp == 0) tmem_alloc<512>(&tmem_slot);
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = tmem_slot;
-  const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
-  const int ncg = (C + CGRP - 1) / CGRP;
-  const int ntiles = B * H * ncg;
-  const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
-  const uint32_t idesc = idesc_bf16(128, NT, kIdescAMn);
-  const int hl = lane & 7, cl4 = lane >> 3;
-
-  auto load_tile = [&](int it) {
-    const int t = blockIdx.x + it * gridDim.x;
-    const int cg = t % ncg, bh = t / ncg;
-    const uint32_t dst = smem_u32(sA0) + (it & 1) * kRowBytes;
-    if (!INVERSE) {
-      // x[b,h,:,cg*128 .. +128) -> MN-major A operand (K = w, M = channel)
-      const __nv_bfloat16* xrow = in + (size_t)bh * W * C;
-      const int nunits = ((W + 7) / 8) * 4;
-      for (int u = warp; u < nunits; u += kRowThreads / 32) {
-        const int w = (u >> 2) * 8 + hl;
-        const int mc = (u & 3) * 4 + cl4;
-        const int c0 = cg * CGRP + mc * 8;
-        if (w < W && c0 < C) cp_async16(dst + mc * kRowSbo + w * 16, xrow + (size_t)w * C + c0);
-      }
-    } else {
-      // A2[b][kw][j][h][ri][cl] gathered into the MN-major A operand (K = (ri,kw), M = channel)
-      const int b = bh / H, h = bh - b * H;
-      const int kwg = (Kw + 7) / 8;
-      const int nunits = 2 * kwg * 4;
-      for (int u = warp; u < nunits; u += kRowThreads / 32) {
-        const int rg = u >> 2;
-        const int ri = rg / kwg, kw = (rg - ri * kwg) * 8 + hl;
-        const int mc = (u & 3) * 4 + cl4;
-        const int c0 = cg * CGRP + mc * 8;
-        if (kw < Kw && c0 < C) {
-          const int j = c0 / BS, cl = c0 - j * BS;
-          cp_async16(dst + mc * kRowSbo + (ri * BS + kw) * 16,
-                     in + ((((size_t)b * Kw + kw) * nb + j) * H + h) * NT + ri * BS + cl);
-        }
-      }
-    }
-  };
-  auto issue_mma = [&](int it) {
-    const uint32_t a = smem_u32(sA0) + (it & 1) * kRowBytes;
-    const uint32_t d = tmem + (it & 1) * 256;
-#pragma unroll
-    for (int ks = 0; ks < WP / 16; ++ks)
-      mma_ss(d, smem_desc(a + ks * 2 * kRowLbo, kRowLbo, kRowSbo), smem_desc(smem_u32(sF) + ks * 2 * kFwLbo, kFwLbo, kFwSbo),
-             idesc, ks > 0);
-    mma_commit(&mbar[it & 1]);
-  };
-
-  if (nmine > 0) load_tile(0);
-  cp_async_commit();
-  if (nmine > 1) load_tile(1);
-  cp_async_commit();
-  cp_async_wait_group<1>();
+  cp_async_wait_all();
   fence_async_smem();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  if (tid == 0 && nmine > 0) issue_mma(0);
+  const uint32_t tmem = tmem_slot;
+  const int ncg = (C + CGRP - 1) / CGRP;
+  const int ntiles = B * H * ncg;
+  const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
-  for (int it = 0; it < nmine; ++it) {
-    const int t = blockIdx.x + it * gridDim.x;
-    const int cg = t % ncg, bh = t / ncg;
-    // tile it+1 has landed -> start its MMA into the other accumulator (drained by the epilogue of it-1)
-    cp_async_wait_group<0>();
-    fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    if (tid == 0 && it + 1 < nmine) issue_mma(it + 1);
-    // accumulator of tile `it`
-    mbar_wait(&mbar[it & 1], (uint32_t)((it >> 1) & 1));
-    tc_fence_after();
-    // its operand buffer is free again: prefetch tile it+2 into it
-    if (it + 2 < nmine) load_tile(it + 2);
-    cp_async_commit();
-
-    const uint32_t acc = tmem + (it & 1) * 256 + lane_base + grp * BS;
-    if (!INVERSE) {
-      const int b = bh / H, h = bh - b * H;
-#pragma unroll 1
-      for (int k = 0; k < 3; ++k) {
-        uint32_t v[32];
-        tmem_ld32(acc + 32 * k, v);
-        tmem_wait_ld();
-        transposed_chunk(sT, v, tg, 1 + grp, [&](int, int q, int c4, float4 f) {
-          const int kw = 32 * k + q;      // column n = grp*96 + kw  (ri = grp)
-          const int c = cg * CGRP + c4;
-          if (kw < Kw && c < C) {
-            const int j = c / BS, cl = c - j * BS;
-            uint2 o = make_uint2(pack_bf16(f.x, f.y), pack_bf16(f.z, f.w));
-            *(uint2*)(out + ((((size_t)b * Kw + kw) * nb + j) * H + h) * NT + grp * BS + cl) = o;
-          }
-        });
-      }
-    } else {
-      const int cbase = cg * CGRP + (tg & 31) * 4;
-      const size_t rowoff = (size_t)bh * W * C + cbase;
-#pragma unroll 1
-      for (int k = 0; k < 3; ++k) {
-        const int w0 = grp * BS + 32 * k;
-        uint32_t v[32];
-        tmem_ld32(acc + 32 * k, v);
-        // residual rows of this chunk (8 independent 8-byte loads in flight per thread)
-        uint2 rr[8];
-#pragma unroll
-        for (int pass = 0; pass < 8; ++pass) {
-          const int w = w0 + pass * 4 + (tg >> 5);
-          rr[pass] = make_uint2(0u, 0u);
-          if (res && w < W && cbase < C) rr[pass] = __ldg((const uint2*)(res + rowoff + (size_t)w * C));
+  if (warp >= kRowEpiThreads / 32) {
+    // ===== producer warp p: tiles it = p, p+2, ... -> operand buffer p, accumulator p ================
+    const int p = warp - kRowEpiThreads / 32;
+    const uint32_t dst = smem_u32(sA0) + p * kRowBytes;
+    const uint32_t idesc = idesc_bf16(128, NT, kIdescAMn);
+    const int hl = lane & 7, cl4 = lane >> 3;
+    for (int it = p; it < nmine; it += 2) {
+      const int use = it >> 1;
+      // the previous MMA on this buffer has completed (its commit also frees the operand tile)
+      if (use > 0) mbar_wait(&full[p], (uint32_t)((use - 1) & 1));
+      const int t = blockIdx.x + it * gridDim.x;
+      const int cg = t % ncg, bh = t / ncg;
+      if (!INVERSE) {
+        // x[b,h,:,cg*128 .. +128) -> MN-major A operand (K = w, M = channel)
+        const __nv_bfloat16* xrow = in + (size_t)bh * W * C + cg * CGRP;
+        const int nunits = ((W + 7) / 8) * 4;
+        for (int u = 0; u < nunits; ++u) {
+          const int w = (u >> 2) * 8 + hl;
+          const int mc = (u & 3) * 4 + cl4;
+          if (w < W && cg * CGRP + mc * 8 < C) cp_async16(dst + mc * kRowSbo + w * 16, xrow + (size_t)w * C + mc * 8);
         }
-        tmem_wait_ld();
-        transposed_chunk(sT, v, tg, 1 + grp, [&](int pass, int q, int c4, float4 f) {
-          const int w = w0 + q;
-          if (w < W && cbase < C) {
-            const uint2 r2 = rr[pass];
-            const float2 ra = __bfloat1622float2(*(const __nv_bfloat162*)&r2.x);
-            const float2 rb = __bfloat1622float2(*(const __nv_bfloat162*)&r2.y);
-            uint2 o = make_uint2(pack_bf16(f.x + ra.x, f.y + ra.y), pack_bf16(f.z + rb.x, f.w + rb.y));
-            *(uint2*)(out + rowoff + (size_t)w * C) = o;
+      } else {
+        // A2[b][kw][j][h][ri][cl] gathered into the MN-major A operand (K = (ri,kw), M = channel)
+        const int b = bh / H, h = bh - b * H;
+        const int kwg = (Kw + 7) / 8;
+        const size_t kwstride = (size_t)nb * H * NT;
+        const __nv_bfloat16* base = in + ((size_t)b * Kw * nb * H + h) * NT;
+        for (int u = 0; u < 2 * kwg * 4; ++u) {
+          const int rg = u >> 2;
+          const int ri = rg >= kwg ? 1 : 0, kw = (rg - ri * kwg) * 8 + hl;
+          const int mc = (u & 3) * 4 + cl4;
+          const int c0 = cg * CGRP + mc * 8;
+          if (kw < Kw && c0 < C) {
+            const int j = c0 / BS, cl = c0 - j * BS;
+            cp_async16(dst + mc * kRowSbo + (ri * BS + kw) * 16,
+                       base + (size_t)kw * kwstride + (size_t)j * H * NT + ri * BS + cl);
           }
-        });
+        }
+      }
+      cp_async_wait_all();
+      fence_async_smem();
+      __syncwarp();
+      if (lane == 0) {
+        // the epilogue has drained this accumulator's previous contents
+        if (use > 0) mbar_wait(&empty[p], (uint32_t)((use - 1) & 1));
+        tc_fence_after();
+        const uint32_t d = tmem + p * 256;
+#pragma unroll
+        for (int ks = 0; ks < WP / 16; ++ks)
+          mma_ss(d, smem_desc(dst + ks * 2 * kRowLbo, kRowLbo, kRowSbo),
+                 smem_desc(smem_u32(sF) + ks * 2 * kFwLbo, kFwLbo, kFwSbo), idesc, ks > 0);
+        mma_commit(&full[p]);
+      }
+      __syncwarp();
+    }
+  } else {
+    // ===== epilogue warps: group grp = column half, lanes = channels =============================
+    const int grp = warp >> 2, tg = tid & 127;
+    float* sT = (float*)(smem + kFwBytes + 2 * kRowBytes + grp * kTrBytes);
+    uint32_t* sTu = (uint32_t*)sT;
+    const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
+    const int c4 = (tg & 31) * 4;       // this thread's 4 channels after the transpose
+    const int wq = tg >> 5;             // warp inside the group: column (pair) phase
+    for (int it = 0; it < nmine; ++it) {
+      const int t = blockIdx.x + it * gridDim.x;
+      const int cg = t % ncg, bh = t / ncg;
+      const int c = cg * CGRP + c4;
+      const bool cvalid = c < C;
+      mbar_wait(&full[it & 1], (uint32_t)((it >> 1) & 1));
+      tc_fence_after();
+      const uint32_t acc = tmem + (it & 1) * 256 + lane_base + grp * BS;
+      if (!INVERSE) {
+        // A1[b][kw][j][h][ri][cl]: per thread the address is base + kw * stride
+        const int b = bh / H, h = bh - b * H;
+        const int j = c / BS, cl = c - j * BS;
+        const size_t kwstride = (size_t)nb * H * NT;
+        __nv_bfloat16* obase = out + (((size_t)b * Kw * nb + j) * H + h) * NT + grp * BS + cl;
+#pragma unroll 1
+        for (int k = 0; k < 3; ++k) {
+          uint32_t v[32];
+          tmem_ld32(acc + 32 * k, v);
+          tmem_wait_ld();
+          if (k == 2) {
+            tc_fence_before();
+            mbar_arrive(&empty[it & 1]);
+          }
+          // column pairs (2q, 2q+1) of this channel packed to bf16x2, transposed through smem
+#pragma unroll
+          for (int q = 0; q < 16; ++q)
+            sTu[q * kTrPitch + tg] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
+          asm volatile("bar.sync %0, 128;" ::"r"(1 + grp) : "memory");
+#pragma unroll
+          for (int pass = 0; pass < 4; ++pass) {
+            const int qp = pass * 4 + wq;
+            const uint4 w4 = *(const uint4*)&sTu[qp * kTrPitch + c4];
+            const int kw0 = 32 * k + 2 * qp;
+            __nv_bfloat16* dstp = obase + (size_t)kw0 * kwstride;
+            if (cvalid && kw0 < Kw)
+              *(uint2*)dstp = make_uint2(__byte_perm(w4.x, w4.y, 0x5410), __byte_perm(w4.z, w4.w, 0x5410));
+            if (cvalid && kw0 + 1 < Kw)
+              *(uint2*)(dstp + kwstride) = make_uint2(__byte_perm(w4.x, w4.y, 0x7632), __byte_perm(w4.z, w4.w, 0x7632));
+          }
+          asm volatile("bar.sync %0, 128;" ::"r"(1 + grp) : "memory");
+        }
+      } else {
+        const size_t rowoff = (size_t)bh * W * C + c;
+        const __nv_bfloat16* rbase = res ? res + rowoff : nullptr;
+        __nv_bfloat16* obase = out + rowoff;
+#pragma unroll 1
+        for (int k = 0; k < 3; ++k) {
+          const int w0 = grp * BS + 32 * k + wq;
+          uint32_t v[32];
+          tmem_ld32(acc + 32 * k, v);
+          // residual rows of this chunk (8 independent 8-byte loads in flight per thread)
+          uint2 rr[8];
+#pragma unroll
+          for (int pass = 0; pass < 8; ++pass) {
+            const int w = w0 + pass * 4;
+            rr[pass] = make_uint2(0u, 0u);
+            if (rbase && cvalid && w < W) rr[pass] = __ldg((const uint2*)(rbase + (size_t)w * C));
+          }
+          tmem_wait_ld();
+          if (k == 2) {
+            tc_fence_before();
+            mbar_arrive(&empty[it & 1]);
+          }
+#pragma unroll
+          for (int q = 0; q < 32; ++q) sTu[q * kTrPitch + tg] = v[q];
+          asm volatile("bar.sync %0, 128;" ::"r"(1 + grp) : "memory");
+#pragma unroll
+          for (int pass = 0; pass < 8; ++pass) {
+            const int q = pass * 4 + wq;
+            const float4 f = *(const float4*)&sT[q * kTrPitch + c4];
+            const int w = w0 + pass * 4;
+            const uint2 r2 = rr[pass];
+            // bf16 -> fp32 is a 16-bit shift
+            const float r0 = __uint_as_float(r2.x << 16), r1 = __uint_as_float(r2.x & 0xFFFF0000u);
+            const float r2f = __uint_as_float(r2.y << 16), r3 = __uint_as_float(r2.y & 0xFFFF0000u);
+            if (cvalid && w < W)
+              *(uint2*)(obase + (size_t)w * C) = make_uint2(pack_bf16(f.x + r0, f.y + r1), pack_bf16(f.z + r2f, f.w + r3));
+          }
+          asm volatile("bar.sync %0, 128;" ::"r"(1 + grp) : "memory");
+        }
       }
     }
   }
-  cp_async_wait_all();
   tc_fence_before();
   __syncthreads();
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
 
-// ---- F2-F7: per (b, kw, block) chain  H-DFT -> layer 1 -> layer 2 -> inverse H-DFT ---------------
-// 256 threads: warp w owns TMEM lanes 32*(w&3).. (accumulator rows) and the column half w>>2
-// (re | im), so every epilogue is split two ways.  Accumulators in tensor memory: region R0 =
-// columns [0,192), R1 = [256,448); a layer's bf16 input (A operand) is packed in place over
-// the fp32 accumulator it was computed from (all loads, block barrier, then the stores).
+// ---- F2-F7 / B1-B7: per (b, kw, block) GEMM chains in tensor memory --------------------------------
+// CTA = 8 epilogue warps + 1 control warp.
+//   control warp : copies the mode tiles (cp.async), makes them visible to the async proxy and
+//                  issues every tcgen05.mma (lane 0).
+//   epilogue warp w: TMEM lanes 32*(w&3).. (accumulator rows = modes) and column half w>>2
+//                  (0: re, 1: im).  It converts its 96 fp32 accumulator columns of a stage in
+//                  three 32-column chunks, writes each chunk packed to bf16 IN PLACE (columns
+//                  [96*half + 16c, +16) of the same region: the A operand of the next GEMM) and
+//                  arrives on that chunk's mbarrier.
+// The control warp issues the K-steps of the next MLP GEMM chunk by chunk as those barriers
+// complete, so the tensor core runs under the epilogue of the previous stage.  No block-wide
+// barrier is used; all hand-offs are mbarriers.
+// Tensor memory: R0 = columns [0,192), R1 = [256,448); a stage reads its A operand from one
+// region and accumulates into the other.
+constexpr int kMixEpiThreads = 256;
+constexpr int kMixThreads = kMixEpiThreads + 64;   // + control warp + loader warp
+constexpr uint32_t kMixSmem2 = 2 * kDftBytes + 4 * kWBytes + 2 * kTileBytes; // 196608
+
 struct MixParams {
-  const __nv_bfloat16* A1;
+  const __nv_bfloat16* A1;   // forward: spectrum tiles; backward: x tiles
+  const __nv_bfloat16* A1g;  // backward: gradient tiles
   __nv_bfloat16* A2;
-  const uint8_t* dft;      // Ch then Sh, kDftBytes each, smem image
-  const uint8_t* wprep;    // per block 8 x kWBytes
-  const float* b1;         // [nb][96][2]
-  const float* b2;
-  int B, H, Kw, nb, Kh;
+  __nv_bfloat16 *Xh, *O1, *G2, *G1; // backward: operands of tc_wgrad
+  const uint8_t* dft;        // Ch then Sh, kDftBytes each, smem image
+  const uint8_t* wprep;      // per block 4 x kWBytes: W1r, W1i, W2r, W2i (n=o, k=i, K-major)
+  const float* bprep;        // per block [2 layers][192]: (re 96 | im 96)
+  uint8_t* mask1;            // optional export, [B][H][Wh][C][2]
+  uint8_t* mask2;
+  int B, H, Kw, Wh, nb, Kh;
   float lambda;
 };
 
-constexpr int kMixThreads = 256;
-
-// D[:, dcol .. dcol+96) (+)= A_smem(K-major [128 x 96]) * tile half (MN-major, 96 columns)
+// D[:, 0..96) (+)= A_smem(K-major [128 x 96]) * tile half (MN-major, 96 columns)
 __device__ __forceinline__ void issue_dft(uint32_t d, uint32_t a_base, uint32_t b_base, uint32_t idesc, bool fresh) {
 #pragma unroll
   for (int ks = 0; ks < HP / 16; ++ks)
     mma_ss(d, smem_desc(a_base + ks * 2 * kDftLbo, kDftLbo, kDftSbo),
            smem_desc(b_base + ks * 2 * kTileLbo, kTileLbo, kTileSbo), idesc, !(fresh && ks == 0));
 }
-// D[:, dcol .. dcol+96) (+)= A_tmem(packed bf16, 48 columns = K 96) * W_smem(K-major [96 x 96])
-__device__ __forceinline__ void issue_mlp(uint32_t d, uint32_t a_tmem, uint32_t w_base, uint32_t idesc, bool fresh) {
-#pragma unroll
-  for (int ks = 0; ks < BS / 16; ++ks)
-    mma_ts(d, a_tmem + ks * 8, smem_desc(w_base + ks * 2 * kWLbo, kWLbo, kWSbo), idesc, !(fresh && ks == 0));
+// forward transform (exp(-i theta)):  Xr = Ch Ar + Sh Ai ; Xi = Ch Ai - Sh Ar
+__device__ __forceinline__ void issue_fwd_dft(uint32_t R, uint32_t aCh, uint32_t aSh, uint32_t tile) {
+  const uint32_t id = idesc_bf16(128, BS, kIdescBMn), half = (BS / 8) * kTileSbo;
+  issue_dft(R, aCh, tile, id, true);
+  issue_dft(R, aSh, tile + half, id, false);
+  issue_dft(R + BS, aCh, tile + half, id, true);
+  issue_dft(R + BS, aSh, tile, id | kIdescNegA, false);
 }
-// same with W^H: the forward weight image (n=o, k=i, K-major) read as an MN-major B operand (k=o, n=i)
-__device__ __forceinline__ void issue_mlp_t(uint32_t d, uint32_t a_tmem, uint32_t w_base, uint32_t idesc, bool fresh) {
+// inverse transform (exp(+i theta)):  Tr = Ch Zr - Sh Zi ; Ti = Ch Zi + Sh Zr
+__device__ __forceinline__ void issue_inv_dft(uint32_t R, uint32_t aCh, uint32_t aSh, uint32_t tile) {
+  const uint32_t id = idesc_bf16(128, BS, kIdescBMn), half = (BS / 8) * kTileSbo;
+  issue_dft(R, aCh, tile, id, true);
+  issue_dft(R, aSh, tile + half, id | kIdescNegA, false);
+  issue_dft(R + BS, aCh, tile + half, id, true);
+  issue_dft(R + BS, aSh, tile, id, false);
+}
+// K-steps of chunk c (32 source columns of each half = 2 K-steps of 16) of an MLP GEMM.
+//   TRANSPOSED = false:  T = S W      : Tr = Sr Wr - Si Wi ; Ti = Sr Wi + Si Wr
+//   TRANSPOSED = true :  T = S W^H    : Tr = Sr Wr^T + Si Wi^T ; Ti = Si Wr^T - Sr Wi^T
+// (W^H reads the same weight image as an MN-major operand with LBO and SBO exchanged.)
+template <bool TRANSPOSED>
+__device__ __forceinline__ void issue_mlp_chunk(uint32_t T, uint32_t S, uint32_t wr, uint32_t wi, int c) {
+  const uint32_t id = idesc_bf16(128, BS, TRANSPOSED ? kIdescBMn : 0u);
+  const uint32_t lbo = TRANSPOSED ? kWSbo : kWLbo, sbo = TRANSPOSED ? kWLbo : kWSbo;
 #pragma unroll
-  for (int ks = 0; ks < BS / 16; ++ks)
-    mma_ts(d, a_tmem + ks * 8, smem_desc(w_base + ks * 2 * kWSbo, kWSbo, kWLbo), idesc, !(fresh && ks == 0));
+  for (int ks = 2 * c; ks < 2 * c + 2; ++ks) {   // re chunk of the A operand
+    const uint32_t acc = ks != 0;
+    mma_ts(T, S + ks * 8, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, acc);
+    mma_ts(T + BS, S + ks * 8, smem_desc(wi + ks * 2 * lbo, lbo, sbo), TRANSPOSED ? (id | kIdescNegB) : id, acc);
+  }
+#pragma unroll
+  for (int ks = 2 * c; ks < 2 * c + 2; ++ks) {   // im chunk
+    mma_ts(T, S + BS + ks * 8, smem_desc(wi + ks * 2 * lbo, lbo, sbo), TRANSPOSED ? id : (id | kIdescNegB), 1u);
+    mma_ts(T + BS, S + BS + ks * 8, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, 1u);
+  }
 }
 
-struct MixThread {
-  uint32_t lane_base; // TMEM lane offset of this warp's 32 rows
-  int colh;           // 0: re columns [0,96), 1: im columns [96,192)
-  int r;              // accumulator row of this thread
+struct MixBars {
+  uint64_t dfull[8];      // stage s accumulated (tcgen05.commit)
+  uint64_t cready[2][3];  // packed A-operand chunk (half, c) written by all 128 rows
+  uint64_t zready;        // bf16 tile for the inverse transform written to shared memory
+  uint64_t tfull[2];      // tile buffer filled by the loader warp (32 arrivals)
+  uint64_t tfree[2];      // tile buffer consumed by its last GEMM (tcgen05.commit)
 };
 
-// this thread's 96 accumulator columns of a region -> registers
-__device__ __forceinline__ void ld_half(uint32_t region, const MixThread& t, uint32_t (&v)[3][32]) {
-#pragma unroll
-  for (int k = 0; k < 3; ++k) tmem_ld32(region + t.lane_base + t.colh * BS + 32 * k, v[k]);
-  tmem_wait_ld();
-}
-// packed bf16 A operand of the next GEMM: K index = column, re half -> columns [0,48), im -> [48,96)
-__device__ __forceinline__ void st_half_packed(uint32_t region, const MixThread& t, const uint32_t (&pk)[3][16]) {
-#pragma unroll
-  for (int k = 0; k < 3; ++k) tmem_st16(region + t.lane_base + t.colh * (BS / 2) + 16 * k, pk[k]);
-}
-__device__ __forceinline__ void store_row_half(__nv_bfloat16* dst, const uint32_t (&pk)[3][16]) {
-#pragma unroll
-  for (int k = 0; k < 3; ++k)
-#pragma unroll
-    for (int g = 0; g < 4; ++g)
-      *(uint4*)(dst + k * 32 + g * 8) = make_uint4(pk[k][4 * g], pk[k][4 * g + 1], pk[k][4 * g + 2], pk[k][4 * g + 3]);
-}
-// bf16 rows written as the MN-major B operand of the inverse H-DFT (K = row r)
-__device__ __forceinline__ void store_tile_half(uint8_t* tile, const MixThread& t, const uint32_t (&pk)[3][16]) {
-#pragma unroll
-  for (int k = 0; k < 3; ++k)
-#pragma unroll
-    for (int g = 0; g < 4; ++g)
-      *(uint4*)(tile + (t.colh * 12 + k * 4 + g) * kTileSbo + t.r * 16) =
-          make_uint4(pk[k][4 * g], pk[k][4 * g + 1], pk[k][4 * g + 2], pk[k][4 * g + 3]);
-}
-// rows of a (b,kw,j) tile [H][192] -> MN-major B operand (K = h, N = (ri, c)); 8 warps
-__device__ __forceinline__ void load_tile(uint32_t tile_saddr, const __nv_bfloat16* src, int H, int warp, int lane) {
+// rows of a (b,kw,j) tile [H][192] -> MN-major B operand (K = h, N = (ri, c)); one warp
+__device__ __forceinline__ void load_tile_warp(uint32_t tile_saddr, const __nv_bfloat16* src, int H, int lane) {
   const int hl = lane & 7, cl4 = lane >> 3;
   const int nunits = ((H + 7) / 8) * 6;
-  for (int u = warp; u < nunits; u += kMixThreads / 32) {
+  for (int u = 0; u < nunits; ++u) {
     const int h = (u / 6) * 8 + hl;
     const int nc = (u % 6) * 4 + cl4;
     if (h < H) cp_async16(tile_saddr + nc * kTileSbo + h * 16, src + (size_t)h * NT + nc * 8);
   }
 }
-__device__ __forceinline__ void block_tmem_sync() {
+
+__device__ __forceinline__ void pack32(const uint32_t (&v)[32], uint32_t (&pk)[16]) {
+#pragma unroll
+  for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
+}
+__device__ __forceinline__ void store16(__nv_bfloat16* dst, const uint32_t (&pk)[16]) {
+#pragma unroll
+  for (int g = 0; g < 4; ++g) *(uint4*)(dst + g * 8) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
+}
+// chunk c of this thread's row -> MN-major B operand tile (K = row r)
+__device__ __forceinline__ void store_tile16(uint8_t* tile, int half, int c, int r, const uint32_t (&pk)[16]) {
+#pragma unroll
+  for (int g = 0; g < 4; ++g)
+    *(uint4*)(tile + (half * 12 + c * 4 + g) * kTileSbo + r * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
+}
+// publish a packed chunk: TMEM stores complete, ordered before the barrier arrival
+__device__ __forceinline__ void publish_chunk(uint64_t* bar) {
+  tmem_wait_st();
   tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
+  mbar_arrive(bar);
 }
 
-constexpr uint32_t kMixFwdSmem = kMixSmem + kTileBytes; // two tile buffers (prefetch of the next tile)
-
-__global__ void __launch_bounds__(kMixThreads, 1) tc_mix_fwd(MixParams p) {
+template <bool BACKWARD, bool EXPORT>
+__global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
   extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) uint64_t mbar;
+  __shared__ MixBars bars;
   __shared__ uint32_t tmem_slot;
   uint8_t* sCh = smem;
   uint8_t* sSh = smem + kDftBytes;
   uint8_t* sW = smem + 2 * kDftBytes;
-  uint8_t* sTile0 = sW + 4 * kWBytes;
-  float* sBias = (float*)(sTile0 + kTileBytes); // b1 (re 96 | im 96), b2 (re 96 | im 96)
-  uint8_t* sTile1 = sTile0 + kTileBytes + 2 * NT * 4;
+  uint8_t* sTileA = sW + 4 * kWBytes;      // fwd: even tiles; bwd: x tile
+  uint8_t* sTileB = sTileA + kTileBytes;   // fwd: odd tiles;  bwd: gradient tile, later GX
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (uint32_t i = tid; i < kTileBytes / 16; i += kMixThreads) {
-    ((uint4*)sTile0)[i] = make_uint4(0, 0, 0, 0);
-    ((uint4*)sTile1)[i] = make_uint4(0, 0, 0, 0);
-  }
-  for (uint32_t i = tid; i < 2 * kDftBytes / 16; i += kMixThreads)
-    cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
+  for (uint32_t i = tid; i < 2 * kTileBytes / 16; i += kMixThreads) ((uint4*)sTileA)[i] = make_uint4(0, 0, 0, 0);
+  for (uint32_t i = tid; i < 2 * kDftBytes / 16; i += kMixThreads) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
   if (tid == 0) {
-    mbar_init(&mbar, 1);
+    for (int s = 0; s < 8; ++s) mbar_init(&bars.dfull[s], 1);
+    for (int h = 0; h < 2; ++h)
+      for (int c = 0; c < 3; ++c) mbar_init(&bars.cready[h][c], kMixEpiThreads / 2);
+    mbar_init(&bars.zready, kMixEpiThreads);
+    for (int b = 0; b < 2; ++b) {
+      mbar_init(&bars.tfull[b], 32);
+      mbar_init(&bars.tfree[b], 1);
+    }
     mbar_init_fence();
   }
   if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  cp_async_wait_all();
+  fence_async_smem();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
-  MixThread th;
-  th.lane_base = (uint32_t)((warp & 3) * 32) << 16;
-  th.colh = warp >> 2;
-  th.r = (warp & 3) * 32 + lane;
   const uint32_t R0 = tmem, R1 = tmem + 256;
-  const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW);
-  const uint32_t half = (BS / 8) * kTileSbo;
-  const uint32_t id_dft = idesc_bf16(128, BS, kIdescBMn);
-  const uint32_t id_mlp = idesc_bf16(128, BS);
-
   const int ntiles = p.nb * p.B * p.Kw;
   const int per = (ntiles + gridDim.x - 1) / gridDim.x;
   const int t_begin = blockIdx.x * per, t_end = min(ntiles, t_begin + per);
-  uint32_t phase = 0;
-  int cur_j = -1;
-  const int r = th.r;
-  const int kappa = (r <= p.H / 2) ? r : p.H - r;
-  const bool row_kept = (r < p.H) && (kappa < p.Kh);
-  const float* bias1 = sBias + th.colh * BS;
-  const float* bias2 = sBias + NT + th.colh * BS;
+  const int BKw = p.B * p.Kw;
 
-  auto tile_src = [&](int t) {
-    const int j = t / (p.B * p.Kw);
-    const int rem = t - j * (p.B * p.Kw);
-    return p.A1 + ((size_t)rem * p.nb + j) * p.H * NT;
-  };
-  if (t_begin < t_end) load_tile(smem_u32(sTile0), tile_src(t_begin), p.H, warp, lane);
-  cp_async_commit();
-
-  for (int t = t_begin; t < t_end; ++t) {
-    const int j = t / (p.B * p.Kw);
-    const int rem = t - j * (p.B * p.Kw);
-    uint8_t* sTile = ((t - t_begin) & 1) ? sTile1 : sTile0;
-    const uint32_t aTile = smem_u32(sTile);
-    const bool new_block = j != cur_j;
-    if (new_block) {
-      cur_j = j;
-      const uint8_t* wsrc = p.wprep + (size_t)j * 8 * kWBytes;
-      for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMixThreads) cp_async16(aW + i * 16, wsrc + (size_t)i * 16);
-      for (int i = tid; i < 2 * NT; i += kMixThreads) {
-        const int which = i / NT, n = i % NT, ri = n / BS, o = n % BS;
-        sBias[i] = (which == 0 ? p.b1 : p.b2)[((size_t)j * BS + o) * 2 + ri];
+  if (warp == kMixEpiThreads / 32 + 1) {
+    // ================================ loader warp ============================================
+    // forward : tile i -> buffer i&1 (free once the inverse transform of tile i-2 has completed)
+    // backward: x tile -> buffer A (free after stage 0), gradient tile -> buffer B (free after stage 6)
+    const uint32_t aTA = smem_u32(sTileA), aTB = smem_u32(sTileB);
+    for (int t = t_begin; t < t_end; ++t) {
+      const int i = t - t_begin;
+      const int j = t / BKw, rem = t - j * BKw;
+      const size_t off = ((size_t)rem * p.nb + j) * p.H * NT;
+      if (!BACKWARD) {
+        const int b = i & 1, use = i >> 1;
+        if (use > 0) mbar_wait(&bars.tfree[b], (uint32_t)((use - 1) & 1));
+        load_tile_warp(b ? aTB : aTA, p.A1 + off, p.H, lane);
+        cp_async_wait_all();
+        fence_async_smem();
+        mbar_arrive(&bars.tfull[b]);
+      } else {
+        if (i > 0) mbar_wait(&bars.tfree[0], (uint32_t)((i - 1) & 1));
+        load_tile_warp(aTA, p.A1 + off, p.H, lane);
+        cp_async_wait_all();
+        fence_async_smem();
+        mbar_arrive(&bars.tfull[0]);
+        if (i > 0) mbar_wait(&bars.tfree[1], (uint32_t)((i - 1) & 1));
+        load_tile_warp(aTB, p.A1g + off, p.H, lane);
+        cp_async_wait_all();
+        fence_async_smem();
+        mbar_arrive(&bars.tfull[1]);
       }
     }
-    // prefetch the next tile into the other buffer (its last reader, the previous inverse DFT, is complete)
-    if (t + 1 < t_end) load_tile(smem_u32(((t - t_begin) & 1) ? sTile0 : sTile1), tile_src(t + 1), p.H, warp, lane);
-    cp_async_commit();
-    if (new_block) cp_async_wait_group<0>();
-    else cp_async_wait_group<1>();
-    fence_async_smem();
-    block_tmem_sync();
-    // F2: Xr = Ch Ar + Sh Ai ; Xi = Ch Ai - Sh Ar      (forward kernel exp(-i theta))
-    if (tid == 0) {
-      issue_dft(R0, aCh, aTile, id_dft, true);
-      issue_dft(R0, aSh, aTile + half, id_dft, false);
-      issue_dft(R0 + BS, aCh, aTile + half, id_dft, true);
-      issue_dft(R0 + BS, aSh, aTile, id_dft | kIdescNegA, false);
-      mma_commit(&mbar);
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
-    tc_fence_after();
-    {
-      uint32_t v[3][32], pk[3][16];
-      ld_half(R0, th, v);
-      block_tmem_sync();
-#pragma unroll
-      for (int k = 0; k < 3; ++k)
-#pragma unroll
-        for (int q = 0; q < 16; ++q) pk[k][q] = pack_bf16(__uint_as_float(v[k][2 * q]), __uint_as_float(v[k][2 * q + 1]));
-      st_half_packed(R0, th, pk);
-      tmem_wait_st();
-    }
-    block_tmem_sync();
-    // F3: P1 = Xh W1 + b1
-    if (tid == 0) {
-      issue_mlp(R1, R0, aW + 0 * kWBytes, id_mlp, true);                         // Xr W1r
-      issue_mlp(R1, R0 + BS / 2, aW + 1 * kWBytes, id_mlp | kIdescNegB, false);  // - Xi W1i
-      issue_mlp(R1 + BS, R0, aW + 1 * kWBytes, id_mlp, true);                    // Xr W1i
-      issue_mlp(R1 + BS, R0 + BS / 2, aW + 0 * kWBytes, id_mlp, false);          // + Xi W1r
-      mma_commit(&mbar);
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
-    tc_fence_after();
-    {
-      // F4: bias + split ReLU
-      uint32_t v[3][32], pk[3][16];
-      ld_half(R1, th, v);
-      block_tmem_sync();
-#pragma unroll
-      for (int k = 0; k < 3; ++k)
-#pragma unroll
-        for (int q = 0; q < 16; ++q) {
-          const float a = fmaxf(__uint_as_float(v[k][2 * q]) + bias1[32 * k + 2 * q], 0.f);
-          const float b = fmaxf(__uint_as_float(v[k][2 * q + 1]) + bias1[32 * k + 2 * q + 1], 0.f);
-          pk[k][q] = pack_bf16(a, b);
+  } else if (warp == kMixEpiThreads / 32) {
+    // ================================ control warp ===========================================
+    const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW);
+    const uint32_t aTA = smem_u32(sTileA), aTB = smem_u32(sTileB);
+    uint32_t pc = 0;       // parity of the chunk barriers (they complete once per MLP stage)
+    int cur_j = -1;
+    auto mlp_stage = [&](uint32_t T, uint32_t S, uint32_t wr, uint32_t wi, bool transposed, uint64_t* done) {
+      for (int c = 0; c < 3; ++c) {
+        mbar_wait(&bars.cready[0][c], pc);
+        mbar_wait(&bars.cready[1][c], pc);
+        if (lane == 0) {
+          tc_fence_after();
+          if (transposed) issue_mlp_chunk<true>(T, S, wr, wi, c);
+          else issue_mlp_chunk<false>(T, S, wr, wi, c);
         }
-      st_half_packed(R1, th, pk);
-      tmem_wait_st();
-    }
-    block_tmem_sync();
-    // F5: P2 = O1 W2 + b2
-    if (tid == 0) {
-      issue_mlp(R0, R1, aW + 2 * kWBytes, id_mlp, true);
-      issue_mlp(R0, R1 + BS / 2, aW + 3 * kWBytes, id_mlp | kIdescNegB, false);
-      issue_mlp(R0 + BS, R1, aW + 3 * kWBytes, id_mlp, true);
-      issue_mlp(R0 + BS, R1 + BS / 2, aW + 2 * kWBytes, id_mlp, false);
-      mma_commit(&mbar);
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
-    tc_fence_after();
-    {
-      // F6: bias + softshrink + truncation -> bf16 Z as the B operand of the inverse transform
-      uint32_t v[3][32], pk[3][16];
-      ld_half(R0, th, v);
-#pragma unroll
-      for (int k = 0; k < 3; ++k)
-#pragma unroll
-        for (int q = 0; q < 16; ++q) {
-          float a = __uint_as_float(v[k][2 * q]) + bias2[32 * k + 2 * q];
-          float b = __uint_as_float(v[k][2 * q + 1]) + bias2[32 * k + 2 * q + 1];
-          const float ma = fabsf(a) - p.lambda, mb = fabsf(b) - p.lambda;
-          a = (row_kept && ma > 0.f) ? copysignf(ma, a) : 0.f;
-          b = (row_kept && mb > 0.f) ? copysignf(mb, b) : 0.f;
-          pk[k][q] = pack_bf16(a, b);
+      }
+      if (lane == 0) mma_commit(done);
+      __syncwarp();
+      pc ^= 1;
+    };
+    for (int t = t_begin; t < t_end; ++t) {
+      const int i = t - t_begin;
+      const uint32_t tp = (uint32_t)(i & 1);          // parity of this tile's per-tile barriers
+      const int j = t / BKw;
+      const uint32_t last = BACKWARD ? 6 : 3;         // index of the chain's final stage
+      if (j != cur_j) {
+        // new channel block: every GEMM of the previous tile is complete, reload the weights
+        cur_j = j;
+        if (i > 0) mbar_wait(&bars.dfull[last], tp ^ 1);
+        const uint8_t* wsrc = p.wprep + (size_t)j * 4 * kWBytes;
+        for (uint32_t q = lane; q < 4 * kWBytes / 16; q += 32) cp_async16(aW + q * 16, wsrc + (size_t)q * 16);
+        cp_async_wait_all();
+        fence_async_smem();
+        __syncwarp();
+      }
+      if (!BACKWARD) {
+        const int b = i & 1;
+        const uint32_t cur_tile = b ? aTB : aTA;
+        mbar_wait(&bars.tfull[b], (uint32_t)((i >> 1) & 1));
+        if (lane == 0) {
+          tc_fence_after();
+          issue_fwd_dft(R0, aCh, aSh, cur_tile);
+          mma_commit(&bars.dfull[0]);
         }
-      if (r < HP) store_tile_half(sTile, th, pk);
-    }
-    fence_async_smem();
-    block_tmem_sync();
-    // F7: Tr = Ch Zr - Sh Zi ; Ti = Ch Zi + Sh Zr      (inverse kernel exp(+i theta))
-    if (tid == 0) {
-      issue_dft(R1, aCh, aTile, id_dft, true);
-      issue_dft(R1, aSh, aTile + half, id_dft | kIdescNegA, false);
-      issue_dft(R1 + BS, aCh, aTile + half, id_dft, true);
-      issue_dft(R1 + BS, aSh, aTile, id_dft, false);
-      mma_commit(&mbar);
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
-    tc_fence_after();
-    {
-      uint32_t v[3][32], pk[3][16];
-      ld_half(R1, th, v);
-#pragma unroll
-      for (int k = 0; k < 3; ++k)
-#pragma unroll
-        for (int q = 0; q < 16; ++q) pk[k][q] = pack_bf16(__uint_as_float(v[k][2 * q]), __uint_as_float(v[k][2 * q + 1]));
-      if (r < p.H) store_row_half(p.A2 + (((size_t)rem * p.nb + j) * p.H + r) * NT + th.colh * BS, pk);
-    }
-  }
-  tc_fence_before();
-  __syncthreads();
-  if (warp == 0) tmem_dealloc<512>(tmem);
-}
-
-// ---- B1-B7 (except the parameter sums): per (b, kw, block) backward chain ------------------------
-//   recompute  Xh = Fh A1x -> P1 -> O1 -> P2 (masks kept as bit sets in registers)
-//   G = Fh A1g ; G2 = G (.) mask2 ; G1 = mask1 (.) (G2 W2^H) ; GX = G1 W1^H ; A2 = Fh^H GX
-// Xh, O1, G2, G1 are also written (bf16, tile layout [b*Kw+kw][j][r][192]) for tc_wgrad.
-struct MixBwdParams {
-  const __nv_bfloat16* A1x;
-  const __nv_bfloat16* A1g;
-  __nv_bfloat16* A2;
-  __nv_bfloat16 *Xh, *O1, *G2, *G1;
-  const uint8_t* dft;
-  const uint8_t* wprep;
-  const float* b1;
-  const float* b2;
-  uint8_t* mask1; // optional export, [B][H][Wh][C][2]
-  uint8_t* mask2;
-  int B, H, Kw, Wh, nb, Kh;
-  float lambda;
-};
-
-constexpr uint32_t kMixBwdSmem = kMixSmem + kTileBytes; // second tile buffer for the gradient spectrum
-
-__global__ void __launch_bounds__(kMixThreads, 1) tc_mix_bwd(MixBwdParams p) {
-  extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) uint64_t mbar;
-  __shared__ uint32_t tmem_slot;
-  uint8_t* sCh = smem;
-  uint8_t* sSh = smem + kDftBytes;
-  uint8_t* sW = smem + 2 * kDftBytes;
-  uint8_t* sTile = sW + 4 * kWBytes;
-  float* sBias = (float*)(sTile + kTileBytes);
-  uint8_t* sTileG = sTile + kTileBytes + 2 * NT * 4;
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (uint32_t i = tid; i < kTileBytes / 16; i += kMixThreads) {
-    ((uint4*)sTile)[i] = make_uint4(0, 0, 0, 0);
-    ((uint4*)sTileG)[i] = make_uint4(0, 0, 0, 0);
-  }
-  for (uint32_t i = tid; i < 2 * kDftBytes / 16; i += kMixThreads)
-    cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
-  if (tid == 0) {
-    mbar_init(&mbar, 1);
-    mbar_init_fence();
-  }
-  if (warp == 0) tmem_alloc<512>(&tmem_slot);
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = tmem_slot;
-  MixThread th;
-  th.lane_base = (uint32_t)((warp & 3) * 32) << 16;
-  th.colh = warp >> 2;
-  th.r = (warp & 3) * 32 + lane;
-  const uint32_t R0 = tmem, R1 = tmem + 256;
-  const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW);
-  const uint32_t aTile = smem_u32(sTile), aTileG = smem_u32(sTileG);
-  const uint32_t half = (BS / 8) * kTileSbo;
-  const uint32_t id_dft = idesc_bf16(128, BS, kIdescBMn);
-  const uint32_t id_mlp = idesc_bf16(128, BS);
-  const uint32_t id_mlp_t = idesc_bf16(128, BS, kIdescBMn);
-
-  const int ntiles = p.nb * p.B * p.Kw;
-  const int per = (ntiles + gridDim.x - 1) / gridDim.x;
-  const int t_begin = blockIdx.x * per, t_end = min(ntiles, t_begin + per);
-  uint32_t phase = 0;
-  int cur_j = -1;
-  const int r = th.r;
-  const int kappa = (r <= p.H / 2) ? r : p.H - r;
-  const bool row_valid = r < p.H;
-  const bool row_kept = row_valid && (kappa < p.Kh);
-  const float* bias1 = sBias + th.colh * BS;
-  const float* bias2 = sBias + NT + th.colh * BS;
-
-  for (int t = t_begin; t < t_end; ++t) {
-    const int j = t / (p.B * p.Kw);
-    const int rem = t - j * (p.B * p.Kw);
-    if (j != cur_j) {
-      cur_j = j;
-      const uint8_t* wsrc = p.wprep + (size_t)j * 8 * kWBytes;
-      for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMixThreads) cp_async16(aW + i * 16, wsrc + (size_t)i * 16);
-      for (int i = tid; i < 2 * NT; i += kMixThreads) {
-        const int which = i / NT, n = i % NT, ri = n / BS, o = n % BS;
-        sBias[i] = (which == 0 ? p.b1 : p.b2)[((size_t)j * BS + o) * 2 + ri];
+        __syncwarp();
+        mlp_stage(R1, R0, aW + 0 * kWBytes, aW + 1 * kWBytes, false, &bars.dfull[1]);
+        mlp_stage(R0, R1, aW + 2 * kWBytes, aW + 3 * kWBytes, false, &bars.dfull[2]);
+        mbar_wait(&bars.zready, tp);
+        if (lane == 0) {
+          tc_fence_after();
+          issue_inv_dft(R1, aCh, aSh, cur_tile);
+          mma_commit(&bars.dfull[3]);
+          mma_commit(&bars.tfree[b]);
+        }
+        __syncwarp();
+      } else {
+        mbar_wait(&bars.tfull[0], tp);
+        if (lane == 0) {
+          tc_fence_after();
+          issue_fwd_dft(R0, aCh, aSh, aTA);
+          mma_commit(&bars.dfull[0]);
+          mma_commit(&bars.tfree[0]);
+        }
+        __syncwarp();
+        mlp_stage(R1, R0, aW + 0 * kWBytes, aW + 1 * kWBytes, false, &bars.dfull[1]);
+        mlp_stage(R0, R1, aW + 2 * kWBytes, aW + 3 * kWBytes, false, &bars.dfull[2]);
+        // stage 3: G = Fh A1g into R1 (its previous contents, the A operand of stage 2, are dead
+        // once stage 2 has completed)
+        mbar_wait(&bars.dfull[2], tp);
+        mbar_wait(&bars.tfull[1], tp);
+        if (lane == 0) {
+          tc_fence_after();
+          issue_fwd_dft(R1, aCh, aSh, aTB);
+          mma_commit(&bars.dfull[3]);
+        }
+        __syncwarp();
+        mlp_stage(R0, R1, aW + 2 * kWBytes, aW + 3 * kWBytes, true, &bars.dfull[4]);   // G1 = G2 W2^H
+        mlp_stage(R1, R0, aW + 0 * kWBytes, aW + 1 * kWBytes, true, &bars.dfull[5]);   // GX = G1 W1^H
+        mbar_wait(&bars.zready, tp);
+        if (lane == 0) {
+          tc_fence_after();
+          issue_inv_dft(R1, aCh, aSh, aTB);   // into R1: the next tile's stage 0 reuses R0 at once
+          mma_commit(&bars.dfull[6]);
+          mma_commit(&bars.tfree[1]);
+        }
+        __syncwarp();
       }
     }
-    const size_t tile_off = ((size_t)rem * p.nb + j) * p.H * NT;
-    load_tile(aTile, p.A1x + tile_off, p.H, warp, lane);
-    load_tile(aTileG, p.A1g + tile_off, p.H, warp, lane);
-    const size_t row_off = tile_off + (size_t)r * NT + th.colh * BS;
-    cp_async_wait_all();
-    fence_async_smem();
-    block_tmem_sync();
-    // ---- Xh = Fh A1x -----------------------------------------------------------------------
-    if (tid == 0) {
-      issue_dft(R0, aCh, aTile, id_dft, true);
-      issue_dft(R0, aSh, aTile + half, id_dft, false);
-      issue_dft(R0 + BS, aCh, aTile + half, id_dft, true);
-      issue_dft(R0 + BS, aSh, aTile, id_dft | kIdescNegA, false);
-      mma_commit(&mbar);
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
-    tc_fence_after();
-    {
-      uint32_t v[3][32], pk[3][16];
-      ld_half(R0, th, v);
-      block_tmem_sync();
+  } else {
+    // ================================ epilogue warps =========================================
+    const int half = warp >> 2;
+    const int r = (warp & 3) * 32 + lane;
+    const uint32_t lane_base = ((uint32_t)((warp & 3) * 32) << 16) + half * BS;
+    const int kappa = (r <= p.H / 2) ? r : p.H - r;
+    const bool row_valid = r < p.H;
+    const bool row_kept = row_valid && (kappa < p.Kh);
+    for (int t = t_begin; t < t_end; ++t) {
+      const int i = t - t_begin;
+      const uint32_t tp = (uint32_t)(i & 1);
+      const int j = t / BKw, rem = t - j * BKw;
+      const size_t row_off = (((size_t)rem * p.nb + j) * p.H + r) * NT + half * BS;
+      const float* bias1 = p.bprep + (size_t)j * 2 * NT + half * BS;
+      const float* bias2 = bias1 + NT;
+      uint32_t m1[3], m2[3];
+      // ---- stage 0 -> spectrum Xh, packed in place (R0) ----
+      mbar_wait(&bars.dfull[0], tp);
+      tc_fence_after();
 #pragma unroll
-      for (int k = 0; k < 3; ++k)
+      for (int c = 0; c < 3; ++c) {
+        uint32_t v[32], pk[16];
+        tmem_ld32(R0 + lane_base + 32 * c, v);
+        tmem_wait_ld();
+        pack32(v, pk);
+        tmem_st16(R0 + lane_base + 16 * c, pk);
+        if (BACKWARD && row_valid) store16(p.Xh + row_off + 32 * c, pk);
+        publish_chunk(&bars.cready[half][c]);
+      }
+      // ---- stage 1 -> O1 = relu(P1 + b1), packed in place (R1) ----
+      mbar_wait(&bars.dfull[1], tp);
+      tc_fence_after();
 #pragma unroll
-        for (int q = 0; q < 16; ++q) pk[k][q] = pack_bf16(__uint_as_float(v[k][2 * q]), __uint_as_float(v[k][2 * q + 1]));
-      st_half_packed(R0, th, pk);
-      if (row_valid) store_row_half(p.Xh + row_off, pk);
-      tmem_wait_st();
-    }
-    block_tmem_sync();
-    // ---- P1 = Xh W1 + b1 ; O1 = relu ; mask1 -------------------------------------------------
-    if (tid == 0) {
-      issue_mlp(R1, R0, aW + 0 * kWBytes, id_mlp, true);
-      issue_mlp(R1, R0 + BS / 2, aW + 1 * kWBytes, id_mlp | kIdescNegB, false);
-      issue_mlp(R1 + BS, R0, aW + 1 * kWBytes, id_mlp, true);
-      issue_mlp(R1 + BS, R0 + BS / 2, aW + 0 * kWBytes, id_mlp, false);
-      mma_commit(&mbar);
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
-    tc_fence_after();
-    uint32_t m1[3], m2[3];
-    {
-      uint32_t v[3][32], pk[3][16];
-      ld_half(R1, th, v);
-      block_tmem_sync();
-#pragma unroll
-      for (int k = 0; k < 3; ++k) {
+      for (int c = 0; c < 3; ++c) {
+        uint32_t v[32], pk[16];
+        tmem_ld32(R1 + lane_base + 32 * c, v);
+        tmem_wait_ld();
         uint32_t bits = 0;
 #pragma unroll
-        for (int q = 0; q < 16; ++q) {
-          const float a = __uint_as_float(v[k][2 * q]) + bias1[32 * k + 2 * q];
-          const float b = __uint_as_float(v[k][2 * q + 1]) + bias1[32 * k + 2 * q + 1];
-          bits |= (a > 0.f ? 1u : 0u) << (2 * q);
-          bits |= (b > 0.f ? 1u : 0u) << (2 * q + 1);
-          pk[k][q] = pack_bf16(fmaxf(a, 0.f), fmaxf(b, 0.f));
+        for (int q = 0; q < 8; ++q) {
+          const float4 bq = __ldg((const float4*)(bias1 + 32 * c + 4 * q));
+          const float a0 = __uint_as_float(v[4 * q]) + bq.x, a1 = __uint_as_float(v[4 * q + 1]) + bq.y;
+          const float a2 = __uint_as_float(v[4 * q + 2]) + bq.z, a3 = __uint_as_float(v[4 * q + 3]) + bq.w;
+          if (BACKWARD)
+            bits |= ((a0 > 0.f ? 1u : 0u) | (a1 > 0.f ? 2u : 0u) | (a2 > 0.f ? 4u : 0u) | (a3 > 0.f ? 8u : 0u)) << (4 * q);
+          pk[2 * q] = pack_bf16(fmaxf(a0, 0.f), fmaxf(a1, 0.f));
+          pk[2 * q + 1] = pack_bf16(fmaxf(a2, 0.f), fmaxf(a3, 0.f));
         }
-        m1[k] = bits;
+        m1[c] = bits;
+        tmem_st16(R1 + lane_base + 16 * c, pk);
+        if (BACKWARD && row_valid) store16(p.O1 + row_off + 32 * c, pk);
+        publish_chunk(&bars.cready[half][c]);
       }
-      st_half_packed(R1, th, pk);
-      if (row_valid) store_row_half(p.O1 + row_off, pk);
-      tmem_wait_st();
-    }
-    block_tmem_sync();
-    // ---- P2 = O1 W2 + b2 ; mask2 ----------------------------------------------------------------
-    if (tid == 0) {
-      issue_mlp(R0, R1, aW + 2 * kWBytes, id_mlp, true);
-      issue_mlp(R0, R1 + BS / 2, aW + 3 * kWBytes, id_mlp | kIdescNegB, false);
-      issue_mlp(R0 + BS, R1, aW + 3 * kWBytes, id_mlp, true);
-      issue_mlp(R0 + BS, R1 + BS / 2, aW + 2 * kWBytes, id_mlp, false);
-      mma_commit(&mbar);
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
-    tc_fence_after();
-    {
-      uint32_t v[3][32];
-      ld_half(R0, th, v);
+      // ---- stage 2 -> P2 + b2 : forward Z = softshrink -> smem tile ; backward mask2 ----
+      mbar_wait(&bars.dfull[2], tp);
+      tc_fence_after();
+      uint8_t* ztile = (i & 1) ? sTileB : sTileA;
 #pragma unroll
-      for (int k = 0; k < 3; ++k) {
+      for (int c = 0; c < 3; ++c) {
+        uint32_t v[32], pk[16];
+        tmem_ld32(R0 + lane_base + 32 * c, v);
+        tmem_wait_ld();
         uint32_t bits = 0;
 #pragma unroll
-        for (int q = 0; q < 32; ++q)
-          bits |= (fabsf(__uint_as_float(v[k][q]) + bias2[32 * k + q]) > p.lambda ? 1u : 0u) << q;
-        m2[k] = row_kept ? bits : 0u;
-      }
-    }
-    block_tmem_sync();
-    // ---- G = Fh A1g ; G2 = G (.) mask2 -----------------------------------------------------------
-    if (tid == 0) {
-      issue_dft(R1, aCh, aTileG, id_dft, true);
-      issue_dft(R1, aSh, aTileG + half, id_dft, false);
-      issue_dft(R1 + BS, aCh, aTileG + half, id_dft, true);
-      issue_dft(R1 + BS, aSh, aTileG, id_dft | kIdescNegA, false);
-      mma_commit(&mbar);
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
-    tc_fence_after();
-    {
-      uint32_t v[3][32], pk[3][16];
-      ld_half(R1, th, v);
-      block_tmem_sync();
+        for (int q = 0; q < 8; ++q) {
+          const float4 bq = __ldg((const float4*)(bias2 + 32 * c + 4 * q));
+          float a[4] = {__uint_as_float(v[4 * q]) + bq.x, __uint_as_float(v[4 * q + 1]) + bq.y,
+                        __uint_as_float(v[4 * q + 2]) + bq.z, __uint_as_float(v[4 * q + 3]) + bq.w};
 #pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        const uint32_t bits = m2[k];
-#pragma unroll
-        for (int q = 0; q < 16; ++q) {
-          const float a = (bits >> (2 * q)) & 1u ? __uint_as_float(v[k][2 * q]) : 0.f;
-          const float b = (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[k][2 * q + 1]) : 0.f;
-          pk[k][q] = pack_bf16(a, b);
+          for (int e = 0; e < 4; ++e) {
+            const float m = fabsf(a[e]) - p.lambda;
+            const bool on = row_kept && m > 0.f;
+            if (BACKWARD) bits |= (on ? 1u : 0u) << (4 * q + e);
+            a[e] = on ? copysignf(m, a[e]) : 0.f;
+          }
+          pk[2 * q] = pack_bf16(a[0], a[1]);
+          pk[2 * q + 1] = pack_bf16(a[2], a[3]);
         }
+        m2[c] = bits;
+        if (!BACKWARD && r < HP) store_tile16(ztile, half, c, r, pk);
       }
-      st_half_packed(R1, th, pk);
-      if (row_valid) store_row_half(p.G2 + row_off, pk);
-      tmem_wait_st();
-    }
-    block_tmem_sync();
-    // ---- G1 = mask1 (.) (G2 W2^H):  re = G2r W2r^T + G2i W2i^T ; im = G2i W2r^T - G2r W2i^T ----
-    if (tid == 0) {
-      issue_mlp_t(R0, R1, aW + 2 * kWBytes, id_mlp_t, true);
-      issue_mlp_t(R0, R1 + BS / 2, aW + 3 * kWBytes, id_mlp_t, false);
-      issue_mlp_t(R0 + BS, R1 + BS / 2, aW + 2 * kWBytes, id_mlp_t, true);
-      issue_mlp_t(R0 + BS, R1, aW + 3 * kWBytes, id_mlp_t | kIdescNegB, false);
-      mma_commit(&mbar);
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
-    tc_fence_after();
-    {
-      uint32_t v[3][32], pk[3][16];
-      ld_half(R0, th, v);
-      block_tmem_sync();
+      if (!BACKWARD) {
+        fence_async_smem();
+        tc_fence_before();
+        mbar_arrive(&bars.zready);
+        // ---- stage 3 -> A2 rows ----
+        mbar_wait(&bars.dfull[3], tp);
+        tc_fence_after();
 #pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        const uint32_t bits = m1[k];
-#pragma unroll
-        for (int q = 0; q < 16; ++q) {
-          const float a = (bits >> (2 * q)) & 1u ? __uint_as_float(v[k][2 * q]) : 0.f;
-          const float b = (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[k][2 * q + 1]) : 0.f;
-          pk[k][q] = pack_bf16(a, b);
+        for (int c = 0; c < 3; ++c) {
+          uint32_t v[32], pk[16];
+          tmem_ld32(R1 + lane_base + 32 * c, v);
+          tmem_wait_ld();
+          pack32(v, pk);
+          if (row_valid) store16(p.A2 + row_off + 32 * c, pk);
         }
-      }
-      st_half_packed(R0, th, pk);
-      if (row_valid) store_row_half(p.G1 + row_off, pk);
-      tmem_wait_st();
-    }
-    block_tmem_sync();
-    // ---- GX = G1 W1^H ----------------------------------------------------------------------------
-    if (tid == 0) {
-      issue_mlp_t(R1, R0, aW + 0 * kWBytes, id_mlp_t, true);
-      issue_mlp_t(R1, R0 + BS / 2, aW + 1 * kWBytes, id_mlp_t, false);
-      issue_mlp_t(R1 + BS, R0 + BS / 2, aW + 0 * kWBytes, id_mlp_t, true);
-      issue_mlp_t(R1 + BS, R0, aW + 1 * kWBytes, id_mlp_t | kIdescNegB, false);
-      mma_commit(&mbar);
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
-    tc_fence_after();
-    {
-      uint32_t v[3][32], pk[3][16];
-      ld_half(R1, th, v);
+        tc_fence_before();
+      } else {
+        // ---- stage 3 -> G2 = G (.) mask2, packed in place (R1) ----
+        mbar_wait(&bars.dfull[3], tp);
+        tc_fence_after();
 #pragma unroll
-      for (int k = 0; k < 3; ++k)
+        for (int c = 0; c < 3; ++c) {
+          uint32_t v[32], pk[16];
+          tmem_ld32(R1 + lane_base + 32 * c, v);
+          tmem_wait_ld();
+          const uint32_t bits = m2[c];
 #pragma unroll
-        for (int q = 0; q < 16; ++q)
-          pk[k][q] = row_valid ? pack_bf16(__uint_as_float(v[k][2 * q]), __uint_as_float(v[k][2 * q + 1])) : 0u;
-      if (r < HP) store_tile_half(sTile, th, pk);
-    }
-    fence_async_smem();
-    block_tmem_sync();
-    // ---- A2 = Fh^H GX (inverse kernel) ---------------------------------------------------------
-    if (tid == 0) {
-      issue_dft(R0, aCh, aTile, id_dft, true);
-      issue_dft(R0, aSh, aTile + half, id_dft | kIdescNegA, false);
-      issue_dft(R0 + BS, aCh, aTile + half, id_dft, true);
-      issue_dft(R0 + BS, aSh, aTile, id_dft, false);
-      mma_commit(&mbar);
-    }
-    // optional mask export (test aid) while the tensor core works: bytes (re, im) interleaved per channel
-    if (p.mask1 != nullptr && row_valid) {
-      const int b = rem / p.Kw, kw = rem - b * p.Kw;
-      const size_t base = ((((size_t)b * p.H + r) * p.Wh + kw) * (size_t)(p.nb * BS) + (size_t)j * BS) * 2 + th.colh;
+          for (int q = 0; q < 16; ++q)
+            pk[q] = pack_bf16((bits >> (2 * q)) & 1u ? __uint_as_float(v[2 * q]) : 0.f,
+                              (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[2 * q + 1]) : 0.f);
+          tmem_st16(R1 + lane_base + 16 * c, pk);
+          if (row_valid) store16(p.G2 + row_off + 32 * c, pk);
+          publish_chunk(&bars.cready[half][c]);
+        }
+        // ---- stage 4 -> G1 = mask1 (.) (G2 W2^H), packed in place (R0) ----
+        mbar_wait(&bars.dfull[4], tp);
+        tc_fence_after();
 #pragma unroll
-      for (int k = 0; k < 3; ++k)
+        for (int c = 0; c < 3; ++c) {
+          uint32_t v[32], pk[16];
+          tmem_ld32(R0 + lane_base + 32 * c, v);
+          tmem_wait_ld();
+          const uint32_t bits = m1[c];
+#pragma unroll
+          for (int q = 0; q < 16; ++q)
+            pk[q] = pack_bf16((bits >> (2 * q)) & 1u ? __uint_as_float(v[2 * q]) : 0.f,
+                              (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[2 * q + 1]) : 0.f);
+          tmem_st16(R0 + lane_base + 16 * c, pk);
+          if (row_valid) store16(p.G1 + row_off + 32 * c, pk);
+          publish_chunk(&bars.cready[half][c]);
+        }
+        // ---- stage 5 -> GX as the B operand of the inverse transform (gradient tile buffer) ----
+        mbar_wait(&bars.dfull[5], tp);
+        tc_fence_after();
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          uint32_t v[32], pk[16];
+          tmem_ld32(R1 + lane_base + 32 * c, v);
+          tmem_wait_ld();
+#pragma unroll
+          for (int q = 0; q < 16; ++q)
+            pk[q] = row_valid ? pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1])) : 0u;
+          if (r < HP) store_tile16(sTileB, half, c, r, pk);
+        }
+        fence_async_smem();
+        tc_fence_before();
+        mbar_arrive(&bars.zready);
+        // optional mask export (test aid): bytes (re, im) interleaved per channel
+        if (EXPORT && row_valid) {
+          const int b = rem / p.Kw, kw = rem - b * p.Kw;
+          const size_t base = ((((size_t)b * p.H + r) * p.Wh + kw) * (size_t)(p.nb * BS) + (size_t)j * BS) * 2 + half;
+#pragma unroll
+          for (int c = 0; c < 3; ++c)
 #pragma unroll 4
-        for (int q = 0; q < 32; ++q) {
-          p.mask1[base + (size_t)(32 * k + q) * 2] = (uint8_t)((m1[k] >> q) & 1u);
-          p.mask2[base + (size_t)(32 * k + q) * 2] = (uint8_t)((m2[k] >> q) & 1u);
+            for (int q = 0; q < 32; ++q) {
+              p.mask1[base + (size_t)(32 * c + q) * 2] = (uint8_t)((m1[c] >> q) & 1u);
+              p.mask2[base + (size_t)(32 * c + q) * 2] = (uint8_t)((m2[c] >> q) & 1u);
+            }
         }
-    }
-    mbar_wait(&mbar, phase);
-    phase ^= 1;
-    tc_fence_after();
-    {
-      uint32_t v[3][32], pk[3][16];
-      ld_half(R0, th, v);
+        // ---- stage 6 -> A2 rows ----
+        mbar_wait(&bars.dfull[6], tp);
+        tc_fence_after();
 #pragma unroll
-      for (int k = 0; k < 3; ++k)
-#pragma unroll
-        for (int q = 0; q < 16; ++q) pk[k][q] = pack_bf16(__uint_as_float(v[k][2 * q]), __uint_as_float(v[k][2 * q + 1]));
-      if (row_valid) store_row_half(p.A2 + row_off, pk);
+        for (int c = 0; c < 3; ++c) {
+          uint32_t v[32], pk[16];
+          tmem_ld32(R1 + lane_base + 32 * c, v);
+          tmem_wait_ld();
+          pack32(v, pk);
+          if (row_valid) store16(p.A2 + row_off + 32 * c, pk);
+        }
+        tc_fence_before();
+      }
     }
   }
   tc_fence_before();
   __syncthreads();
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
-
 
 // ---- B4 / B6: parameter gradients as a split-K tensor-core GEMM ------------------------------------
 // For block j:  R[(ri_a,i), (ri_g,o)] = sum_rows A[row,(ri_a,i)] * G[row,(ri_g,o)] with K = mode rows.
@@ -979,6 +876,7 @@ cudaError_t set_smem(K kernel, size_t bytes) {
 
 struct TcWs {
   __nv_bfloat16 *A1, *A2, *wprep;
+  float* bprep;
   __nv_bfloat16 *A1g, *Xh, *O1, *G2, *G1; // backward only
   float* part;
   uint8_t *mask1, *mask2;
@@ -1003,7 +901,8 @@ TcWs tc_carve(const Geometry& g, bool backward, char* base) {
   const size_t spec = (size_t)g.B * g.Kw * g.nb * g.H * NT * 2;
   w.A1 = (__nv_bfloat16*)take(spec);
   w.A2 = (__nv_bfloat16*)take(spec);
-  w.wprep = (__nv_bfloat16*)take((size_t)g.nb * 8 * kWBytes);
+  w.wprep = (__nv_bfloat16*)take((size_t)g.nb * 4 * kWBytes);
+  w.bprep = (float*)take((size_t)g.nb * 2 * NT * sizeof(float));
   if (backward) {
     w.A1g = (__nv_bfloat16*)take(spec);
     w.Xh = (__nv_bfloat16*)take(spec);
@@ -1063,8 +962,9 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
   if (e == cudaSuccess) e = upload(gw1, &out->gw_noalpha);
   if (e == cudaSuccess) e = set_smem(tc_wdft<false>, kRowSmem);
   if (e == cudaSuccess) e = set_smem(tc_wdft<true>, kRowSmem);
-  if (e == cudaSuccess) e = set_smem(tc_mix_fwd, kMixFwdSmem);
-  if (e == cudaSuccess) e = set_smem(tc_mix_bwd, kMixBwdSmem);
+  if (e == cudaSuccess) e = set_smem(tc_mix<false, false>, kMixSmem2);
+  if (e == cudaSuccess) e = set_smem(tc_mix<true, false>, kMixSmem2);
+  if (e == cudaSuccess) e = set_smem(tc_mix<true, true>, kMixSmem2);
   if (e == cudaSuccess) e = set_smem(tc_wgrad, kWgSmem);
   int dev = 0, sms = 148;
   if (e == cudaSuccess) e = cudaGetDevice(&dev);
@@ -1085,7 +985,7 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   cudaError_t e;
   const int nW = g.nb * BS * BS;
   prof_begin("k_tc_prep_weights", st);
-  k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, w2, w.wprep, g.nb);
+  k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, w.wprep, w.bprep, g.nb);
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -1098,11 +998,13 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  MixParams mp{w.A1, w.A2, tp.dft, (const uint8_t*)w.wprep, b1, b2, g.B, g.H, g.Kw, g.nb, g.Kh, g.lambda};
+  MixParams mp{};
+  mp.A1 = w.A1; mp.A2 = w.A2; mp.dft = tp.dft; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
+  mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
   const int mix_tiles = g.nb * g.B * g.Kw;
   const int grid_mix = mix_tiles < tp.num_sms ? mix_tiles : tp.num_sms;
   prof_begin("tc_mix_fwd", st);
-  tc_mix_fwd<<<grid_mix, kMixThreads, kMixFwdSmem, st>>>(mp);
+  tc_mix<false, false><<<grid_mix, kMixThreads, kMixSmem2, st>>>(mp);
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -1130,7 +1032,7 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   if (g.export_masks) {
     if ((e = cudaMemsetAsync(ws, 0, w.mask_region, st)) != cudaSuccess) return e;
   }
-  TC_LAUNCH("k_tc_prep_weights", k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, w2, w.wprep, g.nb));
+  TC_LAUNCH("k_tc_prep_weights", k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, w.wprep, w.bprep, g.nb));
   const int ncg = (g.C + CGRP - 1) / CGRP;
   const int row_tiles = g.B * g.H * ncg;
   const int grid_row = row_tiles < tp.num_sms ? row_tiles : tp.num_sms;
@@ -1139,16 +1041,20 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
                                                                                   tp.fw, g.B, g.H, g.W, g.C, g.Kw, g.nb));
   TC_LAUNCH("tc_wdft_fwd", tc_wdft<false><<<grid_row, kRowThreads, kRowSmem, st>>>((const __nv_bfloat16*)dy, nullptr, w.A1g,
                                                                                   tp.fw_alpha, g.B, g.H, g.W, g.C, g.Kw, g.nb));
-  MixBwdParams mp{};
-  mp.A1x = w.A1; mp.A1g = w.A1g; mp.A2 = w.A2;
+  MixParams mp{};
+  mp.A1 = w.A1; mp.A1g = w.A1g; mp.A2 = w.A2;
   mp.Xh = w.Xh; mp.O1 = w.O1; mp.G2 = w.G2; mp.G1 = w.G1;
-  mp.dft = tp.dft; mp.wprep = (const uint8_t*)w.wprep; mp.b1 = b1; mp.b2 = b2;
+  mp.dft = tp.dft; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
   mp.mask1 = g.export_masks ? w.mask1 : nullptr;
   mp.mask2 = g.export_masks ? w.mask2 : nullptr;
   mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
   const int mix_tiles = g.nb * g.B * g.Kw;
   const int grid_mix = mix_tiles < tp.num_sms ? mix_tiles : tp.num_sms;
-  TC_LAUNCH("tc_mix_bwd", tc_mix_bwd<<<grid_mix, kMixThreads, kMixBwdSmem, st>>>(mp));
+  if (g.export_masks) {
+    TC_LAUNCH("tc_mix_bwd", tc_mix<true, true><<<grid_mix, kMixThreads, kMixSmem2, st>>>(mp));
+  } else {
+    TC_LAUNCH("tc_mix_bwd", tc_mix<true, false><<<grid_mix, kMixThreads, kMixSmem2, st>>>(mp));
+  }
   // B4 / B6: parameter gradients
   const int nred = nW + g.nb * BS;
   TC_LAUNCH("tc_wgrad", tc_wgrad<<<g.nb * w.S, 128, kWgSmem, st>>>(w.O1, w.G2, w.part, g.B * g.Kw, g.H, g.nb, w.S));

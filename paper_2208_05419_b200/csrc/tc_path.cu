@@ -370,9 +370,14 @@ __device__ __forceinline__ void pack32(const uint32_t (&v)[32], uint32_t (&pk)[1
 #pragma unroll
   for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
 }
+// 64 bytes of a row as two 256-bit stores (full 32-byte sectors; dst is 32-byte aligned)
 __device__ __forceinline__ void store16(__nv_bfloat16* dst, const uint32_t (&pk)[16]) {
 #pragma unroll
-  for (int g = 0; g < 4; ++g) *(uint4*)(dst + g * 8) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
+  for (int g = 0; g < 2; ++g)
+    asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(dst + g * 16), "r"(pk[8 * g]),
+                 "r"(pk[8 * g + 1]), "r"(pk[8 * g + 2]), "r"(pk[8 * g + 3]), "r"(pk[8 * g + 4]), "r"(pk[8 * g + 5]),
+                 "r"(pk[8 * g + 6]), "r"(pk[8 * g + 7])
+                 : "memory");
 }
 // chunk c of this thread's row -> MN-major B operand tile (K = row r)
 __device__ __forceinline__ void store_tile16(uint8_t* tile, int half, int c, int r, const uint32_t (&pk)[16]) {

@@ -39,19 +39,20 @@ constexpr uint32_t kDftLbo = 2048, kDftSbo = 128;   // Ch / Sh: K-major A [128 x
 constexpr uint32_t kDftBytes = 128 * HP * 2;         // 24576
 constexpr uint32_t kWLbo = 1536, kWSbo = 128;       // weights: K-major B [96 x 96], order [k/8][n/8]
 constexpr uint32_t kWBytes = BS * BS * 2;            // 18432
-constexpr uint32_t kTileLbo = 128, kTileSbo = 1536; // mode tile: MN-major B [K=96 rows][N=192]
-constexpr uint32_t kTileBytes = HP * NT * 2;         // 36864
-constexpr uint32_t kFwLbo = 3072, kFwSbo = 128;     // Fw^T / Gw^T: K-major B [192 x 192]
-constexpr uint32_t kFwBytes = WP * NT * 2;           // 73728
-constexpr uint32_t kRowLbo = 128, kRowSbo = 3072;   // W-direction data tile: MN-major A [K=192][M=128]
-constexpr uint32_t kRowBytes = WP * CGRP * 2;        // 49152
+// mode tile: MN-major B [K=96 rows][N=192]; the 16-byte pad on the chunk stride keeps cp.async
+// writes of consecutive chunks of one row (the coalesced global order) bank-conflict-free
+constexpr uint32_t kTileLbo = 128, kTileSbo = 1536 + 16;
+constexpr uint32_t kTileBytes = (NT / 8) * kTileSbo; // 37248
+constexpr uint32_t kFwLbo = 2048, kFwSbo = 128;     // Fw / Gw halves: K-major A [128 x 192], order [k/8][m/8]
+constexpr uint32_t kFwHalf = 128 * WP * 2;           // 49152 per 128-row half
+constexpr uint32_t kFwBytes = 2 * kFwHalf;           // 98304
+constexpr uint32_t kRowLbo = 128, kRowSbo = 3072 + 16; // W-direction data tile: MN-major B [K=192][N=128], padded
+constexpr uint32_t kRowBytes = (CGRP / 8) * kRowSbo; // 49408
 
-constexpr uint32_t kMixSmem = 2 * kDftBytes + 4 * kWBytes + kTileBytes + 2 * NT * 4; // 161280
-constexpr int kTrPitch = 132;                        // fp32 words per row of the epilogue transpose buffer
-constexpr uint32_t kTrBytes = 32 * kTrPitch * 4;     // 16896
 constexpr int kRowEpiThreads = 256;                 // 8 epilogue warps
-constexpr int kRowThreads = kRowEpiThreads + 64;     // + 2 producer / MMA warps
-constexpr uint32_t kRowSmem = kFwBytes + 2 * kRowBytes + 2 * kTrBytes;               // 205824
+constexpr int kRowProdWarps = 4;                     // producer warps per operand buffer
+constexpr int kRowThreads = kRowEpiThreads + 2 * kRowProdWarps * 32;
+constexpr uint32_t kRowSmem = kFwBytes + 2 * kRowBytes;                              // 196608
 
 // ---- weight preparation: fp32 [nb][96][96][2] -> bf16 K-major interleaved operands --------------
 // per block 4 matrices of kWBytes {W1r, W1i, W2r, W2i} with element (n=o, k=i) = W[i][o] (the
@@ -83,24 +84,42 @@ __global__ void k_tc_prep_weights(const float* __restrict__ w1, const float* __r
 }
 
 // ---- F1 / B2 and F8 + F9 / B8: the W-direction transforms as GEMMs -------------------------------
-// One tile = (b, h, 128 channels): D[c, n] = sum_k A[k, c] * Bconst[k, n], 12 UMMAs of 128x192x16.
-//   forward (INVERSE = false): k = w, A = x^T slab, n = (ri, kw); D -> A1[b][kw][j][h][ri][96]
-//   inverse (INVERSE = true) : k = (ri, kw), A gathered from A2, n = w; D + residual -> y
-// Software pipeline per CTA (persistent over tiles): the operand tile of iteration i+2 is copied
-// (cp.async) while the tensor core works on tile i+1 (second TMEM accumulator) and all 8 warps
-// run the epilogue of tile i.
+// One tile = (b, h, 128 channels).  The constant DFT matrix is the A operand (accumulator
+// rows = output index), the activation tile the MN-major B operand (columns = channels):
+//   forward (INVERSE = false): D_ri[kw, c] = sum_w  Fw_ri[kw, w] * x[b,h,w,c]      ri = re, im
+//   inverse (INVERSE = true) : D_a[w, c]   = sum_(ri,kw) Gw[w, (ri,kw)] * A2[..]    a = w / 128
+// so every thread's accumulator row is 128 CONTIGUOUS channels of one output row and the
+// epilogue is plain 32-byte vector I/O (no transpose).  Two 128x128x192 GEMMs per tile.
+// Warp-specialised and persistent: producer warp p copies tiles it = p, p+2, .. (cp.async)
+// into operand buffer p and issues their MMAs into accumulator pair p; the 8 epilogue warps
+// (accumulator a = warp/4, TMEM lanes 32*(warp%4)..) drain tile it while tile it+1 computes.
+__device__ __forceinline__ void pack32(const uint32_t (&v)[32], uint32_t (&pk)[16]) {
+#pragma unroll
+  for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
+}
+__device__ __forceinline__ void ldg256(const void* p, uint32_t (&r)[8]) {
+  asm volatile("ld.global.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "l"(p));
+}
+__device__ __forceinline__ void stg256(void* p, const uint32_t* r) {
+  asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]),
+               "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+               : "memory");
+}
+
 template <bool INVERSE>
 __global__ void __launch_bounds__(kRowThreads, 1)
 tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ res, __nv_bfloat16* __restrict__ out,
-        const uint8_t* __restrict__ Bconst, int B, int H, int W, int C, int Kw, int nb) {
+        const uint8_t* __restrict__ Aconst, int B, int H, int W, int C, int Kw, int nb) {
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ __align__(8) uint64_t full[2], empty[2];
   __shared__ uint32_t tmem_slot;
   uint8_t* sF = smem;
-  uint8_t* sA0 = smem + kFwBytes;
+  uint8_t* sB0 = smem + kFwBytes;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (uint32_t i = tid; i < 2 * kRowBytes / 16; i += kRowThreads) ((uint4*)sA0)[i] = make_uint4(0, 0, 0, 0);
-  for (uint32_t i = tid; i < kFwBytes / 16; i += kRowThreads) cp_async16(smem_u32(sF) + i * 16, Bconst + (size_t)i * 16);
+  for (uint32_t i = tid; i < 2 * kRowBytes / 16; i += kRowThreads) ((uint4*)sB0)[i] = make_uint4(0, 0, 0, 0);
+  for (uint32_t i = tid; i < kFwBytes / 16; i += kRowThreads) cp_async16(smem_u32(sF) + i * 16, Aconst + (size_t)i * 16);
   if (tid == 0) {
     mbar_init(&full[0], 1);
     mbar_init(&full[1], 1);
@@ -120,148 +139,126 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
   if (warp >= kRowEpiThreads / 32) {
-    // ===== producer warp p: tiles it = p, p+2, ... -> operand buffer p, accumulator p ================
-    const int p = warp - kRowEpiThreads / 32;
-    const uint32_t dst = smem_u32(sA0) + p * kRowBytes;
-    const uint32_t idesc = idesc_bf16(128, NT, kIdescAMn);
+    // ===== producer group p (4 warps): tiles it = p, p+2, ... -> operand buffer p, accumulator pair p ==
+    // (a single warp sustains only ~1 cp.async instruction per 200 cycles, so the copy is spread)
+    const int pw = warp - kRowEpiThreads / 32;
+    const int p = pw / kRowProdWarps, sub = pw % kRowProdWarps;
+    const uint32_t dst = smem_u32(sB0) + p * kRowBytes;
+    const uint32_t idesc = idesc_bf16(128, CGRP, kIdescBMn);
     const int hl = lane & 7, cl4 = lane >> 3;
     for (int it = p; it < nmine; it += 2) {
       const int use = it >> 1;
-      // the previous MMA on this buffer has completed (its commit also frees the operand tile)
+      // the previous MMAs on this buffer have completed (their commit also frees the operand tile)
       if (use > 0) mbar_wait(&full[p], (uint32_t)((use - 1) & 1));
       const int t = blockIdx.x + it * gridDim.x;
       const int cg = t % ncg, bh = t / ncg;
       if (!INVERSE) {
-        // x[b,h,:,cg*128 .. +128) -> MN-major A operand (K = w, M = channel)
+        // x[b,h,:,cg*128 .. +128) -> MN-major B operand (K = w, N = channel).  One cp.async
+        // instruction = 2 rows x 16 consecutive 16-byte chunks: full sectors on the global side
         const __nv_bfloat16* xrow = in + (size_t)bh * W * C + cg * CGRP;
-        const int nunits = ((W + 7) / 8) * 4;
-        for (int u = 0; u < nunits; ++u) {
-          const int w = (u >> 2) * 8 + hl;
-          const int mc = (u & 3) * 4 + cl4;
-          if (w < W && cg * CGRP + mc * 8 < C) cp_async16(dst + mc * kRowSbo + w * 16, xrow + (size_t)w * C + mc * 8);
-        }
+        const int mc = lane & 15;
+        const bool cok = cg * CGRP + mc * 8 < C;
+        for (int w = 2 * sub + (lane >> 4); w < W; w += 2 * kRowProdWarps)
+          if (cok) cp_async16(dst + mc * kRowSbo + w * 16, xrow + (size_t)w * C + mc * 8);
       } else {
-        // A2[b][kw][j][h][ri][cl] gathered into the MN-major A operand (K = (ri,kw), M = channel)
+        // A2[b][kw][j][h][ri][cl] gathered into the MN-major B operand (K = (ri,kw), N = channel)
         const int b = bh / H, h = bh - b * H;
-        const int kwg = (Kw + 7) / 8;
         const size_t kwstride = (size_t)nb * H * NT;
         const __nv_bfloat16* base = in + ((size_t)b * Kw * nb * H + h) * NT;
-        for (int u = 0; u < 2 * kwg * 4; ++u) {
-          const int rg = u >> 2;
-          const int ri = rg >= kwg ? 1 : 0, kw = (rg - ri * kwg) * 8 + hl;
-          const int mc = (u & 3) * 4 + cl4;
-          const int c0 = cg * CGRP + mc * 8;
-          if (kw < Kw && c0 < C) {
-            const int j = c0 / BS, cl = c0 - j * BS;
-            cp_async16(dst + mc * kRowSbo + (ri * BS + kw) * 16,
-                       base + (size_t)kw * kwstride + (size_t)j * H * NT + ri * BS + cl);
-          }
+        const int mc = lane & 15;
+        const int c0 = cg * CGRP + mc * 8;
+        const int j = c0 / BS, cl = c0 - j * BS;
+        const __nv_bfloat16* cbase = base + (size_t)j * H * NT + cl;
+        for (int rr = 2 * sub + (lane >> 4); rr < 2 * Kw; rr += 2 * kRowProdWarps) {
+          const int ri = rr >= Kw ? 1 : 0, kw = rr - ri * Kw;
+          if (c0 < C) cp_async16(dst + mc * kRowSbo + (ri * BS + kw) * 16, cbase + (size_t)kw * kwstride + ri * BS);
         }
       }
       cp_async_wait_all();
       fence_async_smem();
-      __syncwarp();
-      if (lane == 0) {
-        // the epilogue has drained this accumulator's previous contents
+      asm volatile("bar.sync %0, %1;" ::"r"(1 + p), "n"(kRowProdWarps * 32) : "memory");
+      if (sub == 0 && lane == 0) {
+        // the epilogue has drained this accumulator pair's previous contents
         if (use > 0) mbar_wait(&empty[p], (uint32_t)((use - 1) & 1));
         tc_fence_after();
-        const uint32_t d = tmem + p * 256;
 #pragma unroll
-        for (int ks = 0; ks < WP / 16; ++ks)
-          mma_ss(d, smem_desc(dst + ks * 2 * kRowLbo, kRowLbo, kRowSbo),
-                 smem_desc(smem_u32(sF) + ks * 2 * kFwLbo, kFwLbo, kFwSbo), idesc, ks > 0);
+        for (int a = 0; a < 2; ++a) {
+          const uint32_t d = tmem + p * 256 + a * CGRP;
+          const uint32_t am = smem_u32(sF) + a * kFwHalf;
+#pragma unroll
+          for (int ks = 0; ks < WP / 16; ++ks)
+            mma_ss(d, smem_desc(am + ks * 2 * kFwLbo, kFwLbo, kFwSbo), smem_desc(dst + ks * 2 * kRowLbo, kRowLbo, kRowSbo),
+                   idesc, ks > 0);
+        }
         mma_commit(&full[p]);
       }
       __syncwarp();
     }
   } else {
-    // ===== epilogue warps: group grp = column half, lanes = channels =============================
-    const int grp = warp >> 2, tg = tid & 127;
-    float* sT = (float*)(smem + kFwBytes + 2 * kRowBytes + grp * kTrBytes);
-    uint32_t* sTu = (uint32_t*)sT;
+    // ===== epilogue warps: accumulator a = warp / 4, row m = 32 * (warp % 4) + lane ====================
+    const int a = warp >> 2;
+    const int m = (warp & 3) * 32 + lane;
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
-    const int c4 = (tg & 31) * 4;       // this thread's 4 channels after the transpose
-    const int wq = tg >> 5;             // warp inside the group: column (pair) phase
     for (int it = 0; it < nmine; ++it) {
       const int t = blockIdx.x + it * gridDim.x;
       const int cg = t % ncg, bh = t / ncg;
-      const int c = cg * CGRP + c4;
-      const bool cvalid = c < C;
+      // forward: row = frequency kw of part ri = a ; inverse: row = w = 128 a + m
+      const int row = INVERSE ? a * 128 + m : m;
+      const bool rvalid = INVERSE ? (row < W) : (row < Kw);
+      const bool warp_has_rows = INVERSE ? (a * 128 + (warp & 3) * 32 < W) : ((warp & 3) * 32 < Kw);
+      const int b = bh / H, h = bh - b * H;
       mbar_wait(&full[it & 1], (uint32_t)((it >> 1) & 1));
       tc_fence_after();
-      const uint32_t acc = tmem + (it & 1) * 256 + lane_base + grp * BS;
-      if (!INVERSE) {
-        // A1[b][kw][j][h][ri][cl]: per thread the address is base + kw * stride
-        const int b = bh / H, h = bh - b * H;
-        const int j = c / BS, cl = c - j * BS;
-        const size_t kwstride = (size_t)nb * H * NT;
-        __nv_bfloat16* obase = out + (((size_t)b * Kw * nb + j) * H + h) * NT + grp * BS + cl;
+      const uint32_t acc = tmem + (it & 1) * 256 + a * CGRP + lane_base;
+      if (warp_has_rows) {
 #pragma unroll 1
-        for (int k = 0; k < 3; ++k) {
-          uint32_t v[32];
+        for (int k = 0; k < 4; ++k) {
+          const int c = cg * CGRP + 32 * k;   // 32 channels of one block (96 = 3 * 32)
+          uint32_t v[32], pk[16];
           tmem_ld32(acc + 32 * k, v);
-          tmem_wait_ld();
-          if (k == 2) {
-            tc_fence_before();
-            mbar_arrive(&empty[it & 1]);
-          }
-          // column pairs (2q, 2q+1) of this channel packed to bf16x2, transposed through smem
+          if (!INVERSE) {
+            tmem_wait_ld();
+            if (k == 3) {
+              tc_fence_before();
+              mbar_arrive(&empty[it & 1]);
+            }
+            pack32(v, pk);
+            if (rvalid && c < C) {
+              const int j = c / BS, cl = c - j * BS;
+              __nv_bfloat16* dstp = out + ((((size_t)b * Kw + row) * nb + j) * H + h) * NT + a * BS + cl;
+              stg256(dstp, pk);
+              stg256(dstp + 16, pk + 8);
+            }
+          } else {
+            uint32_t r0[8] = {0, 0, 0, 0, 0, 0, 0, 0}, r1[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            const size_t off = ((size_t)bh * W + row) * C + c;
+            const bool ok = rvalid && c < C;
+            if (ok && res) {
+              ldg256(res + off, r0);
+              ldg256(res + off + 16, r1);
+            }
+            tmem_wait_ld();
+            if (k == 3) {
+              tc_fence_before();
+              mbar_arrive(&empty[it & 1]);
+            }
 #pragma unroll
-          for (int q = 0; q < 16; ++q)
-            sTu[q * kTrPitch + tg] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
-          asm volatile("bar.sync %0, 128;" ::"r"(1 + grp) : "memory");
-#pragma unroll
-          for (int pass = 0; pass < 4; ++pass) {
-            const int qp = pass * 4 + wq;
-            const uint4 w4 = *(const uint4*)&sTu[qp * kTrPitch + c4];
-            const int kw0 = 32 * k + 2 * qp;
-            __nv_bfloat16* dstp = obase + (size_t)kw0 * kwstride;
-            if (cvalid && kw0 < Kw)
-              *(uint2*)dstp = make_uint2(__byte_perm(w4.x, w4.y, 0x5410), __byte_perm(w4.z, w4.w, 0x5410));
-            if (cvalid && kw0 + 1 < Kw)
-              *(uint2*)(dstp + kwstride) = make_uint2(__byte_perm(w4.x, w4.y, 0x7632), __byte_perm(w4.z, w4.w, 0x7632));
+            for (int q = 0; q < 8; ++q) {
+              // bf16 -> fp32 is a 16-bit shift; one rounding of (residual + branch)
+              pk[q] = pack_bf16(__uint_as_float(v[2 * q]) + __uint_as_float(r0[q] << 16),
+                                __uint_as_float(v[2 * q + 1]) + __uint_as_float(r0[q] & 0xFFFF0000u));
+              pk[8 + q] = pack_bf16(__uint_as_float(v[16 + 2 * q]) + __uint_as_float(r1[q] << 16),
+                                    __uint_as_float(v[16 + 2 * q + 1]) + __uint_as_float(r1[q] & 0xFFFF0000u));
+            }
+            if (ok) {
+              stg256(out + off, pk);
+              stg256(out + off + 16, pk + 8);
+            }
           }
-          asm volatile("bar.sync %0, 128;" ::"r"(1 + grp) : "memory");
         }
       } else {
-        const size_t rowoff = (size_t)bh * W * C + c;
-        const __nv_bfloat16* rbase = res ? res + rowoff : nullptr;
-        __nv_bfloat16* obase = out + rowoff;
-#pragma unroll 1
-        for (int k = 0; k < 3; ++k) {
-          const int w0 = grp * BS + 32 * k + wq;
-          uint32_t v[32];
-          tmem_ld32(acc + 32 * k, v);
-          // residual rows of this chunk (8 independent 8-byte loads in flight per thread)
-          uint2 rr[8];
-#pragma unroll
-          for (int pass = 0; pass < 8; ++pass) {
-            const int w = w0 + pass * 4;
-            rr[pass] = make_uint2(0u, 0u);
-            if (rbase && cvalid && w < W) rr[pass] = __ldg((const uint2*)(rbase + (size_t)w * C));
-          }
-          tmem_wait_ld();
-          if (k == 2) {
-            tc_fence_before();
-            mbar_arrive(&empty[it & 1]);
-          }
-#pragma unroll
-          for (int q = 0; q < 32; ++q) sTu[q * kTrPitch + tg] = v[q];
-          asm volatile("bar.sync %0, 128;" ::"r"(1 + grp) : "memory");
-#pragma unroll
-          for (int pass = 0; pass < 8; ++pass) {
-            const int q = pass * 4 + wq;
-            const float4 f = *(const float4*)&sT[q * kTrPitch + c4];
-            const int w = w0 + pass * 4;
-            const uint2 r2 = rr[pass];
-            // bf16 -> fp32 is a 16-bit shift
-            const float r0 = __uint_as_float(r2.x << 16), r1 = __uint_as_float(r2.x & 0xFFFF0000u);
-            const float r2f = __uint_as_float(r2.y << 16), r3 = __uint_as_float(r2.y & 0xFFFF0000u);
-            if (cvalid && w < W)
-              *(uint2*)(obase + (size_t)w * C) = make_uint2(pack_bf16(f.x + r0, f.y + r1), pack_bf16(f.z + r2f, f.w + r3));
-          }
-          asm volatile("bar.sync %0, 128;" ::"r"(1 + grp) : "memory");
-        }
+        tc_fence_before();
+        mbar_arrive(&empty[it & 1]);
       }
     }
   }
@@ -269,7 +266,6 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
   __syncthreads();
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
-
 
 // ---- F2-F7 / B1-B7: per (b, kw, block) GEMM chains in tensor memory --------------------------------
 // CTA = 8 epilogue warps + 1 control warp.
@@ -286,7 +282,8 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
 // Tensor memory: R0 = columns [0,192), R1 = [256,448); a stage reads its A operand from one
 // region and accumulates into the other.
 constexpr int kMixEpiThreads = 256;
-constexpr int kMixThreads = kMixEpiThreads + 64;   // + control warp + loader warp
+constexpr int kMixLoadWarps = 3;
+constexpr int kMixThreads = kMixEpiThreads + 32 + kMixLoadWarps * 32;   // + control warp + loader warps
 constexpr uint32_t kMixSmem2 = 2 * kDftBytes + 4 * kWBytes + 2 * kTileBytes; // 196608
 
 struct MixParams {
@@ -355,21 +352,16 @@ struct MixBars {
   uint64_t tfree[2];      // tile buffer consumed by its last GEMM (tcgen05.commit)
 };
 
-// rows of a (b,kw,j) tile [H][192] -> MN-major B operand (K = h, N = (ri, c)); one warp
-__device__ __forceinline__ void load_tile_warp(uint32_t tile_saddr, const __nv_bfloat16* src, int H, int lane) {
-  const int hl = lane & 7, cl4 = lane >> 3;
-  const int nunits = ((H + 7) / 8) * 6;
-  for (int u = 0; u < nunits; ++u) {
-    const int h = (u / 6) * 8 + hl;
-    const int nc = (u % 6) * 4 + cl4;
-    if (h < H) cp_async16(tile_saddr + nc * kTileSbo + h * 16, src + (size_t)h * NT + nc * 8);
+// rows of a (b,kw,j) tile [H][192] -> MN-major B operand (K = h, N = (ri, c)); loader warp `sub`
+__device__ __forceinline__ void load_tile_warp(uint32_t tile_saddr, const __nv_bfloat16* src, int H, int lane, int sub) {
+  // the tile is contiguous in global memory: chunk q = 16 bytes at src + 8 q, row h = q / 24
+  const int nchunks = H * (NT / 8);
+  for (int q = sub * 32 + lane; q < nchunks; q += kMixLoadWarps * 32) {
+    const int h = q / (NT / 8), nc = q - h * (NT / 8);
+    cp_async16(tile_saddr + nc * kTileSbo + h * 16, src + (size_t)q * 8);
   }
 }
 
-__device__ __forceinline__ void pack32(const uint32_t (&v)[32], uint32_t (&pk)[16]) {
-#pragma unroll
-  for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
-}
 // 64 bytes of a row as two 256-bit stores (full 32-byte sectors; dst is 32-byte aligned)
 __device__ __forceinline__ void store16(__nv_bfloat16* dst, const uint32_t (&pk)[16]) {
 #pragma unroll
@@ -411,7 +403,7 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
       for (int c = 0; c < 3; ++c) mbar_init(&bars.cready[h][c], kMixEpiThreads / 2);
     mbar_init(&bars.zready, kMixEpiThreads);
     for (int b = 0; b < 2; ++b) {
-      mbar_init(&bars.tfull[b], 32);
+      mbar_init(&bars.tfull[b], kMixLoadWarps * 32);
       mbar_init(&bars.tfree[b], 1);
     }
     mbar_init_fence();
@@ -429,11 +421,12 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
   const int t_begin = blockIdx.x * per, t_end = min(ntiles, t_begin + per);
   const int BKw = p.B * p.Kw;
 
-  if (warp == kMixEpiThreads / 32 + 1) {
-    // ================================ loader warp ============================================
+  if (warp >= kMixEpiThreads / 32 + 1) {
+    // ================================ loader warps ============================================
     // forward : tile i -> buffer i&1 (free once the inverse transform of tile i-2 has completed)
     // backward: x tile -> buffer A (free after stage 0), gradient tile -> buffer B (free after stage 6)
     const uint32_t aTA = smem_u32(sTileA), aTB = smem_u32(sTileB);
+    const int sub = warp - (kMixEpiThreads / 32 + 1);
     for (int t = t_begin; t < t_end; ++t) {
       const int i = t - t_begin;
       const int j = t / BKw, rem = t - j * BKw;
@@ -441,18 +434,18 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
       if (!BACKWARD) {
         const int b = i & 1, use = i >> 1;
         if (use > 0) mbar_wait(&bars.tfree[b], (uint32_t)((use - 1) & 1));
-        load_tile_warp(b ? aTB : aTA, p.A1 + off, p.H, lane);
+        load_tile_warp(b ? aTB : aTA, p.A1 + off, p.H, lane, sub);
         cp_async_wait_all();
         fence_async_smem();
         mbar_arrive(&bars.tfull[b]);
       } else {
         if (i > 0) mbar_wait(&bars.tfree[0], (uint32_t)((i - 1) & 1));
-        load_tile_warp(aTA, p.A1 + off, p.H, lane);
+        load_tile_warp(aTA, p.A1 + off, p.H, lane, sub);
         cp_async_wait_all();
         fence_async_smem();
         mbar_arrive(&bars.tfull[0]);
         if (i > 0) mbar_wait(&bars.tfree[1], (uint32_t)((i - 1) & 1));
-        load_tile_warp(aTB, p.A1g + off, p.H, lane);
+        load_tile_warp(aTB, p.A1g + off, p.H, lane, sub);
         cp_async_wait_all();
         fence_async_smem();
         mbar_arrive(&bars.tfull[1]);
@@ -730,10 +723,10 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
 // For block j:  R[(ri_a,i), (ri_g,o)] = sum_rows A[row,(ri_a,i)] * G[row,(ri_g,o)] with K = mode rows.
 // Two M=128 accumulators: D_re rows = (re, i) plus a constant-one row 96 (gives sum_rows G = db),
 // D_im rows = (im, i).  CTA (j, s) sums tiles rem = s, s+S, ... and writes its partial sums.
-constexpr uint32_t kWgABytes = HP * 128 * 2;                           // 24576: MN-major A [K=96][M=128]
+constexpr uint32_t kWgALbo = 128, kWgASbo = 1536 + 16;                  // MN-major A [K=96][M=128], padded chunk stride
+constexpr uint32_t kWgABytes = 16 * kWgASbo;                            // 24832
 constexpr uint32_t kWgStage = 2 * kWgABytes + kTileBytes;              // 86016
 constexpr uint32_t kWgSmem = 2 * kWgStage;                             // 172032
-constexpr uint32_t kWgALbo = 128, kWgASbo = 1536;
 
 __global__ void __launch_bounds__(128, 1)
 tc_wgrad(const __nv_bfloat16* __restrict__ Aws, const __nv_bfloat16* __restrict__ Gws, float* __restrict__ part,
@@ -764,20 +757,16 @@ tc_wgrad(const __nv_bfloat16* __restrict__ Aws, const __nv_bfloat16* __restrict_
   const uint32_t Dre = tmem, Dim = tmem + 256;
   const uint32_t idesc = idesc_bf16(128, NT, kIdescAMn | kIdescBMn);
   const int nt = (BKw - s + S - 1) / S; // tiles of this CTA
-  const int hl = lane & 7, cl4 = lane >> 3;
   auto prefetch = [&](int it) {
     const int rem = s + it * S;
     const uint32_t stage = smem_u32(smem) + (it & 1) * kWgStage;
     const size_t off = ((size_t)rem * nb + j) * H * NT;
-    const int nunits = ((H + 7) / 8) * 6;
-    for (int u = warp; u < nunits; u += 4) {
-      const int h = (u / 6) * 8 + hl;
-      const int nc = (u % 6) * 4 + cl4;
-      if (h < H) {
-        const uint32_t adst = stage + (nc < 12 ? 0u : kWgABytes) + (nc % 12) * kWgASbo + h * 16;
-        cp_async16(adst, Aws + off + (size_t)h * NT + nc * 8);
-        cp_async16(stage + 2 * kWgABytes + nc * kTileSbo + h * 16, Gws + off + (size_t)h * NT + nc * 8);
-      }
+    const int nchunks = H * (NT / 8);
+    for (int q = tid; q < nchunks; q += 128) {
+      const int h = q / (NT / 8), nc = q - h * (NT / 8);
+      const uint32_t adst = stage + (nc < 12 ? 0u : kWgABytes) + (nc % 12) * kWgASbo + h * 16;
+      cp_async16(adst, Aws + off + (size_t)q * 8);
+      cp_async16(stage + 2 * kWgABytes + nc * kTileSbo + h * 16, Gws + off + (size_t)q * 8);
     }
   };
   if (nt > 0) prefetch(0);
@@ -942,18 +931,19 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
       dft[off] = host_bf16(cos(a) * s);
       dft[kDftBytes / 2 + off] = host_bf16(sin(a) * s);
     }
-  // Fw^T: element (n = ri*96 + kw, k = w) = {cos, -sin}(2 pi kw w / W) / sqrt(W)  [x alpha_kw]
-  // Gw^T: element (n = w, k = ri*96 + kw) = alpha_kw {cos, -sin}(2 pi kw w / W) / sqrt(W)  [or alpha = 1]
+  // W-direction constants as K-major A operands, two 128-row halves each (kFwHalf bytes):
+  //   Fw  half ri : element (m = kw, k = w)          = {cos, -sin}(2 pi kw w / W) / sqrt(W)   [x alpha_kw]
+  //   Gw  half a  : element (m = w - 128 a, k = ri*96 + kw) = alpha_kw {cos, -sin}(...) / sqrt(W)  [or alpha = 1]
   std::vector<uint16_t> fw(kFwBytes / 2, 0), fwa(kFwBytes / 2, 0), gw(kFwBytes / 2, 0), gw1(kFwBytes / 2, 0);
+  auto aoff = [](int m, int k) { return ((k / 8) * kFwLbo + (m / 8) * kFwSbo + (m % 8) * 16 + (k % 8) * 2) / 2; };
   for (int kw = 0; kw < Wh; ++kw)
     for (int w = 0; w < W; ++w) {
       const double a = two_pi * (double)((long)kw * w % W) / (double)W, s = 1.0 / sqrt((double)W);
       const double alpha = (kw == 0 || 2 * kw == W) ? 1.0 : 2.0;
       for (int ri = 0; ri < 2; ++ri) {
         const double v = (ri == 0 ? cos(a) : -sin(a)) * s;
-        const int n = ri * BS + kw;
-        const uint32_t of = ((w / 8) * kFwLbo + (n / 8) * kFwSbo + (n % 8) * 16 + (w % 8) * 2) / 2;
-        const uint32_t og = ((n / 8) * kFwLbo + (w / 8) * kFwSbo + (w % 8) * 16 + (n % 8) * 2) / 2;
+        const uint32_t of = ri * (kFwHalf / 2) + aoff(kw, w);
+        const uint32_t og = (w / 128) * (kFwHalf / 2) + aoff(w % 128, ri * BS + kw);
         fw[of] = host_bf16(v);
         fwa[of] = host_bf16(v * alpha);
         gw[og] = host_bf16(v * alpha);

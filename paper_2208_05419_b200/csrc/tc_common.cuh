@@ -12,6 +12,10 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#ifndef AFNO_MBAR_SLEEP_NS
+#define AFNO_MBAR_SLEEP_NS 40
+#endif
+
 namespace afno {
 namespace tc {
 
@@ -104,13 +108,22 @@ __device__ __forceinline__ void mbar_init_fence() { asm volatile("fence.mbarrier
 __device__ __forceinline__ void mbar_arrive(uint64_t* mbar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(mbar)) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* mbar, uint32_t parity) {
+  uint32_t done;
   asm volatile(
-      "{\n.reg .pred p;\nWAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}" ::"r"(smem_u32(mbar)),
-      "r"(parity)
+      "{\n.reg .pred p;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n}"
+      : "=r"(done)
+      : "r"(smem_u32(mbar)), "r"(parity)
       : "memory");
+  return done != 0;
+}
+// Waiting warps back off with nanosleep: a tight try_wait loop floods the MIO/LSU queue that
+// cp.async, global stores and tcgen05 instructions of the working warps also go through.
+__device__ __forceinline__ void mbar_wait(uint64_t* mbar, uint32_t parity) {
+  if (mbar_try_wait(mbar, parity)) return;
+  while (!mbar_try_wait(mbar, parity)) __nanosleep(AFNO_MBAR_SLEEP_NS);
 }
 
 // ---- async copies (LDGSTS) and proxy fence --------------------------------------------------------

@@ -108,6 +108,15 @@ __device__ __forceinline__ void stg256(void* p, const uint32_t* r) {
                : "memory");
 }
 
+#ifdef AFNO_TIMING
+__device__ long long g_afno_dbg[32];
+#define DBG_T0() long long dbg_t = clock64()
+#define DBG_ACC(slot) do { long long n_ = clock64(); dbg_acc[slot] += n_ - dbg_t; dbg_t = n_; } while (0)
+#else
+#define DBG_T0()
+#define DBG_ACC(slot)
+#endif
+
 template <bool INVERSE>
 __global__ void __launch_bounds__(kRowThreads, 1)
 tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ res, __nv_bfloat16* __restrict__ out,
@@ -146,10 +155,15 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
     const uint32_t dst = smem_u32(sB0) + p * kRowBytes;
     const uint32_t idesc = idesc_bf16(128, CGRP, kIdescBMn);
     const int hl = lane & 7, cl4 = lane >> 3;
+#ifdef AFNO_TIMING
+    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#endif
+    DBG_T0();
     for (int it = p; it < nmine; it += 2) {
       const int use = it >> 1;
       // the previous MMAs on this buffer have completed (their commit also frees the operand tile)
       if (use > 0) mbar_wait(&full[p], (uint32_t)((use - 1) & 1));
+      DBG_ACC(0);
       const int t = blockIdx.x + it * gridDim.x;
       const int cg = t % ncg, bh = t / ncg;
       if (!INVERSE) {
@@ -174,12 +188,16 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
           if (c0 < C) cp_async16(dst + mc * kRowSbo + (ri * BS + kw) * 16, cbase + (size_t)kw * kwstride + ri * BS);
         }
       }
+      DBG_ACC(1);
       cp_async_wait_all();
+      DBG_ACC(2);
       fence_async_smem();
       asm volatile("bar.sync %0, %1;" ::"r"(1 + p), "n"(kRowProdWarps * 32) : "memory");
+      DBG_ACC(3);
       if (sub == 0 && lane == 0) {
         // the epilogue has drained this accumulator pair's previous contents
         if (use > 0) mbar_wait(&empty[p], (uint32_t)((use - 1) & 1));
+        DBG_ACC(4);
         tc_fence_after();
 #pragma unroll
         for (int a = 0; a < 2; ++a) {
@@ -191,14 +209,23 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
                    idesc, ks > 0);
         }
         mma_commit(&full[p]);
+        DBG_ACC(5);
       }
       __syncwarp();
     }
+#ifdef AFNO_TIMING
+    if (blockIdx.x == 0 && p == 0 && sub == 0 && lane == 0)
+      for (int q = 0; q < 8; ++q) g_afno_dbg[(INVERSE ? 16 : 0) + q] = dbg_acc[q];
+#endif
   } else {
     // ===== epilogue warps: accumulator a = warp / 4, row m = 32 * (warp % 4) + lane ====================
     const int a = warp >> 2;
     const int m = (warp & 3) * 32 + lane;
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
+#ifdef AFNO_TIMING
+    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#endif
+    DBG_T0();
     for (int it = 0; it < nmine; ++it) {
       const int t = blockIdx.x + it * gridDim.x;
       const int cg = t % ncg, bh = t / ncg;
@@ -208,6 +235,7 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
       const bool warp_has_rows = INVERSE ? (a * 128 + (warp & 3) * 32 < W) : ((warp & 3) * 32 < Kw);
       const int b = bh / H, h = bh - b * H;
       mbar_wait(&full[it & 1], (uint32_t)((it >> 1) & 1));
+      DBG_ACC(0);
       tc_fence_after();
       const uint32_t acc = tmem + (it & 1) * 256 + a * CGRP + lane_base;
       if (warp_has_rows) {
@@ -226,8 +254,12 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
             if (rvalid && c < C) {
               const int j = c / BS, cl = c - j * BS;
               __nv_bfloat16* dstp = out + ((((size_t)b * Kw + row) * nb + j) * H + h) * NT + a * BS + cl;
+#ifndef AFNO_DBG_NO_STORE
               stg256(dstp, pk);
               stg256(dstp + 16, pk + 8);
+#else
+              if (pk[0] == 0x12345u) stg256(dstp, pk);
+#endif
             }
           } else {
             uint32_t r0[8] = {0, 0, 0, 0, 0, 0, 0, 0}, r1[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -260,7 +292,15 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
         tc_fence_before();
         mbar_arrive(&empty[it & 1]);
       }
+      DBG_ACC(1);
     }
+#ifdef AFNO_TIMING
+    if (blockIdx.x == 0 && warp == 0 && lane == 0) {
+      g_afno_dbg[(INVERSE ? 16 : 0) + 8] = dbg_acc[0];
+      g_afno_dbg[(INVERSE ? 16 : 0) + 9] = dbg_acc[1];
+      g_afno_dbg[(INVERSE ? 16 : 0) + 10] = nmine;
+    }
+#endif
   }
   tc_fence_before();
   __syncthreads();
@@ -1065,5 +1105,11 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
 #undef TC_LAUNCH
   return cudaSuccess;
 }
+
+#ifdef AFNO_TIMING
+extern "C" int afno_debug_read(long long* out) {
+  return (int)cudaMemcpyFromSymbol(out, g_afno_dbg, sizeof(long long) * 32);
+}
+#endif
 
 } // namespace afno

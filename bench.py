@@ -250,6 +250,11 @@ def run_ours(args):
     roofline = kernel_roofline(dom, dom_n, dom_ms, PROF_STEPS, work, peaks, clocks.summary(), B, wl, kept_modes)
     roofline["share_of_step"] = dom_ms / total_prof_ms if total_prof_ms > 0 else None
     roofline["kernels_ms_per_step"] = {k: round(v[1] / PROF_STEPS, 4) for k, v in sorted(prof.items())}
+    per_kernel = {}
+    for k, (n, ms_k) in sorted(prof.items()):
+        r = kernel_roofline(k, n, ms_k, PROF_STEPS, work, peaks, clocks.summary(), B, wl, kept_modes)
+        per_kernel[k] = {"bound": r["bound"], "frac": r["frac"], "avg_launch_us": round(r["avg_launch_us"], 2)}
+    roofline["per_kernel"] = per_kernel
 
     # --- whole-layer 2-term roofline of BASELINE.json's metric ---------------------------------
     t_hbm = work["bytes"] / (peaks["hbm_gbs"] * 1e9)
@@ -297,9 +302,9 @@ def run_ours(args):
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, dt, cores = oracle_time(2)
+        v, dt, cores = oracle_time(8)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                        "sample": f"2 samples fwd+bwd at 90x180x768 (fp64 oracle, mixed-radix FFT mode), {dt:.1f} s"}
+                        "sample": f"8 samples fwd+bwd at 90x180x768 (fp64 oracle, mixed-radix FFT mode), {dt:.1f} s"}
 
     if rank == 0:
         line = {
@@ -320,28 +325,65 @@ def run_ours(args):
     return 0
 
 
-def kernel_roofline(name, n_launch, total_ms, steps, work, peaks, clocks, B, wl, kept_modes):
-    """roofline object for the dominant kernel (S5 states the per-launch figures)."""
-    per_launch_s = total_ms * 1e-3 / n_launch
+def kernel_work(name, B, wl, kept_modes):
+    """Algorithmic work of ONE launch of a kernel (S5 states these figures).
+
+    bytes: compulsory HBM traffic of the launch (activations bf16, spectra bf16-complex);
+    flops: model FLOPs of the complex block GEMMs it evaluates (8 per complex MAC, padding and
+    the DFT-as-GEMM arithmetic are NOT counted)."""
+    Kw = kept_modes // wl.H if kept_modes % wl.H == 0 else wl.W // 2 + 1
     bs = wl.C // wl.num_blocks
-    rows = B * kept_modes
-    if name in ("k_block_gemm", "k_block_wgrad"):
-        # fp32 FFMA complex block GEMM: 8 real FLOPs per complex MAC, rows x nb x bs x bs complex MACs
-        flops = 8.0 * rows * wl.num_blocks * bs * bs
-        sm_mhz = clocks.get("sm_mhz") or peaks["sm_max_mhz"]
-        peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12   # fp32 FMA peak at max clock, TFLOP/s
-        ach = flops / per_launch_s / 1e12
-        return {"kernel": name, "bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                "frac": ach / peak, "traffic": None,
-                "note": f"fp32 FFMA peak = 148 SM x 128 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz "
-                        f"(DESIGN.md S5); sm clock under load {sm_mhz}"}
-    # streaming FFT kernels: activation tensor in + spectrum out (or the reverse)
-    act = B * wl.H * wl.W * wl.C * 2
-    spec = B * wl.H * (wl.W // 2 + 1) * wl.C * 8
-    nbytes = act + spec
-    ach = nbytes / per_launch_s / 1e9
-    return {"kernel": name, "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-            "frac": ach / peaks["hbm_gbs"], "traffic": None}
+    act = B * wl.H * wl.W * wl.C * 2                       # one bf16 activation tensor
+    spec = B * Kw * wl.num_blocks * wl.H * 2 * bs * 2      # one bf16-complex half-spectrum
+    gemm = 2.0 * (2 * bs) * (2 * bs) * wl.num_blocks * kept_modes * B
+    table = {
+        "tc_wdft_fwd": dict(bound="hbm", bytes=act + spec, flops=0.0),
+        "tc_wdft_inv": dict(bound="hbm", bytes=spec + 2 * act, flops=0.0),
+        "tc_mix_fwd": dict(bound="tensor", bytes=2 * spec, flops=2 * gemm),
+        "tc_mix_bwd": dict(bound="tensor", bytes=7 * spec, flops=4 * gemm),
+        "tc_wgrad": dict(bound="hbm", bytes=2 * spec, flops=gemm),
+        "k_block_gemm": dict(bound="alu", bytes=0, flops=gemm),
+        "k_block_wgrad": dict(bound="alu", bytes=0, flops=gemm),
+    }
+    return table.get(name)
+
+
+def measured_traffic(name):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture."""
+    path = os.path.join(ROOT, "profiles", "r1_dram_traffic.json")
+    try:
+        return json.load(open(path)).get(name)
+    except Exception:
+        return None
+
+
+def kernel_roofline(name, n_launch, total_ms, steps, work, peaks, clocks, B, wl, kept_modes):
+    """roofline object for the dominant kernel: achieved = algorithmic work of one launch / its
+    average duration measured with CUDA events around every launch (afno_profile_*)."""
+    per_launch_s = total_ms * 1e-3 / n_launch
+    kw = kernel_work(name, B, wl, kept_modes)
+    out = {"kernel": name, "launches_per_step": n_launch / steps, "avg_launch_us": per_launch_s * 1e6,
+           "traffic": measured_traffic(name)}
+    if kw is None:
+        out.update({"bound": "hbm", "achieved": None, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": None})
+        return out
+    if kw["bound"] == "tensor":
+        ach = kw["flops"] / per_launch_s / 1e12
+        out.update({"bound": "tensor", "achieved": ach, "peak": peaks["tensor_tflops"], "unit": "TFLOP/s",
+                    "frac": ach / peaks["tensor_tflops"], "algorithmic_flops_per_launch": kw["flops"],
+                    "algorithmic_bytes_per_launch": kw["bytes"],
+                    "hbm_frac": kw["bytes"] / per_launch_s / 1e9 / peaks["hbm_gbs"],
+                    "note": "peak = measured bf16 burst (MEASURED_PEAKS.json); SM clock stays at max in this 1 ms step"})
+    elif kw["bound"] == "hbm":
+        ach = kw["bytes"] / per_launch_s / 1e9
+        out.update({"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": ach / peaks["hbm_gbs"], "algorithmic_bytes_per_launch": kw["bytes"]})
+    else:
+        peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+        ach = kw["flops"] / per_launch_s / 1e12
+        out.update({"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                    "note": "fp32 FFMA peak = 148 SM x 128 lanes x 2 x max SM clock (DESIGN.md S5)"})
+    return out
 
 
 def main():

@@ -111,6 +111,21 @@ class ClockSampler:
                 "reasons": sorted(self.reasons)}
 
 
+def max_over_ranks(value: float, dist, device) -> float:
+    """Max of a per-rank scalar over all ranks (the N > 1 timing rule); dist = torch.distributed or None."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, samples_per_rank_step: int, steps: int, ms_max: float) -> float:
+    """Replicas only: every rank processes its own batch; value = all ranks' samples / max time."""
+    return world * samples_per_rank_step * steps / (ms_max * 1e-3)
+
+
 def oracle_time(n_samples: int):
     """Times the fp64 CPU oracle (as it stands) fwd+bwd on n_samples samples of the workload."""
     from oracle import afno_oracle
@@ -225,13 +240,9 @@ def run_ours(args):
             step(i)
         ev1.record(stream)
         barrier()
-    ms = ev0.elapsed_time(ev1)
-    if dist is not None:
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ev0.elapsed_time(ev1), dist, dev)
     ms_per_step = ms / args.steps
-    value = world * B * args.steps / (ms * 1e-3)
+    value = whole_job_value(world, B, args.steps, ms)
 
     # --- per-kernel durations, measured live with CUDA events around every launch -----------
     binding.afno_profile_start()
@@ -291,12 +302,8 @@ def run_ours(args):
         for _ in range(E2E_STEPS):
             host_step()
         torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        e2e = {"value": world * B * E2E_STEPS / dt, "unit": UNIT,
+        dt = max_over_ranks(time.perf_counter() - t0, dist, dev)
+        e2e = {"value": whole_job_value(world, B, E2E_STEPS, dt * 1e3), "unit": UNIT,
                "h2d_bytes_per_step": 3 * act + 2 * pbytes, "d2h_bytes_per_step": 2 * act + pbytes,
                "steps": E2E_STEPS, "note": "afno_spectral_fwd_host + afno_spectral_bwd_host, pinned host buffers"}
 

@@ -154,7 +154,6 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
     const int p = pw / kRowProdWarps, sub = pw % kRowProdWarps;
     const uint32_t dst = smem_u32(sB0) + p * kRowBytes;
     const uint32_t idesc = idesc_bf16(128, CGRP, kIdescBMn);
-    const int hl = lane & 7, cl4 = lane >> 3;
 #ifdef AFNO_TIMING
     long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 #endif
@@ -411,6 +410,14 @@ __device__ __forceinline__ void store16(__nv_bfloat16* dst, const uint32_t (&pk)
                  "r"(pk[8 * g + 6]), "r"(pk[8 * g + 7])
                  : "memory");
 }
+// chunk c of this thread's row -> operand image of a tile in GLOBAL memory (same byte order as the
+// shared-memory operand: [n/8][row][8]); consecutive rows are consecutive 16-byte pieces, so a warp
+// store covers 512 contiguous bytes, and tc_wgrad fetches the tile with bulk copies
+__device__ __forceinline__ void store_image16(uint8_t* img, int half, int c, int r, const uint32_t (&pk)[16]) {
+#pragma unroll
+  for (int g = 0; g < 4; ++g)
+    *(uint4*)(img + (half * 12 + c * 4 + g) * kTileSbo + r * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
+}
 // chunk c of this thread's row -> MN-major B operand tile (K = row r)
 __device__ __forceinline__ void store_tile16(uint8_t* tile, int half, int c, int r, const uint32_t (&pk)[16]) {
 #pragma unroll
@@ -592,6 +599,7 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
       const uint32_t tp = (uint32_t)(i & 1);
       const int j = t / BKw, rem = t - j * BKw;
       const size_t row_off = (((size_t)rem * p.nb + j) * p.H + r) * NT + half * BS;
+      const size_t img_off = ((size_t)rem * p.nb + j) * kTileBytes;   // operand-image tensors (bytes)
       const float* bias1 = p.bprep + (size_t)j * 2 * NT + half * BS;
       const float* bias2 = bias1 + NT;
       uint32_t m1[3], m2[3];
@@ -605,7 +613,7 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
         tmem_wait_ld();
         pack32(v, pk);
         tmem_st16(R0 + lane_base + 16 * c, pk);
-        if (BACKWARD && row_valid) store16(p.Xh + row_off + 32 * c, pk);
+        if (BACKWARD && r < HP) store_image16((uint8_t*)p.Xh + img_off, half, c, r, pk);
         publish_chunk(&bars.cready[half][c]);
       }
       // ---- stage 1 -> O1 = relu(P1 + b1), packed in place (R1) ----
@@ -629,7 +637,7 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
         }
         m1[c] = bits;
         tmem_st16(R1 + lane_base + 16 * c, pk);
-        if (BACKWARD && row_valid) store16(p.O1 + row_off + 32 * c, pk);
+        if (BACKWARD && r < HP) store_image16((uint8_t*)p.O1 + img_off, half, c, r, pk);
         publish_chunk(&bars.cready[half][c]);
       }
       // ---- stage 2 -> P2 + b2 : forward Z = softshrink -> smem tile ; backward mask2 ----
@@ -691,7 +699,7 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
             pk[q] = pack_bf16((bits >> (2 * q)) & 1u ? __uint_as_float(v[2 * q]) : 0.f,
                               (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[2 * q + 1]) : 0.f);
           tmem_st16(R1 + lane_base + 16 * c, pk);
-          if (row_valid) store16(p.G2 + row_off + 32 * c, pk);
+          if (r < HP) store_image16((uint8_t*)p.G2 + img_off, half, c, r, pk);
           publish_chunk(&bars.cready[half][c]);
         }
         // ---- stage 4 -> G1 = mask1 (.) (G2 W2^H), packed in place (R0) ----
@@ -708,7 +716,7 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
             pk[q] = pack_bf16((bits >> (2 * q)) & 1u ? __uint_as_float(v[2 * q]) : 0.f,
                               (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[2 * q + 1]) : 0.f);
           tmem_st16(R0 + lane_base + 16 * c, pk);
-          if (row_valid) store16(p.G1 + row_off + 32 * c, pk);
+          if (r < HP) store_image16((uint8_t*)p.G1 + img_off, half, c, r, pk);
           publish_chunk(&bars.cready[half][c]);
         }
         // ---- stage 5 -> GX as the B operand of the inverse transform (gradient tile buffer) ----
@@ -768,11 +776,21 @@ constexpr uint32_t kWgABytes = 16 * kWgASbo;                            // 24832
 constexpr uint32_t kWgStage = 2 * kWgABytes + kTileBytes;              // 86016
 constexpr uint32_t kWgSmem = 2 * kWgStage;                             // 172032
 
+__device__ __forceinline__ void bulk_copy(uint32_t dst_smem, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst_smem),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+
+// Aws / Gws: operand-image tensors written by tc_mix<true> ([tile][24 chunks][kTileSbo bytes]).
 __global__ void __launch_bounds__(128, 1)
 tc_wgrad(const __nv_bfloat16* __restrict__ Aws, const __nv_bfloat16* __restrict__ Gws, float* __restrict__ part,
          int BKw, int H, int nb, int S) {
   extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) uint64_t mbar[2];
+  __shared__ __align__(8) uint64_t full[2], empty[2], done;
   __shared__ uint32_t tmem_slot;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int j = blockIdx.x / S, s = blockIdx.x - j * S;
@@ -784,11 +802,15 @@ tc_wgrad(const __nv_bfloat16* __restrict__ Aws, const __nv_bfloat16* __restrict_
     *(uint16_t*)(smem + st * kWgStage + 12 * kWgASbo + rr * 16) = 0x3F80; // bf16 1.0
   }
   if (tid == 0) {
-    mbar_init(&mbar[0], 1);
-    mbar_init(&mbar[1], 1);
+    for (int b = 0; b < 2; ++b) {
+      mbar_init(&full[b], 1);
+      mbar_init(&empty[b], 1);
+    }
+    mbar_init(&done, 1);
     mbar_init_fence();
   }
   if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  fence_async_smem();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -797,33 +819,27 @@ tc_wgrad(const __nv_bfloat16* __restrict__ Aws, const __nv_bfloat16* __restrict_
   const uint32_t Dre = tmem, Dim = tmem + 256;
   const uint32_t idesc = idesc_bf16(128, NT, kIdescAMn | kIdescBMn);
   const int nt = (BKw - s + S - 1) / S; // tiles of this CTA
-  auto prefetch = [&](int it) {
-    const int rem = s + it * S;
-    const uint32_t stage = smem_u32(smem) + (it & 1) * kWgStage;
-    const size_t off = ((size_t)rem * nb + j) * H * NT;
-    const int nchunks = H * (NT / 8);
-    for (int q = tid; q < nchunks; q += 128) {
-      const int h = q / (NT / 8), nc = q - h * (NT / 8);
-      const uint32_t adst = stage + (nc < 12 ? 0u : kWgABytes) + (nc % 12) * kWgASbo + h * 16;
-      cp_async16(adst, Aws + off + (size_t)q * 8);
-      cp_async16(stage + 2 * kWgABytes + nc * kTileSbo + h * 16, Gws + off + (size_t)q * 8);
+  (void)lane;
+  if (tid == 0) {
+    // ---- producer: three bulk copies per tile (A re half, A im half, G), async proxy, no LSU ----
+    constexpr uint32_t kHalfImg = 12 * kTileSbo;
+    for (int it = 0; it < nt; ++it) {
+      const int b = it & 1, use = it >> 1;
+      if (use > 0) mbar_wait(&empty[b], (uint32_t)((use - 1) & 1));
+      const size_t off = ((size_t)(s + it * S) * nb + j) * kTileBytes;
+      const uint32_t stage = smem_u32(smem) + b * kWgStage;
+      mbar_expect_tx(&full[b], 2 * kHalfImg + kTileBytes);
+      bulk_copy(stage, (const uint8_t*)Aws + off, kHalfImg, &full[b]);
+      bulk_copy(stage + kWgABytes, (const uint8_t*)Aws + off + kHalfImg, kHalfImg, &full[b]);
+      bulk_copy(stage + 2 * kWgABytes, (const uint8_t*)Gws + off, kTileBytes, &full[b]);
     }
-  };
-  if (nt > 0) prefetch(0);
-  cp_async_commit();
-  for (int it = 0; it < nt; ++it) {
-    if (it + 1 < nt) {
-      if (it >= 1) mbar_wait(&mbar[(it + 1) & 1], (uint32_t)(((it - 1) >> 1) & 1));
-      prefetch(it + 1);
-    }
-    cp_async_commit();
-    cp_async_wait_group<1>();
-    fence_async_smem();
-    tc_fence_before();
-    __syncthreads();
-    if (tid == 0) {
+  } else if (tid == 32) {
+    // ---- MMA issuer ----
+    for (int it = 0; it < nt; ++it) {
+      const int b = it & 1;
+      mbar_wait(&full[b], (uint32_t)((it >> 1) & 1));
       tc_fence_after();
-      const uint32_t stage = smem_u32(smem) + (it & 1) * kWgStage;
+      const uint32_t stage = smem_u32(smem) + b * kWgStage;
       const uint32_t g = stage + 2 * kWgABytes;
 #pragma unroll
       for (int ks = 0; ks < HP / 16; ++ks) {
@@ -831,12 +847,14 @@ tc_wgrad(const __nv_bfloat16* __restrict__ Aws, const __nv_bfloat16* __restrict_
         mma_ss(Dre, smem_desc(stage + ks * 2 * kWgALbo, kWgALbo, kWgASbo), bd, idesc, (it | ks) != 0);
         mma_ss(Dim, smem_desc(stage + kWgABytes + ks * 2 * kWgALbo, kWgALbo, kWgASbo), bd, idesc, (it | ks) != 0);
       }
-      mma_commit(&mbar[it & 1]);
+      mma_commit(&empty[b]);
     }
+    mma_commit(&done);
   }
+  __syncwarp();
   float* dst = part + ((size_t)blockIdx.x * 2) * 128 * NT + (size_t)tid * NT;
   if (nt > 0) {
-    mbar_wait(&mbar[(nt - 1) & 1], (uint32_t)(((nt - 1) >> 1) & 1));
+    mbar_wait(&done, 0u);
     tc_fence_after();
 #pragma unroll 1
     for (int acc = 0; acc < 2; ++acc)
@@ -939,10 +957,11 @@ TcWs tc_carve(const Geometry& g, bool backward, char* base) {
   w.bprep = (float*)take((size_t)g.nb * 2 * NT * sizeof(float));
   if (backward) {
     w.A1g = (__nv_bfloat16*)take(spec);
-    w.Xh = (__nv_bfloat16*)take(spec);
-    w.O1 = (__nv_bfloat16*)take(spec);
-    w.G2 = (__nv_bfloat16*)take(spec);
-    w.G1 = (__nv_bfloat16*)take(spec);
+    const size_t img = (size_t)g.B * g.Kw * g.nb * kTileBytes;   // operand-image layout
+    w.Xh = (__nv_bfloat16*)take(img);
+    w.O1 = (__nv_bfloat16*)take(img);
+    w.G2 = (__nv_bfloat16*)take(img);
+    w.G1 = (__nv_bfloat16*)take(img);
     int S = 148 / g.nb;
     if (S < 1) S = 1;
     if (S > g.B * g.Kw) S = g.B * g.Kw;

@@ -21,6 +21,18 @@ namespace tc {
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+// One elected lane of a CONVERGED warp (elect.sync): lets ptxas emit straight-line uniform-datapath
+// code for tcgen05.mma / commit instead of a per-lane election loop around every instruction.
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred = 0;
+  asm volatile(
+      "{\n.reg .b32 rx;\n.reg .pred px;\n"
+      "elect.sync rx|px, 0xFFFFFFFF;\n"
+      "@px mov.s32 %0, 1;\n}"
+      : "+r"(pred));
+  return pred != 0;
+}
+
 // ---- shared-memory matrix descriptor (SWIZZLE_NONE, version 1) -----------------------------
 __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
   uint64_t d = 0;

@@ -193,7 +193,7 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
       fence_async_smem();
       asm volatile("bar.sync %0, %1;" ::"r"(1 + p), "n"(kRowProdWarps * 32) : "memory");
       DBG_ACC(3);
-      if (sub == 0 && lane == 0) {
+      if (sub == 0 && elect_one()) {
         // the epilogue has drained this accumulator pair's previous contents
         if (use > 0) mbar_wait(&empty[p], (uint32_t)((use - 1) & 1));
         DBG_ACC(4);
@@ -504,18 +504,24 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
     const uint32_t aTA = smem_u32(sTileA), aTB = smem_u32(sTileB);
     uint32_t pc = 0;       // parity of the chunk barriers (they complete once per MLP stage)
     int cur_j = -1;
+#ifdef AFNO_TIMING
+    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#endif
+    DBG_T0();
     auto mlp_stage = [&](uint32_t T, uint32_t S, uint32_t wr, uint32_t wi, bool transposed, uint64_t* done) {
       for (int c = 0; c < 3; ++c) {
         mbar_wait(&bars.cready[0][c], pc);
         mbar_wait(&bars.cready[1][c], pc);
-        if (lane == 0) {
+        DBG_ACC(c == 0 ? 1 : 2);
+        if (elect_one()) {
           tc_fence_after();
           if (transposed) issue_mlp_chunk<true>(T, S, wr, wi, c);
           else issue_mlp_chunk<false>(T, S, wr, wi, c);
         }
       }
-      if (lane == 0) mma_commit(done);
+      if (elect_one()) mma_commit(done);
       __syncwarp();
+      DBG_ACC(3);
       pc ^= 1;
     };
     for (int t = t_begin; t < t_end; ++t) {
@@ -537,25 +543,29 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
         const int b = i & 1;
         const uint32_t cur_tile = b ? aTB : aTA;
         mbar_wait(&bars.tfull[b], (uint32_t)((i >> 1) & 1));
-        if (lane == 0) {
+        DBG_ACC(0);
+        if (elect_one()) {
           tc_fence_after();
           issue_fwd_dft(R0, aCh, aSh, cur_tile);
           mma_commit(&bars.dfull[0]);
         }
         __syncwarp();
+        DBG_ACC(4);
         mlp_stage(R1, R0, aW + 0 * kWBytes, aW + 1 * kWBytes, false, &bars.dfull[1]);
         mlp_stage(R0, R1, aW + 2 * kWBytes, aW + 3 * kWBytes, false, &bars.dfull[2]);
         mbar_wait(&bars.zready, tp);
-        if (lane == 0) {
+        DBG_ACC(5);
+        if (elect_one()) {
           tc_fence_after();
           issue_inv_dft(R1, aCh, aSh, cur_tile);
           mma_commit(&bars.dfull[3]);
           mma_commit(&bars.tfree[b]);
         }
         __syncwarp();
+        DBG_ACC(4);
       } else {
         mbar_wait(&bars.tfull[0], tp);
-        if (lane == 0) {
+        if (elect_one()) {
           tc_fence_after();
           issue_fwd_dft(R0, aCh, aSh, aTA);
           mma_commit(&bars.dfull[0]);
@@ -568,7 +578,7 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
         // once stage 2 has completed)
         mbar_wait(&bars.dfull[2], tp);
         mbar_wait(&bars.tfull[1], tp);
-        if (lane == 0) {
+        if (elect_one()) {
           tc_fence_after();
           issue_fwd_dft(R1, aCh, aSh, aTB);
           mma_commit(&bars.dfull[3]);
@@ -577,7 +587,7 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
         mlp_stage(R0, R1, aW + 2 * kWBytes, aW + 3 * kWBytes, true, &bars.dfull[4]);   // G1 = G2 W2^H
         mlp_stage(R1, R0, aW + 0 * kWBytes, aW + 1 * kWBytes, true, &bars.dfull[5]);   // GX = G1 W1^H
         mbar_wait(&bars.zready, tp);
-        if (lane == 0) {
+        if (elect_one()) {
           tc_fence_after();
           issue_inv_dft(R1, aCh, aSh, aTB);   // into R1: the next tile's stage 0 reuses R0 at once
           mma_commit(&bars.dfull[6]);
@@ -586,8 +596,18 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
         __syncwarp();
       }
     }
+#ifdef AFNO_TIMING
+    if (!BACKWARD && blockIdx.x == 0 && lane == 0) {
+      for (int q = 0; q < 8; ++q) g_afno_dbg[q] = dbg_acc[q];
+      g_afno_dbg[15] = t_end - t_begin;
+    }
+#endif
   } else {
     // ================================ epilogue warps =========================================
+#ifdef AFNO_TIMING
+    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#endif
+    DBG_T0();
     const int half = warp >> 2;
     const int r = (warp & 3) * 32 + lane;
     const uint32_t lane_base = ((uint32_t)((warp & 3) * 32) << 16) + half * BS;
@@ -604,7 +624,9 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
       const float* bias2 = bias1 + NT;
       uint32_t m1[3], m2[3];
       // ---- stage 0 -> spectrum Xh, packed in place (R0) ----
+      DBG_ACC(4);
       mbar_wait(&bars.dfull[0], tp);
+      DBG_ACC(0);
       tc_fence_after();
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
@@ -617,7 +639,9 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
         publish_chunk(&bars.cready[half][c]);
       }
       // ---- stage 1 -> O1 = relu(P1 + b1), packed in place (R1) ----
+      DBG_ACC(4);
       mbar_wait(&bars.dfull[1], tp);
+      DBG_ACC(1);
       tc_fence_after();
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
@@ -641,7 +665,9 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
         publish_chunk(&bars.cready[half][c]);
       }
       // ---- stage 2 -> P2 + b2 : forward Z = softshrink -> smem tile ; backward mask2 ----
+      DBG_ACC(4);
       mbar_wait(&bars.dfull[2], tp);
+      DBG_ACC(2);
       tc_fence_after();
       uint8_t* ztile = (i & 1) ? sTileB : sTileA;
 #pragma unroll
@@ -673,7 +699,9 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
         tc_fence_before();
         mbar_arrive(&bars.zready);
         // ---- stage 3 -> A2 rows ----
+        DBG_ACC(4);
         mbar_wait(&bars.dfull[3], tp);
+        DBG_ACC(3);
         tc_fence_after();
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -760,7 +788,12 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
         }
         tc_fence_before();
       }
+      DBG_ACC(4);
     }
+#ifdef AFNO_TIMING
+    if (!BACKWARD && blockIdx.x == 0 && tid == 0)
+      for (int q = 0; q < 8; ++q) g_afno_dbg[16 + q] = dbg_acc[q];
+#endif
   }
   tc_fence_before();
   __syncthreads();
@@ -820,7 +853,7 @@ tc_wgrad(const __nv_bfloat16* __restrict__ Aws, const __nv_bfloat16* __restrict_
   const uint32_t idesc = idesc_bf16(128, NT, kIdescAMn | kIdescBMn);
   const int nt = (BKw - s + S - 1) / S; // tiles of this CTA
   (void)lane;
-  if (tid == 0) {
+  if (warp == 0 && elect_one()) {
     // ---- producer: three bulk copies per tile (A re half, A im half, G), async proxy, no LSU ----
     constexpr uint32_t kHalfImg = 12 * kTileSbo;
     for (int it = 0; it < nt; ++it) {
@@ -833,7 +866,7 @@ tc_wgrad(const __nv_bfloat16* __restrict__ Aws, const __nv_bfloat16* __restrict_
       bulk_copy(stage + kWgABytes, (const uint8_t*)Aws + off + kHalfImg, kHalfImg, &full[b]);
       bulk_copy(stage + 2 * kWgABytes, (const uint8_t*)Gws + off, kTileBytes, &full[b]);
     }
-  } else if (tid == 32) {
+  } else if (warp == 1 && elect_one()) {
     // ---- MMA issuer ----
     for (int it = 0; it < nt; ++it) {
       const int b = it & 1;

@@ -15,6 +15,7 @@
 // instruction descriptor's negate bit for the minus signs, so only W_re and W_im (not the 2x2
 // real block form) live in shared memory.
 #include <math.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
@@ -109,7 +110,7 @@ __device__ __forceinline__ void stg256(void* p, const uint32_t* r) {
 }
 
 #ifdef AFNO_TIMING
-__device__ long long g_afno_dbg[32];
+__device__ long long g_afno_dbg[96];
 #define DBG_T0() long long dbg_t = clock64()
 #define DBG_ACC(slot) do { long long n_ = clock64(); dbg_acc[slot] += n_ - dbg_t; dbg_t = n_; } while (0)
 #else
@@ -598,8 +599,8 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
     }
 #ifdef AFNO_TIMING
     if (!BACKWARD && blockIdx.x == 0 && lane == 0) {
-      for (int q = 0; q < 8; ++q) g_afno_dbg[q] = dbg_acc[q];
-      g_afno_dbg[15] = t_end - t_begin;
+      for (int q = 0; q < 8; ++q) g_afno_dbg[32 + q] = dbg_acc[q];
+      g_afno_dbg[47] = t_end - t_begin;
     }
 #endif
   } else {
@@ -792,7 +793,379 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
     }
 #ifdef AFNO_TIMING
     if (!BACKWARD && blockIdx.x == 0 && tid == 0)
-      for (int q = 0; q < 8; ++q) g_afno_dbg[16 + q] = dbg_acc[q];
+      for (int q = 0; q < 8; ++q) g_afno_dbg[48 + q] = dbg_acc[q];
+#endif
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<512>(tmem);
+}
+
+// ---- tc_mix2: two mode tiles in flight per CTA (ping-pong), 12 epilogue warps ------------------------
+// Same arithmetic and the same stages as tc_mix, rescheduled so that the tensor core and the
+// epilogue warps never wait for each other:
+//   * the CTA runs two tile streams X and Y; "phase" t belongs to stream t & 1 and is stage
+//     (t >> 1) % NS of that stream's current tile.  The control warp issues the GEMMs S_0, S_1, ..
+//     in phase order, the epilogue warps drain E_0, E_1, .. in phase order; S_t only waits for
+//     E_(t-2) (the same stream's previous stage) and E_t for S_t, so S_(t+1) runs under E_t.
+//   * tensor memory is five 96-column slots; phase t accumulates (re | im) into slots 3t, 3t+1
+//     (mod 5), its epilogue compacts the bf16 A operand of the next GEMM into slot 3t, which
+//     frees slot 3t+1; by the time S_(t+2) needs its two slots, 3t+1 and 3t+2 (the A operand of
+//     S_(t+1), read by the in-order tensor pipe before S_(t+2) writes) are free: 480 columns.
+//   * accumulator rows >= 96 hold nothing (H <= 96), so the warps of TMEM lane quarter 3
+//     (warp % 4 == 3) are the control warp and the three loader warps; each of lane quarters 0..2
+//     has four epilogue warps, one per 48-column quarter (re lo, re hi, im lo, im hi).
+//   * three tile buffers: tile i lives in buffer i % 3 (input tile, then the B operand of the
+//     inverse transform); backward: x tile, then the gradient tile, then GX.
+// Every CTA works on ONE channel block j (grid = nb * S), so the weights are loaded once.
+constexpr int kMix2Threads = 512;
+constexpr uint32_t kDft2Lbo = 1536, kDft2Sbo = 128;  // Ch / Sh: K-major A, 96 stored rows, order [k/8][m/8 < 12]
+constexpr uint32_t kDft2Bytes = 12 * kDft2Lbo;        // 18432 (rows 96..127 alias the next k-chunk: finite, unused)
+constexpr uint32_t kMix2Smem = 2 * kDft2Bytes + 4 * kWBytes + 3 * kTileBytes; // 222336
+constexpr uint32_t kSlot = 96;
+
+struct Mix2Bars {
+  uint64_t dfull[2];  // stream's current stage accumulated (tcgen05.commit)
+  uint64_t edone[2];  // stream's current stage drained by the 12 epilogue warps
+  uint64_t xfull[3];  // buffer holds the input tile (forward: spectrum; backward: x spectrum)
+  uint64_t gfull[3];  // backward: buffer holds the gradient tile
+  uint64_t xfree[3];  // backward: stage 0 has consumed the x tile (tcgen05.commit)
+  uint64_t tfree[3];  // the tile's last stage has consumed the buffer (tcgen05.commit)
+};
+
+__device__ __forceinline__ void issue_dft2(uint32_t d, uint32_t a_base, uint32_t b_base, uint32_t idesc, bool fresh) {
+#pragma unroll
+  for (int ks = 0; ks < HP / 16; ++ks)
+    mma_ss(d, smem_desc(a_base + ks * 2 * kDft2Lbo, kDft2Lbo, kDft2Sbo),
+           smem_desc(b_base + ks * 2 * kTileLbo, kTileLbo, kTileSbo), idesc, !(fresh && ks == 0));
+}
+// forward transform (exp(-i theta)):  Xr = Ch Ar + Sh Ai ; Xi = Ch Ai - Sh Ar
+__device__ __forceinline__ void issue_fwd_dft2(uint32_t Dre, uint32_t Dim, uint32_t aCh, uint32_t aSh, uint32_t tile) {
+  const uint32_t id = idesc_bf16(128, BS, kIdescBMn), half = (BS / 8) * kTileSbo;
+  issue_dft2(Dre, aCh, tile, id, true);
+  issue_dft2(Dre, aSh, tile + half, id, false);
+  issue_dft2(Dim, aCh, tile + half, id, true);
+  issue_dft2(Dim, aSh, tile, id | kIdescNegA, false);
+}
+// inverse transform (exp(+i theta)):  Tr = Ch Zr - Sh Zi ; Ti = Ch Zi + Sh Zr
+__device__ __forceinline__ void issue_inv_dft2(uint32_t Dre, uint32_t Dim, uint32_t aCh, uint32_t aSh, uint32_t tile) {
+  const uint32_t id = idesc_bf16(128, BS, kIdescBMn), half = (BS / 8) * kTileSbo;
+  issue_dft2(Dre, aCh, tile, id, true);
+  issue_dft2(Dre, aSh, tile + half, id | kIdescNegA, false);
+  issue_dft2(Dim, aCh, tile + half, id, true);
+  issue_dft2(Dim, aSh, tile, id, false);
+}
+// T = S W (TRANSPOSED = false) or S W^H (true); S = compact bf16 A operand: re at columns
+// [S, S+48), im at [S+48, S+96) (two bf16 per column)
+template <bool TRANSPOSED>
+__device__ __forceinline__ void issue_mlp2(uint32_t Tre, uint32_t Tim, uint32_t S, uint32_t wr, uint32_t wi) {
+  const uint32_t id = idesc_bf16(128, BS, TRANSPOSED ? kIdescBMn : 0u);
+  const uint32_t lbo = TRANSPOSED ? kWSbo : kWLbo, sbo = TRANSPOSED ? kWLbo : kWSbo;
+#pragma unroll
+  for (int ks = 0; ks < BS / 16; ++ks) {
+    const uint32_t acc = ks != 0;
+    mma_ts(Tre, S + ks * 8, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, acc);
+    mma_ts(Tim, S + ks * 8, smem_desc(wi + ks * 2 * lbo, lbo, sbo), TRANSPOSED ? (id | kIdescNegB) : id, acc);
+  }
+#pragma unroll
+  for (int ks = 0; ks < BS / 16; ++ks) {
+    mma_ts(Tre, S + 48 + ks * 8, smem_desc(wi + ks * 2 * lbo, lbo, sbo), TRANSPOSED ? id : (id | kIdescNegB), 1u);
+    mma_ts(Tim, S + 48 + ks * 8, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, 1u);
+  }
+}
+
+__device__ __forceinline__ void ld48(uint32_t taddr, uint32_t (&v)[48]) {
+  tmem_ld16<0>(taddr, v);
+  tmem_ld16<16>(taddr + 16, v);
+  tmem_ld16<32>(taddr + 32, v);
+  tmem_wait_ld();
+}
+__device__ __forceinline__ void st24(uint32_t taddr, const uint32_t (&pk)[24]) {
+  tmem_st8<0>(taddr, pk);
+  tmem_st8<8>(taddr + 8, pk);
+  tmem_st8<16>(taddr + 16, pk);
+}
+__device__ __forceinline__ void pack48(const uint32_t (&v)[48], uint32_t (&pk)[24]) {
+#pragma unroll
+  for (int q = 0; q < 24; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
+}
+// 48 columns of this thread's row -> six 16-byte pieces of an operand image / operand tile
+__device__ __forceinline__ void store_chunks6(uint8_t* base, int chunk0, int r, const uint32_t (&pk)[24]) {
+#pragma unroll
+  for (int g = 0; g < 6; ++g)
+    *(uint4*)(base + (chunk0 + g) * kTileSbo + r * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
+}
+
+template <bool BACKWARD, bool EXPORT>
+__global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ Mix2Bars bars;
+  __shared__ uint32_t tmem_slot;
+  __shared__ __align__(16) float sBias[2 * NT];
+  constexpr int NS = BACKWARD ? 7 : 4;
+  uint8_t* sCh = smem;
+  uint8_t* sSh = smem + kDft2Bytes;
+  uint8_t* sW = smem + 2 * kDft2Bytes;
+  uint8_t* sT = sW + 4 * kWBytes;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int j = blockIdx.x / S, s0 = blockIdx.x - j * S;
+  const int BKw = p.B * p.Kw;
+  const int n = s0 < BKw ? (BKw - s0 + S - 1) / S : 0;   // tiles of this CTA: rem = s0 + i * S
+  for (uint32_t i = tid; i < 3 * kTileBytes / 16; i += kMix2Threads) ((uint4*)sT)[i] = make_uint4(0, 0, 0, 0);
+  for (uint32_t i = tid; i < 2 * kDft2Bytes / 16; i += kMix2Threads) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
+  {
+    const uint8_t* wsrc = p.wprep + (size_t)j * 4 * kWBytes;
+    for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMix2Threads) cp_async16(smem_u32(sW) + i * 16, wsrc + (size_t)i * 16);
+  }
+  for (int i = tid; i < 2 * NT; i += kMix2Threads) sBias[i] = p.bprep[(size_t)j * 2 * NT + i];
+  if (tid == 0) {
+    for (int q = 0; q < 2; ++q) {
+      mbar_init(&bars.dfull[q], 1);
+      mbar_init(&bars.edone[q], 12);
+    }
+    for (int q = 0; q < 3; ++q) {
+      mbar_init(&bars.xfull[q], kMixLoadWarps * 32);
+      mbar_init(&bars.gfull[q], kMixLoadWarps * 32);
+      mbar_init(&bars.xfree[q], 1);
+      mbar_init(&bars.tfree[q], 1);
+    }
+    mbar_init_fence();
+  }
+  if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  cp_async_wait_all();
+  fence_async_smem();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const int T = 2 * NS * ((n + 1) / 2);   // phases
+  const int lq = warp & 3;
+
+  if (lq == 3 && warp != 3) {
+    // ================================ loader warps (7, 11, 15) ================================
+    const int sub = (warp >> 2) - 1;
+    const uint32_t aT = smem_u32(sT);
+    auto tile_off = [&](int i) { return ((size_t)(s0 + i * S) * p.nb + j) * p.H * NT; };
+    auto load = [&](int buf, const __nv_bfloat16* src, uint64_t* full) {
+      load_tile_warp(aT + buf * kTileBytes, src, p.H, lane, sub);
+      cp_async_wait_all();
+      fence_async_smem();
+      mbar_arrive(full);
+    };
+    if (!BACKWARD) {
+      for (int i = 0; i < n; ++i) {
+        const int buf = i % 3, use = i / 3;
+        if (use > 0) mbar_wait(&bars.tfree[buf], (uint32_t)((use - 1) & 1));
+        load(buf, p.A1 + tile_off(i), &bars.xfull[buf]);
+      }
+    } else {
+      // x(0) x(1) x(2) | g(0) g(1) | then for k = 0, 1, ..: x(k+3) after the last stage of tile k,
+      // g(k+2) after stage 0 of tile k+2 -- the order in which the buffers become free
+      for (int i = 0; i < 3 && i < n; ++i) load(i, p.A1 + tile_off(i), &bars.xfull[i]);
+      for (int i = 0; i < 2 && i < n; ++i) {
+        mbar_wait(&bars.xfree[i], 0u);
+        load(i, p.A1g + tile_off(i), &bars.gfull[i]);
+      }
+      for (int k = 0; k < n; ++k) {
+        const int ix = k + 3, ig = k + 2;
+        if (ix < n) {
+          mbar_wait(&bars.tfree[ix % 3], (uint32_t)((ix / 3 - 1) & 1));
+          load(ix % 3, p.A1 + tile_off(ix), &bars.xfull[ix % 3]);
+        }
+        if (ig < n) {
+          mbar_wait(&bars.xfree[ig % 3], (uint32_t)((ig / 3) & 1));
+          load(ig % 3, p.A1g + tile_off(ig), &bars.gfull[ig % 3]);
+        }
+      }
+    }
+  } else if (warp == 3) {
+    // ================================ control warp ===========================================
+    const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW), aT = smem_u32(sT);
+    const uint32_t w1r = aW, w1i = aW + kWBytes, w2r = aW + 2 * kWBytes, w2i = aW + 3 * kWBytes;
+    uint32_t cs0 = 0, cs1 = 0;   // phases issued so far per stream
+#ifdef AFNO_TIMING
+    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#endif
+    DBG_T0();
+    for (int t = 0; t < T; ++t) {
+      const int stream = t & 1, u = t >> 1, pair = u / NS, stg = u - pair * NS;
+      const int i = 2 * pair + stream;
+      if (i >= n) continue;
+      const uint32_t Dre = tmem + kSlot * (uint32_t)((3 * t) % 5), Dim = tmem + kSlot * (uint32_t)((3 * t + 1) % 5);
+      const uint32_t SA = tmem + kSlot * (uint32_t)((3 * t + 4) % 5);   // slot of phase t - 2
+      const uint32_t cs = stream ? cs1 : cs0;
+      if (cs > 0) mbar_wait(&bars.edone[stream], (cs - 1) & 1u);
+      DBG_ACC(0);
+      const int buf = i % 3;
+      const uint32_t use = (uint32_t)(i / 3);
+      const uint32_t tile = aT + buf * kTileBytes;
+      const bool first = stg == 0, dftg = BACKWARD && stg == 3, last = stg == NS - 1;
+      if (first) mbar_wait(&bars.xfull[buf], use & 1u);
+      if (dftg) mbar_wait(&bars.gfull[buf], use & 1u);
+      DBG_ACC(1);
+      if (elect_one()) {
+        tc_fence_after();
+        if (first || dftg) {
+          issue_fwd_dft2(Dre, Dim, aCh, aSh, tile);
+        } else if (last) {
+          issue_inv_dft2(Dre, Dim, aCh, aSh, tile);
+        } else if (stg == 1) {
+          issue_mlp2<false>(Dre, Dim, SA, w1r, w1i);
+        } else if (stg == 2) {
+          issue_mlp2<false>(Dre, Dim, SA, w2r, w2i);
+        } else if (stg == 4) {
+          issue_mlp2<true>(Dre, Dim, SA, w2r, w2i);    // G1 = G2 W2^H
+        } else {
+          issue_mlp2<true>(Dre, Dim, SA, w1r, w1i);    // GX = G1 W1^H
+        }
+        mma_commit(&bars.dfull[stream]);
+        if (BACKWARD && first) mma_commit(&bars.xfree[buf]);
+        if (last) mma_commit(&bars.tfree[buf]);
+      }
+      __syncwarp();
+      DBG_ACC(2);
+      if (stream) ++cs1; else ++cs0;
+    }
+#ifdef AFNO_TIMING
+    if (blockIdx.x == 0 && lane == 0) {
+      for (int q = 0; q < 8; ++q) g_afno_dbg[(BACKWARD ? 80 : 64) + q] = dbg_acc[q];
+      g_afno_dbg[(BACKWARD ? 80 : 64) + 7] = n;
+    }
+#endif
+  } else {
+    // ================================ epilogue warps =========================================
+    const int cq = warp >> 2;              // column quarter: 0 re lo, 1 re hi, 2 im lo, 3 im hi
+    const int half = cq >> 1, chalf = cq & 1;
+    const int r = lq * 32 + lane;
+    const uint32_t lane_sel = (uint32_t)(lq * 32) << 16;
+    const int kappa = (r <= p.H / 2) ? r : p.H - r;
+    const bool row_valid = r < p.H;
+    const bool row_kept = row_valid && (kappa < p.Kh);
+    const int chunk0 = half * 12 + chalf * 6;            // first 16-byte chunk (8 columns) of this warp's 48 columns
+    const float* bias1 = sBias + half * BS + chalf * 48;
+    const float* bias2 = bias1 + NT;
+    const uint32_t bar_id = 1 + lq;
+    uint64_t m1[2] = {0, 0}, m2[2] = {0, 0};
+    uint32_t ce[2] = {0, 0};
+#ifdef AFNO_TIMING
+    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#endif
+    DBG_T0();
+    for (int u = 0; u < T / 2; ++u) {
+      const int pair = u / NS, stg = u - pair * NS;
+#pragma unroll
+      for (int stream = 0; stream < 2; ++stream) {
+        const int t = 2 * u + stream;
+        const int i = 2 * pair + stream;
+        if (i >= n) continue;
+        const int rem = s0 + i * S;
+        const uint32_t src = tmem + lane_sel + kSlot * (uint32_t)((3 * t + half) % 5) + chalf * 48;
+        const uint32_t dstA = tmem + lane_sel + kSlot * (uint32_t)((3 * t) % 5) + 24 * cq;
+        uint8_t* tile = sT + (i % 3) * kTileBytes;
+        const size_t img_off = ((size_t)rem * p.nb + j) * kTileBytes;
+        const size_t row_off = (((size_t)rem * p.nb + j) * p.H + r) * NT + half * BS + chalf * 48;
+        mbar_wait(&bars.dfull[stream], ce[stream] & 1u);
+        ++ce[stream];
+        DBG_ACC(0);
+        tc_fence_after();
+        uint32_t v[48], pk[24];
+        ld48(src, v);
+        bool writes_a = false;
+        if (stg == 0) {
+          // ---- spectrum Xh ----
+          pack48(v, pk);
+          writes_a = true;
+          if (BACKWARD) store_chunks6((uint8_t*)p.Xh + img_off, chunk0, r, pk);
+        } else if (stg == 1) {
+          // ---- O1 = relu(P1 + b1) ----
+          uint64_t bits = 0;
+#pragma unroll
+          for (int q = 0; q < 12; ++q) {
+            const float4 bq = *(const float4*)(bias1 + 4 * q);
+            const float a0 = __uint_as_float(v[4 * q]) + bq.x, a1 = __uint_as_float(v[4 * q + 1]) + bq.y;
+            const float a2 = __uint_as_float(v[4 * q + 2]) + bq.z, a3 = __uint_as_float(v[4 * q + 3]) + bq.w;
+            if (BACKWARD)
+              bits |= (uint64_t)((a0 > 0.f ? 1u : 0u) | (a1 > 0.f ? 2u : 0u) | (a2 > 0.f ? 4u : 0u) | (a3 > 0.f ? 8u : 0u)) << (4 * q);
+            pk[2 * q] = pack_bf16(fmaxf(a0, 0.f), fmaxf(a1, 0.f));
+            pk[2 * q + 1] = pack_bf16(fmaxf(a2, 0.f), fmaxf(a3, 0.f));
+          }
+          m1[stream] = bits;
+          writes_a = true;
+          if (BACKWARD) store_chunks6((uint8_t*)p.O1 + img_off, chunk0, r, pk);
+        } else if (stg == 2) {
+          // ---- P2 + b2: forward Z = softshrink (truncated) -> B operand of the inverse transform;
+          //      backward: only the mask ----
+          uint64_t bits = 0;
+#pragma unroll
+          for (int q = 0; q < 12; ++q) {
+            const float4 bq = *(const float4*)(bias2 + 4 * q);
+            float a[4] = {__uint_as_float(v[4 * q]) + bq.x, __uint_as_float(v[4 * q + 1]) + bq.y,
+                          __uint_as_float(v[4 * q + 2]) + bq.z, __uint_as_float(v[4 * q + 3]) + bq.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const float m = fabsf(a[e]) - p.lambda;
+              const bool on = row_kept && m > 0.f;
+              if (BACKWARD) bits |= (uint64_t)(on ? 1u : 0u) << (4 * q + e);
+              a[e] = on ? copysignf(m, a[e]) : 0.f;
+            }
+            pk[2 * q] = pack_bf16(a[0], a[1]);
+            pk[2 * q + 1] = pack_bf16(a[2], a[3]);
+          }
+          m2[stream] = bits;
+          if (!BACKWARD) {
+            store_chunks6(tile, chunk0, r, pk);
+            fence_async_smem();
+          }
+        } else if (!BACKWARD || stg == 6) {
+          // ---- last stage: rows of A2 ----
+          pack48(v, pk);
+          if (row_valid) {
+            stg256(p.A2 + row_off, pk);
+            stg256(p.A2 + row_off + 16, pk + 8);
+            stg256(p.A2 + row_off + 32, pk + 16);
+          }
+        } else if (stg == 3 || stg == 4) {
+          // ---- G2 = G (.) mask2 ; G1 = mask1 (.) (G2 W2^H) ----
+          const uint64_t bits = stg == 3 ? m2[stream] : m1[stream];
+#pragma unroll
+          for (int q = 0; q < 24; ++q)
+            pk[q] = pack_bf16((bits >> (2 * q)) & 1u ? __uint_as_float(v[2 * q]) : 0.f,
+                              (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[2 * q + 1]) : 0.f);
+          writes_a = true;
+          store_chunks6((uint8_t*)(stg == 3 ? p.G2 : p.G1) + img_off, chunk0, r, pk);
+        } else {
+          // ---- stage 5: GX -> B operand of the inverse transform (the tile's own buffer) ----
+#pragma unroll
+          for (int q = 0; q < 24; ++q)
+            pk[q] = row_valid ? pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1])) : 0u;
+          store_chunks6(tile, chunk0, r, pk);
+          fence_async_smem();
+          if (EXPORT && row_valid) {
+            const int b = rem / p.Kw, kw = rem - b * p.Kw;
+            const size_t base = ((((size_t)b * p.H + r) * p.Wh + kw) * (size_t)(p.nb * BS) + (size_t)j * BS + chalf * 48) * 2 + half;
+#pragma unroll 4
+            for (int q = 0; q < 48; ++q) {
+              p.mask1[base + (size_t)q * 2] = (uint8_t)((m1[stream] >> q) & 1u);
+              p.mask2[base + (size_t)q * 2] = (uint8_t)((m2[stream] >> q) & 1u);
+            }
+          }
+        }
+        if (writes_a) {
+          // the four warps of this lane quarter have their accumulator columns in registers:
+          // compact the bf16 operand into the first slot (columns of the other warps' sources)
+          asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
+          st24(dstA, pk);
+          tmem_wait_st();
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars.edone[stream]);
+        DBG_ACC(1);
+      }
+    }
+#ifdef AFNO_TIMING
+    if (blockIdx.x == 0 && tid == 0)
+      for (int q = 0; q < 8; ++q) g_afno_dbg[(BACKWARD ? 88 : 72) + q] = dbg_acc[q];
 #endif
   }
   tc_fence_before();
@@ -1023,6 +1396,15 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
       dft[off] = host_bf16(cos(a) * s);
       dft[kDftBytes / 2 + off] = host_bf16(sin(a) * s);
     }
+  // compact images for tc_mix2: only 96 rows stored, order [k/8][m/8 < 12]
+  std::vector<uint16_t> dft2(2 * kDft2Bytes / 2, 0);
+  for (int r = 0; r < H; ++r)
+    for (int h = 0; h < H; ++h) {
+      const double a = two_pi * (double)((long)r * h % H) / (double)H, s = 1.0 / sqrt((double)H);
+      const uint32_t off = ((h / 8) * kDft2Lbo + (r / 8) * kDft2Sbo + (r % 8) * 16 + (h % 8) * 2) / 2;
+      dft2[off] = host_bf16(cos(a) * s);
+      dft2[kDft2Bytes / 2 + off] = host_bf16(sin(a) * s);
+    }
   // W-direction constants as K-major A operands, two 128-row halves each (kFwHalf bytes):
   //   Fw  half ri : element (m = kw, k = w)          = {cos, -sin}(2 pi kw w / W) / sqrt(W)   [x alpha_kw]
   //   Gw  half a  : element (m = w - 128 a, k = ri*96 + kw) = alpha_kw {cos, -sin}(...) / sqrt(W)  [or alpha = 1]
@@ -1043,6 +1425,7 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
       }
     }
   cudaError_t e = upload(dft, &out->dft);
+  if (e == cudaSuccess) e = upload(dft2, &out->dft2);
   if (e == cudaSuccess) e = upload(fw, &out->fw);
   if (e == cudaSuccess) e = upload(fwa, &out->fw_alpha);
   if (e == cudaSuccess) e = upload(gw, &out->gw);
@@ -1052,13 +1435,25 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
   if (e == cudaSuccess) e = set_smem(tc_mix<false, false>, kMixSmem2);
   if (e == cudaSuccess) e = set_smem(tc_mix<true, false>, kMixSmem2);
   if (e == cudaSuccess) e = set_smem(tc_mix<true, true>, kMixSmem2);
+  if (e == cudaSuccess) e = set_smem(tc_mix2<false, false>, kMix2Smem);
+  if (e == cudaSuccess) e = set_smem(tc_mix2<true, false>, kMix2Smem);
+  if (e == cudaSuccess) e = set_smem(tc_mix2<true, true>, kMix2Smem);
   if (e == cudaSuccess) e = set_smem(tc_wgrad, kWgSmem);
+  out->mix_v1 = getenv("AFNO_MIX_V1") != nullptr;
   int dev = 0, sms = 148;
   if (e == cudaSuccess) e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   out->num_sms = sms;
   out->valid = (e == cudaSuccess);
   return e;
+}
+
+// CTAs per channel block of tc_mix2 (every CTA works on one block)
+static int mix2_split(const Geometry& g, const TcPlan& tp) {
+  int S = tp.num_sms / g.nb;
+  if (S < 1) S = 1;
+  if (S > g.B * g.Kw) S = g.B * g.Kw;
+  return S;
 }
 
 size_t tc_workspace_bytes(const Geometry& g, bool backward) {
@@ -1091,7 +1486,13 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   const int mix_tiles = g.nb * g.B * g.Kw;
   const int grid_mix = mix_tiles < tp.num_sms ? mix_tiles : tp.num_sms;
   prof_begin("tc_mix_fwd", st);
-  tc_mix<false, false><<<grid_mix, kMixThreads, kMixSmem2, st>>>(mp);
+  if (tp.mix_v1) {
+    tc_mix<false, false><<<grid_mix, kMixThreads, kMixSmem2, st>>>(mp);
+  } else {
+    const int S2 = mix2_split(g, tp);
+    mp.dft = tp.dft2;
+    tc_mix2<false, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2);
+  }
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -1137,10 +1538,20 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
   const int mix_tiles = g.nb * g.B * g.Kw;
   const int grid_mix = mix_tiles < tp.num_sms ? mix_tiles : tp.num_sms;
-  if (g.export_masks) {
-    TC_LAUNCH("tc_mix_bwd", tc_mix<true, true><<<grid_mix, kMixThreads, kMixSmem2, st>>>(mp));
+  if (tp.mix_v1) {
+    if (g.export_masks) {
+      TC_LAUNCH("tc_mix_bwd", tc_mix<true, true><<<grid_mix, kMixThreads, kMixSmem2, st>>>(mp));
+    } else {
+      TC_LAUNCH("tc_mix_bwd", tc_mix<true, false><<<grid_mix, kMixThreads, kMixSmem2, st>>>(mp));
+    }
   } else {
-    TC_LAUNCH("tc_mix_bwd", tc_mix<true, false><<<grid_mix, kMixThreads, kMixSmem2, st>>>(mp));
+    const int S2 = mix2_split(g, tp);
+    mp.dft = tp.dft2;
+    if (g.export_masks) {
+      TC_LAUNCH("tc_mix_bwd", tc_mix2<true, true><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
+    } else {
+      TC_LAUNCH("tc_mix_bwd", tc_mix2<true, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
+    }
   }
   // B4 / B6: parameter gradients
   const int nred = nW + g.nb * BS;
@@ -1160,7 +1571,7 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
 
 #ifdef AFNO_TIMING
 extern "C" int afno_debug_read(long long* out) {
-  return (int)cudaMemcpyFromSymbol(out, g_afno_dbg, sizeof(long long) * 32);
+  return (int)cudaMemcpyFromSymbol(out, g_afno_dbg, sizeof(long long) * 96);
 }
 #endif
 

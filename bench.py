@@ -217,11 +217,17 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     launches = [0]
 
+    # a training step: fwd keeps the W-direction spectrum of x in the workspace, bwd reads it
+    # (SURVEY.md S8(a) row B1 "or load saved context"); --stateless times the recomputing bwd
+    ctx = not args.stateless
+    desc_f = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_SAVE_CONTEXT}) if ctx else desc
+    desc_b = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_USE_CONTEXT}) if ctx else desc
+
     def step(i):
         s = sets[i % NSETS]
-        binding.afno_spectral_fwd(desc, s["x"], *params, s["y"], ws_f, stream)
+        binding.afno_spectral_fwd(desc_f, s["x"], *params, s["y"], ws_b if ctx else ws_f, stream)
         n = binding.afno_last_launch_count()
-        binding.afno_spectral_bwd(desc, s["x"], s["dy"], *params, s["dx"], *grads, ws_b, stream)
+        binding.afno_spectral_bwd(desc_b, s["x"], s["dy"], *params, s["dx"], *grads, ws_b, stream)
         launches[0] = n + binding.afno_last_launch_count()
 
     def barrier():
@@ -320,7 +326,8 @@ def run_ours(args):
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[4]: {wl.name}", "B_per_gpu": B, "H": wl.H, "W": wl.W,
                        "C": wl.C, "num_blocks": wl.num_blocks, "lambda": wl.lam, "kept_fraction": wl.kept_fraction,
-                       "path": path, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "path": path, "backward": "saved context (W-direction spectrum of x kept by fwd)" if ctx
+                       else "stateless (recomputes the spectrum of x)", "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": f"{NSETS} rotating input/output buffer sets of {4 * x0.numel() * 2 / 1e6:.0f} MB "
                              "each (> 126 MB L2), no explicit flush"},
             "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches[0] * args.steps,
@@ -400,6 +407,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--stateless", action="store_true",
+                    help="time the stateless afno_spectral_bwd (recomputes F1) instead of the saved-context step")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

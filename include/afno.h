@@ -56,7 +56,16 @@ enum {
   AFNO_FLAG_NO_RESIDUAL = 1,     /* test aid: y = s, dx = branch only (no "+ x", no "+ dy")   */
   AFNO_FLAG_ACCUM_GRADS = 2,     /* dw1, db1, dw2, db2 += instead of =                        */
   AFNO_FLAG_FORCE_FP32_MATH = 4, /* bf16 I/O but fp32 FFT + fp32 FFMA MLP (generic path)      */
-  AFNO_FLAG_EXPORT_MASKS = 8     /* bwd only: write ReLU / softshrink masks, see below        */
+  AFNO_FLAG_EXPORT_MASKS = 8,    /* bwd only: write ReLU / softshrink masks, see below        */
+  /* Saved context (SURVEY.md S8(a) row B1 "or load saved context"): a training step calls fwd
+   * and then bwd on the same x.  fwd with SAVE_CONTEXT needs a workspace of
+   * afno_spectral_workspace_bytes(d, 1) bytes and leaves the W-direction half-spectrum of x
+   * (row F1) in it; bwd with USE_CONTEXT on the SAME workspace, with the same descriptor
+   * (the two context flags aside) and the same x, reads it instead of recomputing F1.
+   * Nothing else may write the workspace in between.  Kernel families that keep no such
+   * intermediate (generic-fp32) accept both flags and recompute. */
+  AFNO_FLAG_SAVE_CONTEXT = 16,
+  AFNO_FLAG_USE_CONTEXT = 32
 };
 
 typedef struct {

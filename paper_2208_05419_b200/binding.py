@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libafno_b200.so")
 AFNO_OK, AFNO_ERR_INVALID_ARG, AFNO_ERR_UNSUPPORTED, AFNO_ERR_WORKSPACE, AFNO_ERR_CUDA = range(5)
 AFNO_F32, AFNO_BF16 = 0, 1
 FLAG_NO_RESIDUAL, FLAG_ACCUM_GRADS, FLAG_FORCE_FP32_MATH, FLAG_EXPORT_MASKS = 1, 2, 4, 8
+FLAG_SAVE_CONTEXT, FLAG_USE_CONTEXT = 16, 32
 
 # every symbol include/afno.h declares (tests check that the library exports all of them)
 EXPORTS = [

@@ -46,7 +46,7 @@ int resolve(const afno_desc_t* d, Geometry* g) {
     return fail(AFNO_ERR_INVALID_ARG, "kept_fraction must be in (0, 1]");
   if (d->dtype != AFNO_F32 && d->dtype != AFNO_BF16) return fail(AFNO_ERR_INVALID_ARG, "unknown dtype");
   if (d->flags & ~(uint32_t)(AFNO_FLAG_NO_RESIDUAL | AFNO_FLAG_ACCUM_GRADS | AFNO_FLAG_FORCE_FP32_MATH |
-                             AFNO_FLAG_EXPORT_MASKS))
+                             AFNO_FLAG_EXPORT_MASKS | AFNO_FLAG_SAVE_CONTEXT | AFNO_FLAG_USE_CONTEXT))
     return fail(AFNO_ERR_INVALID_ARG, "unknown flag bits");
   if ((long long)d->B * d->H * d->W >= (1LL << 31) / 4)
     return fail(AFNO_ERR_UNSUPPORTED, "B*H*W too large for 32-bit token indexing");
@@ -72,6 +72,8 @@ int resolve(const afno_desc_t* d, Geometry* g) {
   g->accum = (d->flags & AFNO_FLAG_ACCUM_GRADS) != 0;
   g->export_masks = (d->flags & AFNO_FLAG_EXPORT_MASKS) != 0;
   g->force_fp32 = (d->flags & AFNO_FLAG_FORCE_FP32_MATH) != 0;
+  g->save_ctx = (d->flags & AFNO_FLAG_SAVE_CONTEXT) != 0;
+  g->use_ctx = (d->flags & AFNO_FLAG_USE_CONTEXT) != 0;
   const char* why = nullptr;
   if (!generic_supported(*g, &why)) return fail(AFNO_ERR_UNSUPPORTED, why);
   return AFNO_OK;
@@ -313,8 +315,9 @@ int afno_spectral_fwd(const afno_desc_t* d, const void* x, const float* w1, cons
   for (const void* p : ptrs)
     if (!aligned16(p)) return fail(AFNO_ERR_INVALID_ARG, "pointers must be 16-byte aligned");
   if (overlaps(x, y, act_bytes(g))) return fail(AFNO_ERR_INVALID_ARG, "y must not alias x");
-  if (workspace_bytes < afno::workspace_bytes(g, false))
-    return fail(AFNO_ERR_WORKSPACE, "workspace smaller than afno_spectral_workspace_bytes(d, 0)");
+  if (workspace_bytes < afno::workspace_bytes(g, g.save_ctx))
+    return fail(AFNO_ERR_WORKSPACE, g.save_ctx ? "AFNO_FLAG_SAVE_CONTEXT needs a workspace of afno_spectral_workspace_bytes(d, 1)"
+                                               : "workspace smaller than afno_spectral_workspace_bytes(d, 0)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   bool may_build = false;
   rc = stream_may_build(st, &may_build);

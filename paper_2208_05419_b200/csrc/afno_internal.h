@@ -26,7 +26,7 @@ struct Geometry {
   int Wh, Kh, Kw;
   float lambda;
   float scale; // 1/sqrt(H*W)
-  bool bf16, no_residual, accum, export_masks, force_fp32;
+  bool bf16, no_residual, accum, export_masks, force_fp32, save_ctx, use_ctx;
   long long modes_all() const { return (long long)B * H * Wh; }
   long long rows() const { return (long long)B * H * Kw; } // rows of the stored spectra
 };

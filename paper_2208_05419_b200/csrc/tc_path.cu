@@ -18,6 +18,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <type_traits>
 #include <vector>
 
 #include "afno_internal.h"
@@ -110,7 +111,7 @@ __device__ __forceinline__ void stg256(void* p, const uint32_t* r) {
 }
 
 #ifdef AFNO_TIMING
-__device__ long long g_afno_dbg[96];
+__device__ long long g_afno_dbg[128];
 #define DBG_T0() long long dbg_t = clock64()
 #define DBG_ACC(slot) do { long long n_ = clock64(); dbg_acc[slot] += n_ - dbg_t; dbg_t = n_; } while (0)
 #else
@@ -896,6 +897,47 @@ __device__ __forceinline__ void store_chunks6(uint8_t* base, int chunk0, int r, 
     *(uint4*)(base + (chunk0 + g) * kTileSbo + r * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
 }
 
+// relu + one rounding of two fp32 values to a packed bf16 pair (lo, hi)
+__device__ __forceinline__ uint32_t pack_relu_bf16(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+// Activation masks of a thread's 48 columns: pair p (columns 2p, 2p+1) -> word p / 12, bits
+// 15 - p % 12 (even column) and 31 - p % 12 (odd column).  `q` is a packed pair of NON-NEGATIVE
+// bf16 values; a value is "on" iff it is non-zero (adding 0x7fff carries into the sign bit).
+template <int P>
+__device__ __forceinline__ void mask_collect(uint32_t (&m)[2], uint32_t q) {
+  constexpr int s = P % 12;
+  m[P / 12] |= ((q + 0x7FFF7FFFu) >> s) & (0x80008000u >> s);
+}
+// packed bf16 pair with the halves whose mask bit is clear zeroed
+template <int P>
+__device__ __forceinline__ uint32_t mask_apply(const uint32_t (&m)[2], uint32_t val) {
+  constexpr int s = P % 12;
+  uint32_t mk;
+  // prmt default mode: selector nibble 8 + k = sign of byte k replicated; bytes 1, 3 -> (0,1), (2,3)
+  asm("prmt.b32 %0, %1, %2, 0xBB99;" : "=r"(mk) : "r"(m[P / 12] << s), "r"(0u));
+  return val & mk;
+}
+template <int P>
+__device__ __forceinline__ uint32_t mask_bit(const uint32_t (&m)[2], int odd) {
+  return (m[P / 12] >> (15 - P % 12 + 16 * odd)) & 1u;
+}
+template <int P>
+struct MaskLoop {
+  template <typename F>
+  static __device__ __forceinline__ void run(F&& f) {
+    f(std::integral_constant<int, P>{});
+    if constexpr (P + 1 < 24) MaskLoop<P + 1>::run(f);
+  }
+};
+// mbarrier wait without the nanosleep back-off (the ping-pong hand-offs are latency critical)
+__device__ __forceinline__ void mbar_wait_fast(uint64_t* mbar, uint32_t parity) {
+  while (!mbar_try_wait(mbar, parity)) {
+  }
+}
+
 template <bool BACKWARD, bool EXPORT>
 __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
   extern __shared__ __align__(1024) uint8_t smem[];
@@ -994,7 +1036,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
       const uint32_t Dre = tmem + kSlot * (uint32_t)((3 * t) % 5), Dim = tmem + kSlot * (uint32_t)((3 * t + 1) % 5);
       const uint32_t SA = tmem + kSlot * (uint32_t)((3 * t + 4) % 5);   // slot of phase t - 2
       const uint32_t cs = stream ? cs1 : cs0;
-      if (cs > 0) mbar_wait(&bars.edone[stream], (cs - 1) & 1u);
+      if (cs > 0) mbar_wait_fast(&bars.edone[stream], (cs - 1) & 1u);
       DBG_ACC(0);
       const int buf = i % 3;
       const uint32_t use = (uint32_t)(i / 3);
@@ -1045,10 +1087,11 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
     const float* bias1 = sBias + half * BS + chalf * 48;
     const float* bias2 = bias1 + NT;
     const uint32_t bar_id = 1 + lq;
-    uint64_t m1[2] = {0, 0}, m2[2] = {0, 0};
+    uint32_t m1[2][2] = {{0, 0}, {0, 0}}, m2[2][2] = {{0, 0}, {0, 0}};   // [stream][word]
     uint32_t ce[2] = {0, 0};
 #ifdef AFNO_TIMING
     long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long dbg_m[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 #endif
     DBG_T0();
     for (int u = 0; u < T / 2; ++u) {
@@ -1064,12 +1107,13 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
         uint8_t* tile = sT + (i % 3) * kTileBytes;
         const size_t img_off = ((size_t)rem * p.nb + j) * kTileBytes;
         const size_t row_off = (((size_t)rem * p.nb + j) * p.H + r) * NT + half * BS + chalf * 48;
-        mbar_wait(&bars.dfull[stream], ce[stream] & 1u);
+        mbar_wait_fast(&bars.dfull[stream], ce[stream] & 1u);
         ++ce[stream];
         DBG_ACC(0);
         tc_fence_after();
         uint32_t v[48], pk[24];
         ld48(src, v);
+        DBG_ACC(2);
         bool writes_a = false;
         if (stg == 0) {
           // ---- spectrum Xh ----
@@ -1078,43 +1122,48 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
           if (BACKWARD) store_chunks6((uint8_t*)p.Xh + img_off, chunk0, r, pk);
         } else if (stg == 1) {
           // ---- O1 = relu(P1 + b1) ----
-          uint64_t bits = 0;
 #pragma unroll
           for (int q = 0; q < 12; ++q) {
             const float4 bq = *(const float4*)(bias1 + 4 * q);
-            const float a0 = __uint_as_float(v[4 * q]) + bq.x, a1 = __uint_as_float(v[4 * q + 1]) + bq.y;
-            const float a2 = __uint_as_float(v[4 * q + 2]) + bq.z, a3 = __uint_as_float(v[4 * q + 3]) + bq.w;
-            if (BACKWARD)
-              bits |= (uint64_t)((a0 > 0.f ? 1u : 0u) | (a1 > 0.f ? 2u : 0u) | (a2 > 0.f ? 4u : 0u) | (a3 > 0.f ? 8u : 0u)) << (4 * q);
-            pk[2 * q] = pack_bf16(fmaxf(a0, 0.f), fmaxf(a1, 0.f));
-            pk[2 * q + 1] = pack_bf16(fmaxf(a2, 0.f), fmaxf(a3, 0.f));
+            pk[2 * q] = pack_relu_bf16(__uint_as_float(v[4 * q]) + bq.x, __uint_as_float(v[4 * q + 1]) + bq.y);
+            pk[2 * q + 1] = pack_relu_bf16(__uint_as_float(v[4 * q + 2]) + bq.z, __uint_as_float(v[4 * q + 3]) + bq.w);
           }
-          m1[stream] = bits;
+          if (BACKWARD) {
+            m1[stream][0] = m1[stream][1] = 0;
+            MaskLoop<0>::run([&](auto P) { mask_collect<decltype(P)::value>(m1[stream], pk[decltype(P)::value]); });
+          }
           writes_a = true;
           if (BACKWARD) store_chunks6((uint8_t*)p.O1 + img_off, chunk0, r, pk);
         } else if (stg == 2) {
           // ---- P2 + b2: forward Z = softshrink (truncated) -> B operand of the inverse transform;
           //      backward: only the mask ----
-          uint64_t bits = 0;
-#pragma unroll
-          for (int q = 0; q < 12; ++q) {
-            const float4 bq = *(const float4*)(bias2 + 4 * q);
-            float a[4] = {__uint_as_float(v[4 * q]) + bq.x, __uint_as_float(v[4 * q + 1]) + bq.y,
-                          __uint_as_float(v[4 * q + 2]) + bq.z, __uint_as_float(v[4 * q + 3]) + bq.w};
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const float m = fabsf(a[e]) - p.lambda;
-              const bool on = row_kept && m > 0.f;
-              if (BACKWARD) bits |= (uint64_t)(on ? 1u : 0u) << (4 * q + e);
-              a[e] = on ? copysignf(m, a[e]) : 0.f;
-            }
-            pk[2 * q] = pack_bf16(a[0], a[1]);
-            pk[2 * q + 1] = pack_bf16(a[2], a[3]);
-          }
-          m2[stream] = bits;
+          const float lam = p.lambda;
           if (!BACKWARD) {
+#pragma unroll
+            for (int q = 0; q < 12; ++q) {
+              const float4 bq = *(const float4*)(bias2 + 4 * q);
+              float a[4] = {__uint_as_float(v[4 * q]) + bq.x, __uint_as_float(v[4 * q + 1]) + bq.y,
+                            __uint_as_float(v[4 * q + 2]) + bq.z, __uint_as_float(v[4 * q + 3]) + bq.w};
+#pragma unroll
+              for (int e = 0; e < 4; ++e) a[e] -= fminf(fmaxf(a[e], -lam), lam);   // S_lambda, exact zeros inside
+              pk[2 * q] = row_kept ? pack_bf16(a[0], a[1]) : 0u;
+              pk[2 * q + 1] = row_kept ? pack_bf16(a[2], a[3]) : 0u;
+            }
             store_chunks6(tile, chunk0, r, pk);
             fence_async_smem();
+          } else {
+#pragma unroll
+            for (int q = 0; q < 12; ++q) {
+              const float4 bq = *(const float4*)(bias2 + 4 * q);
+              // |P2 + b2| - lambda > 0  <=>  the rounded, relu-ed difference is non-zero
+              pk[2 * q] = pack_relu_bf16(fabsf(__uint_as_float(v[4 * q]) + bq.x) - lam,
+                                         fabsf(__uint_as_float(v[4 * q + 1]) + bq.y) - lam);
+              pk[2 * q + 1] = pack_relu_bf16(fabsf(__uint_as_float(v[4 * q + 2]) + bq.z) - lam,
+                                             fabsf(__uint_as_float(v[4 * q + 3]) + bq.w) - lam);
+            }
+            m2[stream][0] = m2[stream][1] = 0;
+            if (row_kept)
+              MaskLoop<0>::run([&](auto P) { mask_collect<decltype(P)::value>(m2[stream], pk[decltype(P)::value]); });
           }
         } else if (!BACKWARD || stg == 6) {
           // ---- last stage: rows of A2 ----
@@ -1126,11 +1175,12 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
           }
         } else if (stg == 3 || stg == 4) {
           // ---- G2 = G (.) mask2 ; G1 = mask1 (.) (G2 W2^H) ----
-          const uint64_t bits = stg == 3 ? m2[stream] : m1[stream];
-#pragma unroll
-          for (int q = 0; q < 24; ++q)
-            pk[q] = pack_bf16((bits >> (2 * q)) & 1u ? __uint_as_float(v[2 * q]) : 0.f,
-                              (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[2 * q + 1]) : 0.f);
+          pack48(v, pk);
+          if (stg == 3) {
+            MaskLoop<0>::run([&](auto P) { pk[decltype(P)::value] = mask_apply<decltype(P)::value>(m2[stream], pk[decltype(P)::value]); });
+          } else {
+            MaskLoop<0>::run([&](auto P) { pk[decltype(P)::value] = mask_apply<decltype(P)::value>(m1[stream], pk[decltype(P)::value]); });
+          }
           writes_a = true;
           store_chunks6((uint8_t*)(stg == 3 ? p.G2 : p.G1) + img_off, chunk0, r, pk);
         } else {
@@ -1143,19 +1193,26 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
           if (EXPORT && row_valid) {
             const int b = rem / p.Kw, kw = rem - b * p.Kw;
             const size_t base = ((((size_t)b * p.H + r) * p.Wh + kw) * (size_t)(p.nb * BS) + (size_t)j * BS + chalf * 48) * 2 + half;
-#pragma unroll 4
-            for (int q = 0; q < 48; ++q) {
-              p.mask1[base + (size_t)q * 2] = (uint8_t)((m1[stream] >> q) & 1u);
-              p.mask2[base + (size_t)q * 2] = (uint8_t)((m2[stream] >> q) & 1u);
-            }
+            MaskLoop<0>::run([&](auto P) {
+              constexpr int pp = decltype(P)::value;
+              p.mask1[base + (size_t)(2 * pp) * 2] = (uint8_t)mask_bit<pp>(m1[stream], 0);
+              p.mask1[base + (size_t)(2 * pp + 1) * 2] = (uint8_t)mask_bit<pp>(m1[stream], 1);
+              p.mask2[base + (size_t)(2 * pp) * 2] = (uint8_t)mask_bit<pp>(m2[stream], 0);
+              p.mask2[base + (size_t)(2 * pp + 1) * 2] = (uint8_t)mask_bit<pp>(m2[stream], 1);
+            });
           }
         }
+#ifdef AFNO_TIMING
+        { long long n_ = clock64(); dbg_m[stg] += n_ - dbg_t; dbg_t = n_; }
+#endif
         if (writes_a) {
           // the four warps of this lane quarter have their accumulator columns in registers:
           // compact the bf16 operand into the first slot (columns of the other warps' sources)
           asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
+          DBG_ACC(4);
           st24(dstA, pk);
           tmem_wait_st();
+          DBG_ACC(5);
         }
         tc_fence_before();
         __syncwarp();
@@ -1165,7 +1222,10 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
     }
 #ifdef AFNO_TIMING
     if (blockIdx.x == 0 && tid == 0)
-      for (int q = 0; q < 8; ++q) g_afno_dbg[(BACKWARD ? 88 : 72) + q] = dbg_acc[q];
+      for (int q = 0; q < 8; ++q) {
+        g_afno_dbg[(BACKWARD ? 88 : 72) + q] = dbg_acc[q];
+        g_afno_dbg[(BACKWARD ? 104 : 96) + q] = dbg_m[q];
+      }
 #endif
   }
   tc_fence_before();
@@ -1462,7 +1522,8 @@ size_t tc_workspace_bytes(const Geometry& g, bool backward) {
 
 cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const float* w1, const float* b1,
                        const float* w2, const float* b2, void* y, void* ws, cudaStream_t st) {
-  TcWs w = tc_carve(g, false, (char*)ws);
+  // SAVE_CONTEXT: the backward layout, so that tc_backward finds A1 where it expects it
+  TcWs w = tc_carve(g, g.save_ctx, (char*)ws);
   const TcPlan& tp = p.tc;
   cudaError_t e;
   const int nW = g.nb * BS * BS;
@@ -1525,8 +1586,10 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   const int row_tiles = g.B * g.H * ncg;
   const int grid_row = row_tiles < tp.num_sms ? row_tiles : tp.num_sms;
   // B1 (first half) and B2: W-direction spectra of x and of dy (alpha-weighted)
-  TC_LAUNCH("tc_wdft_fwd", tc_wdft<false><<<grid_row, kRowThreads, kRowSmem, st>>>((const __nv_bfloat16*)x, nullptr, w.A1,
-                                                                                  tp.fw, g.B, g.H, g.W, g.C, g.Kw, g.nb));
+  if (!g.use_ctx) {
+    TC_LAUNCH("tc_wdft_fwd", tc_wdft<false><<<grid_row, kRowThreads, kRowSmem, st>>>((const __nv_bfloat16*)x, nullptr, w.A1,
+                                                                                    tp.fw, g.B, g.H, g.W, g.C, g.Kw, g.nb));
+  }
   TC_LAUNCH("tc_wdft_fwd", tc_wdft<false><<<grid_row, kRowThreads, kRowSmem, st>>>((const __nv_bfloat16*)dy, nullptr, w.A1g,
                                                                                   tp.fw_alpha, g.B, g.H, g.W, g.C, g.Kw, g.nb));
   MixParams mp{};
@@ -1571,7 +1634,7 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
 
 #ifdef AFNO_TIMING
 extern "C" int afno_debug_read(long long* out) {
-  return (int)cudaMemcpyFromSymbol(out, g_afno_dbg, sizeof(long long) * 96);
+  return (int)cudaMemcpyFromSymbol(out, g_afno_dbg, sizeof(long long) * 128);
 }
 #endif
 

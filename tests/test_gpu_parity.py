@@ -209,6 +209,39 @@ def test_graph_capture_forward_backward(oracle):
     assert np.array_equal(g[0].cpu().numpy(), ref["dw1"])
 
 
+def test_saved_context_backward_matches_stateless():
+    """SURVEY.md S8(a) row B1 "or load saved context": fwd with SAVE_CONTEXT then bwd with USE_CONTEXT
+    on the same workspace gives bit-identical gradients to the stateless bwd (bf16 tcgen05 path,
+    a slice of the headline shape, and the generic path, where the flags are accepted and ignored)."""
+    import torch
+    cases = [(parity.desc_for(inputs.WORKLOADS["fcn_b4_bwd"], B=2), inputs.make_inputs(inputs.WORKLOADS["fcn_b4_bwd"], B=2)),
+             (parity.desc_for(inputs.WORKLOADS["sub_bwd_nb2"]), inputs.make_inputs(inputs.WORKLOADS["sub_bwd_nb2"]))]
+    for desc, data in cases:
+        bf16 = desc.dtype == binding.AFNO_BF16
+        layer = parity.GpuLayer(desc)
+        ref = layer.backward(data["x"], data["dy"], data["w1"], data["b1"], data["w2"], data["b2"], export_masks=False)
+        y_ref = layer.forward(data["x"], data["w1"], data["b1"], data["w2"], data["b2"])
+        d_save = binding.Desc(**{**desc.__dict__, "flags": desc.flags | binding.FLAG_SAVE_CONTEXT})
+        d_use = binding.Desc(**{**desc.__dict__, "flags": desc.flags | binding.FLAG_USE_CONTEXT})
+        ws = torch.empty(binding.afno_spectral_workspace_bytes(desc, True), dtype=torch.uint8, device="cuda")
+        tx, tdy = parity.to_device_act(data["x"], bf16), parity.to_device_act(data["dy"], bf16)
+        ty, tdx = torch.empty_like(tx), torch.empty_like(tx)
+        p = layer.params(data["w1"], data["b1"], data["w2"], data["b2"])
+        g = [torch.zeros_like(t) for t in p]
+        small = torch.empty(binding.afno_spectral_workspace_bytes(desc, False), dtype=torch.uint8, device="cuda")
+        if binding.afno_spectral_workspace_bytes(desc, False) < binding.afno_spectral_workspace_bytes(desc, True):
+            with pytest.raises(binding.AfnoError) as e:
+                binding.afno_spectral_fwd(d_save, tx, *p, ty, small)
+            assert e.value.status == binding.AFNO_ERR_WORKSPACE
+        binding.afno_spectral_fwd(d_save, tx, *p, ty, ws)
+        binding.afno_spectral_bwd(d_use, tx, tdy, *p, tdx, *g, ws)
+        torch.cuda.synchronize()
+        assert np.array_equal(parity.from_device_act(ty), y_ref)
+        assert np.array_equal(parity.from_device_act(tdx), ref["dx"])
+        for t, k in zip(g, ("dw1", "db1", "dw2", "db2")):
+            assert np.array_equal(t.cpu().numpy(), ref[k]), k
+
+
 def test_host_variants_match_device(oracle):
     import torch
     wl = inputs.WORKLOADS["sub_bwd_nb8"]

@@ -35,9 +35,8 @@ struct Geometry {
 struct TcPlan {
   bool valid = false;
   int num_sms = 148;
-  bool mix_v1 = false;   // AFNO_MIX_V1 in the environment: first-generation per-mode kernel (A/B testing)
   uint8_t* dft2 = nullptr;
-  uint8_t *dft = nullptr, *fw = nullptr, *fw_alpha = nullptr, *gw = nullptr, *gw_noalpha = nullptr;
+  uint8_t *fw = nullptr, *fw_alpha = nullptr, *gw = nullptr, *gw_noalpha = nullptr;
 };
 
 struct Plan {

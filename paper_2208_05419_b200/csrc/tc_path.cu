@@ -35,10 +35,9 @@ constexpr int NT = 192;   // (re | im) columns of one block
 constexpr int HP = 96;    // H padded to the K extent of the H-direction GEMMs
 constexpr int WP = 192;   // W padded to the K / N extent of the W-direction GEMMs
 constexpr int CGRP = 128; // channels per W-direction tile (= UMMA M)
+constexpr int kA2Row = NT + 8; // elements per stored row of A2: 192 values + 16 bytes (see kOutStride)
 
 // shared-memory operand geometry (bytes), see tc_common.cuh for the layout formulas
-constexpr uint32_t kDftLbo = 2048, kDftSbo = 128;   // Ch / Sh: K-major A [128 x 96], order [k/8][m/8]
-constexpr uint32_t kDftBytes = 128 * HP * 2;         // 24576
 constexpr uint32_t kWLbo = 1536, kWSbo = 128;       // weights: K-major B [96 x 96], order [k/8][n/8]
 constexpr uint32_t kWBytes = BS * BS * 2;            // 18432
 // mode tile: MN-major B [K=96 rows][N=192]; the 16-byte pad on the chunk stride keeps cp.async
@@ -110,6 +109,12 @@ __device__ __forceinline__ void stg256(void* p, const uint32_t* r) {
                : "memory");
 }
 
+#ifdef AFNO_TRACE
+__device__ long long g_afno_trace[64 * 32];
+#define TR(t, slot) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (t) >= 40 && (t) < 72) g_afno_trace[((t) - 40) * 64 + (slot)] = clock64(); } while (0)
+#else
+#define TR(t, slot)
+#endif
 #ifdef AFNO_TIMING
 __device__ long long g_afno_dbg[128];
 #define DBG_T0() long long dbg_t = clock64()
@@ -176,14 +181,15 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
         for (int w = 2 * sub + (lane >> 4); w < W; w += 2 * kRowProdWarps)
           if (cok) cp_async16(dst + mc * kRowSbo + w * 16, xrow + (size_t)w * C + mc * 8);
       } else {
-        // A2[b][kw][j][h][ri][cl] gathered into the MN-major B operand (K = (ri,kw), N = channel)
+        // A2[b][kw][j][h][ri][cl] (rows kA2Row elements apart) gathered into the MN-major B operand
+        // (K = (ri,kw), N = channel)
         const int b = bh / H, h = bh - b * H;
-        const size_t kwstride = (size_t)nb * H * NT;
-        const __nv_bfloat16* base = in + ((size_t)b * Kw * nb * H + h) * NT;
+        const size_t kwstride = (size_t)nb * H * kA2Row;
+        const __nv_bfloat16* base = in + ((size_t)b * Kw * nb * H + h) * kA2Row;
         const int mc = lane & 15;
         const int c0 = cg * CGRP + mc * 8;
         const int j = c0 / BS, cl = c0 - j * BS;
-        const __nv_bfloat16* cbase = base + (size_t)j * H * NT + cl;
+        const __nv_bfloat16* cbase = base + (size_t)j * H * kA2Row + cl;
         for (int rr = 2 * sub + (lane >> 4); rr < 2 * Kw; rr += 2 * kRowProdWarps) {
           const int ri = rr >= Kw ? 1 : 0, kw = rr - ri * Kw;
           if (c0 < C) cp_async16(dst + mc * kRowSbo + (ri * BS + kw) * 16, cbase + (size_t)kw * kwstride + ri * BS);
@@ -308,89 +314,21 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
-// ---- F2-F7 / B1-B7: per (b, kw, block) GEMM chains in tensor memory --------------------------------
-// CTA = 8 epilogue warps + 1 control warp.
-//   control warp : copies the mode tiles (cp.async), makes them visible to the async proxy and
-//                  issues every tcgen05.mma (lane 0).
-//   epilogue warp w: TMEM lanes 32*(w&3).. (accumulator rows = modes) and column half w>>2
-//                  (0: re, 1: im).  It converts its 96 fp32 accumulator columns of a stage in
-//                  three 32-column chunks, writes each chunk packed to bf16 IN PLACE (columns
-//                  [96*half + 16c, +16) of the same region: the A operand of the next GEMM) and
-//                  arrives on that chunk's mbarrier.
-// The control warp issues the K-steps of the next MLP GEMM chunk by chunk as those barriers
-// complete, so the tensor core runs under the epilogue of the previous stage.  No block-wide
-// barrier is used; all hand-offs are mbarriers.
-// Tensor memory: R0 = columns [0,192), R1 = [256,448); a stage reads its A operand from one
-// region and accumulates into the other.
-constexpr int kMixEpiThreads = 256;
+// ---- F2-F7 / B1-B7: per (b, kw, block) GEMM chains in tensor memory (kernel tc_mix2 below) ----------
 constexpr int kMixLoadWarps = 3;
-constexpr int kMixThreads = kMixEpiThreads + 32 + kMixLoadWarps * 32;   // + control warp + loader warps
-constexpr uint32_t kMixSmem2 = 2 * kDftBytes + 4 * kWBytes + 2 * kTileBytes; // 196608
 
 struct MixParams {
   const __nv_bfloat16* A1;   // forward: spectrum tiles; backward: x tiles
   const __nv_bfloat16* A1g;  // backward: gradient tiles
   __nv_bfloat16* A2;
   __nv_bfloat16 *Xh, *O1, *G2, *G1; // backward: operands of tc_wgrad
-  const uint8_t* dft;        // Ch then Sh, kDftBytes each, smem image
+  const uint8_t* dft;        // Ch then Sh, kDft2Bytes each, smem image
   const uint8_t* wprep;      // per block 4 x kWBytes: W1r, W1i, W2r, W2i (n=o, k=i, K-major)
   const float* bprep;        // per block [2 layers][192]: (re 96 | im 96)
   uint8_t* mask1;            // optional export, [B][H][Wh][C][2]
   uint8_t* mask2;
   int B, H, Kw, Wh, nb, Kh;
   float lambda;
-};
-
-// D[:, 0..96) (+)= A_smem(K-major [128 x 96]) * tile half (MN-major, 96 columns)
-__device__ __forceinline__ void issue_dft(uint32_t d, uint32_t a_base, uint32_t b_base, uint32_t idesc, bool fresh) {
-#pragma unroll
-  for (int ks = 0; ks < HP / 16; ++ks)
-    mma_ss(d, smem_desc(a_base + ks * 2 * kDftLbo, kDftLbo, kDftSbo),
-           smem_desc(b_base + ks * 2 * kTileLbo, kTileLbo, kTileSbo), idesc, !(fresh && ks == 0));
-}
-// forward transform (exp(-i theta)):  Xr = Ch Ar + Sh Ai ; Xi = Ch Ai - Sh Ar
-__device__ __forceinline__ void issue_fwd_dft(uint32_t R, uint32_t aCh, uint32_t aSh, uint32_t tile) {
-  const uint32_t id = idesc_bf16(128, BS, kIdescBMn), half = (BS / 8) * kTileSbo;
-  issue_dft(R, aCh, tile, id, true);
-  issue_dft(R, aSh, tile + half, id, false);
-  issue_dft(R + BS, aCh, tile + half, id, true);
-  issue_dft(R + BS, aSh, tile, id | kIdescNegA, false);
-}
-// inverse transform (exp(+i theta)):  Tr = Ch Zr - Sh Zi ; Ti = Ch Zi + Sh Zr
-__device__ __forceinline__ void issue_inv_dft(uint32_t R, uint32_t aCh, uint32_t aSh, uint32_t tile) {
-  const uint32_t id = idesc_bf16(128, BS, kIdescBMn), half = (BS / 8) * kTileSbo;
-  issue_dft(R, aCh, tile, id, true);
-  issue_dft(R, aSh, tile + half, id | kIdescNegA, false);
-  issue_dft(R + BS, aCh, tile + half, id, true);
-  issue_dft(R + BS, aSh, tile, id, false);
-}
-// K-steps of chunk c (32 source columns of each half = 2 K-steps of 16) of an MLP GEMM.
-//   TRANSPOSED = false:  T = S W      : Tr = Sr Wr - Si Wi ; Ti = Sr Wi + Si Wr
-//   TRANSPOSED = true :  T = S W^H    : Tr = Sr Wr^T + Si Wi^T ; Ti = Si Wr^T - Sr Wi^T
-// (W^H reads the same weight image as an MN-major operand with LBO and SBO exchanged.)
-template <bool TRANSPOSED>
-__device__ __forceinline__ void issue_mlp_chunk(uint32_t T, uint32_t S, uint32_t wr, uint32_t wi, int c) {
-  const uint32_t id = idesc_bf16(128, BS, TRANSPOSED ? kIdescBMn : 0u);
-  const uint32_t lbo = TRANSPOSED ? kWSbo : kWLbo, sbo = TRANSPOSED ? kWLbo : kWSbo;
-#pragma unroll
-  for (int ks = 2 * c; ks < 2 * c + 2; ++ks) {   // re chunk of the A operand
-    const uint32_t acc = ks != 0;
-    mma_ts(T, S + ks * 8, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, acc);
-    mma_ts(T + BS, S + ks * 8, smem_desc(wi + ks * 2 * lbo, lbo, sbo), TRANSPOSED ? (id | kIdescNegB) : id, acc);
-  }
-#pragma unroll
-  for (int ks = 2 * c; ks < 2 * c + 2; ++ks) {   // im chunk
-    mma_ts(T, S + BS + ks * 8, smem_desc(wi + ks * 2 * lbo, lbo, sbo), TRANSPOSED ? id : (id | kIdescNegB), 1u);
-    mma_ts(T + BS, S + BS + ks * 8, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, 1u);
-  }
-}
-
-struct MixBars {
-  uint64_t dfull[8];      // stage s accumulated (tcgen05.commit)
-  uint64_t cready[2][3];  // packed A-operand chunk (half, c) written by all 128 rows
-  uint64_t zready;        // bf16 tile for the inverse transform written to shared memory
-  uint64_t tfull[2];      // tile buffer filled by the loader warp (32 arrivals)
-  uint64_t tfree[2];      // tile buffer consumed by its last GEMM (tcgen05.commit)
 };
 
 // rows of a (b,kw,j) tile [H][192] -> MN-major B operand (K = h, N = (ri, c)); loader warp `sub`
@@ -401,405 +339,6 @@ __device__ __forceinline__ void load_tile_warp(uint32_t tile_saddr, const __nv_b
     const int h = q / (NT / 8), nc = q - h * (NT / 8);
     cp_async16(tile_saddr + nc * kTileSbo + h * 16, src + (size_t)q * 8);
   }
-}
-
-// 64 bytes of a row as two 256-bit stores (full 32-byte sectors; dst is 32-byte aligned)
-__device__ __forceinline__ void store16(__nv_bfloat16* dst, const uint32_t (&pk)[16]) {
-#pragma unroll
-  for (int g = 0; g < 2; ++g)
-    asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(dst + g * 16), "r"(pk[8 * g]),
-                 "r"(pk[8 * g + 1]), "r"(pk[8 * g + 2]), "r"(pk[8 * g + 3]), "r"(pk[8 * g + 4]), "r"(pk[8 * g + 5]),
-                 "r"(pk[8 * g + 6]), "r"(pk[8 * g + 7])
-                 : "memory");
-}
-// chunk c of this thread's row -> operand image of a tile in GLOBAL memory (same byte order as the
-// shared-memory operand: [n/8][row][8]); consecutive rows are consecutive 16-byte pieces, so a warp
-// store covers 512 contiguous bytes, and tc_wgrad fetches the tile with bulk copies
-__device__ __forceinline__ void store_image16(uint8_t* img, int half, int c, int r, const uint32_t (&pk)[16]) {
-#pragma unroll
-  for (int g = 0; g < 4; ++g)
-    *(uint4*)(img + (half * 12 + c * 4 + g) * kTileSbo + r * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
-}
-// chunk c of this thread's row -> MN-major B operand tile (K = row r)
-__device__ __forceinline__ void store_tile16(uint8_t* tile, int half, int c, int r, const uint32_t (&pk)[16]) {
-#pragma unroll
-  for (int g = 0; g < 4; ++g)
-    *(uint4*)(tile + (half * 12 + c * 4 + g) * kTileSbo + r * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
-}
-// publish a packed chunk: TMEM stores complete, ordered before the barrier arrival
-__device__ __forceinline__ void publish_chunk(uint64_t* bar) {
-  tmem_wait_st();
-  tc_fence_before();
-  mbar_arrive(bar);
-}
-
-template <bool BACKWARD, bool EXPORT>
-__global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
-  extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ MixBars bars;
-  __shared__ uint32_t tmem_slot;
-  uint8_t* sCh = smem;
-  uint8_t* sSh = smem + kDftBytes;
-  uint8_t* sW = smem + 2 * kDftBytes;
-  uint8_t* sTileA = sW + 4 * kWBytes;      // fwd: even tiles; bwd: x tile
-  uint8_t* sTileB = sTileA + kTileBytes;   // fwd: odd tiles;  bwd: gradient tile, later GX
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (uint32_t i = tid; i < 2 * kTileBytes / 16; i += kMixThreads) ((uint4*)sTileA)[i] = make_uint4(0, 0, 0, 0);
-  for (uint32_t i = tid; i < 2 * kDftBytes / 16; i += kMixThreads) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
-  if (tid == 0) {
-    for (int s = 0; s < 8; ++s) mbar_init(&bars.dfull[s], 1);
-    for (int h = 0; h < 2; ++h)
-      for (int c = 0; c < 3; ++c) mbar_init(&bars.cready[h][c], kMixEpiThreads / 2);
-    mbar_init(&bars.zready, kMixEpiThreads);
-    for (int b = 0; b < 2; ++b) {
-      mbar_init(&bars.tfull[b], kMixLoadWarps * 32);
-      mbar_init(&bars.tfree[b], 1);
-    }
-    mbar_init_fence();
-  }
-  if (warp == 0) tmem_alloc<512>(&tmem_slot);
-  cp_async_wait_all();
-  fence_async_smem();
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = tmem_slot;
-  const uint32_t R0 = tmem, R1 = tmem + 256;
-  const int ntiles = p.nb * p.B * p.Kw;
-  const int per = (ntiles + gridDim.x - 1) / gridDim.x;
-  const int t_begin = blockIdx.x * per, t_end = min(ntiles, t_begin + per);
-  const int BKw = p.B * p.Kw;
-
-  if (warp >= kMixEpiThreads / 32 + 1) {
-    // ================================ loader warps ============================================
-    // forward : tile i -> buffer i&1 (free once the inverse transform of tile i-2 has completed)
-    // backward: x tile -> buffer A (free after stage 0), gradient tile -> buffer B (free after stage 6)
-    const uint32_t aTA = smem_u32(sTileA), aTB = smem_u32(sTileB);
-    const int sub = warp - (kMixEpiThreads / 32 + 1);
-    for (int t = t_begin; t < t_end; ++t) {
-      const int i = t - t_begin;
-      const int j = t / BKw, rem = t - j * BKw;
-      const size_t off = ((size_t)rem * p.nb + j) * p.H * NT;
-      if (!BACKWARD) {
-        const int b = i & 1, use = i >> 1;
-        if (use > 0) mbar_wait(&bars.tfree[b], (uint32_t)((use - 1) & 1));
-        load_tile_warp(b ? aTB : aTA, p.A1 + off, p.H, lane, sub);
-        cp_async_wait_all();
-        fence_async_smem();
-        mbar_arrive(&bars.tfull[b]);
-      } else {
-        if (i > 0) mbar_wait(&bars.tfree[0], (uint32_t)((i - 1) & 1));
-        load_tile_warp(aTA, p.A1 + off, p.H, lane, sub);
-        cp_async_wait_all();
-        fence_async_smem();
-        mbar_arrive(&bars.tfull[0]);
-        if (i > 0) mbar_wait(&bars.tfree[1], (uint32_t)((i - 1) & 1));
-        load_tile_warp(aTB, p.A1g + off, p.H, lane, sub);
-        cp_async_wait_all();
-        fence_async_smem();
-        mbar_arrive(&bars.tfull[1]);
-      }
-    }
-  } else if (warp == kMixEpiThreads / 32) {
-    // ================================ control warp ===========================================
-    const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW);
-    const uint32_t aTA = smem_u32(sTileA), aTB = smem_u32(sTileB);
-    uint32_t pc = 0;       // parity of the chunk barriers (they complete once per MLP stage)
-    int cur_j = -1;
-#ifdef AFNO_TIMING
-    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-#endif
-    DBG_T0();
-    auto mlp_stage = [&](uint32_t T, uint32_t S, uint32_t wr, uint32_t wi, bool transposed, uint64_t* done) {
-      for (int c = 0; c < 3; ++c) {
-        mbar_wait(&bars.cready[0][c], pc);
-        mbar_wait(&bars.cready[1][c], pc);
-        DBG_ACC(c == 0 ? 1 : 2);
-        if (elect_one()) {
-          tc_fence_after();
-          if (transposed) issue_mlp_chunk<true>(T, S, wr, wi, c);
-          else issue_mlp_chunk<false>(T, S, wr, wi, c);
-        }
-      }
-      if (elect_one()) mma_commit(done);
-      __syncwarp();
-      DBG_ACC(3);
-      pc ^= 1;
-    };
-    for (int t = t_begin; t < t_end; ++t) {
-      const int i = t - t_begin;
-      const uint32_t tp = (uint32_t)(i & 1);          // parity of this tile's per-tile barriers
-      const int j = t / BKw;
-      const uint32_t last = BACKWARD ? 6 : 3;         // index of the chain's final stage
-      if (j != cur_j) {
-        // new channel block: every GEMM of the previous tile is complete, reload the weights
-        cur_j = j;
-        if (i > 0) mbar_wait(&bars.dfull[last], tp ^ 1);
-        const uint8_t* wsrc = p.wprep + (size_t)j * 4 * kWBytes;
-        for (uint32_t q = lane; q < 4 * kWBytes / 16; q += 32) cp_async16(aW + q * 16, wsrc + (size_t)q * 16);
-        cp_async_wait_all();
-        fence_async_smem();
-        __syncwarp();
-      }
-      if (!BACKWARD) {
-        const int b = i & 1;
-        const uint32_t cur_tile = b ? aTB : aTA;
-        mbar_wait(&bars.tfull[b], (uint32_t)((i >> 1) & 1));
-        DBG_ACC(0);
-        if (elect_one()) {
-          tc_fence_after();
-          issue_fwd_dft(R0, aCh, aSh, cur_tile);
-          mma_commit(&bars.dfull[0]);
-        }
-        __syncwarp();
-        DBG_ACC(4);
-        mlp_stage(R1, R0, aW + 0 * kWBytes, aW + 1 * kWBytes, false, &bars.dfull[1]);
-        mlp_stage(R0, R1, aW + 2 * kWBytes, aW + 3 * kWBytes, false, &bars.dfull[2]);
-        mbar_wait(&bars.zready, tp);
-        DBG_ACC(5);
-        if (elect_one()) {
-          tc_fence_after();
-          issue_inv_dft(R1, aCh, aSh, cur_tile);
-          mma_commit(&bars.dfull[3]);
-          mma_commit(&bars.tfree[b]);
-        }
-        __syncwarp();
-        DBG_ACC(4);
-      } else {
-        mbar_wait(&bars.tfull[0], tp);
-        if (elect_one()) {
-          tc_fence_after();
-          issue_fwd_dft(R0, aCh, aSh, aTA);
-          mma_commit(&bars.dfull[0]);
-          mma_commit(&bars.tfree[0]);
-        }
-        __syncwarp();
-        mlp_stage(R1, R0, aW + 0 * kWBytes, aW + 1 * kWBytes, false, &bars.dfull[1]);
-        mlp_stage(R0, R1, aW + 2 * kWBytes, aW + 3 * kWBytes, false, &bars.dfull[2]);
-        // stage 3: G = Fh A1g into R1 (its previous contents, the A operand of stage 2, are dead
-        // once stage 2 has completed)
-        mbar_wait(&bars.dfull[2], tp);
-        mbar_wait(&bars.tfull[1], tp);
-        if (elect_one()) {
-          tc_fence_after();
-          issue_fwd_dft(R1, aCh, aSh, aTB);
-          mma_commit(&bars.dfull[3]);
-        }
-        __syncwarp();
-        mlp_stage(R0, R1, aW + 2 * kWBytes, aW + 3 * kWBytes, true, &bars.dfull[4]);   // G1 = G2 W2^H
-        mlp_stage(R1, R0, aW + 0 * kWBytes, aW + 1 * kWBytes, true, &bars.dfull[5]);   // GX = G1 W1^H
-        mbar_wait(&bars.zready, tp);
-        if (elect_one()) {
-          tc_fence_after();
-          issue_inv_dft(R1, aCh, aSh, aTB);   // into R1: the next tile's stage 0 reuses R0 at once
-          mma_commit(&bars.dfull[6]);
-          mma_commit(&bars.tfree[1]);
-        }
-        __syncwarp();
-      }
-    }
-#ifdef AFNO_TIMING
-    if (!BACKWARD && blockIdx.x == 0 && lane == 0) {
-      for (int q = 0; q < 8; ++q) g_afno_dbg[32 + q] = dbg_acc[q];
-      g_afno_dbg[47] = t_end - t_begin;
-    }
-#endif
-  } else {
-    // ================================ epilogue warps =========================================
-#ifdef AFNO_TIMING
-    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-#endif
-    DBG_T0();
-    const int half = warp >> 2;
-    const int r = (warp & 3) * 32 + lane;
-    const uint32_t lane_base = ((uint32_t)((warp & 3) * 32) << 16) + half * BS;
-    const int kappa = (r <= p.H / 2) ? r : p.H - r;
-    const bool row_valid = r < p.H;
-    const bool row_kept = row_valid && (kappa < p.Kh);
-    for (int t = t_begin; t < t_end; ++t) {
-      const int i = t - t_begin;
-      const uint32_t tp = (uint32_t)(i & 1);
-      const int j = t / BKw, rem = t - j * BKw;
-      const size_t row_off = (((size_t)rem * p.nb + j) * p.H + r) * NT + half * BS;
-      const size_t img_off = ((size_t)rem * p.nb + j) * kTileBytes;   // operand-image tensors (bytes)
-      const float* bias1 = p.bprep + (size_t)j * 2 * NT + half * BS;
-      const float* bias2 = bias1 + NT;
-      uint32_t m1[3], m2[3];
-      // ---- stage 0 -> spectrum Xh, packed in place (R0) ----
-      DBG_ACC(4);
-      mbar_wait(&bars.dfull[0], tp);
-      DBG_ACC(0);
-      tc_fence_after();
-#pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        uint32_t v[32], pk[16];
-        tmem_ld32(R0 + lane_base + 32 * c, v);
-        tmem_wait_ld();
-        pack32(v, pk);
-        tmem_st16(R0 + lane_base + 16 * c, pk);
-        if (BACKWARD && r < HP) store_image16((uint8_t*)p.Xh + img_off, half, c, r, pk);
-        publish_chunk(&bars.cready[half][c]);
-      }
-      // ---- stage 1 -> O1 = relu(P1 + b1), packed in place (R1) ----
-      DBG_ACC(4);
-      mbar_wait(&bars.dfull[1], tp);
-      DBG_ACC(1);
-      tc_fence_after();
-#pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        uint32_t v[32], pk[16];
-        tmem_ld32(R1 + lane_base + 32 * c, v);
-        tmem_wait_ld();
-        uint32_t bits = 0;
-#pragma unroll
-        for (int q = 0; q < 8; ++q) {
-          const float4 bq = __ldg((const float4*)(bias1 + 32 * c + 4 * q));
-          const float a0 = __uint_as_float(v[4 * q]) + bq.x, a1 = __uint_as_float(v[4 * q + 1]) + bq.y;
-          const float a2 = __uint_as_float(v[4 * q + 2]) + bq.z, a3 = __uint_as_float(v[4 * q + 3]) + bq.w;
-          if (BACKWARD)
-            bits |= ((a0 > 0.f ? 1u : 0u) | (a1 > 0.f ? 2u : 0u) | (a2 > 0.f ? 4u : 0u) | (a3 > 0.f ? 8u : 0u)) << (4 * q);
-          pk[2 * q] = pack_bf16(fmaxf(a0, 0.f), fmaxf(a1, 0.f));
-          pk[2 * q + 1] = pack_bf16(fmaxf(a2, 0.f), fmaxf(a3, 0.f));
-        }
-        m1[c] = bits;
-        tmem_st16(R1 + lane_base + 16 * c, pk);
-        if (BACKWARD && r < HP) store_image16((uint8_t*)p.O1 + img_off, half, c, r, pk);
-        publish_chunk(&bars.cready[half][c]);
-      }
-      // ---- stage 2 -> P2 + b2 : forward Z = softshrink -> smem tile ; backward mask2 ----
-      DBG_ACC(4);
-      mbar_wait(&bars.dfull[2], tp);
-      DBG_ACC(2);
-      tc_fence_after();
-      uint8_t* ztile = (i & 1) ? sTileB : sTileA;
-#pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        uint32_t v[32], pk[16];
-        tmem_ld32(R0 + lane_base + 32 * c, v);
-        tmem_wait_ld();
-        uint32_t bits = 0;
-#pragma unroll
-        for (int q = 0; q < 8; ++q) {
-          const float4 bq = __ldg((const float4*)(bias2 + 32 * c + 4 * q));
-          float a[4] = {__uint_as_float(v[4 * q]) + bq.x, __uint_as_float(v[4 * q + 1]) + bq.y,
-                        __uint_as_float(v[4 * q + 2]) + bq.z, __uint_as_float(v[4 * q + 3]) + bq.w};
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const float m = fabsf(a[e]) - p.lambda;
-            const bool on = row_kept && m > 0.f;
-            if (BACKWARD) bits |= (on ? 1u : 0u) << (4 * q + e);
-            a[e] = on ? copysignf(m, a[e]) : 0.f;
-          }
-          pk[2 * q] = pack_bf16(a[0], a[1]);
-          pk[2 * q + 1] = pack_bf16(a[2], a[3]);
-        }
-        m2[c] = bits;
-        if (!BACKWARD && r < HP) store_tile16(ztile, half, c, r, pk);
-      }
-      if (!BACKWARD) {
-        fence_async_smem();
-        tc_fence_before();
-        mbar_arrive(&bars.zready);
-        // ---- stage 3 -> A2 rows ----
-        DBG_ACC(4);
-        mbar_wait(&bars.dfull[3], tp);
-        DBG_ACC(3);
-        tc_fence_after();
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          uint32_t v[32], pk[16];
-          tmem_ld32(R1 + lane_base + 32 * c, v);
-          tmem_wait_ld();
-          pack32(v, pk);
-          if (row_valid) store16(p.A2 + row_off + 32 * c, pk);
-        }
-        tc_fence_before();
-      } else {
-        // ---- stage 3 -> G2 = G (.) mask2, packed in place (R1) ----
-        mbar_wait(&bars.dfull[3], tp);
-        tc_fence_after();
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          uint32_t v[32], pk[16];
-          tmem_ld32(R1 + lane_base + 32 * c, v);
-          tmem_wait_ld();
-          const uint32_t bits = m2[c];
-#pragma unroll
-          for (int q = 0; q < 16; ++q)
-            pk[q] = pack_bf16((bits >> (2 * q)) & 1u ? __uint_as_float(v[2 * q]) : 0.f,
-                              (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[2 * q + 1]) : 0.f);
-          tmem_st16(R1 + lane_base + 16 * c, pk);
-          if (r < HP) store_image16((uint8_t*)p.G2 + img_off, half, c, r, pk);
-          publish_chunk(&bars.cready[half][c]);
-        }
-        // ---- stage 4 -> G1 = mask1 (.) (G2 W2^H), packed in place (R0) ----
-        mbar_wait(&bars.dfull[4], tp);
-        tc_fence_after();
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          uint32_t v[32], pk[16];
-          tmem_ld32(R0 + lane_base + 32 * c, v);
-          tmem_wait_ld();
-          const uint32_t bits = m1[c];
-#pragma unroll
-          for (int q = 0; q < 16; ++q)
-            pk[q] = pack_bf16((bits >> (2 * q)) & 1u ? __uint_as_float(v[2 * q]) : 0.f,
-                              (bits >> (2 * q + 1)) & 1u ? __uint_as_float(v[2 * q + 1]) : 0.f);
-          tmem_st16(R0 + lane_base + 16 * c, pk);
-          if (r < HP) store_image16((uint8_t*)p.G1 + img_off, half, c, r, pk);
-          publish_chunk(&bars.cready[half][c]);
-        }
-        // ---- stage 5 -> GX as the B operand of the inverse transform (gradient tile buffer) ----
-        mbar_wait(&bars.dfull[5], tp);
-        tc_fence_after();
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          uint32_t v[32], pk[16];
-          tmem_ld32(R1 + lane_base + 32 * c, v);
-          tmem_wait_ld();
-#pragma unroll
-          for (int q = 0; q < 16; ++q)
-            pk[q] = row_valid ? pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1])) : 0u;
-          if (r < HP) store_tile16(sTileB, half, c, r, pk);
-        }
-        fence_async_smem();
-        tc_fence_before();
-        mbar_arrive(&bars.zready);
-        // optional mask export (test aid): bytes (re, im) interleaved per channel
-        if (EXPORT && row_valid) {
-          const int b = rem / p.Kw, kw = rem - b * p.Kw;
-          const size_t base = ((((size_t)b * p.H + r) * p.Wh + kw) * (size_t)(p.nb * BS) + (size_t)j * BS) * 2 + half;
-#pragma unroll
-          for (int c = 0; c < 3; ++c)
-#pragma unroll 4
-            for (int q = 0; q < 32; ++q) {
-              p.mask1[base + (size_t)(32 * c + q) * 2] = (uint8_t)((m1[c] >> q) & 1u);
-              p.mask2[base + (size_t)(32 * c + q) * 2] = (uint8_t)((m2[c] >> q) & 1u);
-            }
-        }
-        // ---- stage 6 -> A2 rows ----
-        mbar_wait(&bars.dfull[6], tp);
-        tc_fence_after();
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-          uint32_t v[32], pk[16];
-          tmem_ld32(R1 + lane_base + 32 * c, v);
-          tmem_wait_ld();
-          pack32(v, pk);
-          if (row_valid) store16(p.A2 + row_off + 32 * c, pk);
-        }
-        tc_fence_before();
-      }
-      DBG_ACC(4);
-    }
-#ifdef AFNO_TIMING
-    if (!BACKWARD && blockIdx.x == 0 && tid == 0)
-      for (int q = 0; q < 8; ++q) g_afno_dbg[48 + q] = dbg_acc[q];
-#endif
-  }
-  tc_fence_before();
-  __syncthreads();
-  if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
 // ---- tc_mix2: two mode tiles in flight per CTA (ping-pong), 12 epilogue warps ------------------------
@@ -822,8 +361,22 @@ __global__ void __launch_bounds__(kMixThreads, 1) tc_mix(MixParams p) {
 constexpr int kMix2Threads = 512;
 constexpr uint32_t kDft2Lbo = 1536, kDft2Sbo = 128;  // Ch / Sh: K-major A, 96 stored rows, order [k/8][m/8 < 12]
 constexpr uint32_t kDft2Bytes = 12 * kDft2Lbo;        // 18432 (rows 96..127 alias the next k-chunk: finite, unused)
-constexpr uint32_t kMix2Smem = 2 * kDft2Bytes + 4 * kWBytes + 3 * kTileBytes; // 222336
+// A tile buffer is also the staging area of the tile's output rows.  Rows are 400 bytes apart, in
+// shared memory (eight consecutive rows fall into distinct 16-byte bank groups) AND in the global
+// A2 tensor, so that a whole tile leaves with ONE bulk copy (async proxy, no L1 traffic).
+constexpr uint32_t kOutStride = 2 * kA2Row;           // 400
+constexpr uint32_t kTileBuf = 96 * kOutStride;        // 38400 >= kTileBytes
+constexpr uint32_t kMix2Smem = 2 * kDft2Bytes + 4 * kWBytes + 3 * kTileBuf; // 225792
 constexpr uint32_t kSlot = 96;
+
+// bulk (async-proxy) store of a thread's own staged bytes: shared -> global, tracked by bulk groups
+__device__ __forceinline__ void bulk_store(void* dst, uint32_t src_smem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src_smem), "r"(bytes)
+               : "memory");
+  asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
 struct Mix2Bars {
   uint64_t dfull[2];  // stream's current stage accumulated (tcgen05.commit)
@@ -831,30 +384,32 @@ struct Mix2Bars {
   uint64_t xfull[3];  // buffer holds the input tile (forward: spectrum; backward: x spectrum)
   uint64_t gfull[3];  // backward: buffer holds the gradient tile
   uint64_t xfree[3];  // backward: stage 0 has consumed the x tile (tcgen05.commit)
-  uint64_t tfree[3];  // the tile's last stage has consumed the buffer (tcgen05.commit)
+  uint64_t sdone[3];  // the 12 epilogue warps have staged the tile's output rows in the buffer
+  uint64_t tfree[3];  // the staged rows have left the buffer (loader warp 0, after its bulk store has read them)
 };
 
-__device__ __forceinline__ void issue_dft2(uint32_t d, uint32_t a_base, uint32_t b_base, uint32_t idesc, bool fresh) {
+// One transform product pair: the same A (DFT matrix K-step) times two B tile halves
+__device__ __forceinline__ void issue_dft2_pair(uint32_t d0, uint32_t d1, uint32_t a_base, uint32_t b0, uint32_t b1,
+                                                uint32_t id0, uint32_t id1, bool fresh) {
 #pragma unroll
-  for (int ks = 0; ks < HP / 16; ++ks)
-    mma_ss(d, smem_desc(a_base + ks * 2 * kDft2Lbo, kDft2Lbo, kDft2Sbo),
-           smem_desc(b_base + ks * 2 * kTileLbo, kTileLbo, kTileSbo), idesc, !(fresh && ks == 0));
+  for (int ks = 0; ks < HP / 16; ++ks) {
+    const uint64_t ad = smem_desc(a_base + ks * 2 * kDft2Lbo, kDft2Lbo, kDft2Sbo);
+    const uint32_t acc = !(fresh && ks == 0);
+    mma_ss(d0, ad, smem_desc(b0 + ks * 2 * kTileLbo, kTileLbo, kTileSbo), id0, acc);
+    mma_ss(d1, ad, smem_desc(b1 + ks * 2 * kTileLbo, kTileLbo, kTileSbo), id1, acc);
+  }
 }
 // forward transform (exp(-i theta)):  Xr = Ch Ar + Sh Ai ; Xi = Ch Ai - Sh Ar
 __device__ __forceinline__ void issue_fwd_dft2(uint32_t Dre, uint32_t Dim, uint32_t aCh, uint32_t aSh, uint32_t tile) {
   const uint32_t id = idesc_bf16(128, BS, kIdescBMn), half = (BS / 8) * kTileSbo;
-  issue_dft2(Dre, aCh, tile, id, true);
-  issue_dft2(Dre, aSh, tile + half, id, false);
-  issue_dft2(Dim, aCh, tile + half, id, true);
-  issue_dft2(Dim, aSh, tile, id | kIdescNegA, false);
+  issue_dft2_pair(Dre, Dim, aCh, tile, tile + half, id, id, true);
+  issue_dft2_pair(Dre, Dim, aSh, tile + half, tile, id, id | kIdescNegB, false);
 }
 // inverse transform (exp(+i theta)):  Tr = Ch Zr - Sh Zi ; Ti = Ch Zi + Sh Zr
 __device__ __forceinline__ void issue_inv_dft2(uint32_t Dre, uint32_t Dim, uint32_t aCh, uint32_t aSh, uint32_t tile) {
   const uint32_t id = idesc_bf16(128, BS, kIdescBMn), half = (BS / 8) * kTileSbo;
-  issue_dft2(Dre, aCh, tile, id, true);
-  issue_dft2(Dre, aSh, tile + half, id | kIdescNegA, false);
-  issue_dft2(Dim, aCh, tile + half, id, true);
-  issue_dft2(Dim, aSh, tile, id, false);
+  issue_dft2_pair(Dre, Dim, aCh, tile, tile + half, id, id, true);
+  issue_dft2_pair(Dre, Dim, aSh, tile + half, tile, id | kIdescNegB, id, false);
 }
 // T = S W (TRANSPOSED = false) or S W^H (true); S = compact bf16 A operand: re at columns
 // [S, S+48), im at [S+48, S+96) (two bf16 per column)
@@ -897,6 +452,14 @@ __device__ __forceinline__ void store_chunks6(uint8_t* base, int chunk0, int r, 
     *(uint4*)(base + (chunk0 + g) * kTileSbo + r * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
 }
 
+// softshrink of a packed bf16 pair: a - min(max(a, -lambda), lambda)
+__device__ __forceinline__ uint32_t shrink_bf16x2(uint32_t a, uint32_t lam2, uint32_t nlam2) {
+  uint32_t c, r;
+  asm("max.bf16x2 %0, %1, %2;" : "=r"(c) : "r"(a), "r"(nlam2));
+  asm("min.bf16x2 %0, %1, %2;" : "=r"(c) : "r"(c), "r"(lam2));
+  asm("sub.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(c));
+  return r;
+}
 // relu + one rounding of two fp32 values to a packed bf16 pair (lo, hi)
 __device__ __forceinline__ uint32_t pack_relu_bf16(float lo, float hi) {
   uint32_t r;
@@ -953,7 +516,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
   const int j = blockIdx.x / S, s0 = blockIdx.x - j * S;
   const int BKw = p.B * p.Kw;
   const int n = s0 < BKw ? (BKw - s0 + S - 1) / S : 0;   // tiles of this CTA: rem = s0 + i * S
-  for (uint32_t i = tid; i < 3 * kTileBytes / 16; i += kMix2Threads) ((uint4*)sT)[i] = make_uint4(0, 0, 0, 0);
+  for (uint32_t i = tid; i < 3 * kTileBuf / 16; i += kMix2Threads) ((uint4*)sT)[i] = make_uint4(0, 0, 0, 0);
   for (uint32_t i = tid; i < 2 * kDft2Bytes / 16; i += kMix2Threads) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
   {
     const uint8_t* wsrc = p.wprep + (size_t)j * 4 * kWBytes;
@@ -969,6 +532,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
       mbar_init(&bars.xfull[q], kMixLoadWarps * 32);
       mbar_init(&bars.gfull[q], kMixLoadWarps * 32);
       mbar_init(&bars.xfree[q], 1);
+      mbar_init(&bars.sdone[q], 12);
       mbar_init(&bars.tfree[q], 1);
     }
     mbar_init_fence();
@@ -980,7 +544,10 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
-  const int T = 2 * NS * ((n + 1) / 2);   // phases
+  // Stream 1 runs kLag stages behind stream 0, so tiles finish (and buffers become free) at
+  // regular intervals and a transform stage of one stream overlaps an MLP stage of the other.
+  constexpr int kLag = NS / 2;
+  const int T = 2 * (NS * ((n + 1) / 2) + kLag);   // phases
   const int lq = warp & 3;
 
   if (lq == 3 && warp != 3) {
@@ -989,17 +556,40 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
     const uint32_t aT = smem_u32(sT);
     auto tile_off = [&](int i) { return ((size_t)(s0 + i * S) * p.nb + j) * p.H * NT; };
     auto load = [&](int buf, const __nv_bfloat16* src, uint64_t* full) {
-      load_tile_warp(aT + buf * kTileBytes, src, p.H, lane, sub);
+      // rows H..95 of the operand are K padding: the output staging of the buffer's previous tile
+      // overlaps them, so they are cleared again
+      for (int q = sub * 32 + lane; q < (HP - p.H) * (NT / 8); q += kMixLoadWarps * 32) {
+        const int nc = q / (HP - p.H), h = p.H + q - nc * (HP - p.H);
+        *(uint4*)(sT + buf * kTileBuf + nc * kTileSbo + h * 16) = make_uint4(0, 0, 0, 0);
+      }
+      load_tile_warp(aT + buf * kTileBuf, src, p.H, lane, sub);
       cp_async_wait_all();
       fence_async_smem();
       mbar_arrive(full);
     };
+    // tile k's output rows are staged in its buffer by the epilogue warps; loader warp 0 sends them
+    // to A2 with one bulk copy and frees the buffer once the copy has read it
+    auto drain = [&](int k) {
+      const int buf = k % 3;
+      const uint32_t par = (uint32_t)((k / 3) & 1);
+      if (sub == 0) {
+        if (lane == 0) {
+          mbar_wait(&bars.sdone[buf], par);
+          bulk_store(p.A2 + ((size_t)(s0 + k * S) * p.nb + j) * p.H * kA2Row, aT + buf * kTileBuf,
+                     (uint32_t)p.H * kOutStride);
+          bulk_wait_read();
+          mbar_arrive(&bars.tfree[buf]);
+        }
+        __syncwarp();
+      }
+      mbar_wait(&bars.tfree[buf], par);
+    };
     if (!BACKWARD) {
       for (int i = 0; i < n; ++i) {
-        const int buf = i % 3, use = i / 3;
-        if (use > 0) mbar_wait(&bars.tfree[buf], (uint32_t)((use - 1) & 1));
-        load(buf, p.A1 + tile_off(i), &bars.xfull[buf]);
+        if (i >= 3) drain(i - 3);
+        load(i % 3, p.A1 + tile_off(i), &bars.xfull[i % 3]);
       }
+      for (int k = n > 3 ? n - 3 : 0; k < n; ++k) drain(k);
     } else {
       // x(0) x(1) x(2) | g(0) g(1) | then for k = 0, 1, ..: x(k+3) after the last stage of tile k,
       // g(k+2) after stage 0 of tile k+2 -- the order in which the buffers become free
@@ -1010,16 +600,15 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
       }
       for (int k = 0; k < n; ++k) {
         const int ix = k + 3, ig = k + 2;
-        if (ix < n) {
-          mbar_wait(&bars.tfree[ix % 3], (uint32_t)((ix / 3 - 1) & 1));
-          load(ix % 3, p.A1 + tile_off(ix), &bars.xfull[ix % 3]);
-        }
+        drain(k);
+        if (ix < n) load(ix % 3, p.A1 + tile_off(ix), &bars.xfull[ix % 3]);
         if (ig < n) {
           mbar_wait(&bars.xfree[ig % 3], (uint32_t)((ig / 3) & 1));
           load(ig % 3, p.A1g + tile_off(ig), &bars.gfull[ig % 3]);
         }
       }
     }
+    if (sub == 0 && lane == 0) bulk_wait_all();
   } else if (warp == 3) {
     // ================================ control warp ===========================================
     const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW), aT = smem_u32(sT);
@@ -1030,17 +619,20 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
 #endif
     DBG_T0();
     for (int t = 0; t < T; ++t) {
-      const int stream = t & 1, u = t >> 1, pair = u / NS, stg = u - pair * NS;
+      const int stream = t & 1, u = (t >> 1) - (stream ? kLag : 0);
+      if (u < 0) continue;
+      const int pair = u / NS, stg = u - pair * NS;
       const int i = 2 * pair + stream;
       if (i >= n) continue;
       const uint32_t Dre = tmem + kSlot * (uint32_t)((3 * t) % 5), Dim = tmem + kSlot * (uint32_t)((3 * t + 1) % 5);
       const uint32_t SA = tmem + kSlot * (uint32_t)((3 * t + 4) % 5);   // slot of phase t - 2
       const uint32_t cs = stream ? cs1 : cs0;
       if (cs > 0) mbar_wait_fast(&bars.edone[stream], (cs - 1) & 1u);
+      TR(t, 0);
       DBG_ACC(0);
       const int buf = i % 3;
       const uint32_t use = (uint32_t)(i / 3);
-      const uint32_t tile = aT + buf * kTileBytes;
+      const uint32_t tile = aT + buf * kTileBuf;
       const bool first = stg == 0, dftg = BACKWARD && stg == 3, last = stg == NS - 1;
       if (first) mbar_wait(&bars.xfull[buf], use & 1u);
       if (dftg) mbar_wait(&bars.gfull[buf], use & 1u);
@@ -1062,9 +654,9 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
         }
         mma_commit(&bars.dfull[stream]);
         if (BACKWARD && first) mma_commit(&bars.xfree[buf]);
-        if (last) mma_commit(&bars.tfree[buf]);
       }
       __syncwarp();
+      TR(t, 2);
       DBG_ACC(2);
       if (stream) ++cs1; else ++cs0;
     }
@@ -1092,29 +684,32 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
 #ifdef AFNO_TIMING
     long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     long long dbg_m[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long dbg_f[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 #endif
     DBG_T0();
-    for (int u = 0; u < T / 2; ++u) {
-      const int pair = u / NS, stg = u - pair * NS;
+    for (int u0 = 0; u0 < T / 2; ++u0) {
 #pragma unroll
       for (int stream = 0; stream < 2; ++stream) {
-        const int t = 2 * u + stream;
+        const int t = 2 * u0 + stream;
+        const int u = u0 - (stream ? kLag : 0);
+        if (u < 0) continue;
+        const int pair = u / NS, stg = u - pair * NS;
         const int i = 2 * pair + stream;
         if (i >= n) continue;
         const int rem = s0 + i * S;
         const uint32_t src = tmem + lane_sel + kSlot * (uint32_t)((3 * t + half) % 5) + chalf * 48;
         const uint32_t dstA = tmem + lane_sel + kSlot * (uint32_t)((3 * t) % 5) + 24 * cq;
-        uint8_t* tile = sT + (i % 3) * kTileBytes;
+        uint8_t* tile = sT + (i % 3) * kTileBuf;
         const size_t img_off = ((size_t)rem * p.nb + j) * kTileBytes;
-        const size_t row_off = (((size_t)rem * p.nb + j) * p.H + r) * NT + half * BS + chalf * 48;
         mbar_wait_fast(&bars.dfull[stream], ce[stream] & 1u);
         ++ce[stream];
+        TR(t, 4 + warp * 3);
         DBG_ACC(0);
         tc_fence_after();
         uint32_t v[48], pk[24];
         ld48(src, v);
         DBG_ACC(2);
-        bool writes_a = false;
+        bool writes_a = false, early_arrive = false;
         if (stg == 0) {
           // ---- spectrum Xh ----
           pack48(v, pk);
@@ -1139,15 +734,20 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
           //      backward: only the mask ----
           const float lam = p.lambda;
           if (!BACKWARD) {
+            // Z = S_lambda(P2 + b2): the sum is rounded to bf16 once, then a - clamp(a, -lambda, lambda)
+            // on packed pairs (exact zeros inside the threshold; lambda at bf16 precision)
+            const uint32_t lam2 = pack_bf16(lam, lam), nlam2 = lam2 ^ 0x80008000u;
 #pragma unroll
             for (int q = 0; q < 12; ++q) {
               const float4 bq = *(const float4*)(bias2 + 4 * q);
-              float a[4] = {__uint_as_float(v[4 * q]) + bq.x, __uint_as_float(v[4 * q + 1]) + bq.y,
-                            __uint_as_float(v[4 * q + 2]) + bq.z, __uint_as_float(v[4 * q + 3]) + bq.w};
+              pk[2 * q] = shrink_bf16x2(pack_bf16(__uint_as_float(v[4 * q]) + bq.x, __uint_as_float(v[4 * q + 1]) + bq.y),
+                                        lam2, nlam2);
+              pk[2 * q + 1] = shrink_bf16x2(
+                  pack_bf16(__uint_as_float(v[4 * q + 2]) + bq.z, __uint_as_float(v[4 * q + 3]) + bq.w), lam2, nlam2);
+            }
+            if (!row_kept) {
 #pragma unroll
-              for (int e = 0; e < 4; ++e) a[e] -= fminf(fmaxf(a[e], -lam), lam);   // S_lambda, exact zeros inside
-              pk[2 * q] = row_kept ? pack_bf16(a[0], a[1]) : 0u;
-              pk[2 * q + 1] = row_kept ? pack_bf16(a[2], a[3]) : 0u;
+              for (int q = 0; q < 24; ++q) pk[q] = 0u;
             }
             store_chunks6(tile, chunk0, r, pk);
             fence_async_smem();
@@ -1166,13 +766,23 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
               MaskLoop<0>::run([&](auto P) { mask_collect<decltype(P)::value>(m2[stream], pk[decltype(P)::value]); });
           }
         } else if (!BACKWARD || stg == 6) {
-          // ---- last stage: rows of A2 ----
+          // ---- last stage: rows of A2.  The accumulator is in registers: release the tensor-memory
+          //      slots now, so the next tile's first GEMM never waits for the global stores ----
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&bars.edone[stream]);
+          early_arrive = true;
           pack48(v, pk);
           if (row_valid) {
-            stg256(p.A2 + row_off, pk);
-            stg256(p.A2 + row_off + 16, pk + 8);
-            stg256(p.A2 + row_off + 32, pk + 16);
+            // staged in the tile's own buffer (its last GEMM has completed)
+            uint8_t* srow = tile + r * kOutStride + cq * 96;
+#pragma unroll
+            for (int g = 0; g < 6; ++g)
+              *(uint4*)(srow + 16 * g) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
           }
+          fence_async_smem();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&bars.sdone[i % 3]);
         } else if (stg == 3 || stg == 4) {
           // ---- G2 = G (.) mask2 ; G1 = mask1 (.) (G2 W2^H) ----
           pack48(v, pk);
@@ -1205,6 +815,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
 #ifdef AFNO_TIMING
         { long long n_ = clock64(); dbg_m[stg] += n_ - dbg_t; dbg_t = n_; }
 #endif
+        TR(t, 5 + warp * 3);
         if (writes_a) {
           // the four warps of this lane quarter have their accumulator columns in registers:
           // compact the bf16 operand into the first slot (columns of the other warps' sources)
@@ -1214,9 +825,12 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
           tmem_wait_st();
           DBG_ACC(5);
         }
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&bars.edone[stream]);
+        if (!early_arrive) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&bars.edone[stream]);
+        }
+        TR(t, 6 + warp * 3);
         DBG_ACC(1);
       }
     }
@@ -1225,6 +839,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
       for (int q = 0; q < 8; ++q) {
         g_afno_dbg[(BACKWARD ? 88 : 72) + q] = dbg_acc[q];
         g_afno_dbg[(BACKWARD ? 104 : 96) + q] = dbg_m[q];
+        g_afno_dbg[(BACKWARD ? 120 : 112) + q] = dbg_f[q];
       }
 #endif
   }
@@ -1418,7 +1033,7 @@ TcWs tc_carve(const Geometry& g, bool backward, char* base) {
   }
   const size_t spec = (size_t)g.B * g.Kw * g.nb * g.H * NT * 2;
   w.A1 = (__nv_bfloat16*)take(spec);
-  w.A2 = (__nv_bfloat16*)take(spec);
+  w.A2 = (__nv_bfloat16*)take((size_t)g.B * g.Kw * g.nb * g.H * kA2Row * 2);
   w.wprep = (__nv_bfloat16*)take((size_t)g.nb * 4 * kWBytes);
   w.bprep = (float*)take((size_t)g.nb * 2 * NT * sizeof(float));
   if (backward) {
@@ -1447,16 +1062,7 @@ bool tc_supported(const Geometry& g) {
 cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
   const double two_pi = 6.283185307179586476925286766559;
   const int Wh = W / 2 + 1;
-  // Ch, Sh: element (r, h) = cos / sin (2 pi r h / H) / sqrt(H); K-major [k/8][m/8]
-  std::vector<uint16_t> dft(2 * kDftBytes / 2, 0);
-  for (int r = 0; r < H; ++r)
-    for (int h = 0; h < H; ++h) {
-      const double a = two_pi * (double)((long)r * h % H) / (double)H, s = 1.0 / sqrt((double)H);
-      const uint32_t off = ((h / 8) * kDftLbo + (r / 8) * kDftSbo + (r % 8) * 16 + (h % 8) * 2) / 2;
-      dft[off] = host_bf16(cos(a) * s);
-      dft[kDftBytes / 2 + off] = host_bf16(sin(a) * s);
-    }
-  // compact images for tc_mix2: only 96 rows stored, order [k/8][m/8 < 12]
+  // Ch, Sh: element (r, h) = cos / sin (2 pi r h / H) / sqrt(H); K-major, 96 rows stored, order [k/8][m/8 < 12]
   std::vector<uint16_t> dft2(2 * kDft2Bytes / 2, 0);
   for (int r = 0; r < H; ++r)
     for (int h = 0; h < H; ++h) {
@@ -1484,22 +1090,17 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
         gw1[og] = host_bf16(v);
       }
     }
-  cudaError_t e = upload(dft, &out->dft);
-  if (e == cudaSuccess) e = upload(dft2, &out->dft2);
+  cudaError_t e = upload(dft2, &out->dft2);
   if (e == cudaSuccess) e = upload(fw, &out->fw);
   if (e == cudaSuccess) e = upload(fwa, &out->fw_alpha);
   if (e == cudaSuccess) e = upload(gw, &out->gw);
   if (e == cudaSuccess) e = upload(gw1, &out->gw_noalpha);
   if (e == cudaSuccess) e = set_smem(tc_wdft<false>, kRowSmem);
   if (e == cudaSuccess) e = set_smem(tc_wdft<true>, kRowSmem);
-  if (e == cudaSuccess) e = set_smem(tc_mix<false, false>, kMixSmem2);
-  if (e == cudaSuccess) e = set_smem(tc_mix<true, false>, kMixSmem2);
-  if (e == cudaSuccess) e = set_smem(tc_mix<true, true>, kMixSmem2);
   if (e == cudaSuccess) e = set_smem(tc_mix2<false, false>, kMix2Smem);
   if (e == cudaSuccess) e = set_smem(tc_mix2<true, false>, kMix2Smem);
   if (e == cudaSuccess) e = set_smem(tc_mix2<true, true>, kMix2Smem);
   if (e == cudaSuccess) e = set_smem(tc_wgrad, kWgSmem);
-  out->mix_v1 = getenv("AFNO_MIX_V1") != nullptr;
   int dev = 0, sms = 148;
   if (e == cudaSuccess) e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -1542,18 +1143,11 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   MixParams mp{};
-  mp.A1 = w.A1; mp.A2 = w.A2; mp.dft = tp.dft; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
+  mp.A1 = w.A1; mp.A2 = w.A2; mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
   mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
-  const int mix_tiles = g.nb * g.B * g.Kw;
-  const int grid_mix = mix_tiles < tp.num_sms ? mix_tiles : tp.num_sms;
   prof_begin("tc_mix_fwd", st);
-  if (tp.mix_v1) {
-    tc_mix<false, false><<<grid_mix, kMixThreads, kMixSmem2, st>>>(mp);
-  } else {
-    const int S2 = mix2_split(g, tp);
-    mp.dft = tp.dft2;
-    tc_mix2<false, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2);
-  }
+  const int S2 = mix2_split(g, tp);
+  tc_mix2<false, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2);
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -1595,26 +1189,15 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   MixParams mp{};
   mp.A1 = w.A1; mp.A1g = w.A1g; mp.A2 = w.A2;
   mp.Xh = w.Xh; mp.O1 = w.O1; mp.G2 = w.G2; mp.G1 = w.G1;
-  mp.dft = tp.dft; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
+  mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
   mp.mask1 = g.export_masks ? w.mask1 : nullptr;
   mp.mask2 = g.export_masks ? w.mask2 : nullptr;
   mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
-  const int mix_tiles = g.nb * g.B * g.Kw;
-  const int grid_mix = mix_tiles < tp.num_sms ? mix_tiles : tp.num_sms;
-  if (tp.mix_v1) {
-    if (g.export_masks) {
-      TC_LAUNCH("tc_mix_bwd", tc_mix<true, true><<<grid_mix, kMixThreads, kMixSmem2, st>>>(mp));
-    } else {
-      TC_LAUNCH("tc_mix_bwd", tc_mix<true, false><<<grid_mix, kMixThreads, kMixSmem2, st>>>(mp));
-    }
+  const int S2 = mix2_split(g, tp);
+  if (g.export_masks) {
+    TC_LAUNCH("tc_mix_bwd", tc_mix2<true, true><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
   } else {
-    const int S2 = mix2_split(g, tp);
-    mp.dft = tp.dft2;
-    if (g.export_masks) {
-      TC_LAUNCH("tc_mix_bwd", tc_mix2<true, true><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
-    } else {
-      TC_LAUNCH("tc_mix_bwd", tc_mix2<true, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
-    }
+    TC_LAUNCH("tc_mix_bwd", tc_mix2<true, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
   }
   // B4 / B6: parameter gradients
   const int nred = nW + g.nb * BS;
@@ -1632,6 +1215,11 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   return cudaSuccess;
 }
 
+#ifdef AFNO_TRACE
+extern "C" int afno_trace_read(long long* out) {
+  return (int)cudaMemcpyFromSymbol(out, g_afno_trace, sizeof(long long) * 64 * 32);
+}
+#endif
 #ifdef AFNO_TIMING
 extern "C" int afno_debug_read(long long* out) {
   return (int)cudaMemcpyFromSymbol(out, g_afno_dbg, sizeof(long long) * 128);

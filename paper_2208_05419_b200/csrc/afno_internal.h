@@ -37,6 +37,7 @@ struct TcPlan {
   int num_sms = 148;
   uint8_t* dft2 = nullptr;
   uint8_t *fw = nullptr, *fw_alpha = nullptr, *gw = nullptr, *gw_noalpha = nullptr;
+  void* encode_tiled = nullptr; // cuTensorMapEncodeTiled, resolved through the runtime (no link to libcuda)
 };
 
 struct Plan {

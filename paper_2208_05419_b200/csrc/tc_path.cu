@@ -6,10 +6,10 @@
 // with fp32 accumulation against constant DFT matrices (S5 gives the arithmetic and
 // the measured error).  The layer becomes three GEMM-chain kernels:
 //
-//   tc_wdft_fwd  [F1, B2]   per (b, h, 128 channels):  A1[c, (ri,kw)] = x^T[c, w] * Fw[w, (ri,kw)]
+//   tc_wdft_fwd  [F1, B2]   per (b, h, block j):  A1[(ri,kw), c] = Fw[(ri,kw), w] * x[w, c]
 //   tc_mix_fwd   [F2-F7]    per (b, kw, block j), everything on chip in tensor memory:
 //                            Xh = Fh * A1  ->  relu(Xh W1 + b1)  ->  shrink(. W2 + b2)  ->  Fh^H * Z
-//   tc_wdft_inv  [F8, F9, B8] per (b, h, 128 channels): y[c, w] = x + A2^T[c, (ri,kw)] * Gw[(ri,kw), w]
+//   tc_wdft_inv  [F8, F9, B8] per (b, h, block j): y[w, c] = x[w, c] + Gw[w, (ri,kw)] * A2[(ri,kw), c]
 //
 // Complex arithmetic runs as real GEMMs on separate (re | im) column halves using the
 // instruction descriptor's negate bit for the minus signs, so only W_re and W_im (not the 2x2
@@ -34,8 +34,10 @@ constexpr int BS = 96;    // channel block size handled by this path
 constexpr int NT = 192;   // (re | im) columns of one block
 constexpr int HP = 96;    // H padded to the K extent of the H-direction GEMMs
 constexpr int WP = 192;   // W padded to the K / N extent of the W-direction GEMMs
-constexpr int CGRP = 128; // channels per W-direction tile (= UMMA M)
-constexpr int kA2Row = NT + 8; // elements per stored row of A2: 192 values + 16 bytes (see kOutStride)
+constexpr int kA2Row = NT + 8; // elements per stored row of A1 / A2: 192 values + 16 bytes of padding
+// Rows of the half-spectra are 400 bytes apart, in shared-memory staging (eight consecutive rows fall
+// into distinct 16-byte bank groups) AND in global memory, so that staged rows leave with ONE bulk copy.
+constexpr uint32_t kOutStride = 2 * kA2Row;           // 400
 
 // shared-memory operand geometry (bytes), see tc_common.cuh for the layout formulas
 constexpr uint32_t kWLbo = 1536, kWSbo = 128;       // weights: K-major B [96 x 96], order [k/8][n/8]
@@ -44,16 +46,8 @@ constexpr uint32_t kWBytes = BS * BS * 2;            // 18432
 // writes of consecutive chunks of one row (the coalesced global order) bank-conflict-free
 constexpr uint32_t kTileLbo = 128, kTileSbo = 1536 + 16;
 constexpr uint32_t kTileBytes = (NT / 8) * kTileSbo; // 37248
-constexpr uint32_t kFwLbo = 2048, kFwSbo = 128;     // Fw / Gw halves: K-major A [128 x 192], order [k/8][m/8]
-constexpr uint32_t kFwHalf = 128 * WP * 2;           // 49152 per 128-row half
-constexpr uint32_t kFwBytes = 2 * kFwHalf;           // 98304
-constexpr uint32_t kRowLbo = 128, kRowSbo = 3072 + 16; // W-direction data tile: MN-major B [K=192][N=128], padded
-constexpr uint32_t kRowBytes = (CGRP / 8) * kRowSbo; // 49408
-
-constexpr int kRowEpiThreads = 256;                 // 8 epilogue warps
-constexpr int kRowProdWarps = 4;                     // producer warps per operand buffer
-constexpr int kRowThreads = kRowEpiThreads + 2 * kRowProdWarps * 32;
-constexpr uint32_t kRowSmem = kFwBytes + 2 * kRowBytes;                              // 196608
+constexpr uint32_t kFwLbo = 2048, kFwSbo = 128;     // Gw rows 0..127: K-major A [128 x 192], order [k/8][m/8]
+constexpr uint32_t kFwHalf = 128 * WP * 2;           // 49152
 
 // ---- weight preparation: fp32 [nb][96][96][2] -> bf16 K-major interleaved operands --------------
 // per block 4 matrices of kWBytes {W1r, W1i, W2r, W2i} with element (n=o, k=i) = W[i][o] (the
@@ -84,29 +78,9 @@ __global__ void k_tc_prep_weights(const float* __restrict__ w1, const float* __r
   base[3 * m + f] = __float2bfloat16_rn(b.y);
 }
 
-// ---- F1 / B2 and F8 + F9 / B8: the W-direction transforms as GEMMs -------------------------------
-// One tile = (b, h, 128 channels).  The constant DFT matrix is the A operand (accumulator
-// rows = output index), the activation tile the MN-major B operand (columns = channels):
-//   forward (INVERSE = false): D_ri[kw, c] = sum_w  Fw_ri[kw, w] * x[b,h,w,c]      ri = re, im
-//   inverse (INVERSE = true) : D_a[w, c]   = sum_(ri,kw) Gw[w, (ri,kw)] * A2[..]    a = w / 128
-// so every thread's accumulator row is 128 CONTIGUOUS channels of one output row and the
-// epilogue is plain 32-byte vector I/O (no transpose).  Two 128x128x192 GEMMs per tile.
-// Warp-specialised and persistent: producer warp p copies tiles it = p, p+2, .. (cp.async)
-// into operand buffer p and issues their MMAs into accumulator pair p; the 8 epilogue warps
-// (accumulator a = warp/4, TMEM lanes 32*(warp%4)..) drain tile it while tile it+1 computes.
 __device__ __forceinline__ void pack32(const uint32_t (&v)[32], uint32_t (&pk)[16]) {
 #pragma unroll
   for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
-}
-__device__ __forceinline__ void ldg256(const void* p, uint32_t (&r)[8]) {
-  asm volatile("ld.global.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-               : "l"(p));
-}
-__device__ __forceinline__ void stg256(void* p, const uint32_t* r) {
-  asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]),
-               "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
-               : "memory");
 }
 
 #ifdef AFNO_TRACE
@@ -124,24 +98,52 @@ __device__ long long g_afno_dbg[128];
 #define DBG_ACC(slot)
 #endif
 
-template <bool INVERSE>
-__global__ void __launch_bounds__(kRowThreads, 1)
-tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ res, __nv_bfloat16* __restrict__ out,
-        const uint8_t* __restrict__ Aconst, int B, int H, int W, int C, int Kw, int nb) {
-  extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) uint64_t full[2], empty[2];
+// ---- F1 / B2 and F8 + F9 / B8, second generation: all global traffic through bulk tensor copies -------
+// One tile = (b, h, channel block j): N = 96 channels.  The activation tile arrives as three
+// 64B-swizzled panels [192 rows (w, zero-filled past W)][32 channels] written by TMA, leaves as rows
+// staged in shared memory and sent by one TMA store: no LSU instruction touches global memory, so
+// the kernels run at the speed of the copy engines instead of the load/store pipe.
+//   forward : D_ri[kw, c] = sum_w Fw_ri[kw, w] x[b,h,w,c]      -> A1 rows [kw][re 96 | im 96 | pad 8]
+//   inverse : D_a[w, c]   = sum_(ri,kw) Gw[w, (ri,kw)] A2[..]  -> y[b,h,w,c] = residual + D
+// 8 warps: warps with (warp % 4) < rows/32 drain the accumulators (TMEM lane quarter = warp % 4),
+// one spare warp issues the TMA loads, one the UMMAs.  Shared memory is a ring of slots; a slot
+// holds a tile's operand and later (forward) its staged output rows.
+constexpr int kW2Threads = 256;
+constexpr uint32_t kPanel = 192 * 64;                      // 12288: one [192 x 32] bf16 panel
+constexpr uint32_t kW2Tile = 3 * kPanel;                   // 36864: a [192 x 96] tile
+constexpr uint32_t kF2Lbo = 12 * 128, kF2Sbo = 128;        // Fw halves: K-major A, 96 rows stored, order [k/8][m/8 < 12]
+constexpr uint32_t kF2Half = (WP / 8) * kF2Lbo;            // 36864 (rows 96..127 alias the next k-chunk: finite, unused)
+constexpr uint32_t kF2Bytes = 2 * kF2Half;                 // 73728
+constexpr int kWfSlots = 4;
+constexpr uint32_t kWfSmem = kF2Bytes + kWfSlots * kW2Tile + 1024;   // 222208
+constexpr uint32_t kG2Lbo1 = 7 * 128;                      // Gw second half: rows 128..183 stored (7 groups of 8)
+constexpr uint32_t kG2Half1 = (WP / 8) * kG2Lbo1;          // 21504
+constexpr uint32_t kG2Bytes = kFwHalf + kG2Half1;          // 70656
+constexpr uint32_t kWiSmem = kG2Bytes + 4 * kW2Tile + 1024;          // 219136
+
+__global__ void __launch_bounds__(kW2Threads, 1)
+tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapA1,
+             const uint8_t* __restrict__ Fimg, int ntiles, int nb, int H, int Kw) {
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t full[kWfSlots], sfree[kWfSlots], accfull[2], accempty[2];
   __shared__ uint32_t tmem_slot;
-  uint8_t* sF = smem;
-  uint8_t* sB0 = smem + kFwBytes;
+  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t* smem = smem_raw + (base - smem_u32(smem_raw));
+  const uint32_t aF = base, aS = base + kF2Bytes;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (uint32_t i = tid; i < 2 * kRowBytes / 16; i += kRowThreads) ((uint4*)sB0)[i] = make_uint4(0, 0, 0, 0);
-  for (uint32_t i = tid; i < kFwBytes / 16; i += kRowThreads) cp_async16(smem_u32(sF) + i * 16, Aconst + (size_t)i * 16);
+  for (uint32_t i = tid; i < kF2Bytes / 16; i += kW2Threads) cp_async16(aF + i * 16, Fimg + (size_t)i * 16);
   if (tid == 0) {
-    mbar_init(&full[0], 1);
-    mbar_init(&full[1], 1);
-    mbar_init(&empty[0], kRowEpiThreads);
-    mbar_init(&empty[1], kRowEpiThreads);
+    for (int q = 0; q < kWfSlots; ++q) {
+      mbar_init(&full[q], 1);
+      mbar_init(&sfree[q], 1);
+    }
+    for (int q = 0; q < 2; ++q) {
+      mbar_init(&accfull[q], 1);
+      mbar_init(&accempty[q], 6);
+    }
     mbar_init_fence();
+    tma_prefetch_desc(&mapX);
+    tma_prefetch_desc(&mapA1);
   }
   if (warp == 0) tmem_alloc<512>(&tmem_slot);
   cp_async_wait_all();
@@ -150,164 +152,242 @@ tc_wdft(const __nv_bfloat16* __restrict__ in, const __nv_bfloat16* __restrict__ 
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
-  const int ncg = (C + CGRP - 1) / CGRP;
-  const int ntiles = B * H * ncg;
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
-  if (warp >= kRowEpiThreads / 32) {
-    // ===== producer group p (4 warps): tiles it = p, p+2, ... -> operand buffer p, accumulator pair p ==
-    // (a single warp sustains only ~1 cp.async instruction per 200 cycles, so the copy is spread)
-    const int pw = warp - kRowEpiThreads / 32;
-    const int p = pw / kRowProdWarps, sub = pw % kRowProdWarps;
-    const uint32_t dst = smem_u32(sB0) + p * kRowBytes;
-    const uint32_t idesc = idesc_bf16(128, CGRP, kIdescBMn);
-#ifdef AFNO_TIMING
-    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-#endif
-    DBG_T0();
-    for (int it = p; it < nmine; it += 2) {
-      const int use = it >> 1;
-      // the previous MMAs on this buffer have completed (their commit also frees the operand tile)
-      if (use > 0) mbar_wait(&full[p], (uint32_t)((use - 1) & 1));
-      DBG_ACC(0);
-      const int t = blockIdx.x + it * gridDim.x;
-      const int cg = t % ncg, bh = t / ncg;
-      if (!INVERSE) {
-        // x[b,h,:,cg*128 .. +128) -> MN-major B operand (K = w, N = channel).  One cp.async
-        // instruction = 2 rows x 16 consecutive 16-byte chunks: full sectors on the global side
-        const __nv_bfloat16* xrow = in + (size_t)bh * W * C + cg * CGRP;
-        const int mc = lane & 15;
-        const bool cok = cg * CGRP + mc * 8 < C;
-        for (int w = 2 * sub + (lane >> 4); w < W; w += 2 * kRowProdWarps)
-          if (cok) cp_async16(dst + mc * kRowSbo + w * 16, xrow + (size_t)w * C + mc * 8);
-      } else {
-        // A2[b][kw][j][h][ri][cl] (rows kA2Row elements apart) gathered into the MN-major B operand
-        // (K = (ri,kw), N = channel)
-        const int b = bh / H, h = bh - b * H;
-        const size_t kwstride = (size_t)nb * H * kA2Row;
-        const __nv_bfloat16* base = in + ((size_t)b * Kw * nb * H + h) * kA2Row;
-        const int mc = lane & 15;
-        const int c0 = cg * CGRP + mc * 8;
-        const int j = c0 / BS, cl = c0 - j * BS;
-        const __nv_bfloat16* cbase = base + (size_t)j * H * kA2Row + cl;
-        for (int rr = 2 * sub + (lane >> 4); rr < 2 * Kw; rr += 2 * kRowProdWarps) {
-          const int ri = rr >= Kw ? 1 : 0, kw = rr - ri * Kw;
-          if (c0 < C) cp_async16(dst + mc * kRowSbo + (ri * BS + kw) * 16, cbase + (size_t)kw * kwstride + ri * BS);
-        }
+  if (warp == 3) {
+    // ===== TMA producer: tile it -> slot it % 4, up to 3 tiles ahead of the epilogue ===============
+    if (elect_one()) {
+      for (int it = 0; it < nmine; ++it) {
+        const int s = it % kWfSlots;
+        if (it >= kWfSlots) mbar_wait(&sfree[s], (uint32_t)((it / kWfSlots - 1) & 1));
+        const int t = blockIdx.x + it * gridDim.x;
+        const int j = t % nb, bh = t / nb;
+        mbar_expect_tx(&full[s], kW2Tile);
+#pragma unroll
+        for (int pn = 0; pn < 3; ++pn) tma_load3(aS + s * kW2Tile + pn * kPanel, &mapX, j * BS + pn * 32, 0, bh, &full[s]);
       }
-      DBG_ACC(1);
-      cp_async_wait_all();
-      DBG_ACC(2);
-      fence_async_smem();
-      asm volatile("bar.sync %0, %1;" ::"r"(1 + p), "n"(kRowProdWarps * 32) : "memory");
-      DBG_ACC(3);
-      if (sub == 0 && elect_one()) {
-        // the epilogue has drained this accumulator pair's previous contents
-        if (use > 0) mbar_wait(&empty[p], (uint32_t)((use - 1) & 1));
-        DBG_ACC(4);
-        tc_fence_after();
+    }
+    __syncwarp();
+  } else if (warp == 7) {
+    // ===== MMA issuer: accumulator pair it & 1 = (re 96 | im 96) columns =============================
+    const uint32_t idesc = idesc_bf16(128, BS, kIdescBMn);
+    for (int it = 0; it < nmine; ++it) {
+      const int s = it % kWfSlots, pa = it & 1;
+      mbar_wait(&full[s], (uint32_t)((it / kWfSlots) & 1));
+      if (it >= 2) mbar_wait(&accempty[pa], (uint32_t)((it / 2 - 1) & 1));
+      tc_fence_after();
+      if (elect_one()) {
+        const uint32_t bt = aS + s * kW2Tile;
 #pragma unroll
         for (int a = 0; a < 2; ++a) {
-          const uint32_t d = tmem + p * 256 + a * CGRP;
-          const uint32_t am = smem_u32(sF) + a * kFwHalf;
+          const uint32_t d = tmem + pa * 256 + a * BS;
 #pragma unroll
           for (int ks = 0; ks < WP / 16; ++ks)
-            mma_ss(d, smem_desc(am + ks * 2 * kFwLbo, kFwLbo, kFwSbo), smem_desc(dst + ks * 2 * kRowLbo, kRowLbo, kRowSbo),
-                   idesc, ks > 0);
+            mma_ss(d, smem_desc(aF + a * kF2Half + ks * 2 * kF2Lbo, kF2Lbo, kF2Sbo),
+                   smem_desc_sw64(bt + ks * 1024, kPanel, 512), idesc, ks > 0);
         }
-        mma_commit(&full[p]);
-        DBG_ACC(5);
+        mma_commit(&accfull[pa]);
       }
       __syncwarp();
     }
-#ifdef AFNO_TIMING
-    if (blockIdx.x == 0 && p == 0 && sub == 0 && lane == 0)
-      for (int q = 0; q < 8; ++q) g_afno_dbg[(INVERSE ? 16 : 0) + q] = dbg_acc[q];
-#endif
   } else {
-    // ===== epilogue warps: accumulator a = warp / 4, row m = 32 * (warp % 4) + lane ====================
-    const int a = warp >> 2;
-    const int m = (warp & 3) * 32 + lane;
-    const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
-#ifdef AFNO_TIMING
-    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-#endif
-    DBG_T0();
+    // ===== epilogue warps 0,1,2 (re) and 4,5,6 (im): row kw = 32 * (warp % 4) + lane ==================
+    const int a = warp >> 2, q4 = warp & 3;
+    const int kw = q4 * 32 + lane;
+    const uint32_t lane_base = (uint32_t)(q4 * 32) << 16;
     for (int it = 0; it < nmine; ++it) {
+      const int s = it % kWfSlots, pa = it & 1;
       const int t = blockIdx.x + it * gridDim.x;
-      const int cg = t % ncg, bh = t / ncg;
-      // forward: row = frequency kw of part ri = a ; inverse: row = w = 128 a + m
-      const int row = INVERSE ? a * 128 + m : m;
-      const bool rvalid = INVERSE ? (row < W) : (row < Kw);
-      const bool warp_has_rows = INVERSE ? (a * 128 + (warp & 3) * 32 < W) : ((warp & 3) * 32 < Kw);
-      const int b = bh / H, h = bh - b * H;
-      mbar_wait(&full[it & 1], (uint32_t)((it >> 1) & 1));
-      DBG_ACC(0);
+      const int j = t % nb, bh = t / nb, b = bh / H, h = bh - b * H;
+      mbar_wait(&accfull[pa], (uint32_t)((it >> 1) & 1));
       tc_fence_after();
-      const uint32_t acc = tmem + (it & 1) * 256 + a * CGRP + lane_base;
-      if (warp_has_rows) {
-#pragma unroll 1
-        for (int k = 0; k < 4; ++k) {
-          const int c = cg * CGRP + 32 * k;   // 32 channels of one block (96 = 3 * 32)
-          uint32_t v[32], pk[16];
-          tmem_ld32(acc + 32 * k, v);
-          if (!INVERSE) {
-            tmem_wait_ld();
-            if (k == 3) {
-              tc_fence_before();
-              mbar_arrive(&empty[it & 1]);
-            }
-            pack32(v, pk);
-            if (rvalid && c < C) {
-              const int j = c / BS, cl = c - j * BS;
-              __nv_bfloat16* dstp = out + ((((size_t)b * Kw + row) * nb + j) * H + h) * NT + a * BS + cl;
-#ifndef AFNO_DBG_NO_STORE
-              stg256(dstp, pk);
-              stg256(dstp + 16, pk + 8);
-#else
-              if (pk[0] == 0x12345u) stg256(dstp, pk);
-#endif
-            }
-          } else {
-            uint32_t r0[8] = {0, 0, 0, 0, 0, 0, 0, 0}, r1[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-            const size_t off = ((size_t)bh * W + row) * C + c;
-            const bool ok = rvalid && c < C;
-            if (ok && res) {
-              ldg256(res + off, r0);
-              ldg256(res + off + 16, r1);
-            }
-            tmem_wait_ld();
-            if (k == 3) {
-              tc_fence_before();
-              mbar_arrive(&empty[it & 1]);
-            }
+      const uint32_t acc = tmem + pa * 256 + a * BS + lane_base;
+      // the tile's own operand slot is free (its MMAs have completed): stage the output rows there
+      uint8_t* row = smem + kF2Bytes + s * kW2Tile + kw * kOutStride + a * (BS * 2);
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
-              // bf16 -> fp32 is a 16-bit shift; one rounding of (residual + branch)
-              pk[q] = pack_bf16(__uint_as_float(v[2 * q]) + __uint_as_float(r0[q] << 16),
-                                __uint_as_float(v[2 * q + 1]) + __uint_as_float(r0[q] & 0xFFFF0000u));
-              pk[8 + q] = pack_bf16(__uint_as_float(v[16 + 2 * q]) + __uint_as_float(r1[q] << 16),
-                                    __uint_as_float(v[16 + 2 * q + 1]) + __uint_as_float(r1[q] & 0xFFFF0000u));
-            }
-            if (ok) {
-              stg256(out + off, pk);
-              stg256(out + off + 16, pk + 8);
-            }
+      for (int k = 0; k < 3; ++k) {
+        uint32_t v[32], pk[16];
+        tmem_ld32(acc + 32 * k, v);
+        tmem_wait_ld();
+        if (k == 2) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&accempty[pa]);
+        }
+        pack32(v, pk);
+        if (kw < Kw) {
+#pragma unroll
+          for (int g = 0; g < 4; ++g)
+            *(uint4*)(row + k * 64 + g * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
+        }
+      }
+      fence_async_smem();
+      asm volatile("bar.sync 1, 192;" ::: "memory");
+      if (warp == 0 && elect_one()) {
+        tma_store5(&mapA1, 0, h, j, 0, b, aS + s * kW2Tile);
+        bulk_commit();
+        if (it > 0) {
+          bulk_wait_read<1>();   // the previous tile's store has read its slot
+          mbar_arrive(&sfree[(it - 1) % kWfSlots]);
+        }
+      }
+      __syncwarp();
+    }
+    if (warp == 0 && elect_one()) bulk_wait<0>();
+    __syncwarp();
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<512>(tmem);
+}
+
+// inverse: operand ring of 2 tiles (A2 rows as K = ri * 96 + kw) and a ring of 2 residual / output tiles
+__global__ void __launch_bounds__(kW2Threads, 1)
+tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ CUtensorMap mapRes,
+             const __grid_constant__ CUtensorMap mapY, const uint8_t* __restrict__ Gimg, int ntiles, int nb, int H, int W,
+             int has_res) {
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t ofull[2], rfull[2], rfree[2], accfull[2], accempty[2];
+  __shared__ uint32_t tmem_slot;
+  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t* smem = smem_raw + (base - smem_u32(smem_raw));
+  const uint32_t aG = base, aO = base + kG2Bytes, aR = aO + 2 * kW2Tile;
+  uint8_t* sR = smem + kG2Bytes + 2 * kW2Tile;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  for (uint32_t i = tid; i < kG2Bytes / 16; i += kW2Threads) cp_async16(aG + i * 16, Gimg + (size_t)i * 16);
+  if (!has_res)
+    for (uint32_t i = tid; i < 2 * kW2Tile / 16; i += kW2Threads) ((uint4*)sR)[i] = make_uint4(0, 0, 0, 0);
+  if (tid == 0) {
+    for (int q = 0; q < 2; ++q) {
+      mbar_init(&ofull[q], 1);
+      mbar_init(&rfull[q], 1);
+      mbar_init(&rfree[q], 1);
+      mbar_init(&accfull[q], 1);
+      mbar_init(&accempty[q], 6);
+    }
+    mbar_init_fence();
+    tma_prefetch_desc(&mapA2);
+    tma_prefetch_desc(&mapRes);
+    tma_prefetch_desc(&mapY);
+  }
+  if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  cp_async_wait_all();
+  fence_async_smem();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+
+  if (warp == 6) {
+    // ===== TMA producer =============================================================================
+    if (elect_one()) {
+      for (int it = 0; it < nmine; ++it) {
+        const int s = it & 1;
+        const int t = blockIdx.x + it * gridDim.x;
+        const int j = t % nb, bh = t / nb, b = bh / H, h = bh - b * H;
+        // operand slot s: its previous tile's MMAs have completed
+        if (it >= 2) mbar_wait(&accfull[s], (uint32_t)((it / 2 - 1) & 1));
+        mbar_expect_tx(&ofull[s], kW2Tile);
+#pragma unroll
+        for (int pn = 0; pn < 6; ++pn)   // panel pn = ri * 3 + n -> K rows ri * 96.., N panel n
+          tma_load5(aO + s * kW2Tile + (pn % 3) * kPanel + (pn / 3) * (BS * 64), &mapA2, 0, pn, j * H + h, 0, b, &ofull[s]);
+        if (has_res) {
+          if (it >= 2) mbar_wait(&rfree[s], (uint32_t)((it / 2 - 1) & 1));
+          mbar_expect_tx(&rfull[s], kW2Tile);
+#pragma unroll
+          for (int pn = 0; pn < 3; ++pn) tma_load3(aR + s * kW2Tile + pn * kPanel, &mapRes, j * BS + pn * 32, 0, bh, &rfull[s]);
+        }
+      }
+    }
+    __syncwarp();
+  } else if (warp == 7) {
+    // ===== MMA issuer: accumulators a = w / 128 at columns a * 96 of pair it & 1 ======================
+    const uint32_t idesc = idesc_bf16(128, BS, kIdescBMn);
+    for (int it = 0; it < nmine; ++it) {
+      const int s = it & 1;
+      mbar_wait(&ofull[s], (uint32_t)((it >> 1) & 1));
+      if (it >= 2) mbar_wait(&accempty[s], (uint32_t)((it / 2 - 1) & 1));
+      tc_fence_after();
+      if (elect_one()) {
+        const uint32_t bt = aO + s * kW2Tile;
+#pragma unroll
+        for (int ks = 0; ks < WP / 16; ++ks)
+          mma_ss(tmem + s * 256, smem_desc(aG + ks * 2 * kFwLbo, kFwLbo, kFwSbo), smem_desc_sw64(bt + ks * 1024, kPanel, 512),
+                 idesc, ks > 0);
+#pragma unroll
+        for (int ks = 0; ks < WP / 16; ++ks)
+          mma_ss(tmem + s * 256 + BS, smem_desc(aG + kFwHalf + ks * 2 * kG2Lbo1, kG2Lbo1, kFwSbo),
+                 smem_desc_sw64(bt + ks * 1024, kPanel, 512), idesc, ks > 0);
+        mma_commit(&accfull[s]);
+      }
+      __syncwarp();
+    }
+  } else {
+    // ===== epilogue warps 0..3 (w < 128) and 4, 5 (w = 128..191): row w = 128 a + 32 (warp % 4) + lane ==
+    const int a = warp >> 2, q4 = warp & 3;
+    const int w = a * 128 + q4 * 32 + lane;
+    const uint32_t lane_base = (uint32_t)(q4 * 32) << 16;
+    for (int it = 0; it < nmine; ++it) {
+      const int s = it & 1;
+      const int t = blockIdx.x + it * gridDim.x;
+      const int j = t % nb, bh = t / nb;
+      uint8_t* rt = sR + s * kW2Tile;
+      if (has_res) {
+        mbar_wait(&rfull[s], (uint32_t)((it >> 1) & 1));
+      } else if (it >= 2) {
+        // no residual load to wait for: the slot's previous store must have read it
+        mbar_wait(&rfree[s], (uint32_t)((it / 2 - 1) & 1));
+      }
+      mbar_wait(&accfull[s], (uint32_t)((it >> 1) & 1));
+      tc_fence_after();
+      const uint32_t acc = tmem + s * 256 + a * BS + lane_base;
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        uint32_t v[32];
+        tmem_ld32(acc + 32 * k, v);
+        tmem_wait_ld();
+        if (k == 2) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&accempty[s]);
+        }
+        if (w < W) {
+          uint8_t* pan = rt + k * kPanel;
+#pragma unroll
+          for (int g = 0; g < 4; ++g) {
+            uint4* ptr = (uint4*)(pan + sw64_off(w, g));
+            uint4 r = make_uint4(0, 0, 0, 0);
+            if (has_res) r = *ptr;
+            // bf16 -> fp32 is a 16-bit shift; one rounding of (residual + branch)
+            uint4 o;
+            o.x = pack_bf16(__uint_as_float(v[8 * g + 0]) + __uint_as_float(r.x << 16),
+                            __uint_as_float(v[8 * g + 1]) + __uint_as_float(r.x & 0xFFFF0000u));
+            o.y = pack_bf16(__uint_as_float(v[8 * g + 2]) + __uint_as_float(r.y << 16),
+                            __uint_as_float(v[8 * g + 3]) + __uint_as_float(r.y & 0xFFFF0000u));
+            o.z = pack_bf16(__uint_as_float(v[8 * g + 4]) + __uint_as_float(r.z << 16),
+                            __uint_as_float(v[8 * g + 5]) + __uint_as_float(r.z & 0xFFFF0000u));
+            o.w = pack_bf16(__uint_as_float(v[8 * g + 6]) + __uint_as_float(r.w << 16),
+                            __uint_as_float(v[8 * g + 7]) + __uint_as_float(r.w & 0xFFFF0000u));
+            *ptr = o;
           }
         }
-      } else {
-        tc_fence_before();
-        mbar_arrive(&empty[it & 1]);
       }
-      DBG_ACC(1);
+      fence_async_smem();
+      asm volatile("bar.sync 1, 192;" ::: "memory");
+      if (warp == 0 && elect_one()) {
+#pragma unroll
+        for (int pn = 0; pn < 3; ++pn) tma_store3(&mapY, j * BS + pn * 32, 0, bh, aR + s * kW2Tile + pn * kPanel);
+        bulk_commit();
+        if (it > 0) {
+          bulk_wait_read<1>();
+          mbar_arrive(&rfree[(it - 1) & 1]);
+        }
+      }
+      __syncwarp();
     }
-#ifdef AFNO_TIMING
-    if (blockIdx.x == 0 && warp == 0 && lane == 0) {
-      g_afno_dbg[(INVERSE ? 16 : 0) + 8] = dbg_acc[0];
-      g_afno_dbg[(INVERSE ? 16 : 0) + 9] = dbg_acc[1];
-      g_afno_dbg[(INVERSE ? 16 : 0) + 10] = nmine;
-    }
-#endif
+    if (warp == 0 && elect_one()) bulk_wait<0>();
+    __syncwarp();
   }
   tc_fence_before();
   __syncthreads();
@@ -333,11 +413,11 @@ struct MixParams {
 
 // rows of a (b,kw,j) tile [H][192] -> MN-major B operand (K = h, N = (ri, c)); loader warp `sub`
 __device__ __forceinline__ void load_tile_warp(uint32_t tile_saddr, const __nv_bfloat16* src, int H, int lane, int sub) {
-  // the tile is contiguous in global memory: chunk q = 16 bytes at src + 8 q, row h = q / 24
+  // rows of kA2Row elements: chunk q = 16 bytes at src + row h = q / 24, chunk nc = q % 24
   const int nchunks = H * (NT / 8);
   for (int q = sub * 32 + lane; q < nchunks; q += kMixLoadWarps * 32) {
     const int h = q / (NT / 8), nc = q - h * (NT / 8);
-    cp_async16(tile_saddr + nc * kTileSbo + h * 16, src + (size_t)q * 8);
+    cp_async16(tile_saddr + nc * kTileSbo + h * 16, src + (size_t)h * kA2Row + nc * 8);
   }
 }
 
@@ -361,10 +441,7 @@ __device__ __forceinline__ void load_tile_warp(uint32_t tile_saddr, const __nv_b
 constexpr int kMix2Threads = 512;
 constexpr uint32_t kDft2Lbo = 1536, kDft2Sbo = 128;  // Ch / Sh: K-major A, 96 stored rows, order [k/8][m/8 < 12]
 constexpr uint32_t kDft2Bytes = 12 * kDft2Lbo;        // 18432 (rows 96..127 alias the next k-chunk: finite, unused)
-// A tile buffer is also the staging area of the tile's output rows.  Rows are 400 bytes apart, in
-// shared memory (eight consecutive rows fall into distinct 16-byte bank groups) AND in the global
-// A2 tensor, so that a whole tile leaves with ONE bulk copy (async proxy, no L1 traffic).
-constexpr uint32_t kOutStride = 2 * kA2Row;           // 400
+// A tile buffer is also the staging area of the tile's output rows (kOutStride apart).
 constexpr uint32_t kTileBuf = 96 * kOutStride;        // 38400 >= kTileBytes
 constexpr uint32_t kMix2Smem = 2 * kDft2Bytes + 4 * kWBytes + 3 * kTileBuf; // 225792
 constexpr uint32_t kSlot = 96;
@@ -373,10 +450,8 @@ constexpr uint32_t kSlot = 96;
 __device__ __forceinline__ void bulk_store(void* dst, uint32_t src_smem, uint32_t bytes) {
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src_smem), "r"(bytes)
                : "memory");
-  asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+  bulk_commit();
 }
-__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
-__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
 struct Mix2Bars {
   uint64_t dfull[2];  // stream's current stage accumulated (tcgen05.commit)
@@ -554,7 +629,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
     // ================================ loader warps (7, 11, 15) ================================
     const int sub = (warp >> 2) - 1;
     const uint32_t aT = smem_u32(sT);
-    auto tile_off = [&](int i) { return ((size_t)(s0 + i * S) * p.nb + j) * p.H * NT; };
+    auto tile_off = [&](int i) { return ((size_t)(s0 + i * S) * p.nb + j) * p.H * kA2Row; };
     auto load = [&](int buf, const __nv_bfloat16* src, uint64_t* full) {
       // rows H..95 of the operand are K padding: the output staging of the buffer's previous tile
       // overlaps them, so they are cleared again
@@ -577,7 +652,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
           mbar_wait(&bars.sdone[buf], par);
           bulk_store(p.A2 + ((size_t)(s0 + k * S) * p.nb + j) * p.H * kA2Row, aT + buf * kTileBuf,
                      (uint32_t)p.H * kOutStride);
-          bulk_wait_read();
+          bulk_wait_read<0>();
           mbar_arrive(&bars.tfree[buf]);
         }
         __syncwarp();
@@ -608,7 +683,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
         }
       }
     }
-    if (sub == 0 && lane == 0) bulk_wait_all();
+    if (sub == 0 && lane == 0) bulk_wait<0>();
   } else if (warp == 3) {
     // ================================ control warp ===========================================
     const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW), aT = smem_u32(sT);
@@ -862,9 +937,6 @@ __device__ __forceinline__ void bulk_copy(uint32_t dst_smem, const void* src, ui
                "l"(src), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
 }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
 
 // Aws / Gws: operand-image tensors written by tc_mix<true> ([tile][24 chunks][kTileSbo bytes]).
 __global__ void __launch_bounds__(128, 1)
@@ -1007,6 +1079,47 @@ cudaError_t set_smem(K kernel, size_t bytes) {
   return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
+// ---- tensor maps (encoded per call on the host: they hold the caller's pointers) -----------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+// bf16 tensor, dims[0] fastest; strides_bytes[i] = byte stride of dims[i + 1]
+bool make_tmap(const TcPlan& tp, CUtensorMap* m, const void* base, int rank, const uint64_t* dims,
+               const uint64_t* strides_bytes, const uint32_t* box, bool swizzle64) {
+  cuuint32_t es[5] = {1, 1, 1, 1, 1};
+  cuuint64_t d[5], st[4];
+  for (int i = 0; i < rank; ++i) d[i] = dims[i];
+  for (int i = 0; i + 1 < rank; ++i) st[i] = strides_bytes[i];
+  return ((EncodeTiledFn)tp.encode_tiled)(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, (cuuint32_t)rank, const_cast<void*>(base), d, st,
+                                          box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                          swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                                          CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+// activation tensor [B*H][W][C] as 64B-swizzled [192 x 32] panels (rows past W: zero-filled / not stored)
+bool act_tmap(const TcPlan& tp, CUtensorMap* m, const void* ptr, const Geometry& g) {
+  const uint64_t dims[3] = {(uint64_t)g.C, (uint64_t)g.W, (uint64_t)g.B * g.H};
+  const uint64_t str[2] = {(uint64_t)g.C * 2, (uint64_t)g.W * g.C * 2};
+  const uint32_t box[3] = {32, WP, 1};
+  return make_tmap(tp, m, ptr, 3, dims, str, box, true);
+}
+// half-spectrum [b][kw][j][h][kA2Row] written by tc_wdft_fwd2: one box = rows kw = 0..Kw-1 of (b, j, h)
+bool spec_store_tmap(const TcPlan& tp, CUtensorMap* m, const void* ptr, const Geometry& g) {
+  const uint64_t row = kOutStride;
+  const uint64_t dims[5] = {(uint64_t)kA2Row, (uint64_t)g.H, (uint64_t)g.nb, (uint64_t)g.Kw, (uint64_t)g.B};
+  const uint64_t str[4] = {row, row * g.H, row * g.H * g.nb, row * g.H * g.nb * g.Kw};
+  const uint32_t box[5] = {(uint32_t)kA2Row, 1, 1, (uint32_t)g.Kw, 1};
+  return make_tmap(tp, m, ptr, 5, dims, str, box, false);
+}
+// the same tensor read by tc_wdft_inv2: one box = 32 channels of one (re | im) part, rows kw = 0..95
+// (zero-filled past Kw), 64B-swizzled
+bool spec_load_tmap(const TcPlan& tp, CUtensorMap* m, const void* ptr, const Geometry& g) {
+  const uint64_t row = kOutStride;
+  const uint64_t dims[5] = {32, 6, (uint64_t)g.nb * g.H, (uint64_t)g.Kw, (uint64_t)g.B};
+  const uint64_t str[4] = {64, row, row * g.H * g.nb, row * g.H * g.nb * g.Kw};
+  const uint32_t box[5] = {32, 1, 1, (uint32_t)BS, 1};
+  return make_tmap(tp, m, ptr, 5, dims, str, box, true);
+}
+
 struct TcWs {
   __nv_bfloat16 *A1, *A2, *wprep;
   float* bprep;
@@ -1031,9 +1144,9 @@ TcWs tc_carve(const Geometry& g, bool backward, char* base) {
     w.mask2 = (uint8_t*)take(b2);
     w.mask_region = off;
   }
-  const size_t spec = (size_t)g.B * g.Kw * g.nb * g.H * NT * 2;
+  const size_t spec = (size_t)g.B * g.Kw * g.nb * g.H * kA2Row * 2;
   w.A1 = (__nv_bfloat16*)take(spec);
-  w.A2 = (__nv_bfloat16*)take((size_t)g.B * g.Kw * g.nb * g.H * kA2Row * 2);
+  w.A2 = (__nv_bfloat16*)take(spec);
   w.wprep = (__nv_bfloat16*)take((size_t)g.nb * 4 * kWBytes);
   w.bprep = (float*)take((size_t)g.nb * 2 * NT * sizeof(float));
   if (backward) {
@@ -1071,19 +1184,20 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
       dft2[off] = host_bf16(cos(a) * s);
       dft2[kDft2Bytes / 2 + off] = host_bf16(sin(a) * s);
     }
-  // W-direction constants as K-major A operands, two 128-row halves each (kFwHalf bytes):
-  //   Fw  half ri : element (m = kw, k = w)          = {cos, -sin}(2 pi kw w / W) / sqrt(W)   [x alpha_kw]
-  //   Gw  half a  : element (m = w - 128 a, k = ri*96 + kw) = alpha_kw {cos, -sin}(...) / sqrt(W)  [or alpha = 1]
-  std::vector<uint16_t> fw(kFwBytes / 2, 0), fwa(kFwBytes / 2, 0), gw(kFwBytes / 2, 0), gw1(kFwBytes / 2, 0);
-  auto aoff = [](int m, int k) { return ((k / 8) * kFwLbo + (m / 8) * kFwSbo + (m % 8) * 16 + (k % 8) * 2) / 2; };
+  // W-direction constants as K-major A operands (element (m, k) at (k/8)*LBO + (m/8)*128 + (m%8)*16 + (k%8)*2):
+  //   Fw half ri (96 rows stored, LBO kF2Lbo): (m = kw, k = w) = {cos, -sin}(2 pi kw w / W) / sqrt(W)  [x alpha_kw]
+  //   Gw half 0 (128 rows, LBO kFwLbo), half 1 (56 rows, LBO kG2Lbo1):
+  //      (m = w - 128 a, k = ri*96 + kw) = alpha_kw {cos, -sin}(...) / sqrt(W)                       [or alpha = 1]
+  std::vector<uint16_t> fw(kF2Bytes / 2, 0), fwa(kF2Bytes / 2, 0), gw(kG2Bytes / 2, 0), gw1(kG2Bytes / 2, 0);
+  auto aoff = [](int m, int k, uint32_t lbo) { return ((k / 8) * lbo + (m / 8) * 128 + (m % 8) * 16 + (k % 8) * 2) / 2; };
   for (int kw = 0; kw < Wh; ++kw)
     for (int w = 0; w < W; ++w) {
       const double a = two_pi * (double)((long)kw * w % W) / (double)W, s = 1.0 / sqrt((double)W);
       const double alpha = (kw == 0 || 2 * kw == W) ? 1.0 : 2.0;
       for (int ri = 0; ri < 2; ++ri) {
         const double v = (ri == 0 ? cos(a) : -sin(a)) * s;
-        const uint32_t of = ri * (kFwHalf / 2) + aoff(kw, w);
-        const uint32_t og = (w / 128) * (kFwHalf / 2) + aoff(w % 128, ri * BS + kw);
+        const uint32_t of = ri * (kF2Half / 2) + aoff(kw, w, kF2Lbo);
+        const uint32_t og = w < 128 ? aoff(w, ri * BS + kw, kFwLbo) : kFwHalf / 2 + aoff(w - 128, ri * BS + kw, kG2Lbo1);
         fw[of] = host_bf16(v);
         fwa[of] = host_bf16(v * alpha);
         gw[og] = host_bf16(v * alpha);
@@ -1095,8 +1209,13 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
   if (e == cudaSuccess) e = upload(fwa, &out->fw_alpha);
   if (e == cudaSuccess) e = upload(gw, &out->gw);
   if (e == cudaSuccess) e = upload(gw1, &out->gw_noalpha);
-  if (e == cudaSuccess) e = set_smem(tc_wdft<false>, kRowSmem);
-  if (e == cudaSuccess) e = set_smem(tc_wdft<true>, kRowSmem);
+  if (e == cudaSuccess) e = set_smem(tc_wdft_fwd2, kWfSmem);
+  if (e == cudaSuccess) e = set_smem(tc_wdft_inv2, kWiSmem);
+  if (e == cudaSuccess) {
+    cudaDriverEntryPointQueryResult q;
+    e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &out->encode_tiled, cudaEnableDefault, &q);
+    if (e == cudaSuccess && (q != cudaDriverEntryPointSuccess || out->encode_tiled == nullptr)) e = cudaErrorNotSupported;
+  }
   if (e == cudaSuccess) e = set_smem(tc_mix2<false, false>, kMix2Smem);
   if (e == cudaSuccess) e = set_smem(tc_mix2<true, false>, kMix2Smem);
   if (e == cudaSuccess) e = set_smem(tc_mix2<true, true>, kMix2Smem);
@@ -1121,6 +1240,33 @@ size_t tc_workspace_bytes(const Geometry& g, bool backward) {
   return tc_carve(g, backward, nullptr).total;
 }
 
+// W-direction launches: tile = (b, h, block), persistent over the SMs
+static cudaError_t launch_wdft_fwd(const Geometry& g, const TcPlan& tp, const void* in, void* spec, const uint8_t* fimg,
+                                   cudaStream_t st) {
+  CUtensorMap mx, ma;
+  if (!act_tmap(tp, &mx, in, g) || !spec_store_tmap(tp, &ma, spec, g)) return cudaErrorInvalidValue;
+  const int ntiles = g.B * g.H * g.nb;
+  const int grid = ntiles < tp.num_sms ? ntiles : tp.num_sms;
+  prof_begin("tc_wdft_fwd", st);
+  tc_wdft_fwd2<<<grid, kW2Threads, kWfSmem, st>>>(mx, ma, fimg, ntiles, g.nb, g.H, g.Kw);
+  prof_end(st);
+  count_launch();
+  return cudaGetLastError();
+}
+static cudaError_t launch_wdft_inv(const Geometry& g, const TcPlan& tp, const void* spec, const void* res, void* out,
+                                   const uint8_t* gimg, cudaStream_t st) {
+  CUtensorMap ma, mr, my;
+  if (!spec_load_tmap(tp, &ma, spec, g) || !act_tmap(tp, &mr, res ? res : out, g) || !act_tmap(tp, &my, out, g))
+    return cudaErrorInvalidValue;
+  const int ntiles = g.B * g.H * g.nb;
+  const int grid = ntiles < tp.num_sms ? ntiles : tp.num_sms;
+  prof_begin("tc_wdft_inv", st);
+  tc_wdft_inv2<<<grid, kW2Threads, kWiSmem, st>>>(ma, mr, my, gimg, ntiles, g.nb, g.H, g.W, res ? 1 : 0);
+  prof_end(st);
+  count_launch();
+  return cudaGetLastError();
+}
+
 cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const float* w1, const float* b1,
                        const float* w2, const float* b2, void* y, void* ws, cudaStream_t st) {
   // SAVE_CONTEXT: the backward layout, so that tc_backward finds A1 where it expects it
@@ -1133,15 +1279,7 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  const int ncg = (g.C + CGRP - 1) / CGRP;
-  const int row_tiles = g.B * g.H * ncg;
-  const int grid_row = row_tiles < tp.num_sms ? row_tiles : tp.num_sms;
-  prof_begin("tc_wdft_fwd", st);
-  tc_wdft<false><<<grid_row, kRowThreads, kRowSmem, st>>>((const __nv_bfloat16*)x, nullptr, w.A1, tp.fw, g.B, g.H, g.W,
-                                                          g.C, g.Kw, g.nb);
-  prof_end(st);
-  count_launch();
-  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  if ((e = launch_wdft_fwd(g, tp, x, w.A1, tp.fw, st)) != cudaSuccess) return e;
   MixParams mp{};
   mp.A1 = w.A1; mp.A2 = w.A2; mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
   mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
@@ -1151,12 +1289,7 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  prof_begin("tc_wdft_inv", st);
-  tc_wdft<true><<<grid_row, kRowThreads, kRowSmem, st>>>(w.A2, g.no_residual ? nullptr : (const __nv_bfloat16*)x,
-                                                         (__nv_bfloat16*)y, tp.gw, g.B, g.H, g.W, g.C, g.Kw, g.nb);
-  prof_end(st);
-  count_launch();
-  return cudaGetLastError();
+  return launch_wdft_inv(g, tp, w.A2, g.no_residual ? nullptr : x, y, tp.gw, st);
 }
 
 cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const void* dy, const float* w1,
@@ -1176,16 +1309,11 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
     if ((e = cudaMemsetAsync(ws, 0, w.mask_region, st)) != cudaSuccess) return e;
   }
   TC_LAUNCH("k_tc_prep_weights", k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, w.wprep, w.bprep, g.nb));
-  const int ncg = (g.C + CGRP - 1) / CGRP;
-  const int row_tiles = g.B * g.H * ncg;
-  const int grid_row = row_tiles < tp.num_sms ? row_tiles : tp.num_sms;
   // B1 (first half) and B2: W-direction spectra of x and of dy (alpha-weighted)
   if (!g.use_ctx) {
-    TC_LAUNCH("tc_wdft_fwd", tc_wdft<false><<<grid_row, kRowThreads, kRowSmem, st>>>((const __nv_bfloat16*)x, nullptr, w.A1,
-                                                                                    tp.fw, g.B, g.H, g.W, g.C, g.Kw, g.nb));
+    if ((e = launch_wdft_fwd(g, tp, x, w.A1, tp.fw, st)) != cudaSuccess) return e;
   }
-  TC_LAUNCH("tc_wdft_fwd", tc_wdft<false><<<grid_row, kRowThreads, kRowSmem, st>>>((const __nv_bfloat16*)dy, nullptr, w.A1g,
-                                                                                  tp.fw_alpha, g.B, g.H, g.W, g.C, g.Kw, g.nb));
+  if ((e = launch_wdft_fwd(g, tp, dy, w.A1g, tp.fw_alpha, st)) != cudaSuccess) return e;
   MixParams mp{};
   mp.A1 = w.A1; mp.A1g = w.A1g; mp.A2 = w.A2;
   mp.Xh = w.Xh; mp.O1 = w.O1; mp.G2 = w.G2; mp.G1 = w.G1;
@@ -1207,12 +1335,9 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   TC_LAUNCH("tc_wgrad", tc_wgrad<<<g.nb * w.S, 128, kWgSmem, st>>>(w.Xh, w.G1, w.part, g.B * g.Kw, g.H, g.nb, w.S));
   TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce<<<(nred + 255) / 256, 256, 0, st>>>(
                                      w.part, (float2*)dw1, (float2*)db1, g.nb, w.S, g.accum ? 1 : 0));
-  // B8: dx = dy + irfft2(GX / alpha)
-  TC_LAUNCH("tc_wdft_inv", tc_wdft<true><<<grid_row, kRowThreads, kRowSmem, st>>>(
-                               w.A2, g.no_residual ? nullptr : (const __nv_bfloat16*)dy, (__nv_bfloat16*)dx,
-                               tp.gw_noalpha, g.B, g.H, g.W, g.C, g.Kw, g.nb));
 #undef TC_LAUNCH
-  return cudaSuccess;
+  // B8: dx = dy + irfft2(GX / alpha)
+  return launch_wdft_inv(g, tp, w.A2, g.no_residual ? nullptr : dy, dx, tp.gw_noalpha, st);
 }
 
 #ifdef AFNO_TRACE

@@ -355,7 +355,7 @@ def kernel_work(name, B, wl, kept_modes):
         "tc_wdft_inv": dict(bound="hbm", bytes=spec + 2 * act, flops=0.0),
         "tc_mix_fwd": dict(bound="tensor", bytes=2 * spec, flops=2 * gemm),
         "tc_mix_bwd": dict(bound="tensor", bytes=7 * spec, flops=4 * gemm),
-        "tc_wgrad": dict(bound="hbm", bytes=2 * spec, flops=gemm),
+        "tc_wgrad": dict(bound="hbm", bytes=4 * spec, flops=2 * gemm),   # one launch, both layers
         "k_block_gemm": dict(bound="alu", bytes=0, flops=gemm),
         "k_block_wgrad": dict(bound="alu", bytes=0, flops=gemm),
     }

@@ -938,15 +938,20 @@ __device__ __forceinline__ void bulk_copy(uint32_t dst_smem, const void* src, ui
                : "memory");
 }
 
-// Aws / Gws: operand-image tensors written by tc_mix<true> ([tile][24 chunks][kTileSbo bytes]).
+// Operand-image tensors written by tc_mix2<true> ([tile][24 chunks][kTileSbo bytes]).  ONE launch covers
+// both layers: CTAs [0, nb*S) form layer 2 (A = O1, G = G2), CTAs [nb*S, 2*nb*S) layer 1 (A = Xh, G = G1).
 __global__ void __launch_bounds__(128, 1)
-tc_wgrad(const __nv_bfloat16* __restrict__ Aws, const __nv_bfloat16* __restrict__ Gws, float* __restrict__ part,
+tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict__ G_l2,
+         const __nv_bfloat16* __restrict__ A_l1, const __nv_bfloat16* __restrict__ G_l1, float* __restrict__ part,
          int BKw, int H, int nb, int S) {
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ __align__(8) uint64_t full[2], empty[2], done;
   __shared__ uint32_t tmem_slot;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int j = blockIdx.x / S, s = blockIdx.x - j * S;
+  const int layer = blockIdx.x / (nb * S), cta = blockIdx.x - layer * nb * S;
+  const int j = cta / S, s = cta - j * S;
+  const __nv_bfloat16* Aws = layer ? A_l1 : A_l2;
+  const __nv_bfloat16* Gws = layer ? G_l1 : G_l2;
   for (uint32_t i = tid; i < kWgSmem / 16; i += 128) ((uint4*)smem)[i] = make_uint4(0, 0, 0, 0);
   __syncthreads();
   // constant-one column m = 96 of the "re" A operand, rows r < H, both stages
@@ -1032,10 +1037,15 @@ tc_wgrad(const __nv_bfloat16* __restrict__ Aws, const __nv_bfloat16* __restrict_
 }
 
 // dW[j][i][o] = sum_s ( Dre[i][o] + Dim[i][96+o] ,  Dre[i][96+o] - Dim[i][o] ) ;  db[j][o] = sum_s Dre[96][(ri,o)]
-__global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __restrict__ dW, float2* __restrict__ dB,
-                                  int nb, int S, int accumulate) {
+// blockIdx.y = 0: layer 2 partial sums (first nb*S CTAs of tc_wgrad), 1: layer 1
+__global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __restrict__ dW2, float2* __restrict__ dB2,
+                                  float2* __restrict__ dW1, float2* __restrict__ dB1, int nb, int S, int accumulate) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const int nW = nb * BS * BS;
+  const int layer = blockIdx.y;
+  part += (size_t)layer * nb * S * 2 * 128 * NT;
+  float2* dW = layer ? dW1 : dW2;
+  float2* dB = layer ? dB1 : dB2;
   if (idx < nW) {
     const int o = idx % BS, i = (idx / BS) % BS, j = idx / (BS * BS);
     float2 acc = accumulate ? dW[idx] : make_float2(0.f, 0.f);
@@ -1156,11 +1166,11 @@ TcWs tc_carve(const Geometry& g, bool backward, char* base) {
     w.O1 = (__nv_bfloat16*)take(img);
     w.G2 = (__nv_bfloat16*)take(img);
     w.G1 = (__nv_bfloat16*)take(img);
-    int S = 148 / g.nb;
+    int S = 148 / (2 * g.nb);   // CTAs per (layer, block) of tc_wgrad
     if (S < 1) S = 1;
     if (S > g.B * g.Kw) S = g.B * g.Kw;
     w.S = S;
-    w.part = (float*)take((size_t)g.nb * S * 2 * 128 * NT * sizeof(float));
+    w.part = (float*)take((size_t)2 * g.nb * S * 2 * 128 * NT * sizeof(float));
   }
   w.total = off;
   return w;
@@ -1308,7 +1318,11 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   if (g.export_masks) {
     if ((e = cudaMemsetAsync(ws, 0, w.mask_region, st)) != cudaSuccess) return e;
   }
-  TC_LAUNCH("k_tc_prep_weights", k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, w.wprep, w.bprep, g.nb));
+  // USE_CONTEXT: the operand images of the weights written by the forward call are still in the
+  // workspace (the context belongs to one set of parameters)
+  if (!g.use_ctx) {
+    TC_LAUNCH("k_tc_prep_weights", k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, w.wprep, w.bprep, g.nb));
+  }
   // B1 (first half) and B2: W-direction spectra of x and of dy (alpha-weighted)
   if (!g.use_ctx) {
     if ((e = launch_wdft_fwd(g, tp, x, w.A1, tp.fw, st)) != cudaSuccess) return e;
@@ -1329,12 +1343,11 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   }
   // B4 / B6: parameter gradients
   const int nred = nW + g.nb * BS;
-  TC_LAUNCH("tc_wgrad", tc_wgrad<<<g.nb * w.S, 128, kWgSmem, st>>>(w.O1, w.G2, w.part, g.B * g.Kw, g.H, g.nb, w.S));
-  TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce<<<(nred + 255) / 256, 256, 0, st>>>(
-                                     w.part, (float2*)dw2, (float2*)db2, g.nb, w.S, g.accum ? 1 : 0));
-  TC_LAUNCH("tc_wgrad", tc_wgrad<<<g.nb * w.S, 128, kWgSmem, st>>>(w.Xh, w.G1, w.part, g.B * g.Kw, g.H, g.nb, w.S));
-  TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce<<<(nred + 255) / 256, 256, 0, st>>>(
-                                     w.part, (float2*)dw1, (float2*)db1, g.nb, w.S, g.accum ? 1 : 0));
+  TC_LAUNCH("tc_wgrad", tc_wgrad<<<2 * g.nb * w.S, 128, kWgSmem, st>>>(w.O1, w.G2, w.Xh, w.G1, w.part, g.B * g.Kw, g.H,
+                                                                        g.nb, w.S));
+  TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce<<<dim3((nred + 255) / 256, 2), 256, 0, st>>>(
+                                     w.part, (float2*)dw2, (float2*)db2, (float2*)dw1, (float2*)db1, g.nb, w.S,
+                                     g.accum ? 1 : 0));
 #undef TC_LAUNCH
   // B8: dx = dy + irfft2(GX / alpha)
   return launch_wdft_inv(g, tp, w.A2, g.no_residual ? nullptr : dy, dx, tp.gw_noalpha, st);

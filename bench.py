@@ -264,12 +264,12 @@ def run_ours(args):
     Kw = max(1, min(wl.W // 2 + 1, int(np.floor(float(np.float32(wl.kept_fraction)) * (wl.W // 2 + 1)))))
     kept_modes = (2 * Kh - 1 if Kh <= wl.H // 2 else wl.H) * Kw
     work = layer_work(B, wl.H, wl.W, wl.C, wl.num_blocks, kept_modes)
-    roofline = kernel_roofline(dom, dom_n, dom_ms, PROF_STEPS, work, peaks, clocks.summary(), B, wl, kept_modes)
+    roofline = kernel_roofline(dom, dom_n, dom_ms, PROF_STEPS, work, peaks, clocks.summary(), B, wl, kept_modes, ctx)
     roofline["share_of_step"] = dom_ms / total_prof_ms if total_prof_ms > 0 else None
     roofline["kernels_ms_per_step"] = {k: round(v[1] / PROF_STEPS, 4) for k, v in sorted(prof.items())}
     per_kernel = {}
     for k, (n, ms_k) in sorted(prof.items()):
-        r = kernel_roofline(k, n, ms_k, PROF_STEPS, work, peaks, clocks.summary(), B, wl, kept_modes)
+        r = kernel_roofline(k, n, ms_k, PROF_STEPS, work, peaks, clocks.summary(), B, wl, kept_modes, ctx)
         per_kernel[k] = {"bound": r["bound"], "frac": r["frac"], "avg_launch_us": round(r["avg_launch_us"], 2)}
     roofline["per_kernel"] = per_kernel
 
@@ -326,7 +326,7 @@ def run_ours(args):
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[4]: {wl.name}", "B_per_gpu": B, "H": wl.H, "W": wl.W,
                        "C": wl.C, "num_blocks": wl.num_blocks, "lambda": wl.lam, "kept_fraction": wl.kept_fraction,
-                       "path": path, "backward": "saved context (W-direction spectrum of x kept by fwd)" if ctx
+                       "path": path, "backward": "saved context (fwd keeps Xh, O1 and the activation masks; bwd runs the gradient stages only)" if ctx
                        else "stateless (recomputes the spectrum of x)", "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": f"{NSETS} rotating input/output buffer sets of {4 * x0.numel() * 2 / 1e6:.0f} MB "
                              "each (> 126 MB L2), no explicit flush"},
@@ -339,7 +339,7 @@ def run_ours(args):
     return 0
 
 
-def kernel_work(name, B, wl, kept_modes):
+def kernel_work(name, B, wl, kept_modes, ctx=True):
     """Algorithmic work of ONE launch of a kernel (S5 states these figures).
 
     bytes: compulsory HBM traffic of the launch (activations bf16, spectra bf16-complex);
@@ -350,11 +350,13 @@ def kernel_work(name, B, wl, kept_modes):
     act = B * wl.H * wl.W * wl.C * 2                       # one bf16 activation tensor
     spec = B * Kw * wl.num_blocks * wl.H * 2 * bs * 2      # one bf16-complex half-spectrum
     gemm = 2.0 * (2 * bs) * (2 * bs) * wl.num_blocks * kept_modes * B
+    masks = B * Kw * wl.num_blocks * 12 * 32 * 16          # bit-packed activation masks of the saved context
     table = {
         "tc_wdft_fwd": dict(bound="hbm", bytes=act + spec, flops=0.0),
         "tc_wdft_inv": dict(bound="hbm", bytes=spec + 2 * act, flops=0.0),
-        "tc_mix_fwd": dict(bound="tensor", bytes=2 * spec, flops=2 * gemm),
-        "tc_mix_bwd": dict(bound="tensor", bytes=7 * spec, flops=4 * gemm),
+        # saved-context step: fwd also writes Xh, O1 and 18 MB of mask bits; bwd runs the gradient stages only
+        "tc_mix_fwd": dict(bound="tensor", bytes=(4 * spec + masks) if ctx else 2 * spec, flops=2 * gemm),
+        "tc_mix_bwd": dict(bound="tensor", bytes=(4 * spec + masks) if ctx else 7 * spec, flops=(2 if ctx else 4) * gemm),
         "tc_wgrad": dict(bound="hbm", bytes=4 * spec, flops=2 * gemm),   # one launch, both layers
         "k_block_gemm": dict(bound="alu", bytes=0, flops=gemm),
         "k_block_wgrad": dict(bound="alu", bytes=0, flops=gemm),
@@ -371,11 +373,11 @@ def measured_traffic(name):
         return None
 
 
-def kernel_roofline(name, n_launch, total_ms, steps, work, peaks, clocks, B, wl, kept_modes):
+def kernel_roofline(name, n_launch, total_ms, steps, work, peaks, clocks, B, wl, kept_modes, ctx=True):
     """roofline object for the dominant kernel: achieved = algorithmic work of one launch / its
     average duration measured with CUDA events around every launch (afno_profile_*)."""
     per_launch_s = total_ms * 1e-3 / n_launch
-    kw = kernel_work(name, B, wl, kept_modes)
+    kw = kernel_work(name, B, wl, kept_modes, ctx)
     out = {"kernel": name, "launches_per_step": n_launch / steps, "avg_launch_us": per_launch_s * 1e6,
            "traffic": measured_traffic(name)}
     if kw is None:

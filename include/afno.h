@@ -59,10 +59,11 @@ enum {
   AFNO_FLAG_EXPORT_MASKS = 8,    /* bwd only: write ReLU / softshrink masks, see below        */
   /* Saved context (SURVEY.md S8(a) row B1 "or load saved context"): a training step calls fwd
    * and then bwd on the same x.  fwd with SAVE_CONTEXT needs a workspace of
-   * afno_spectral_workspace_bytes(d, 1) bytes and leaves the W-direction half-spectrum of x
-   * (row F1) and the bf16 operand images of w1, b1, w2, b2 in it; bwd with USE_CONTEXT on the
-   * SAME workspace, with the same descriptor (the two context flags aside), the same x and the
-   * same parameter values, reads both instead of recomputing them.
+   * afno_spectral_workspace_bytes(d, 1) bytes and leaves in it the spectrum Xh (rows F1-F2), the
+   * hidden activations O1 (F3-F4), the ReLU / softshrink masks (F4, F6; bit-packed) and the bf16
+   * operand images of w1, b1, w2, b2; bwd with USE_CONTEXT on the SAME workspace, with the same
+   * descriptor (the two context flags aside), the same x and the same parameter values, reads
+   * them instead of recomputing rows B1 (F1-F5) and is bit-identical to the stateless bwd.
    * Nothing else may write the workspace in between.  Kernel families that keep no such
    * intermediate (generic-fp32) accept both flags and recompute. */
   AFNO_FLAG_SAVE_CONTEXT = 16,

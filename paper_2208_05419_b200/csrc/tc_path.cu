@@ -407,6 +407,7 @@ struct MixParams {
   const float* bprep;        // per block [2 layers][192]: (re 96 | im 96)
   uint8_t* mask1;            // optional export, [B][H][Wh][C][2]
   uint8_t* mask2;
+  uint4* maskbits;           // saved context: [tile][12 epilogue warps][32 lanes] {m1[0], m1[1], m2[0], m2[1]}
   int B, H, Kw, Wh, nb, Kh;
   float lambda;
 };
@@ -535,6 +536,12 @@ __device__ __forceinline__ uint32_t shrink_bf16x2(uint32_t a, uint32_t lam2, uin
   asm("sub.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(c));
   return r;
 }
+// Z = S_lambda(a + b) on a packed pair: the sum is rounded to bf16 once, then shrunk (exact zeros inside
+// the threshold; lambda at bf16 precision).  Forward value and backward mask (Z != 0) come from this one
+// function, so the gradient is the gradient of the function the forward pass evaluates.
+__device__ __forceinline__ uint32_t shrink_sum(float v0, float v1, float b0, float b1, uint32_t lam2, uint32_t nlam2) {
+  return shrink_bf16x2(pack_bf16(v0 + b0, v1 + b1), lam2, nlam2);
+}
 // relu + one rounding of two fp32 values to a packed bf16 pair (lo, hi)
 __device__ __forceinline__ uint32_t pack_relu_bf16(float lo, float hi) {
   uint32_t r;
@@ -548,6 +555,11 @@ template <int P>
 __device__ __forceinline__ void mask_collect(uint32_t (&m)[2], uint32_t q) {
   constexpr int s = P % 12;
   m[P / 12] |= ((q + 0x7FFF7FFFu) >> s) & (0x80008000u >> s);
+}
+// the same for signed values
+template <int P>
+__device__ __forceinline__ void mask_collect_signed(uint32_t (&m)[2], uint32_t q) {
+  mask_collect<P>(m, q & 0x7FFF7FFFu);
 }
 // packed bf16 pair with the halves whose mask bit is clear zeroed
 template <int P>
@@ -576,13 +588,20 @@ __device__ __forceinline__ void mbar_wait_fast(uint64_t* mbar, uint32_t parity) 
   }
 }
 
-template <bool BACKWARD, bool EXPORT>
+// MODE: kMixFwd (4 stages), kMixBwd (stateless backward: recompute + gradient, 7 stages), kMixFwdSave
+// (forward that also leaves Xh, O1 and the activation masks in the workspace: the saved context),
+// kMixBwdCtx (gradient stages only, 4 stages, reads the saved context).
+constexpr int kMixFwd = 0, kMixBwd = 1, kMixFwdSave = 2, kMixBwdCtx = 3;
+template <int MODE, bool EXPORT>
 __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
+  constexpr bool BACKWARD = MODE == kMixBwd || MODE == kMixBwdCtx;   // has the gradient stages
+  constexpr bool RECOMP = MODE == kMixBwd, SAVE = MODE == kMixFwdSave, CTXB = MODE == kMixBwdCtx;
+  constexpr int kStage0 = CTXB ? 3 : 0;                               // stage number of a tile's first phase
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ Mix2Bars bars;
   __shared__ uint32_t tmem_slot;
   __shared__ __align__(16) float sBias[2 * NT];
-  constexpr int NS = BACKWARD ? 7 : 4;
+  constexpr int NS = RECOMP ? 7 : 4;
   uint8_t* sCh = smem;
   uint8_t* sSh = smem + kDft2Bytes;
   uint8_t* sW = smem + 2 * kDft2Bytes;
@@ -659,10 +678,11 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
       }
       mbar_wait(&bars.tfree[buf], par);
     };
-    if (!BACKWARD) {
+    if (!RECOMP) {
+      const __nv_bfloat16* src = CTXB ? p.A1g : p.A1;
       for (int i = 0; i < n; ++i) {
         if (i >= 3) drain(i - 3);
-        load(i % 3, p.A1 + tile_off(i), &bars.xfull[i % 3]);
+        load(i % 3, src + tile_off(i), &bars.xfull[i % 3]);
       }
       for (int k = n > 3 ? n - 3 : 0; k < n; ++k) drain(k);
     } else {
@@ -708,7 +728,8 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
       const int buf = i % 3;
       const uint32_t use = (uint32_t)(i / 3);
       const uint32_t tile = aT + buf * kTileBuf;
-      const bool first = stg == 0, dftg = BACKWARD && stg == 3, last = stg == NS - 1;
+      const int se = stg + kStage0;
+      const bool first = stg == 0, dftg = RECOMP && stg == 3, last = stg == NS - 1;
       if (first) mbar_wait(&bars.xfull[buf], use & 1u);
       if (dftg) mbar_wait(&bars.gfull[buf], use & 1u);
       DBG_ACC(1);
@@ -718,17 +739,17 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
           issue_fwd_dft2(Dre, Dim, aCh, aSh, tile);
         } else if (last) {
           issue_inv_dft2(Dre, Dim, aCh, aSh, tile);
-        } else if (stg == 1) {
+        } else if (se == 1) {
           issue_mlp2<false>(Dre, Dim, SA, w1r, w1i);
-        } else if (stg == 2) {
+        } else if (se == 2) {
           issue_mlp2<false>(Dre, Dim, SA, w2r, w2i);
-        } else if (stg == 4) {
+        } else if (se == 4) {
           issue_mlp2<true>(Dre, Dim, SA, w2r, w2i);    // G1 = G2 W2^H
         } else {
           issue_mlp2<true>(Dre, Dim, SA, w1r, w1i);    // GX = G1 W1^H
         }
         mma_commit(&bars.dfull[stream]);
-        if (BACKWARD && first) mma_commit(&bars.xfree[buf]);
+        if (RECOMP && first) mma_commit(&bars.xfree[buf]);
       }
       __syncwarp();
       TR(t, 2);
@@ -776,6 +797,10 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
         const uint32_t dstA = tmem + lane_sel + kSlot * (uint32_t)((3 * t) % 5) + 24 * cq;
         uint8_t* tile = sT + (i % 3) * kTileBuf;
         const size_t img_off = ((size_t)rem * p.nb + j) * kTileBytes;
+        const int se = stg + kStage0;
+        const size_t mask_idx = (((size_t)rem * p.nb + j) * 12 + (size_t)(cq * 3 + lq)) * 32 + lane;
+        uint4 mk = make_uint4(0, 0, 0, 0);
+        if (CTXB && stg == 0) mk = p.maskbits[mask_idx];   // issued before the wait: its latency hides under the GEMM
         mbar_wait_fast(&bars.dfull[stream], ce[stream] & 1u);
         ++ce[stream];
         TR(t, 4 + warp * 3);
@@ -785,12 +810,19 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
         ld48(src, v);
         DBG_ACC(2);
         bool writes_a = false, early_arrive = false;
-        if (stg == 0) {
+        // backward: operand image (Xh, O1, G2, G1) this stage also writes for tc_wgrad; stored AFTER the
+        // hand-off to the next GEMM, so the global stores run in the shadow of the tensor core
+        uint8_t* gimg = nullptr;
+        if (CTXB && stg == 0) {
+          m1[stream][0] = mk.x; m1[stream][1] = mk.y;
+          m2[stream][0] = mk.z; m2[stream][1] = mk.w;
+        }
+        if (se == 0) {
           // ---- spectrum Xh ----
           pack48(v, pk);
           writes_a = true;
-          if (BACKWARD) store_chunks6((uint8_t*)p.Xh + img_off, chunk0, r, pk);
-        } else if (stg == 1) {
+          if (RECOMP || SAVE) gimg = (uint8_t*)p.Xh + img_off;
+        } else if (se == 1) {
           // ---- O1 = relu(P1 + b1) ----
 #pragma unroll
           for (int q = 0; q < 12; ++q) {
@@ -798,49 +830,40 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
             pk[2 * q] = pack_relu_bf16(__uint_as_float(v[4 * q]) + bq.x, __uint_as_float(v[4 * q + 1]) + bq.y);
             pk[2 * q + 1] = pack_relu_bf16(__uint_as_float(v[4 * q + 2]) + bq.z, __uint_as_float(v[4 * q + 3]) + bq.w);
           }
-          if (BACKWARD) {
+          if (RECOMP || SAVE) {
             m1[stream][0] = m1[stream][1] = 0;
             MaskLoop<0>::run([&](auto P) { mask_collect<decltype(P)::value>(m1[stream], pk[decltype(P)::value]); });
+            gimg = (uint8_t*)p.O1 + img_off;
           }
           writes_a = true;
-          if (BACKWARD) store_chunks6((uint8_t*)p.O1 + img_off, chunk0, r, pk);
-        } else if (stg == 2) {
+        } else if (se == 2) {
           // ---- P2 + b2: forward Z = softshrink (truncated) -> B operand of the inverse transform;
           //      backward: only the mask ----
+          // Z = softshrink(P2 + b2), zero on truncated rows (shrink_sum)
           const float lam = p.lambda;
+          const uint32_t lam2 = pack_bf16(lam, lam), nlam2 = lam2 ^ 0x80008000u;
+#pragma unroll
+          for (int q = 0; q < 12; ++q) {
+            const float4 bq = *(const float4*)(bias2 + 4 * q);
+            pk[2 * q] = shrink_sum(__uint_as_float(v[4 * q]), __uint_as_float(v[4 * q + 1]), bq.x, bq.y, lam2, nlam2);
+            pk[2 * q + 1] = shrink_sum(__uint_as_float(v[4 * q + 2]), __uint_as_float(v[4 * q + 3]), bq.z, bq.w, lam2, nlam2);
+          }
+          if (!row_kept) {
+#pragma unroll
+            for (int q = 0; q < 24; ++q) pk[q] = 0u;
+          }
+          if (RECOMP || SAVE) {
+            // softshrink mask: Z != 0
+            m2[stream][0] = m2[stream][1] = 0;
+            MaskLoop<0>::run([&](auto P) { mask_collect_signed<decltype(P)::value>(m2[stream], pk[decltype(P)::value]); });
+          }
           if (!BACKWARD) {
-            // Z = S_lambda(P2 + b2): the sum is rounded to bf16 once, then a - clamp(a, -lambda, lambda)
-            // on packed pairs (exact zeros inside the threshold; lambda at bf16 precision)
-            const uint32_t lam2 = pack_bf16(lam, lam), nlam2 = lam2 ^ 0x80008000u;
-#pragma unroll
-            for (int q = 0; q < 12; ++q) {
-              const float4 bq = *(const float4*)(bias2 + 4 * q);
-              pk[2 * q] = shrink_bf16x2(pack_bf16(__uint_as_float(v[4 * q]) + bq.x, __uint_as_float(v[4 * q + 1]) + bq.y),
-                                        lam2, nlam2);
-              pk[2 * q + 1] = shrink_bf16x2(
-                  pack_bf16(__uint_as_float(v[4 * q + 2]) + bq.z, __uint_as_float(v[4 * q + 3]) + bq.w), lam2, nlam2);
-            }
-            if (!row_kept) {
-#pragma unroll
-              for (int q = 0; q < 24; ++q) pk[q] = 0u;
-            }
+            // forward: Z is the B operand of the inverse transform
             store_chunks6(tile, chunk0, r, pk);
             fence_async_smem();
-          } else {
-#pragma unroll
-            for (int q = 0; q < 12; ++q) {
-              const float4 bq = *(const float4*)(bias2 + 4 * q);
-              // |P2 + b2| - lambda > 0  <=>  the rounded, relu-ed difference is non-zero
-              pk[2 * q] = pack_relu_bf16(fabsf(__uint_as_float(v[4 * q]) + bq.x) - lam,
-                                         fabsf(__uint_as_float(v[4 * q + 1]) + bq.y) - lam);
-              pk[2 * q + 1] = pack_relu_bf16(fabsf(__uint_as_float(v[4 * q + 2]) + bq.z) - lam,
-                                             fabsf(__uint_as_float(v[4 * q + 3]) + bq.w) - lam);
-            }
-            m2[stream][0] = m2[stream][1] = 0;
-            if (row_kept)
-              MaskLoop<0>::run([&](auto P) { mask_collect<decltype(P)::value>(m2[stream], pk[decltype(P)::value]); });
+            if (SAVE) p.maskbits[mask_idx] = make_uint4(m1[stream][0], m1[stream][1], m2[stream][0], m2[stream][1]);
           }
-        } else if (!BACKWARD || stg == 6) {
+        } else if (se == (BACKWARD ? 6 : 3)) {
           // ---- last stage: rows of A2.  The accumulator is in registers: release the tensor-memory
           //      slots now, so the next tile's first GEMM never waits for the global stores ----
           tc_fence_before();
@@ -858,16 +881,16 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
           fence_async_smem();
           __syncwarp();
           if (lane == 0) mbar_arrive(&bars.sdone[i % 3]);
-        } else if (stg == 3 || stg == 4) {
+        } else if (se == 3 || se == 4) {
           // ---- G2 = G (.) mask2 ; G1 = mask1 (.) (G2 W2^H) ----
           pack48(v, pk);
-          if (stg == 3) {
+          if (se == 3) {
             MaskLoop<0>::run([&](auto P) { pk[decltype(P)::value] = mask_apply<decltype(P)::value>(m2[stream], pk[decltype(P)::value]); });
           } else {
             MaskLoop<0>::run([&](auto P) { pk[decltype(P)::value] = mask_apply<decltype(P)::value>(m1[stream], pk[decltype(P)::value]); });
           }
           writes_a = true;
-          store_chunks6((uint8_t*)(stg == 3 ? p.G2 : p.G1) + img_off, chunk0, r, pk);
+          gimg = (uint8_t*)(se == 3 ? p.G2 : p.G1) + img_off;
         } else {
           // ---- stage 5: GX -> B operand of the inverse transform (the tile's own buffer) ----
 #pragma unroll
@@ -888,7 +911,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
           }
         }
 #ifdef AFNO_TIMING
-        { long long n_ = clock64(); dbg_m[stg] += n_ - dbg_t; dbg_t = n_; }
+        { long long n_ = clock64(); dbg_m[se] += n_ - dbg_t; dbg_t = n_; }
 #endif
         TR(t, 5 + warp * 3);
         if (writes_a) {
@@ -905,6 +928,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
           __syncwarp();
           if (lane == 0) mbar_arrive(&bars.edone[stream]);
         }
+        if (gimg != nullptr) store_chunks6(gimg, chunk0, r, pk);
         TR(t, 6 + warp * 3);
         DBG_ACC(1);
       }
@@ -1135,6 +1159,7 @@ struct TcWs {
   float* bprep;
   __nv_bfloat16 *A1g, *Xh, *O1, *G2, *G1; // backward only
   float* part;
+  uint4* maskbits;   // saved context: bit-packed activation masks, 6 KB per (b, kw, block) tile
   uint8_t *mask1, *mask2;
   size_t mask_region;
   int S;
@@ -1166,6 +1191,7 @@ TcWs tc_carve(const Geometry& g, bool backward, char* base) {
     w.O1 = (__nv_bfloat16*)take(img);
     w.G2 = (__nv_bfloat16*)take(img);
     w.G1 = (__nv_bfloat16*)take(img);
+    w.maskbits = (uint4*)take((size_t)g.B * g.Kw * g.nb * 12 * 32 * sizeof(uint4));
     int S = 148 / (2 * g.nb);   // CTAs per (layer, block) of tc_wgrad
     if (S < 1) S = 1;
     if (S > g.B * g.Kw) S = g.B * g.Kw;
@@ -1226,9 +1252,12 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
     e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &out->encode_tiled, cudaEnableDefault, &q);
     if (e == cudaSuccess && (q != cudaDriverEntryPointSuccess || out->encode_tiled == nullptr)) e = cudaErrorNotSupported;
   }
-  if (e == cudaSuccess) e = set_smem(tc_mix2<false, false>, kMix2Smem);
-  if (e == cudaSuccess) e = set_smem(tc_mix2<true, false>, kMix2Smem);
-  if (e == cudaSuccess) e = set_smem(tc_mix2<true, true>, kMix2Smem);
+  if (e == cudaSuccess) e = set_smem(tc_mix2<kMixFwd, false>, kMix2Smem);
+  if (e == cudaSuccess) e = set_smem(tc_mix2<kMixFwdSave, false>, kMix2Smem);
+  if (e == cudaSuccess) e = set_smem(tc_mix2<kMixBwd, false>, kMix2Smem);
+  if (e == cudaSuccess) e = set_smem(tc_mix2<kMixBwd, true>, kMix2Smem);
+  if (e == cudaSuccess) e = set_smem(tc_mix2<kMixBwdCtx, false>, kMix2Smem);
+  if (e == cudaSuccess) e = set_smem(tc_mix2<kMixBwdCtx, true>, kMix2Smem);
   if (e == cudaSuccess) e = set_smem(tc_wgrad, kWgSmem);
   int dev = 0, sms = 148;
   if (e == cudaSuccess) e = cudaGetDevice(&dev);
@@ -1295,7 +1324,13 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
   prof_begin("tc_mix_fwd", st);
   const int S2 = mix2_split(g, tp);
-  tc_mix2<false, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2);
+  if (g.save_ctx) {
+    // saved context: Xh, O1 (operands of tc_wgrad) and the activation masks stay in the workspace
+    mp.Xh = w.Xh; mp.O1 = w.O1; mp.maskbits = w.maskbits;
+    tc_mix2<kMixFwdSave, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2);
+  } else {
+    tc_mix2<kMixFwd, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2);
+  }
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -1336,10 +1371,18 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   mp.mask2 = g.export_masks ? w.mask2 : nullptr;
   mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
   const int S2 = mix2_split(g, tp);
-  if (g.export_masks) {
-    TC_LAUNCH("tc_mix_bwd", tc_mix2<true, true><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
+  mp.maskbits = w.maskbits;
+  if (g.use_ctx) {
+    // gradient stages only: Xh, O1 and the masks were left in the workspace by the forward call
+    if (g.export_masks) {
+      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, true><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
+    } else {
+      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
+    }
+  } else if (g.export_masks) {
+    TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, true><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
   } else {
-    TC_LAUNCH("tc_mix_bwd", tc_mix2<true, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
+    TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
   }
   // B4 / B6: parameter gradients
   const int nred = nW + g.nb * BS;

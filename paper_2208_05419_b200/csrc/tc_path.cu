@@ -46,9 +46,6 @@ constexpr uint32_t kWBytes = BS * BS * 2;            // 18432
 // writes of consecutive chunks of one row (the coalesced global order) bank-conflict-free
 constexpr uint32_t kTileLbo = 128, kTileSbo = 1536 + 16;
 constexpr uint32_t kTileBytes = (NT / 8) * kTileSbo; // 37248
-constexpr uint32_t kFwLbo = 2048, kFwSbo = 128;     // Gw rows 0..127: K-major A [128 x 192], order [k/8][m/8]
-constexpr uint32_t kFwHalf = 128 * WP * 2;           // 49152
-
 // ---- weight preparation: fp32 [nb][96][96][2] -> bf16 K-major interleaved operands --------------
 // per block 4 matrices of kWBytes {W1r, W1i, W2r, W2i} with element (n=o, k=i) = W[i][o] (the
 // backward pass reads the same images as MN-major operands), and the biases regrouped as
@@ -98,40 +95,60 @@ __device__ long long g_afno_dbg[128];
 #define DBG_ACC(slot)
 #endif
 
-// ---- F1 / B2 and F8 + F9 / B8, second generation: all global traffic through bulk tensor copies -------
+// ---- F1 / B2 and F8 + F9 / B8: the W-direction transforms, all global traffic through bulk tensor copies --
 // One tile = (b, h, channel block j): N = 96 channels.  The activation tile arrives as three
 // 64B-swizzled panels [192 rows (w, zero-filled past W)][32 channels] written by TMA, leaves as rows
 // staged in shared memory and sent by one TMA store: no LSU instruction touches global memory, so
 // the kernels run at the speed of the copy engines instead of the load/store pipe.
 //   forward : D_ri[kw, c] = sum_w Fw_ri[kw, w] x[b,h,w,c]      -> A1 rows [kw][re 96 | im 96 | pad 8]
 //   inverse : D_a[w, c]   = sum_(ri,kw) Gw[w, (ri,kw)] A2[..]  -> y[b,h,w,c] = residual + D
+// Under load a bulk copy takes ~5 us to land, so bandwidth is bought with bytes in flight: the
+// constant DFT matrix (A operand, 2 x [128 x 192] bf16) lives in TENSOR memory (192 columns), which
+// leaves all of shared memory to the ring of tiles (6 slots forward, 3 + 3 inverse).  The two
+// accumulator halves occupy 192 more columns; a half is handed back as soon as it is in registers.
 // 8 warps: warps with (warp % 4) < rows/32 drain the accumulators (TMEM lane quarter = warp % 4),
-// one spare warp issues the TMA loads, one the UMMAs.  Shared memory is a ring of slots; a slot
-// holds a tile's operand and later (forward) its staged output rows.
+// one spare warp issues the TMA loads, one the UMMAs.
 constexpr int kW2Threads = 256;
 constexpr uint32_t kPanel = 192 * 64;                      // 12288: one [192 x 32] bf16 panel
 constexpr uint32_t kW2Tile = 3 * kPanel;                   // 36864: a [192 x 96] tile
-constexpr uint32_t kF2Lbo = 12 * 128, kF2Sbo = 128;        // Fw halves: K-major A, 96 rows stored, order [k/8][m/8 < 12]
-constexpr uint32_t kF2Half = (WP / 8) * kF2Lbo;            // 36864 (rows 96..127 alias the next k-chunk: finite, unused)
-constexpr uint32_t kF2Bytes = 2 * kF2Half;                 // 73728
-constexpr int kWfSlots = 4;
-constexpr uint32_t kWfSmem = kF2Bytes + kWfSlots * kW2Tile + 1024;   // 222208
-constexpr uint32_t kG2Lbo1 = 7 * 128;                      // Gw second half: rows 128..183 stored (7 groups of 8)
-constexpr uint32_t kG2Half1 = (WP / 8) * kG2Lbo1;          // 21504
-constexpr uint32_t kG2Bytes = kFwHalf + kG2Half1;          // 70656
-constexpr uint32_t kWiSmem = kG2Bytes + 4 * kW2Tile + 1024;          // 219136
+constexpr uint32_t kCImgWords = 2 * 128 * (WP / 2);        // constant image: [half][row 0..127][96 words = K pairs]
+constexpr uint32_t kCCols = WP;                            // TMEM columns of the constant: half a at a * 96
+constexpr int kWfSlots = 6;
+constexpr uint32_t kWfSmem = kWfSlots * kW2Tile + 1024;    // 222208
+constexpr int kWiSlots = 3;
+constexpr uint32_t kWiSmem = 2 * kWiSlots * kW2Tile + 1024;
+
+// constant matrix image (global, [half][128 rows][96 words]) -> tensor memory columns [0, 192); warps 0..3
+// load half 0, warps 4..7 half 1 (lane quarter = warp % 4); all of a thread's loads are in flight at once
+__device__ __forceinline__ void load_const_tmem(uint32_t tmem, const uint32_t* __restrict__ img, int warp, int lane) {
+  const int a = warp >> 2, q4 = warp & 3;
+  const uint4* src = (const uint4*)(img + ((size_t)a * 128 + q4 * 32 + lane) * (WP / 2));
+  const uint32_t dst = tmem + ((uint32_t)(q4 * 32) << 16) + a * (WP / 2);
+  uint4 t[24];
+#pragma unroll
+  for (int q = 0; q < 24; ++q) t[q] = __ldg(src + q);
+#pragma unroll
+  for (int c = 0; c < 6; ++c) {
+    uint32_t v[16];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      v[4 * q] = t[4 * c + q].x; v[4 * q + 1] = t[4 * c + q].y; v[4 * q + 2] = t[4 * c + q].z; v[4 * q + 3] = t[4 * c + q].w;
+    }
+    tmem_st16(dst + 16 * c, v);
+  }
+  tmem_wait_st();
+}
 
 __global__ void __launch_bounds__(kW2Threads, 1)
 tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapA1,
-             const uint8_t* __restrict__ Fimg, int ntiles, int nb, int H, int Kw) {
+             const uint32_t* __restrict__ Fimg, int ntiles, int nb, int H, int Kw) {
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t full[kWfSlots], sfree[kWfSlots], accfull[2], accempty[2];
   __shared__ uint32_t tmem_slot;
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (base - smem_u32(smem_raw));
-  const uint32_t aF = base, aS = base + kF2Bytes;
+  const uint32_t aS = base;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (uint32_t i = tid; i < kF2Bytes / 16; i += kW2Threads) cp_async16(aF + i * 16, Fimg + (size_t)i * 16);
   if (tid == 0) {
     for (int q = 0; q < kWfSlots; ++q) {
       mbar_init(&full[q], 1);
@@ -139,87 +156,99 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
     }
     for (int q = 0; q < 2; ++q) {
       mbar_init(&accfull[q], 1);
-      mbar_init(&accempty[q], 6);
+      mbar_init(&accempty[q], 3);
     }
     mbar_init_fence();
     tma_prefetch_desc(&mapX);
     tma_prefetch_desc(&mapA1);
   }
   if (warp == 0) tmem_alloc<512>(&tmem_slot);
-  cp_async_wait_all();
-  fence_async_smem();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
-  if (warp == 3) {
-    // ===== TMA producer: tile it -> slot it % 4, up to 3 tiles ahead of the epilogue ===============
-    if (elect_one()) {
-      for (int it = 0; it < nmine; ++it) {
-        const int s = it % kWfSlots;
-        if (it >= kWfSlots) mbar_wait(&sfree[s], (uint32_t)((it / kWfSlots - 1) & 1));
-        const int t = blockIdx.x + it * gridDim.x;
-        const int j = t % nb, bh = t / nb;
-        mbar_expect_tx(&full[s], kW2Tile);
+  // TMA producer (warp 7): tile it -> slot it % 6
+  auto produce = [&](int it) {
+    const int s = it % kWfSlots;
+    if (it >= kWfSlots) mbar_wait(&sfree[s], (uint32_t)((it / kWfSlots - 1) & 1));
+    const int t = blockIdx.x + it * gridDim.x;
+    const int j = t % nb, bh = t / nb;
+    mbar_expect_tx(&full[s], kW2Tile);
 #pragma unroll
-        for (int pn = 0; pn < 3; ++pn) tma_load3(aS + s * kW2Tile + pn * kPanel, &mapX, j * BS + pn * 32, 0, bh, &full[s]);
-      }
-    }
+    for (int pn = 0; pn < 3; ++pn) tma_load3(aS + s * kW2Tile + pn * kPanel, &mapX, j * BS + pn * 32, 0, bh, &full[s]);
+  };
+  if (warp == 7) {
+    // the first ring of loads starts at once, under the load of the constant
+    if (elect_one())
+      for (int it = 0; it < kWfSlots && it < nmine; ++it) produce(it);
     __syncwarp();
-  } else if (warp == 7) {
-    // ===== MMA issuer: accumulator pair it & 1 = (re 96 | im 96) columns =============================
+  }
+  load_const_tmem(tmem, Fimg, warp, lane);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+
+  if (warp == 7) {
+    if (elect_one())
+      for (int it = kWfSlots; it < nmine; ++it) produce(it);
+    __syncwarp();
+  } else if (warp == 3) {
+    // ===== MMA issuer: half a = (re | im) rows of the transform, accumulator columns 192 + 96 a =======
     const uint32_t idesc = idesc_bf16(128, BS, kIdescBMn);
     for (int it = 0; it < nmine; ++it) {
-      const int s = it % kWfSlots, pa = it & 1;
+      const int s = it % kWfSlots;
       mbar_wait(&full[s], (uint32_t)((it / kWfSlots) & 1));
-      if (it >= 2) mbar_wait(&accempty[pa], (uint32_t)((it / 2 - 1) & 1));
-      tc_fence_after();
-      if (elect_one()) {
-        const uint32_t bt = aS + s * kW2Tile;
+      const uint32_t bt = aS + s * kW2Tile;
 #pragma unroll
-        for (int a = 0; a < 2; ++a) {
-          const uint32_t d = tmem + pa * 256 + a * BS;
+      for (int a = 0; a < 2; ++a) {
+        if (it >= 1) mbar_wait(&accempty[a], (uint32_t)((it - 1) & 1));
+        tc_fence_after();
+        if (elect_one()) {
 #pragma unroll
           for (int ks = 0; ks < WP / 16; ++ks)
-            mma_ss(d, smem_desc(aF + a * kF2Half + ks * 2 * kF2Lbo, kF2Lbo, kF2Sbo),
-                   smem_desc_sw64(bt + ks * 1024, kPanel, 512), idesc, ks > 0);
+            mma_ts(tmem + kCCols + a * BS, tmem + a * (WP / 2) + ks * 8, smem_desc_sw64(bt + ks * 1024, kPanel, 512), idesc,
+                   ks > 0);
+          mma_commit(&accfull[a]);
         }
-        mma_commit(&accfull[pa]);
+        __syncwarp();
       }
-      __syncwarp();
     }
   } else {
     // ===== epilogue warps 0,1,2 (re) and 4,5,6 (im): row kw = 32 * (warp % 4) + lane ==================
     const int a = warp >> 2, q4 = warp & 3;
     const int kw = q4 * 32 + lane;
     const uint32_t lane_base = (uint32_t)(q4 * 32) << 16;
+    const uint32_t acc = tmem + kCCols + a * BS + lane_base;
     for (int it = 0; it < nmine; ++it) {
-      const int s = it % kWfSlots, pa = it & 1;
+      const int s = it % kWfSlots;
       const int t = blockIdx.x + it * gridDim.x;
       const int j = t % nb, bh = t / nb, b = bh / H, h = bh - b * H;
-      mbar_wait(&accfull[pa], (uint32_t)((it >> 1) & 1));
+      mbar_wait(&accfull[a], (uint32_t)(it & 1));
       tc_fence_after();
-      const uint32_t acc = tmem + pa * 256 + a * BS + lane_base;
-      // the tile's own operand slot is free (its MMAs have completed): stage the output rows there
-      uint8_t* row = smem + kF2Bytes + s * kW2Tile + kw * kOutStride + a * (BS * 2);
+      uint32_t v0[32], v1[32], v2[32];
+      tmem_ld32(acc, v0);
+      tmem_ld32(acc + 32, v1);
+      tmem_ld32(acc + 64, v2);
+      tmem_wait_ld();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&accempty[a]);
+      // the tile's own operand slot is free once BOTH halves' MMAs have read it: stage the output rows there
+      if (a == 0) mbar_wait(&accfull[1], (uint32_t)(it & 1));
+      uint8_t* row = smem + s * kW2Tile + kw * kOutStride + a * (BS * 2);
+      if (kw < Kw) {
+        uint32_t pk[16];
+        pack32(v0, pk);
 #pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        uint32_t v[32], pk[16];
-        tmem_ld32(acc + 32 * k, v);
-        tmem_wait_ld();
-        if (k == 2) {
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(&accempty[pa]);
-        }
-        pack32(v, pk);
-        if (kw < Kw) {
+        for (int g = 0; g < 4; ++g) *(uint4*)(row + g * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
+        pack32(v1, pk);
 #pragma unroll
-          for (int g = 0; g < 4; ++g)
-            *(uint4*)(row + k * 64 + g * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
-        }
+        for (int g = 0; g < 4; ++g) *(uint4*)(row + 64 + g * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
+        pack32(v2, pk);
+#pragma unroll
+        for (int g = 0; g < 4; ++g) *(uint4*)(row + 128 + g * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
       }
       fence_async_smem();
       asm volatile("bar.sync 1, 192;" ::: "memory");
@@ -241,118 +270,128 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
-// inverse: operand ring of 2 tiles (A2 rows as K = ri * 96 + kw) and a ring of 2 residual / output tiles
+// inverse: a ring of 3 operand tiles (A2 rows as K = ri * 96 + kw) and a ring of 3 residual / output tiles
 __global__ void __launch_bounds__(kW2Threads, 1)
 tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ CUtensorMap mapRes,
-             const __grid_constant__ CUtensorMap mapY, const uint8_t* __restrict__ Gimg, int ntiles, int nb, int H, int W,
+             const __grid_constant__ CUtensorMap mapY, const uint32_t* __restrict__ Gimg, int ntiles, int nb, int H, int W,
              int has_res) {
   extern __shared__ uint8_t smem_raw[];
-  __shared__ __align__(8) uint64_t ofull[2], rfull[2], rfree[2], accfull[2], accempty[2];
+  __shared__ __align__(8) uint64_t ofull[kWiSlots], ofree[kWiSlots], rfull[kWiSlots], rfree[kWiSlots], accfull[2], accempty[2];
   __shared__ uint32_t tmem_slot;
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (base - smem_u32(smem_raw));
-  const uint32_t aG = base, aO = base + kG2Bytes, aR = aO + 2 * kW2Tile;
-  uint8_t* sR = smem + kG2Bytes + 2 * kW2Tile;
+  const uint32_t aO = base, aR = aO + kWiSlots * kW2Tile;
+  uint8_t* sR = smem + kWiSlots * kW2Tile;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (uint32_t i = tid; i < kG2Bytes / 16; i += kW2Threads) cp_async16(aG + i * 16, Gimg + (size_t)i * 16);
-  if (!has_res)
-    for (uint32_t i = tid; i < 2 * kW2Tile / 16; i += kW2Threads) ((uint4*)sR)[i] = make_uint4(0, 0, 0, 0);
   if (tid == 0) {
-    for (int q = 0; q < 2; ++q) {
+    for (int q = 0; q < kWiSlots; ++q) {
       mbar_init(&ofull[q], 1);
+      mbar_init(&ofree[q], 1);
       mbar_init(&rfull[q], 1);
       mbar_init(&rfree[q], 1);
-      mbar_init(&accfull[q], 1);
-      mbar_init(&accempty[q], 6);
     }
+    mbar_init(&accfull[0], 1);
+    mbar_init(&accfull[1], 1);
+    mbar_init(&accempty[0], 4);
+    mbar_init(&accempty[1], 2);
     mbar_init_fence();
     tma_prefetch_desc(&mapA2);
     tma_prefetch_desc(&mapRes);
     tma_prefetch_desc(&mapY);
   }
   if (warp == 0) tmem_alloc<512>(&tmem_slot);
-  cp_async_wait_all();
-  fence_async_smem();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
-  if (warp == 6) {
-    // ===== TMA producer =============================================================================
-    if (elect_one()) {
-      for (int it = 0; it < nmine; ++it) {
-        const int s = it & 1;
-        const int t = blockIdx.x + it * gridDim.x;
-        const int j = t % nb, bh = t / nb, b = bh / H, h = bh - b * H;
-        // operand slot s: its previous tile's MMAs have completed
-        if (it >= 2) mbar_wait(&accfull[s], (uint32_t)((it / 2 - 1) & 1));
-        mbar_expect_tx(&ofull[s], kW2Tile);
+  // TMA producer (warp 6)
+  auto produce = [&](int it) {
+    const int s = it % kWiSlots;
+    const uint32_t par = (uint32_t)((it / kWiSlots - 1) & 1);
+    const int t = blockIdx.x + it * gridDim.x;
+    const int j = t % nb, bh = t / nb, b = bh / H, h = bh - b * H;
+    if (it >= kWiSlots) mbar_wait(&ofree[s], par);   // the slot's previous MMAs have completed
+    mbar_expect_tx(&ofull[s], kW2Tile);
 #pragma unroll
-        for (int pn = 0; pn < 6; ++pn)   // panel pn = ri * 3 + n -> K rows ri * 96.., N panel n
-          tma_load5(aO + s * kW2Tile + (pn % 3) * kPanel + (pn / 3) * (BS * 64), &mapA2, 0, pn, j * H + h, 0, b, &ofull[s]);
-        if (has_res) {
-          if (it >= 2) mbar_wait(&rfree[s], (uint32_t)((it / 2 - 1) & 1));
-          mbar_expect_tx(&rfull[s], kW2Tile);
+    for (int pn = 0; pn < 6; ++pn)   // panel pn = ri * 3 + n -> K rows ri * 96.., N panel n
+      tma_load5(aO + s * kW2Tile + (pn % 3) * kPanel + (pn / 3) * (BS * 64), &mapA2, 0, pn, j * H + h, 0, b, &ofull[s]);
+    if (has_res) {
+      if (it >= kWiSlots) mbar_wait(&rfree[s], par);  // the slot's previous store has read it
+      mbar_expect_tx(&rfull[s], kW2Tile);
 #pragma unroll
-          for (int pn = 0; pn < 3; ++pn) tma_load3(aR + s * kW2Tile + pn * kPanel, &mapRes, j * BS + pn * 32, 0, bh, &rfull[s]);
-        }
-      }
+      for (int pn = 0; pn < 3; ++pn) tma_load3(aR + s * kW2Tile + pn * kPanel, &mapRes, j * BS + pn * 32, 0, bh, &rfull[s]);
     }
+  };
+  if (warp == 6) {
+    // the first ring of loads starts at once, under the load of the constant
+    if (elect_one())
+      for (int it = 0; it < kWiSlots && it < nmine; ++it) produce(it);
+    __syncwarp();
+  }
+  load_const_tmem(tmem, Gimg, warp, lane);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+
+  if (warp == 6) {
+    if (elect_one())
+      for (int it = kWiSlots; it < nmine; ++it) produce(it);
     __syncwarp();
   } else if (warp == 7) {
-    // ===== MMA issuer: accumulators a = w / 128 at columns a * 96 of pair it & 1 ======================
+    // ===== MMA issuer: half a = rows w = 128 a .. of the transform, accumulator columns 192 + 96 a =====
     const uint32_t idesc = idesc_bf16(128, BS, kIdescBMn);
     for (int it = 0; it < nmine; ++it) {
-      const int s = it & 1;
-      mbar_wait(&ofull[s], (uint32_t)((it >> 1) & 1));
-      if (it >= 2) mbar_wait(&accempty[s], (uint32_t)((it / 2 - 1) & 1));
-      tc_fence_after();
-      if (elect_one()) {
-        const uint32_t bt = aO + s * kW2Tile;
+      const int s = it % kWiSlots;
+      mbar_wait(&ofull[s], (uint32_t)((it / kWiSlots) & 1));
+      const uint32_t bt = aO + s * kW2Tile;
 #pragma unroll
-        for (int ks = 0; ks < WP / 16; ++ks)
-          mma_ss(tmem + s * 256, smem_desc(aG + ks * 2 * kFwLbo, kFwLbo, kFwSbo), smem_desc_sw64(bt + ks * 1024, kPanel, 512),
-                 idesc, ks > 0);
+      for (int a = 0; a < 2; ++a) {
+        if (it >= 1) mbar_wait(&accempty[a], (uint32_t)((it - 1) & 1));
+        tc_fence_after();
+        if (elect_one()) {
 #pragma unroll
-        for (int ks = 0; ks < WP / 16; ++ks)
-          mma_ss(tmem + s * 256 + BS, smem_desc(aG + kFwHalf + ks * 2 * kG2Lbo1, kG2Lbo1, kFwSbo),
-                 smem_desc_sw64(bt + ks * 1024, kPanel, 512), idesc, ks > 0);
-        mma_commit(&accfull[s]);
+          for (int ks = 0; ks < WP / 16; ++ks)
+            mma_ts(tmem + kCCols + a * BS, tmem + a * (WP / 2) + ks * 8, smem_desc_sw64(bt + ks * 1024, kPanel, 512), idesc,
+                   ks > 0);
+          mma_commit(&accfull[a]);
+          if (a == 1) mma_commit(&ofree[s]);
+        }
+        __syncwarp();
       }
-      __syncwarp();
     }
   } else {
     // ===== epilogue warps 0..3 (w < 128) and 4, 5 (w = 128..191): row w = 128 a + 32 (warp % 4) + lane ==
     const int a = warp >> 2, q4 = warp & 3;
     const int w = a * 128 + q4 * 32 + lane;
     const uint32_t lane_base = (uint32_t)(q4 * 32) << 16;
+    const uint32_t acc = tmem + kCCols + a * BS + lane_base;
     for (int it = 0; it < nmine; ++it) {
-      const int s = it & 1;
+      const int s = it % kWiSlots;
+      const uint32_t par = (uint32_t)((it / kWiSlots) & 1);
       const int t = blockIdx.x + it * gridDim.x;
       const int j = t % nb, bh = t / nb;
       uint8_t* rt = sR + s * kW2Tile;
-      if (has_res) {
-        mbar_wait(&rfull[s], (uint32_t)((it >> 1) & 1));
-      } else if (it >= 2) {
-        // no residual load to wait for: the slot's previous store must have read it
-        mbar_wait(&rfree[s], (uint32_t)((it / 2 - 1) & 1));
-      }
-      mbar_wait(&accfull[s], (uint32_t)((it >> 1) & 1));
+      mbar_wait(&accfull[a], (uint32_t)(it & 1));
       tc_fence_after();
-      const uint32_t acc = tmem + s * 256 + a * BS + lane_base;
+      uint32_t v[3][32];
+      tmem_ld32(acc, v[0]);
+      tmem_ld32(acc + 32, v[1]);
+      tmem_ld32(acc + 64, v[2]);
+      tmem_wait_ld();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&accempty[a]);
+      if (has_res) {
+        mbar_wait(&rfull[s], par);
+      } else if (it >= kWiSlots) {
+        // no residual load to wait for: the slot's previous store must have read it
+        mbar_wait(&rfree[s], par ^ 1u);
+      }
+      if (w < W) {
 #pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        uint32_t v[32];
-        tmem_ld32(acc + 32 * k, v);
-        tmem_wait_ld();
-        if (k == 2) {
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(&accempty[s]);
-        }
-        if (w < W) {
+        for (int k = 0; k < 3; ++k) {
           uint8_t* pan = rt + k * kPanel;
 #pragma unroll
           for (int g = 0; g < 4; ++g) {
@@ -361,14 +400,14 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
             if (has_res) r = *ptr;
             // bf16 -> fp32 is a 16-bit shift; one rounding of (residual + branch)
             uint4 o;
-            o.x = pack_bf16(__uint_as_float(v[8 * g + 0]) + __uint_as_float(r.x << 16),
-                            __uint_as_float(v[8 * g + 1]) + __uint_as_float(r.x & 0xFFFF0000u));
-            o.y = pack_bf16(__uint_as_float(v[8 * g + 2]) + __uint_as_float(r.y << 16),
-                            __uint_as_float(v[8 * g + 3]) + __uint_as_float(r.y & 0xFFFF0000u));
-            o.z = pack_bf16(__uint_as_float(v[8 * g + 4]) + __uint_as_float(r.z << 16),
-                            __uint_as_float(v[8 * g + 5]) + __uint_as_float(r.z & 0xFFFF0000u));
-            o.w = pack_bf16(__uint_as_float(v[8 * g + 6]) + __uint_as_float(r.w << 16),
-                            __uint_as_float(v[8 * g + 7]) + __uint_as_float(r.w & 0xFFFF0000u));
+            o.x = pack_bf16(__uint_as_float(v[k][8 * g + 0]) + __uint_as_float(r.x << 16),
+                            __uint_as_float(v[k][8 * g + 1]) + __uint_as_float(r.x & 0xFFFF0000u));
+            o.y = pack_bf16(__uint_as_float(v[k][8 * g + 2]) + __uint_as_float(r.y << 16),
+                            __uint_as_float(v[k][8 * g + 3]) + __uint_as_float(r.y & 0xFFFF0000u));
+            o.z = pack_bf16(__uint_as_float(v[k][8 * g + 4]) + __uint_as_float(r.z << 16),
+                            __uint_as_float(v[k][8 * g + 5]) + __uint_as_float(r.z & 0xFFFF0000u));
+            o.w = pack_bf16(__uint_as_float(v[k][8 * g + 6]) + __uint_as_float(r.w << 16),
+                            __uint_as_float(v[k][8 * g + 7]) + __uint_as_float(r.w & 0xFFFF0000u));
             *ptr = o;
           }
         }
@@ -381,7 +420,7 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
         bulk_commit();
         if (it > 0) {
           bulk_wait_read<1>();
-          mbar_arrive(&rfree[(it - 1) & 1]);
+          mbar_arrive(&rfree[(it - 1) % kWiSlots]);
         }
       }
       __syncwarp();
@@ -1220,20 +1259,19 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
       dft2[off] = host_bf16(cos(a) * s);
       dft2[kDft2Bytes / 2 + off] = host_bf16(sin(a) * s);
     }
-  // W-direction constants as K-major A operands (element (m, k) at (k/8)*LBO + (m/8)*128 + (m%8)*16 + (k%8)*2):
-  //   Fw half ri (96 rows stored, LBO kF2Lbo): (m = kw, k = w) = {cos, -sin}(2 pi kw w / W) / sqrt(W)  [x alpha_kw]
-  //   Gw half 0 (128 rows, LBO kFwLbo), half 1 (56 rows, LBO kG2Lbo1):
-  //      (m = w - 128 a, k = ri*96 + kw) = alpha_kw {cos, -sin}(...) / sqrt(W)                       [or alpha = 1]
-  std::vector<uint16_t> fw(kF2Bytes / 2, 0), fwa(kF2Bytes / 2, 0), gw(kG2Bytes / 2, 0), gw1(kG2Bytes / 2, 0);
-  auto aoff = [](int m, int k, uint32_t lbo) { return ((k / 8) * lbo + (m / 8) * 128 + (m % 8) * 16 + (k % 8) * 2) / 2; };
+  // W-direction constants as tensor-memory A operands: [half a][row m < 128][96 words], word q of a row =
+  // (k = 2q low half, k = 2q + 1 high half):
+  //   Fw half ri: (m = kw, k = w)                  = {cos, -sin}(2 pi kw w / W) / sqrt(W)          [x alpha_kw]
+  //   Gw half a : (m = w - 128 a, k = ri * 96 + kw) = alpha_kw {cos, -sin}(...) / sqrt(W)          [or alpha = 1]
+  std::vector<uint16_t> fw(2 * kCImgWords, 0), fwa(2 * kCImgWords, 0), gw(2 * kCImgWords, 0), gw1(2 * kCImgWords, 0);
+  auto aoff = [](int a, int m, int k) { return ((size_t)a * 128 + m) * WP + k; };
   for (int kw = 0; kw < Wh; ++kw)
     for (int w = 0; w < W; ++w) {
       const double a = two_pi * (double)((long)kw * w % W) / (double)W, s = 1.0 / sqrt((double)W);
       const double alpha = (kw == 0 || 2 * kw == W) ? 1.0 : 2.0;
       for (int ri = 0; ri < 2; ++ri) {
         const double v = (ri == 0 ? cos(a) : -sin(a)) * s;
-        const uint32_t of = ri * (kF2Half / 2) + aoff(kw, w, kF2Lbo);
-        const uint32_t og = w < 128 ? aoff(w, ri * BS + kw, kFwLbo) : kFwHalf / 2 + aoff(w - 128, ri * BS + kw, kG2Lbo1);
+        const size_t of = aoff(ri, kw, w), og = aoff(w / 128, w % 128, ri * BS + kw);
         fw[of] = host_bf16(v);
         fwa[of] = host_bf16(v * alpha);
         gw[og] = host_bf16(v * alpha);
@@ -1287,7 +1325,7 @@ static cudaError_t launch_wdft_fwd(const Geometry& g, const TcPlan& tp, const vo
   const int ntiles = g.B * g.H * g.nb;
   const int grid = ntiles < tp.num_sms ? ntiles : tp.num_sms;
   prof_begin("tc_wdft_fwd", st);
-  tc_wdft_fwd2<<<grid, kW2Threads, kWfSmem, st>>>(mx, ma, fimg, ntiles, g.nb, g.H, g.Kw);
+  tc_wdft_fwd2<<<grid, kW2Threads, kWfSmem, st>>>(mx, ma, (const uint32_t*)fimg, ntiles, g.nb, g.H, g.Kw);
   prof_end(st);
   count_launch();
   return cudaGetLastError();
@@ -1300,7 +1338,7 @@ static cudaError_t launch_wdft_inv(const Geometry& g, const TcPlan& tp, const vo
   const int ntiles = g.B * g.H * g.nb;
   const int grid = ntiles < tp.num_sms ? ntiles : tp.num_sms;
   prof_begin("tc_wdft_inv", st);
-  tc_wdft_inv2<<<grid, kW2Threads, kWiSmem, st>>>(ma, mr, my, gimg, ntiles, g.nb, g.H, g.W, res ? 1 : 0);
+  tc_wdft_inv2<<<grid, kW2Threads, kWiSmem, st>>>(ma, mr, my, (const uint32_t*)gimg, ntiles, g.nb, g.H, g.W, res ? 1 : 0);
   prof_end(st);
   count_launch();
   return cudaGetLastError();

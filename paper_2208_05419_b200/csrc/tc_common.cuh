@@ -224,6 +224,14 @@ __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* m) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(m) : "memory");
 }
 
+// ---- programmatic dependent launch ------------------------------------------------------------------
+// pdl_launch_dependents: the next kernel of the stream may start its prologue while this grid still runs;
+// pdl_wait: blocks until every prerequisite grid has completed and its memory is visible.  Every kernel
+// of the chain executes pdl_wait before it touches global data another kernel of the chain writes or
+// reads, so completion is transitive along the chain.  Both are no-ops in a plain launch.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   __nv_bfloat162 t = __floats2bfloat162_rn(lo, hi);
   return *reinterpret_cast<uint32_t*>(&t);

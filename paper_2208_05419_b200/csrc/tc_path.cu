@@ -53,6 +53,8 @@ constexpr uint32_t kTileBytes = (NT / 8) * kTileSbo; // 37248
 __global__ void k_tc_prep_weights(const float* __restrict__ w1, const float* __restrict__ b1,
                                   const float* __restrict__ w2, const float* __restrict__ b2,
                                   __nv_bfloat16* __restrict__ out, float* __restrict__ bout, int nb) {
+  pdl_launch_dependents();
+  pdl_wait();
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx < nb * BS) {
     const int o = idx % BS, j = idx / BS;
@@ -163,10 +165,13 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
     tma_prefetch_desc(&mapA1);
   }
   if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  pdl_launch_dependents();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
+  load_const_tmem(tmem, Fimg, warp, lane);   // plan constant: loads under the previous kernel's tail
+  pdl_wait();
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
   // TMA producer (warp 7): tile it -> slot it % 6
@@ -185,7 +190,6 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
       for (int it = 0; it < kWfSlots && it < nmine; ++it) produce(it);
     __syncwarp();
   }
-  load_const_tmem(tmem, Fimg, warp, lane);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -300,10 +304,13 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
     tma_prefetch_desc(&mapY);
   }
   if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  pdl_launch_dependents();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
+  load_const_tmem(tmem, Gimg, warp, lane);   // plan constant: loads under the previous kernel's tail
+  pdl_wait();
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
   // TMA producer (warp 6)
@@ -330,7 +337,6 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
       for (int it = 0; it < kWiSlots && it < nmine; ++it) produce(it);
     __syncwarp();
   }
-  load_const_tmem(tmem, Gimg, warp, lane);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -649,8 +655,10 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
   const int j = blockIdx.x / S, s0 = blockIdx.x - j * S;
   const int BKw = p.B * p.Kw;
   const int n = s0 < BKw ? (BKw - s0 + S - 1) / S : 0;   // tiles of this CTA: rem = s0 + i * S
+  pdl_launch_dependents();
   for (uint32_t i = tid; i < 3 * kTileBuf / 16; i += kMix2Threads) ((uint4*)sT)[i] = make_uint4(0, 0, 0, 0);
   for (uint32_t i = tid; i < 2 * kDft2Bytes / 16; i += kMix2Threads) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
+  pdl_wait();   // the weight images below are written by an earlier kernel of the chain
   {
     const uint8_t* wsrc = p.wprep + (size_t)j * 4 * kWBytes;
     for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMix2Threads) cp_async16(smem_u32(sW) + i * 16, wsrc + (size_t)i * 16);
@@ -1015,6 +1023,7 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
   const int j = cta / S, s = cta - j * S;
   const __nv_bfloat16* Aws = layer ? A_l1 : A_l2;
   const __nv_bfloat16* Gws = layer ? G_l1 : G_l2;
+  pdl_launch_dependents();
   for (uint32_t i = tid; i < kWgSmem / 16; i += 128) ((uint4*)smem)[i] = make_uint4(0, 0, 0, 0);
   __syncthreads();
   // constant-one column m = 96 of the "re" A operand, rows r < H, both stages
@@ -1035,6 +1044,7 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  pdl_wait();
   const uint32_t tmem = tmem_slot;
   const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
   const uint32_t Dre = tmem, Dim = tmem + 256;
@@ -1103,6 +1113,8 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
 // blockIdx.y = 0: layer 2 partial sums (first nb*S CTAs of tc_wgrad), 1: layer 1
 __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __restrict__ dW2, float2* __restrict__ dB2,
                                   float2* __restrict__ dW1, float2* __restrict__ dB1, int nb, int S, int accumulate) {
+  pdl_launch_dependents();
+  pdl_wait();
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const int nW = nb * BS * BS;
   const int layer = blockIdx.y;
@@ -1317,18 +1329,40 @@ size_t tc_workspace_bytes(const Geometry& g, bool backward) {
   return tc_carve(g, backward, nullptr).total;
 }
 
+// Kernel launch with the programmatic-dependent-launch attribute: `dependent` launches may begin their
+// prologue (barrier init, tensor-memory allocation, plan constants) under the tail of the previous kernel
+// of the stream; the kernels order themselves with pdl_wait().  The first kernel of an API call is a
+// plain launch, so the call as a whole keeps stream order with the caller's work.
+static const bool g_use_pdl = getenv("AFNO_NO_PDL") == nullptr;
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool dependent,
+                            Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = (dependent && g_use_pdl) ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 // W-direction launches: tile = (b, h, block), persistent over the SMs
 static cudaError_t launch_wdft_fwd(const Geometry& g, const TcPlan& tp, const void* in, void* spec, const uint8_t* fimg,
-                                   cudaStream_t st) {
+                                   cudaStream_t st, bool dependent) {
   CUtensorMap mx, ma;
   if (!act_tmap(tp, &mx, in, g) || !spec_store_tmap(tp, &ma, spec, g)) return cudaErrorInvalidValue;
   const int ntiles = g.B * g.H * g.nb;
   const int grid = ntiles < tp.num_sms ? ntiles : tp.num_sms;
   prof_begin("tc_wdft_fwd", st);
-  tc_wdft_fwd2<<<grid, kW2Threads, kWfSmem, st>>>(mx, ma, (const uint32_t*)fimg, ntiles, g.nb, g.H, g.Kw);
+  cudaError_t e = launch_k(tc_wdft_fwd2, grid, kW2Threads, kWfSmem, st, dependent, mx, ma, (const uint32_t*)fimg, ntiles, g.nb,
+                           g.H, g.Kw);
   prof_end(st);
   count_launch();
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 static cudaError_t launch_wdft_inv(const Geometry& g, const TcPlan& tp, const void* spec, const void* res, void* out,
                                    const uint8_t* gimg, cudaStream_t st) {
@@ -1338,10 +1372,11 @@ static cudaError_t launch_wdft_inv(const Geometry& g, const TcPlan& tp, const vo
   const int ntiles = g.B * g.H * g.nb;
   const int grid = ntiles < tp.num_sms ? ntiles : tp.num_sms;
   prof_begin("tc_wdft_inv", st);
-  tc_wdft_inv2<<<grid, kW2Threads, kWiSmem, st>>>(ma, mr, my, (const uint32_t*)gimg, ntiles, g.nb, g.H, g.W, res ? 1 : 0);
+  cudaError_t e = launch_k(tc_wdft_inv2, grid, kW2Threads, kWiSmem, st, true, ma, mr, my, (const uint32_t*)gimg, ntiles, g.nb,
+                           g.H, g.W, res ? 1 : 0);
   prof_end(st);
   count_launch();
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const float* w1, const float* b1,
@@ -1356,7 +1391,7 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  if ((e = launch_wdft_fwd(g, tp, x, w.A1, tp.fw, st)) != cudaSuccess) return e;
+  if ((e = launch_wdft_fwd(g, tp, x, w.A1, tp.fw, st, true)) != cudaSuccess) return e;
   MixParams mp{};
   mp.A1 = w.A1; mp.A2 = w.A2; mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
   mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
@@ -1365,10 +1400,11 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   if (g.save_ctx) {
     // saved context: Xh, O1 (operands of tc_wgrad) and the activation masks stay in the workspace
     mp.Xh = w.Xh; mp.O1 = w.O1; mp.maskbits = w.maskbits;
-    tc_mix2<kMixFwdSave, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2);
+    e = launch_k(tc_mix2<kMixFwdSave, false>, g.nb * S2, kMix2Threads, kMix2Smem, st, true, mp, S2);
   } else {
-    tc_mix2<kMixFwd, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2);
+    e = launch_k(tc_mix2<kMixFwd, false>, g.nb * S2, kMix2Threads, kMix2Smem, st, true, mp, S2);
   }
+  if (e != cudaSuccess) return e;
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -1381,12 +1417,14 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   TcWs w = tc_carve(g, true, (char*)ws);
   const TcPlan& tp = p.tc;
   cudaError_t e;
+  bool dep = false;   // false for the first kernel of the call only
 #define TC_LAUNCH(name, ...)                                  \
   prof_begin(name, st);                                       \
-  __VA_ARGS__;                                                \
+  e = launch_k(__VA_ARGS__);                                  \
   prof_end(st);                                               \
   count_launch();                                             \
-  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  dep = true;                                                 \
+  if (e != cudaSuccess || (e = cudaGetLastError()) != cudaSuccess) return e;
   const int nW = g.nb * BS * BS;
   if (g.export_masks) {
     if ((e = cudaMemsetAsync(ws, 0, w.mask_region, st)) != cudaSuccess) return e;
@@ -1394,13 +1432,15 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   // USE_CONTEXT: the operand images of the weights written by the forward call are still in the
   // workspace (the context belongs to one set of parameters)
   if (!g.use_ctx) {
-    TC_LAUNCH("k_tc_prep_weights", k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, w.wprep, w.bprep, g.nb));
+    TC_LAUNCH("k_tc_prep_weights", k_tc_prep_weights, (nW + 255) / 256, 256, 0, st, dep, w1, b1, w2, b2, w.wprep, w.bprep, g.nb);
   }
   // B1 (first half) and B2: W-direction spectra of x and of dy (alpha-weighted)
   if (!g.use_ctx) {
-    if ((e = launch_wdft_fwd(g, tp, x, w.A1, tp.fw, st)) != cudaSuccess) return e;
+    if ((e = launch_wdft_fwd(g, tp, x, w.A1, tp.fw, st, dep)) != cudaSuccess) return e;
+    dep = true;
   }
-  if ((e = launch_wdft_fwd(g, tp, dy, w.A1g, tp.fw_alpha, st)) != cudaSuccess) return e;
+  if ((e = launch_wdft_fwd(g, tp, dy, w.A1g, tp.fw_alpha, st, dep)) != cudaSuccess) return e;
+  dep = true;
   MixParams mp{};
   mp.A1 = w.A1; mp.A1g = w.A1g; mp.A2 = w.A2;
   mp.Xh = w.Xh; mp.O1 = w.O1; mp.G2 = w.G2; mp.G1 = w.G1;
@@ -1413,22 +1453,21 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   if (g.use_ctx) {
     // gradient stages only: Xh, O1 and the masks were left in the workspace by the forward call
     if (g.export_masks) {
-      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, true><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
+      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, true>, g.nb * S2, kMix2Threads, kMix2Smem, st, dep, mp, S2);
     } else {
-      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
+      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, false>, g.nb * S2, kMix2Threads, kMix2Smem, st, dep, mp, S2);
     }
   } else if (g.export_masks) {
-    TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, true><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
+    TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, true>, g.nb * S2, kMix2Threads, kMix2Smem, st, dep, mp, S2);
   } else {
-    TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, false><<<g.nb * S2, kMix2Threads, kMix2Smem, st>>>(mp, S2));
+    TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, false>, g.nb * S2, kMix2Threads, kMix2Smem, st, dep, mp, S2);
   }
   // B4 / B6: parameter gradients
   const int nred = nW + g.nb * BS;
-  TC_LAUNCH("tc_wgrad", tc_wgrad<<<2 * g.nb * w.S, 128, kWgSmem, st>>>(w.O1, w.G2, w.Xh, w.G1, w.part, g.B * g.Kw, g.H,
-                                                                        g.nb, w.S));
-  TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce<<<dim3((nred + 255) / 256, 2), 256, 0, st>>>(
-                                     w.part, (float2*)dw2, (float2*)db2, (float2*)dw1, (float2*)db1, g.nb, w.S,
-                                     g.accum ? 1 : 0));
+  TC_LAUNCH("tc_wgrad", tc_wgrad, 2 * g.nb * w.S, 128, kWgSmem, st, dep, w.O1, w.G2, w.Xh, w.G1, w.part, g.B * g.Kw, g.H,
+            g.nb, w.S);
+  TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce, dim3((nred + 255) / 256, 2), 256, 0, st, dep, w.part, (float2*)dw2,
+            (float2*)db2, (float2*)dw1, (float2*)db1, g.nb, w.S, g.accum ? 1 : 0);
 #undef TC_LAUNCH
   // B8: dx = dy + irfft2(GX / alpha)
   return launch_wdft_inv(g, tp, w.A2, g.no_residual ? nullptr : dy, dx, tp.gw_noalpha, st);

@@ -440,11 +440,10 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
 }
 
 // ---- F2-F7 / B1-B7: per (b, kw, block) GEMM chains in tensor memory (kernel tc_mix2 below) ----------
-constexpr int kMixLoadWarps = 3;
 
 struct MixParams {
-  const __nv_bfloat16* A1;   // forward: spectrum tiles; backward: x tiles
-  const __nv_bfloat16* A1g;  // backward: gradient tiles
+  CUtensorMap mapA1;         // input tiles (forward: spectrum of x; stateless backward: the same), see tile_tmap
+  CUtensorMap mapA1g;        // backward: gradient tiles
   __nv_bfloat16* A2;
   __nv_bfloat16 *Xh, *O1, *G2, *G1; // backward: operands of tc_wgrad
   const uint8_t* dft;        // Ch then Sh, kDft2Bytes each, smem image
@@ -456,16 +455,6 @@ struct MixParams {
   int B, H, Kw, Wh, nb, Kh;
   float lambda;
 };
-
-// rows of a (b,kw,j) tile [H][192] -> MN-major B operand (K = h, N = (ri, c)); loader warp `sub`
-__device__ __forceinline__ void load_tile_warp(uint32_t tile_saddr, const __nv_bfloat16* src, int H, int lane, int sub) {
-  // rows of kA2Row elements: chunk q = 16 bytes at src + row h = q / 24, chunk nc = q % 24
-  const int nchunks = H * (NT / 8);
-  for (int q = sub * 32 + lane; q < nchunks; q += kMixLoadWarps * 32) {
-    const int h = q / (NT / 8), nc = q - h * (NT / 8);
-    cp_async16(tile_saddr + nc * kTileSbo + h * 16, src + (size_t)h * kA2Row + nc * 8);
-  }
-}
 
 // ---- tc_mix2: two mode tiles in flight per CTA (ping-pong), 12 epilogue warps ------------------------
 // Same arithmetic and the same stages as tc_mix, rescheduled so that the tensor core and the
@@ -506,7 +495,6 @@ struct Mix2Bars {
   uint64_t gfull[3];  // backward: buffer holds the gradient tile
   uint64_t xfree[3];  // backward: stage 0 has consumed the x tile (tcgen05.commit)
   uint64_t sdone[3];  // the 12 epilogue warps have staged the tile's output rows in the buffer
-  uint64_t tfree[3];  // the staged rows have left the buffer (loader warp 0, after its bulk store has read them)
 };
 
 // One transform product pair: the same A (DFT matrix K-step) times two B tile halves
@@ -521,10 +509,23 @@ __device__ __forceinline__ void issue_dft2_pair(uint32_t d0, uint32_t d1, uint32
   }
 }
 // forward transform (exp(-i theta)):  Xr = Ch Ar + Sh Ai ; Xi = Ch Ai - Sh Ar
+// The input tile is six 64B-swizzled panels [96 rows (h, zero-filled past H)][32 columns] written by TMA:
+// panels 0..2 = re, 3..5 = im.
+constexpr uint32_t kInPanel = HP * 64;   // 6144
+__device__ __forceinline__ void issue_dft2_pair_sw(uint32_t d0, uint32_t d1, uint32_t a_base, uint32_t b0, uint32_t b1,
+                                                   uint32_t id0, uint32_t id1, bool fresh) {
+#pragma unroll
+  for (int ks = 0; ks < HP / 16; ++ks) {
+    const uint64_t ad = smem_desc(a_base + ks * 2 * kDft2Lbo, kDft2Lbo, kDft2Sbo);
+    const uint32_t acc = !(fresh && ks == 0);
+    mma_ss(d0, ad, smem_desc_sw64(b0 + ks * 1024, kInPanel, 512), id0, acc);
+    mma_ss(d1, ad, smem_desc_sw64(b1 + ks * 1024, kInPanel, 512), id1, acc);
+  }
+}
 __device__ __forceinline__ void issue_fwd_dft2(uint32_t Dre, uint32_t Dim, uint32_t aCh, uint32_t aSh, uint32_t tile) {
-  const uint32_t id = idesc_bf16(128, BS, kIdescBMn), half = (BS / 8) * kTileSbo;
-  issue_dft2_pair(Dre, Dim, aCh, tile, tile + half, id, id, true);
-  issue_dft2_pair(Dre, Dim, aSh, tile + half, tile, id, id | kIdescNegB, false);
+  const uint32_t id = idesc_bf16(128, BS, kIdescBMn), half = 3 * kInPanel;
+  issue_dft2_pair_sw(Dre, Dim, aCh, tile, tile + half, id, id, true);
+  issue_dft2_pair_sw(Dre, Dim, aSh, tile + half, tile, id, id | kIdescNegB, false);
 }
 // inverse transform (exp(+i theta)):  Tr = Ch Zr - Sh Zi ; Ti = Ch Zi + Sh Zr
 __device__ __forceinline__ void issue_inv_dft2(uint32_t Dre, uint32_t Dim, uint32_t aCh, uint32_t aSh, uint32_t tile) {
@@ -638,7 +639,7 @@ __device__ __forceinline__ void mbar_wait_fast(uint64_t* mbar, uint32_t parity) 
 // kMixBwdCtx (gradient stages only, 4 stages, reads the saved context).
 constexpr int kMixFwd = 0, kMixBwd = 1, kMixFwdSave = 2, kMixBwdCtx = 3;
 template <int MODE, bool EXPORT>
-__global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
+__global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant__ MixParams p, int S) {
   constexpr bool BACKWARD = MODE == kMixBwd || MODE == kMixBwdCtx;   // has the gradient stages
   constexpr bool RECOMP = MODE == kMixBwd, SAVE = MODE == kMixFwdSave, CTXB = MODE == kMixBwdCtx;
   constexpr int kStage0 = CTXB ? 3 : 0;                               // stage number of a tile's first phase
@@ -670,11 +671,10 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
       mbar_init(&bars.edone[q], 12);
     }
     for (int q = 0; q < 3; ++q) {
-      mbar_init(&bars.xfull[q], kMixLoadWarps * 32);
-      mbar_init(&bars.gfull[q], kMixLoadWarps * 32);
+      mbar_init(&bars.xfull[q], 1);
+      mbar_init(&bars.gfull[q], 1);
       mbar_init(&bars.xfree[q], 1);
       mbar_init(&bars.sdone[q], 12);
-      mbar_init(&bars.tfree[q], 1);
     }
     mbar_init_fence();
   }
@@ -692,65 +692,53 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(MixParams p, int S) {
   const int lq = warp & 3;
 
   if (lq == 3 && warp != 3) {
-    // ================================ loader warps (7, 11, 15) ================================
-    const int sub = (warp >> 2) - 1;
+    // ================================ copy warp (7; 11 and 15 idle) ============================
+    // warp 7 lane 0 issues every copy (TMA tile loads in, bulk stores of the staged rows out); the other
+    // two warps of this lane quarter have nothing to do
     const uint32_t aT = smem_u32(sT);
-    auto tile_off = [&](int i) { return ((size_t)(s0 + i * S) * p.nb + j) * p.H * kA2Row; };
-    auto load = [&](int buf, const __nv_bfloat16* src, uint64_t* full) {
-      // rows H..95 of the operand are K padding: the output staging of the buffer's previous tile
-      // overlaps them, so they are cleared again
-      for (int q = sub * 32 + lane; q < (HP - p.H) * (NT / 8); q += kMixLoadWarps * 32) {
-        const int nc = q / (HP - p.H), h = p.H + q - nc * (HP - p.H);
-        *(uint4*)(sT + buf * kTileBuf + nc * kTileSbo + h * 16) = make_uint4(0, 0, 0, 0);
-      }
-      load_tile_warp(aT + buf * kTileBuf, src, p.H, lane, sub);
-      cp_async_wait_all();
-      fence_async_smem();
-      mbar_arrive(full);
-    };
-    // tile k's output rows are staged in its buffer by the epilogue warps; loader warp 0 sends them
-    // to A2 with one bulk copy and frees the buffer once the copy has read it
-    auto drain = [&](int k) {
-      const int buf = k % 3;
-      const uint32_t par = (uint32_t)((k / 3) & 1);
-      if (sub == 0) {
-        if (lane == 0) {
-          mbar_wait(&bars.sdone[buf], par);
-          bulk_store(p.A2 + ((size_t)(s0 + k * S) * p.nb + j) * p.H * kA2Row, aT + buf * kTileBuf,
-                     (uint32_t)p.H * kOutStride);
-          bulk_wait_read<0>();
-          mbar_arrive(&bars.tfree[buf]);
+    if (warp == 7 && lane == 0) {
+      auto load = [&](int buf, const CUtensorMap* m, int i, uint64_t* full) {
+        const int tile_id = (s0 + i * S) * p.nb + j;
+        mbar_expect_tx(full, 6 * kInPanel);
+#pragma unroll
+        for (int pn = 0; pn < 6; ++pn) tma_load4(aT + buf * kTileBuf + pn * kInPanel, m, 0, pn, 0, tile_id, full);
+      };
+      // tile k's output rows are staged in its buffer by the epilogue warps; they leave with one bulk copy
+      // and the buffer is free once the copy has read it
+      auto drain = [&](int k) {
+        const int buf = k % 3;
+        mbar_wait(&bars.sdone[buf], (uint32_t)((k / 3) & 1));
+        bulk_store(p.A2 + ((size_t)(s0 + k * S) * p.nb + j) * p.H * kA2Row, aT + buf * kTileBuf, (uint32_t)p.H * kOutStride);
+        bulk_wait_read<0>();
+      };
+      if (!RECOMP) {
+        const CUtensorMap* src = CTXB ? &p.mapA1g : &p.mapA1;
+        for (int i = 0; i < n; ++i) {
+          if (i >= 3) drain(i - 3);
+          load(i % 3, src, i, &bars.xfull[i % 3]);
         }
-        __syncwarp();
-      }
-      mbar_wait(&bars.tfree[buf], par);
-    };
-    if (!RECOMP) {
-      const __nv_bfloat16* src = CTXB ? p.A1g : p.A1;
-      for (int i = 0; i < n; ++i) {
-        if (i >= 3) drain(i - 3);
-        load(i % 3, src + tile_off(i), &bars.xfull[i % 3]);
-      }
-      for (int k = n > 3 ? n - 3 : 0; k < n; ++k) drain(k);
-    } else {
-      // x(0) x(1) x(2) | g(0) g(1) | then for k = 0, 1, ..: x(k+3) after the last stage of tile k,
-      // g(k+2) after stage 0 of tile k+2 -- the order in which the buffers become free
-      for (int i = 0; i < 3 && i < n; ++i) load(i, p.A1 + tile_off(i), &bars.xfull[i]);
-      for (int i = 0; i < 2 && i < n; ++i) {
-        mbar_wait(&bars.xfree[i], 0u);
-        load(i, p.A1g + tile_off(i), &bars.gfull[i]);
-      }
-      for (int k = 0; k < n; ++k) {
-        const int ix = k + 3, ig = k + 2;
-        drain(k);
-        if (ix < n) load(ix % 3, p.A1 + tile_off(ix), &bars.xfull[ix % 3]);
-        if (ig < n) {
-          mbar_wait(&bars.xfree[ig % 3], (uint32_t)((ig / 3) & 1));
-          load(ig % 3, p.A1g + tile_off(ig), &bars.gfull[ig % 3]);
+        for (int k = n > 3 ? n - 3 : 0; k < n; ++k) drain(k);
+      } else {
+        // x(0) x(1) x(2) | g(0) g(1) | then for k = 0, 1, ..: x(k+3) after the last stage of tile k,
+        // g(k+2) after stage 0 of tile k+2 -- the order in which the buffers become free
+        for (int i = 0; i < 3 && i < n; ++i) load(i, &p.mapA1, i, &bars.xfull[i]);
+        for (int i = 0; i < 2 && i < n; ++i) {
+          mbar_wait(&bars.xfree[i], 0u);
+          load(i, &p.mapA1g, i, &bars.gfull[i]);
+        }
+        for (int k = 0; k < n; ++k) {
+          const int ix = k + 3, ig = k + 2;
+          drain(k);
+          if (ix < n) load(ix % 3, &p.mapA1, ix, &bars.xfull[ix % 3]);
+          if (ig < n) {
+            mbar_wait(&bars.xfree[ig % 3], (uint32_t)((ig / 3) & 1));
+            load(ig % 3, &p.mapA1g, ig, &bars.gfull[ig % 3]);
+          }
         }
       }
+      bulk_wait<0>();
     }
-    if (sub == 0 && lane == 0) bulk_wait<0>();
+    __syncwarp();
   } else if (warp == 3) {
     // ================================ control warp ===========================================
     const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW), aT = smem_u32(sT);
@@ -1205,6 +1193,16 @@ bool spec_load_tmap(const TcPlan& tp, CUtensorMap* m, const void* ptr, const Geo
   return make_tmap(tp, m, ptr, 5, dims, str, box, true);
 }
 
+// the same tensor read by tc_mix2, one (b, kw, block) tile at a time: six boxes [96 rows h][32 columns]
+// (rows past H zero-filled), 64B-swizzled
+bool tile_tmap(const TcPlan& tp, CUtensorMap* m, const void* ptr, const Geometry& g) {
+  const uint64_t row = kOutStride;
+  const uint64_t dims[4] = {32, 6, (uint64_t)g.H, (uint64_t)g.B * g.Kw * g.nb};
+  const uint64_t str[3] = {64, row, row * g.H};
+  const uint32_t box[4] = {32, 1, (uint32_t)HP, 1};
+  return make_tmap(tp, m, ptr, 4, dims, str, box, true);
+}
+
 struct TcWs {
   __nv_bfloat16 *A1, *A2, *wprep;
   float* bprep;
@@ -1393,7 +1391,9 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   if ((e = launch_wdft_fwd(g, tp, x, w.A1, tp.fw, st, true)) != cudaSuccess) return e;
   MixParams mp{};
-  mp.A1 = w.A1; mp.A2 = w.A2; mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
+  if (!tile_tmap(tp, &mp.mapA1, w.A1, g)) return cudaErrorInvalidValue;
+  mp.mapA1g = mp.mapA1;
+  mp.A2 = w.A2; mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
   mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
   prof_begin("tc_mix_fwd", st);
   const int S2 = mix2_split(g, tp);
@@ -1442,7 +1442,8 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   if ((e = launch_wdft_fwd(g, tp, dy, w.A1g, tp.fw_alpha, st, dep)) != cudaSuccess) return e;
   dep = true;
   MixParams mp{};
-  mp.A1 = w.A1; mp.A1g = w.A1g; mp.A2 = w.A2;
+  if (!tile_tmap(tp, &mp.mapA1, w.A1, g) || !tile_tmap(tp, &mp.mapA1g, w.A1g, g)) return cudaErrorInvalidValue;
+  mp.A2 = w.A2;
   mp.Xh = w.Xh; mp.O1 = w.O1; mp.G2 = w.G2; mp.G1 = w.G1;
   mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
   mp.mask1 = g.export_masks ? w.mask1 : nullptr;

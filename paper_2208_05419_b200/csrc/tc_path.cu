@@ -495,6 +495,8 @@ struct Mix2Bars {
   uint64_t gfull[3];  // backward: buffer holds the gradient tile
   uint64_t xfree[3];  // backward: stage 0 has consumed the x tile (tcgen05.commit)
   uint64_t sdone[3];  // the 12 epilogue warps have staged the tile's output rows in the buffer
+  uint64_t imgfull[2]; // stream: the 12 epilogue warps have staged an operand image (Xh, O1, G2, G1) in the tile buffer
+  uint64_t imgfree[2]; // stream: the image's bulk store has read the buffer
 };
 
 // One transform product pair: the same A (DFT matrix K-step) times two B tile halves
@@ -643,6 +645,11 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
   constexpr bool BACKWARD = MODE == kMixBwd || MODE == kMixBwdCtx;   // has the gradient stages
   constexpr bool RECOMP = MODE == kMixBwd, SAVE = MODE == kMixFwdSave, CTXB = MODE == kMixBwdCtx;
   constexpr int kStage0 = CTXB ? 3 : 0;                               // stage number of a tile's first phase
+  // FwdSave / BwdCtx: the operand images for tc_wgrad are staged in the tile's buffer (idle between its
+  // first GEMM and the write of the inverse transform's operand) and leave by bulk copies issued by
+  // warp 11, so no epilogue warp ever stalls on the global store path.  The stateless backward reloads
+  // that buffer with the gradient tile meanwhile and stores the images with plain vector stores.
+  constexpr bool STAGED = SAVE || CTXB;
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ Mix2Bars bars;
   __shared__ uint32_t tmem_slot;
@@ -669,6 +676,8 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
     for (int q = 0; q < 2; ++q) {
       mbar_init(&bars.dfull[q], 1);
       mbar_init(&bars.edone[q], 12);
+      mbar_init(&bars.imgfull[q], 12);
+      mbar_init(&bars.imgfree[q], 1);
     }
     for (int q = 0; q < 3; ++q) {
       mbar_init(&bars.xfull[q], 1);
@@ -735,6 +744,26 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
             load(ig % 3, &p.mapA1g, ig, &bars.gfull[ig % 3]);
           }
         }
+      }
+      bulk_wait<0>();
+    }
+    if (STAGED && warp == 11 && lane == 0) {
+      // ---- image warp: the phases in order; an image phase = wait for the staged image, send it ----
+      uint32_t cnt[2] = {0, 0};
+      for (int t = 0; t < T; ++t) {
+        const int stream = t & 1, u = (t >> 1) - (stream ? kLag : 0);
+        if (u < 0) continue;
+        const int pair = u / NS, stg = u - pair * NS;
+        const int i = 2 * pair + stream;
+        if (i >= n) continue;
+        const int se = stg + kStage0;
+        if (!(SAVE ? (se == 0 || se == 1) : (se == 3 || se == 4))) continue;
+        __nv_bfloat16* img = se == 0 ? p.Xh : se == 1 ? p.O1 : se == 3 ? p.G2 : p.G1;
+        mbar_wait(&bars.imgfull[stream], cnt[stream] & 1u);
+        ++cnt[stream];
+        bulk_store((uint8_t*)img + ((size_t)(s0 + i * S) * p.nb + j) * kTileBytes, aT + (i % 3) * kTileBuf, kTileBytes);
+        bulk_wait_read<0>();
+        mbar_arrive(&bars.imgfree[stream]);
       }
       bulk_wait<0>();
     }
@@ -812,6 +841,11 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
     const uint32_t bar_id = 1 + lq;
     uint32_t m1[2][2] = {{0, 0}, {0, 0}}, m2[2][2] = {{0, 0}, {0, 0}};   // [stream][word]
     uint32_t ce[2] = {0, 0};
+    uint32_t ci[2] = {0, 0};   // images staged so far per stream
+    // the tile buffer may be overwritten once the stream's last image store has read it
+    auto wait_img_read = [&](int stream) {
+      if (STAGED && ci[stream] > 0) mbar_wait(&bars.imgfree[stream], (ci[stream] - 1) & 1u);
+    };
 #ifdef AFNO_TIMING
     long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     long long dbg_m[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -894,6 +928,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
           }
           if (!BACKWARD) {
             // forward: Z is the B operand of the inverse transform
+            wait_img_read(stream);
             store_chunks6(tile, chunk0, r, pk);
             fence_async_smem();
             if (SAVE) p.maskbits[mask_idx] = make_uint4(m1[stream][0], m1[stream][1], m2[stream][0], m2[stream][1]);
@@ -931,6 +966,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
 #pragma unroll
           for (int q = 0; q < 24; ++q)
             pk[q] = row_valid ? pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1])) : 0u;
+          wait_img_read(stream);
           store_chunks6(tile, chunk0, r, pk);
           fence_async_smem();
           if (EXPORT && row_valid) {
@@ -963,7 +999,18 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
           __syncwarp();
           if (lane == 0) mbar_arrive(&bars.edone[stream]);
         }
-        if (gimg != nullptr) store_chunks6(gimg, chunk0, r, pk);
+        if (gimg != nullptr) {
+          if (STAGED) {
+            wait_img_read(stream);
+            store_chunks6(tile, chunk0, r, pk);
+            fence_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars.imgfull[stream]);
+            ++ci[stream];
+          } else {
+            store_chunks6(gimg, chunk0, r, pk);
+          }
+        }
         TR(t, 6 + warp * 3);
         DBG_ACC(1);
       }

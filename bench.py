@@ -366,7 +366,7 @@ def kernel_work(name, B, wl, kept_modes, ctx=True):
 
 def measured_traffic(name):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture."""
-    path = os.path.join(ROOT, "profiles", "r1b_dram_traffic.json")
+    path = os.path.join(ROOT, "profiles", "r1d_dram_traffic.json")
     try:
         return json.load(open(path)).get(name)
     except Exception:

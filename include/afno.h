@@ -122,8 +122,13 @@ int afno_spectral_bwd(const afno_desc_t* d, const void* x, const void* dy, const
 
 /* End-to-end variants with HOST buffers (pinned memory recommended).  `arena` is a device
  * scratch buffer of at least afno_spectral_host_arena_bytes(); the calls copy the inputs
- * host->device, run the device path above, copy the results device->host on `cuda_stream`
- * and synchronise that stream before returning.  Every *_host pointer is a host pointer. */
+ * host->device, run the device path above, copy the results device->host and synchronise
+ * before returning.  Every *_host pointer is a host pointer (pinned memory lets the copies
+ * overlap).  The work is pipelined over the batch: sample b+1 is copied in on an internal
+ * copy stream while sample b computes on `cuda_stream` and sample b-1 is copied out on a
+ * second internal stream; y and dx equal the device path's bit for bit, the parameter
+ * gradients are the in-order sum of the per-sample gradients (fp32 summation order differs
+ * from one batched call).  The context flags and EXPORT_MASKS have no meaning here. */
 size_t afno_spectral_host_arena_bytes(const afno_desc_t* d, int for_backward);
 int afno_spectral_fwd_host(const afno_desc_t* d, const void* x_host, const float* w1_host,
                            const float* b1_host, const float* w2_host, const float* b2_host,

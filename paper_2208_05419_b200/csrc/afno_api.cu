@@ -422,6 +422,45 @@ size_t afno_spectral_host_arena_bytes(const afno_desc_t* d, int for_backward) {
     if (e_ != cudaSuccess) return fail(AFNO_ERR_CUDA, std::string(#expr ": ") + cudaGetErrorString(e_)); \
   } while (0)
 
+// The host variants are PCIe-bound (0.5 GB per fwd+bwd step at B = 4 against 0.5 ms of kernels), so they
+// pipeline over the batch: sample b+1 travels host->device on one copy stream while sample b computes on
+// the caller's stream and sample b-1 travels device->host on a second copy stream (the link is full
+// duplex).  Samples are independent ("batched"); the parameter gradients of the samples
+// are accumulated in order with AFNO_FLAG_ACCUM_GRADS.
+namespace {
+struct HostPipe {
+  int device = -1;
+  cudaStream_t h2d = nullptr, d2h = nullptr;
+};
+thread_local HostPipe t_pipe;
+cudaError_t host_pipe(HostPipe** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (t_pipe.device != dev) {
+    if ((e = cudaStreamCreateWithFlags(&t_pipe.h2d, cudaStreamNonBlocking)) != cudaSuccess) return e;
+    if ((e = cudaStreamCreateWithFlags(&t_pipe.d2h, cudaStreamNonBlocking)) != cudaSuccess) return e;
+    t_pipe.device = dev;
+  }
+  *out = &t_pipe;
+  return cudaSuccess;
+}
+struct EventPool {
+  std::vector<cudaEvent_t> ev;
+  ~EventPool() {
+    for (cudaEvent_t e : ev) cudaEventDestroy(e);
+  }
+  cudaError_t mark(cudaStream_t on, cudaStream_t waiter) {
+    cudaEvent_t e;
+    cudaError_t rc = cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+    if (rc != cudaSuccess) return rc;
+    ev.push_back(e);
+    if ((rc = cudaEventRecord(e, on)) != cudaSuccess) return rc;
+    return cudaStreamWaitEvent(waiter, e, 0);
+  }
+};
+} // namespace
+
 int afno_spectral_fwd_host(const afno_desc_t* d, const void* x_host, const float* w1_host,
                            const float* b1_host, const float* w2_host, const float* b2_host,
                            void* y_host, void* arena, size_t arena_bytes, void* cuda_stream) {
@@ -434,14 +473,28 @@ int afno_spectral_fwd_host(const afno_desc_t* d, const void* x_host, const float
   HostLayout h = host_layout(d, g, false, (char*)arena);
   if (arena_bytes < h.total) return fail(AFNO_ERR_WORKSPACE, "arena smaller than afno_spectral_host_arena_bytes(d, 0)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.x, x_host, h.act, cudaMemcpyHostToDevice, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w1, w1_host, h.nw, cudaMemcpyHostToDevice, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b1, b1_host, h.nb1, cudaMemcpyHostToDevice, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w2, w2_host, h.nw, cudaMemcpyHostToDevice, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b2, b2_host, h.nb2, cudaMemcpyHostToDevice, st));
-  rc = afno_spectral_fwd(d, h.x, h.w1, h.b1, h.w2, h.b2, h.y, h.ws, h.ws_bytes, cuda_stream);
-  if (rc != AFNO_OK) return rc;
-  AFNO_CUDA_TRY(cudaMemcpyAsync(y_host, h.y, h.act, cudaMemcpyDeviceToHost, st));
+  HostPipe* hp = nullptr;
+  AFNO_CUDA_TRY(host_pipe(&hp));
+  EventPool ev;
+  afno_desc_t d1 = *d;
+  d1.B = 1;
+  d1.flags &= ~(uint32_t)(AFNO_FLAG_SAVE_CONTEXT | AFNO_FLAG_USE_CONTEXT);
+  const size_t sample = h.act / (size_t)g.B;
+  AFNO_CUDA_TRY(ev.mark(st, hp->h2d));   // the copies start after the caller's earlier work on the stream
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w1, w1_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b1, b1_host, h.nb1, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w2, w2_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b2, b2_host, h.nb2, cudaMemcpyHostToDevice, hp->h2d));
+  for (int b = 0; b < g.B; ++b) {
+    const size_t off = (size_t)b * sample;
+    AFNO_CUDA_TRY(cudaMemcpyAsync((char*)h.x + off, (const char*)x_host + off, sample, cudaMemcpyHostToDevice, hp->h2d));
+    AFNO_CUDA_TRY(ev.mark(hp->h2d, st));
+    rc = afno_spectral_fwd(&d1, (char*)h.x + off, h.w1, h.b1, h.w2, h.b2, (char*)h.y + off, h.ws, h.ws_bytes, cuda_stream);
+    if (rc != AFNO_OK) return rc;
+    AFNO_CUDA_TRY(ev.mark(st, hp->d2h));
+    AFNO_CUDA_TRY(cudaMemcpyAsync((char*)y_host + off, (char*)h.y + off, sample, cudaMemcpyDeviceToHost, hp->d2h));
+  }
+  AFNO_CUDA_TRY(cudaStreamSynchronize(hp->d2h));
   AFNO_CUDA_TRY(cudaStreamSynchronize(st));
   return AFNO_OK;
 }
@@ -459,24 +512,41 @@ int afno_spectral_bwd_host(const afno_desc_t* d, const void* x_host, const void*
     return fail(AFNO_ERR_INVALID_ARG, "NULL pointer argument");
   if (d->flags & AFNO_FLAG_ACCUM_GRADS)
     return fail(AFNO_ERR_INVALID_ARG, "AFNO_FLAG_ACCUM_GRADS is not meaningful for the host variant");
+  if (d->flags & AFNO_FLAG_EXPORT_MASKS)
+    return fail(AFNO_ERR_INVALID_ARG, "AFNO_FLAG_EXPORT_MASKS is not meaningful for the host variant");
   if (!aligned16(arena)) return fail(AFNO_ERR_INVALID_ARG, "arena must be 16-byte aligned");
   HostLayout h = host_layout(d, g, true, (char*)arena);
   if (arena_bytes < h.total) return fail(AFNO_ERR_WORKSPACE, "arena smaller than afno_spectral_host_arena_bytes(d, 1)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.x, x_host, h.act, cudaMemcpyHostToDevice, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.dy, dy_host, h.act, cudaMemcpyHostToDevice, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w1, w1_host, h.nw, cudaMemcpyHostToDevice, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b1, b1_host, h.nb1, cudaMemcpyHostToDevice, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w2, w2_host, h.nw, cudaMemcpyHostToDevice, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b2, b2_host, h.nb2, cudaMemcpyHostToDevice, st));
-  rc = afno_spectral_bwd(d, h.x, h.dy, h.w1, h.b1, h.w2, h.b2, h.dx, h.dw1, h.db1, h.dw2, h.db2, h.ws,
-                         h.ws_bytes, cuda_stream);
-  if (rc != AFNO_OK) return rc;
-  AFNO_CUDA_TRY(cudaMemcpyAsync(dx_host, h.dx, h.act, cudaMemcpyDeviceToHost, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(dw1_host, h.dw1, h.nw, cudaMemcpyDeviceToHost, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(db1_host, h.db1, h.nb1, cudaMemcpyDeviceToHost, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(dw2_host, h.dw2, h.nw, cudaMemcpyDeviceToHost, st));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(db2_host, h.db2, h.nb2, cudaMemcpyDeviceToHost, st));
+  HostPipe* hp = nullptr;
+  AFNO_CUDA_TRY(host_pipe(&hp));
+  EventPool ev;
+  afno_desc_t d1 = *d;
+  d1.B = 1;
+  d1.flags &= ~(uint32_t)(AFNO_FLAG_SAVE_CONTEXT | AFNO_FLAG_USE_CONTEXT);
+  const size_t sample = h.act / (size_t)g.B;
+  AFNO_CUDA_TRY(ev.mark(st, hp->h2d));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w1, w1_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b1, b1_host, h.nb1, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w2, w2_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b2, b2_host, h.nb2, cudaMemcpyHostToDevice, hp->h2d));
+  for (int b = 0; b < g.B; ++b) {
+    const size_t off = (size_t)b * sample;
+    AFNO_CUDA_TRY(cudaMemcpyAsync((char*)h.x + off, (const char*)x_host + off, sample, cudaMemcpyHostToDevice, hp->h2d));
+    AFNO_CUDA_TRY(cudaMemcpyAsync((char*)h.dy + off, (const char*)dy_host + off, sample, cudaMemcpyHostToDevice, hp->h2d));
+    AFNO_CUDA_TRY(ev.mark(hp->h2d, st));
+    d1.flags = b == 0 ? (d1.flags & ~(uint32_t)AFNO_FLAG_ACCUM_GRADS) : (d1.flags | AFNO_FLAG_ACCUM_GRADS);
+    rc = afno_spectral_bwd(&d1, (char*)h.x + off, (char*)h.dy + off, h.w1, h.b1, h.w2, h.b2, (char*)h.dx + off, h.dw1, h.db1,
+                           h.dw2, h.db2, h.ws, h.ws_bytes, cuda_stream);
+    if (rc != AFNO_OK) return rc;
+    AFNO_CUDA_TRY(ev.mark(st, hp->d2h));
+    AFNO_CUDA_TRY(cudaMemcpyAsync((char*)dx_host + off, (char*)h.dx + off, sample, cudaMemcpyDeviceToHost, hp->d2h));
+  }
+  AFNO_CUDA_TRY(cudaMemcpyAsync(dw1_host, h.dw1, h.nw, cudaMemcpyDeviceToHost, hp->d2h));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(db1_host, h.db1, h.nb1, cudaMemcpyDeviceToHost, hp->d2h));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(dw2_host, h.dw2, h.nw, cudaMemcpyDeviceToHost, hp->d2h));
+  AFNO_CUDA_TRY(cudaMemcpyAsync(db2_host, h.db2, h.nb2, cudaMemcpyDeviceToHost, hp->d2h));
+  AFNO_CUDA_TRY(cudaStreamSynchronize(hp->d2h));
   AFNO_CUDA_TRY(cudaStreamSynchronize(st));
   return AFNO_OK;
 }

@@ -261,5 +261,7 @@ def test_host_variants_match_device(oracle):
     hg = [torch.empty_like(t).pin_memory() for t in hp]
     binding.afno_spectral_bwd_host(desc, hx, hdy, *hp, hdx, *hg, arena)
     assert np.array_equal(hdx.numpy(), g_dev["dx"])
+    # the host variant pipelines over the batch: parameter gradients are the in-order sum of the
+    # per-sample gradients (include/afno.h), i.e. the device result up to fp32 summation order
     for t, k in zip(hg, ("dw1", "db1", "dw2", "db2")):
-        assert np.array_equal(t.numpy(), g_dev[k]), k
+        assert parity.rel_l2(t.numpy(), g_dev[k]) <= 2e-6, k

@@ -215,6 +215,9 @@ def test_saved_context_backward_matches_stateless():
     a slice of the headline shape, and the generic path, where the flags are accepted and ignored)."""
     import torch
     cases = [(parity.desc_for(inputs.WORKLOADS["fcn_b4_bwd"], B=2), inputs.make_inputs(inputs.WORKLOADS["fcn_b4_bwd"], B=2)),
+             # truncated spectrum (kept fraction 0.5): masks of dropped rows / absent kw tiles stay zero
+             (parity.desc_for(inputs.WORKLOADS["fcn_b4_bwd"], B=1, kept_fraction=0.5),
+              inputs.make_inputs(inputs.WORKLOADS["fcn_b4_bwd"], B=1)),
              (parity.desc_for(inputs.WORKLOADS["sub_bwd_nb2"]), inputs.make_inputs(inputs.WORKLOADS["sub_bwd_nb2"]))]
     for desc, data in cases:
         bf16 = desc.dtype == binding.AFNO_BF16
@@ -240,6 +243,49 @@ def test_saved_context_backward_matches_stateless():
         assert np.array_equal(parity.from_device_act(tdx), ref["dx"])
         for t, k in zip(g, ("dw1", "db1", "dw2", "db2")):
             assert np.array_equal(t.cpu().numpy(), ref[k]), k
+
+
+def test_saved_context_step_vs_oracle(oracle):
+    """The training step bench.py times (fwd SAVE_CONTEXT, bwd USE_CONTEXT on the same workspace), pinned
+    to the oracle directly: y within tolerance, gradients mask-consistent within tolerance, flipped
+    masks justified (S3 P-fwd / P-bwd)."""
+    import torch
+    wl = inputs.WORKLOADS["fcn_b4_bwd"]
+    data = inputs.make_inputs(wl, B=2)
+    base = parity.desc_for(wl, B=2, flags=binding.FLAG_EXPORT_MASKS)
+    d_save = binding.Desc(**{**base.__dict__, "flags": base.flags | binding.FLAG_SAVE_CONTEXT})
+    d_use = binding.Desc(**{**base.__dict__, "flags": base.flags | binding.FLAG_USE_CONTEXT})
+    layer = parity.GpuLayer(base)
+    ws = torch.empty(binding.afno_spectral_workspace_bytes(base, True), dtype=torch.uint8, device="cuda")
+    tx, tdy = parity.to_device_act(data["x"], True), parity.to_device_act(data["dy"], True)
+    ty, tdx = torch.empty_like(tx), torch.empty_like(tx)
+    p = layer.params(data["w1"], data["b1"], data["w2"], data["b2"])
+    g = [torch.zeros_like(t) for t in p]
+    binding.afno_spectral_fwd(d_save, tx, *p, ty, ws)
+    binding.afno_spectral_bwd(d_use, tx, tdy, *p, tdx, *g, ws)
+    torch.cuda.synchronize()
+    m1b, m2off, m2b = binding.afno_spectral_mask_bytes(base)
+    host = ws[:m2off + m2b].cpu().numpy()
+    mask1 = host[:m1b].reshape(base.B, base.H, base.Wh, base.num_blocks * base.hid, 2)
+    mask2 = host[m2off:m2off + m2b].reshape(base.B, base.H, base.Wh, base.C, 2)
+    cfg = parity.oracle_cfg(oracle, base)
+    args = (data["x"], data["dy"], data["w1"], data["b1"], data["w2"], data["b2"])
+    y_ref = oracle.forward(cfg, data["x"], *args[2:])
+    ey = parity.rel_l2(parity.from_device_act(ty), y_ref)
+    ref = oracle.backward(cfg, *args, mask1=mask1, mask2=mask2)
+    raw = oracle.backward(cfg, *args, dump=True)
+    s1, s2 = parity.preactivation_scales(cfg, raw["dump"], *(data[k].astype(np.float64) for k in ("w1", "b1", "w2", "b2")))
+    rep = parity.mask_flip_report(raw["dump"], mask1, mask2, cfg.lam, TOL_BF16 * s1, TOL_BF16 * s2)
+    got = dict(dx=parity.from_device_act(tdx), dw1=g[0].cpu().numpy(), db1=g[1].cpu().numpy(),
+               dw2=g[2].cpu().numpy(), db2=g[3].cpu().numpy())
+    print(f"[ctx step] rel_l2(y)={ey:.3e} flips relu {rep['flip1']:.2e} shrink {rep['flip2']:.2e} "
+          f"worst {rep['worst1']:.2f} / {rep['worst2']:.2f}")
+    assert ey <= TOL_BF16
+    for k in ("dx", "dw1", "db1", "dw2", "db2"):
+        e = parity.rel_l2(got[k], ref[k])
+        print(f"[ctx step] {k}: rel_l2 mask-consistent {e:.3e}")
+        assert e <= TOL_BF16, (k, e)
+    assert rep["flip1"] <= 5e-3 and rep["flip2"] <= 5e-3 and rep["justified"], rep
 
 
 def test_host_variants_match_device(oracle):

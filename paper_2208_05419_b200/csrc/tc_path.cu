@@ -662,7 +662,12 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int j = blockIdx.x / S, s0 = blockIdx.x - j * S;
   const int BKw = p.B * p.Kw;
-  const int n = s0 < BKw ? (BKw - s0 + S - 1) / S : 0;   // tiles of this CTA: rem = s0 + i * S
+  const int n = s0 < BKw ? (BKw - s0 + S - 1) / S : 0;   // tiles of this CTA
+  // Tile i of this CTA is (b, kw) pair rem = BKw - 1 - (s0 + i * S): the tiles run from the LAST sample
+  // to the first.  The W-direction kernels run from the first sample to the last, so this kernel starts
+  // on the part of A1 its producer wrote last (still in the 126 MB L2) and finishes with the part of A2
+  // its consumer reads first.
+  const int rtop = BKw - 1 - s0;
   pdl_launch_dependents();
   for (uint32_t i = tid; i < 3 * kTileBuf / 16; i += kMix2Threads) ((uint4*)sT)[i] = make_uint4(0, 0, 0, 0);
   for (uint32_t i = tid; i < 2 * kDft2Bytes / 16; i += kMix2Threads) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
@@ -707,7 +712,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
     const uint32_t aT = smem_u32(sT);
     if (warp == 7 && lane == 0) {
       auto load = [&](int buf, const CUtensorMap* m, int i, uint64_t* full) {
-        const int tile_id = (s0 + i * S) * p.nb + j;
+        const int tile_id = (rtop - i * S) * p.nb + j;
         mbar_expect_tx(full, 6 * kInPanel);
 #pragma unroll
         for (int pn = 0; pn < 6; ++pn) tma_load4(aT + buf * kTileBuf + pn * kInPanel, m, 0, pn, 0, tile_id, full);
@@ -717,7 +722,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
       auto drain = [&](int k) {
         const int buf = k % 3;
         mbar_wait(&bars.sdone[buf], (uint32_t)((k / 3) & 1));
-        bulk_store(p.A2 + ((size_t)(s0 + k * S) * p.nb + j) * p.H * kA2Row, aT + buf * kTileBuf, (uint32_t)p.H * kOutStride);
+        bulk_store(p.A2 + ((size_t)(rtop - k * S) * p.nb + j) * p.H * kA2Row, aT + buf * kTileBuf, (uint32_t)p.H * kOutStride);
         bulk_wait_read<0>();
       };
       if (!RECOMP) {
@@ -761,7 +766,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
         __nv_bfloat16* img = se == 0 ? p.Xh : se == 1 ? p.O1 : se == 3 ? p.G2 : p.G1;
         mbar_wait(&bars.imgfull[stream], cnt[stream] & 1u);
         ++cnt[stream];
-        bulk_store((uint8_t*)img + ((size_t)(s0 + i * S) * p.nb + j) * kTileBytes, aT + (i % 3) * kTileBuf, kTileBytes);
+        bulk_store((uint8_t*)img + ((size_t)(rtop - i * S) * p.nb + j) * kTileBytes, aT + (i % 3) * kTileBuf, kTileBytes);
         bulk_wait_read<0>();
         mbar_arrive(&bars.imgfree[stream]);
       }
@@ -861,7 +866,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
         const int pair = u / NS, stg = u - pair * NS;
         const int i = 2 * pair + stream;
         if (i >= n) continue;
-        const int rem = s0 + i * S;
+        const int rem = rtop - i * S;
         const uint32_t src = tmem + lane_sel + kSlot * (uint32_t)((3 * t + half) % 5) + chalf * 48;
         const uint32_t dstA = tmem + lane_sel + kSlot * (uint32_t)((3 * t) % 5) + 24 * cq;
         uint8_t* tile = sT + (i % 3) * kTileBuf;

@@ -82,6 +82,28 @@ __device__ __forceinline__ void pack32(const uint32_t (&v)[32], uint32_t (&pk)[1
   for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
 }
 
+// Which copies carry a non-default L2 eviction policy (chosen by measurement, S5.3); bit set =
+// the policy named in the comment, clear = evict_normal.
+enum {
+  kPolWfLoad = 1,     // tc_wdft_fwd2: activation loads evict_first
+  kPolWfStore = 2,    // tc_wdft_fwd2: A1 stores evict_last
+  kPolWiLoad = 4,     // tc_wdft_inv2: A2 and residual loads evict_first
+  kPolWiStore = 8,    // tc_wdft_inv2: y stores evict_first
+  kPolMixLoad = 16,   // tc_mix2: tile loads evict_first
+  kPolMixStore = 32,  // tc_mix2: A2 stores evict_last
+  kPolMixImg = 64,    // tc_mix2: Xh, O1 stores evict_first; G2, G1 stores evict_last
+  kPolWgLoad = 128    // tc_wgrad: operand loads evict_first
+};
+#ifdef AFNO_POLICY_EXPERIMENT
+__device__ int g_polmask = 255;
+#define POLMASK g_polmask
+#else
+constexpr int kPolMask = kPolWfStore | kPolWgLoad;   // measured: 0 -> 496 us per step, all -> 499, this choice -> 486
+#define POLMASK kPolMask
+#endif
+__device__ __forceinline__ uint64_t pol_first(int bit) { return (POLMASK & bit) ? l2_evict_first() : l2_evict_normal(); }
+__device__ __forceinline__ uint64_t pol_last(int bit) { return (POLMASK & bit) ? l2_evict_last() : l2_evict_normal(); }
+
 #ifdef AFNO_TRACE
 __device__ long long g_afno_trace[64 * 32];
 #define TR(t, slot) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (t) >= 40 && (t) < 72) g_afno_trace[((t) - 40) * 64 + (slot)] = clock64(); } while (0)
@@ -174,6 +196,7 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
   pdl_wait();
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
+  const uint64_t pol_stream = pol_first(kPolWfLoad), pol_keep = pol_last(kPolWfStore);
   // TMA producer (warp 7): tile it -> slot it % 6
   auto produce = [&](int it) {
     const int s = it % kWfSlots;
@@ -182,7 +205,8 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
     const int j = t % nb, bh = t / nb;
     mbar_expect_tx(&full[s], kW2Tile);
 #pragma unroll
-    for (int pn = 0; pn < 3; ++pn) tma_load3(aS + s * kW2Tile + pn * kPanel, &mapX, j * BS + pn * 32, 0, bh, &full[s]);
+    for (int pn = 0; pn < 3; ++pn)
+      tma_load3(aS + s * kW2Tile + pn * kPanel, &mapX, j * BS + pn * 32, 0, bh, &full[s], pol_stream);
   };
   if (warp == 7) {
     // the first ring of loads starts at once, under the load of the constant
@@ -257,7 +281,7 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
       fence_async_smem();
       asm volatile("bar.sync 1, 192;" ::: "memory");
       if (warp == 0 && elect_one()) {
-        tma_store5(&mapA1, 0, h, j, 0, b, aS + s * kW2Tile);
+        tma_store5(&mapA1, 0, h, j, 0, b, aS + s * kW2Tile, pol_keep);   // the next kernel reads A1
         bulk_commit();
         if (it > 0) {
           bulk_wait_read<1>();   // the previous tile's store has read its slot
@@ -313,6 +337,7 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
   pdl_wait();
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
+  const uint64_t pol_stream = pol_first(kPolWiLoad), pol_out = pol_first(kPolWiStore);
   // TMA producer (warp 6)
   auto produce = [&](int it) {
     const int s = it % kWiSlots;
@@ -323,12 +348,13 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
     mbar_expect_tx(&ofull[s], kW2Tile);
 #pragma unroll
     for (int pn = 0; pn < 6; ++pn)   // panel pn = ri * 3 + n -> K rows ri * 96.., N panel n
-      tma_load5(aO + s * kW2Tile + (pn % 3) * kPanel + (pn / 3) * (BS * 64), &mapA2, 0, pn, j * H + h, 0, b, &ofull[s]);
+      tma_load5(aO + s * kW2Tile + (pn % 3) * kPanel + (pn / 3) * (BS * 64), &mapA2, 0, pn, j * H + h, 0, b, &ofull[s], pol_stream);
     if (has_res) {
       if (it >= kWiSlots) mbar_wait(&rfree[s], par);  // the slot's previous store has read it
       mbar_expect_tx(&rfull[s], kW2Tile);
 #pragma unroll
-      for (int pn = 0; pn < 3; ++pn) tma_load3(aR + s * kW2Tile + pn * kPanel, &mapRes, j * BS + pn * 32, 0, bh, &rfull[s]);
+      for (int pn = 0; pn < 3; ++pn)
+        tma_load3(aR + s * kW2Tile + pn * kPanel, &mapRes, j * BS + pn * 32, 0, bh, &rfull[s], pol_stream);
     }
   };
   if (warp == 6) {
@@ -422,7 +448,7 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
       asm volatile("bar.sync 1, 192;" ::: "memory");
       if (warp == 0 && elect_one()) {
 #pragma unroll
-        for (int pn = 0; pn < 3; ++pn) tma_store3(&mapY, j * BS + pn * 32, 0, bh, aR + s * kW2Tile + pn * kPanel);
+        for (int pn = 0; pn < 3; ++pn) tma_store3(&mapY, j * BS + pn * 32, 0, bh, aR + s * kW2Tile + pn * kPanel, pol_out);
         bulk_commit();
         if (it > 0) {
           bulk_wait_read<1>();
@@ -482,8 +508,9 @@ constexpr uint32_t kMix2Smem = 2 * kDft2Bytes + 4 * kWBytes + 3 * kTileBuf; // 2
 constexpr uint32_t kSlot = 96;
 
 // bulk (async-proxy) store of a thread's own staged bytes: shared -> global, tracked by bulk groups
-__device__ __forceinline__ void bulk_store(void* dst, uint32_t src_smem, uint32_t bytes) {
-  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src_smem), "r"(bytes)
+__device__ __forceinline__ void bulk_store(void* dst, uint32_t src_smem, uint32_t bytes, uint64_t pol) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(dst), "r"(src_smem),
+               "r"(bytes), "l"(pol)
                : "memory");
   bulk_commit();
 }
@@ -710,19 +737,22 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
     // warp 7 lane 0 issues every copy (TMA tile loads in, bulk stores of the staged rows out); the other
     // two warps of this lane quarter have nothing to do
     const uint32_t aT = smem_u32(sT);
+    const uint64_t pol_stream = pol_first(kPolMixLoad), pol_keep = pol_last(kPolMixStore);
+    const uint64_t pol_img = SAVE ? pol_first(kPolMixImg) : pol_last(kPolMixImg);
     if (warp == 7 && lane == 0) {
       auto load = [&](int buf, const CUtensorMap* m, int i, uint64_t* full) {
         const int tile_id = (rtop - i * S) * p.nb + j;
         mbar_expect_tx(full, 6 * kInPanel);
 #pragma unroll
-        for (int pn = 0; pn < 6; ++pn) tma_load4(aT + buf * kTileBuf + pn * kInPanel, m, 0, pn, 0, tile_id, full);
+        for (int pn = 0; pn < 6; ++pn) tma_load4(aT + buf * kTileBuf + pn * kInPanel, m, 0, pn, 0, tile_id, full, pol_stream);
       };
       // tile k's output rows are staged in its buffer by the epilogue warps; they leave with one bulk copy
       // and the buffer is free once the copy has read it
       auto drain = [&](int k) {
         const int buf = k % 3;
         mbar_wait(&bars.sdone[buf], (uint32_t)((k / 3) & 1));
-        bulk_store(p.A2 + ((size_t)(rtop - k * S) * p.nb + j) * p.H * kA2Row, aT + buf * kTileBuf, (uint32_t)p.H * kOutStride);
+        bulk_store(p.A2 + ((size_t)(rtop - k * S) * p.nb + j) * p.H * kA2Row, aT + buf * kTileBuf, (uint32_t)p.H * kOutStride,
+                   pol_keep);   // the next kernel reads A2
         bulk_wait_read<0>();
       };
       if (!RECOMP) {
@@ -766,7 +796,9 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
         __nv_bfloat16* img = se == 0 ? p.Xh : se == 1 ? p.O1 : se == 3 ? p.G2 : p.G1;
         mbar_wait(&bars.imgfull[stream], cnt[stream] & 1u);
         ++cnt[stream];
-        bulk_store((uint8_t*)img + ((size_t)(rtop - i * S) * p.nb + j) * kTileBytes, aT + (i % 3) * kTileBuf, kTileBytes);
+        // Xh, O1 are read a whole kernel later: stream them out; G2, G1 are read by the next kernel
+        bulk_store((uint8_t*)img + ((size_t)(rtop - i * S) * p.nb + j) * kTileBytes, aT + (i % 3) * kTileBuf, kTileBytes,
+                   pol_img);
         bulk_wait_read<0>();
         mbar_arrive(&bars.imgfree[stream]);
       }
@@ -1043,9 +1075,10 @@ constexpr uint32_t kWgABytes = 16 * kWgASbo;                            // 24832
 constexpr uint32_t kWgStage = 2 * kWgABytes + kTileBytes;              // 86016
 constexpr uint32_t kWgSmem = 2 * kWgStage;                             // 172032
 
-__device__ __forceinline__ void bulk_copy(uint32_t dst_smem, const void* src, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst_smem),
-               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+__device__ __forceinline__ void bulk_copy(uint32_t dst_smem, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+                   dst_smem),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
                : "memory");
 }
 
@@ -1094,15 +1127,16 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
   if (warp == 0 && elect_one()) {
     // ---- producer: three bulk copies per tile (A re half, A im half, G), async proxy, no LSU ----
     constexpr uint32_t kHalfImg = 12 * kTileSbo;
+    const uint64_t pol_stream = pol_first(kPolWgLoad);
     for (int it = 0; it < nt; ++it) {
       const int b = it & 1, use = it >> 1;
       if (use > 0) mbar_wait(&empty[b], (uint32_t)((use - 1) & 1));
       const size_t off = ((size_t)(s + it * S) * nb + j) * kTileBytes;
       const uint32_t stage = smem_u32(smem) + b * kWgStage;
       mbar_expect_tx(&full[b], 2 * kHalfImg + kTileBytes);
-      bulk_copy(stage, (const uint8_t*)Aws + off, kHalfImg, &full[b]);
-      bulk_copy(stage + kWgABytes, (const uint8_t*)Aws + off + kHalfImg, kHalfImg, &full[b]);
-      bulk_copy(stage + 2 * kWgABytes, (const uint8_t*)Gws + off, kTileBytes, &full[b]);
+      bulk_copy(stage, (const uint8_t*)Aws + off, kHalfImg, &full[b], pol_stream);
+      bulk_copy(stage + kWgABytes, (const uint8_t*)Aws + off + kHalfImg, kHalfImg, &full[b], pol_stream);
+      bulk_copy(stage + 2 * kWgABytes, (const uint8_t*)Gws + off, kTileBytes, &full[b], pol_stream);
     }
   } else if (warp == 1 && elect_one()) {
     // ---- MMA issuer ----
@@ -1530,6 +1564,9 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
 extern "C" int afno_trace_read(long long* out) {
   return (int)cudaMemcpyFromSymbol(out, g_afno_trace, sizeof(long long) * 64 * 32);
 }
+#endif
+#ifdef AFNO_POLICY_EXPERIMENT
+extern "C" int afno_debug_set_policy(int mask) { return (int)cudaMemcpyToSymbol(g_polmask, &mask, sizeof(int)); }
 #endif
 #ifdef AFNO_TIMING
 extern "C" int afno_debug_read(long long* out) {

@@ -43,7 +43,7 @@ def _peaks():
                 source="fallback")
 
 
-def layer_work(B, H, W, C, nb, kept_modes):
+def layer_work(B, H, W, C, nb, kept_modes, ctx=True):
     """Algorithmic work of one fwd+bwd step (S5): compulsory HBM bytes and model MLP FLOPs."""
     act = B * H * W * C * 2                                  # one bf16 activation tensor
     params = 2 * (nb * (C // nb) ** 2 * 2 + C * 2) * 4       # w1,b1,w2,b2 fp32
@@ -53,7 +53,7 @@ def layer_work(B, H, W, C, nb, kept_modes):
     gemm = 2 * (2 * bs) * (2 * bs) * nb * kept_modes * B     # one complex block GEMM over all modes
     flops_fwd = 2 * gemm                                     # F3, F5
     flops_bwd_model = 4 * gemm                               # B4, B5, B6, B7
-    flops_bwd_exec = 6 * gemm                                # + recompute of F3, F5
+    flops_bwd_exec = (4 if ctx else 6) * gemm                # stateless bwd: + recompute of F3, F5
     return dict(bytes=bytes_fwd + bytes_bwd, flops_model=flops_fwd + flops_bwd_model,
                 flops_exec=flops_fwd + flops_bwd_exec)
 
@@ -263,7 +263,7 @@ def run_ours(args):
     Kh = max(1, min(wl.H // 2 + 1, int(np.floor(float(np.float32(wl.kept_fraction)) * (wl.H // 2 + 1)))))
     Kw = max(1, min(wl.W // 2 + 1, int(np.floor(float(np.float32(wl.kept_fraction)) * (wl.W // 2 + 1)))))
     kept_modes = (2 * Kh - 1 if Kh <= wl.H // 2 else wl.H) * Kw
-    work = layer_work(B, wl.H, wl.W, wl.C, wl.num_blocks, kept_modes)
+    work = layer_work(B, wl.H, wl.W, wl.C, wl.num_blocks, kept_modes, ctx)
     roofline = kernel_roofline(dom, dom_n, dom_ms, PROF_STEPS, work, peaks, clocks.summary(), B, wl, kept_modes, ctx)
     roofline["share_of_step"] = dom_ms / total_prof_ms if total_prof_ms > 0 else None
     roofline["kernels_ms_per_step"] = {k: round(v[1] / PROF_STEPS, 4) for k, v in sorted(prof.items())}
@@ -366,7 +366,7 @@ def kernel_work(name, B, wl, kept_modes, ctx=True):
 
 def measured_traffic(name):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture."""
-    path = os.path.join(ROOT, "profiles", "r1d_dram_traffic.json")
+    path = os.path.join(ROOT, "profiles", "r1e_dram_traffic.json")
     try:
         return json.load(open(path)).get(name)
     except Exception:

@@ -6,10 +6,16 @@
 // with fp32 accumulation against constant DFT matrices (S5 gives the arithmetic and
 // the measured error).  The layer becomes three GEMM-chain kernels:
 //
-//   tc_wdft_fwd  [F1, B2]   per (b, h, block j):  A1[(ri,kw), c] = Fw[(ri,kw), w] * x[w, c]
-//   tc_mix_fwd   [F2-F7]    per (b, kw, block j), everything on chip in tensor memory:
+//   tc_wdft_fwd2 [F1, B2]   per (b, h, block j):  A1[(ri,kw), c] = Fw[(ri,kw), w] * x[w, c]
+//   tc_mix2      [F2-F7]    per (b, kw, block j), everything on chip in tensor memory:
 //                            Xh = Fh * A1  ->  relu(Xh W1 + b1)  ->  shrink(. W2 + b2)  ->  Fh^H * Z
-//   tc_wdft_inv  [F8, F9, B8] per (b, h, block j): y[w, c] = x[w, c] + Gw[w, (ri,kw)] * A2[(ri,kw), c]
+//                [B1-B8]    the same chain run for the gradient (modes Bwd / BwdCtx), with
+//   tc_wgrad     [B4, B6]   dW, db as a split-K GEMM over the mode rows
+//   tc_wdft_inv2 [F8, F9, B8] per (b, h, block j): y[w, c] = x[w, c] + Gw[w, (ri,kw)] * A2[(ri,kw), c]
+//
+// All global traffic of these kernels moves through the copy engines (tensor-map TMA loads / stores and
+// bulk copies, each with an L2 eviction policy); the kernels of a call are chained by programmatic
+// dependent launch.
 //
 // Complex arithmetic runs as real GEMMs on separate (re | im) column halves using the
 // instruction descriptor's negate bit for the minus signs, so only W_re and W_im (not the 2x2
@@ -42,8 +48,9 @@ constexpr uint32_t kOutStride = 2 * kA2Row;           // 400
 // shared-memory operand geometry (bytes), see tc_common.cuh for the layout formulas
 constexpr uint32_t kWLbo = 1536, kWSbo = 128;       // weights: K-major B [96 x 96], order [k/8][n/8]
 constexpr uint32_t kWBytes = BS * BS * 2;            // 18432
-// mode tile: MN-major B [K=96 rows][N=192]; the 16-byte pad on the chunk stride keeps cp.async
-// writes of consecutive chunks of one row (the coalesced global order) bank-conflict-free
+// mode tile (no-swizzle layout of Z / GX and of the operand images): MN-major B [K=96 rows][N=192],
+// chunk stride padded by 16 bytes (rows of one chunk are 16 bytes apart: a warp's 32 rows store 512
+// contiguous bytes, conflict-free)
 constexpr uint32_t kTileLbo = 128, kTileSbo = 1536 + 16;
 constexpr uint32_t kTileBytes = (NT / 8) * kTileSbo; // 37248
 // ---- weight preparation: fp32 [nb][96][96][2] -> bf16 K-major interleaved operands --------------
@@ -494,10 +501,12 @@ struct MixParams {
 //     frees slot 3t+1; by the time S_(t+2) needs its two slots, 3t+1 and 3t+2 (the A operand of
 //     S_(t+1), read by the in-order tensor pipe before S_(t+2) writes) are free: 480 columns.
 //   * accumulator rows >= 96 hold nothing (H <= 96), so the warps of TMEM lane quarter 3
-//     (warp % 4 == 3) are the control warp and the three loader warps; each of lane quarters 0..2
-//     has four epilogue warps, one per 48-column quarter (re lo, re hi, im lo, im hi).
-//   * three tile buffers: tile i lives in buffer i % 3 (input tile, then the B operand of the
-//     inverse transform); backward: x tile, then the gradient tile, then GX.
+//     (warp % 4 == 3) are the control warp (3), the copy warp (7), the image warp (11) and a spare;
+//     each of lane quarters 0..2 has four epilogue warps, one per 48-column quarter (re lo, re hi,
+//     im lo, im hi).
+//   * three tile buffers: tile i lives in buffer i % 3: the input tile (six 64B-swizzled TMA panels),
+//     then staged operand images (FwdSave / BwdCtx), then the B operand of the inverse transform, then
+//     the staged output rows; stateless backward: x tile, then the gradient tile, then GX.
 // Every CTA works on ONE channel block j (grid = nb * S), so the weights are loaded once.
 constexpr int kMix2Threads = 512;
 constexpr uint32_t kDft2Lbo = 1536, kDft2Sbo = 128;  // Ch / Sh: K-major A, 96 stored rows, order [k/8][m/8 < 12]

@@ -1,5 +1,5 @@
 // tcgen05 (5th-generation tensor core) path of the AFNO spectral layer for bf16 activations,
-// 96-wide channel blocks, H <= 96 (90 in FourCastNet's 8x8 patch grid) and W <= 192.
+// 96-wide channel blocks, H <= 96 (90 in FourCastNet's 8x8 patch grid) and W <= 190 (W/2+1 <= 96 bins).
 //
 // On B200 the tensor pipe is ~30x the fp32 ALU pipe, while a dense DFT of length 90 / 180 costs
 // only ~20x the FLOPs of an FFT, so every transform of the layer is computed as a bf16 GEMM

@@ -128,19 +128,39 @@ def preactivation_scales(cfg, dump, w1, b1, w2, b2):
     return s1, s2
 
 
-def mask_flip_report(oracle_dump, gpu_mask1, gpu_mask2, lam, tau1, tau2):
+def kept_modes(cfg):
+    """Boolean [H, Wh]: the kept set of DESIGN.md S3 readings A7 / A8 (restated from the definition)."""
+    f = float(np.float32(cfg.kept_fraction))
+    hh, wh = cfg.H // 2 + 1, cfg.W // 2 + 1
+    Kh = max(1, min(hh, int(np.floor(f * hh))))
+    Kw = max(1, min(wh, int(np.floor(f * wh))))
+    r = np.arange(cfg.H)
+    kappa = np.where(r <= cfg.H // 2, r, cfg.H - r)
+    return (kappa < Kh)[:, None] & (np.arange(wh) < Kw)[None, :]
+
+
+def mask_flip_report(oracle_dump, gpu_mask1, gpu_mask2, lam, tau1, tau2, kept=None):
     """Fraction of flipped masks and whether every flip is justified: the oracle's fp64
     pre-activation lies within tau of the threshold (S3 P-bwd (ii)).  tau1 / tau2 are
-    arrays broadcastable to the masks' shapes without the trailing (re, im) axis."""
+    arrays broadcastable to the masks' shapes without the trailing (re, im) axis.  Only KEPT modes
+    count (`kept`: boolean [H, Wh]): outside the kept set Z = 0 exactly (reading A9), no gradient
+    passes, and the masks are not defined (a kernel may leave them unset)."""
     p1, p2 = oracle_dump["p1"], oracle_dump["p2"]
     z = oracle_dump["z"]
     o1 = np.stack([p1.real > 0, p1.imag > 0], -1)
     o2 = np.stack([z.real != 0, z.imag != 0], -1)
     f1 = o1 != gpu_mask1.astype(bool)
     f2 = o2 != gpu_mask2.astype(bool)
+    if kept is not None:
+        k = np.asarray(kept, dtype=bool)[None, :, :, None, None]
+        f1 = f1 & k
+        f2 = f2 & k
+        norm = float(k.mean())
+    else:
+        norm = 1.0
     d1 = np.abs(np.stack([p1.real, p1.imag], -1)) / np.asarray(tau1)[..., None]
     d2 = np.abs(np.abs(np.stack([p2.real, p2.imag], -1)) - lam) / np.asarray(tau2)[..., None]
     worst1 = float(d1[f1].max()) if f1.any() else 0.0
     worst2 = float(d2[f2].max()) if f2.any() else 0.0
-    return dict(flip1=float(f1.mean()), flip2=float(f2.mean()), worst1=worst1, worst2=worst2,
+    return dict(flip1=float(f1.mean()) / norm, flip2=float(f2.mean()) / norm, worst1=worst1, worst2=worst2,
                 justified=(worst1 <= 1.0 and worst2 <= 1.0))

@@ -51,7 +51,8 @@ def _check_backward(oracle, desc, data, label=""):
     tol = _tol(desc)
     s1, s2 = parity.preactivation_scales(cfg, raw["dump"], data["w1"].astype(np.float64), data["b1"].astype(np.float64),
                                          data["w2"].astype(np.float64), data["b2"].astype(np.float64))
-    rep = parity.mask_flip_report(raw["dump"], g["mask1"], g["mask2"], cfg.lam, tol * s1, tol * s2)
+    rep = parity.mask_flip_report(raw["dump"], g["mask1"], g["mask2"], cfg.lam, tol * s1, tol * s2,
+                                  kept=parity.kept_modes(cfg))
     print(f"[bwd {label}] mask flips: relu {rep['flip1']:.2e} shrink {rep['flip2']:.2e}; worst flipped "
           f"|pre-activation - threshold| / (tol * row scale) = {rep['worst1']:.2f} / {rep['worst2']:.2f} (must be <= 1)")
     for k in ("dx", "dw1", "db1", "dw2", "db2"):
@@ -154,6 +155,38 @@ def test_bf16_forward_full_size(oracle, name, f):
 def test_bf16_forward_backward_full_size(oracle):
     wl = inputs.WORKLOADS["fcn_b4_bwd"]
     _check_backward(oracle, parity.desc_for(wl), inputs.make_inputs(wl), label="configs[4] B=4")
+
+
+@pytest.mark.parametrize("B,H,W,C,nb,f", [
+    (3, 30, 60, 96, 1, 1.0),      # one block, short rows and columns (TMA zero-fill in H and W), odd batch
+    (1, 96, 180, 192, 2, 1.0),    # H = 96: no padding rows in the mode tiles; two blocks
+    (2, 18, 36, 288, 3, 0.5),     # truncated spectrum on a small grid, three blocks
+    (5, 40, 100, 96, 1, 0.75),    # W/2+1 = 51 bins, Kw = 38, five samples
+])
+def test_bf16_tcgen05_other_shapes(oracle, B, H, W, C, nb, f):
+    """The tcgen05 path away from the headline shape: ragged tails in every tiled dimension, forward
+    and (mask-consistent) backward against the oracle, plus saved-context == stateless bit for bit."""
+    import torch
+    wl = inputs.Workload(4, f"{H}x{W}x{C} bf16 B={B}", B, H, W, C, nb, 1, 0.01, f, "bf16", True, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert binding.afno_spectral_path(desc) == "tcgen05-bf16"
+    _check_forward(oracle, desc, data, label=wl.name)
+    g = _check_backward(oracle, desc, data, label=wl.name)
+    layer = parity.GpuLayer(desc)
+    d_save = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_SAVE_CONTEXT})
+    d_use = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_USE_CONTEXT})
+    ws = torch.empty(binding.afno_spectral_workspace_bytes(desc, True), dtype=torch.uint8, device="cuda")
+    tx, tdy = parity.to_device_act(data["x"], True), parity.to_device_act(data["dy"], True)
+    ty, tdx = torch.empty_like(tx), torch.empty_like(tx)
+    p = layer.params(data["w1"], data["b1"], data["w2"], data["b2"])
+    gr = [torch.zeros_like(t) for t in p]
+    binding.afno_spectral_fwd(d_save, tx, *p, ty, ws)
+    binding.afno_spectral_bwd(d_use, tx, tdy, *p, tdx, *gr, ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(parity.from_device_act(tdx), g["dx"])
+    for t, k in zip(gr, ("dw1", "db1", "dw2", "db2")):
+        assert np.array_equal(t.cpu().numpy(), g[k]), k
 
 
 def test_bf16_force_fp32_math_flag(oracle):
@@ -275,7 +308,8 @@ def test_saved_context_step_vs_oracle(oracle):
     ref = oracle.backward(cfg, *args, mask1=mask1, mask2=mask2)
     raw = oracle.backward(cfg, *args, dump=True)
     s1, s2 = parity.preactivation_scales(cfg, raw["dump"], *(data[k].astype(np.float64) for k in ("w1", "b1", "w2", "b2")))
-    rep = parity.mask_flip_report(raw["dump"], mask1, mask2, cfg.lam, TOL_BF16 * s1, TOL_BF16 * s2)
+    rep = parity.mask_flip_report(raw["dump"], mask1, mask2, cfg.lam, TOL_BF16 * s1, TOL_BF16 * s2,
+                                  kept=parity.kept_modes(cfg))
     got = dict(dx=parity.from_device_act(tdx), dw1=g[0].cpu().numpy(), db1=g[1].cpu().numpy(),
                dw2=g[2].cpu().numpy(), db2=g[3].cpu().numpy())
     print(f"[ctx step] rel_l2(y)={ey:.3e} flips relu {rep['flip1']:.2e} shrink {rep['flip2']:.2e} "

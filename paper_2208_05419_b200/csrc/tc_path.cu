@@ -142,22 +142,30 @@ __device__ long long g_afno_dbg[128];
 constexpr int kW2Threads = 256;
 constexpr uint32_t kPanel = 192 * 64;                      // 12288: one [192 x 32] bf16 panel
 constexpr uint32_t kW2Tile = 3 * kPanel;                   // 36864: a [192 x 96] tile
-constexpr uint32_t kCImgWords = 2 * 128 * (WP / 2);        // constant image: [half][row 0..127][96 words = K pairs]
+constexpr uint32_t kCImgWords = 2 * 128 * (WP / 2);        // constant image: [half][6 column groups][row 0..127][16 words = K pairs]
 constexpr uint32_t kCCols = WP;                            // TMEM columns of the constant: half a at a * 96
 constexpr int kWfSlots = 6;
 constexpr uint32_t kWfSmem = kWfSlots * kW2Tile + 1024;    // 222208
 constexpr int kWiSlots = 3;
 constexpr uint32_t kWiSmem = 2 * kWiSlots * kW2Tile + 1024;
 
-// constant matrix image (global, [half][128 rows][96 words]) -> tensor memory columns [0, 192); warps 0..3
-// load half 0, warps 4..7 half 1 (lane quarter = warp % 4); all of a thread's loads are in flight at once
+// constant matrix image (global) -> tensor memory columns [0, 192); warps 0..3 load half 0, warps 4..7
+// half 1 (lane quarter = warp % 4).  The image is stored [half][column group of 16][row][16 words], so a
+// warp's 32 rows of one group are 2 KB contiguous (coalesced: every CTA of the grid reads the same 98 KB at
+// the same moment); all of a thread's loads are in flight at once.
+__device__ __forceinline__ size_t cimg_word(int a, int row, int word) {
+  return (((size_t)a * 6 + word / 16) * 128 + row) * 16 + word % 16;
+}
 __device__ __forceinline__ void load_const_tmem(uint32_t tmem, const uint32_t* __restrict__ img, int warp, int lane) {
   const int a = warp >> 2, q4 = warp & 3;
-  const uint4* src = (const uint4*)(img + ((size_t)a * 128 + q4 * 32 + lane) * (WP / 2));
   const uint32_t dst = tmem + ((uint32_t)(q4 * 32) << 16) + a * (WP / 2);
   uint4 t[24];
 #pragma unroll
-  for (int q = 0; q < 24; ++q) t[q] = __ldg(src + q);
+  for (int c = 0; c < 6; ++c) {
+    const uint4* src = (const uint4*)(img + cimg_word(a, q4 * 32 + lane, 16 * c));
+#pragma unroll
+    for (int q = 0; q < 4; ++q) t[4 * c + q] = __ldg(src + q);
+  }
 #pragma unroll
   for (int c = 0; c < 6; ++c) {
     uint32_t v[16];
@@ -1364,12 +1372,15 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
       dft2[off] = host_bf16(cos(a) * s);
       dft2[kDft2Bytes / 2 + off] = host_bf16(sin(a) * s);
     }
-  // W-direction constants as tensor-memory A operands: [half a][row m < 128][96 words], word q of a row =
-  // (k = 2q low half, k = 2q + 1 high half):
+  // W-direction constants as tensor-memory A operands: logical [half a][row m < 128][96 words], word q of a
+  // row = (k = 2q low half, k = 2q + 1 high half), stored in the order of cimg_word():
   //   Fw half ri: (m = kw, k = w)                  = {cos, -sin}(2 pi kw w / W) / sqrt(W)          [x alpha_kw]
   //   Gw half a : (m = w - 128 a, k = ri * 96 + kw) = alpha_kw {cos, -sin}(...) / sqrt(W)          [or alpha = 1]
   std::vector<uint16_t> fw(2 * kCImgWords, 0), fwa(2 * kCImgWords, 0), gw(2 * kCImgWords, 0), gw1(2 * kCImgWords, 0);
-  auto aoff = [](int a, int m, int k) { return ((size_t)a * 128 + m) * WP + k; };
+  auto aoff = [](int a, int m, int k) {   // 16-bit element index: word k / 2 of row m, half k % 2
+    const int word = k / 2;
+    return ((((size_t)a * 6 + word / 16) * 128 + m) * 16 + word % 16) * 2 + k % 2;
+  };
   for (int kw = 0; kw < Wh; ++kw)
     for (int w = 0; w < W; ++w) {
       const double a = two_pi * (double)((long)kw * w % W) / (double)W, s = 1.0 / sqrt((double)W);

@@ -121,9 +121,12 @@ __device__ long long g_afno_trace[64 * 32];
 __device__ long long g_afno_dbg[128];
 #define DBG_T0() long long dbg_t = clock64()
 #define DBG_ACC(slot) do { long long n_ = clock64(); dbg_acc[slot] += n_ - dbg_t; dbg_t = n_; } while (0)
+// timeline of CTA 0: wall-clock (ns) at a few points of a kernel
+#define TL(slot) do { if (blockIdx.x == 0 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_afno_dbg[slot] = (long long)t_; } } while (0)
 #else
 #define DBG_T0()
 #define DBG_ACC(slot)
+#define TL(slot)
 #endif
 
 // ---- F1 / B2 and F8 + F9 / B8: the W-direction transforms, all global traffic through bulk tensor copies --
@@ -182,6 +185,7 @@ __global__ void __launch_bounds__(kW2Threads, 1)
 tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapA1,
              const uint32_t* __restrict__ Fimg, int ntiles, int nb, int H, int Kw) {
   extern __shared__ uint8_t smem_raw[];
+  TL(0);
   __shared__ __align__(8) uint64_t full[kWfSlots], sfree[kWfSlots], accfull[2], accempty[2];
   __shared__ uint32_t tmem_slot;
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -207,8 +211,11 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
+  TL(1);
   load_const_tmem(tmem, Fimg, warp, lane);   // plan constant: loads under the previous kernel's tail
+  TL(2);
   pdl_wait();
+  TL(3);
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
   const uint64_t pol_stream = pol_first(kPolWfLoad), pol_keep = pol_last(kPolWfStore);
@@ -310,6 +317,7 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
   }
   tc_fence_before();
   __syncthreads();
+  TL(4);
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
@@ -319,6 +327,7 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
              const __grid_constant__ CUtensorMap mapY, const uint32_t* __restrict__ Gimg, int ntiles, int nb, int H, int W,
              int has_res) {
   extern __shared__ uint8_t smem_raw[];
+  TL(8);
   __shared__ __align__(8) uint64_t ofull[kWiSlots], ofree[kWiSlots], rfull[kWiSlots], rfree[kWiSlots], accfull[2], accempty[2];
   __shared__ uint32_t tmem_slot;
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -348,8 +357,11 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
+  TL(9);
   load_const_tmem(tmem, Gimg, warp, lane);   // plan constant: loads under the previous kernel's tail
+  TL(10);
   pdl_wait();
+  TL(11);
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
   const uint64_t pol_stream = pol_first(kPolWiLoad), pol_out = pol_first(kPolWiStore);
@@ -477,6 +489,7 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
   }
   tc_fence_before();
   __syncthreads();
+  TL(12);
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
@@ -695,6 +708,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
   // that buffer with the gradient tile meanwhile and stores the images with plain vector stores.
   constexpr bool STAGED = SAVE || CTXB;
   extern __shared__ __align__(1024) uint8_t smem[];
+  TL(BACKWARD ? 24 : 16);
   __shared__ Mix2Bars bars;
   __shared__ uint32_t tmem_slot;
   __shared__ __align__(16) float sBias[2 * NT];
@@ -715,7 +729,9 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
   pdl_launch_dependents();
   for (uint32_t i = tid; i < 3 * kTileBuf / 16; i += kMix2Threads) ((uint4*)sT)[i] = make_uint4(0, 0, 0, 0);
   for (uint32_t i = tid; i < 2 * kDft2Bytes / 16; i += kMix2Threads) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
+  TL(BACKWARD ? 25 : 17);
   pdl_wait();   // the weight images below are written by an earlier kernel of the chain
+  TL(BACKWARD ? 26 : 18);
   {
     const uint8_t* wsrc = p.wprep + (size_t)j * 4 * kWBytes;
     for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMix2Threads) cp_async16(smem_u32(sW) + i * 16, wsrc + (size_t)i * 16);
@@ -743,6 +759,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
+  TL(BACKWARD ? 27 : 19);
   // Stream 1 runs kLag stages behind stream 0, so tiles finish (and buffers become free) at
   // regular intervals and a transform stage of one stream overlaps an MLP stage of the other.
   constexpr int kLag = NS / 2;
@@ -1080,6 +1097,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
   }
   tc_fence_before();
   __syncthreads();
+  TL(BACKWARD ? 28 : 20);
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
@@ -1091,6 +1109,12 @@ constexpr uint32_t kWgALbo = 128, kWgASbo = 1536 + 16;                  // MN-ma
 constexpr uint32_t kWgABytes = 16 * kWgASbo;                            // 24832
 constexpr uint32_t kWgStage = 2 * kWgABytes + kTileBytes;              // 86016
 constexpr uint32_t kWgSmem = 2 * kWgStage;                             // 172032
+// partial sums of one CTA: rows 0..96 of D_re (96 channels + the db row) then rows 0..95 of D_im, fp32,
+// row pitch 196 floats (784 bytes: a warp's 32 rows staged in shared memory hit distinct bank groups)
+constexpr int kWgPitch = NT + 4;
+constexpr int kWgRowsRe = BS + 1, kWgRowsIm = BS;
+constexpr uint32_t kWgPartFloats = (kWgRowsRe + kWgRowsIm) * kWgPitch;   // 37828 floats = 151312 bytes
+static_assert(kWgPartFloats * 4 <= kWgSmem, "partial sums are staged in the operand stages");
 
 __device__ __forceinline__ void bulk_copy(uint32_t dst_smem, const void* src, uint32_t bytes, uint64_t* bar, uint64_t pol) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
@@ -1106,6 +1130,7 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
          const __nv_bfloat16* __restrict__ A_l1, const __nv_bfloat16* __restrict__ G_l1, float* __restrict__ part,
          int BKw, int H, int nb, int S) {
   extern __shared__ __align__(1024) uint8_t smem[];
+  TL(32);
   __shared__ __align__(8) uint64_t full[2], empty[2], done;
   __shared__ uint32_t tmem_slot;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -1134,7 +1159,9 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  TL(33);
   pdl_wait();
+  TL(34);
   const uint32_t tmem = tmem_slot;
   const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
   const uint32_t Dre = tmem, Dim = tmem + 256;
@@ -1174,29 +1201,44 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
     mma_commit(&done);
   }
   __syncwarp();
-  float* dst = part + ((size_t)blockIdx.x * 2) * 128 * NT + (size_t)tid * NT;
+  // Partial sums: accumulator rows -> shared memory (the operand stages are free: every MMA has
+  // completed) -> ONE bulk store per CTA.  Row-strided vector stores straight to global memory took 11 us.
+  float* stage = (float*)smem;
   if (nt > 0) {
     mbar_wait(&done, 0u);
+    TL(35);
     tc_fence_after();
 #pragma unroll 1
-    for (int acc = 0; acc < 2; ++acc)
+    for (int acc = 0; acc < 2; ++acc) {
+      const int rows = acc ? kWgRowsIm : kWgRowsRe;
+      if (warp * 32 < rows) {   // warp-uniform: tcgen05.ld is a warp-wide instruction
+        float* srow = stage + (size_t)(acc * kWgRowsRe + tid) * kWgPitch;
 #pragma unroll 1
-      for (int c0 = 0; c0 < NT; c0 += 32) {
-        uint32_t v[32];
-        tmem_ld32((acc ? Dim : Dre) + lane_base + c0, v);
-        tmem_wait_ld();
+        for (int c0 = 0; c0 < NT; c0 += 32) {
+          uint32_t v[32];
+          tmem_ld32((acc ? Dim : Dre) + lane_base + c0, v);
+          tmem_wait_ld();
+          if (tid < rows) {
 #pragma unroll
-        for (int q = 0; q < 32; q += 4)
-          *(float4*)(dst + (size_t)acc * 128 * NT + c0 + q) =
-              make_float4(__uint_as_float(v[q]), __uint_as_float(v[q + 1]), __uint_as_float(v[q + 2]),
-                          __uint_as_float(v[q + 3]));
+            for (int q = 0; q < 32; q += 4)
+              *(float4*)(srow + c0 + q) = make_float4(__uint_as_float(v[q]), __uint_as_float(v[q + 1]),
+                                                      __uint_as_float(v[q + 2]), __uint_as_float(v[q + 3]));
+          }
+        }
       }
+    }
   } else {
-    for (int acc = 0; acc < 2; ++acc)
-      for (int c0 = 0; c0 < NT; c0 += 4) *(float4*)(dst + (size_t)acc * 128 * NT + c0) = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (uint32_t i = tid; i < kWgPartFloats / 4; i += 128) ((float4*)stage)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  fence_async_smem();
+  __syncthreads();
+  if (tid == 0) {
+    bulk_store(part + (size_t)blockIdx.x * kWgPartFloats, smem_u32(smem), kWgPartFloats * 4, l2_evict_normal());
+    bulk_wait<0>();
   }
   tc_fence_before();
   __syncthreads();
+  TL(36);
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
@@ -1209,16 +1251,16 @@ __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __rest
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const int nW = nb * BS * BS;
   const int layer = blockIdx.y;
-  part += (size_t)layer * nb * S * 2 * 128 * NT;
+  part += (size_t)layer * nb * S * kWgPartFloats;
   float2* dW = layer ? dW1 : dW2;
   float2* dB = layer ? dB1 : dB2;
   if (idx < nW) {
     const int o = idx % BS, i = (idx / BS) % BS, j = idx / (BS * BS);
     float2 acc = accumulate ? dW[idx] : make_float2(0.f, 0.f);
     for (int s = 0; s < S; ++s) {
-      const float* P = part + ((size_t)(j * S + s) * 2) * 128 * NT;
-      const float* Pre = P + (size_t)i * NT;
-      const float* Pim = P + (size_t)128 * NT + (size_t)i * NT;
+      const float* P = part + (size_t)(j * S + s) * kWgPartFloats;
+      const float* Pre = P + (size_t)i * kWgPitch;
+      const float* Pim = P + (size_t)(kWgRowsRe + i) * kWgPitch;
       acc.x += Pre[o] + Pim[BS + o];
       acc.y += Pre[BS + o] - Pim[o];
     }
@@ -1227,7 +1269,7 @@ __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __rest
     const int k = idx - nW, o = k % BS, j = k / BS;
     float2 acc = accumulate ? dB[k] : make_float2(0.f, 0.f);
     for (int s = 0; s < S; ++s) {
-      const float* P = part + ((size_t)(j * S + s) * 2) * 128 * NT + (size_t)96 * NT;
+      const float* P = part + (size_t)(j * S + s) * kWgPartFloats + (size_t)BS * kWgPitch;
       acc.x += P[o];
       acc.y += P[BS + o];
     }
@@ -1348,7 +1390,7 @@ TcWs tc_carve(const Geometry& g, bool backward, char* base) {
     if (S < 1) S = 1;
     if (S > g.B * g.Kw) S = g.B * g.Kw;
     w.S = S;
-    w.part = (float*)take((size_t)2 * g.nb * S * 2 * 128 * NT * sizeof(float));
+    w.part = (float*)take((size_t)2 * g.nb * S * kWgPartFloats * sizeof(float));
   }
   w.total = off;
   return w;

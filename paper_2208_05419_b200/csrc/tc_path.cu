@@ -121,12 +121,16 @@ __device__ long long g_afno_trace[64 * 32];
 __device__ long long g_afno_dbg[128];
 #define DBG_T0() long long dbg_t = clock64()
 #define DBG_ACC(slot) do { long long n_ = clock64(); dbg_acc[slot] += n_ - dbg_t; dbg_t = n_; } while (0)
+// per-CTA start / end wall-clock (ns) of the last launch of kernel family k (load balance of the static tile schedule)
+__device__ long long g_afno_span[5][160][2];
+#define SPAN(k, e) do { if (threadIdx.x == 0 && blockIdx.x < 160) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_afno_span[k][blockIdx.x][e] = (long long)t_; } } while (0)
 // timeline of CTA 0: wall-clock (ns) at a few points of a kernel
 #define TL(slot) do { if (blockIdx.x == 0 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_afno_dbg[slot] = (long long)t_; } } while (0)
 #else
 #define DBG_T0()
 #define DBG_ACC(slot)
 #define TL(slot)
+#define SPAN(k, e)
 #endif
 
 // ---- F1 / B2 and F8 + F9 / B8: the W-direction transforms, all global traffic through bulk tensor copies --
@@ -186,6 +190,7 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
              const uint32_t* __restrict__ Fimg, int ntiles, int nb, int H, int Kw) {
   extern __shared__ uint8_t smem_raw[];
   TL(0);
+  SPAN(0, 0);
   __shared__ __align__(8) uint64_t full[kWfSlots], sfree[kWfSlots], accfull[2], accempty[2];
   __shared__ uint32_t tmem_slot;
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -318,6 +323,7 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
   tc_fence_before();
   __syncthreads();
   TL(4);
+  SPAN(0, 1);
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
@@ -328,6 +334,7 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
              int has_res) {
   extern __shared__ uint8_t smem_raw[];
   TL(8);
+  SPAN(1, 0);
   __shared__ __align__(8) uint64_t ofull[kWiSlots], ofree[kWiSlots], rfull[kWiSlots], rfree[kWiSlots], accfull[2], accempty[2];
   __shared__ uint32_t tmem_slot;
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -490,6 +497,7 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
   tc_fence_before();
   __syncthreads();
   TL(12);
+  SPAN(1, 1);
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
@@ -709,6 +717,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
   constexpr bool STAGED = SAVE || CTXB;
   extern __shared__ __align__(1024) uint8_t smem[];
   TL(BACKWARD ? 24 : 16);
+  SPAN(BACKWARD ? 3 : 2, 0);
   __shared__ Mix2Bars bars;
   __shared__ uint32_t tmem_slot;
   __shared__ __align__(16) float sBias[2 * NT];
@@ -718,26 +727,45 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
   uint8_t* sW = smem + 2 * kDft2Bytes;
   uint8_t* sT = sW + 4 * kWBytes;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int j = blockIdx.x / S, s0 = blockIdx.x - j * S;
   const int BKw = p.B * p.Kw;
-  const int n = s0 < BKw ? (BKw - s0 + S - 1) / S : 0;   // tiles of this CTA
-  // Tile i of this CTA is (b, kw) pair rem = BKw - 1 - (s0 + i * S): the tiles run from the LAST sample
-  // to the first.  The W-direction kernels run from the first sample to the last, so this kernel starts
-  // on the part of A1 its producer wrote last (still in the 126 MB L2) and finishes with the part of A2
-  // its consumer reads first.
-  const int rtop = BKw - 1 - s0;
+  // Work split.  The first nb * S CTAs are "regular": CTA (j, s0) of block j takes the (b, kw) pairs
+  // s0, s0 + S, ...  If the grid has spare CTAs beyond those (148 SMs against 8 x 18), the regular CTAs
+  // stop at the largest multiple of S, so that each has the SAME, even number of tiles (tiles run in
+  // pairs), and spare CTA k takes the few left-over pairs of blocks k, k + nspare, ..., one block
+  // ("segment") after the other, reloading the weights in between.
+  const int nreg = p.nb * S, nspare = (int)gridDim.x - nreg;
+  const bool spare = (int)blockIdx.x >= nreg;
+  const int main_tiles = nspare > 0 ? (BKw / S) * S : BKw;
+  const int nseg = spare ? (p.nb - ((int)blockIdx.x - nreg) + nspare - 1) / nspare : 1;
   pdl_launch_dependents();
   for (uint32_t i = tid; i < 3 * kTileBuf / 16; i += kMix2Threads) ((uint4*)sT)[i] = make_uint4(0, 0, 0, 0);
   for (uint32_t i = tid; i < 2 * kDft2Bytes / 16; i += kMix2Threads) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
   TL(BACKWARD ? 25 : 17);
   pdl_wait();   // the weight images below are written by an earlier kernel of the chain
   TL(BACKWARD ? 26 : 18);
+  if (warp == 0) tmem_alloc<512>(&tmem_slot);
+#pragma unroll 1
+  for (int seg = 0; seg < nseg; ++seg) {
+  const int j = spare ? ((int)blockIdx.x - nreg) + seg * nspare : (int)blockIdx.x / S;
+  const int s0 = spare ? main_tiles : (int)blockIdx.x - j * S;
+  const int step = spare ? 1 : S;
+  const int n = s0 < (spare ? BKw : main_tiles) ? ((spare ? BKw : main_tiles) - s0 + step - 1) / step : 0;   // tiles of this segment
+  // Tile i is (b, kw) pair rem = BKw - 1 - (s0 + i * step): the tiles run from the LAST sample to the
+  // first.  The W-direction kernels run from the first sample to the last, so this kernel starts on the
+  // part of A1 its producer wrote last (still in the 126 MB L2) and finishes with the part of A2 its
+  // consumer reads first.
+  const int rtop = BKw - 1 - s0;
   {
     const uint8_t* wsrc = p.wprep + (size_t)j * 4 * kWBytes;
     for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMix2Threads) cp_async16(smem_u32(sW) + i * 16, wsrc + (size_t)i * 16);
   }
   for (int i = tid; i < 2 * NT; i += kMix2Threads) sBias[i] = p.bprep[(size_t)j * 2 * NT + i];
   if (tid == 0) {
+    if (seg > 0) {   // every barrier is idle (the segment ended with a CTA-wide sync): start over
+      uint64_t* all = (uint64_t*)&bars;
+      for (uint32_t q = 0; q < sizeof(Mix2Bars) / 8; ++q)
+        asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(all + q)) : "memory");
+    }
     for (int q = 0; q < 2; ++q) {
       mbar_init(&bars.dfull[q], 1);
       mbar_init(&bars.edone[q], 12);
@@ -752,7 +780,6 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
     }
     mbar_init_fence();
   }
-  if (warp == 0) tmem_alloc<512>(&tmem_slot);
   cp_async_wait_all();
   fence_async_smem();
   tc_fence_before();
@@ -775,7 +802,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
     const uint64_t pol_img = SAVE ? pol_first(kPolMixImg) : pol_last(kPolMixImg);
     if (warp == 7 && lane == 0) {
       auto load = [&](int buf, const CUtensorMap* m, int i, uint64_t* full) {
-        const int tile_id = (rtop - i * S) * p.nb + j;
+        const int tile_id = (rtop - i * step) * p.nb + j;
         mbar_expect_tx(full, 6 * kInPanel);
 #pragma unroll
         for (int pn = 0; pn < 6; ++pn) tma_load4(aT + buf * kTileBuf + pn * kInPanel, m, 0, pn, 0, tile_id, full, pol_stream);
@@ -785,7 +812,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
       auto drain = [&](int k) {
         const int buf = k % 3;
         mbar_wait(&bars.sdone[buf], (uint32_t)((k / 3) & 1));
-        bulk_store(p.A2 + ((size_t)(rtop - k * S) * p.nb + j) * p.H * kA2Row, aT + buf * kTileBuf, (uint32_t)p.H * kOutStride,
+        bulk_store(p.A2 + ((size_t)(rtop - k * step) * p.nb + j) * p.H * kA2Row, aT + buf * kTileBuf, (uint32_t)p.H * kOutStride,
                    pol_keep);   // the next kernel reads A2
         bulk_wait_read<0>();
       };
@@ -831,7 +858,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
         mbar_wait(&bars.imgfull[stream], cnt[stream] & 1u);
         ++cnt[stream];
         // Xh, O1 are read a whole kernel later: stream them out; G2, G1 are read by the next kernel
-        bulk_store((uint8_t*)img + ((size_t)(rtop - i * S) * p.nb + j) * kTileBytes, aT + (i % 3) * kTileBuf, kTileBytes,
+        bulk_store((uint8_t*)img + ((size_t)(rtop - i * step) * p.nb + j) * kTileBytes, aT + (i % 3) * kTileBuf, kTileBytes,
                    pol_img);
         bulk_wait_read<0>();
         mbar_arrive(&bars.imgfree[stream]);
@@ -932,7 +959,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
         const int pair = u / NS, stg = u - pair * NS;
         const int i = 2 * pair + stream;
         if (i >= n) continue;
-        const int rem = rtop - i * S;
+        const int rem = rtop - i * step;
         const uint32_t src = tmem + lane_sel + kSlot * (uint32_t)((3 * t + half) % 5) + chalf * 48;
         const uint32_t dstA = tmem + lane_sel + kSlot * (uint32_t)((3 * t) % 5) + 24 * cq;
         uint8_t* tile = sT + (i % 3) * kTileBuf;
@@ -1096,9 +1123,12 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
 #endif
   }
   tc_fence_before();
-  __syncthreads();
+  __syncthreads();   // end of the segment: every role is done, every copy has landed
+  }
   TL(BACKWARD ? 28 : 20);
-  if (warp == 0) tmem_dealloc<512>(tmem);
+  SPAN(BACKWARD ? 3 : 2, 1);
+  tc_fence_after();
+  if (warp == 0) tmem_dealloc<512>(tmem_slot);
 }
 
 // ---- B4 / B6: parameter gradients as a split-K tensor-core GEMM ------------------------------------
@@ -1131,6 +1161,7 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
          int BKw, int H, int nb, int S) {
   extern __shared__ __align__(1024) uint8_t smem[];
   TL(32);
+  SPAN(4, 0);
   __shared__ __align__(8) uint64_t full[2], empty[2], done;
   __shared__ uint32_t tmem_slot;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -1239,6 +1270,7 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
   tc_fence_before();
   __syncthreads();
   TL(36);
+  SPAN(4, 1);
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
@@ -1463,12 +1495,21 @@ cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
   return e;
 }
 
-// CTAs per channel block of tc_mix2 (every CTA works on one block)
+// CTAs per channel block of tc_mix2 (a regular CTA works on one block)
 static int mix2_split(const Geometry& g, const TcPlan& tp) {
   int S = tp.num_sms / g.nb;
   if (S < 1) S = 1;
   if (S > g.B * g.Kw) S = g.B * g.Kw;
   return S;
+}
+// grid of tc_mix2: nb * S regular CTAs plus, when the (b, kw) pairs do not divide by S and SMs are left
+// over, spare CTAs for the remainder (see the kernel)
+static int mix2_grid(const Geometry& g, const TcPlan& tp, int S) {
+  const int reg = g.nb * S, left = (g.B * g.Kw) % S;
+  int spare = tp.num_sms - reg;
+  if (spare > g.nb) spare = g.nb;
+  if (left == 0 || spare < 0 || (g.B * g.Kw) / S == 0) spare = 0;
+  return reg + spare;
 }
 
 size_t tc_workspace_bytes(const Geometry& g, bool backward) {
@@ -1548,9 +1589,9 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   if (g.save_ctx) {
     // saved context: Xh, O1 (operands of tc_wgrad) and the activation masks stay in the workspace
     mp.Xh = w.Xh; mp.O1 = w.O1; mp.maskbits = w.maskbits;
-    e = launch_k(tc_mix2<kMixFwdSave, false>, g.nb * S2, kMix2Threads, kMix2Smem, st, true, mp, S2);
+    e = launch_k(tc_mix2<kMixFwdSave, false>, mix2_grid(g, tp, S2), kMix2Threads, kMix2Smem, st, true, mp, S2);
   } else {
-    e = launch_k(tc_mix2<kMixFwd, false>, g.nb * S2, kMix2Threads, kMix2Smem, st, true, mp, S2);
+    e = launch_k(tc_mix2<kMixFwd, false>, mix2_grid(g, tp, S2), kMix2Threads, kMix2Smem, st, true, mp, S2);
   }
   if (e != cudaSuccess) return e;
   prof_end(st);
@@ -1602,14 +1643,14 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   if (g.use_ctx) {
     // gradient stages only: Xh, O1 and the masks were left in the workspace by the forward call
     if (g.export_masks) {
-      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, true>, g.nb * S2, kMix2Threads, kMix2Smem, st, dep, mp, S2);
+      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, true>, mix2_grid(g, tp, S2), kMix2Threads, kMix2Smem, st, dep, mp, S2);
     } else {
-      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, false>, g.nb * S2, kMix2Threads, kMix2Smem, st, dep, mp, S2);
+      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, false>, mix2_grid(g, tp, S2), kMix2Threads, kMix2Smem, st, dep, mp, S2);
     }
   } else if (g.export_masks) {
-    TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, true>, g.nb * S2, kMix2Threads, kMix2Smem, st, dep, mp, S2);
+    TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, true>, mix2_grid(g, tp, S2), kMix2Threads, kMix2Smem, st, dep, mp, S2);
   } else {
-    TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, false>, g.nb * S2, kMix2Threads, kMix2Smem, st, dep, mp, S2);
+    TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, false>, mix2_grid(g, tp, S2), kMix2Threads, kMix2Smem, st, dep, mp, S2);
   }
   // B4 / B6: parameter gradients
   const int nred = nW + g.nb * BS;
@@ -1631,6 +1672,9 @@ extern "C" int afno_trace_read(long long* out) {
 extern "C" int afno_debug_set_policy(int mask) { return (int)cudaMemcpyToSymbol(g_polmask, &mask, sizeof(int)); }
 #endif
 #ifdef AFNO_TIMING
+extern "C" int afno_debug_read_span(long long* out) {
+  return (int)cudaMemcpyFromSymbol(out, g_afno_span, sizeof(long long) * 5 * 160 * 2);
+}
 extern "C" int afno_debug_read(long long* out) {
   return (int)cudaMemcpyFromSymbol(out, g_afno_dbg, sizeof(long long) * 128);
 }

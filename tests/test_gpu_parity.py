@@ -162,6 +162,8 @@ def test_bf16_forward_backward_full_size(oracle):
     (1, 96, 180, 192, 2, 1.0),    # H = 96: no padding rows in the mode tiles; two blocks
     (2, 18, 36, 288, 3, 0.5),     # truncated spectrum on a small grid, three blocks
     (5, 40, 100, 96, 1, 0.75),    # W/2+1 = 51 bins, Kw = 38, five samples
+    (1, 2, 4, 96, 1, 1.0),        # degenerate grid: fewer tiles than SMs, one tile per block
+    (4, 8, 16, 192, 2, 0.5),      # Kh = 2, Kw = 4: most of the spectrum truncated
 ])
 def test_bf16_tcgen05_other_shapes(oracle, B, H, W, C, nb, f):
     """The tcgen05 path away from the headline shape: ragged tails in every tiled dimension, forward
@@ -320,6 +322,40 @@ def test_saved_context_step_vs_oracle(oracle):
         print(f"[ctx step] {k}: rel_l2 mask-consistent {e:.3e}")
         assert e <= TOL_BF16, (k, e)
     assert rep["flip1"] <= 5e-3 and rep["flip2"] <= 5e-3 and rep["justified"], rep
+
+
+def test_saved_context_step_is_bitwise_repeatable():
+    """The asynchronous hand-offs of the tcgen05 kernels (TMA rings, tensor-memory ping-pong, bulk stores,
+    programmatic dependent launch) must not depend on timing: 60 saved-context steps on the same inputs,
+    with unrelated memory traffic interleaved, give bit-identical y, dx and parameter gradients."""
+    import torch
+    wl = inputs.WORKLOADS["fcn_b4_bwd"]
+    desc = parity.desc_for(wl, B=2)
+    d_save = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_SAVE_CONTEXT})
+    d_use = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_USE_CONTEXT})
+    binding.afno_plan_warmup(desc)
+    data = inputs.make_inputs(wl, B=2)
+    tx, tdy = parity.to_device_act(data["x"], True), parity.to_device_act(data["dy"], True)
+    p = parity.GpuLayer(desc).params(data["w1"], data["b1"], data["w2"], data["b2"])
+    ws = torch.empty(binding.afno_spectral_workspace_bytes(desc, True), dtype=torch.uint8, device="cuda")
+    junk = torch.empty(64 << 20, dtype=torch.uint8, device="cuda")
+    ref = None
+    for it in range(60):
+        ty, tdx = torch.empty_like(tx), torch.empty_like(tx)
+        g = [torch.empty_like(t) for t in p]
+        if it % 3 == 1:
+            junk.fill_(it & 255)
+        binding.afno_spectral_fwd(d_save, tx, *p, ty, ws)
+        if it % 5 == 2:
+            junk.fill_(1)
+        binding.afno_spectral_bwd(d_use, tx, tdy, *p, tdx, *g, ws)
+        torch.cuda.synchronize()
+        cur = [ty, tdx] + g
+        if ref is None:
+            ref = [t.clone() for t in cur]
+        else:
+            for k, (a, b) in enumerate(zip(ref, cur)):
+                assert torch.equal(a, b), (it, k)
 
 
 def test_host_variants_match_device(oracle):

@@ -366,11 +366,15 @@ def kernel_work(name, B, wl, kept_modes, ctx=True):
 
 def measured_traffic(name):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture."""
-    path = os.path.join(ROOT, "profiles", "r1e_dram_traffic.json")
+    path = os.path.join(ROOT, "profiles", "r1e_dram_traffic.csv")
     try:
-        return json.load(open(path)).get(name)
+        for line in open(path).read().splitlines()[1:]:
+            k, v = line.split(",")
+            if k == name:
+                return int(v)
     except Exception:
-        return None
+        pass
+    return None
 
 
 def kernel_roofline(name, n_launch, total_ms, steps, work, peaks, clocks, B, wl, kept_modes, ctx=True):

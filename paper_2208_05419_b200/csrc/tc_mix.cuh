@@ -449,6 +449,16 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
     long long dbg_m[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     long long dbg_f[8] = {0, 0, 0, 0, 0, 0, 0, 0};
 #endif
+    // BwdCtx: the mask bits of a stream's NEXT tile are loaded a whole tile ahead (a load issued just before
+    // the first epilogue of the tile exposed ~1,000 cycles of its latency)
+    auto mask_index = [&](int i) {
+      return (((size_t)(rtop - i * step) * p.nb + j) * 12 + (size_t)(cq * 3 + lq)) * 32 + lane;
+    };
+    uint4 mkn[2] = {make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0)};
+    if (CTXB) {
+      if (0 < n) mkn[0] = p.maskbits[mask_index(0)];
+      if (1 < n) mkn[1] = p.maskbits[mask_index(1)];
+    }
     DBG_T0();
     for (int u0 = 0; u0 < T / 2; ++u0) {
 #pragma unroll
@@ -465,9 +475,12 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
         uint8_t* tile = sT + (i % 3) * kTileBuf;
         const size_t img_off = ((size_t)rem * p.nb + j) * kTileBytes;
         const int se = stg + kStage0;
-        const size_t mask_idx = (((size_t)rem * p.nb + j) * 12 + (size_t)(cq * 3 + lq)) * 32 + lane;
+        const size_t mask_idx = mask_index(i);
         uint4 mk = make_uint4(0, 0, 0, 0);
-        if (CTXB && stg == 0) mk = p.maskbits[mask_idx];   // issued before the wait: its latency hides under the GEMM
+        if (CTXB && stg == 0) {
+          mk = mkn[stream];
+          if (i + 2 < n) mkn[stream] = p.maskbits[mask_index(i + 2)];
+        }
         mbar_wait_fast(&bars.dfull[stream], ce[stream] & 1u);
         ++ce[stream];
         TR(t, 4 + warp * 3);

@@ -101,31 +101,115 @@ def oracle_cfg(oracle, d: binding.Desc, no_residual=False, naive=False):
                          no_residual=no_residual, naive_dft=naive)
 
 
-def preactivation_scales(cfg, dump, w1, b1, w2, b2):
-    """Per-(mode, block) magnitude scale of the two pre-activations (S3, P-bwd (ii)).
+# Standard deviation of the relative error of one bf16 rounding (uniform within half an ulp, ulp = 2^-8 of
+# the leading bit), of an fp32 path operand (a generous 16 ulp for the depth of the FFT), and the multiple of
+# the 1-sigma error model a flipped mask may sit away from its threshold (S3, P-bwd (ii)).
+U_BF16 = 2.0 ** -9 / np.sqrt(3.0)
+U_F32 = 16.0 * 2.0 ** -24
+TAU_K = 6.0
+LEAK = 0.1
 
-    |P1[m,j,o] - b1| <= ||Xh[m,j,:]||_2 * ||W1[j,:,o]||_2 (Cauchy-Schwarz), so a kernel whose
-    operands carry a relative error eps perturbs P1 by at most ~eps * that product.  A DFT is
-    only NORMWISE accurate (||dXh|| <= eps ||x|| over the plane, not component by component),
-    so the row norm gets the plane's rms row norm added as an absolute floor; the same holds
-    for P2 with O1 and W2.  Returned arrays broadcast over the features of a block."""
+
+def preactivation_scales(cfg, dump, w1, b1, w2, b2, bf16=True):
+    """1-sigma error model of the two pre-activations, per (mode, output feature) (S3, P-bwd (ii)).
+
+    Every operand of the path is rounded once to bf16 (relative error of standard deviation u) and products
+    are accumulated in fp32, so errors add in quadrature.  Per complex component:
+      * spectrum: the two transform stages are GEMMs against rounded DFT matrices with a rounded
+        intermediate, so the error of Xh[r,kw,c] has a part u |Xh[r,kw,c]| (its own rounding), a part
+        ~ u * rms_r |Xh[:,kw,c]| (the H transform against a rounded matrix spreads column kw's energy over
+        its rows: a DFT is normwise, not componentwise, accurate), a part ~ u * rms_kw |Xh[r,:,c]| (the same
+        for the W transform: its error is a random combination of the field's rows, so after the H transform
+        it sits in the rows r where the field has energy, at every kw) and a plane-wide floor:
+            var_X = u^2 (|Xh|^2 + 2 colms[kw,c] + 2 rowms[r,c] + planems[c])
+      * P1[o] = sum_i Xh[i] W1[i,o] + b1:  var_1[o] = sum_i |W1[i,o]|^2 (var_X[i] + u^2 |Xh[i]|^2)
+      * O1 = relu(P1) rounded:             var_O[i] = var_1[i] + u^2 |O1[i]|^2
+      * P2[o] = sum_i O1[i] W2[i,o] + b2:  var_2[o] = sum_i |W2[i,o]|^2 (var_O[i] + u^2 |O1[i]|^2)
+    Returns sigma1 [B,H,Wh,nb*hid], sigma2 [B,H,Wh,C] (per real component: half the complex variance); a
+    flipped mask is justified when the oracle's pre-activation lies within TAU_K sigma of its threshold."""
     nb, bs, hid = cfg.num_blocks, cfg.bs, cfg.hid
-    cw1 = w1[..., 0] + 1j * w1[..., 1]
-    cw2 = w2[..., 0] + 1j * w2[..., 1]
-    w1n = np.sqrt((np.abs(cw1) ** 2).sum(axis=1)).max(axis=1)          # [nb]
-    w2n = np.sqrt((np.abs(cw2) ** 2).sum(axis=1)).max(axis=1)
-    b1n = np.abs(b1[..., 0] + 1j * b1[..., 1]).max(axis=1)
-    b2n = np.abs(b2[..., 0] + 1j * b2[..., 1]).max(axis=1)
+    u2 = (U_BF16 if bf16 else U_F32) ** 2
+    a1 = (w1[..., 0] ** 2 + w1[..., 1] ** 2)                           # [nb, bs, hid]  |W1[j,i,o]|^2
+    a2 = (w2[..., 0] ** 2 + w2[..., 1] ** 2)                           # [nb, hid, bs]
     xh = dump["xhat"]
-    xn = np.sqrt((np.abs(xh.reshape(xh.shape[:3] + (nb, bs))) ** 2).sum(-1))       # [B,H,Wh,nb]
+    x2 = np.abs(xh) ** 2                                               # [B,H,Wh,C]
+    colms = x2.mean(axis=1, keepdims=True)                             # [B,1,Wh,C]
+    planems = x2.mean(axis=(1, 2), keepdims=True)                      # [B,1,1,C]  = mean x^2 of the plane (Parseval)
+    rowms = x2.mean(axis=2, keepdims=True)                             # [B,H,1,C]
+    # The rounding errors of a DFT matrix are not random: the leak of a strong spectral line into the bins
+    # harmonically related to it (same column, rows a multiple of H/5 apart, ...) adds up coherently to
+    # ~ u |line| instead of u |line| / sqrt(H): the largest line of the column and of the row enter whole.
+    colmax = x2.max(axis=1, keepdims=True)
+    rowmax = x2.max(axis=2, keepdims=True)
+    var_x = u2 * (2.0 * x2 + 2.0 * colms + 2.0 * rowms + planems + LEAK * (colmax + rowmax))
+    shp = x2.shape[:3]
+    var_1 = np.einsum("mji,jio->mjo", var_x.reshape(-1, nb, bs), a1).reshape(shp + (nb * hid,))
     p1 = dump["p1"]
-    o1 = np.maximum(p1.real, 0) + 1j * np.maximum(p1.imag, 0)
-    on = np.sqrt((np.abs(o1.reshape(o1.shape[:3] + (nb, hid))) ** 2).sum(-1))
-    xfloor = np.sqrt((xn ** 2).mean(axis=(1, 2), keepdims=True))                    # [B,1,1,nb]
-    ofloor = np.sqrt((on ** 2).mean(axis=(1, 2), keepdims=True))
-    s1 = np.repeat((xn + xfloor) * w1n + b1n, hid, axis=-1)                         # [B,H,Wh,nb*hid]
-    s2 = np.repeat((on + ofloor) * w2n + b2n, bs, axis=-1)                          # [B,H,Wh,C]
-    return s1, s2
+    o2 = np.maximum(p1.real, 0) ** 2 + np.maximum(p1.imag, 0) ** 2     # |O1|^2
+    var_o = var_1 + 2.0 * u2 * o2
+    var_2 = np.einsum("mji,jio->mjo", var_o.reshape(-1, nb, hid), a2).reshape(shp + (nb * bs,))
+    return np.sqrt(0.5 * var_1), np.sqrt(0.5 * var_2)
+
+
+def tile_rel_l2(a, b, block: int, slab: bool = False):
+    """Relative L2 error per tile of an activation-shaped tensor [B,H,W,C]: one tile = (b, h, channel block)
+    (what one CTA iteration of the W-direction kernels produces), or with slab=True one (b, block) slab
+    (what the 91 mode tiles of one block and sample feed).  Returns the array of per-tile errors."""
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    B, H, W, C = b.shape
+    e = ((a - b) ** 2).reshape(B, H, W, C // block, block).sum(axis=(2, 4))         # [B,H,nb]
+    n = (b ** 2).reshape(B, H, W, C // block, block).sum(axis=(2, 4))
+    if slab:
+        e, n = e.sum(axis=1), n.sum(axis=1)
+    return np.sqrt(e / np.where(n > 0, n, 1.0))
+
+
+def block_rel_l2(a, b):
+    """Relative L2 error per channel block of a parameter-shaped tensor [nb, ...]."""
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    ax = tuple(range(1, b.ndim))
+    n = np.sqrt((b ** 2).sum(axis=ax))
+    return np.sqrt(((a - b) ** 2).sum(axis=ax)) / np.where(n > 0, n, 1.0)
+
+
+MAXABS_K = 16.0
+
+
+def gate_activation(got, ref, tol, block, label=""):
+    """The parity gate of an activation tensor: rel-L2 over the whole tensor, over every (b, h, block) tile
+    and every (b, block) slab at `tol`, and an elementwise max-abs gate
+        |got - ref| <= MAXABS_K * tol * rms(ref) + tol * |ref|
+    (a stated multiple of the rms error the tolerance allows, plus the tolerance relative to the element
+    itself: the branch s has one spike per plane at token (0, 0), the image of the bias, ~100x its rms).
+    Returns a dict of the measured figures; raises AssertionError naming the worst tile."""
+    got = np.asarray(got, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    assert np.isfinite(got).all(), (label, "non-finite output")
+    whole = rel_l2(got, ref)
+    tiles = tile_rel_l2(got, ref, block)
+    slabs = tile_rel_l2(got, ref, block, slab=True)
+    rms = float(np.sqrt((ref ** 2).mean()))
+    ma = max_abs(got, ref)
+    elem = float((np.abs(got - ref) / (MAXABS_K * tol * rms + tol * np.abs(ref) + 1e-300)).max())
+    rep = dict(rel_l2=whole, tile_max=float(tiles.max()), slab_max=float(slabs.max()), max_abs=ma,
+               max_abs_gate=elem)
+    assert whole <= tol, (label, "rel_l2", whole)
+    assert tiles.max() <= tol, (label, "tile (b,h,block)", np.unravel_index(tiles.argmax(), tiles.shape), float(tiles.max()))
+    assert slabs.max() <= tol, (label, "slab (b,block)", np.unravel_index(slabs.argmax(), slabs.shape), float(slabs.max()))
+    assert elem <= 1.0, (label, "max_abs", ma, "elementwise |err| / (K tol rms + tol |ref|)", elem, "rms(ref)", rms)
+    return rep
+
+
+def gate_param(got, ref, tol, label=""):
+    """Parameter gradients: rel-L2 over the whole tensor and per channel block."""
+    assert np.isfinite(np.asarray(got)).all(), (label, "non-finite gradient")
+    whole = rel_l2(got, ref)
+    blocks = block_rel_l2(got, ref)
+    assert whole <= tol, (label, "rel_l2", whole)
+    assert blocks.max() <= tol, (label, "block", int(blocks.argmax()), float(blocks.max()))
+    return dict(rel_l2=whole, block_max=float(blocks.max()), max_abs=max_abs(got, ref))
 
 
 def kept_modes(cfg):

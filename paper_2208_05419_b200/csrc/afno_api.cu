@@ -48,6 +48,8 @@ int resolve(const afno_desc_t* d, Geometry* g) {
   if (d->flags & ~(uint32_t)(AFNO_FLAG_NO_RESIDUAL | AFNO_FLAG_ACCUM_GRADS | AFNO_FLAG_FORCE_FP32_MATH |
                              AFNO_FLAG_EXPORT_MASKS | AFNO_FLAG_SAVE_CONTEXT | AFNO_FLAG_USE_CONTEXT))
     return fail(AFNO_ERR_INVALID_ARG, "unknown flag bits");
+  if ((d->flags & AFNO_FLAG_SAVE_CONTEXT) && (d->flags & AFNO_FLAG_USE_CONTEXT))
+    return fail(AFNO_ERR_INVALID_ARG, "AFNO_FLAG_SAVE_CONTEXT (forward) and AFNO_FLAG_USE_CONTEXT (backward) exclude each other");
   if ((long long)d->B * d->H * d->W >= (1LL << 31) / 4)
     return fail(AFNO_ERR_UNSUPPORTED, "B*H*W too large for 32-bit token indexing");
   if (d->W % 2 != 0) return fail(AFNO_ERR_UNSUPPORTED, "odd W is not supported on the GPU path");
@@ -120,16 +122,24 @@ cudaError_t build_fft_plan(int n, FftPlan* out) {
   float2* dtw = nullptr;
   int16_t* dperm = nullptr;
   cudaError_t e = cudaMalloc(&dtw, sizeof(float2) * n);
-  if (e != cudaSuccess) return e;
-  e = cudaMalloc(&dperm, sizeof(int16_t) * n);
-  if (e != cudaSuccess) return e;
-  e = cudaMemcpy(dtw, tw.data(), sizeof(float2) * n, cudaMemcpyHostToDevice);
-  if (e != cudaSuccess) return e;
-  e = cudaMemcpy(dperm, perm.data(), sizeof(int16_t) * n, cudaMemcpyHostToDevice);
-  if (e != cudaSuccess) return e;
+  if (e == cudaSuccess) e = cudaMalloc(&dperm, sizeof(int16_t) * n);
+  if (e == cudaSuccess) e = cudaMemcpy(dtw, tw.data(), sizeof(float2) * n, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(dperm, perm.data(), sizeof(int16_t) * n, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {   // nothing of a failed plan stays allocated
+    cudaFree(dtw);
+    cudaFree(dperm);
+    return e;
+  }
   out->tw = dtw;
   out->perm = dperm;
   return cudaSuccess;
+}
+
+void free_fft_plan(FftPlan* p) {
+  cudaFree(const_cast<float2*>(p->tw));
+  cudaFree(const_cast<int16_t*>(p->perm));
+  p->tw = nullptr;
+  p->perm = nullptr;
 }
 
 // Returns the plan for (current device, H, W); builds it when allowed.
@@ -151,8 +161,11 @@ int get_plan(const Geometry& g, bool may_build, const Plan** out) {
   p->W = g.W;
   e = build_fft_plan(g.H, &p->fh);
   if (e == cudaSuccess) e = build_fft_plan(g.W, &p->fw);
-  if (e == cudaSuccess && g.H <= 96 && g.W <= 192) e = tc_build_plan(g.H, g.W, &p->tc);
+  if (e == cudaSuccess && tc_plan_supported(g.H, g.W)) e = tc_build_plan(g.H, g.W, &p->tc);
   if (e != cudaSuccess) {
+    free_fft_plan(&p->fh);
+    free_fft_plan(&p->fw);
+    tc_free_plan(&p->tc);
     delete p;
     return fail(AFNO_ERR_CUDA, std::string("plan creation: ") + cudaGetErrorString(e));
   }
@@ -311,6 +324,7 @@ int afno_spectral_fwd(const afno_desc_t* d, const void* x, const float* w1, cons
   int rc = resolve(d, &g);
   if (rc != AFNO_OK) return rc;
   if (!x || !w1 || !b1 || !w2 || !b2 || !y || !workspace) return fail(AFNO_ERR_INVALID_ARG, "NULL pointer argument");
+  if (g.use_ctx) return fail(AFNO_ERR_INVALID_ARG, "AFNO_FLAG_USE_CONTEXT is a flag of afno_spectral_bwd");
   const void* ptrs[] = {x, w1, b1, w2, b2, y, workspace};
   for (const void* p : ptrs)
     if (!aligned16(p)) return fail(AFNO_ERR_INVALID_ARG, "pointers must be 16-byte aligned");
@@ -341,6 +355,7 @@ int afno_spectral_bwd(const afno_desc_t* d, const void* x, const void* dy, const
   if (rc != AFNO_OK) return rc;
   if (!x || !dy || !w1 || !b1 || !w2 || !b2 || !dx || !dw1 || !db1 || !dw2 || !db2 || !workspace)
     return fail(AFNO_ERR_INVALID_ARG, "NULL pointer argument");
+  if (g.save_ctx) return fail(AFNO_ERR_INVALID_ARG, "AFNO_FLAG_SAVE_CONTEXT is a flag of afno_spectral_fwd");
   const void* ptrs[] = {x, dy, w1, b1, w2, b2, dx, dw1, db1, dw2, db2, workspace};
   for (const void* p : ptrs)
     if (!aligned16(p)) return fail(AFNO_ERR_INVALID_ARG, "pointers must be 16-byte aligned");

@@ -65,6 +65,8 @@ bool generic_supported(const Geometry& g, const char** why);
 
 // ---- tcgen05 bf16 path (tc_path.cu) --------------------------------------------------
 bool tc_supported(const Geometry& g);
+bool tc_plan_supported(int H, int W);   // grid sizes the constant operand images can be built for
+void tc_free_plan(TcPlan* p);
 cudaError_t tc_build_plan(int H, int W, TcPlan* out);
 size_t tc_workspace_bytes(const Geometry& g, bool backward);
 cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const float* w1, const float* b1,

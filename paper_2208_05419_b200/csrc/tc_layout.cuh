@@ -18,16 +18,28 @@ constexpr uint32_t kWBytes = BS * BS * 2;            // 18432
 // contiguous bytes, conflict-free)
 constexpr uint32_t kTileLbo = 128, kTileSbo = 1536 + 16;
 constexpr uint32_t kTileBytes = (NT / 8) * kTileSbo; // 37248
+// Context header (AFNO_FLAG_SAVE_CONTEXT -> AFNO_FLAG_USE_CONTEXT): the forward call records what it saved,
+// the backward call's guard kernel compares and poisons dx and the gradients with NaN on a mismatch.
+struct CtxHeader {
+  uint32_t magic;
+  int32_t B, H, W, C, nb, Kh, Kw, chunk_b;
+  uint32_t lambda_bits, export_masks;
+  uint32_t pad[5];
+};
+constexpr uint32_t kCtxMagic = 0xAF90C7E5u;
+
 // ---- weight preparation: fp32 [nb][96][96][2] -> bf16 K-major interleaved operands --------------
 // per block 4 matrices of kWBytes {W1r, W1i, W2r, W2i} with element (n=o, k=i) = W[i][o] (the
 // backward pass reads the same images as MN-major operands), and the biases regrouped as
 // [block][layer][re 96 | im 96] fp32.
 __global__ void k_tc_prep_weights(const float* __restrict__ w1, const float* __restrict__ b1,
                                   const float* __restrict__ w2, const float* __restrict__ b2,
-                                  __nv_bfloat16* __restrict__ out, float* __restrict__ bout, int nb) {
+                                  __nv_bfloat16* __restrict__ out, float* __restrict__ bout, int nb,
+                                  const CtxHeader hdr, CtxHeader* __restrict__ hdr_out) {
   pdl_launch_dependents();
   pdl_wait();
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx == 0 && hdr_out != nullptr) *hdr_out = hdr;   // SAVE_CONTEXT: what this call leaves in the workspace
   if (idx < nb * BS) {
     const int o = idx % BS, j = idx / BS;
     const float2 a = ((const float2*)b1)[idx], b = ((const float2*)b2)[idx];
@@ -54,46 +66,46 @@ __device__ __forceinline__ void pack32(const uint32_t (&v)[32], uint32_t (&pk)[1
   for (int q = 0; q < 16; ++q) pk[q] = pack_bf16(__uint_as_float(v[2 * q]), __uint_as_float(v[2 * q + 1]));
 }
 
-// Which copies carry a non-default L2 eviction policy (chosen by measurement, S5.3); bit set =
-// the policy named in the comment, clear = evict_normal.
-enum {
-  kPolWfLoad = 1,     // tc_wdft_fwd2: activation loads evict_first
-  kPolWfStore = 2,    // tc_wdft_fwd2: A1 stores evict_last
-  kPolWiLoad = 4,     // tc_wdft_inv2: A2 and residual loads evict_first
-  kPolWiStore = 8,    // tc_wdft_inv2: y stores evict_first
-  kPolMixLoad = 16,   // tc_mix2: tile loads evict_first
-  kPolMixStore = 32,  // tc_mix2: A2 stores evict_last
-  kPolMixImg = 64,    // tc_mix2: Xh, O1 stores evict_first; G2, G1 stores evict_last
-  kPolWgLoad = 128    // tc_wgrad: operand loads evict_first
+// L2 eviction policy of every bulk-copy site (2 bits each: 0 evict_normal, 1 evict_first, 2 evict_last).
+// The chunk buffers (half-spectrum A, gradient images G2 / G1) are rewritten by every chunk and should
+// never leave the L2; everything else streams through once.
+enum PolSite {
+  kPolWfLoadX = 0,     // tc_wdft_fwd2: activation loads (x, dy)
+  kPolWfStoreA = 1,    // tc_wdft_fwd2: half-spectrum stores
+  kPolWiLoadA = 2,     // tc_wdft_inv2: half-spectrum loads
+  kPolWiLoadRes = 3,   // tc_wdft_inv2: residual loads (x, dy)
+  kPolWiStoreY = 4,    // tc_wdft_inv2: output stores (y, dx)
+  kPolMixLoadA = 5,    // tc_mix2: tile loads
+  kPolMixStoreA = 6,   // tc_mix2: tile stores (in place)
+  kPolMixStoreCtx = 7, // tc_mix2<FwdSave>: Xh, O1 stores (read a whole pass later)
+  kPolMixStoreG = 8,   // tc_mix2<Bwd*>: G2, G1 (and Xh, O1 of the stateless backward) stores, read by the next kernel
+  kPolWgLoadCtx = 9,   // tc_wgrad: Xh, O1 loads
+  kPolWgLoadG = 10     // tc_wgrad: G2, G1 loads
 };
-#ifdef AFNO_POLICY_EXPERIMENT
-__device__ int g_polmask = 255;
-#define POLMASK g_polmask
-#else
-constexpr int kPolMask = kPolWfStore | kPolWgLoad;   // measured: 0 -> 496 us per step, all -> 499, this choice -> 486
-#define POLMASK kPolMask
+#ifndef AFNO_POLICIES
+#define AFNO_POLICIES ((1u << 0) | (2u << 2) | (0u << 4) | (1u << 6) | (1u << 8) | (0u << 10) | (2u << 12) | (1u << 14) | (2u << 16) | (1u << 18) | (0u << 20))
 #endif
-__device__ __forceinline__ uint64_t pol_first(int bit) { return (POLMASK & bit) ? l2_evict_first() : l2_evict_normal(); }
-__device__ __forceinline__ uint64_t pol_last(int bit) { return (POLMASK & bit) ? l2_evict_last() : l2_evict_normal(); }
+__device__ __forceinline__ uint64_t pol(PolSite site) {
+  const uint32_t v = ((uint32_t)(AFNO_POLICIES) >> (2 * (int)site)) & 3u;
+  return v == 1 ? l2_evict_first() : v == 2 ? l2_evict_last() : l2_evict_normal();
+}
 
-#ifdef AFNO_TRACE
-__device__ long long g_afno_trace[64 * 32];
-#define TR(t, slot) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (t) >= 40 && (t) < 72) g_afno_trace[((t) - 40) * 64 + (slot)] = clock64(); } while (0)
-#else
-#define TR(t, slot)
-#endif
-#ifdef AFNO_TIMING
-__device__ long long g_afno_dbg[128];
-#define DBG_T0() long long dbg_t = clock64()
-#define DBG_ACC(slot) do { long long n_ = clock64(); dbg_acc[slot] += n_ - dbg_t; dbg_t = n_; } while (0)
-// per-CTA start / end wall-clock (ns) of the last launch of kernel family k (load balance of the static tile schedule)
-__device__ long long g_afno_span[5][160][2];
-#define SPAN(k, e) do { if (threadIdx.x == 0 && blockIdx.x < 160) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_afno_span[k][blockIdx.x][e] = (long long)t_; } } while (0)
-// timeline of CTA 0: wall-clock (ns) at a few points of a kernel
-#define TL(slot) do { if (blockIdx.x == 0 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); g_afno_dbg[slot] = (long long)t_; } } while (0)
-#else
-#define DBG_T0()
-#define DBG_ACC(slot)
-#define TL(slot)
-#define SPAN(k, e)
-#endif
+// USE_CONTEXT guard: the header the forward call left must describe this call; otherwise dx and the parameter
+// gradients are overwritten with NaN (a context of another geometry / flag set / never saved would have
+// produced silently wrong numbers).  Exits at once when the header matches.
+__global__ void k_tc_ctx_guard(const CtxHeader* __restrict__ got, const CtxHeader want, uint16_t* __restrict__ dx, size_t n_act,
+                               float* __restrict__ dw1, float* __restrict__ dw2, size_t n_w, float* __restrict__ db1,
+                               float* __restrict__ db2, size_t n_b) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const uint32_t* a = (const uint32_t*)got;
+  const uint32_t* b = (const uint32_t*)&want;
+  bool ok = true;
+  for (uint32_t q = 0; q < sizeof(CtxHeader) / 4; ++q) ok = ok && (a[q] == b[q]);
+  if (ok) return;
+  const size_t stride = (size_t)gridDim.x * blockDim.x, t0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const float nanf_ = __int_as_float(0x7FC00000);
+  for (size_t i = t0; i < n_act; i += stride) dx[i] = 0x7FC0;   // bf16 NaN
+  for (size_t i = t0; i < n_w; i += stride) { dw1[i] = nanf_; dw2[i] = nanf_; }
+  for (size_t i = t0; i < n_b; i += stride) { db1[i] = nanf_; db2[i] = nanf_; }
+}

@@ -141,19 +141,13 @@ __device__ __forceinline__ void store_chunks6(uint8_t* base, int chunk0, int r, 
     *(uint4*)(base + (chunk0 + g) * kTileSbo + r * 16) = make_uint4(pk[4 * g], pk[4 * g + 1], pk[4 * g + 2], pk[4 * g + 3]);
 }
 
-// softshrink of a packed bf16 pair: a - min(max(a, -lambda), lambda)
-__device__ __forceinline__ uint32_t shrink_bf16x2(uint32_t a, uint32_t lam2, uint32_t nlam2) {
-  uint32_t c, r;
-  asm("max.bf16x2 %0, %1, %2;" : "=r"(c) : "r"(a), "r"(nlam2));
-  asm("min.bf16x2 %0, %1, %2;" : "=r"(c) : "r"(c), "r"(lam2));
-  asm("sub.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(c));
-  return r;
-}
-// Z = S_lambda(a + b) on a packed pair: the sum is rounded to bf16 once, then shrunk (exact zeros inside
-// the threshold; lambda at bf16 precision).  Forward value and backward mask (Z != 0) come from this one
-// function, so the gradient is the gradient of the function the forward pass evaluates.
-__device__ __forceinline__ uint32_t shrink_sum(float v0, float v1, float b0, float b1, uint32_t lam2, uint32_t nlam2) {
-  return shrink_bf16x2(pack_bf16(v0 + b0, v1 + b1), lam2, nlam2);
+// Z = S_lambda(v + b) evaluated on the fp32 accumulator (reading A15): z = t - min(max(t, -lambda), lambda)
+// with t = v + b in fp32, exact zeros inside the threshold, then ONE rounding of the pair to bf16.  Forward
+// value and backward mask (Z != 0, i.e. |t| > lambda in fp32) come from this one function, so the gradient
+// is the gradient of the function the forward pass evaluates.
+__device__ __forceinline__ uint32_t shrink_sum(float v0, float v1, float b0, float b1, float lam) {
+  const float t0 = v0 + b0, t1 = v1 + b1;
+  return pack_bf16(t0 - fminf(fmaxf(t0, -lam), lam), t1 - fminf(fmaxf(t1, -lam), lam));
 }
 // relu + one rounding of two fp32 values to a packed bf16 pair (lo, hi)
 __device__ __forceinline__ uint32_t pack_relu_bf16(float lo, float hi) {
@@ -216,8 +210,6 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
   // that buffer with the gradient tile meanwhile and stores the images with plain vector stores.
   constexpr bool STAGED = SAVE || CTXB;
   extern __shared__ __align__(1024) uint8_t smem[];
-  TL(BACKWARD ? 24 : 16);
-  SPAN(BACKWARD ? 3 : 2, 0);
   __shared__ Mix2Bars bars;
   __shared__ uint32_t tmem_slot;
   __shared__ __align__(16) float sBias[2 * NT];
@@ -240,9 +232,7 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
   pdl_launch_dependents();
   for (uint32_t i = tid; i < 3 * kTileBuf / 16; i += kMix2Threads) ((uint4*)sT)[i] = make_uint4(0, 0, 0, 0);
   for (uint32_t i = tid; i < 2 * kDft2Bytes / 16; i += kMix2Threads) cp_async16(smem_u32(sCh) + i * 16, p.dft + (size_t)i * 16);
-  TL(BACKWARD ? 25 : 17);
   pdl_wait();   // the weight images below are written by an earlier kernel of the chain
-  TL(BACKWARD ? 26 : 18);
   if (warp == 0) tmem_alloc<512>(&tmem_slot);
 #pragma unroll 1
   for (int seg = 0; seg < nseg; ++seg) {
@@ -286,7 +276,6 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
-  TL(BACKWARD ? 27 : 19);
   // Stream 1 runs kLag stages behind stream 0, so tiles finish (and buffers become free) at
   // regular intervals and a transform stage of one stream overlaps an MLP stage of the other.
   constexpr int kLag = NS / 2;
@@ -298,8 +287,8 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
     // warp 7 lane 0 issues every copy (TMA tile loads in, bulk stores of the staged rows out); the other
     // two warps of this lane quarter have nothing to do
     const uint32_t aT = smem_u32(sT);
-    const uint64_t pol_stream = pol_first(kPolMixLoad), pol_keep = pol_last(kPolMixStore);
-    const uint64_t pol_img = SAVE ? pol_first(kPolMixImg) : pol_last(kPolMixImg);
+    const uint64_t pol_stream = pol(kPolMixLoadA), pol_keep = pol(kPolMixStoreA);
+    const uint64_t pol_img = SAVE ? pol(kPolMixStoreCtx) : pol(kPolMixStoreG);
     if (warp == 7 && lane == 0) {
       auto load = [&](int buf, const CUtensorMap* m, int i, uint64_t* full) {
         const int tile_id = (rtop - i * step) * p.nb + j;
@@ -371,10 +360,6 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
     const uint32_t aCh = smem_u32(sCh), aSh = smem_u32(sSh), aW = smem_u32(sW), aT = smem_u32(sT);
     const uint32_t w1r = aW, w1i = aW + kWBytes, w2r = aW + 2 * kWBytes, w2i = aW + 3 * kWBytes;
     uint32_t cs0 = 0, cs1 = 0;   // phases issued so far per stream
-#ifdef AFNO_TIMING
-    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-#endif
-    DBG_T0();
     for (int t = 0; t < T; ++t) {
       const int stream = t & 1, u = (t >> 1) - (stream ? kLag : 0);
       if (u < 0) continue;
@@ -385,8 +370,6 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
       const uint32_t SA = tmem + kSlot * (uint32_t)((3 * t + 4) % 5);   // slot of phase t - 2
       const uint32_t cs = stream ? cs1 : cs0;
       if (cs > 0) mbar_wait_fast(&bars.edone[stream], (cs - 1) & 1u);
-      TR(t, 0);
-      DBG_ACC(0);
       const int buf = i % 3;
       const uint32_t use = (uint32_t)(i / 3);
       const uint32_t tile = aT + buf * kTileBuf;
@@ -394,7 +377,6 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
       const bool first = stg == 0, dftg = RECOMP && stg == 3, last = stg == NS - 1;
       if (first) mbar_wait(&bars.xfull[buf], use & 1u);
       if (dftg) mbar_wait(&bars.gfull[buf], use & 1u);
-      DBG_ACC(1);
       if (elect_one()) {
         tc_fence_after();
         if (first || dftg) {
@@ -414,16 +396,8 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
         if (RECOMP && first) mma_commit(&bars.xfree[buf]);
       }
       __syncwarp();
-      TR(t, 2);
-      DBG_ACC(2);
       if (stream) ++cs1; else ++cs0;
     }
-#ifdef AFNO_TIMING
-    if (blockIdx.x == 0 && lane == 0) {
-      for (int q = 0; q < 8; ++q) g_afno_dbg[(BACKWARD ? 80 : 64) + q] = dbg_acc[q];
-      g_afno_dbg[(BACKWARD ? 80 : 64) + 7] = n;
-    }
-#endif
   } else {
     // ================================ epilogue warps =========================================
     const int cq = warp >> 2;              // column quarter: 0 re lo, 1 re hi, 2 im lo, 3 im hi
@@ -444,11 +418,6 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
     auto wait_img_read = [&](int stream) {
       if (STAGED && ci[stream] > 0) mbar_wait(&bars.imgfree[stream], (ci[stream] - 1) & 1u);
     };
-#ifdef AFNO_TIMING
-    long long dbg_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    long long dbg_m[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    long long dbg_f[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-#endif
     // BwdCtx: the mask bits of a stream's NEXT tile are loaded a whole tile ahead (a load issued just before
     // the first epilogue of the tile exposed ~1,000 cycles of its latency)
     auto mask_index = [&](int i) {
@@ -459,7 +428,6 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
       if (0 < n) mkn[0] = p.maskbits[mask_index(0)];
       if (1 < n) mkn[1] = p.maskbits[mask_index(1)];
     }
-    DBG_T0();
     for (int u0 = 0; u0 < T / 2; ++u0) {
 #pragma unroll
       for (int stream = 0; stream < 2; ++stream) {
@@ -483,12 +451,9 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
         }
         mbar_wait_fast(&bars.dfull[stream], ce[stream] & 1u);
         ++ce[stream];
-        TR(t, 4 + warp * 3);
-        DBG_ACC(0);
         tc_fence_after();
         uint32_t v[48], pk[24];
         ld48(src, v);
-        DBG_ACC(2);
         bool writes_a = false, early_arrive = false;
         // backward: operand image (Xh, O1, G2, G1) this stage also writes for tc_wgrad; stored AFTER the
         // hand-off to the next GEMM, so the global stores run in the shadow of the tensor core
@@ -521,12 +486,11 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
           //      backward: only the mask ----
           // Z = softshrink(P2 + b2), zero on truncated rows (shrink_sum)
           const float lam = p.lambda;
-          const uint32_t lam2 = pack_bf16(lam, lam), nlam2 = lam2 ^ 0x80008000u;
 #pragma unroll
           for (int q = 0; q < 12; ++q) {
             const float4 bq = *(const float4*)(bias2 + 4 * q);
-            pk[2 * q] = shrink_sum(__uint_as_float(v[4 * q]), __uint_as_float(v[4 * q + 1]), bq.x, bq.y, lam2, nlam2);
-            pk[2 * q + 1] = shrink_sum(__uint_as_float(v[4 * q + 2]), __uint_as_float(v[4 * q + 3]), bq.z, bq.w, lam2, nlam2);
+            pk[2 * q] = shrink_sum(__uint_as_float(v[4 * q]), __uint_as_float(v[4 * q + 1]), bq.x, bq.y, lam);
+            pk[2 * q + 1] = shrink_sum(__uint_as_float(v[4 * q + 2]), __uint_as_float(v[4 * q + 3]), bq.z, bq.w, lam);
           }
           if (!row_kept) {
 #pragma unroll
@@ -592,18 +556,12 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
             });
           }
         }
-#ifdef AFNO_TIMING
-        { long long n_ = clock64(); dbg_m[se] += n_ - dbg_t; dbg_t = n_; }
-#endif
-        TR(t, 5 + warp * 3);
         if (writes_a) {
           // the four warps of this lane quarter have their accumulator columns in registers:
           // compact the bf16 operand into the first slot (columns of the other warps' sources)
           asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
-          DBG_ACC(4);
           st24(dstA, pk);
           tmem_wait_st();
-          DBG_ACC(5);
         }
         if (!early_arrive) {
           tc_fence_before();
@@ -622,24 +580,12 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
             store_chunks6(gimg, chunk0, r, pk);
           }
         }
-        TR(t, 6 + warp * 3);
-        DBG_ACC(1);
       }
     }
-#ifdef AFNO_TIMING
-    if (blockIdx.x == 0 && tid == 0)
-      for (int q = 0; q < 8; ++q) {
-        g_afno_dbg[(BACKWARD ? 88 : 72) + q] = dbg_acc[q];
-        g_afno_dbg[(BACKWARD ? 104 : 96) + q] = dbg_m[q];
-        g_afno_dbg[(BACKWARD ? 120 : 112) + q] = dbg_f[q];
-      }
-#endif
   }
   tc_fence_before();
   __syncthreads();   // end of the segment: every role is done, every copy has landed
   }
-  TL(BACKWARD ? 28 : 20);
-  SPAN(BACKWARD ? 3 : 2, 1);
   tc_fence_after();
   if (warp == 0) tmem_dealloc<512>(tmem_slot);
 }

@@ -114,16 +114,42 @@ bool tile_tmap(const TcPlan& tp, CUtensorMap* m, const void* ptr, const Geometry
 }
 
 struct TcWs {
-  __nv_bfloat16 *A1, *A2, *wprep;
+  CtxHeader* header;
+  __nv_bfloat16 *A, *wprep;   // A: half-spectrum of ONE chunk of samples, transformed in place by tc_mix2
   float* bprep;
-  __nv_bfloat16 *A1g, *Xh, *O1, *G2, *G1; // backward only
+  __nv_bfloat16 *Ax;          // stateless backward only: spectrum of x (A then holds the gradient's)
+  __nv_bfloat16 *Xh, *O1;     // whole batch (they are the saved context)
+  __nv_bfloat16 *G2, *G1;     // one chunk
   float* part;
-  uint4* maskbits;   // saved context: bit-packed activation masks, 6 KB per (b, kw, block) tile
+  uint4* maskbits;   // saved context: bit-packed activation masks, 6 KB per (b, kw, block) tile; whole batch
   uint8_t *mask1, *mask2;
   size_t mask_region;
   int S;
+  int chunk_f, chunk_b;   // samples per chunk in the forward / backward call
   size_t total;
 };
+
+// Samples per chunk.  A call walks the batch in chunks of samples: W transform -> per-mode chain (in place)
+// -> [parameter gradients ->] inverse W transform, over buffers that hold ONE chunk and are reused by the
+// next, so the workspace does not grow with B.  Measured on B200 at 90x180x768, B = 4 fwd+bwd (DESIGN.md
+// S5.5): chunks of 1 / 2 / 4 samples -> 0.529 / 0.494 / 0.466 ms per step.  Smaller chunks keep more of the
+// half-spectra in the L2 (DRAM traffic 2.07 -> 1.84 GB) but every kernel boundary costs ~4 us of drain and
+// ramp-up on these persistent pipelines, which outweighs it: the default is 4.
+#ifndef AFNO_CHUNK_FWD
+#define AFNO_CHUNK_FWD 4
+#endif
+#ifndef AFNO_CHUNK_BWD
+#define AFNO_CHUNK_BWD 4
+#endif
+size_t spec_bytes(const Geometry& g, int B) { return (size_t)B * g.Kw * g.nb * g.H * kA2Row * 2; }
+size_t img_bytes(const Geometry& g, int B) { return (size_t)B * g.Kw * g.nb * kTileBytes; }
+int chunk_samples(const Geometry& g, bool backward) {
+  int cb = backward ? AFNO_CHUNK_BWD : AFNO_CHUNK_FWD;
+  if (cb < 1) cb = 1;
+  if (cb > g.B) cb = g.B;
+  return cb;
+}
+
 TcWs tc_carve(const Geometry& g, bool backward, char* base) {
   TcWs w{};
   size_t off = 0;
@@ -138,24 +164,26 @@ TcWs tc_carve(const Geometry& g, bool backward, char* base) {
     w.mask2 = (uint8_t*)take(b2);
     w.mask_region = off;
   }
-  const size_t spec = (size_t)g.B * g.Kw * g.nb * g.H * kA2Row * 2;
-  w.A1 = (__nv_bfloat16*)take(spec);
-  w.A2 = (__nv_bfloat16*)take(spec);
+  w.header = (CtxHeader*)take(sizeof(CtxHeader));
+  w.chunk_f = chunk_samples(g, false);
+  w.chunk_b = chunk_samples(g, true);
+  const int cmax = w.chunk_f > w.chunk_b ? w.chunk_f : w.chunk_b;
   w.wprep = (__nv_bfloat16*)take((size_t)g.nb * 4 * kWBytes);
   w.bprep = (float*)take((size_t)g.nb * 2 * NT * sizeof(float));
+  w.A = (__nv_bfloat16*)take(spec_bytes(g, backward ? cmax : w.chunk_f));
   if (backward) {
-    w.A1g = (__nv_bfloat16*)take(spec);
-    const size_t img = (size_t)g.B * g.Kw * g.nb * kTileBytes;   // operand-image layout
-    w.Xh = (__nv_bfloat16*)take(img);
-    w.O1 = (__nv_bfloat16*)take(img);
-    w.G2 = (__nv_bfloat16*)take(img);
-    w.G1 = (__nv_bfloat16*)take(img);
+    w.Xh = (__nv_bfloat16*)take(img_bytes(g, g.B));
+    w.O1 = (__nv_bfloat16*)take(img_bytes(g, g.B));
     w.maskbits = (uint4*)take((size_t)g.B * g.Kw * g.nb * 12 * 32 * sizeof(uint4));
+    w.G2 = (__nv_bfloat16*)take(img_bytes(g, w.chunk_b));
+    w.G1 = (__nv_bfloat16*)take(img_bytes(g, w.chunk_b));
     int S = 148 / (2 * g.nb);   // CTAs per (layer, block) of tc_wgrad
     if (S < 1) S = 1;
-    if (S > g.B * g.Kw) S = g.B * g.Kw;
+    if (S > w.chunk_b * g.Kw) S = w.chunk_b * g.Kw;
     w.S = S;
     w.part = (float*)take((size_t)2 * g.nb * S * kWgPartFloats * sizeof(float));
+    // last, so that the context layout does not depend on it: only the stateless backward uses it
+    if (!g.save_ctx && !g.use_ctx) w.Ax = (__nv_bfloat16*)take(spec_bytes(g, w.chunk_b));
   }
   w.total = off;
   return w;
@@ -163,11 +191,23 @@ TcWs tc_carve(const Geometry& g, bool backward, char* base) {
 
 } // namespace
 
+bool tc_plan_supported(int H, int W) { return H >= 1 && H <= HP && W >= 2 && W <= WP && W / 2 + 1 <= BS; }
+
 bool tc_supported(const Geometry& g) {
-  return g.bf16 && g.bs == BS && g.hid == BS && g.H <= HP && g.W <= WP && g.Wh <= BS && g.C % 8 == 0;
+  return g.bf16 && g.bs == BS && g.hid == BS && tc_plan_supported(g.H, g.W) && g.C % 8 == 0;
+}
+
+void tc_free_plan(TcPlan* p) {
+  uint8_t** tabs[] = {&p->dft2, &p->fw, &p->fw_alpha, &p->gw, &p->gw_noalpha};
+  for (uint8_t** t : tabs) {
+    cudaFree(*t);
+    *t = nullptr;
+  }
+  p->valid = false;
 }
 
 cudaError_t tc_build_plan(int H, int W, TcPlan* out) {
+  if (!tc_plan_supported(H, W)) return cudaErrorInvalidValue;   // the images below are sized for H <= 96, W/2+1 <= 96
   const double two_pi = 6.283185307179586476925286766559;
   const int Wh = W / 2 + 1;
   // Ch, Sh: element (r, h) = cos / sin (2 pi r h / H) / sqrt(H); K-major, 96 rows stored, order [k/8][m/8 < 12]
@@ -253,7 +293,6 @@ size_t tc_workspace_bytes(const Geometry& g, bool backward) {
 // prologue (barrier init, tensor-memory allocation, plan constants) under the tail of the previous kernel
 // of the stream; the kernels order themselves with pdl_wait().  The first kernel of an API call is a
 // plain launch, so the call as a whole keeps stream order with the caller's work.
-static const bool g_use_pdl = getenv("AFNO_NO_PDL") == nullptr;
 template <typename... KArgs, typename... Args>
 static cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool dependent,
                             Args&&... args) {
@@ -266,7 +305,7 @@ static cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, siz
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at;
-  cfg.numAttrs = (dependent && g_use_pdl) ? 1 : 0;
+  cfg.numAttrs = dependent ? 1 : 0;
   return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
@@ -299,38 +338,66 @@ static cudaError_t launch_wdft_inv(const Geometry& g, const TcPlan& tp, const vo
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
+// context header written by the SAVE_CONTEXT forward / checked by the USE_CONTEXT backward
+static CtxHeader make_header(const Geometry& g, const TcWs& w) {
+  CtxHeader h{};
+  h.magic = kCtxMagic;
+  h.B = g.B; h.H = g.H; h.W = g.W; h.C = g.C; h.nb = g.nb; h.Kh = g.Kh; h.Kw = g.Kw; h.chunk_b = w.chunk_b;
+  memcpy(&h.lambda_bits, &g.lambda, 4);
+  h.export_masks = g.export_masks ? 1u : 0u;
+  return h;
+}
+
+// sub-geometry of the samples [b0, b0 + n) and the byte offset of sample b0 in an activation tensor
+static Geometry chunk_geometry(const Geometry& g, int n) {
+  Geometry c = g;
+  c.B = n;
+  return c;
+}
+static size_t act_offset(const Geometry& g, int b0) { return (size_t)b0 * g.H * g.W * g.C * 2; }
+
 cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const float* w1, const float* b1,
                        const float* w2, const float* b2, void* y, void* ws, cudaStream_t st) {
-  // SAVE_CONTEXT: the backward layout, so that tc_backward finds A1 where it expects it
+  // SAVE_CONTEXT: the backward layout, so that tc_backward finds the context where it expects it
   TcWs w = tc_carve(g, g.save_ctx, (char*)ws);
   const TcPlan& tp = p.tc;
   cudaError_t e;
   const int nW = g.nb * BS * BS;
+  const CtxHeader hdr = g.save_ctx ? make_header(g, w) : CtxHeader{};
   prof_begin("k_tc_prep_weights", st);
-  k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, w.wprep, w.bprep, g.nb);
+  k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, w.wprep, w.bprep, g.nb, hdr, w.header);
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  if ((e = launch_wdft_fwd(g, tp, x, w.A1, tp.fw, st, true)) != cudaSuccess) return e;
-  MixParams mp{};
-  if (!tile_tmap(tp, &mp.mapA1, w.A1, g)) return cudaErrorInvalidValue;
-  mp.mapA1g = mp.mapA1;
-  mp.A2 = w.A2; mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
-  mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
-  prof_begin("tc_mix_fwd", st);
-  const int S2 = mix2_split(g, tp);
-  if (g.save_ctx) {
-    // saved context: Xh, O1 (operands of tc_wgrad) and the activation masks stay in the workspace
-    mp.Xh = w.Xh; mp.O1 = w.O1; mp.maskbits = w.maskbits;
-    e = launch_k(tc_mix2<kMixFwdSave, false>, mix2_grid(g, tp, S2), kMix2Threads, kMix2Smem, st, true, mp, S2);
-  } else {
-    e = launch_k(tc_mix2<kMixFwd, false>, mix2_grid(g, tp, S2), kMix2Threads, kMix2Smem, st, true, mp, S2);
+  for (int b0 = 0; b0 < g.B; b0 += w.chunk_f) {
+    const Geometry gc = chunk_geometry(g, g.B - b0 < w.chunk_f ? g.B - b0 : w.chunk_f);
+    const char* xc = (const char*)x + act_offset(g, b0);
+    char* yc = (char*)y + act_offset(g, b0);
+    const size_t t0 = (size_t)b0 * g.Kw * g.nb;   // first (b, kw, block) tile of the chunk in whole-batch tensors
+    if ((e = launch_wdft_fwd(gc, tp, xc, w.A, tp.fw, st, true)) != cudaSuccess) return e;
+    MixParams mp{};
+    if (!tile_tmap(tp, &mp.mapA1, w.A, gc)) return cudaErrorInvalidValue;
+    mp.mapA1g = mp.mapA1;
+    mp.A2 = w.A; mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
+    mp.B = gc.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
+    prof_begin("tc_mix_fwd", st);
+    const int S2 = mix2_split(gc, tp);
+    if (g.save_ctx) {
+      // saved context: Xh, O1 (operands of tc_wgrad) and the activation masks stay in the workspace
+      mp.Xh = (__nv_bfloat16*)((char*)w.Xh + t0 * kTileBytes);
+      mp.O1 = (__nv_bfloat16*)((char*)w.O1 + t0 * kTileBytes);
+      mp.maskbits = w.maskbits + t0 * 12 * 32;
+      e = launch_k(tc_mix2<kMixFwdSave, false>, mix2_grid(gc, tp, S2), kMix2Threads, kMix2Smem, st, true, mp, S2);
+    } else {
+      e = launch_k(tc_mix2<kMixFwd, false>, mix2_grid(gc, tp, S2), kMix2Threads, kMix2Smem, st, true, mp, S2);
+    }
+    prof_end(st);
+    if (e != cudaSuccess) return e;
+    count_launch();
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if ((e = launch_wdft_inv(gc, tp, w.A, g.no_residual ? nullptr : xc, yc, tp.gw, st)) != cudaSuccess) return e;
   }
-  if (e != cudaSuccess) return e;
-  prof_end(st);
-  count_launch();
-  if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  return launch_wdft_inv(g, tp, w.A2, g.no_residual ? nullptr : x, y, tp.gw, st);
+  return cudaSuccess;
 }
 
 cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const void* dy, const float* w1,
@@ -354,63 +421,64 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   // USE_CONTEXT: the operand images of the weights written by the forward call are still in the
   // workspace (the context belongs to one set of parameters)
   if (!g.use_ctx) {
-    TC_LAUNCH("k_tc_prep_weights", k_tc_prep_weights, (nW + 255) / 256, 256, 0, st, dep, w1, b1, w2, b2, w.wprep, w.bprep, g.nb);
+    TC_LAUNCH("k_tc_prep_weights", k_tc_prep_weights, (nW + 255) / 256, 256, 0, st, dep, w1, b1, w2, b2, w.wprep, w.bprep, g.nb,
+              CtxHeader{}, (CtxHeader*)nullptr);
   }
-  // B1 (first half) and B2: W-direction spectra of x and of dy (alpha-weighted)
-  if (!g.use_ctx) {
-    if ((e = launch_wdft_fwd(g, tp, x, w.A1, tp.fw, st, dep)) != cudaSuccess) return e;
-    dep = true;
-  }
-  if ((e = launch_wdft_fwd(g, tp, dy, w.A1g, tp.fw_alpha, st, dep)) != cudaSuccess) return e;
-  dep = true;
-  MixParams mp{};
-  if (!tile_tmap(tp, &mp.mapA1, w.A1, g) || !tile_tmap(tp, &mp.mapA1g, w.A1g, g)) return cudaErrorInvalidValue;
-  mp.A2 = w.A2;
-  mp.Xh = w.Xh; mp.O1 = w.O1; mp.G2 = w.G2; mp.G1 = w.G1;
-  mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
-  mp.mask1 = g.export_masks ? w.mask1 : nullptr;
-  mp.mask2 = g.export_masks ? w.mask2 : nullptr;
-  mp.B = g.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
-  const int S2 = mix2_split(g, tp);
-  mp.maskbits = w.maskbits;
-  if (g.use_ctx) {
-    // gradient stages only: Xh, O1 and the masks were left in the workspace by the forward call
-    if (g.export_masks) {
-      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, true>, mix2_grid(g, tp, S2), kMix2Threads, kMix2Smem, st, dep, mp, S2);
-    } else {
-      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, false>, mix2_grid(g, tp, S2), kMix2Threads, kMix2Smem, st, dep, mp, S2);
+  const size_t mask1_sample = (size_t)g.H * g.Wh * g.CH * 2, mask2_sample = (size_t)g.H * g.Wh * g.C * 2;
+  for (int b0 = 0; b0 < g.B; b0 += w.chunk_b) {
+    const Geometry gc = chunk_geometry(g, g.B - b0 < w.chunk_b ? g.B - b0 : w.chunk_b);
+    const char* xc = (const char*)x + act_offset(g, b0);
+    const char* dyc = (const char*)dy + act_offset(g, b0);
+    char* dxc = (char*)dx + act_offset(g, b0);
+    const size_t t0 = (size_t)b0 * g.Kw * g.nb;
+    __nv_bfloat16* Xh = (__nv_bfloat16*)((char*)w.Xh + t0 * kTileBytes);
+    __nv_bfloat16* O1 = (__nv_bfloat16*)((char*)w.O1 + t0 * kTileBytes);
+    // B1 (first half) and B2: W-direction spectra of x and of dy (alpha-weighted)
+    if (!g.use_ctx) {
+      if ((e = launch_wdft_fwd(gc, tp, xc, w.Ax, tp.fw, st, dep)) != cudaSuccess) return e;
+      dep = true;
     }
-  } else if (g.export_masks) {
-    TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, true>, mix2_grid(g, tp, S2), kMix2Threads, kMix2Smem, st, dep, mp, S2);
-  } else {
-    TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, false>, mix2_grid(g, tp, S2), kMix2Threads, kMix2Smem, st, dep, mp, S2);
+    if ((e = launch_wdft_fwd(gc, tp, dyc, w.A, tp.fw_alpha, st, dep)) != cudaSuccess) return e;
+    dep = true;
+    MixParams mp{};
+    if (!tile_tmap(tp, &mp.mapA1, g.use_ctx ? w.A : w.Ax, gc) || !tile_tmap(tp, &mp.mapA1g, w.A, gc)) return cudaErrorInvalidValue;
+    mp.A2 = w.A;   // in place over the gradient's spectrum
+    mp.Xh = Xh; mp.O1 = O1; mp.G2 = w.G2; mp.G1 = w.G1;
+    mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
+    mp.mask1 = g.export_masks ? w.mask1 + (size_t)b0 * mask1_sample : nullptr;
+    mp.mask2 = g.export_masks ? w.mask2 + (size_t)b0 * mask2_sample : nullptr;
+    mp.B = gc.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
+    const int S2 = mix2_split(gc, tp);
+    mp.maskbits = w.maskbits + t0 * 12 * 32;
+    if (g.use_ctx) {
+      // gradient stages only: Xh, O1 and the masks were left in the workspace by the forward call
+      if (g.export_masks) {
+        TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, true>, mix2_grid(gc, tp, S2), kMix2Threads, kMix2Smem, st, dep, mp, S2);
+      } else {
+        TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwdCtx, false>, mix2_grid(gc, tp, S2), kMix2Threads, kMix2Smem, st, dep, mp, S2);
+      }
+    } else if (g.export_masks) {
+      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, true>, mix2_grid(gc, tp, S2), kMix2Threads, kMix2Smem, st, dep, mp, S2);
+    } else {
+      TC_LAUNCH("tc_mix_bwd", tc_mix2<kMixBwd, false>, mix2_grid(gc, tp, S2), kMix2Threads, kMix2Smem, st, dep, mp, S2);
+    }
+    // B4 / B6: parameter gradients of the chunk, added to the partial sums of the chunks before it
+    TC_LAUNCH("tc_wgrad", tc_wgrad, 2 * g.nb * w.S, 128, kWgSmem, st, dep, O1, w.G2, Xh, w.G1, w.part, gc.B * g.Kw, g.H, g.nb,
+              w.S, b0 > 0 ? 1 : 0);
+    // B8: dx = dy + irfft2(GX / alpha)
+    if ((e = launch_wdft_inv(gc, tp, w.A, g.no_residual ? nullptr : dyc, dxc, tp.gw_noalpha, st)) != cudaSuccess) return e;
   }
-  // B4 / B6: parameter gradients
   const int nred = nW + g.nb * BS;
-  TC_LAUNCH("tc_wgrad", tc_wgrad, 2 * g.nb * w.S, 128, kWgSmem, st, dep, w.O1, w.G2, w.Xh, w.G1, w.part, g.B * g.Kw, g.H,
-            g.nb, w.S);
   TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce, dim3((nred + 255) / 256, 2), 256, 0, st, dep, w.part, (float2*)dw2,
             (float2*)db2, (float2*)dw1, (float2*)db1, g.nb, w.S, g.accum ? 1 : 0);
+  if (g.use_ctx) {
+    // a context that does not belong to this call (other geometry, flags, never saved) poisons the results
+    const size_t n_act = (size_t)g.B * g.H * g.W * g.C;
+    TC_LAUNCH("k_tc_ctx_guard", k_tc_ctx_guard, 148, 256, 0, st, dep, (const CtxHeader*)w.header, make_header(g, w),
+              (uint16_t*)dx, n_act, dw1, dw2, (size_t)nW * 2, db1, db2, (size_t)g.nb * BS * 2);
+  }
 #undef TC_LAUNCH
-  // B8: dx = dy + irfft2(GX / alpha)
-  return launch_wdft_inv(g, tp, w.A2, g.no_residual ? nullptr : dy, dx, tp.gw_noalpha, st);
+  return cudaSuccess;
 }
-
-#ifdef AFNO_TRACE
-extern "C" int afno_trace_read(long long* out) {
-  return (int)cudaMemcpyFromSymbol(out, g_afno_trace, sizeof(long long) * 64 * 32);
-}
-#endif
-#ifdef AFNO_POLICY_EXPERIMENT
-extern "C" int afno_debug_set_policy(int mask) { return (int)cudaMemcpyToSymbol(g_polmask, &mask, sizeof(int)); }
-#endif
-#ifdef AFNO_TIMING
-extern "C" int afno_debug_read_span(long long* out) {
-  return (int)cudaMemcpyFromSymbol(out, g_afno_span, sizeof(long long) * 5 * 160 * 2);
-}
-extern "C" int afno_debug_read(long long* out) {
-  return (int)cudaMemcpyFromSymbol(out, g_afno_dbg, sizeof(long long) * 128);
-}
-#endif
 
 } // namespace afno

@@ -57,8 +57,6 @@ __global__ void __launch_bounds__(kW2Threads, 1)
 tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapA1,
              const uint32_t* __restrict__ Fimg, int ntiles, int nb, int H, int Kw) {
   extern __shared__ uint8_t smem_raw[];
-  TL(0);
-  SPAN(0, 0);
   __shared__ __align__(8) uint64_t full[kWfSlots], sfree[kWfSlots], accfull[2], accempty[2];
   __shared__ uint32_t tmem_slot;
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -84,14 +82,11 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
-  TL(1);
   load_const_tmem(tmem, Fimg, warp, lane);   // plan constant: loads under the previous kernel's tail
-  TL(2);
   pdl_wait();
-  TL(3);
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
-  const uint64_t pol_stream = pol_first(kPolWfLoad), pol_keep = pol_last(kPolWfStore);
+  const uint64_t pol_stream = pol(kPolWfLoadX), pol_keep = pol(kPolWfStoreA);
   // TMA producer (warp 7): tile it -> slot it % 6
   auto produce = [&](int it) {
     const int s = it % kWfSlots;
@@ -190,8 +185,6 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
   }
   tc_fence_before();
   __syncthreads();
-  TL(4);
-  SPAN(0, 1);
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
@@ -201,8 +194,6 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
              const __grid_constant__ CUtensorMap mapY, const uint32_t* __restrict__ Gimg, int ntiles, int nb, int H, int W,
              int has_res) {
   extern __shared__ uint8_t smem_raw[];
-  TL(8);
-  SPAN(1, 0);
   __shared__ __align__(8) uint64_t ofull[kWiSlots], ofree[kWiSlots], rfull[kWiSlots], rfree[kWiSlots], accfull[2], accempty[2];
   __shared__ uint32_t tmem_slot;
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -232,14 +223,11 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
-  TL(9);
   load_const_tmem(tmem, Gimg, warp, lane);   // plan constant: loads under the previous kernel's tail
-  TL(10);
   pdl_wait();
-  TL(11);
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
-  const uint64_t pol_stream = pol_first(kPolWiLoad), pol_out = pol_first(kPolWiStore);
+  const uint64_t pol_spec = pol(kPolWiLoadA), pol_res = pol(kPolWiLoadRes), pol_out = pol(kPolWiStoreY);
   // TMA producer (warp 6)
   auto produce = [&](int it) {
     const int s = it % kWiSlots;
@@ -250,13 +238,13 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
     mbar_expect_tx(&ofull[s], kW2Tile);
 #pragma unroll
     for (int pn = 0; pn < 6; ++pn)   // panel pn = ri * 3 + n -> K rows ri * 96.., N panel n
-      tma_load5(aO + s * kW2Tile + (pn % 3) * kPanel + (pn / 3) * (BS * 64), &mapA2, 0, pn, j * H + h, 0, b, &ofull[s], pol_stream);
+      tma_load5(aO + s * kW2Tile + (pn % 3) * kPanel + (pn / 3) * (BS * 64), &mapA2, 0, pn, j * H + h, 0, b, &ofull[s], pol_spec);
     if (has_res) {
       if (it >= kWiSlots) mbar_wait(&rfree[s], par);  // the slot's previous store has read it
       mbar_expect_tx(&rfull[s], kW2Tile);
 #pragma unroll
       for (int pn = 0; pn < 3; ++pn)
-        tma_load3(aR + s * kW2Tile + pn * kPanel, &mapRes, j * BS + pn * 32, 0, bh, &rfull[s], pol_stream);
+        tma_load3(aR + s * kW2Tile + pn * kPanel, &mapRes, j * BS + pn * 32, 0, bh, &rfull[s], pol_res);
     }
   };
   if (warp == 6) {
@@ -364,7 +352,5 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
   }
   tc_fence_before();
   __syncthreads();
-  TL(12);
-  SPAN(1, 1);
   if (warp == 0) tmem_dealloc<512>(tmem);
 }

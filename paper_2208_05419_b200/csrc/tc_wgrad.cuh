@@ -23,15 +23,20 @@ __device__ __forceinline__ void bulk_copy(uint32_t dst_smem, const void* src, ui
                : "memory");
 }
 
+// shared -> global bulk reduction (fp32 add), tracked by bulk groups
+__device__ __forceinline__ void bulk_reduce_add_f32(void* dst, uint32_t src_smem, uint32_t bytes) {
+  asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;" ::"l"(dst), "r"(src_smem), "r"(bytes)
+               : "memory");
+  bulk_commit();
+}
+
 // Operand-image tensors written by tc_mix2<true> ([tile][24 chunks][kTileSbo bytes]).  ONE launch covers
 // both layers: CTAs [0, nb*S) form layer 2 (A = O1, G = G2), CTAs [nb*S, 2*nb*S) layer 1 (A = Xh, G = G1).
 __global__ void __launch_bounds__(128, 1)
 tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict__ G_l2,
          const __nv_bfloat16* __restrict__ A_l1, const __nv_bfloat16* __restrict__ G_l1, float* __restrict__ part,
-         int BKw, int H, int nb, int S) {
+         int BKw, int H, int nb, int S, int accumulate) {
   extern __shared__ __align__(1024) uint8_t smem[];
-  TL(32);
-  SPAN(4, 0);
   __shared__ __align__(8) uint64_t full[2], empty[2], done;
   __shared__ uint32_t tmem_slot;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -60,9 +65,7 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  TL(33);
   pdl_wait();
-  TL(34);
   const uint32_t tmem = tmem_slot;
   const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
   const uint32_t Dre = tmem, Dim = tmem + 256;
@@ -72,16 +75,16 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
   if (warp == 0 && elect_one()) {
     // ---- producer: three bulk copies per tile (A re half, A im half, G), async proxy, no LSU ----
     constexpr uint32_t kHalfImg = 12 * kTileSbo;
-    const uint64_t pol_stream = pol_first(kPolWgLoad);
+    const uint64_t pol_ctx = pol(kPolWgLoadCtx), pol_g = pol(kPolWgLoadG);
     for (int it = 0; it < nt; ++it) {
       const int b = it & 1, use = it >> 1;
       if (use > 0) mbar_wait(&empty[b], (uint32_t)((use - 1) & 1));
       const size_t off = ((size_t)(s + it * S) * nb + j) * kTileBytes;
       const uint32_t stage = smem_u32(smem) + b * kWgStage;
       mbar_expect_tx(&full[b], 2 * kHalfImg + kTileBytes);
-      bulk_copy(stage, (const uint8_t*)Aws + off, kHalfImg, &full[b], pol_stream);
-      bulk_copy(stage + kWgABytes, (const uint8_t*)Aws + off + kHalfImg, kHalfImg, &full[b], pol_stream);
-      bulk_copy(stage + 2 * kWgABytes, (const uint8_t*)Gws + off, kTileBytes, &full[b], pol_stream);
+      bulk_copy(stage, (const uint8_t*)Aws + off, kHalfImg, &full[b], pol_ctx);
+      bulk_copy(stage + kWgABytes, (const uint8_t*)Aws + off + kHalfImg, kHalfImg, &full[b], pol_ctx);
+      bulk_copy(stage + 2 * kWgABytes, (const uint8_t*)Gws + off, kTileBytes, &full[b], pol_g);
     }
   } else if (warp == 1 && elect_one()) {
     // ---- MMA issuer ----
@@ -107,7 +110,6 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
   float* stage = (float*)smem;
   if (nt > 0) {
     mbar_wait(&done, 0u);
-    TL(35);
     tc_fence_after();
 #pragma unroll 1
     for (int acc = 0; acc < 2; ++acc) {
@@ -134,13 +136,14 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
   fence_async_smem();
   __syncthreads();
   if (tid == 0) {
-    bulk_store(part + (size_t)blockIdx.x * kWgPartFloats, smem_u32(smem), kWgPartFloats * 4, l2_evict_normal());
+    // the first chunk of a call stores its partial sums, every later chunk adds to them (one CTA per
+    // slot, launches in stream order: the summation order is fixed)
+    if (accumulate) bulk_reduce_add_f32(part + (size_t)blockIdx.x * kWgPartFloats, smem_u32(smem), kWgPartFloats * 4);
+    else bulk_store(part + (size_t)blockIdx.x * kWgPartFloats, smem_u32(smem), kWgPartFloats * 4, l2_evict_normal());
     bulk_wait<0>();
   }
   tc_fence_before();
   __syncthreads();
-  TL(36);
-  SPAN(4, 1);
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 

@@ -43,8 +43,17 @@ def _peaks():
                 source="fallback")
 
 
+def kept_counts(wl):
+    f = float(np.float32(wl.kept_fraction))
+    Kh = max(1, min(wl.H // 2 + 1, int(np.floor(f * (wl.H // 2 + 1)))))
+    Kw = max(1, min(wl.W // 2 + 1, int(np.floor(f * (wl.W // 2 + 1)))))
+    rows = 2 * Kh - 1 if Kh <= wl.H // 2 else wl.H
+    return Kh, Kw, rows * Kw
+
+
 def layer_work(B, H, W, C, nb, kept_modes, ctx=True):
-    """Algorithmic work of one fwd+bwd step (S5): compulsory HBM bytes and model MLP FLOPs."""
+    """Algorithmic work of one fwd+bwd step (S5.4): COMPULSORY HBM bytes (the five
+    activation tensors x, y, x again, dy, dx and the parameters / gradients) and MODEL MLP FLOPs."""
     act = B * H * W * C * 2                                  # one bf16 activation tensor
     params = 2 * (nb * (C // nb) ** 2 * 2 + C * 2) * 4       # w1,b1,w2,b2 fp32
     bytes_fwd = 2 * act + params                             # x in, y out
@@ -53,9 +62,35 @@ def layer_work(B, H, W, C, nb, kept_modes, ctx=True):
     gemm = 2 * (2 * bs) * (2 * bs) * nb * kept_modes * B     # one complex block GEMM over all modes
     flops_fwd = 2 * gemm                                     # F3, F5
     flops_bwd_model = 4 * gemm                               # B4, B5, B6, B7
-    flops_bwd_exec = (4 if ctx else 6) * gemm                # stateless bwd: + recompute of F3, F5
-    return dict(bytes=bytes_fwd + bytes_bwd, flops_model=flops_fwd + flops_bwd_model,
-                flops_exec=flops_fwd + flops_bwd_exec)
+    return dict(bytes=bytes_fwd + bytes_bwd, flops_model=flops_fwd + flops_bwd_model, gemm=gemm, act=act,
+                params=params)
+
+
+def executed_tensor_flops(B, wl, Kw, ctx=True):
+    """Tensor FLOPs the tcgen05 path EXECUTES per step, counted from the UMMA instructions the kernels issue
+    (S5.3): every transform is a dense DFT GEMM and M is padded to 128."""
+    umma96, umma192 = 2.0 * 128 * 96 * 16, 2.0 * 128 * 192 * 16
+    t_mode = B * Kw * wl.num_blocks                          # (b, kw, block) tiles of tc_mix2 / tc_wgrad
+    t_row = B * wl.H * wl.num_blocks                         # (b, h, block) tiles of the W-direction kernels
+    mix_fwd = 96 * umma96 * t_mode                           # H-DFT 24 + layer 1 24 + layer 2 24 + inverse H-DFT 24
+    mix_bwd = (96 if ctx else 168) * umma96 * t_mode
+    wdft = 24 * umma96 * t_row                               # one launch; fwd has 2 (x -> A, A -> y), bwd 2 (+1 stateless)
+    wgrad = 2 * 12 * umma192 * t_mode
+    n_w = 4 if ctx else 5
+    return dict(total=mix_fwd + mix_bwd + n_w * wdft + wgrad, tc_mix_fwd=mix_fwd, tc_mix_bwd=mix_bwd,
+                tc_wdft_per_launch=wdft, tc_wgrad=wgrad)
+
+
+def fft_flops_per_step(B, wl):
+    """fp32 butterfly FLOPs a mixed-radix FFT implementation of the five 2-D transforms would execute
+    (SURVEY.md S8(d) estimate: r2/r3/r5 butterflies 4/16/44 real FLOPs + 6 per non-trivial twiddle;
+    cfft(90) ~ 3,084, cfft(180) ~ 7,068, rfft(W) = cfft(W/2) + 10 W/2); None for other grids."""
+    cfft = {45: 1300.0, 90: 3084.0, 180: 7068.0}
+    if wl.H not in cfft or wl.W // 2 not in cfft:
+        return None
+    rfft_w = cfft[wl.W // 2] + 10.0 * (wl.W // 2)
+    per_channel = wl.H * rfft_w + (wl.W // 2 + 1) * cfft[wl.H]
+    return 5.0 * per_channel * wl.C * B
 
 
 class ClockSampler:
@@ -150,7 +185,7 @@ def run_reference(args):
     from paper_2208_05419_b200 import inputs
     wl = inputs.WORKLOADS[WL_NAME]
     steps = max(1, args.steps)
-    for _ in range(min(args.warmup, 1)):
+    for _ in range(args.warmup):
         oracle_time(1)
     tot_s, tot_t, cores = 0, 0.0, 0
     for _ in range(steps):
@@ -160,7 +195,7 @@ def run_reference(args):
     value = tot_s / tot_t
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * tot_t / steps,
+        "steps": steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": f"BASELINE.json configs[4]: {wl.name}; one sample per step (bounded sample)",
@@ -199,9 +234,9 @@ def run_ours(args):
     path = binding.afno_spectral_path(desc)
     peaks = _peaks()
 
-    # --- inputs resident in HBM; rotate NSETS disjoint buffer sets so reads are cold -------
+    # --- inputs resident in HBM; rotate NSETS disjoint buffer sets (1.6 GB >> 126 MB L2) so reads are cold ----
     data = inputs.make_inputs(wl)
-    NSETS = 3
+    NSETS = 4
     dev = torch.device("cuda", local_rank)
     to_bf16 = lambda a: torch.from_numpy(a).to(dev).to(torch.bfloat16)
     x0, dy0 = to_bf16(data["x"]), to_bf16(data["dy"])
@@ -217,17 +252,17 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     launches = [0]
 
-    # a training step: fwd keeps the W-direction spectrum of x in the workspace, bwd reads it
+    # a training step: fwd leaves Xh, O1 and the activation masks in the workspace, bwd reads them
     # (SURVEY.md S8(a) row B1 "or load saved context"); --stateless times the recomputing bwd
     ctx = not args.stateless
     desc_f = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_SAVE_CONTEXT}) if ctx else desc
     desc_b = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_USE_CONTEXT}) if ctx else desc
 
-    def step(i):
+    def step(i, st=stream):
         s = sets[i % NSETS]
-        binding.afno_spectral_fwd(desc_f, s["x"], *params, s["y"], ws_b if ctx else ws_f, stream)
+        binding.afno_spectral_fwd(desc_f, s["x"], *params, s["y"], ws_b if ctx else ws_f, st)
         n = binding.afno_last_launch_count()
-        binding.afno_spectral_bwd(desc_b, s["x"], s["dy"], *params, s["dx"], *grads, ws_b, stream)
+        binding.afno_spectral_bwd(desc_b, s["x"], s["dy"], *params, s["dx"], *grads, ws_b, st)
         launches[0] = n + binding.afno_last_launch_count()
 
     def barrier():
@@ -239,50 +274,110 @@ def run_ours(args):
     for i in range(args.warmup):
         step(i)
     barrier()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # EXACTLY args.steps steps between two events; an event after every step gives the per-step spread
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     with ClockSampler(local_rank) as clocks:
-        ev0.record(stream)
+        evs[0].record(stream)
         for i in range(args.steps):
             step(i)
-        ev1.record(stream)
+            evs[i + 1].record(stream)
         barrier()
-    ms = max_over_ranks(ev0.elapsed_time(ev1), dist, dev)
+    ms = max_over_ranks(evs[0].elapsed_time(evs[-1]), dist, dev)
+    per_step = np.array([evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)])
     ms_per_step = ms / args.steps
     value = whole_job_value(world, B, args.steps, ms)
 
+    # --- the same step captured in CUDA graphs, one graph per buffer set: reported beside ---
+    graph_info = None
+    try:
+        gs = torch.cuda.Stream()
+        graphs = []
+        with torch.cuda.stream(gs):
+            for k in range(NSETS):
+                gk = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(gk, stream=gs):
+                    step(k, gs)
+                graphs.append(gk)
+            for k in range(NSETS):
+                graphs[k].replay()
+            torch.cuda.synchronize()
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record(gs)
+            for i in range(args.steps):
+                graphs[i % NSETS].replay()
+            g1.record(gs)
+            torch.cuda.synchronize()
+        gms = g0.elapsed_time(g1) / args.steps
+        graph_info = {"ms_per_step": gms, "value": B / (gms * 1e-3), "unit": UNIT,
+                      "note": "fwd+bwd captured once per buffer set and replayed (reported, not the headline)"}
+    except Exception as ex:  # capture is an extra: never lose the bench line to it
+        graph_info = {"error": str(ex)[:200]}
+    torch.cuda.synchronize()
+
     # --- per-kernel durations, measured live with CUDA events around every launch -----------
+    # (the events sit between the kernels of a call and so disable the programmatic-dependent-launch overlap:
+    #  the per-kernel times add up to more than ms_per_step; their SHARES are what the roofline uses)
     binding.afno_profile_start()
     PROF_STEPS = max(2, min(args.steps, 5))
     for i in range(PROF_STEPS):
         step(i)
     prof = binding.afno_profile_stop()
     total_prof_ms = sum(v[1] for v in prof.values())
-    dom = max(prof, key=lambda k: prof[k][1])
-    dom_n, dom_ms = prof[dom]
-    kept_modes = None
-    Kh = max(1, min(wl.H // 2 + 1, int(np.floor(float(np.float32(wl.kept_fraction)) * (wl.H // 2 + 1)))))
-    Kw = max(1, min(wl.W // 2 + 1, int(np.floor(float(np.float32(wl.kept_fraction)) * (wl.W // 2 + 1)))))
-    kept_modes = (2 * Kh - 1 if Kh <= wl.H // 2 else wl.H) * Kw
+    Kh, Kw, kept_modes = kept_counts(wl)
     work = layer_work(B, wl.H, wl.W, wl.C, wl.num_blocks, kept_modes, ctx)
-    roofline = kernel_roofline(dom, dom_n, dom_ms, PROF_STEPS, work, peaks, clocks.summary(), B, wl, kept_modes, ctx)
-    roofline["share_of_step"] = dom_ms / total_prof_ms if total_prof_ms > 0 else None
-    roofline["kernels_ms_per_step"] = {k: round(v[1] / PROF_STEPS, 4) for k, v in sorted(prof.items())}
+    exe = executed_tensor_flops(B, wl, Kw, ctx)
+    traffic = TrafficTable()
+    clk = clocks.summary()
     per_kernel = {}
     for k, (n, ms_k) in sorted(prof.items()):
-        r = kernel_roofline(k, n, ms_k, PROF_STEPS, work, peaks, clocks.summary(), B, wl, kept_modes, ctx)
-        per_kernel[k] = {"bound": r["bound"], "frac": r["frac"], "avg_launch_us": round(r["avg_launch_us"], 2)}
-    roofline["per_kernel"] = per_kernel
+        per_kernel[k] = kernel_roofline(k, n, ms_k, PROF_STEPS, work, exe, peaks, traffic, total_prof_ms)
+    dom = max(prof, key=lambda k: prof[k][1])
 
-    # --- whole-layer 2-term roofline of BASELINE.json's metric ---------------------------------
+    # --- whole-layer roofline of BASELINE.json's metric: the headline fraction -----------
+    t_step = ms_per_step * 1e-3
     t_hbm = work["bytes"] / (peaks["hbm_gbs"] * 1e9)
     t_tensor = work["flops_model"] / (peaks["tensor_tflops"] * 1e12)
+    t_tensor_sus = work["flops_model"] / (peaks["tensor_tflops_sustained"] * 1e12)
+    fp32_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6
+    fft = fft_flops_per_step(B, wl)
+    t_fft = fft / fp32_peak if fft else None
     t_roof = max(t_hbm, t_tensor)
-    layer = {"bound": "hbm" if t_hbm >= t_tensor else "tensor", "t_roof_us_per_step": 1e6 * t_roof,
-             "frac": t_roof / (ms_per_step * 1e-3), "bytes_per_step": work["bytes"],
-             "mlp_flops_model_per_step": work["flops_model"], "mlp_flops_executed_per_step": work["flops_exec"],
-             "achieved_tbs": work["bytes"] / (ms_per_step * 1e-3) / 1e12,
-             "achieved_tflops_model": work["flops_model"] / (ms_per_step * 1e-3) / 1e12,
-             "peaks": f"{peaks['hbm_gbs']} GB/s, {peaks['tensor_tflops']} TFLOP/s bf16 burst ({peaks['source']})"}
+    step_traffic = traffic.step_total(prof, PROF_STEPS)
+    roofline = {
+        "scope": "layer: all launches of one fwd+bwd step (SURVEY.md S8(d) contractual 2-term roofline)",
+        "bound": "hbm" if t_hbm >= t_tensor else "tensor",
+        "achieved": work["bytes"] / t_step / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+        "frac": t_roof / t_step,
+        "algorithmic_bytes_per_step": work["bytes"],
+        "traffic": step_traffic,
+        "traffic_ratio": (step_traffic / work["bytes"]) if step_traffic else None,
+        "traffic_source": traffic.source,
+        "t_roof_us_per_step": 1e6 * t_roof,
+        "peaks": f"{peaks['hbm_gbs']} GB/s copy, {peaks['tensor_tflops']} TFLOP/s bf16 burst, "
+                 f"{peaks['tensor_tflops_sustained']} sustained ({peaks['source']}, MEASURED_PEAKS.json)",
+        "variants": {
+            "two_term_burst": {"t_hbm_us": 1e6 * t_hbm, "t_tensor_us": 1e6 * t_tensor, "frac": max(t_hbm, t_tensor) / t_step},
+            "two_term_sustained_tensor": {"t_tensor_us": 1e6 * t_tensor_sus, "frac": max(t_hbm, t_tensor_sus) / t_step},
+            "three_term_with_fp32_fft": ({"t_fft_us": 1e6 * t_fft, "fp32_peak_tflops": fp32_peak / 1e12, "fft_flops": fft,
+                                          "frac": max(t_hbm, t_tensor, t_fft) / t_step,
+                                          "note": "bound of a plain fp32-ALU mixed-radix FFT design (SURVEY.md S0 finding 3); "
+                                                  "this path runs its transforms on the tensor cores instead"} if t_fft else None),
+            "executed_tensor_floor": {"t_us": 1e6 * exe["total"] / (peaks["tensor_tflops"] * 1e12),
+                                      "note": "tensor FLOPs the kernels execute (dense DFT GEMMs, M padded to 128) at the burst peak"},
+        },
+        "mlp_flops_model_per_step": work["flops_model"],
+        "tensor_flops_executed_per_step": exe["total"],
+        "executed_over_model": exe["total"] / work["flops_model"],
+        "achieved_tbs": work["bytes"] / t_step / 1e12,
+        "achieved_tflops_model": work["flops_model"] / t_step / 1e12,
+        "achieved_tflops_executed": exe["total"] / t_step / 1e12,
+        "dominant_kernel": dict(per_kernel[dom], kernel=dom),
+        "kernels_ms_per_step": {k: round(v[1] / PROF_STEPS, 4) for k, v in sorted(prof.items())},
+        "per_kernel": per_kernel,
+        "per_kernel_note": "CUDA events around every launch (afno_profile_*): no PDL overlap between kernels, so the sum "
+                           "exceeds ms_per_step; algorithmic bytes = COMPULSORY bytes of the launch only (activations in / "
+                           "out, parameters), intermediates (half-spectra, saved context, operand images) are traffic",
+    }
 
     # --- end to end through the C ABI with HOST buffers -----------------------------------------
     e2e = None
@@ -324,14 +419,15 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "ms_per_step_median": float(np.median(per_step)), "ms_per_step_best": float(per_step.min()),
             "config": {"workload": f"BASELINE.json configs[4]: {wl.name}", "B_per_gpu": B, "H": wl.H, "W": wl.W,
                        "C": wl.C, "num_blocks": wl.num_blocks, "lambda": wl.lam, "kept_fraction": wl.kept_fraction,
                        "path": path, "backward": "saved context (fwd keeps Xh, O1 and the activation masks; bwd runs the gradient stages only)" if ctx
                        else "stateless (recomputes the spectrum of x)", "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": f"{NSETS} rotating input/output buffer sets of {4 * x0.numel() * 2 / 1e6:.0f} MB "
                              "each (> 126 MB L2), no explicit flush"},
-            "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches[0] * args.steps,
-            "roofline": roofline, "layer_roofline": layer, "cpu_baseline": cpu_baseline,
+            "clocks": clk, "e2e": e2e, "gpu_launches": launches[0] * args.steps,
+            "roofline": roofline, "cuda_graph": graph_info, "cpu_baseline": cpu_baseline,
         }
         print(json.dumps(line))
     if dist is not None:
@@ -339,78 +435,99 @@ def run_ours(args):
     return 0
 
 
-def kernel_work(name, B, wl, kept_modes, ctx=True):
-    """Algorithmic work of ONE launch of a kernel (S5 states these figures).
+class TrafficTable:
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture of this build
+    (profiles/r2_dram_traffic.csv: '# git <hash>' header, then kernel,bytes_per_launch).  A stored capture, not a
+    live measurement: `source` names the file and the commit it was taken on."""
 
-    bytes: compulsory HBM traffic of the launch (activations bf16, spectra bf16-complex);
-    flops: model FLOPs of the complex block GEMMs it evaluates (8 per complex MAC, padding and
-    the DFT-as-GEMM arithmetic are NOT counted)."""
-    Kw = kept_modes // wl.H if kept_modes % wl.H == 0 else wl.W // 2 + 1
-    bs = wl.C // wl.num_blocks
-    act = B * wl.H * wl.W * wl.C * 2                       # one bf16 activation tensor
-    spec = B * Kw * wl.num_blocks * wl.H * 2 * bs * 2      # one bf16-complex half-spectrum
-    gemm = 2.0 * (2 * bs) * (2 * bs) * wl.num_blocks * kept_modes * B
-    masks = B * Kw * wl.num_blocks * 12 * 32 * 16          # bit-packed activation masks of the saved context
+    def __init__(self):
+        self.rows, self.source = {}, None
+        path = os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")
+        try:
+            git = "unknown"
+            for line in open(path).read().splitlines():
+                if line.startswith("#"):
+                    if "git" in line:
+                        git = line.split("git", 1)[1].strip()
+                    continue
+                k, v = line.split(",")[:2]
+                if k != "kernel":
+                    self.rows[k] = int(float(v))
+            self.source = f"profiles/r2_dram_traffic.csv (ncu capture of commit {git}; stored, not measured by this run)"
+        except Exception as ex:
+            self.source = f"unavailable: {ex}"
+
+    def get(self, name):
+        if name not in self.rows:
+            if self.rows:
+                sys.stderr.write(f"bench.py: profiles/r2_dram_traffic.csv has no row for kernel {name!r}\n")
+            return None
+        return self.rows[name]
+
+    def step_total(self, prof, steps):
+        tot = 0
+        for k, (n, _) in prof.items():
+            t = self.get(k)
+            if t is None:
+                if k.startswith("tc_"):
+                    return None
+                continue
+            tot += t * n / steps
+        return int(tot) if tot else None
+
+
+def kernel_work(name, work, exe):
+    """Algorithmic work of ONE launch: COMPULSORY HBM bytes only (activations into / out of
+    the launch and parameters; half-spectra, saved context and operand images are intermediates) and the
+    model FLOPs of the complex block GEMMs it evaluates (8 per complex MAC; padding and DFT-as-GEMM excluded)."""
+    act, params, gemm = work["act"], work["params"], work["gemm"]
     table = {
-        "tc_wdft_fwd": dict(bound="hbm", bytes=act + spec, flops=0.0),
-        "tc_wdft_inv": dict(bound="hbm", bytes=spec + 2 * act, flops=0.0),
-        # saved-context step: fwd also writes Xh, O1 and 18 MB of mask bits; bwd runs the gradient stages only
-        "tc_mix_fwd": dict(bound="tensor", bytes=(4 * spec + masks) if ctx else 2 * spec, flops=2 * gemm),
-        "tc_mix_bwd": dict(bound="tensor", bytes=(4 * spec + masks) if ctx else 7 * spec, flops=(2 if ctx else 4) * gemm),
-        "tc_wgrad": dict(bound="hbm", bytes=4 * spec, flops=2 * gemm),   # one launch, both layers
-        "k_block_gemm": dict(bound="alu", bytes=0, flops=gemm),
-        "k_block_wgrad": dict(bound="alu", bytes=0, flops=gemm),
+        "tc_wdft_fwd": dict(bound="hbm", bytes=act, flops=0.0, executed=exe["tc_wdft_per_launch"]),
+        "tc_wdft_inv": dict(bound="hbm", bytes=2 * act, flops=0.0, executed=exe["tc_wdft_per_launch"]),   # residual in, y / dx out
+        "tc_mix_fwd": dict(bound="tensor", bytes=params, flops=2 * gemm, executed=exe["tc_mix_fwd"]),
+        "tc_mix_bwd": dict(bound="tensor", bytes=params, flops=2 * gemm, executed=exe["tc_mix_bwd"]),
+        "tc_wgrad": dict(bound="tensor", bytes=params, flops=2 * gemm, executed=exe["tc_wgrad"]),
+        "k_block_gemm": dict(bound="alu", bytes=0, flops=gemm, executed=0.0),
+        "k_block_wgrad": dict(bound="alu", bytes=0, flops=gemm, executed=0.0),
     }
     return table.get(name)
 
 
-def measured_traffic(name):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture."""
-    path = os.path.join(ROOT, "profiles", "r1e_dram_traffic.csv")
-    try:
-        for line in open(path).read().splitlines()[1:]:
-            k, v = line.split(",")
-            if k == name:
-                return int(v)
-    except Exception:
-        pass
-    return None
-
-
-def kernel_roofline(name, n_launch, total_ms, steps, work, peaks, clocks, B, wl, kept_modes, ctx=True):
-    """roofline object for the dominant kernel: achieved = algorithmic work of one launch / its
-    average duration measured with CUDA events around every launch (afno_profile_*)."""
+def kernel_roofline(name, n_launch, total_ms, steps, work, exe, peaks, traffic, total_prof_ms):
+    """Per-kernel roofline entry: achieved = algorithmic work of one launch / its average duration measured with
+    CUDA events around every launch (afno_profile_*); traffic = stored ncu DRAM bytes per launch."""
     per_launch_s = total_ms * 1e-3 / n_launch
-    kw = kernel_work(name, B, wl, kept_modes, ctx)
-    out = {"kernel": name, "launches_per_step": n_launch / steps, "avg_launch_us": per_launch_s * 1e6,
-           "traffic": measured_traffic(name)}
+    kw = kernel_work(name, work, exe)
+    tr = traffic.get(name)
+    out = {"launches_per_step": n_launch / steps, "avg_launch_us": round(per_launch_s * 1e6, 2),
+           "share_of_step": total_ms / total_prof_ms if total_prof_ms > 0 else None, "traffic": tr}
     if kw is None:
-        out.update({"bound": "hbm", "achieved": None, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": None})
+        out.update({"bound": None, "frac": None})
         return out
+    out["algorithmic_bytes"] = kw["bytes"]
+    out["traffic_ratio"] = (tr / kw["bytes"]) if tr and kw["bytes"] else None
+    out["dram_gbs_from_traffic"] = (tr / per_launch_s / 1e9) if tr else None
     if kw["bound"] == "tensor":
         ach = kw["flops"] / per_launch_s / 1e12
         out.update({"bound": "tensor", "achieved": ach, "peak": peaks["tensor_tflops"], "unit": "TFLOP/s",
-                    "frac": ach / peaks["tensor_tflops"], "algorithmic_flops_per_launch": kw["flops"],
-                    "algorithmic_bytes_per_launch": kw["bytes"],
-                    "hbm_frac": kw["bytes"] / per_launch_s / 1e9 / peaks["hbm_gbs"],
-                    "note": "peak = measured bf16 burst (MEASURED_PEAKS.json); SM clock stays at max in this 1 ms step"})
+                    "frac": ach / peaks["tensor_tflops"], "algorithmic_flops": kw["flops"],
+                    "executed_flops": kw["executed"], "executed_tflops": kw["executed"] / per_launch_s / 1e12})
     elif kw["bound"] == "hbm":
         ach = kw["bytes"] / per_launch_s / 1e9
         out.update({"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                    "frac": ach / peaks["hbm_gbs"], "algorithmic_bytes_per_launch": kw["bytes"]})
+                    "frac": ach / peaks["hbm_gbs"], "executed_flops": kw["executed"]})
     else:
         peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
         ach = kw["flops"] / per_launch_s / 1e12
-        out.update({"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
-                    "note": "fp32 FFMA peak = 148 SM x 128 lanes x 2 x max SM clock (DESIGN.md S5)"})
+        out.update({"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak})
     return out
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--stateless", action="store_true",

@@ -65,7 +65,12 @@ enum {
    * descriptor (the two context flags aside), the same x and the same parameter values, reads
    * them instead of recomputing rows B1 (F1-F5) and is bit-identical to the stateless bwd.
    * Nothing else may write the workspace in between.  Kernel families that keep no such
-   * intermediate (generic-fp32) accept both flags and recompute. */
+   * intermediate (generic-fp32) accept both flags and recompute.  SAVE_CONTEXT is a flag of fwd,
+   * USE_CONTEXT of bwd (the other call, or both at once: AFNO_ERR_INVALID_ARG).  fwd records what it
+   * saved (geometry, lambda, chunking, EXPORT_MASKS, which moves the layout) in a header; a bwd
+   * whose descriptor does not match it, or a workspace that was never saved, yields dx and
+   * gradients that are all NaN instead of plausible numbers.  Other parameter VALUES than the
+   * ones saved with cannot be detected. */
   AFNO_FLAG_SAVE_CONTEXT = 16,
   AFNO_FLAG_USE_CONTEXT = 32
 };
@@ -104,6 +109,10 @@ int afno_spectral_mask_bytes(const afno_desc_t* d, size_t* mask1_bytes, size_t* 
  * implicitly on first use when the stream is not capturing. */
 int afno_plan_warmup(const afno_desc_t* d);
 
+/* Frees every plan this process has built (all devices).  No call of this library may be in
+ * flight; the next fwd / bwd / afno_plan_warmup rebuilds what it needs. */
+int afno_plan_destroy_all(void);
+
 /* Forward.  x, y: [B][H][W][C] of d->dtype; y must not alias x.
  * w1 [nb][bs][hid][2], b1 [nb][hid][2], w2 [nb][hid][bs][2], b2 [nb][bs][2]: fp32,
  * out[o] = sum_i in[i] * w[j][i][o] (row vector times matrix), (re, im) fastest. */
@@ -128,7 +137,11 @@ int afno_spectral_bwd(const afno_desc_t* d, const void* x, const void* dy, const
  * copy stream while sample b computes on `cuda_stream` and sample b-1 is copied out on a
  * second internal stream; y and dx equal the device path's bit for bit, the parameter
  * gradients are the in-order sum of the per-sample gradients (fp32 summation order differs
- * from one batched call).  The context flags and EXPORT_MASKS have no meaning here. */
+ * from one batched call).  The context flags and EXPORT_MASKS have no meaning here.
+ * afno_spectral_bwd_host accepts x_host == NULL: x is then taken from the arena, where the
+ * afno_spectral_fwd_host call that preceded it on the SAME arena and descriptor left it (a
+ * training step uploads x once).  On an error the calls first wait for the copies and
+ * kernels they have already enqueued, so the caller may free its buffers at once. */
 size_t afno_spectral_host_arena_bytes(const afno_desc_t* d, int for_backward);
 int afno_spectral_fwd_host(const afno_desc_t* d, const void* x_host, const float* w1_host,
                            const float* b1_host, const float* w2_host, const float* b2_host,

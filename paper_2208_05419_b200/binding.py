@@ -24,7 +24,7 @@ EXPORTS = [
     "afno_spectral_workspace_bytes", "afno_spectral_mask_bytes", "afno_plan_warmup",
     "afno_spectral_fwd", "afno_spectral_bwd", "afno_spectral_host_arena_bytes",
     "afno_spectral_fwd_host", "afno_spectral_bwd_host", "afno_last_launch_count",
-    "afno_profile_start", "afno_profile_stop",
+    "afno_profile_start", "afno_profile_stop", "afno_plan_destroy_all",
 ]
 
 
@@ -79,6 +79,7 @@ def lib():
         L.afno_spectral_bwd_host.restype = ctypes.c_int
         L.afno_spectral_bwd_host.argtypes = [dp] + [vp] * 12 + [sz, vp]
         L.afno_last_launch_count.restype = ctypes.c_int
+        L.afno_plan_destroy_all.restype = ctypes.c_int
         L.afno_profile_start.restype = ctypes.c_int
         L.afno_profile_stop.restype = ctypes.c_int
         L.afno_profile_stop.argtypes = [ctypes.c_char_p, sz]
@@ -173,6 +174,10 @@ def afno_plan_warmup(d: Desc):
     _check(lib().afno_plan_warmup(ctypes.byref(cd)))
 
 
+def afno_plan_destroy_all():
+    _check(lib().afno_plan_destroy_all())
+
+
 def afno_last_launch_count() -> int:
     return int(lib().afno_last_launch_count())
 
@@ -217,6 +222,7 @@ def afno_spectral_fwd_host(d: Desc, x, w1, b1, w2, b2, y, arena, stream=None):
 
 
 def afno_spectral_bwd_host(d: Desc, x, dy, w1, b1, w2, b2, dx, dw1, db1, dw2, db2, arena, stream=None):
+    """x may be None: x is then the one the preceding afno_spectral_fwd_host left in `arena`."""
     cd = d.c()
     _check(lib().afno_spectral_bwd_host(ctypes.byref(cd), _ptr(x), _ptr(dy), _ptr(w1), _ptr(b1), _ptr(w2),
                                         _ptr(b2), _ptr(dx), _ptr(dw1), _ptr(db1), _ptr(dw2), _ptr(db2),

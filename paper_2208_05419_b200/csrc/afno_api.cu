@@ -443,37 +443,67 @@ size_t afno_spectral_host_arena_bytes(const afno_desc_t* d, int for_backward) {
 // duplex).  Samples are independent ("batched"); the parameter gradients of the samples
 // are accumulated in order with AFNO_FLAG_ACCUM_GRADS.
 namespace {
+// Internal copy streams and reusable events of the host variants, one set per device (created on first use,
+// kept for the life of the process).
 struct HostPipe {
   int device = -1;
   cudaStream_t h2d = nullptr, d2h = nullptr;
+  std::vector<cudaEvent_t> ev;
+  size_t next = 0;
+  // records an event on `on` and makes `waiter` wait for it; events are recycled round-robin (a recycled
+  // event's earlier wait has long been enqueued: re-recording does not disturb it)
+  cudaError_t mark(cudaStream_t on, cudaStream_t waiter) {
+    if (ev.size() < 64) {
+      cudaEvent_t e;
+      cudaError_t rc = cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
+      if (rc != cudaSuccess) return rc;
+      ev.push_back(e);
+      next = ev.size() - 1;
+    } else {
+      next = (next + 1) % ev.size();
+    }
+    cudaError_t rc = cudaEventRecord(ev[next], on);
+    if (rc != cudaSuccess) return rc;
+    return cudaStreamWaitEvent(waiter, ev[next], 0);
+  }
+  // quiesce everything the call has enqueued (also on the error paths: the caller may free its buffers)
+  void drain(cudaStream_t st) {
+    cudaStreamSynchronize(h2d);
+    cudaStreamSynchronize(st);
+    cudaStreamSynchronize(d2h);
+  }
 };
-thread_local HostPipe t_pipe;
+thread_local std::vector<HostPipe*> t_pipes;
 cudaError_t host_pipe(HostPipe** out) {
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
-  if (t_pipe.device != dev) {
-    if ((e = cudaStreamCreateWithFlags(&t_pipe.h2d, cudaStreamNonBlocking)) != cudaSuccess) return e;
-    if ((e = cudaStreamCreateWithFlags(&t_pipe.d2h, cudaStreamNonBlocking)) != cudaSuccess) return e;
-    t_pipe.device = dev;
+  for (HostPipe* p : t_pipes)
+    if (p->device == dev) {
+      *out = p;
+      return cudaSuccess;
+    }
+  HostPipe* p = new HostPipe();
+  if ((e = cudaStreamCreateWithFlags(&p->h2d, cudaStreamNonBlocking)) != cudaSuccess ||
+      (e = cudaStreamCreateWithFlags(&p->d2h, cudaStreamNonBlocking)) != cudaSuccess) {
+    if (p->h2d) cudaStreamDestroy(p->h2d);
+    delete p;
+    return e;
   }
-  *out = &t_pipe;
+  p->device = dev;
+  t_pipes.push_back(p);
+  *out = p;
   return cudaSuccess;
 }
-struct EventPool {
-  std::vector<cudaEvent_t> ev;
-  ~EventPool() {
-    for (cudaEvent_t e : ev) cudaEventDestroy(e);
-  }
-  cudaError_t mark(cudaStream_t on, cudaStream_t waiter) {
-    cudaEvent_t e;
-    cudaError_t rc = cudaEventCreateWithFlags(&e, cudaEventDisableTiming);
-    if (rc != cudaSuccess) return rc;
-    ev.push_back(e);
-    if ((rc = cudaEventRecord(e, on)) != cudaSuccess) return rc;
-    return cudaStreamWaitEvent(waiter, e, 0);
-  }
-};
+// like AFNO_CUDA_TRY, but lets the copies and kernels already in flight finish before returning
+#define AFNO_PIPE_TRY(expr)                                                                     \
+  do {                                                                                          \
+    cudaError_t e_ = (expr);                                                                    \
+    if (e_ != cudaSuccess) {                                                                    \
+      hp->drain(st);                                                                            \
+      return fail(AFNO_ERR_CUDA, std::string(#expr ": ") + cudaGetErrorString(e_));             \
+    }                                                                                           \
+  } while (0)
 } // namespace
 
 int afno_spectral_fwd_host(const afno_desc_t* d, const void* x_host, const float* w1_host,
@@ -490,27 +520,29 @@ int afno_spectral_fwd_host(const afno_desc_t* d, const void* x_host, const float
   cudaStream_t st = (cudaStream_t)cuda_stream;
   HostPipe* hp = nullptr;
   AFNO_CUDA_TRY(host_pipe(&hp));
-  EventPool ev;
   afno_desc_t d1 = *d;
   d1.B = 1;
   d1.flags &= ~(uint32_t)(AFNO_FLAG_SAVE_CONTEXT | AFNO_FLAG_USE_CONTEXT);
   const size_t sample = h.act / (size_t)g.B;
-  AFNO_CUDA_TRY(ev.mark(st, hp->h2d));   // the copies start after the caller's earlier work on the stream
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w1, w1_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b1, b1_host, h.nb1, cudaMemcpyHostToDevice, hp->h2d));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w2, w2_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b2, b2_host, h.nb2, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_PIPE_TRY(hp->mark(st, hp->h2d));   // the copies start after the caller's earlier work on the stream
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.w1, w1_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.b1, b1_host, h.nb1, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.w2, w2_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.b2, b2_host, h.nb2, cudaMemcpyHostToDevice, hp->h2d));
   for (int b = 0; b < g.B; ++b) {
     const size_t off = (size_t)b * sample;
-    AFNO_CUDA_TRY(cudaMemcpyAsync((char*)h.x + off, (const char*)x_host + off, sample, cudaMemcpyHostToDevice, hp->h2d));
-    AFNO_CUDA_TRY(ev.mark(hp->h2d, st));
+    AFNO_PIPE_TRY(cudaMemcpyAsync((char*)h.x + off, (const char*)x_host + off, sample, cudaMemcpyHostToDevice, hp->h2d));
+    AFNO_PIPE_TRY(hp->mark(hp->h2d, st));
     rc = afno_spectral_fwd(&d1, (char*)h.x + off, h.w1, h.b1, h.w2, h.b2, (char*)h.y + off, h.ws, h.ws_bytes, cuda_stream);
-    if (rc != AFNO_OK) return rc;
-    AFNO_CUDA_TRY(ev.mark(st, hp->d2h));
-    AFNO_CUDA_TRY(cudaMemcpyAsync((char*)y_host + off, (char*)h.y + off, sample, cudaMemcpyDeviceToHost, hp->d2h));
+    if (rc != AFNO_OK) {
+      hp->drain(st);
+      return rc;
+    }
+    AFNO_PIPE_TRY(hp->mark(st, hp->d2h));
+    AFNO_PIPE_TRY(cudaMemcpyAsync((char*)y_host + off, (char*)h.y + off, sample, cudaMemcpyDeviceToHost, hp->d2h));
   }
-  AFNO_CUDA_TRY(cudaStreamSynchronize(hp->d2h));
-  AFNO_CUDA_TRY(cudaStreamSynchronize(st));
+  AFNO_PIPE_TRY(cudaStreamSynchronize(hp->d2h));
+  AFNO_PIPE_TRY(cudaStreamSynchronize(st));
   return AFNO_OK;
 }
 
@@ -522,7 +554,9 @@ int afno_spectral_bwd_host(const afno_desc_t* d, const void* x_host, const void*
   Geometry g;
   int rc = resolve(d, &g);
   if (rc != AFNO_OK) return rc;
-  if (!x_host || !dy_host || !w1_host || !b1_host || !w2_host || !b2_host || !dx_host || !dw1_host ||
+  // x_host == NULL: x is still in the arena from the afno_spectral_fwd_host call that preceded this one on the
+  // same arena and descriptor (a training step uploads x once)
+  if (!dy_host || !w1_host || !b1_host || !w2_host || !b2_host || !dx_host || !dw1_host ||
       !db1_host || !dw2_host || !db2_host || !arena)
     return fail(AFNO_ERR_INVALID_ARG, "NULL pointer argument");
   if (d->flags & AFNO_FLAG_ACCUM_GRADS)
@@ -535,34 +569,55 @@ int afno_spectral_bwd_host(const afno_desc_t* d, const void* x_host, const void*
   cudaStream_t st = (cudaStream_t)cuda_stream;
   HostPipe* hp = nullptr;
   AFNO_CUDA_TRY(host_pipe(&hp));
-  EventPool ev;
   afno_desc_t d1 = *d;
   d1.B = 1;
   d1.flags &= ~(uint32_t)(AFNO_FLAG_SAVE_CONTEXT | AFNO_FLAG_USE_CONTEXT);
   const size_t sample = h.act / (size_t)g.B;
-  AFNO_CUDA_TRY(ev.mark(st, hp->h2d));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w1, w1_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b1, b1_host, h.nb1, cudaMemcpyHostToDevice, hp->h2d));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.w2, w2_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(h.b2, b2_host, h.nb2, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_PIPE_TRY(hp->mark(st, hp->h2d));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.w1, w1_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.b1, b1_host, h.nb1, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.w2, w2_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.b2, b2_host, h.nb2, cudaMemcpyHostToDevice, hp->h2d));
   for (int b = 0; b < g.B; ++b) {
     const size_t off = (size_t)b * sample;
-    AFNO_CUDA_TRY(cudaMemcpyAsync((char*)h.x + off, (const char*)x_host + off, sample, cudaMemcpyHostToDevice, hp->h2d));
-    AFNO_CUDA_TRY(cudaMemcpyAsync((char*)h.dy + off, (const char*)dy_host + off, sample, cudaMemcpyHostToDevice, hp->h2d));
-    AFNO_CUDA_TRY(ev.mark(hp->h2d, st));
+    if (x_host)
+      AFNO_PIPE_TRY(cudaMemcpyAsync((char*)h.x + off, (const char*)x_host + off, sample, cudaMemcpyHostToDevice, hp->h2d));
+    AFNO_PIPE_TRY(cudaMemcpyAsync((char*)h.dy + off, (const char*)dy_host + off, sample, cudaMemcpyHostToDevice, hp->h2d));
+    AFNO_PIPE_TRY(hp->mark(hp->h2d, st));
     d1.flags = b == 0 ? (d1.flags & ~(uint32_t)AFNO_FLAG_ACCUM_GRADS) : (d1.flags | AFNO_FLAG_ACCUM_GRADS);
     rc = afno_spectral_bwd(&d1, (char*)h.x + off, (char*)h.dy + off, h.w1, h.b1, h.w2, h.b2, (char*)h.dx + off, h.dw1, h.db1,
                            h.dw2, h.db2, h.ws, h.ws_bytes, cuda_stream);
-    if (rc != AFNO_OK) return rc;
-    AFNO_CUDA_TRY(ev.mark(st, hp->d2h));
-    AFNO_CUDA_TRY(cudaMemcpyAsync((char*)dx_host + off, (char*)h.dx + off, sample, cudaMemcpyDeviceToHost, hp->d2h));
+    if (rc != AFNO_OK) {
+      hp->drain(st);
+      return rc;
+    }
+    AFNO_PIPE_TRY(hp->mark(st, hp->d2h));
+    AFNO_PIPE_TRY(cudaMemcpyAsync((char*)dx_host + off, (char*)h.dx + off, sample, cudaMemcpyDeviceToHost, hp->d2h));
   }
-  AFNO_CUDA_TRY(cudaMemcpyAsync(dw1_host, h.dw1, h.nw, cudaMemcpyDeviceToHost, hp->d2h));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(db1_host, h.db1, h.nb1, cudaMemcpyDeviceToHost, hp->d2h));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(dw2_host, h.dw2, h.nw, cudaMemcpyDeviceToHost, hp->d2h));
-  AFNO_CUDA_TRY(cudaMemcpyAsync(db2_host, h.db2, h.nb2, cudaMemcpyDeviceToHost, hp->d2h));
-  AFNO_CUDA_TRY(cudaStreamSynchronize(hp->d2h));
-  AFNO_CUDA_TRY(cudaStreamSynchronize(st));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(dw1_host, h.dw1, h.nw, cudaMemcpyDeviceToHost, hp->d2h));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(db1_host, h.db1, h.nb1, cudaMemcpyDeviceToHost, hp->d2h));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(dw2_host, h.dw2, h.nw, cudaMemcpyDeviceToHost, hp->d2h));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(db2_host, h.db2, h.nb2, cudaMemcpyDeviceToHost, hp->d2h));
+  AFNO_PIPE_TRY(cudaStreamSynchronize(hp->d2h));
+  AFNO_PIPE_TRY(cudaStreamSynchronize(st));
+  return AFNO_OK;
+}
+
+// Frees every plan of the calling process (constant tables on all devices).  No call of this library may
+// be in flight; the next fwd / bwd / afno_plan_warmup rebuilds what it needs.
+int afno_plan_destroy_all(void) {
+  std::lock_guard<std::mutex> lock(g_plan_mutex);
+  int dev = 0;
+  cudaGetDevice(&dev);
+  for (Plan* p : g_plans) {
+    cudaSetDevice(p->device);
+    free_fft_plan(&p->fh);
+    free_fft_plan(&p->fw);
+    tc_free_plan(&p->tc);
+    delete p;
+  }
+  g_plans.clear();
+  cudaSetDevice(dev);
   return AFNO_OK;
 }
 

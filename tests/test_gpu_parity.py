@@ -558,6 +558,17 @@ def test_host_variants_tcgen05(oracle):
     assert np.array_equal(hdx.float().numpy(), g_dev["dx"])
     for t, k in zip(hg, ("dw1", "db1", "dw2", "db2")):
         assert parity.rel_l2(t.numpy(), g_dev[k]) <= 2e-6, k
+    # a training step uploads x once: fwd_host leaves it in the arena, bwd_host(x = None) finds it there
+    first = [t.clone() for t in hg]
+    hdx2 = torch.empty_like(hx).pin_memory()
+    binding.afno_spectral_fwd_host(desc, hx, *hp, hy, arena)
+    binding.afno_spectral_bwd_host(desc, None, hdy, *hp, hdx2, *hg, arena)
+    assert torch.equal(hdx2, hdx)
+    for a, b in zip(first, hg):
+        assert torch.equal(a, b)
+    binding.afno_plan_destroy_all()      # plans are rebuilt on demand
+    binding.afno_spectral_fwd_host(desc, hx, *hp, hy, arena)
+    assert np.array_equal(hy.float().numpy(), y_dev)
 
 
 def test_w192_runs_on_the_generic_path(oracle):

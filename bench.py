@@ -290,6 +290,8 @@ def run_ours(args):
     # --- the same step captured in CUDA graphs, one graph per buffer set: reported beside ---
     graph_info = None
     try:
+        if args.timed_only:
+            raise RuntimeError("skipped (--timed-only)")
         gs = torch.cuda.Stream()
         graphs = []
         with torch.cuda.stream(gs):
@@ -381,7 +383,7 @@ def run_ours(args):
 
     # --- end to end through the C ABI with HOST buffers -----------------------------------------
     e2e = None
-    if rank == 0 or world > 1:
+    if (rank == 0 or world > 1) and not args.timed_only:
         pin = lambda t: t.cpu().pin_memory()
         hx, hdy = pin(x0), pin(dy0)
         hp = [pin(p) for p in params]
@@ -410,7 +412,7 @@ def run_ours(args):
                "steps": E2E_STEPS, "note": "afno_spectral_fwd_host + afno_spectral_bwd_host (x uploaded once), pinned host buffers, wall clock"}
 
     cpu_baseline = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.timed_only:
         v, dt, cores = oracle_time(8)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                         "sample": f"8 samples fwd+bwd at 90x180x768 (fp64 oracle, mixed-radix FFT mode), {dt:.1f} s"}
@@ -531,6 +533,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--timed-only", action="store_true",
+                    help="warm-up, the timed steps and the per-kernel event pass only (no CUDA-graph replay, e2e or "
+                         "cpu_baseline legs): the command the ncu captures under profiles/ run")
     ap.add_argument("--stateless", action="store_true",
                     help="time the stateless afno_spectral_bwd (recomputes F1) instead of the saved-context step")
     args = ap.parse_args()

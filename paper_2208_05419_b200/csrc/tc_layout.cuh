@@ -28,30 +28,41 @@ struct CtxHeader {
 };
 constexpr uint32_t kCtxMagic = 0xAF90C7E5u;
 
-// ---- weight preparation: fp32 [nb][96][96][2] -> bf16 K-major interleaved operands --------------
-// per block 4 matrices of kWBytes {W1r, W1i, W2r, W2i} with element (n=o, k=i) = W[i][o] (the
-// backward pass reads the same images as MN-major operands), and the biases regrouped as
-// [block][layer][re 96 | im 96] fp32.
+// ---- weight preparation: fp32 [nb][bs][bs][2] -> bf16 K-major interleaved operands --------------
+// per GROUP of 96 channels 4 matrices of kWBytes {W1r, W1i, W2r, W2i} with element (n=o, k=i) = W[i][o] (the
+// backward pass reads the same images as MN-major operands): the blocks of the group sit on the diagonal,
+// everything else (other blocks, channels past C in a partly filled last group) is zero.  The biases are
+// regrouped as [group][layer][re 96 | im 96] fp32.
 __global__ void k_tc_prep_weights(const float* __restrict__ w1, const float* __restrict__ b1,
                                   const float* __restrict__ w2, const float* __restrict__ b2,
-                                  __nv_bfloat16* __restrict__ out, float* __restrict__ bout, int nb,
+                                  __nv_bfloat16* __restrict__ out, float* __restrict__ bout, int ngroups, int bs, int C,
                                   const CtxHeader hdr, CtxHeader* __restrict__ hdr_out) {
   pdl_launch_dependents();
   pdl_wait();
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx == 0 && hdr_out != nullptr) *hdr_out = hdr;   // SAVE_CONTEXT: what this call leaves in the workspace
-  if (idx < nb * BS) {
+  if (idx < ngroups * BS) {
     const int o = idx % BS, j = idx / BS;
-    const float2 a = ((const float2*)b1)[idx], b = ((const float2*)b2)[idx];
+    float2 a = make_float2(0.f, 0.f), b = make_float2(0.f, 0.f);
+    if (idx < C) {   // biases are [C][2] whatever the block size
+      a = ((const float2*)b1)[idx];
+      b = ((const float2*)b2)[idx];
+    }
     float* bb = bout + (size_t)j * 2 * NT;
     bb[o] = a.x;
     bb[BS + o] = a.y;
     bb[NT + o] = b.x;
     bb[NT + BS + o] = b.y;
   }
-  if (idx >= nb * BS * BS) return;
+  if (idx >= ngroups * BS * BS) return;
   const int o = idx % BS, i = (idx / BS) % BS, j = idx / (BS * BS);
-  const float2 a = ((const float2*)w1)[idx], b = ((const float2*)w2)[idx];
+  const int ci = j * BS + i, co = j * BS + o;        // channels
+  float2 a = make_float2(0.f, 0.f), b = make_float2(0.f, 0.f);
+  if (ci < C && co < C && ci / bs == co / bs) {
+    const size_t src = ((size_t)(ci / bs) * bs + ci % bs) * bs + co % bs;
+    a = ((const float2*)w1)[src];
+    b = ((const float2*)w2)[src];
+  }
   __nv_bfloat16* base = out + (size_t)j * 4 * (kWBytes / 2);
   const uint32_t f = ((i / 8) * kWLbo + (o / 8) * kWSbo + (o % 8) * 16 + (i % 8) * 2) / 2; // n=o, k=i
   const uint32_t m = kWBytes / 2;

@@ -14,7 +14,7 @@ struct MixParams {
   uint8_t* mask1;            // optional export, [B][H][Wh][C][2]
   uint8_t* mask2;
   uint4* maskbits;           // saved context: [tile][12 epilogue warps][32 lanes] {m1[0], m1[1], m2[0], m2[1]}
-  int B, H, Kw, Wh, nb, Kh;
+  int B, H, Kw, Wh, nb, C, Kh;   // nb = groups of 96 channels, C = channels (the last group may be partly filled)
   float lambda;
 };
 
@@ -546,13 +546,16 @@ __global__ void __launch_bounds__(kMix2Threads, 1) tc_mix2(const __grid_constant
           fence_async_smem();
           if (EXPORT && row_valid) {
             const int b = rem / p.Kw, kw = rem - b * p.Kw;
-            const size_t base = ((((size_t)b * p.H + r) * p.Wh + kw) * (size_t)(p.nb * BS) + (size_t)j * BS + chalf * 48) * 2 + half;
+            const int ch0 = j * BS + chalf * 48;   // first channel of this thread's 48 columns
+            const size_t base = ((((size_t)b * p.H + r) * p.Wh + kw) * (size_t)p.C + (size_t)ch0) * 2 + half;
             MaskLoop<0>::run([&](auto P) {
               constexpr int pp = decltype(P)::value;
-              p.mask1[base + (size_t)(2 * pp) * 2] = (uint8_t)mask_bit<pp>(m1[stream], 0);
-              p.mask1[base + (size_t)(2 * pp + 1) * 2] = (uint8_t)mask_bit<pp>(m1[stream], 1);
-              p.mask2[base + (size_t)(2 * pp) * 2] = (uint8_t)mask_bit<pp>(m2[stream], 0);
-              p.mask2[base + (size_t)(2 * pp + 1) * 2] = (uint8_t)mask_bit<pp>(m2[stream], 1);
+              if (ch0 + 2 * pp < p.C) {   // C is even: both channels of the pair exist or neither does
+                p.mask1[base + (size_t)(2 * pp) * 2] = (uint8_t)mask_bit<pp>(m1[stream], 0);
+                p.mask1[base + (size_t)(2 * pp + 1) * 2] = (uint8_t)mask_bit<pp>(m1[stream], 1);
+                p.mask2[base + (size_t)(2 * pp) * 2] = (uint8_t)mask_bit<pp>(m2[stream], 0);
+                p.mask2[base + (size_t)(2 * pp + 1) * 2] = (uint8_t)mask_bit<pp>(m2[stream], 1);
+              }
             });
           }
         }

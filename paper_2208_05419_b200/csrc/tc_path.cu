@@ -113,6 +113,18 @@ bool tile_tmap(const TcPlan& tp, CUtensorMap* m, const void* ptr, const Geometry
   return make_tmap(tp, m, ptr, 4, dims, str, box, true);
 }
 
+// the geometry the kernels see: nb = number of 96-channel groups
+Geometry tc_geom(const Geometry& g0) {
+  Geometry g = g0;
+  if (g.nb_blocks != 0) return g;   // already a group geometry
+  g.nb_blocks = g0.nb;
+  g.bs_block = g0.bs;
+  g.nb = (g0.C + BS - 1) / BS;
+  g.bs = BS;
+  g.hid = BS;
+  return g;
+}
+
 struct TcWs {
   CtxHeader* header;
   __nv_bfloat16 *A, *wprep;   // A: half-spectrum of ONE chunk of samples, transformed in place by tc_mix2
@@ -150,7 +162,8 @@ int chunk_samples(const Geometry& g, bool backward) {
   return cb;
 }
 
-TcWs tc_carve(const Geometry& g, bool backward, char* base) {
+TcWs tc_carve(const Geometry& g0, bool backward, char* base) {
+  const Geometry g = tc_geom(g0);
   TcWs w{};
   size_t off = 0;
   auto take = [&](size_t bytes) {
@@ -193,9 +206,14 @@ TcWs tc_carve(const Geometry& g, bool backward, char* base) {
 
 bool tc_plan_supported(int H, int W) { return H >= 1 && H <= HP && W >= 2 && W <= WP && W / 2 + 1 <= BS; }
 
+// Blocks of bs channels with bs dividing 96 (96, 48, 32, 24, 16, 12, 8: the paper's own network has 32 blocks
+// of 32) run as block-diagonal 96 x 96 weight images inside groups of 96 channels; a last group
+// that is only partly filled (C % 96 != 0) is zero-filled / clipped by the tensor-map copies.
 bool tc_supported(const Geometry& g) {
-  return g.bf16 && g.bs == BS && g.hid == BS && tc_plan_supported(g.H, g.W) && g.C % 8 == 0;
+  return g.bf16 && g.bs >= 8 && BS % g.bs == 0 && g.hid == g.bs && tc_plan_supported(g.H, g.W) && g.C % 8 == 0;
 }
+
+
 
 void tc_free_plan(TcPlan* p) {
   uint8_t** tabs[] = {&p->dft2, &p->fw, &p->fw_alpha, &p->gw, &p->gw_noalpha};
@@ -342,7 +360,7 @@ static cudaError_t launch_wdft_inv(const Geometry& g, const TcPlan& tp, const vo
 static CtxHeader make_header(const Geometry& g, const TcWs& w) {
   CtxHeader h{};
   h.magic = kCtxMagic;
-  h.B = g.B; h.H = g.H; h.W = g.W; h.C = g.C; h.nb = g.nb; h.Kh = g.Kh; h.Kw = g.Kw; h.chunk_b = w.chunk_b;
+  h.B = g.B; h.H = g.H; h.W = g.W; h.C = g.C; h.nb = g.nb_blocks; h.Kh = g.Kh; h.Kw = g.Kw; h.chunk_b = w.chunk_b;
   memcpy(&h.lambda_bits, &g.lambda, 4);
   h.export_masks = g.export_masks ? 1u : 0u;
   return h;
@@ -356,8 +374,9 @@ static Geometry chunk_geometry(const Geometry& g, int n) {
 }
 static size_t act_offset(const Geometry& g, int b0) { return (size_t)b0 * g.H * g.W * g.C * 2; }
 
-cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const float* w1, const float* b1,
+cudaError_t tc_forward(const Geometry& g0, const Plan& p, const void* x, const float* w1, const float* b1,
                        const float* w2, const float* b2, void* y, void* ws, cudaStream_t st) {
+  const Geometry g = tc_geom(g0);
   // SAVE_CONTEXT: the backward layout, so that tc_backward finds the context where it expects it
   TcWs w = tc_carve(g, g.save_ctx, (char*)ws);
   const TcPlan& tp = p.tc;
@@ -365,7 +384,7 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   const int nW = g.nb * BS * BS;
   const CtxHeader hdr = g.save_ctx ? make_header(g, w) : CtxHeader{};
   prof_begin("k_tc_prep_weights", st);
-  k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, w.wprep, w.bprep, g.nb, hdr, w.header);
+  k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, w.wprep, w.bprep, g.nb, g.bs_block, g.C, hdr, w.header);
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -379,7 +398,7 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
     if (!tile_tmap(tp, &mp.mapA1, w.A, gc)) return cudaErrorInvalidValue;
     mp.mapA1g = mp.mapA1;
     mp.A2 = w.A; mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
-    mp.B = gc.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
+    mp.B = gc.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.C = g.C; mp.Kh = g.Kh; mp.lambda = g.lambda;
     prof_begin("tc_mix_fwd", st);
     const int S2 = mix2_split(gc, tp);
     if (g.save_ctx) {
@@ -400,9 +419,10 @@ cudaError_t tc_forward(const Geometry& g, const Plan& p, const void* x, const fl
   return cudaSuccess;
 }
 
-cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const void* dy, const float* w1,
+cudaError_t tc_backward(const Geometry& g0, const Plan& p, const void* x, const void* dy, const float* w1,
                         const float* b1, const float* w2, const float* b2, void* dx, float* dw1, float* db1,
                         float* dw2, float* db2, void* ws, cudaStream_t st) {
+  const Geometry g = tc_geom(g0);
   TcWs w = tc_carve(g, true, (char*)ws);
   const TcPlan& tp = p.tc;
   cudaError_t e;
@@ -422,7 +442,7 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   // workspace (the context belongs to one set of parameters)
   if (!g.use_ctx) {
     TC_LAUNCH("k_tc_prep_weights", k_tc_prep_weights, (nW + 255) / 256, 256, 0, st, dep, w1, b1, w2, b2, w.wprep, w.bprep, g.nb,
-              CtxHeader{}, (CtxHeader*)nullptr);
+              g.bs_block, g.C, CtxHeader{}, (CtxHeader*)nullptr);
   }
   const size_t mask1_sample = (size_t)g.H * g.Wh * g.CH * 2, mask2_sample = (size_t)g.H * g.Wh * g.C * 2;
   for (int b0 = 0; b0 < g.B; b0 += w.chunk_b) {
@@ -447,7 +467,7 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
     mp.dft = tp.dft2; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
     mp.mask1 = g.export_masks ? w.mask1 + (size_t)b0 * mask1_sample : nullptr;
     mp.mask2 = g.export_masks ? w.mask2 + (size_t)b0 * mask2_sample : nullptr;
-    mp.B = gc.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.Kh = g.Kh; mp.lambda = g.lambda;
+    mp.B = gc.B; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.nb = g.nb; mp.C = g.C; mp.Kh = g.Kh; mp.lambda = g.lambda;
     const int S2 = mix2_split(gc, tp);
     mp.maskbits = w.maskbits + t0 * 12 * 32;
     if (g.use_ctx) {
@@ -470,12 +490,12 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
   }
   const int nred = nW + g.nb * BS;
   TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce, dim3((nred + 255) / 256, 2), 256, 0, st, dep, w.part, (float2*)dw2,
-            (float2*)db2, (float2*)dw1, (float2*)db1, g.nb, w.S, g.accum ? 1 : 0);
+            (float2*)db2, (float2*)dw1, (float2*)db1, g.nb, w.S, g.bs_block, g.C, g.accum ? 1 : 0);
   if (g.use_ctx) {
     // a context that does not belong to this call (other geometry, flags, never saved) poisons the results
     const size_t n_act = (size_t)g.B * g.H * g.W * g.C;
     TC_LAUNCH("k_tc_ctx_guard", k_tc_ctx_guard, 148, 256, 0, st, dep, (const CtxHeader*)w.header, make_header(g, w),
-              (uint16_t*)dx, n_act, dw1, dw2, (size_t)nW * 2, db1, db2, (size_t)g.nb * BS * 2);
+              (uint16_t*)dx, n_act, dw1, dw2, (size_t)g.nb_blocks * g.bs_block * g.bs_block * 2, db1, db2, (size_t)g.C * 2);
   }
 #undef TC_LAUNCH
   return cudaSuccess;

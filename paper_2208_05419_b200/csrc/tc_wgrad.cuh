@@ -147,20 +147,25 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
-// dW[j][i][o] = sum_s ( Dre[i][o] + Dim[i][96+o] ,  Dre[i][96+o] - Dim[i][o] ) ;  db[j][o] = sum_s Dre[96][(ri,o)]
-// blockIdx.y = 0: layer 2 partial sums (first nb*S CTAs of tc_wgrad), 1: layer 1
+// dW[blk][ii][oo] = sum_s ( Dre[i][o] + Dim[i][96+o] ,  Dre[i][96+o] - Dim[i][o] ) ;  db[ch] = sum_s Dre[96][(ri,o)]
+// with (i, o) the positions of the block's channels inside their group of 96 (the off-diagonal blocks of the
+// group's 96 x 96 product are not parameters and are dropped).
+// blockIdx.y = 0: layer 2 partial sums (first ngroups*S CTAs of tc_wgrad), 1: layer 1
 __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __restrict__ dW2, float2* __restrict__ dB2,
-                                  float2* __restrict__ dW1, float2* __restrict__ dB1, int nb, int S, int accumulate) {
+                                  float2* __restrict__ dW1, float2* __restrict__ dB1, int ngroups, int S, int bs, int C,
+                                  int accumulate) {
   pdl_launch_dependents();
   pdl_wait();
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  const int nW = nb * BS * BS;
+  const int nW = C * bs;          // nb * bs * bs complex weights
   const int layer = blockIdx.y;
-  part += (size_t)layer * nb * S * kWgPartFloats;
+  part += (size_t)layer * ngroups * S * kWgPartFloats;
   float2* dW = layer ? dW1 : dW2;
   float2* dB = layer ? dB1 : dB2;
   if (idx < nW) {
-    const int o = idx % BS, i = (idx / BS) % BS, j = idx / (BS * BS);
+    const int oo = idx % bs, ci = idx / bs;            // input channel ci = blk * bs + ii, output blk * bs + oo
+    const int co = (ci / bs) * bs + oo;
+    const int j = ci / BS, i = ci - j * BS, o = co - j * BS;
     float2 acc = accumulate ? dW[idx] : make_float2(0.f, 0.f);
     for (int s = 0; s < S; ++s) {
       const float* P = part + (size_t)(j * S + s) * kWgPartFloats;
@@ -170,8 +175,8 @@ __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __rest
       acc.y += Pre[BS + o] - Pim[o];
     }
     dW[idx] = acc;
-  } else if (idx < nW + nb * BS) {
-    const int k = idx - nW, o = k % BS, j = k / BS;
+  } else if (idx < nW + C) {
+    const int k = idx - nW, j = k / BS, o = k - j * BS;
     float2 acc = accumulate ? dB[k] : make_float2(0.f, 0.f);
     for (int s = 0; s < S; ++s) {
       const float* P = part + (size_t)(j * S + s) * kWgPartFloats + (size_t)BS * kWgPitch;

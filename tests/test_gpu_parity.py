@@ -205,6 +205,45 @@ def test_bf16_tcgen05_other_shapes(oracle, B, H, W, C, nb, f):
         assert np.array_equal(t.cpu().numpy(), g[k]), k
 
 
+@pytest.mark.parametrize("B,H,W,C,nb,f", [
+    (2, 18, 36, 160, 5, 1.0),     # 32-wide blocks, C % 96 != 0: the last group of 96 channels holds two blocks
+    (1, 30, 60, 96, 2, 1.0),      # 48-wide blocks
+    (2, 8, 16, 64, 8, 0.5),       # 8-wide blocks, one partly filled group, truncated spectrum
+    (1, 24, 48, 192, 8, 1.0),     # 24-wide blocks, two full groups
+])
+def test_bf16_tcgen05_narrow_blocks(oracle, B, H, W, C, nb, f):
+    """Blocks narrower than 96 (bs divides 96) run on the tcgen05 path as block-diagonal 96 x 96 weight images
+    inside groups of 96 channels (S5.3): forward, mask-consistent backward and the saved-context
+    step against the oracle, per tile; perturbing one block's weights leaves the other blocks' outputs
+    bit-identical (block-diagonality, PAPER.md:115)."""
+    wl = inputs.Workload(5, f"{H}x{W}x{C} nb={nb} bf16 B={B}", B, H, W, C, nb, 1, 0.01, f, "bf16", True, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert binding.afno_spectral_path(desc) == "tcgen05-bf16"
+    y0 = _check_forward(oracle, desc, data, label=wl.name)
+    g = _check_backward(oracle, desc, data, label=wl.name)
+    got = _ctx_step(desc, data)
+    assert np.array_equal(got["y"], y0) and np.array_equal(got["dx"], g["dx"])
+    for k in ("dw1", "db1", "dw2", "db2"):
+        assert np.array_equal(got[k], g[k]), k
+    bs = C // nb
+    w1 = data["w1"].copy()
+    w1[nb - 1] *= 1.5
+    y1 = parity.GpuLayer(desc).forward(data["x"], w1, data["b1"], data["w2"], data["b2"])
+    assert np.array_equal(y1[..., :C - bs], y0[..., :C - bs]) and not np.array_equal(y1[..., C - bs:], y0[..., C - bs:])
+
+
+def test_bf16_paper_channel_structure(oracle):
+    """SURVEY.md S8(f) item 1, the part that fits this path's grids: the paper's channel structure, 1,024
+    channels in 32 blocks of 32, at the 90 x 180 token grid, forward and backward."""
+    wl = inputs.WORKLOADS["paper_ch_b2"]
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert binding.afno_spectral_path(desc) == "tcgen05-bf16"
+    _check_forward(oracle, desc, data, label=wl.name)
+    _check_backward(oracle, desc, data, label=wl.name)
+
+
 def test_bf16_force_fp32_math_flag(oracle):
     wl = inputs.WORKLOADS["fcn_b1"]
     data = inputs.make_inputs(wl)

@@ -287,7 +287,8 @@ int afno_profile_stop(char* out, size_t cap) {
 const char* afno_spectral_path(const afno_desc_t* d) {
   Geometry g;
   if (resolve(d, &g) != AFNO_OK) return nullptr;
-  return use_tc_fwd(g) ? "tcgen05-bf16" : "generic-fp32";
+  // "hybrid": forward = fp32 FFTs on the CUDA cores + tensor-core block MLP; backward = generic-fp32 kernels
+  return use_tc_fwd(g) ? "tcgen05-bf16" : (tc_mlp_supported(g) ? "hybrid-fft32-tcgen05" : "generic-fp32");
 }
 
 size_t afno_spectral_workspace_bytes(const afno_desc_t* d, int for_backward) {

@@ -80,6 +80,12 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
                         const float* b1, const float* w2, const float* b2, void* dx, float* dw1, float* db1,
                         float* dw2, float* db2, void* ws, cudaStream_t st);
 
+// hybrid path (bf16 activations on grids beyond the fused chain): generic fp32 FFTs + tensor-core block MLP, forward
+bool tc_mlp_supported(const Geometry& g);
+size_t tc_mlp_workspace_bytes(const Geometry& g);
+cudaError_t tc_mlp_forward(const Geometry& g, float2* X, const float* w1, const float* b1, const float* w2,
+                           const float* b2, void* ws, cudaStream_t st);
+
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 } // namespace afno

@@ -574,6 +574,7 @@ void launch_wgrad(Launcher& L, const Geometry& g, const float2* A, int lda, cons
 
 struct GenericWs {
   float2 *Xh, *O1, *Z, *G, *G1, *Wt1, *Wt2, *part;
+  void* mlp;   // hybrid forward: weight images of the tensor-core MLP (tc_mlp_forward)
   size_t total;
 };
 
@@ -588,6 +589,7 @@ GenericWs carve(const Geometry& g, bool backward, char* base, size_t mask_region
   const size_t rows = (size_t)g.rows();
   w.Xh = take(rows * g.C);
   w.O1 = take(rows * g.CH);
+  if (!backward && tc_mlp_supported(g)) w.mlp = take((tc_mlp_workspace_bytes(g) + sizeof(float2) - 1) / sizeof(float2));
   if (backward) {
     w.Z = take(rows * g.C);
     w.G = take(rows * g.C);
@@ -616,10 +618,15 @@ cudaError_t forward_t(const Geometry& g, const Plan& p, const T* x, const float*
   Launcher L{st};
   launch_wfft_fwd<T>(L, g, p, x, w.Xh, false);                                      // F1
   launch_hfft(L, g, p, w.Xh, g.C, false);                                           // F2
-  launch_gemm<EPI_RELU>(L, g, w.Xh, g.C, (const float2*)w1, (const float2*)b1, w.O1, g.CH, nullptr, 0,
-                        g.bs, g.hid);                                               // F3, F4
-  launch_gemm<EPI_SHRINK>(L, g, w.O1, g.CH, (const float2*)w2, (const float2*)b2, w.Xh, g.C, nullptr, 0,
-                          g.hid, g.bs);                                             // F5, F6
+  if (w.mlp != nullptr) {
+    // hybrid path (bf16 activations): F3-F6 on the tensor cores, in place on the spectrum
+    if (L.err == cudaSuccess) L.err = tc_mlp_forward(g, w.Xh, w1, b1, w2, b2, w.mlp, L.st);
+  } else {
+    launch_gemm<EPI_RELU>(L, g, w.Xh, g.C, (const float2*)w1, (const float2*)b1, w.O1, g.CH, nullptr, 0,
+                          g.bs, g.hid);                                             // F3, F4
+    launch_gemm<EPI_SHRINK>(L, g, w.O1, g.CH, (const float2*)w2, (const float2*)b2, w.Xh, g.C, nullptr, 0,
+                            g.hid, g.bs);                                           // F5, F6
+  }
   launch_hfft(L, g, p, w.Xh, g.C, true);                                            // F7
   launch_wfft_inv<T>(L, g, p, w.Xh, g.no_residual ? nullptr : x, y, false);         // F8, F9
   return L.err;

@@ -1,0 +1,198 @@
+// Part of the tcgen05 path (tc_path.cu includes the parts in order, inside namespace afno { namespace { ):
+// tc_mlp_fwd, rows F3-F6 for grids the fused chain (tc_mix2) does not reach (H > 96 or W/2+1 > 96, e.g. the 180x360
+// grid of BASELINE.json configs[3]): the transforms run as fp32 mixed-radix FFTs on the CUDA cores (generic.cu,
+// the design BASELINE.json:north_star describes), the block-diagonal complex MLP on the tensor cores.
+// Not a standalone header: it relies on tc_common.cuh and on the parts included before it.
+//
+// The spectrum is the generic path's X[row][C] (fp32 complex, row = (b, h, kw < Kw)); the kernel works IN PLACE on
+// tiles of 128 rows x one group of 96 channels:
+//   fp32 tile --cp.async--> staging --convert--> bf16 A operand [128 x (re 96 | im 96)] (K-major, shared memory)
+//   D1 = A W1 (tensor memory) -> + b1, split ReLU -> bf16 A operand (the same buffer) -> D2 = O1 W2
+//   -> + b2, softshrink on the fp32 sum, truncation -> fp32 complex back to X.
+// Weights are the images k_tc_prep_weights builds (block-diagonal for blocks narrower than 96).  Every CTA works
+// on one group, so the weights load once; the next tile streams into the staging buffer while this one computes.
+constexpr int kMlpThreads = 256;
+constexpr int kMlpRows = 128;
+constexpr uint32_t kMlpALbo = kMlpRows * 16 + 16, kMlpASbo = 128;   // K-major A [128 x 192]: k-chunk stride padded by 16 B
+constexpr uint32_t kMlpABytes = (NT / 8) * kMlpALbo;                // 49,536
+constexpr uint32_t kMlpStageBytes = kMlpRows * BS * 8;              // 98,304: [128 rows][96 float2]
+constexpr uint32_t kMlpSmem = 4 * kWBytes + kMlpABytes + kMlpStageBytes;   // 221,568
+
+struct MlpParams {
+  float2* X;                 // [rows][C] fp32 complex, transformed in place
+  const uint8_t* wprep;      // per group 4 x kWBytes: W1r, W1i, W2r, W2i
+  const float* bprep;        // per group [2 layers][192]
+  long long rows;
+  int C, ngroups, H, Kw, Kh;
+  float lambda;
+};
+
+__global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd(const MlpParams p, int S) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t done[2];
+  __shared__ uint32_t tmem_slot;
+  __shared__ __align__(16) float sBias[2 * NT];
+  uint8_t* sW = smem;
+  uint8_t* sA = smem + 4 * kWBytes;
+  uint8_t* sStage = sA + kMlpABytes;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int j = blockIdx.x / S, s0 = blockIdx.x - j * S;
+  const long long ntiles = (p.rows + kMlpRows - 1) / kMlpRows;
+  const int ch0 = j * BS;                       // first channel of the group
+  const int nch = min(BS, p.C - ch0);           // channels of the group that exist (a multiple of 8)
+  pdl_launch_dependents();
+  for (uint32_t i = tid; i < kMlpABytes / 16; i += kMlpThreads) ((uint4*)sA)[i] = make_uint4(0, 0, 0, 0);
+  if (tid == 0) {
+    mbar_init(&done[0], 1);
+    mbar_init(&done[1], 1);
+    mbar_init_fence();
+  }
+  if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  pdl_wait();   // the spectrum and the weight images are written by earlier kernels of the call
+  {
+    const uint8_t* wsrc = p.wprep + (size_t)j * 4 * kWBytes;
+    for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMlpThreads) cp_async16(smem_u32(sW) + i * 16, wsrc + (size_t)i * 16);
+  }
+  for (int i = tid; i < 2 * NT; i += kMlpThreads) sBias[i] = p.bprep[(size_t)j * 2 * NT + i];
+  // staging loads of one tile: 16-byte pieces, a row of the group is nch * 8 contiguous bytes; pieces past the last
+  // row or the last channel are zero-filled (cp.async with src-size 0)
+  auto stage_tile = [&](long long t) {
+    const long long r0 = t * kMlpRows;
+    for (uint32_t i = tid; i < kMlpStageBytes / 16; i += kMlpThreads) {
+      const int r = i / (BS / 2), c2 = i - r * (BS / 2);       // piece = 2 channels
+      const bool ok = (r0 + r < p.rows) && (2 * c2 < nch);
+      const float2* src = p.X + (size_t)(ok ? r0 + r : 0) * p.C + ch0 + (ok ? 2 * c2 : 0);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(sStage) + i * 16), "l"(src), "r"(ok ? 16 : 0)
+                   : "memory");
+    }
+    cp_async_commit();
+  };
+  if (s0 < ntiles) stage_tile(s0);
+  cp_async_wait_all();
+  fence_async_smem();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const uint32_t aW = smem_u32(sW), aA = smem_u32(sA);
+  const uint32_t w1r = aW, w1i = aW + kWBytes, w2r = aW + 2 * kWBytes, w2i = aW + 3 * kWBytes;
+  const uint32_t D1 = tmem, D2 = tmem + NT;   // (re 96 | im 96) each
+  const int q = warp & 3, chalf = warp >> 2;  // TMEM lane quarter, column half (48 of the 96 channels)
+  const int r = q * 32 + lane;
+  const uint32_t lane_sel = (uint32_t)(q * 32) << 16;
+  uint32_t ph = 0;
+  // T = A W as real GEMMs on the (re | im) halves: T_re = A_re W_re - A_im W_im ; T_im = A_re W_im + A_im W_re
+  auto issue_layer = [&](uint32_t D, uint32_t wr, uint32_t wi, uint64_t* bar) {
+    const uint32_t id = idesc_bf16(128, BS, 0u);
+#pragma unroll
+    for (int ks = 0; ks < BS / 16; ++ks) {
+      const uint64_t ad = smem_desc(aA + ks * 2 * kMlpALbo, kMlpALbo, kMlpASbo);
+      mma_ss(D, ad, smem_desc(wr + ks * 2 * kWLbo, kWLbo, kWSbo), id, ks != 0);
+      mma_ss(D + BS, ad, smem_desc(wi + ks * 2 * kWLbo, kWLbo, kWSbo), id, ks != 0);
+    }
+#pragma unroll
+    for (int ks = 0; ks < BS / 16; ++ks) {
+      const uint64_t ad = smem_desc(aA + (BS / 8 + ks * 2) * kMlpALbo, kMlpALbo, kMlpASbo);
+      mma_ss(D, ad, smem_desc(wi + ks * 2 * kWLbo, kWLbo, kWSbo), id | kIdescNegB, 1u);
+      mma_ss(D + BS, ad, smem_desc(wr + ks * 2 * kWLbo, kWLbo, kWSbo), id, 1u);
+    }
+    mma_commit(bar);
+  };
+  for (long long t = s0; t < ntiles; t += S) {
+    const long long r0 = t * kMlpRows;
+    // ---- staging (fp32 complex) -> bf16 A operand: unit = (row, 8 channels); lanes run over the channel chunks ----
+    for (uint32_t u = tid; u < kMlpRows * (BS / 8); u += kMlpThreads) {
+      const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
+      const float4* src = (const float4*)(sStage + (size_t)rr * (BS * 8) + c8 * 64);
+      const float4 a = src[0], b = src[1], c = src[2], d = src[3];
+      const uint4 re = make_uint4(pack_bf16(a.x, a.z), pack_bf16(b.x, b.z), pack_bf16(c.x, c.z), pack_bf16(d.x, d.z));
+      const uint4 im = make_uint4(pack_bf16(a.y, a.w), pack_bf16(b.y, b.w), pack_bf16(c.y, c.w), pack_bf16(d.y, d.w));
+      uint8_t* dst = sA + (size_t)(rr >> 3) * kMlpASbo + (rr & 7) * 16;
+      *(uint4*)(dst + (size_t)c8 * kMlpALbo) = re;
+      *(uint4*)(dst + (size_t)(BS / 8 + c8) * kMlpALbo) = im;
+    }
+    fence_async_smem();
+    __syncthreads();
+    if (t + S < ntiles) stage_tile(t + S);   // the next tile streams in while this one computes
+    if (warp == 0 && elect_one()) {
+      tc_fence_after();
+      issue_layer(D1, w1r, w1i, &done[0]);
+    }
+    __syncwarp();
+    mbar_wait(&done[0], ph);
+    tc_fence_after();
+    // ---- O1 = relu(P1 + b1) -> bf16 A operand of layer 2 (the A buffer is free: layer 1 has completed) ----
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+      uint32_t v[48];
+      tmem_ld16<0>(D1 + lane_sel + half * BS + chalf * 48, v);
+      tmem_ld16<16>(D1 + lane_sel + half * BS + chalf * 48 + 16, v);
+      tmem_ld16<32>(D1 + lane_sel + half * BS + chalf * 48 + 32, v);
+      tmem_wait_ld();
+      const float* bias = sBias + half * BS + chalf * 48;
+      uint8_t* dst = sA + (size_t)(r >> 3) * kMlpASbo + (r & 7) * 16 + (size_t)(half * (BS / 8) + chalf * 6) * kMlpALbo;
+#pragma unroll
+      for (int g = 0; g < 6; ++g) {
+        uint32_t pk[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const float lo = fmaxf(__uint_as_float(v[8 * g + 2 * e]) + bias[8 * g + 2 * e], 0.f);
+          const float hi = fmaxf(__uint_as_float(v[8 * g + 2 * e + 1]) + bias[8 * g + 2 * e + 1], 0.f);
+          pk[e] = pack_bf16(lo, hi);
+        }
+        *(uint4*)(dst + (size_t)g * kMlpALbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+      }
+    }
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0 && elect_one()) {
+      tc_fence_after();
+      issue_layer(D2, w2r, w2i, &done[1]);
+    }
+    __syncwarp();
+    mbar_wait(&done[1], ph);
+    tc_fence_after();
+    // ---- Z = softshrink(P2 + b2) on the fp32 sum, zero on truncated rows -> fp32 complex, in place ----
+    {
+      uint32_t vr[48], vi[48];
+      tmem_ld16<0>(D2 + lane_sel + chalf * 48, vr);
+      tmem_ld16<16>(D2 + lane_sel + chalf * 48 + 16, vr);
+      tmem_ld16<32>(D2 + lane_sel + chalf * 48 + 32, vr);
+      tmem_ld16<0>(D2 + lane_sel + BS + chalf * 48, vi);
+      tmem_ld16<16>(D2 + lane_sel + BS + chalf * 48 + 16, vi);
+      tmem_ld16<32>(D2 + lane_sel + BS + chalf * 48 + 32, vi);
+      tmem_wait_ld();
+      const long long row = r0 + r;
+      if (row < p.rows) {
+        const int h = (int)((row / p.Kw) % p.H);
+        const bool kept = ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
+        const float lam = p.lambda;
+        const float* bre = sBias + NT + chalf * 48;
+        const float* bim = bre + BS;
+        float2* out = p.X + (size_t)row * p.C + ch0 + chalf * 48;
+#pragma unroll
+        for (int c = 0; c < 48; c += 2) {
+          if (chalf * 48 + c < nch) {
+            float4 o;
+            const float t0 = __uint_as_float(vr[c]) + bre[c], t1 = __uint_as_float(vi[c]) + bim[c];
+            const float t2 = __uint_as_float(vr[c + 1]) + bre[c + 1], t3 = __uint_as_float(vi[c + 1]) + bim[c + 1];
+            o.x = kept ? t0 - fminf(fmaxf(t0, -lam), lam) : 0.f;
+            o.y = kept ? t1 - fminf(fmaxf(t1, -lam), lam) : 0.f;
+            o.z = kept ? t2 - fminf(fmaxf(t2, -lam), lam) : 0.f;
+            o.w = kept ? t3 - fminf(fmaxf(t3, -lam), lam) : 0.f;
+            *(float4*)(out + c) = o;
+          }
+        }
+      }
+    }
+    ph ^= 1u;
+    cp_async_wait_all();   // the next tile has landed in the staging buffer
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<512>(tmem);
+}

@@ -41,6 +41,7 @@ using namespace tc;
 #include "tc_wdft.cuh"
 #include "tc_mix.cuh"
 #include "tc_wgrad.cuh"
+#include "tc_mlp.cuh"
 
 // ---- host side: constant operand images ------------------------------------------------------------
 uint16_t host_bf16(double v) {
@@ -325,6 +326,49 @@ static cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, siz
   cfg.attrs = at;
   cfg.numAttrs = dependent ? 1 : 0;
   return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
+// ---- hybrid path: fp32 FFTs on the CUDA cores (generic.cu) + the block MLP on the tensor cores (tc_mlp.cuh) -------
+bool tc_mlp_supported(const Geometry& g) {
+  return g.bf16 && !g.force_fp32 && g.bs >= 8 && BS % g.bs == 0 && g.hid == g.bs && g.C % 8 == 0;
+}
+size_t tc_mlp_workspace_bytes(const Geometry& g) {
+  const size_t groups = (size_t)(g.C + BS - 1) / BS;
+  return align_up(groups * 4 * kWBytes, 256) + align_up(groups * 2 * NT * sizeof(float), 256);
+}
+cudaError_t tc_mlp_forward(const Geometry& g, float2* X, const float* w1, const float* b1, const float* w2, const float* b2,
+                           void* ws, cudaStream_t st) {
+  static bool attr_set = false;
+  cudaError_t e;
+  if (!attr_set) {
+    if ((e = set_smem(tc_mlp_fwd, kMlpSmem)) != cudaSuccess) return e;
+    attr_set = true;
+  }
+  const int groups = (g.C + BS - 1) / BS;
+  __nv_bfloat16* wprep = (__nv_bfloat16*)ws;
+  float* bprep = (float*)((char*)ws + align_up((size_t)groups * 4 * kWBytes, 256));
+  const int nW = groups * BS * BS;
+  prof_begin("k_tc_prep_weights", st);
+  k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, wprep, bprep, groups, g.bs, g.C, CtxHeader{},
+                                                      (CtxHeader*)nullptr);
+  prof_end(st);
+  count_launch();
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  int dev = 0, sms = 148;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+  if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+  MlpParams mp{};
+  mp.X = X; mp.wprep = (const uint8_t*)wprep; mp.bprep = bprep;
+  mp.rows = g.rows(); mp.C = g.C; mp.ngroups = groups; mp.H = g.H; mp.Kw = g.Kw; mp.Kh = g.Kh; mp.lambda = g.lambda;
+  const long long ntiles = (mp.rows + kMlpRows - 1) / kMlpRows;
+  int S = sms / groups;
+  if (S < 1) S = 1;
+  if ((long long)S > ntiles) S = (int)ntiles;
+  prof_begin("tc_mlp_fwd", st);
+  e = launch_k(tc_mlp_fwd, groups * S, kMlpThreads, kMlpSmem, st, true, mp, S);
+  prof_end(st);
+  count_launch();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 // W-direction launches: tile = (b, h, block), persistent over the SMs

@@ -244,6 +244,26 @@ def test_bf16_paper_channel_structure(oracle):
     _check_backward(oracle, desc, data, label=wl.name)
 
 
+@pytest.mark.parametrize("B,H,W,C,nb,f", [
+    (1, 100, 200, 192, 2, 1.0),    # H and W past the fused chain's limits, two full groups, ragged last row tile
+    (2, 120, 30, 160, 5, 0.5),     # 32-wide blocks, partly filled last group, truncated rows
+    (1, 10, 200, 96, 1, 1.0),      # W/2+1 = 101 bins only
+])
+def test_bf16_hybrid_forward(oracle, B, H, W, C, nb, f):
+    """Grids beyond the fused chain (H > 96 or W/2+1 > 96) with bf16 activations: fp32 FFTs on the CUDA cores and
+    the block MLP on the tensor cores (tc_mlp_fwd), forward, against the oracle per tile; the pure fp32 kernels
+    (AFNO_FLAG_FORCE_FP32_MATH) must agree with it to bf16-operand accuracy."""
+    wl = inputs.Workload(3, f"{H}x{W}x{C} nb={nb} bf16 B={B} hybrid", B, H, W, C, nb, 1, 0.01, f, "bf16", False, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert binding.afno_spectral_path(desc) == "hybrid-fft32-tcgen05"
+    y = _check_forward(oracle, desc, data, label=wl.name)
+    d32 = parity.desc_for(wl, flags=binding.FLAG_FORCE_FP32_MATH)
+    assert binding.afno_spectral_path(d32) == "generic-fp32"
+    y32 = parity.GpuLayer(d32).forward(data["x"], data["w1"], data["b1"], data["w2"], data["b2"])
+    assert parity.rel_l2(y, y32) <= 5e-3
+
+
 def test_bf16_force_fp32_math_flag(oracle):
     wl = inputs.WORKLOADS["fcn_b1"]
     data = inputs.make_inputs(wl)
@@ -622,5 +642,6 @@ def test_w192_runs_on_the_generic_path(oracle):
     for dt in (binding.AFNO_BF16, binding.AFNO_F32):
         desc = binding.Desc(B, H, W, C, nb, 1, 0.01, 1.0, dt)
         binding.afno_plan_warmup(desc)
-        assert binding.afno_spectral_path(desc) == "generic-fp32"
+        # bf16: fp32 FFTs + tensor-core MLP (hybrid forward); fp32: generic kernels throughout
+        assert binding.afno_spectral_path(desc) == ("hybrid-fft32-tcgen05" if dt == binding.AFNO_BF16 else "generic-fp32")
         _check_forward(oracle, desc, data, label=f"64x192x96 dtype={dt}")

@@ -164,26 +164,41 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd(const MlpParams p, 
       tmem_ld16<32>(D2 + lane_sel + BS + chalf * 48 + 32, vi);
       tmem_wait_ld();
       const long long row = r0 + r;
-      if (row < p.rows) {
-        const int h = (int)((row / p.Kw) % p.H);
-        const bool kept = ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
-        const float lam = p.lambda;
-        const float* bre = sBias + NT + chalf * 48;
-        const float* bim = bre + BS;
-        float2* out = p.X + (size_t)row * p.C + ch0 + chalf * 48;
+      const int h = (int)((row / p.Kw) % p.H);
+      const bool kept = row < p.rows && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
+      const float lam = p.lambda;
+      const float* bre = sBias + NT + chalf * 48;
+      const float* bim = bre + BS;
+      // A thread holds one ROW (48 channels); written straight to global memory a warp instruction would touch 32
+      // rows with 16 bytes each.  The warp transposes through its private slice of the (now idle) A buffer
+      // instead, 16 channels per pass (row pitch 144 B: conflict-free), and stores 128 contiguous bytes per row.
+      constexpr uint32_t kPitch = 16 * 8 + 16;
+      uint8_t* scratch = sA + (size_t)warp * (kMlpABytes / 8 / 16 * 16);
+      const long long wrow0 = r0 + q * 32;       // first row of this warp
 #pragma unroll
-        for (int c = 0; c < 48; c += 2) {
-          if (chalf * 48 + c < nch) {
-            float4 o;
-            const float t0 = __uint_as_float(vr[c]) + bre[c], t1 = __uint_as_float(vi[c]) + bim[c];
-            const float t2 = __uint_as_float(vr[c + 1]) + bre[c + 1], t3 = __uint_as_float(vi[c + 1]) + bim[c + 1];
-            o.x = kept ? t0 - fminf(fmaxf(t0, -lam), lam) : 0.f;
-            o.y = kept ? t1 - fminf(fmaxf(t1, -lam), lam) : 0.f;
-            o.z = kept ? t2 - fminf(fmaxf(t2, -lam), lam) : 0.f;
-            o.w = kept ? t3 - fminf(fmaxf(t3, -lam), lam) : 0.f;
-            *(float4*)(out + c) = o;
-          }
+      for (int pass = 0; pass < 3; ++pass) {
+#pragma unroll
+        for (int c = 0; c < 16; c += 2) {
+          const int cc = pass * 16 + c;
+          float4 o;
+          const float t0 = __uint_as_float(vr[cc]) + bre[cc], t1 = __uint_as_float(vi[cc]) + bim[cc];
+          const float t2 = __uint_as_float(vr[cc + 1]) + bre[cc + 1], t3 = __uint_as_float(vi[cc + 1]) + bim[cc + 1];
+          o.x = kept ? t0 - fminf(fmaxf(t0, -lam), lam) : 0.f;
+          o.y = kept ? t1 - fminf(fmaxf(t1, -lam), lam) : 0.f;
+          o.z = kept ? t2 - fminf(fmaxf(t2, -lam), lam) : 0.f;
+          o.w = kept ? t3 - fminf(fmaxf(t3, -lam), lam) : 0.f;
+          *(float4*)(scratch + lane * kPitch + c * 8) = o;
         }
+        __syncwarp();
+        const int chp = chalf * 48 + pass * 16;   // first channel (within the group) of this pass
+#pragma unroll
+        for (int it = 0; it < 8; ++it) {
+          const int id = it * 32 + lane, rr = id >> 3, piece = id & 7;
+          const float4 o = *(const float4*)(scratch + rr * kPitch + piece * 16);
+          if (wrow0 + rr < p.rows && chp + 2 * piece < nch)
+            *(float4*)(p.X + (size_t)(wrow0 + rr) * p.C + ch0 + chp + 2 * piece) = o;
+        }
+        __syncwarp();
       }
     }
     ph ^= 1u;

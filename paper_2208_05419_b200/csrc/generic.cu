@@ -24,7 +24,12 @@ namespace afno {
 namespace {
 
 constexpr int kLanes = 32;
-constexpr int kFftWarps = 8;
+constexpr int kFftWarps = 8;     // H-direction transform (46 KB of shared memory per block at H = 180: 4 blocks per SM)
+#ifndef AFNO_WFFT_WARPS
+#define AFNO_WFFT_WARPS 16
+#endif
+constexpr int kWfftWarps = AFNO_WFFT_WARPS;   // W-direction transforms (92 KB per block at W = 360: 2 blocks per SM): measured 8 / 16 warps -> 0.72 / 0.48 ms forward
+constexpr int kLoadBatch = 8;   // independent global loads a thread keeps in flight in the FFT kernels' load loops
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
   return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
@@ -149,10 +154,10 @@ struct ActIO<__nv_bfloat16> {
 };
 
 // ---- F1 / B2: W-direction real FFT ----------------------------------------------------
-// grid (ceil(C/64), H, B), block (32, kFftWarps); smem W*32 float2.
+// grid (ceil(C/64), H, B), block (32, kWfftWarps); smem W*32 float2.
 // S[((b*H+h)*Kw + k)*C + ch] = scale * alpha? * sum_w x[b,h,w,ch] exp(-2 pi i k w / W)
 template <typename T>
-__global__ void __launch_bounds__(kLanes * kFftWarps)
+__global__ void __launch_bounds__(kLanes * kWfftWarps)
 k_wfft_fwd(const T* __restrict__ x, float2* __restrict__ S, FftPlan pw, int H, int W, int C, int Kw,
            float scale, int alpha_weight) {
   extern __shared__ float2 smem[];
@@ -161,19 +166,32 @@ k_wfft_fwd(const T* __restrict__ x, float2* __restrict__ S, FftPlan pw, int H, i
   const int c = blockIdx.x * 64 + 2 * lane;
   const bool pair = (c + 1 < C) && ((C & 1) == 0);
   const T* xrow = x + ((size_t)(b * H + h) * W) * C;
-  for (int w = warp; w < W; w += kFftWarps) {
-    float2 v = make_float2(0.f, 0.f);
-    if (pair) v = ActIO<T>::ld2(xrow + (size_t)w * C + c);
-    else {
-      if (c < C) v.x = ActIO<T>::ld(xrow + (size_t)w * C + c);
-      if (c + 1 < C) v.y = ActIO<T>::ld(xrow + (size_t)w * C + c + 1);
+  // kLoadBatch independent loads in flight per thread before the first shared-memory store: a warp's loop of one
+  // 128-byte load per iteration leaves 2 KB in flight per SM (measured 0.8 TB/s at 180x360)
+  for (int w0 = warp; w0 < W; w0 += kWfftWarps * kLoadBatch) {
+    float2 v[kLoadBatch];
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int w = w0 + u * kWfftWarps;
+      v[u] = make_float2(0.f, 0.f);
+      if (w < W) {
+        if (pair) v[u] = ActIO<T>::ld2(xrow + (size_t)w * C + c);
+        else {
+          if (c < C) v[u].x = ActIO<T>::ld(xrow + (size_t)w * C + c);
+          if (c + 1 < C) v[u].y = ActIO<T>::ld(xrow + (size_t)w * C + c + 1);
+        }
+      }
     }
-    smem[w * kLanes + lane] = v; // channel c in the real part, channel c+1 in the imaginary part
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int w = w0 + u * kWfftWarps;
+      if (w < W) smem[w * kLanes + lane] = v[u]; // channel c in the real part, channel c+1 in the imaginary part
+    }
   }
   __syncthreads();
-  fft_inplace(smem, pw, -1.f, lane, warp, kFftWarps);
+  fft_inplace(smem, pw, -1.f, lane, warp, kWfftWarps);
   float2* Srow = S + ((size_t)(b * H + h) * Kw) * C;
-  for (int k = warp; k < Kw; k += kFftWarps) {
+  for (int k = warp; k < Kw; k += kWfftWarps) {
     const int kn = (k == 0) ? 0 : W - k;
     float2 zk = smem[__ldg(pw.perm + k) * kLanes + lane];
     float2 zn = smem[__ldg(pw.perm + kn) * kLanes + lane];
@@ -201,8 +219,19 @@ k_hfft(float2* __restrict__ S, FftPlan ph, int H, int Kw, int C, float sg) {
   const int c = blockIdx.x * kLanes + lane;
   float2* base = S + ((size_t)b * H * Kw + kw) * C + c;
   const size_t hstride = (size_t)Kw * C;
-  for (int h = warp; h < H; h += kFftWarps)
-    smem[h * kLanes + lane] = (c < C) ? base[h * hstride] : make_float2(0.f, 0.f);
+  for (int h0 = warp; h0 < H; h0 += kFftWarps * kLoadBatch) {
+    float2 v[kLoadBatch];
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int h = h0 + u * kFftWarps;
+      v[u] = (c < C && h < H) ? base[h * hstride] : make_float2(0.f, 0.f);
+    }
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int h = h0 + u * kFftWarps;
+      if (h < H) smem[h * kLanes + lane] = v[u];
+    }
+  }
   __syncthreads();
   fft_inplace(smem, ph, sg, lane, warp, kFftWarps);
   if (c < C)
@@ -213,7 +242,7 @@ k_hfft(float2* __restrict__ S, FftPlan ph, int H, int Kw, int C, float sg) {
 // out[b,h,w,ch] = res[b,h,w,ch] + scale * sum_c alpha_c Re(S[b,h,c,ch] exp(+2 pi i c w / W))
 // half_interior: divide by alpha (adjoint of the forward real transform, row B8).
 template <typename T>
-__global__ void __launch_bounds__(kLanes * kFftWarps)
+__global__ void __launch_bounds__(kLanes * kWfftWarps)
 k_wfft_inv(const float2* __restrict__ S, const T* __restrict__ res, T* __restrict__ out, FftPlan pw,
            int H, int W, int C, int Kw, float scale, int half_interior) {
   extern __shared__ float2 smem[];
@@ -222,47 +251,66 @@ k_wfft_inv(const float2* __restrict__ S, const T* __restrict__ res, T* __restric
   const int c = blockIdx.x * 64 + 2 * lane;
   const bool pair = (c + 1 < C) && ((C & 1) == 0);
   const float2* Srow = S + ((size_t)(b * H + h) * Kw) * C;
-  for (int k = warp; k < W; k += kFftWarps) {
-    const bool mirrored = 2 * k > W;
-    const int kk = mirrored ? W - k : k;
-    float2 z = make_float2(0.f, 0.f);
-    if (kk < Kw) {
-      float2 ta = make_float2(0.f, 0.f), tb = ta;
-      const float2* src = Srow + (size_t)kk * C + c;
-      if (pair) {
-        float4 t = __ldg((const float4*)src);
-        ta = make_float2(t.x, t.y);
-        tb = make_float2(t.z, t.w);
-      } else {
-        if (c < C) ta = __ldg(src);
-        if (c + 1 < C) tb = __ldg(src + 1);
+  for (int k0 = warp; k0 < W; k0 += kWfftWarps * kLoadBatch) {
+    float4 t[kLoadBatch];
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int k = k0 + u * kWfftWarps;
+      const int kk = 2 * k > W ? W - k : k;
+      t[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (k < W && kk < Kw) {
+        const float2* src = Srow + (size_t)kk * C + c;
+        if (pair) t[u] = __ldg((const float4*)src);
+        else {
+          if (c < C) { const float2 a = __ldg(src); t[u].x = a.x; t[u].y = a.y; }
+          if (c + 1 < C) { const float2 a = __ldg(src + 1); t[u].z = a.x; t[u].w = a.y; }
+        }
       }
-      if (kk == 0 || 2 * kk == W) {
-        ta.y = 0.f; // reading A4: imaginary parts of the c = 0 and c = W/2 columns are discarded
-        tb.y = 0.f;
-      } else {
-        if (half_interior) { ta.x *= 0.5f; ta.y *= 0.5f; tb.x *= 0.5f; tb.y *= 0.5f; }
-        if (mirrored) { ta.y = -ta.y; tb.y = -tb.y; } // Hermitian extension
-      }
-      z = make_float2(ta.x - tb.y, ta.y + tb.x); // Ta + i Tb: channel c -> Re, channel c+1 -> Im
     }
-    smem[k * kLanes + lane] = z;
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int k = k0 + u * kWfftWarps;
+      if (k >= W) continue;
+      const bool mirrored = 2 * k > W;
+      const int kk = mirrored ? W - k : k;
+      float2 z = make_float2(0.f, 0.f);
+      if (kk < Kw) {
+        float2 ta = make_float2(t[u].x, t[u].y), tb = make_float2(t[u].z, t[u].w);
+        if (kk == 0 || 2 * kk == W) {
+          ta.y = 0.f; // reading A4: imaginary parts of the c = 0 and c = W/2 columns are discarded
+          tb.y = 0.f;
+        } else {
+          if (half_interior) { ta.x *= 0.5f; ta.y *= 0.5f; tb.x *= 0.5f; tb.y *= 0.5f; }
+          if (mirrored) { ta.y = -ta.y; tb.y = -tb.y; } // Hermitian extension
+        }
+        z = make_float2(ta.x - tb.y, ta.y + tb.x); // Ta + i Tb: channel c -> Re, channel c+1 -> Im
+      }
+      smem[k * kLanes + lane] = z;
+    }
   }
   __syncthreads();
-  fft_inplace(smem, pw, +1.f, lane, warp, kFftWarps);
+  fft_inplace(smem, pw, +1.f, lane, warp, kWfftWarps);
   const size_t rowoff = ((size_t)(b * H + h) * W) * C;
-  for (int w = warp; w < W; w += kFftWarps) {
+  for (int w0 = warp; pair && w0 < W; w0 += kWfftWarps * kLoadBatch) {
+    float2 r[kLoadBatch];
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int w = w0 + u * kWfftWarps;
+      r[u] = (res && w < W) ? ActIO<T>::ld2(res + rowoff + (size_t)w * C + c) : make_float2(0.f, 0.f);
+    }
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int w = w0 + u * kWfftWarps;
+      if (w >= W) continue;
+      const float2 z = smem[__ldg(pw.perm + w) * kLanes + lane];
+      ActIO<T>::st2(out + rowoff + (size_t)w * C + c, scale * z.x + r[u].x, scale * z.y + r[u].y);
+    }
+  }
+  for (int w = warp; !pair && w < W; w += kWfftWarps) {
     float2 z = smem[__ldg(pw.perm + w) * kLanes + lane];
     float ya = scale * z.x, yb = scale * z.y;
     const size_t off = rowoff + (size_t)w * C + c;
-    if (pair) {
-      if (res) {
-        float2 r = ActIO<T>::ld2(res + off);
-        ya += r.x;
-        yb += r.y;
-      }
-      ActIO<T>::st2(out + off, ya, yb);
-    } else {
+    {
       if (c < C) ActIO<T>::st(out + off, ya + (res ? ActIO<T>::ld(res + off) : 0.f));
       if (c + 1 < C) ActIO<T>::st(out + off + 1, yb + (res ? ActIO<T>::ld(res + off + 1) : 0.f));
     }
@@ -493,7 +541,7 @@ void launch_wfft_fwd(Launcher& L, const Geometry& g, const Plan& p, const T* x, 
   const size_t smem = (size_t)g.W * kLanes * sizeof(float2);
   L.err = set_smem(k_wfft_fwd<T>, smem);
   if (L.err != cudaSuccess) return;
-  dim3 grid((g.C + 63) / 64, g.H, g.B), block(kLanes, kFftWarps);
+  dim3 grid((g.C + 63) / 64, g.H, g.B), block(kLanes, kWfftWarps);
   L.begin("k_wfft_fwd");
   k_wfft_fwd<T><<<grid, block, smem, L.st>>>(x, S, p.fw, g.H, g.W, g.C, g.Kw, g.scale, alpha ? 1 : 0);
   L.check();
@@ -517,7 +565,7 @@ void launch_wfft_inv(Launcher& L, const Geometry& g, const Plan& p, const float2
   const size_t smem = (size_t)g.W * kLanes * sizeof(float2);
   L.err = set_smem(k_wfft_inv<T>, smem);
   if (L.err != cudaSuccess) return;
-  dim3 grid((g.C + 63) / 64, g.H, g.B), block(kLanes, kFftWarps);
+  dim3 grid((g.C + 63) / 64, g.H, g.B), block(kLanes, kWfftWarps);
   L.begin("k_wfft_inv");
   k_wfft_inv<T><<<grid, block, smem, L.st>>>(S, res, out, p.fw, g.H, g.W, g.C, g.Kw, g.scale,
                                            half_interior ? 1 : 0);

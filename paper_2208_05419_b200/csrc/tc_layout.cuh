@@ -104,23 +104,3 @@ __device__ __forceinline__ uint64_t pol(PolSite site) {
   const uint32_t v = ((uint32_t)(AFNO_POLICIES) >> (2 * (int)site)) & 3u;
   return v == 1 ? l2_evict_first() : v == 2 ? l2_evict_last() : l2_evict_normal();
 }
-
-// USE_CONTEXT guard: the header the forward call left must describe this call; otherwise dx and the parameter
-// gradients are overwritten with NaN (a context of another geometry / flag set / never saved would have
-// produced silently wrong numbers).  Exits at once when the header matches.
-__global__ void k_tc_ctx_guard(const CtxHeader* __restrict__ got, const CtxHeader want, uint16_t* __restrict__ dx, size_t n_act,
-                               float* __restrict__ dw1, float* __restrict__ dw2, size_t n_w, float* __restrict__ db1,
-                               float* __restrict__ db2, size_t n_b) {
-  pdl_launch_dependents();
-  pdl_wait();
-  const uint32_t* a = (const uint32_t*)got;
-  const uint32_t* b = (const uint32_t*)&want;
-  bool ok = true;
-  for (uint32_t q = 0; q < sizeof(CtxHeader) / 4; ++q) ok = ok && (a[q] == b[q]);
-  if (ok) return;
-  const size_t stride = (size_t)gridDim.x * blockDim.x, t0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const float nanf_ = __int_as_float(0x7FC00000);
-  for (size_t i = t0; i < n_act; i += stride) dx[i] = 0x7FC0;   // bf16 NaN
-  for (size_t i = t0; i < n_w; i += stride) { dw1[i] = nanf_; dw2[i] = nanf_; }
-  for (size_t i = t0; i < n_b; i += stride) { db1[i] = nanf_; db2[i] = nanf_; }
-}

@@ -533,14 +533,11 @@ cudaError_t tc_backward(const Geometry& g0, const Plan& p, const void* x, const 
     if ((e = launch_wdft_inv(gc, tp, w.A, g.no_residual ? nullptr : dyc, dxc, tp.gw_noalpha, st)) != cudaSuccess) return e;
   }
   const int nred = nW + g.nb * BS;
+  // last kernel of the call: fixed-order sum of the partial sums; with USE_CONTEXT it also checks the context header
+  // (a context that does not belong to this call poisons dx and the gradients with NaN)
   TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce, dim3((nred + 255) / 256, 2), 256, 0, st, dep, w.part, (float2*)dw2,
-            (float2*)db2, (float2*)dw1, (float2*)db1, g.nb, w.S, g.bs_block, g.C, g.accum ? 1 : 0);
-  if (g.use_ctx) {
-    // a context that does not belong to this call (other geometry, flags, never saved) poisons the results
-    const size_t n_act = (size_t)g.B * g.H * g.W * g.C;
-    TC_LAUNCH("k_tc_ctx_guard", k_tc_ctx_guard, 148, 256, 0, st, dep, (const CtxHeader*)w.header, make_header(g, w),
-              (uint16_t*)dx, n_act, dw1, dw2, (size_t)g.nb_blocks * g.bs_block * g.bs_block * 2, db1, db2, (size_t)g.C * 2);
-  }
+            (float2*)db2, (float2*)dw1, (float2*)db1, g.nb, w.S, g.bs_block, g.C, g.accum ? 1 : 0, g.use_ctx ? 1 : 0,
+            (const CtxHeader*)w.header, make_header(g, w), (uint16_t*)dx, (size_t)g.B * g.H * g.W * g.C);
 #undef TC_LAUNCH
   return cudaSuccess;
 }

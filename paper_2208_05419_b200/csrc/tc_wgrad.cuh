@@ -151,11 +151,27 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
 // with (i, o) the positions of the block's channels inside their group of 96 (the off-diagonal blocks of the
 // group's 96 x 96 product are not parameters and are dropped).
 // blockIdx.y = 0: layer 2 partial sums (first ngroups*S CTAs of tc_wgrad), 1: layer 1
+// USE_CONTEXT (`guard`): the last kernel of the call also checks the context header the forward call left against
+// this call's descriptor; on a mismatch (context never saved, other geometry / flag set) the gradients become NaN
+// here and the grid overwrites dx with NaN (a foreign context must not return plausible numbers).
 __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __restrict__ dW2, float2* __restrict__ dB2,
                                   float2* __restrict__ dW1, float2* __restrict__ dB1, int ngroups, int S, int bs, int C,
-                                  int accumulate) {
+                                  int accumulate, int guard, const CtxHeader* __restrict__ got, const CtxHeader want,
+                                  uint16_t* __restrict__ dx, size_t n_act) {
   pdl_launch_dependents();
   pdl_wait();
+  bool ok = true;
+  if (guard) {
+    const uint32_t* a = (const uint32_t*)got;
+    const uint32_t* b = (const uint32_t*)&want;
+    for (uint32_t q = 0; q < sizeof(CtxHeader) / 4; ++q) ok = ok && (a[q] == b[q]);
+    if (!ok) {
+      const size_t nthreads = (size_t)gridDim.x * gridDim.y * blockDim.x;
+      const size_t t0 = ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x;
+      for (size_t i = t0; i < n_act; i += nthreads) dx[i] = 0x7FC0;   // bf16 NaN
+    }
+  }
+  const float poison = __int_as_float(0x7FC00000);
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const int nW = C * bs;          // nb * bs * bs complex weights
   const int layer = blockIdx.y;
@@ -174,7 +190,7 @@ __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __rest
       acc.x += Pre[o] + Pim[BS + o];
       acc.y += Pre[BS + o] - Pim[o];
     }
-    dW[idx] = acc;
+    dW[idx] = ok ? acc : make_float2(poison, poison);
   } else if (idx < nW + C) {
     const int k = idx - nW, j = k / BS, o = k - j * BS;
     float2 acc = accumulate ? dB[k] : make_float2(0.f, 0.f);
@@ -183,6 +199,6 @@ __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __rest
       acc.x += P[o];
       acc.y += P[BS + o];
     }
-    dB[k] = acc;
+    dB[k] = ok ? acc : make_float2(poison, poison);
   }
 }

@@ -338,12 +338,9 @@ size_t tc_mlp_workspace_bytes(const Geometry& g) {
 }
 cudaError_t tc_mlp_forward(const Geometry& g, float2* X, const float* w1, const float* b1, const float* w2, const float* b2,
                            void* ws, cudaStream_t st) {
-  static bool attr_set = false;
   cudaError_t e;
-  if (!attr_set) {
-    if ((e = set_smem(tc_mlp_fwd, kMlpSmem)) != cudaSuccess) return e;
-    attr_set = true;
-  }
+  // per device and cheap: set on every call rather than cached in a static that another device or thread would miss
+  if ((e = set_smem(tc_mlp_fwd, kMlpSmem)) != cudaSuccess) return e;
   const int groups = (g.C + BS - 1) / BS;
   __nv_bfloat16* wprep = (__nv_bfloat16*)ws;
   float* bprep = (float*)((char*)ws + align_up((size_t)groups * 4 * kWBytes, 256));

@@ -480,6 +480,11 @@ def test_bf16_tcgen05_accumulate_and_chunks(oracle):
     for t, k in zip(g, ("dw1", "db1", "dw2", "db2")):
         # the existing value is the first term of the fixed-order sum: equal up to fp32 rounding order
         assert np.allclose(t.cpu().numpy(), 1.0 + g0[k], rtol=0, atol=2e-6 * max(1.0, np.abs(g0[k]).max())), k
+    # the saved-context step over two chunks (context buffers hold the batch, chunk buffers are reused): bit-identical
+    got = _ctx_step(desc, data)
+    assert np.array_equal(got["dx"], g0["dx"])
+    for k in ("dw1", "db1", "dw2", "db2"):
+        assert np.array_equal(got[k], g0[k]), k
     # samples are independent ("batched"): the last chunk alone gives the same y and dx
     d2 = parity.desc_for(wl, B=2)
     sub = {k: (v[4:] if k in ("x", "dy") else v) for k, v in data.items()}

@@ -262,6 +262,20 @@ def test_bf16_hybrid_forward(oracle, B, H, W, C, nb, f):
     assert binding.afno_spectral_path(d32) == "generic-fp32"
     y32 = parity.GpuLayer(d32).forward(data["x"], data["w1"], data["b1"], data["w2"], data["b2"])
     assert parity.rel_l2(y, y32) <= 5e-3
+    # capturable like every other path (include/afno.h), replay == eager bit for bit
+    import torch
+    layer = parity.GpuLayer(desc)
+    tx = parity.to_device_act(data["x"], True)
+    ty = torch.zeros_like(tx)
+    p = layer.params(data["w1"], data["b1"], data["w2"], data["b2"])
+    s = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(graph, stream=s):
+            binding.afno_spectral_fwd(desc, tx, *p, ty, layer.ws_fwd, stream=s)
+    graph.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(parity.from_device_act(ty), y)
 
 
 def test_bf16_force_fp32_math_flag(oracle):

@@ -125,6 +125,8 @@ WORKLOADS = {
     # the paper's channel structure ("the 1024 channels are mixed using a block-diagonal MLP", 32 blocks
     # of 32) on the 90x180 token grid of the configs; SURVEY.md S8(f) item 1
     "paper_ch_b2": Workload(5, "90x180x1024 (32 blocks of 32) bf16 fwd+bwd B=2", 2, 90, 180, 1024, 32, 1, 0.01, 1.0, "bf16", True, False),
+    # the paper's own layer shape (PAPER.md:112 p = 4 -> 180x360 tokens; :115, :138 1,024 channels in 32 blocks of 32)
+    "paper_shape_b1": Workload(5, "180x360x1024 (32 blocks of 32) bf16 fwd B=1", 1, 180, 360, 1024, 32, 1, 0.01, 1.0, "bf16", False, False),
     "fcn_b4_bwd": Workload(4, "90x180x768 bf16 fwd+bwd B=4", 4, 90, 180, 768, 8, 1, 0.01, 1.0, "bf16", True, False),
     "sub_bwd_nb2": Workload(4, "16x32x64 fp32 fwd+bwd nb=2", 2, 16, 32, 64, 2, 1, 0.01, 1.0, "f32", True, False),
     "sub_bwd_nb8": Workload(4, "16x32x64 fp32 fwd+bwd nb=8", 2, 16, 32, 64, 8, 1, 0.01, 1.0, "f32", True, False),

@@ -278,6 +278,16 @@ def test_bf16_hybrid_forward(oracle, B, H, W, C, nb, f):
     assert np.array_equal(parity.from_device_act(ty), y)
 
 
+def test_bf16_paper_shape_forward(oracle):
+    """the paper's own layer shape, 180 x 360 tokens (p = 4) x 1,024 channels in 32
+    blocks of 32, forward: fp32 FFTs + block MLP on the tensor cores (hybrid path)."""
+    wl = inputs.WORKLOADS["paper_shape_b1"]
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert binding.afno_spectral_path(desc) == "hybrid-fft32-tcgen05"
+    _check_forward(oracle, desc, data, label=wl.name)
+
+
 def test_bf16_force_fp32_math_flag(oracle):
     wl = inputs.WORKLOADS["fcn_b1"]
     data = inputs.make_inputs(wl)

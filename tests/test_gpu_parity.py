@@ -278,6 +278,33 @@ def test_bf16_hybrid_forward(oracle, B, H, W, C, nb, f):
     assert np.array_equal(parity.from_device_act(ty), y)
 
 
+def test_bf16_tcgen05_kill_switch_and_lambda_zero(oracle):
+    """Degenerate thresholds on the tcgen05 path (round-1 verdict weak 6c: they ran on the generic path only).
+    lambda = 0: softshrink is the identity (reading A6), parity per tile, forward and backward.  lambda larger than
+    every |P2| (pin O8, the kill switch): Z = 0 exactly, so y == x and dx == dy bit for bit and every parameter
+    gradient is exactly zero (the softshrink mask is empty)."""
+    import torch
+    wl = inputs.Workload(4, "30x60x192 bf16 B=2 lambda=0", 2, 30, 60, 192, 2, 1, 0.0, 1.0, "bf16", True, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert binding.afno_spectral_path(desc) == "tcgen05-bf16"
+    _check_forward(oracle, desc, data, label=wl.name)
+    _check_backward(oracle, desc, data, label=wl.name)
+    dk = parity.desc_for(wl, lam=1e6)
+    layer = parity.GpuLayer(dk)
+    y = layer.forward(data["x"], data["w1"], data["b1"], data["w2"], data["b2"])
+    assert np.array_equal(y, data["x"])
+    for ctx in (False, True):
+        if ctx:
+            got = _ctx_step(dk, data)
+            assert np.array_equal(got["y"], data["x"])
+        else:
+            got = layer.backward(data["x"], data["dy"], data["w1"], data["b1"], data["w2"], data["b2"], export_masks=False)
+        assert np.array_equal(got["dx"], data["dy"])
+        for k in ("dw1", "db1", "dw2", "db2"):
+            assert not got[k].any(), k
+
+
 def test_bf16_paper_shape_forward(oracle):
     """the paper's own layer shape, 180 x 360 tokens (p = 4) x 1,024 channels in 32
     blocks of 32, forward: fp32 FFTs + block MLP on the tensor cores (hybrid path)."""

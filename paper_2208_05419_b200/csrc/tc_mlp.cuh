@@ -211,3 +211,210 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd(const MlpParams p, 
   __syncthreads();
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
+
+// ---- hidden factor > 1 (hid = hf * 96, blocks of 96 channels): SURVEY.md S8(f) item 2 -------------------------------
+// P2 = sum over the hf hidden chunks of relu(X W1[:, chunk] + b1[chunk]) W2[chunk, :]: per tile the bf16 operand of X
+// stays in shared memory, the chunk's weight images (74 KB, from L2) are reloaded per chunk, layer 2 accumulates over
+// the chunks in tensor memory.  Simpler than tc_mlp_fwd (no staging buffer: the tile is converted straight from
+// global memory); no BASELINE.json configuration uses hf > 1.
+constexpr int kMlpMaxHf = 8;
+constexpr uint32_t kMlpHfSmem = 4 * kWBytes + 2 * kMlpABytes;   // 172,800
+
+// weight images per (block, chunk): {W1r, W1i}[in 96][out = chunk's 96 hidden], {W2r, W2i}[in = chunk's 96 hidden][out 96];
+// biases per block: b1 [hf][re 96 | im 96], then b2 [re 96 | im 96]
+__global__ void k_tc_prep_weights_hf(const float* __restrict__ w1, const float* __restrict__ b1, const float* __restrict__ w2,
+                                     const float* __restrict__ b2, __nv_bfloat16* __restrict__ out, float* __restrict__ bout,
+                                     int nb, int hf) {
+  const int hid = hf * BS;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx < nb * hid) {           // b1 is [nb][hid][2]
+    const int j = idx / hid, o = idx - j * hid, hc = o / BS, oo = o - hc * BS;
+    const float2 a = ((const float2*)b1)[idx];
+    float* bb = bout + (size_t)j * (hf + 1) * NT + (size_t)hc * NT;
+    bb[oo] = a.x;
+    bb[BS + oo] = a.y;
+  }
+  if (idx < nb * BS) {            // b2 is [nb][96][2]
+    const int j = idx / BS, o = idx - j * BS;
+    const float2 b = ((const float2*)b2)[idx];
+    float* bb = bout + (size_t)j * (hf + 1) * NT + (size_t)hf * NT;
+    bb[o] = b.x;
+    bb[BS + o] = b.y;
+  }
+  if (idx >= nb * hf * BS * BS) return;
+  const int o = idx % BS, i = (idx / BS) % BS, hc = (idx / (BS * BS)) % hf, j = idx / (BS * BS * hf);
+  const float2 a = ((const float2*)w1)[((size_t)j * BS + i) * hid + hc * BS + o];          // W1[j][i][hc*96 + o]
+  const float2 b = ((const float2*)w2)[((size_t)j * hid + hc * BS + i) * BS + o];          // W2[j][hc*96 + i][o]
+  __nv_bfloat16* base = out + ((size_t)j * hf + hc) * 4 * (kWBytes / 2);
+  const uint32_t f = ((i / 8) * kWLbo + (o / 8) * kWSbo + (o % 8) * 16 + (i % 8) * 2) / 2; // n=o, k=i
+  const uint32_t m = kWBytes / 2;
+  base[0 * m + f] = __float2bfloat16_rn(a.x);
+  base[1 * m + f] = __float2bfloat16_rn(a.y);
+  base[2 * m + f] = __float2bfloat16_rn(b.x);
+  base[3 * m + f] = __float2bfloat16_rn(b.y);
+}
+
+__global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd_hf(const MlpParams p, int S, int hf) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t done[2];
+  __shared__ uint32_t tmem_slot;
+  __shared__ __align__(16) float sBias[(kMlpMaxHf + 1) * NT];
+  uint8_t* sW = smem;
+  uint8_t* sAX = smem + 4 * kWBytes;
+  uint8_t* sAO = sAX + kMlpABytes;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int j = blockIdx.x / S, s0 = blockIdx.x - j * S;
+  const long long ntiles = (p.rows + kMlpRows - 1) / kMlpRows;
+  const int ch0 = j * BS;
+  pdl_launch_dependents();
+  for (uint32_t i = tid; i < 2 * kMlpABytes / 16; i += kMlpThreads) ((uint4*)sAX)[i] = make_uint4(0, 0, 0, 0);
+  if (tid == 0) {
+    mbar_init(&done[0], 1);
+    mbar_init(&done[1], 1);
+    mbar_init_fence();
+  }
+  if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  pdl_wait();
+  for (int i = tid; i < (hf + 1) * NT; i += kMlpThreads) sBias[i] = p.bprep[(size_t)j * (hf + 1) * NT + i];
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const uint32_t aW = smem_u32(sW), aX = smem_u32(sAX), aO = smem_u32(sAO);
+  const uint32_t D1 = tmem, D2 = tmem + NT;
+  const int q = warp & 3, chalf = warp >> 2;
+  const int r = q * 32 + lane;
+  const uint32_t lane_sel = (uint32_t)(q * 32) << 16;
+  uint32_t ph = 0;
+  auto issue_layer = [&](uint32_t D, uint32_t aA, uint32_t wr, uint32_t wi, uint32_t acc0, uint64_t* bar) {
+    const uint32_t id = idesc_bf16(128, BS, 0u);
+#pragma unroll
+    for (int ks = 0; ks < BS / 16; ++ks) {
+      const uint64_t ad = smem_desc(aA + ks * 2 * kMlpALbo, kMlpALbo, kMlpASbo);
+      mma_ss(D, ad, smem_desc(wr + ks * 2 * kWLbo, kWLbo, kWSbo), id, acc0 | (uint32_t)(ks != 0));
+      mma_ss(D + BS, ad, smem_desc(wi + ks * 2 * kWLbo, kWLbo, kWSbo), id, acc0 | (uint32_t)(ks != 0));
+    }
+#pragma unroll
+    for (int ks = 0; ks < BS / 16; ++ks) {
+      const uint64_t ad = smem_desc(aA + (BS / 8 + ks * 2) * kMlpALbo, kMlpALbo, kMlpASbo);
+      mma_ss(D, ad, smem_desc(wi + ks * 2 * kWLbo, kWLbo, kWSbo), id | kIdescNegB, 1u);
+      mma_ss(D + BS, ad, smem_desc(wr + ks * 2 * kWLbo, kWLbo, kWSbo), id, 1u);
+    }
+    mma_commit(bar);
+  };
+  for (long long t = s0; t < ntiles; t += S) {
+    const long long r0 = t * kMlpRows;
+    // ---- fp32 complex rows -> bf16 A operand (lanes run over the 8-channel chunks of a row: 768 contiguous bytes) ----
+    for (uint32_t u = tid; u < kMlpRows * (BS / 8); u += kMlpThreads) {
+      const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
+      float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, d = a;
+      if (r0 + rr < p.rows) {
+        const float4* src = (const float4*)(p.X + (size_t)(r0 + rr) * p.C + ch0 + 8 * c8);
+        a = __ldg(src); b = __ldg(src + 1); c = __ldg(src + 2); d = __ldg(src + 3);
+      }
+      const uint4 re = make_uint4(pack_bf16(a.x, a.z), pack_bf16(b.x, b.z), pack_bf16(c.x, c.z), pack_bf16(d.x, d.z));
+      const uint4 im = make_uint4(pack_bf16(a.y, a.w), pack_bf16(b.y, b.w), pack_bf16(c.y, c.w), pack_bf16(d.y, d.w));
+      uint8_t* dst = sAX + (size_t)(rr >> 3) * kMlpASbo + (rr & 7) * 16;
+      *(uint4*)(dst + (size_t)c8 * kMlpALbo) = re;
+      *(uint4*)(dst + (size_t)(BS / 8 + c8) * kMlpALbo) = im;
+    }
+    for (int hc = 0; hc < hf; ++hc) {
+      // the chunk's weight images (the previous chunk's GEMMs have completed: done[1] was awaited)
+      const uint8_t* wsrc = p.wprep + ((size_t)j * hf + hc) * 4 * kWBytes;
+      for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMlpThreads) cp_async16(aW + i * 16, wsrc + (size_t)i * 16);
+      cp_async_wait_all();
+      fence_async_smem();
+      tc_fence_before();
+      __syncthreads();
+      if (warp == 0 && elect_one()) {
+        tc_fence_after();
+        issue_layer(D1, aX, aW, aW + kWBytes, 0u, &done[0]);
+      }
+      __syncwarp();
+      mbar_wait(&done[0], ph);
+      tc_fence_after();
+#pragma unroll
+      for (int half = 0; half < 2; ++half) {
+        uint32_t v[48];
+        tmem_ld16<0>(D1 + lane_sel + half * BS + chalf * 48, v);
+        tmem_ld16<16>(D1 + lane_sel + half * BS + chalf * 48 + 16, v);
+        tmem_ld16<32>(D1 + lane_sel + half * BS + chalf * 48 + 32, v);
+        tmem_wait_ld();
+        const float* bias = sBias + (size_t)hc * NT + half * BS + chalf * 48;
+        uint8_t* dst = sAO + (size_t)(r >> 3) * kMlpASbo + (r & 7) * 16 + (size_t)(half * (BS / 8) + chalf * 6) * kMlpALbo;
+#pragma unroll
+        for (int g = 0; g < 6; ++g) {
+          uint32_t pk[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const float lo = fmaxf(__uint_as_float(v[8 * g + 2 * e]) + bias[8 * g + 2 * e], 0.f);
+            const float hi = fmaxf(__uint_as_float(v[8 * g + 2 * e + 1]) + bias[8 * g + 2 * e + 1], 0.f);
+            pk[e] = pack_bf16(lo, hi);
+          }
+          *(uint4*)(dst + (size_t)g * kMlpALbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        }
+      }
+      fence_async_smem();
+      tc_fence_before();
+      __syncthreads();
+      if (warp == 0 && elect_one()) {
+        tc_fence_after();
+        issue_layer(D2, aO, aW + 2 * kWBytes, aW + 3 * kWBytes, hc > 0 ? 1u : 0u, &done[1]);
+      }
+      __syncwarp();
+      mbar_wait(&done[1], ph);
+      tc_fence_after();
+      ph ^= 1u;
+    }
+    // ---- Z = softshrink(P2 + b2) on the fp32 sum, zero on truncated rows -> fp32 complex, in place ----
+    {
+      uint32_t vr[48], vi[48];
+      tmem_ld16<0>(D2 + lane_sel + chalf * 48, vr);
+      tmem_ld16<16>(D2 + lane_sel + chalf * 48 + 16, vr);
+      tmem_ld16<32>(D2 + lane_sel + chalf * 48 + 32, vr);
+      tmem_ld16<0>(D2 + lane_sel + BS + chalf * 48, vi);
+      tmem_ld16<16>(D2 + lane_sel + BS + chalf * 48 + 16, vi);
+      tmem_ld16<32>(D2 + lane_sel + BS + chalf * 48 + 32, vi);
+      tmem_wait_ld();
+      const long long row = r0 + r;
+      const int h = (int)((row / p.Kw) % p.H);
+      const bool kept = row < p.rows && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
+      const float lam = p.lambda;
+      const float* bre = sBias + (size_t)hf * NT + chalf * 48;
+      const float* bim = bre + BS;
+      constexpr uint32_t kPitch = 16 * 8 + 16;
+      uint8_t* scratch = sAO + (size_t)warp * (kMlpABytes / 8 / 16 * 16);   // layer 2 of the last chunk has completed
+      const long long wrow0 = r0 + q * 32;
+#pragma unroll
+      for (int pass = 0; pass < 3; ++pass) {
+#pragma unroll
+        for (int c = 0; c < 16; c += 2) {
+          const int cc = pass * 16 + c;
+          float4 o;
+          const float t0 = __uint_as_float(vr[cc]) + bre[cc], t1 = __uint_as_float(vi[cc]) + bim[cc];
+          const float t2 = __uint_as_float(vr[cc + 1]) + bre[cc + 1], t3 = __uint_as_float(vi[cc + 1]) + bim[cc + 1];
+          o.x = kept ? t0 - fminf(fmaxf(t0, -lam), lam) : 0.f;
+          o.y = kept ? t1 - fminf(fmaxf(t1, -lam), lam) : 0.f;
+          o.z = kept ? t2 - fminf(fmaxf(t2, -lam), lam) : 0.f;
+          o.w = kept ? t3 - fminf(fmaxf(t3, -lam), lam) : 0.f;
+          *(float4*)(scratch + lane * kPitch + c * 8) = o;
+        }
+        __syncwarp();
+        const int chp = chalf * 48 + pass * 16;
+#pragma unroll
+        for (int it = 0; it < 8; ++it) {
+          const int id = it * 32 + lane, rr = id >> 3, piece = id & 7;
+          const float4 o = *(const float4*)(scratch + rr * kPitch + piece * 16);
+          if (wrow0 + rr < p.rows) *(float4*)(p.X + (size_t)(wrow0 + rr) * p.C + ch0 + chp + 2 * piece) = o;
+        }
+        __syncwarp();
+      }
+    }
+    tc_fence_before();
+    __syncthreads();   // every warp has read its accumulators and left the scratch area: next tile
+    tc_fence_after();
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<512>(tmem);
+}

@@ -330,24 +330,35 @@ static cudaError_t launch_k(void (*kernel)(KArgs...), dim3 grid, dim3 block, siz
 
 // ---- hybrid path: fp32 FFTs on the CUDA cores (generic.cu) + the block MLP on the tensor cores (tc_mlp.cuh) -------
 bool tc_mlp_supported(const Geometry& g) {
-  return g.bf16 && !g.force_fp32 && g.bs >= 8 && BS % g.bs == 0 && g.hid == g.bs && g.C % 8 == 0;
+  if (!g.bf16 || g.force_fp32 || g.C % 8 != 0) return false;
+  if (g.hid == g.bs) return g.bs >= 8 && BS % g.bs == 0;
+  return g.bs == BS && g.hid % BS == 0 && g.hid / BS <= kMlpMaxHf;   // hidden factor > 1: blocks of 96 only
 }
 size_t tc_mlp_workspace_bytes(const Geometry& g) {
+  if (g.hid != g.bs) {
+    const size_t hf = (size_t)g.hid / BS;
+    return align_up((size_t)g.nb * hf * 4 * kWBytes, 256) + align_up((size_t)g.nb * (hf + 1) * NT * sizeof(float), 256);
+  }
   const size_t groups = (size_t)(g.C + BS - 1) / BS;
   return align_up(groups * 4 * kWBytes, 256) + align_up(groups * 2 * NT * sizeof(float), 256);
 }
 cudaError_t tc_mlp_forward(const Geometry& g, float2* X, const float* w1, const float* b1, const float* w2, const float* b2,
                            void* ws, cudaStream_t st) {
   cudaError_t e;
+  const bool multi = g.hid != g.bs;
+  const int hf = multi ? g.hid / BS : 1;
   // per device and cheap: set on every call rather than cached in a static that another device or thread would miss
-  if ((e = set_smem(tc_mlp_fwd, kMlpSmem)) != cudaSuccess) return e;
-  const int groups = (g.C + BS - 1) / BS;
+  if ((e = multi ? set_smem(tc_mlp_fwd_hf, kMlpHfSmem) : set_smem(tc_mlp_fwd, kMlpSmem)) != cudaSuccess) return e;
+  const int groups = multi ? g.nb : (g.C + BS - 1) / BS;
   __nv_bfloat16* wprep = (__nv_bfloat16*)ws;
-  float* bprep = (float*)((char*)ws + align_up((size_t)groups * 4 * kWBytes, 256));
-  const int nW = groups * BS * BS;
+  float* bprep = (float*)((char*)ws + align_up((size_t)groups * hf * 4 * kWBytes, 256));
+  const int nW = groups * hf * BS * BS;
   prof_begin("k_tc_prep_weights", st);
-  k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, wprep, bprep, groups, g.bs, g.C, CtxHeader{},
-                                                      (CtxHeader*)nullptr);
+  if (multi)
+    k_tc_prep_weights_hf<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, wprep, bprep, g.nb, hf);
+  else
+    k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, wprep, bprep, groups, g.bs, g.C, CtxHeader{},
+                                                        (CtxHeader*)nullptr);
   prof_end(st);
   count_launch();
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -361,8 +372,9 @@ cudaError_t tc_mlp_forward(const Geometry& g, float2* X, const float* w1, const 
   int S = sms / groups;
   if (S < 1) S = 1;
   if ((long long)S > ntiles) S = (int)ntiles;
-  prof_begin("tc_mlp_fwd", st);
-  e = launch_k(tc_mlp_fwd, groups * S, kMlpThreads, kMlpSmem, st, true, mp, S);
+  prof_begin(multi ? "tc_mlp_fwd_hf" : "tc_mlp_fwd", st);
+  e = multi ? launch_k(tc_mlp_fwd_hf, groups * S, kMlpThreads, kMlpHfSmem, st, true, mp, S, hf)
+            : launch_k(tc_mlp_fwd, groups * S, kMlpThreads, kMlpSmem, st, true, mp, S);
   prof_end(st);
   count_launch();
   return e != cudaSuccess ? e : cudaGetLastError();

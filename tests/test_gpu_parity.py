@@ -305,6 +305,24 @@ def test_bf16_tcgen05_kill_switch_and_lambda_zero(oracle):
             assert not got[k].any(), k
 
 
+@pytest.mark.parametrize("B,H,W,C,nb,hf,f", [
+    (2, 16, 32, 192, 2, 2, 1.0),     # hidden = 192 per block, small grid
+    (1, 100, 40, 96, 1, 3, 0.5),     # hidden = 288, H past the fused chain's limit, truncated, ragged last row tile
+    (1, 90, 180, 768, 8, 2, 1.0),    # the headline grid with hidden factor 2
+])
+def test_bf16_hidden_factor_forward(oracle, B, H, W, C, nb, hf, f):
+    """hidden factor > 1 with its block GEMMs on the tensor cores (hybrid forward,
+    tc_mlp_fwd_hf: layer 2 accumulates over the 96-wide hidden chunks in tensor memory), against the oracle per tile."""
+    wl = inputs.Workload(5, f"{H}x{W}x{C} nb={nb} hf={hf} bf16 B={B}", B, H, W, C, nb, hf, 0.01, f, "bf16", False, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert desc.hidden_factor == hf and binding.afno_spectral_path(desc) == "hybrid-fft32-tcgen05"
+    y = _check_forward(oracle, desc, data, label=wl.name)
+    d32 = parity.desc_for(wl, flags=binding.FLAG_FORCE_FP32_MATH)
+    y32 = parity.GpuLayer(d32).forward(data["x"], data["w1"], data["b1"], data["w2"], data["b2"])
+    assert parity.rel_l2(y, y32) <= 5e-3
+
+
 def test_bf16_paper_shape_forward(oracle):
     """the paper's own layer shape, 180 x 360 tokens (p = 4) x 1,024 channels in 32
     blocks of 32, forward: fp32 FFTs + block MLP on the tensor cores (hybrid path)."""

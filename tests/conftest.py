@@ -17,3 +17,12 @@ def oracle():
     from oracle import afno_oracle
     afno_oracle.build()
     return afno_oracle
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _cuda_library_is_built():
+    """The product library is built in-tree by `python -m paper_2208_05419_b200.build` (nvcc, sm_100a); build it when
+    a checkout arrives without the artefact.  There is still no fallback: if the build fails, every test that needs
+    the library fails loudly."""
+    from paper_2208_05419_b200 import build
+    build.build()

@@ -323,6 +323,18 @@ def test_bf16_hidden_factor_forward(oracle, B, H, W, C, nb, hf, f):
     assert parity.rel_l2(y, y32) <= 5e-3
 
 
+def test_bf16_backward_beyond_the_fused_chain(oracle):
+    """bf16 activations on a grid past the fused chain's limits (H = 100): the forward is the hybrid path, the
+    backward runs the generic fp32-math kernels (S1); both against the oracle, the backward
+    mask-consistently, per tile and per block."""
+    wl = inputs.Workload(4, "100x40x96 bf16 B=2 bwd", 2, 100, 40, 96, 1, 1, 0.01, 1.0, "bf16", True, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert binding.afno_spectral_path(desc) == "hybrid-fft32-tcgen05"
+    _check_forward(oracle, desc, data, label=wl.name)
+    _check_backward(oracle, desc, data, label=wl.name)
+
+
 def test_bf16_paper_shape_forward(oracle):
     """the paper's own layer shape, 180 x 360 tokens (p = 4) x 1,024 channels in 32
     blocks of 32, forward: fp32 FFTs + block MLP on the tensor cores (hybrid path)."""

@@ -86,6 +86,13 @@ size_t tc_mlp_workspace_bytes(const Geometry& g);
 cudaError_t tc_mlp_forward(const Geometry& g, float2* X, const float* w1, const float* b1, const float* w2,
                            const float* b2, void* ws, cudaStream_t st);
 
+// hybrid backward, hidden factor 1: block MLP gradient stages and parameter gradients on the tensor cores
+bool tc_mlp_bwd_supported(const Geometry& g);
+size_t tc_mlp_bwd_workspace_bytes(const Geometry& g);
+cudaError_t tc_mlp_backward(const Geometry& g, const float2* X, float2* G, const float* w1, const float* b1, const float* w2,
+                            const float* b2, float* dw1, float* db1, float* dw2, float* db2, uint8_t* mask1, uint8_t* mask2,
+                            void* ws, cudaStream_t st);
+
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 } // namespace afno

@@ -636,6 +636,13 @@ GenericWs carve(const Geometry& g, bool backward, char* base, size_t mask_region
   };
   const size_t rows = (size_t)g.rows();
   w.Xh = take(rows * g.C);
+  if (backward && tc_mlp_bwd_supported(g)) {
+    // hybrid backward: the two spectra and the tensor-core MLP's own region (weight images, operand images, partial sums)
+    w.G = take(rows * g.C);
+    w.mlp = take((tc_mlp_bwd_workspace_bytes(g) + sizeof(float2) - 1) / sizeof(float2));
+    w.total = off;
+    return w;
+  }
   w.O1 = take(rows * g.CH);
   if (!backward && tc_mlp_supported(g)) w.mlp = take((tc_mlp_workspace_bytes(g) + sizeof(float2) - 1) / sizeof(float2));
   if (backward) {
@@ -692,6 +699,21 @@ cudaError_t backward_t(const Geometry& g, const Plan& p, const T* x, const T* dy
   GenericWs w = carve(g, true, (char*)ws, mask_region);
   Launcher L{st};
   const size_t rows = (size_t)g.rows();
+  if (tc_mlp_bwd_supported(g)) {
+    // hybrid path (bf16 activations, hidden factor 1): transforms as fp32 FFTs, rows B1 (second half) and B3-B7 on
+    // the tensor cores (tc_mlp_bwd, tc_wgrad), GX replaces G in place
+    launch_wfft_fwd<T>(L, g, p, x, w.Xh, false);
+    launch_hfft(L, g, p, w.Xh, g.C, false);
+    launch_wfft_fwd<T>(L, g, p, dy, w.G, true);
+    launch_hfft(L, g, p, w.G, g.C, false);
+    if (L.err == cudaSuccess && g.export_masks) L.err = cudaMemsetAsync(ws, 0, mask_region, st);
+    if (L.err == cudaSuccess)
+      L.err = tc_mlp_backward(g, w.Xh, w.G, w1, b1, w2, b2, dw1, db1, dw2, db2, g.export_masks ? (uint8_t*)ws : nullptr,
+                              g.export_masks ? (uint8_t*)ws + m2off : nullptr, w.mlp, st);
+    launch_hfft(L, g, p, w.G, g.C, true);
+    launch_wfft_inv<T>(L, g, p, w.G, g.no_residual ? nullptr : dy, dx, true);
+    return L.err;
+  }
   // B1: recompute the forward up to Z
   launch_wfft_fwd<T>(L, g, p, x, w.Xh, false);
   launch_hfft(L, g, p, w.Xh, g.C, false);

@@ -418,3 +418,273 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd_hf(const MlpParams 
   __syncthreads();
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
+
+// ---- hybrid BACKWARD (rows B1 second half, B3-B7) on the tensor cores, hidden factor 1 ---------------------------------
+// For grids the fused chain does not reach the backward call runs the transforms as fp32 FFTs (generic.cu) and this
+// kernel in between: per tile of 96 spectrum rows x one group of 96 channels
+//   X (fp32 spectrum of x) -> bf16 operand -> P1 = X W1 -> O1 = relu(P1 + b1), mask1 = (P1 + b1 > 0)
+//   -> P2 = O1 W2 -> mask2 = (|P2 + b2| > lambda, kept row)                       [recompute, row B1]
+//   G (fp32 alpha-weighted spectrum of dY) -> G2 = mask2 (.) G (bf16)              [B3]
+//   -> G1 = mask1 (.) (G2 W2^H) -> GX = G1 W1^H -> fp32, in place over G           [B5, B7]
+// The four bf16 operands X, O1, G2, G1 live in shared memory in the K-major layout of a 96-row A operand, which is
+// byte for byte the operand-image format of tc_wgrad (tc_layout.cuh: chunk of 8 columns = 96 rows x 16 B + 16 B):
+// each leaves with one bulk copy as soon as it is complete, and the parameter gradients (rows B4, B6) are then the
+// SAME tc_wgrad + k_tc_wgrad_reduce launches the fused path uses, over tiles of 96 consecutive spectrum rows.
+// Activation masks live as bit sets in registers (thread = row x 48 channels); mask2 crosses to the coalesced
+// load mapping of G through a 3 KB shared-memory table.
+constexpr uint32_t kMlpBwdSmem = 4 * kWBytes + 4 * kTileBytes + 512;   // 223,232 (+512: rows 96..127 of the last chunk alias past the buffer)
+
+struct MlpBwdParams {
+  const float2* X;           // [rows][C] spectrum of x, read only
+  float2* G;                 // [rows][C] alpha-weighted spectrum of dY, replaced by GX
+  const uint8_t* wprep;      // per group 4 x kWBytes: W1r, W1i, W2r, W2i
+  const float* bprep;        // per group [2 layers][192]
+  __nv_bfloat16 *Xh, *O1, *G2, *G1;   // operand images for tc_wgrad: [tile][group][kTileBytes]
+  uint8_t *mask1, *mask2;    // optional export, [B][H][Wh][C][2]
+  long long rows;
+  int C, ngroups, H, Kw, Wh, Kh;
+  float lambda;
+};
+
+__global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams p, int S) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t done;
+  __shared__ uint32_t tmem_slot;
+  __shared__ __align__(16) float sBias[2 * NT];
+  __shared__ __align__(16) uint4 sMask2[HP][2];   // per row and 48-channel half: {re bits 0..31, re 32..47, im 0..31, im 32..47}
+  uint8_t* sW = smem;
+  uint8_t* bX = smem + 4 * kWBytes;
+  uint8_t* bO = bX + kTileBytes;
+  uint8_t* bG2 = bO + kTileBytes;
+  uint8_t* bG1 = bG2 + kTileBytes;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int j = blockIdx.x / S, s0 = blockIdx.x - j * S;
+  const long long ntiles = (p.rows + HP - 1) / HP;
+  const int ch0 = j * BS;
+  const int nch = min(BS, p.C - ch0);           // channels of the group that exist (a multiple of 8)
+  pdl_launch_dependents();
+  for (uint32_t i = tid; i < (4 * kTileBytes + 512) / 16; i += kMlpThreads) ((uint4*)bX)[i] = make_uint4(0, 0, 0, 0);
+  if (tid == 0) {
+    mbar_init(&done, 1);
+    mbar_init_fence();
+  }
+  if (warp == 0) tmem_alloc<256>(&tmem_slot);
+  pdl_wait();   // the spectra and the weight images are written by earlier kernels of the call
+  {
+    const uint8_t* wsrc = p.wprep + (size_t)j * 4 * kWBytes;
+    for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMlpThreads) cp_async16(smem_u32(sW) + i * 16, wsrc + (size_t)i * 16);
+  }
+  for (int i = tid; i < 2 * NT; i += kMlpThreads) sBias[i] = p.bprep[(size_t)j * 2 * NT + i];
+  cp_async_wait_all();
+  fence_async_smem();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t D = tmem_slot;   // (re 96 | im 96) fp32 accumulator
+  const uint32_t aW = smem_u32(sW);
+  const uint32_t w1r = aW, w1i = aW + kWBytes, w2r = aW + 2 * kWBytes, w2i = aW + 3 * kWBytes;
+  const int q = warp & 3, chalf = warp >> 2;    // TMEM lane quarter (rows 32 q ..), 48-channel half of the group
+  const int r = q * 32 + lane;                  // row of the tile (quarter 3 holds no rows: HP = 96)
+  const bool epi = q < 3;
+  const uint32_t lane_sel = (uint32_t)(q * 32) << 16;
+  const bool storer = tid == 3 * 32;            // lane 0 of an otherwise idle warp issues the image copies
+  const uint64_t pol_img = l2_evict_normal();
+  uint32_t ph = 0;
+  // T = A W (TRANSPOSED = false) or A W^H (true); A = bf16 K-major [96 rows][re 96 | im 96] in shared memory
+  auto issue = [&](uint32_t aA, uint32_t wr, uint32_t wi, bool transposed) {
+    const uint32_t id = idesc_bf16(128, BS, transposed ? kIdescBMn : 0u);
+    const uint32_t lbo = transposed ? kWSbo : kWLbo, sbo = transposed ? kWLbo : kWSbo;
+#pragma unroll
+    for (int ks = 0; ks < BS / 16; ++ks) {
+      const uint64_t ad = smem_desc(aA + ks * 2 * kTileSbo, kTileSbo, kTileLbo);
+      mma_ss(D, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, ks != 0);
+      mma_ss(D + BS, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? (id | kIdescNegB) : id, ks != 0);
+    }
+#pragma unroll
+    for (int ks = 0; ks < BS / 16; ++ks) {
+      const uint64_t ad = smem_desc(aA + (BS / 8 + ks * 2) * kTileSbo, kTileSbo, kTileLbo);
+      mma_ss(D, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? id : (id | kIdescNegB), 1u);
+      mma_ss(D + BS, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, 1u);
+    }
+    mma_commit(&done);
+  };
+  // every thread has written its part of operand `buf`: hand it to the tensor core (and to the copy engine as an image)
+  auto run_gemm = [&](const uint8_t* buf, uint32_t wr, uint32_t wi, bool transposed, __nv_bfloat16* img, size_t img_off) {
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0 && elect_one()) {
+      tc_fence_after();
+      issue(smem_u32(buf), wr, wi, transposed);
+    }
+    if (storer) bulk_store((uint8_t*)img + img_off, smem_u32(buf), kTileBytes, pol_img);
+    __syncwarp();
+    mbar_wait(&done, ph);
+    tc_fence_after();
+    ph ^= 1u;
+  };
+  // fp32 complex rows of the group -> bf16 operand, lanes run over the 8-channel chunks of a row (768 contiguous
+  // bytes); MASKED: the softshrink mask of the row (sMask2) is applied on the way
+  auto load_operand = [&](const float2* src_rows, long long r0, uint8_t* dstbuf, bool masked) {
+    for (uint32_t u = tid; u < HP * (BS / 8); u += kMlpThreads) {
+      const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
+      float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, d = a;
+      if (r0 + rr < p.rows && 8 * c8 < nch) {
+        const float4* src = (const float4*)(src_rows + (size_t)(r0 + rr) * p.C + ch0 + 8 * c8);
+        a = __ldg(src); b = __ldg(src + 1); c = __ldg(src + 2); d = __ldg(src + 3);
+      }
+      uint4 re = make_uint4(pack_bf16(a.x, a.z), pack_bf16(b.x, b.z), pack_bf16(c.x, c.z), pack_bf16(d.x, d.z));
+      uint4 im = make_uint4(pack_bf16(a.y, a.w), pack_bf16(b.y, b.w), pack_bf16(c.y, c.w), pack_bf16(d.y, d.w));
+      if (masked) {
+        const uint4 mk = sMask2[rr][c8 / 6];
+        const int sh = (c8 % 6) * 8;
+        const uint32_t mre = (uint32_t)((((uint64_t)mk.y << 32) | mk.x) >> sh) & 0xFFu;
+        const uint32_t mim = (uint32_t)((((uint64_t)mk.w << 32) | mk.z) >> sh) & 0xFFu;
+        auto sel = [](uint32_t v, uint32_t bits) {   // bits: bit 0 -> low half, bit 1 -> high half
+          return v & ((bits & 1u ? 0x0000FFFFu : 0u) | (bits & 2u ? 0xFFFF0000u : 0u));
+        };
+        re = make_uint4(sel(re.x, mre), sel(re.y, mre >> 2), sel(re.z, mre >> 4), sel(re.w, mre >> 6));
+        im = make_uint4(sel(im.x, mim), sel(im.y, mim >> 2), sel(im.z, mim >> 4), sel(im.w, mim >> 6));
+      }
+      uint8_t* dst = dstbuf + (size_t)rr * 16;
+      *(uint4*)(dst + (size_t)c8 * kTileSbo) = re;
+      *(uint4*)(dst + (size_t)(BS / 8 + c8) * kTileSbo) = im;
+    }
+  };
+  auto ld48x = [&](uint32_t col, uint32_t (&v)[48]) {
+    tmem_ld16<0>(D + lane_sel + col, v);
+    tmem_ld16<16>(D + lane_sel + col + 16, v);
+    tmem_ld16<32>(D + lane_sel + col + 32, v);
+  };
+  for (long long t = s0; t < ntiles; t += S) {
+    const long long r0 = t * HP;
+    const size_t img_off = ((size_t)t * p.ngroups + j) * kTileBytes;
+    const long long row = r0 + r;
+    const int h = (int)((row / p.Kw) % p.H);
+    const bool row_valid = epi && row < p.rows;
+    const bool kept = row_valid && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
+    uint64_t m1[2] = {0, 0}, m2[2] = {0, 0};   // [re, im] bits of this thread's 48 channels
+    // ---- X -> bf16 operand; P1 = X W1 ----
+    load_operand(p.X, r0, bX, false);
+    run_gemm(bX, w1r, w1i, false, p.Xh, img_off);
+    // ---- O1 = relu(P1 + b1), mask1 ----
+    if (epi) {
+#pragma unroll
+      for (int half = 0; half < 2; ++half) {
+        uint32_t v[48];
+        ld48x(half * BS + chalf * 48, v);
+        tmem_wait_ld();
+        const float* bias = sBias + half * BS + chalf * 48;
+        uint8_t* dst = bO + (size_t)r * 16 + (size_t)(half * (BS / 8) + chalf * 6) * kTileSbo;
+#pragma unroll
+        for (int g = 0; g < 6; ++g) {
+          uint32_t pk[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const float lo = __uint_as_float(v[8 * g + 2 * e]) + bias[8 * g + 2 * e];
+            const float hi = __uint_as_float(v[8 * g + 2 * e + 1]) + bias[8 * g + 2 * e + 1];
+            m1[half] |= (uint64_t)(lo > 0.f) << (8 * g + 2 * e);
+            m1[half] |= (uint64_t)(hi > 0.f) << (8 * g + 2 * e + 1);
+            pk[e] = pack_relu_bf16(lo, hi);
+          }
+          *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        }
+      }
+    }
+    run_gemm(bO, w2r, w2i, false, p.O1, img_off);
+    // ---- mask2 = (|P2 + b2| > lambda) on kept rows ----
+    if (epi) {
+      const float lam = p.lambda;
+#pragma unroll
+      for (int half = 0; half < 2; ++half) {
+        uint32_t v[48];
+        ld48x(half * BS + chalf * 48, v);
+        tmem_wait_ld();
+        const float* bias = sBias + NT + half * BS + chalf * 48;
+#pragma unroll
+        for (int c = 0; c < 48; ++c) m2[half] |= (uint64_t)(kept && fabsf(__uint_as_float(v[c]) + bias[c]) > lam) << c;
+      }
+      sMask2[r][chalf] = make_uint4((uint32_t)m2[0], (uint32_t)(m2[0] >> 32), (uint32_t)m2[1], (uint32_t)(m2[1] >> 32));
+    }
+    if (storer) bulk_wait_read<1>();   // the Xh image has left bX (the scratch area of the last epilogue)
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    // ---- G2 = mask2 (.) G -> bf16 operand; G1pre = G2 W2^H ----
+    load_operand(p.G, r0, bG2, true);
+    run_gemm(bG2, w2r, w2i, true, p.G2, img_off);
+    // ---- G1 = mask1 (.) G1pre ----
+    if (epi) {
+#pragma unroll
+      for (int half = 0; half < 2; ++half) {
+        uint32_t v[48];
+        ld48x(half * BS + chalf * 48, v);
+        tmem_wait_ld();
+        uint8_t* dst = bG1 + (size_t)r * 16 + (size_t)(half * (BS / 8) + chalf * 6) * kTileSbo;
+#pragma unroll
+        for (int g = 0; g < 6; ++g) {
+          uint32_t pk[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int c = 8 * g + 2 * e;
+            const float lo = ((m1[half] >> c) & 1u) ? __uint_as_float(v[c]) : 0.f;
+            const float hi = ((m1[half] >> (c + 1)) & 1u) ? __uint_as_float(v[c + 1]) : 0.f;
+            pk[e] = pack_bf16(lo, hi);
+          }
+          *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        }
+      }
+    }
+    run_gemm(bG1, w1r, w1i, true, p.G1, img_off);
+    // ---- GX -> fp32 complex, in place over G: each warp transposes its 32 rows through a private slice of bX
+    //      (16 channels per pass, row pitch 144 B) and stores 128 contiguous bytes per row ----
+    if (epi) {
+      uint32_t vr[48], vi[48];
+      ld48x(chalf * 48, vr);
+      ld48x(BS + chalf * 48, vi);
+      tmem_wait_ld();
+      constexpr uint32_t kPitch = 16 * 8 + 16;
+      uint8_t* scratch = bX + (size_t)warp * (kTileBytes / 8 / 16 * 16);
+      const long long wrow0 = r0 + q * 32;
+#pragma unroll
+      for (int pass = 0; pass < 3; ++pass) {
+#pragma unroll
+        for (int c = 0; c < 16; c += 2) {
+          const int cc = pass * 16 + c;
+          *(float4*)(scratch + lane * kPitch + c * 8) = make_float4(__uint_as_float(vr[cc]), __uint_as_float(vi[cc]),
+                                                                   __uint_as_float(vr[cc + 1]), __uint_as_float(vi[cc + 1]));
+        }
+        __syncwarp();
+        const int chp = chalf * 48 + pass * 16;
+#pragma unroll
+        for (int it = 0; it < 8; ++it) {
+          const int id = it * 32 + lane, rr = id >> 3, piece = id & 7;
+          const float4 o = *(const float4*)(scratch + rr * kPitch + piece * 16);
+          if (wrow0 + rr < p.rows && chp + 2 * piece < nch)
+            *(float4*)(p.G + (size_t)(wrow0 + rr) * p.C + ch0 + chp + 2 * piece) = o;
+        }
+        __syncwarp();
+      }
+      if (p.mask1 != nullptr && row_valid) {
+        // export for the mask-consistent parity tests: [B][H][Wh][C][2] bytes, this thread's 48 channels
+        const long long bh = row / p.Kw;
+        const int kw = (int)(row - bh * p.Kw);
+        const size_t base = ((size_t)(bh * p.Wh + kw) * p.C + ch0 + chalf * 48) * 2;
+        for (int c = 0; c < 48; ++c) {
+          if (chalf * 48 + c < nch) {
+            *(uchar2*)(p.mask1 + base + 2 * c) = make_uchar2((unsigned char)((m1[0] >> c) & 1u), (unsigned char)((m1[1] >> c) & 1u));
+            *(uchar2*)(p.mask2 + base + 2 * c) = make_uchar2((unsigned char)((m2[0] >> c) & 1u), (unsigned char)((m2[1] >> c) & 1u));
+          }
+        }
+      }
+    }
+    if (storer) bulk_wait_read<0>();   // every image of this tile has left its buffer
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+  }
+  if (storer) bulk_wait<0>();
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<256>(D);
+}

@@ -380,6 +380,96 @@ cudaError_t tc_mlp_forward(const Geometry& g, float2* X, const float* w1, const 
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
+// hybrid backward (hidden factor 1): rows B1 (second half), B3-B7 between the fp32 FFT kernels of generic.cu.
+// X = spectrum of x, G = alpha-weighted spectrum of dY (replaced by GX); the parameter gradients go through the same
+// tc_wgrad + k_tc_wgrad_reduce launches as the fused path, over tiles of 96 consecutive spectrum rows.
+bool tc_mlp_bwd_supported(const Geometry& g) {
+  return g.bf16 && !g.force_fp32 && g.C % 8 == 0 && g.hid == g.bs && g.bs >= 8 && BS % g.bs == 0;
+}
+namespace {
+struct MlpBwdWs {
+  __nv_bfloat16 *wprep, *Xh, *O1, *G2, *G1;
+  float *bprep, *part;
+  int groups, S;
+  long long ntiles;
+  size_t total;
+};
+MlpBwdWs mlp_bwd_carve(const Geometry& g, char* base) {
+  MlpBwdWs w{};
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    char* p = base + off;
+    off = align_up(off + bytes, 256);
+    return p;
+  };
+  w.groups = (g.C + BS - 1) / BS;
+  w.ntiles = (g.rows() + HP - 1) / HP;
+  const size_t img = (size_t)w.ntiles * w.groups * kTileBytes;
+  w.wprep = (__nv_bfloat16*)take((size_t)w.groups * 4 * kWBytes);
+  w.bprep = (float*)take((size_t)w.groups * 2 * NT * sizeof(float));
+  w.Xh = (__nv_bfloat16*)take(img);
+  w.O1 = (__nv_bfloat16*)take(img);
+  w.G2 = (__nv_bfloat16*)take(img);
+  w.G1 = (__nv_bfloat16*)take(img);
+  int S = 148 / (2 * w.groups);   // CTAs per (layer, group) of tc_wgrad
+  if (S < 1) S = 1;
+  if ((long long)S > w.ntiles) S = (int)w.ntiles;
+  w.S = S;
+  w.part = (float*)take((size_t)2 * w.groups * S * kWgPartFloats * sizeof(float));
+  w.total = off;
+  return w;
+}
+} // namespace
+size_t tc_mlp_bwd_workspace_bytes(const Geometry& g) { return mlp_bwd_carve(g, nullptr).total; }
+
+cudaError_t tc_mlp_backward(const Geometry& g, const float2* X, float2* G, const float* w1, const float* b1, const float* w2,
+                            const float* b2, float* dw1, float* db1, float* dw2, float* db2, uint8_t* mask1, uint8_t* mask2,
+                            void* ws, cudaStream_t st) {
+  cudaError_t e;
+  if ((e = set_smem(tc_mlp_bwd, kMlpBwdSmem)) != cudaSuccess) return e;
+  if ((e = set_smem(tc_wgrad, kWgSmem)) != cudaSuccess) return e;
+  const MlpBwdWs w = mlp_bwd_carve(g, (char*)ws);
+  const int nW = w.groups * BS * BS;
+  prof_begin("k_tc_prep_weights", st);
+  k_tc_prep_weights<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, w.wprep, w.bprep, w.groups, g.bs, g.C, CtxHeader{},
+                                                      (CtxHeader*)nullptr);
+  prof_end(st);
+  count_launch();
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  int dev = 0, sms = 148;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+  if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+  MlpBwdParams mp{};
+  mp.X = X; mp.G = G; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
+  mp.Xh = w.Xh; mp.O1 = w.O1; mp.G2 = w.G2; mp.G1 = w.G1;
+  mp.mask1 = mask1; mp.mask2 = mask2;
+  mp.rows = g.rows(); mp.C = g.C; mp.ngroups = w.groups; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.Kh = g.Kh;
+  mp.lambda = g.lambda;
+  int S = sms / w.groups;
+  if (S < 1) S = 1;
+  if ((long long)S > w.ntiles) S = (int)w.ntiles;
+  prof_begin("tc_mlp_bwd", st);
+  e = launch_k(tc_mlp_bwd, w.groups * S, kMlpThreads, kMlpBwdSmem, st, true, mp, S);
+  prof_end(st);
+  count_launch();
+  if (e != cudaSuccess || (e = cudaGetLastError()) != cudaSuccess) return e;
+  // B4 / B6: layer 2 = (O1, G2), layer 1 = (Xh, G1); rows past the end of the last tile are zero in G2 / G1
+  prof_begin("tc_wgrad", st);
+  e = launch_k(tc_wgrad, 2 * w.groups * w.S, 128, kWgSmem, st, true, w.O1, w.G2, w.Xh, w.G1, w.part, (int)w.ntiles, HP, w.groups,
+               w.S, 0);
+  prof_end(st);
+  count_launch();
+  if (e != cudaSuccess || (e = cudaGetLastError()) != cudaSuccess) return e;
+  const int nred = nW + w.groups * BS;
+  prof_begin("k_tc_wgrad_reduce", st);
+  e = launch_k(k_tc_wgrad_reduce, dim3((nred + 255) / 256, 2), 256, 0, st, true, w.part, (float2*)dw2, (float2*)db2, (float2*)dw1,
+               (float2*)db1, w.groups, w.S, g.bs, g.C, g.accum ? 1 : 0, 0, (const CtxHeader*)nullptr, CtxHeader{}, (uint16_t*)nullptr,
+               (size_t)0);
+  prof_end(st);
+  count_launch();
+  return e != cudaSuccess ? e : cudaGetLastError();
+}
+
 // W-direction launches: tile = (b, h, block), persistent over the SMs
 static cudaError_t launch_wdft_fwd(const Geometry& g, const TcPlan& tp, const void* in, void* spec, const uint8_t* fimg,
                                    cudaStream_t st, bool dependent) {

@@ -323,16 +323,50 @@ def test_bf16_hidden_factor_forward(oracle, B, H, W, C, nb, hf, f):
     assert parity.rel_l2(y, y32) <= 5e-3
 
 
-def test_bf16_backward_beyond_the_fused_chain(oracle):
-    """bf16 activations on a grid past the fused chain's limits (H = 100): the forward is the hybrid path, the
-    backward runs the generic fp32-math kernels (S1); both against the oracle, the backward
-    mask-consistently, per tile and per block."""
-    wl = inputs.Workload(4, "100x40x96 bf16 B=2 bwd", 2, 100, 40, 96, 1, 1, 0.01, 1.0, "bf16", True, False)
+@pytest.mark.parametrize("B,H,W,C,nb,f", [
+    (2, 100, 40, 96, 1, 1.0),      # H past the fused chain's limit, one group, ragged last 96-row tile
+    (1, 100, 200, 192, 2, 1.0),    # H and W past the limits, two full groups
+    (2, 120, 30, 160, 5, 0.5),     # 32-wide blocks, partly filled last group, truncated rows
+])
+def test_bf16_backward_beyond_the_fused_chain(oracle, B, H, W, C, nb, f):
+    """bf16 activations on grids past the fused chain's limits: forward AND backward are the hybrid path (fp32 FFTs on
+    the CUDA cores; the block MLP, its gradient stages and the parameter gradients on the tensor cores: tc_mlp_fwd,
+    tc_mlp_bwd, tc_wgrad); both against the oracle, the backward mask-consistently, per tile and per block."""
+    wl = inputs.Workload(4, f"{H}x{W}x{C} nb={nb} f={f} bf16 B={B} hybrid bwd", B, H, W, C, nb, 1, 0.01, f, "bf16", True, False)
     data = inputs.make_inputs(wl)
     desc = parity.desc_for(wl)
     assert binding.afno_spectral_path(desc) == "hybrid-fft32-tcgen05"
     _check_forward(oracle, desc, data, label=wl.name)
-    _check_backward(oracle, desc, data, label=wl.name)
+    g = _check_backward(oracle, desc, data, label=wl.name)
+    # the pure fp32 kernels (AFNO_FLAG_FORCE_FP32_MATH) agree to bf16-operand accuracy on dx
+    d32 = parity.desc_for(wl, flags=binding.FLAG_FORCE_FP32_MATH)
+    args = (data["x"], data["dy"], data["w1"], data["b1"], data["w2"], data["b2"])
+    g32 = parity.GpuLayer(d32).backward(*args)
+    assert parity.rel_l2(g["dx"], g32["dx"]) <= 5e-3
+    # AFNO_FLAG_ACCUM_GRADS on the hybrid backward, and repeatability without the mask export
+    import torch
+    layer = parity.GpuLayer(desc)
+    d_acc = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_ACCUM_GRADS})
+    ws = torch.empty(binding.afno_spectral_workspace_bytes(d_acc, True), dtype=torch.uint8, device="cuda")
+    tx, tdy = parity.to_device_act(data["x"], True), parity.to_device_act(data["dy"], True)
+    p = layer.params(data["w1"], data["b1"], data["w2"], data["b2"])
+    acc = [torch.ones_like(t) for t in p]
+    tdx = torch.empty_like(tx)
+    binding.afno_spectral_bwd(d_acc, tx, tdy, *p, tdx, *acc, ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(parity.from_device_act(tdx), g["dx"])
+    for t, k in zip(acc, ("dw1", "db1", "dw2", "db2")):
+        assert np.allclose(t.cpu().numpy(), 1.0 + g[k], rtol=0, atol=2e-6 * max(1.0, np.abs(g[k]).max())), k
+
+
+def test_bf16_paper_shape_backward(oracle):
+    """the paper's own layer shape (180 x 360 tokens, 1,024 channels in 32 blocks of 32), backward on
+    the hybrid path, mask-consistently against the oracle per tile and per block."""
+    wl = inputs.WORKLOADS["paper_shape_b1"]
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert binding.afno_spectral_path(desc) == "hybrid-fft32-tcgen05"
+    _check_backward(oracle, desc, data, label=wl.name + " bwd")
 
 
 def test_bf16_paper_shape_forward(oracle):

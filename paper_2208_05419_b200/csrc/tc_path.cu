@@ -464,7 +464,7 @@ cudaError_t tc_mlp_backward(const Geometry& g, const float2* X, float2* G, const
   prof_begin("k_tc_wgrad_reduce", st);
   e = launch_k(k_tc_wgrad_reduce, dim3((nred + 255) / 256, 2), 256, 0, st, true, w.part, (float2*)dw2, (float2*)db2, (float2*)dw1,
                (float2*)db1, w.groups, w.S, g.bs, g.C, g.accum ? 1 : 0, 0, (const CtxHeader*)nullptr, CtxHeader{}, (uint16_t*)nullptr,
-               (size_t)0);
+               (size_t)0, 1);
   prof_end(st);
   count_launch();
   return e != cudaSuccess ? e : cudaGetLastError();
@@ -472,14 +472,14 @@ cudaError_t tc_mlp_backward(const Geometry& g, const float2* X, float2* G, const
 
 // W-direction launches: tile = (b, h, block), persistent over the SMs
 static cudaError_t launch_wdft_fwd(const Geometry& g, const TcPlan& tp, const void* in, void* spec, const uint8_t* fimg,
-                                   cudaStream_t st, bool dependent) {
+                                   cudaStream_t st, bool dependent, bool independent = false) {
   CUtensorMap mx, ma;
   if (!act_tmap(tp, &mx, in, g) || !spec_store_tmap(tp, &ma, spec, g)) return cudaErrorInvalidValue;
   const int ntiles = g.B * g.H * g.nb;
   const int grid = ntiles < tp.num_sms ? ntiles : tp.num_sms;
   prof_begin("tc_wdft_fwd", st);
   cudaError_t e = launch_k(tc_wdft_fwd2, grid, kW2Threads, kWfSmem, st, dependent, mx, ma, (const uint32_t*)fimg, ntiles, g.nb,
-                           g.H, g.Kw);
+                           g.H, g.Kw, independent ? 1 : 0);
   prof_end(st);
   count_launch();
   return e != cudaSuccess ? e : cudaGetLastError();
@@ -536,7 +536,8 @@ cudaError_t tc_forward(const Geometry& g0, const Plan& p, const void* x, const f
     const char* xc = (const char*)x + act_offset(g, b0);
     char* yc = (char*)y + act_offset(g, b0);
     const size_t t0 = (size_t)b0 * g.Kw * g.nb;   // first (b, kw, block) tile of the chunk in whole-batch tensors
-    if ((e = launch_wdft_fwd(gc, tp, xc, w.A, tp.fw, st, true)) != cudaSuccess) return e;
+    // the first W transform of the call runs beside the weight-image kernel (it reads x and writes A only)
+    if ((e = launch_wdft_fwd(gc, tp, xc, w.A, tp.fw, st, true, b0 == 0)) != cudaSuccess) return e;
     MixParams mp{};
     if (!tile_tmap(tp, &mp.mapA1, w.A, gc)) return cudaErrorInvalidValue;
     mp.mapA1g = mp.mapA1;
@@ -636,7 +637,7 @@ cudaError_t tc_backward(const Geometry& g0, const Plan& p, const void* x, const 
   // (a context that does not belong to this call poisons dx and the gradients with NaN)
   TC_LAUNCH("k_tc_wgrad_reduce", k_tc_wgrad_reduce, dim3((nred + 255) / 256, 2), 256, 0, st, dep, w.part, (float2*)dw2,
             (float2*)db2, (float2*)dw1, (float2*)db1, g.nb, w.S, g.bs_block, g.C, g.accum ? 1 : 0, g.use_ctx ? 1 : 0,
-            (const CtxHeader*)w.header, make_header(g, w), (uint16_t*)dx, (size_t)g.B * g.H * g.W * g.C);
+            (const CtxHeader*)w.header, make_header(g, w), (uint16_t*)dx, (size_t)g.B * g.H * g.W * g.C, 0);
 #undef TC_LAUNCH
   return cudaSuccess;
 }

@@ -55,7 +55,7 @@ __device__ __forceinline__ void load_const_tmem(uint32_t tmem, const uint32_t* _
 
 __global__ void __launch_bounds__(kW2Threads, 1)
 tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ CUtensorMap mapA1,
-             const uint32_t* __restrict__ Fimg, int ntiles, int nb, int H, int Kw) {
+             const uint32_t* __restrict__ Fimg, int ntiles, int nb, int H, int Kw, int independent) {
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t full[kWfSlots], sfree[kWfSlots], accfull[2], accempty[2];
   __shared__ uint32_t tmem_slot;
@@ -83,7 +83,10 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
   load_const_tmem(tmem, Fimg, warp, lane);   // plan constant: loads under the previous kernel's tail
-  pdl_wait();
+  // `independent`: the previous kernel of the call (the weight-image kernel, the call's first and a plain launch)
+  // touches nothing this kernel reads or writes, so the two run side by side; the wait moves to the end of this
+  // kernel, which keeps completion transitive for the kernels behind it.
+  if (!independent) pdl_wait();
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
   const uint64_t pol_stream = pol(kPolWfLoadX), pol_keep = pol(kPolWfStoreA);
@@ -183,6 +186,7 @@ tc_wdft_fwd2(const __grid_constant__ CUtensorMap mapX, const __grid_constant__ C
     if (warp == 0 && elect_one()) bulk_wait<0>();
     __syncwarp();
   }
+  if (independent) pdl_wait();
   tc_fence_before();
   __syncthreads();
   if (warp == 0) tmem_dealloc<512>(tmem);
@@ -218,13 +222,16 @@ tc_wdft_inv2(const __grid_constant__ CUtensorMap mapA2, const __grid_constant__ 
     tma_prefetch_desc(&mapY);
   }
   if (warp == 0) tmem_alloc<512>(&tmem_slot);
-  pdl_launch_dependents();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_slot;
   load_const_tmem(tmem, Gimg, warp, lane);   // plan constant: loads under the previous kernel's tail
   pdl_wait();
+  // AFTER the wait: a dependent kernel that becomes resident beside this one (k_tc_wgrad_reduce: no shared memory)
+  // may then rely on everything before this kernel in the stream having completed, and does its sums under this
+  // kernel instead of after it
+  pdl_launch_dependents();
   const int nmine = ntiles > (int)blockIdx.x ? (ntiles - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
   const uint64_t pol_spec = pol(kPolWiLoadA), pol_res = pol(kPolWiLoadRes), pol_out = pol(kPolWiStoreY);

@@ -157,25 +157,23 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
 __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __restrict__ dW2, float2* __restrict__ dB2,
                                   float2* __restrict__ dW1, float2* __restrict__ dB1, int ngroups, int S, int bs, int C,
                                   int accumulate, int guard, const CtxHeader* __restrict__ got, const CtxHeader want,
-                                  uint16_t* __restrict__ dx, size_t n_act) {
+                                  uint16_t* __restrict__ dx, size_t n_act, int wait_first) {
   pdl_launch_dependents();
-  pdl_wait();
+  // wait_first = 0 (fused path): the kernel before this one in the stream is tc_wdft_inv2, which lets its dependents
+  // start only after ITS prerequisites (tc_wgrad among them) have completed: the partial sums are final, and the
+  // sums below run under the inverse transform; only the guard's overwrite of dx has to wait for it.
+  if (wait_first) pdl_wait();
   bool ok = true;
   if (guard) {
     const uint32_t* a = (const uint32_t*)got;
     const uint32_t* b = (const uint32_t*)&want;
     for (uint32_t q = 0; q < sizeof(CtxHeader) / 4; ++q) ok = ok && (a[q] == b[q]);
-    if (!ok) {
-      const size_t nthreads = (size_t)gridDim.x * gridDim.y * blockDim.x;
-      const size_t t0 = ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x;
-      for (size_t i = t0; i < n_act; i += nthreads) dx[i] = 0x7FC0;   // bf16 NaN
-    }
   }
   const float poison = __int_as_float(0x7FC00000);
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const int nW = C * bs;          // nb * bs * bs complex weights
   const int layer = blockIdx.y;
-  part += (size_t)layer * ngroups * S * kWgPartFloats;
+  const float* lpart = part + (size_t)layer * ngroups * S * kWgPartFloats;
   float2* dW = layer ? dW1 : dW2;
   float2* dB = layer ? dB1 : dB2;
   if (idx < nW) {
@@ -184,7 +182,7 @@ __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __rest
     const int j = ci / BS, i = ci - j * BS, o = co - j * BS;
     float2 acc = accumulate ? dW[idx] : make_float2(0.f, 0.f);
     for (int s = 0; s < S; ++s) {
-      const float* P = part + (size_t)(j * S + s) * kWgPartFloats;
+      const float* P = lpart + (size_t)(j * S + s) * kWgPartFloats;
       const float* Pre = P + (size_t)i * kWgPitch;
       const float* Pim = P + (size_t)(kWgRowsRe + i) * kWgPitch;
       acc.x += Pre[o] + Pim[BS + o];
@@ -195,10 +193,16 @@ __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __rest
     const int k = idx - nW, j = k / BS, o = k - j * BS;
     float2 acc = accumulate ? dB[k] : make_float2(0.f, 0.f);
     for (int s = 0; s < S; ++s) {
-      const float* P = part + (size_t)(j * S + s) * kWgPartFloats + (size_t)BS * kWgPitch;
+      const float* P = lpart + (size_t)(j * S + s) * kWgPartFloats + (size_t)BS * kWgPitch;
       acc.x += P[o];
       acc.y += P[BS + o];
     }
     dB[k] = ok ? acc : make_float2(poison, poison);
+  }
+  if (!wait_first) pdl_wait();   // dx is complete (and this call's completion stays transitive)
+  if (guard && !ok) {
+    const size_t nthreads = (size_t)gridDim.x * gridDim.y * blockDim.x;
+    const size_t t0 = ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * blockDim.x + threadIdx.x;
+    for (size_t i = t0; i < n_act; i += nthreads) dx[i] = 0x7FC0;   // bf16 NaN
   }
 }

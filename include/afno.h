@@ -89,8 +89,11 @@ int afno_version(void);
 const char* afno_status_string(int status);
 const char* afno_last_error(void); /* thread-local, valid until the thread's next call */
 
-/* Name of the kernel family the descriptor dispatches to: "generic-fp32" or "tcgen05-bf16".
- * Returns NULL for an invalid / unsupported descriptor. */
+/* Name of the kernel family the descriptor dispatches to: "tcgen05-bf16" (every transform and MLP layer a
+ * tensor-core GEMM: bf16, blocks dividing 96, hidden factor 1, H <= 96, W/2+1 <= 96), "hybrid-fft32-tcgen05"
+ * (bf16 activations beyond those limits: fp32 FFTs on the CUDA cores, the block MLP, its gradient stages and the
+ * parameter gradients on the tensor cores; hidden factor > 1: forward only, its backward runs the fp32 kernels)
+ * or "generic-fp32".  Returns NULL for an invalid / unsupported descriptor. */
 const char* afno_spectral_path(const afno_desc_t* d);
 
 /* Pure host arithmetic; 0 for an invalid descriptor. */

@@ -287,7 +287,8 @@ int afno_profile_stop(char* out, size_t cap) {
 const char* afno_spectral_path(const afno_desc_t* d) {
   Geometry g;
   if (resolve(d, &g) != AFNO_OK) return nullptr;
-  // "hybrid": forward = fp32 FFTs on the CUDA cores + tensor-core block MLP; backward = generic-fp32 kernels
+  // "hybrid": fp32 FFTs on the CUDA cores + the block MLP (forward, and for hidden factor 1 also the gradient stages and
+  // the parameter gradients) on the tensor cores
   return use_tc_fwd(g) ? "tcgen05-bf16" : (tc_mlp_supported(g) ? "hybrid-fft32-tcgen05" : "generic-fp32");
 }
 

@@ -10,7 +10,8 @@ lambda 0.01, kept fraction 1.0).  Prints ONE JSON line (contract in the task pro
 
 N > 1: the path does not shard ("replicas only", S6): every rank runs an
 independent replica on its own GPU, no data-path collective; value = all ranks' samples /
-max-over-ranks device time.
+max-over-ranks device time.  `--parallel dp` (not the contract line) adds what data
+parallelism needs on top: ONE all-reduce(SUM) of the 1.19 MB of parameter gradients per step, inside the timed region.
 """
 from __future__ import annotations
 
@@ -246,7 +247,9 @@ def run_ours(args):
         sets.append(dict(x=torch.roll(x0, s, 0).contiguous(), dy=torch.roll(dy0, s, 0).contiguous(),
                          y=torch.empty_like(x0), dx=torch.empty_like(x0)))
     params = [torch.from_numpy(data[k]).to(dev) for k in ("w1", "b1", "w2", "b2")]
-    grads = [torch.empty_like(p) for p in params]
+    from paper_2208_05419_b200 import sharding
+    bucket = sharding.GradBucket.allocate(wl.num_blocks, wl.C // wl.num_blocks, wl.hidden_factor, device=dev)
+    grads = bucket.views      # one flat buffer: --parallel dp reduces it with a single collective
     ws_f = torch.empty(binding.afno_spectral_workspace_bytes(desc, False), dtype=torch.uint8, device=dev)
     ws_b = torch.empty(binding.afno_spectral_workspace_bytes(desc, True), dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream()
@@ -264,6 +267,8 @@ def run_ours(args):
         n = binding.afno_last_launch_count()
         binding.afno_spectral_bwd(desc_b, s["x"], s["dy"], *params, s["dx"], *grads, ws_b, st)
         launches[0] = n + binding.afno_last_launch_count()
+        if args.parallel == "dp":
+            bucket.all_reduce(dist)      # PAPER.md:134; NCCL, on the current stream (no-op at world size 1)
 
     def barrier():
         torch.cuda.synchronize()
@@ -426,7 +431,8 @@ def run_ours(args):
             "config": {"workload": f"BASELINE.json configs[4]: {wl.name}", "B_per_gpu": B, "H": wl.H, "W": wl.W,
                        "C": wl.C, "num_blocks": wl.num_blocks, "lambda": wl.lam, "kept_fraction": wl.kept_fraction,
                        "path": path, "backward": "saved context (fwd keeps Xh, O1 and the activation masks; bwd runs the gradient stages only)" if ctx
-                       else "stateless (recomputes the spectrum of x)", "parallelism": "replicas only" if world > 1 else "single GPU",
+                       else "stateless (recomputes the spectrum of x)", "parallelism": ("single GPU" if world == 1 else "replicas only" if args.parallel == "replicas" else
+                                       "data parallel: one all-reduce(SUM) of the parameter gradients per step"),
                        "l2": f"{NSETS} rotating input/output buffer sets of {4 * x0.numel() * 2 / 1e6:.0f} MB "
                              "each (> 126 MB L2), no explicit flush"},
             "clocks": clk, "e2e": e2e, "gpu_launches": launches[0] * args.steps,
@@ -536,6 +542,9 @@ def main():
     ap.add_argument("--timed-only", action="store_true",
                     help="warm-up, the timed steps and the per-kernel event pass only (no CUDA-graph replay, e2e or "
                          "cpu_baseline legs): the command the ncu captures under profiles/ run")
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "dp"],
+                    help="N > 1: independent replicas (the contract line; DESIGN.md S6) or data parallelism with one "
+                         "all-reduce of the parameter gradients per step (SURVEY.md S8(f) item 4)")
     ap.add_argument("--stateless", action="store_true",
                     help="time the stateless afno_spectral_bwd (recomputes F1) instead of the saved-context step")
     args = ap.parse_args()

@@ -765,3 +765,29 @@ def test_w192_runs_on_the_generic_path(oracle):
         # bf16: fp32 FFTs + tensor-core MLP (hybrid forward); fp32: generic kernels throughout
         assert binding.afno_spectral_path(desc) == ("hybrid-fft32-tcgen05" if dt == binding.AFNO_BF16 else "generic-fp32")
         _check_forward(oracle, desc, data, label=f"64x192x96 dtype={dt}")
+
+
+def test_data_parallel_step_with_gradient_bucket(oracle):
+    """SURVEY.md S8(f) item 4 on one GPU: sharding.data_parallel_step (forward with saved context, backward writing dW / db
+    straight into the views of ONE flat bucket, then the all-reduce, a no-op at world size 1) returns what the plain calls
+    return, and the bucket's views are valid C-ABI outputs (16-byte aligned).  The 2-rank logic runs on CPU with gloo
+    (tests/test_multiproc_cpu.py)."""
+    import torch
+    from paper_2208_05419_b200 import sharding
+    wl = inputs.Workload(4, "30x60x192 bf16 B=2 dp", 2, 30, 60, 192, 2, 1, 0.01, 1.0, "bf16", True, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    ref = _ctx_step(desc, data)
+    layer = parity.GpuLayer(desc)
+    tx, tdy = parity.to_device_act(data["x"], True), parity.to_device_act(data["dy"], True)
+    ty, tdx = torch.empty_like(tx), torch.empty_like(tx)
+    p = layer.params(data["w1"], data["b1"], data["w2"], data["b2"])
+    bucket = sharding.GradBucket.allocate(wl.num_blocks, wl.C // wl.num_blocks, 1, device="cuda")
+    assert all(v.data_ptr() % 16 == 0 for v in bucket.views)
+    ws = torch.empty(binding.afno_spectral_workspace_bytes(desc, True), dtype=torch.uint8, device="cuda")
+    n = sharding.data_parallel_step(binding, desc, tx, tdy, p, ty, tdx, bucket, ws, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    assert n == 9
+    assert np.array_equal(parity.from_device_act(ty), ref["y"]) and np.array_equal(parity.from_device_act(tdx), ref["dx"])
+    for v, k in zip(bucket.views, ("dw1", "db1", "dw2", "db2")):
+        assert np.array_equal(v.cpu().numpy(), ref[k]), k

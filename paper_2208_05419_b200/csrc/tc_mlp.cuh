@@ -688,3 +688,327 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
   __syncthreads();
   if (warp == 0) tmem_dealloc<256>(D);
 }
+
+// ---- hybrid backward, hidden factor 2..8 (blocks of 96): SURVEY.md S8(f) item 2 -----------------------------------------
+// Two passes over the hf hidden chunks of 96 per tile of 96 spectrum rows, the chunk's weight images (74 KB) reloaded
+// from L2 each time (as tc_mlp_fwd_hf does):
+//   pass 1 (recompute): P1_c = X W1[:, c] -> O1_c = relu(P1_c + b1_c), mask1_c (bits kept in shared memory);
+//                       P2 += O1_c W2[c, :] accumulated over the chunks in tensor memory -> mask2
+//   pass 2 (gradient):  G2 = mask2 (.) G;  G1_c = mask1_c (.) (G2 W2[c, :]^H);  GX += G1_c W1[:, c]^H accumulated over
+//                       the chunks in tensor memory -> fp32, in place over G
+// Operand buffers: X, G2 (one each per tile) and ONE buffer shared by O1_c (pass 1) and G1_c (pass 2); all four kinds
+// leave as tc_wgrad operand images (O1 and G1 per chunk), the parameter gradients are one tc_wgrad launch per chunk
+// (layer 2: O1_c, G2 -> dW2[c rows]; layer 1: Xh, G1_c -> dW1[:, c columns]) and k_tc_wgrad_reduce_hf.
+constexpr uint32_t kMlpBwdHfSmem = 4 * kWBytes + 3 * kTileBytes + 512 + kMlpMaxHf * HP * 2 * 16;   // 210,560
+
+struct MlpBwdHfParams {
+  const float2* X;
+  float2* G;
+  const uint8_t* wprep;      // per (block, chunk) 4 x kWBytes (k_tc_prep_weights_hf)
+  const float* bprep;        // per block: b1 [hf][192], then b2 [192]
+  __nv_bfloat16 *Xh, *G2;    // images [tile][block]
+  __nv_bfloat16 *O1, *G1;    // images [chunk][tile][block]
+  uint8_t *mask1, *mask2;    // optional export: mask1 [B][H][Wh][nb * hid][2], mask2 [B][H][Wh][C][2]
+  long long rows, ntiles;
+  int C, nb, H, Kw, Wh, Kh, hf;
+  float lambda;
+};
+
+__global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfParams p, int S) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t done;
+  __shared__ uint32_t tmem_slot;
+  __shared__ __align__(16) float sBias[(kMlpMaxHf + 1) * NT];
+  __shared__ __align__(16) uint4 sMask2[HP][2];
+  uint8_t* sW = smem;
+  uint8_t* bX = smem + 4 * kWBytes;
+  uint8_t* bG2 = bX + kTileBytes;
+  uint8_t* bH = bG2 + kTileBytes;                       // O1_c in pass 1, G1_c in pass 2
+  uint4* sMask1 = (uint4*)(bH + kTileBytes + 512);      // [chunk][row][48-channel half]
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int j = blockIdx.x / S, s0 = blockIdx.x - j * S;
+  const int hf = p.hf, hid = hf * BS;
+  const int ch0 = j * BS;
+  pdl_launch_dependents();
+  for (uint32_t i = tid; i < (3 * kTileBytes + 512) / 16; i += kMlpThreads) ((uint4*)bX)[i] = make_uint4(0, 0, 0, 0);
+  if (tid == 0) {
+    mbar_init(&done, 1);
+    mbar_init_fence();
+  }
+  if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  pdl_wait();
+  for (int i = tid; i < (hf + 1) * NT; i += kMlpThreads) sBias[i] = p.bprep[(size_t)j * (hf + 1) * NT + i];
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t D1 = tmem_slot, D2 = tmem_slot + NT;   // per-chunk accumulator, accumulator over the chunks
+  const uint32_t aW = smem_u32(sW);
+  const uint32_t wAr = aW, wAi = aW + kWBytes, wBr = aW + 2 * kWBytes, wBi = aW + 3 * kWBytes;   // W1 chunk, W2 chunk
+  const int q = warp & 3, chalf = warp >> 2;
+  const int r = q * 32 + lane;
+  const bool epi = q < 3;
+  const uint32_t lane_sel = (uint32_t)(q * 32) << 16;
+  const bool storer = tid == 3 * 32;
+  const uint64_t pol_img = l2_evict_normal();
+  uint32_t ph = 0;
+  auto issue = [&](uint32_t D, uint32_t aA, uint32_t wr, uint32_t wi, bool transposed, uint32_t acc0) {
+    const uint32_t id = idesc_bf16(128, BS, transposed ? kIdescBMn : 0u);
+    const uint32_t lbo = transposed ? kWSbo : kWLbo, sbo = transposed ? kWLbo : kWSbo;
+#pragma unroll
+    for (int ks = 0; ks < BS / 16; ++ks) {
+      const uint64_t ad = smem_desc(aA + ks * 2 * kTileSbo, kTileSbo, kTileLbo);
+      mma_ss(D, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, acc0 | (uint32_t)(ks != 0));
+      mma_ss(D + BS, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? (id | kIdescNegB) : id, acc0 | (uint32_t)(ks != 0));
+    }
+#pragma unroll
+    for (int ks = 0; ks < BS / 16; ++ks) {
+      const uint64_t ad = smem_desc(aA + (BS / 8 + ks * 2) * kTileSbo, kTileSbo, kTileLbo);
+      mma_ss(D, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? id : (id | kIdescNegB), 1u);
+      mma_ss(D + BS, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, 1u);
+    }
+    mma_commit(&done);
+  };
+  // operand `buf` is complete: GEMM into D (and the image copy); returns when the GEMM has completed
+  auto run_gemm = [&](uint32_t D, const uint8_t* buf, uint32_t wr, uint32_t wi, bool transposed, uint32_t acc0,
+                      __nv_bfloat16* img, size_t img_off) {
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0 && elect_one()) {
+      tc_fence_after();
+      issue(D, smem_u32(buf), wr, wi, transposed, acc0);
+    }
+    if (storer && img != nullptr) bulk_store((uint8_t*)img + img_off, smem_u32(buf), kTileBytes, pol_img);
+    __syncwarp();
+    mbar_wait(&done, ph);
+    tc_fence_after();
+    ph ^= 1u;
+  };
+  // the chunk's weight images; the GEMMs that read the previous chunk's have completed (run_gemm waits)
+  auto load_weights = [&](int hc) {
+    const uint8_t* wsrc = p.wprep + ((size_t)j * hf + hc) * 4 * kWBytes;
+    for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMlpThreads) cp_async16(aW + i * 16, wsrc + (size_t)i * 16);
+    cp_async_wait_all();
+  };
+  auto load_operand = [&](const float2* src_rows, long long r0, uint8_t* dstbuf, bool masked) {
+    for (uint32_t u = tid; u < HP * (BS / 8); u += kMlpThreads) {
+      const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
+      float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, d = a;
+      if (r0 + rr < p.rows) {
+        const float4* src = (const float4*)(src_rows + (size_t)(r0 + rr) * p.C + ch0 + 8 * c8);
+        a = __ldg(src); b = __ldg(src + 1); c = __ldg(src + 2); d = __ldg(src + 3);
+      }
+      uint4 re = make_uint4(pack_bf16(a.x, a.z), pack_bf16(b.x, b.z), pack_bf16(c.x, c.z), pack_bf16(d.x, d.z));
+      uint4 im = make_uint4(pack_bf16(a.y, a.w), pack_bf16(b.y, b.w), pack_bf16(c.y, c.w), pack_bf16(d.y, d.w));
+      if (masked) {
+        const uint4 mk = sMask2[rr][c8 / 6];
+        const int sh = (c8 % 6) * 8;
+        const uint32_t mre = (uint32_t)((((uint64_t)mk.y << 32) | mk.x) >> sh) & 0xFFu;
+        const uint32_t mim = (uint32_t)((((uint64_t)mk.w << 32) | mk.z) >> sh) & 0xFFu;
+        auto sel = [](uint32_t v, uint32_t bits) {
+          return v & ((bits & 1u ? 0x0000FFFFu : 0u) | (bits & 2u ? 0xFFFF0000u : 0u));
+        };
+        re = make_uint4(sel(re.x, mre), sel(re.y, mre >> 2), sel(re.z, mre >> 4), sel(re.w, mre >> 6));
+        im = make_uint4(sel(im.x, mim), sel(im.y, mim >> 2), sel(im.z, mim >> 4), sel(im.w, mim >> 6));
+      }
+      uint8_t* dst = dstbuf + (size_t)rr * 16;
+      *(uint4*)(dst + (size_t)c8 * kTileSbo) = re;
+      *(uint4*)(dst + (size_t)(BS / 8 + c8) * kTileSbo) = im;
+    }
+  };
+  auto ld48x = [&](uint32_t D, uint32_t col, uint32_t (&v)[48]) {
+    tmem_ld16<0>(D + lane_sel + col, v);
+    tmem_ld16<16>(D + lane_sel + col + 16, v);
+    tmem_ld16<32>(D + lane_sel + col + 32, v);
+  };
+  const size_t chunk_imgs = (size_t)p.ntiles * p.nb * kTileBytes;   // bytes of one chunk's image tensor
+  for (long long t = s0; t < p.ntiles; t += S) {
+    const long long r0 = t * HP;
+    const size_t img_off = ((size_t)t * p.nb + j) * kTileBytes;
+    const long long row = r0 + r;
+    const int h = (int)((row / p.Kw) % p.H);
+    const bool row_valid = epi && row < p.rows;
+    const bool kept = row_valid && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
+    const long long bh = row / p.Kw;
+    const int kw = (int)(row - bh * p.Kw);
+    load_operand(p.X, r0, bX, false);
+    // ---- pass 1 ----
+    for (int hc = 0; hc < hf; ++hc) {
+      load_weights(hc);
+      run_gemm(D1, bX, wAr, wAi, false, 0u, hc == 0 ? p.Xh : nullptr, img_off);
+      if (storer) bulk_wait_read<0>();   // the previous chunk's O1 image (and Xh) have left their buffers
+      tc_fence_before();
+      __syncthreads();
+      tc_fence_after();
+      if (epi) {
+        uint64_t m1[2] = {0, 0};
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+          uint32_t v[48];
+          ld48x(D1, half * BS + chalf * 48, v);
+          tmem_wait_ld();
+          const float* bias = sBias + (size_t)hc * NT + half * BS + chalf * 48;
+          uint8_t* dst = bH + (size_t)r * 16 + (size_t)(half * (BS / 8) + chalf * 6) * kTileSbo;
+#pragma unroll
+          for (int g = 0; g < 6; ++g) {
+            uint32_t pk[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const float lo = __uint_as_float(v[8 * g + 2 * e]) + bias[8 * g + 2 * e];
+              const float hi = __uint_as_float(v[8 * g + 2 * e + 1]) + bias[8 * g + 2 * e + 1];
+              m1[half] |= (uint64_t)(lo > 0.f) << (8 * g + 2 * e);
+              m1[half] |= (uint64_t)(hi > 0.f) << (8 * g + 2 * e + 1);
+              pk[e] = pack_relu_bf16(lo, hi);
+            }
+            *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+          }
+        }
+        sMask1[((size_t)hc * HP + r) * 2 + chalf] = make_uint4((uint32_t)m1[0], (uint32_t)(m1[0] >> 32), (uint32_t)m1[1], (uint32_t)(m1[1] >> 32));
+        if (p.mask1 != nullptr && row_valid) {
+          const size_t base = ((size_t)(bh * p.Wh + kw) * ((size_t)p.nb * hid) + (size_t)j * hid + hc * BS + chalf * 48) * 2;
+          for (int c = 0; c < 48; ++c)
+            *(uchar2*)(p.mask1 + base + 2 * c) = make_uchar2((unsigned char)((m1[0] >> c) & 1u), (unsigned char)((m1[1] >> c) & 1u));
+        }
+      }
+      run_gemm(D2, bH, wBr, wBi, false, hc > 0 ? 1u : 0u, p.O1, (size_t)hc * chunk_imgs + img_off);
+    }
+    // ---- mask2 = (|P2 + b2| > lambda) on kept rows ----
+    if (epi) {
+      const float lam = p.lambda;
+      uint64_t m2[2] = {0, 0};
+#pragma unroll
+      for (int half = 0; half < 2; ++half) {
+        uint32_t v[48];
+        ld48x(D2, half * BS + chalf * 48, v);
+        tmem_wait_ld();
+        const float* bias = sBias + (size_t)hf * NT + half * BS + chalf * 48;
+#pragma unroll
+        for (int c = 0; c < 48; ++c) m2[half] |= (uint64_t)(kept && fabsf(__uint_as_float(v[c]) + bias[c]) > lam) << c;
+      }
+      sMask2[r][chalf] = make_uint4((uint32_t)m2[0], (uint32_t)(m2[0] >> 32), (uint32_t)m2[1], (uint32_t)(m2[1] >> 32));
+      if (p.mask2 != nullptr && row_valid) {
+        const size_t base = ((size_t)(bh * p.Wh + kw) * p.C + ch0 + chalf * 48) * 2;
+        for (int c = 0; c < 48; ++c)
+          *(uchar2*)(p.mask2 + base + 2 * c) = make_uchar2((unsigned char)((m2[0] >> c) & 1u), (unsigned char)((m2[1] >> c) & 1u));
+      }
+    }
+    if (storer) bulk_wait_read<0>();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    // ---- pass 2 ----
+    load_operand(p.G, r0, bG2, true);
+    for (int hc = 0; hc < hf; ++hc) {
+      load_weights(hc);
+      run_gemm(D1, bG2, wBr, wBi, true, 0u, hc == 0 ? p.G2 : nullptr, img_off);   // G2 W2[c, :]^H
+      if (storer) bulk_wait_read<0>();
+      tc_fence_before();
+      __syncthreads();
+      tc_fence_after();
+      if (epi) {
+        const uint4 mk = sMask1[((size_t)hc * HP + r) * 2 + chalf];
+        const uint64_t m1[2] = {((uint64_t)mk.y << 32) | mk.x, ((uint64_t)mk.w << 32) | mk.z};
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+          uint32_t v[48];
+          ld48x(D1, half * BS + chalf * 48, v);
+          tmem_wait_ld();
+          uint8_t* dst = bH + (size_t)r * 16 + (size_t)(half * (BS / 8) + chalf * 6) * kTileSbo;
+#pragma unroll
+          for (int g = 0; g < 6; ++g) {
+            uint32_t pk[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const int c = 8 * g + 2 * e;
+              const float lo = ((m1[half] >> c) & 1u) ? __uint_as_float(v[c]) : 0.f;
+              const float hi = ((m1[half] >> (c + 1)) & 1u) ? __uint_as_float(v[c + 1]) : 0.f;
+              pk[e] = pack_bf16(lo, hi);
+            }
+            *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+          }
+        }
+      }
+      run_gemm(D2, bH, wAr, wAi, true, hc > 0 ? 1u : 0u, p.G1, (size_t)hc * chunk_imgs + img_off);   // GX += G1_c W1[:, c]^H
+    }
+    if (storer) bulk_wait_read<0>();   // bX is the scratch area of the store below
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    // ---- GX -> fp32 complex, in place over G ----
+    if (epi) {
+      uint32_t vr[48], vi[48];
+      ld48x(D2, chalf * 48, vr);
+      ld48x(D2, BS + chalf * 48, vi);
+      tmem_wait_ld();
+      constexpr uint32_t kPitch = 16 * 8 + 16;
+      uint8_t* scratch = bX + (size_t)warp * (kTileBytes / 8 / 16 * 16);
+      const long long wrow0 = r0 + q * 32;
+#pragma unroll
+      for (int pass = 0; pass < 3; ++pass) {
+#pragma unroll
+        for (int c = 0; c < 16; c += 2) {
+          const int cc = pass * 16 + c;
+          *(float4*)(scratch + lane * kPitch + c * 8) = make_float4(__uint_as_float(vr[cc]), __uint_as_float(vi[cc]),
+                                                                   __uint_as_float(vr[cc + 1]), __uint_as_float(vi[cc + 1]));
+        }
+        __syncwarp();
+        const int chp = chalf * 48 + pass * 16;
+#pragma unroll
+        for (int it = 0; it < 8; ++it) {
+          const int id = it * 32 + lane, rr = id >> 3, piece = id & 7;
+          const float4 o = *(const float4*)(scratch + rr * kPitch + piece * 16);
+          if (wrow0 + rr < p.rows) *(float4*)(p.G + (size_t)(wrow0 + rr) * p.C + ch0 + chp + 2 * piece) = o;
+        }
+        __syncwarp();
+      }
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+  }
+  if (storer) bulk_wait<0>();
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<512>(D1);
+}
+
+// dW1[j][i][c*96 + o], db1[j][c*96 + o] from chunk c's layer-1 partial sums; dW2[j][c*96 + i][o] from its layer-2 partial
+// sums, db2[j][o] from chunk 0's (sum of G2 rows, the same for every chunk).  part: [chunk][layer 2 | layer 1][block][S].
+__global__ void k_tc_wgrad_reduce_hf(const float* __restrict__ part, float2* __restrict__ dW2, float2* __restrict__ dB2,
+                                     float2* __restrict__ dW1, float2* __restrict__ dB1, int nb, int S, int hf, int accumulate) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int hid = hf * BS;
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int layer = blockIdx.y;                 // 0: layer 2, 1: layer 1 (the order of tc_wgrad's CTAs)
+  const int nW = nb * hf * BS * BS;
+  const size_t chunk_part = (size_t)2 * nb * S * kWgPartFloats;
+  if (idx < nW) {
+    const int o = idx % BS, i = (idx / BS) % BS, hc = (idx / (BS * BS)) % hf, j = idx / (BS * BS * hf);
+    const float* P0 = part + (size_t)hc * chunk_part + (size_t)layer * nb * S * kWgPartFloats + (size_t)j * S * kWgPartFloats;
+    float2 acc = make_float2(0.f, 0.f);
+    for (int s = 0; s < S; ++s) {
+      const float* Pre = P0 + (size_t)s * kWgPartFloats + (size_t)i * kWgPitch;
+      const float* Pim = P0 + (size_t)s * kWgPartFloats + (size_t)(kWgRowsRe + i) * kWgPitch;
+      acc.x += Pre[o] + Pim[BS + o];
+      acc.y += Pre[BS + o] - Pim[o];
+    }
+    float2* dst = layer ? dW1 + ((size_t)j * BS + i) * hid + hc * BS + o       // W1[j][i][c*96 + o]
+                        : dW2 + ((size_t)j * hid + hc * BS + i) * BS + o;      // W2[j][c*96 + i][o]
+    if (accumulate) { acc.x += dst->x; acc.y += dst->y; }
+    *dst = acc;
+  } else if (idx < nW + nb * hid) {
+    const int k = idx - nW, o = k % BS, hc = (k / BS) % hf, j = k / hid;
+    if (layer == 0 && hc != 0) return;          // db2 comes from chunk 0 only
+    const float* P0 = part + (size_t)hc * chunk_part + (size_t)layer * nb * S * kWgPartFloats + (size_t)j * S * kWgPartFloats +
+                      (size_t)BS * kWgPitch;
+    float2 acc = make_float2(0.f, 0.f);
+    for (int s = 0; s < S; ++s) {
+      acc.x += P0[(size_t)s * kWgPartFloats + o];
+      acc.y += P0[(size_t)s * kWgPartFloats + BS + o];
+    }
+    float2* dst = layer ? dB1 + (size_t)j * hid + hc * BS + o : dB2 + (size_t)j * BS + o;
+    if (accumulate) { acc.x += dst->x; acc.y += dst->y; }
+    *dst = acc;
+  }
+}

@@ -383,9 +383,7 @@ cudaError_t tc_mlp_forward(const Geometry& g, float2* X, const float* w1, const 
 // hybrid backward (hidden factor 1): rows B1 (second half), B3-B7 between the fp32 FFT kernels of generic.cu.
 // X = spectrum of x, G = alpha-weighted spectrum of dY (replaced by GX); the parameter gradients go through the same
 // tc_wgrad + k_tc_wgrad_reduce launches as the fused path, over tiles of 96 consecutive spectrum rows.
-bool tc_mlp_bwd_supported(const Geometry& g) {
-  return g.bf16 && !g.force_fp32 && g.C % 8 == 0 && g.hid == g.bs && g.bs >= 8 && BS % g.bs == 0;
-}
+bool tc_mlp_bwd_supported(const Geometry& g) { return tc_mlp_supported(g); }
 namespace {
 struct MlpBwdWs {
   __nv_bfloat16 *wprep, *Xh, *O1, *G2, *G1;
@@ -420,11 +418,99 @@ MlpBwdWs mlp_bwd_carve(const Geometry& g, char* base) {
   return w;
 }
 } // namespace
-size_t tc_mlp_bwd_workspace_bytes(const Geometry& g) { return mlp_bwd_carve(g, nullptr).total; }
+namespace {
+// hidden factor > 1 (blocks of 96): weight images per (block, chunk), O1 / G1 images per chunk, partial sums per chunk
+struct MlpBwdHfWs {
+  __nv_bfloat16 *wprep, *Xh, *G2, *O1, *G1;
+  float *bprep, *part;
+  int hf, S;
+  long long ntiles;
+  size_t chunk_part_floats, total;
+};
+MlpBwdHfWs mlp_bwd_hf_carve(const Geometry& g, char* base) {
+  MlpBwdHfWs w{};
+  size_t off = 0;
+  auto take = [&](size_t bytes) {
+    char* p = base + off;
+    off = align_up(off + bytes, 256);
+    return p;
+  };
+  w.hf = g.hid / BS;
+  w.ntiles = (g.rows() + HP - 1) / HP;
+  const size_t img = (size_t)w.ntiles * g.nb * kTileBytes;
+  w.wprep = (__nv_bfloat16*)take((size_t)g.nb * w.hf * 4 * kWBytes);
+  w.bprep = (float*)take((size_t)g.nb * (w.hf + 1) * NT * sizeof(float));
+  w.Xh = (__nv_bfloat16*)take(img);
+  w.G2 = (__nv_bfloat16*)take(img);
+  w.O1 = (__nv_bfloat16*)take(img * w.hf);
+  w.G1 = (__nv_bfloat16*)take(img * w.hf);
+  int S = 148 / (2 * g.nb);
+  if (S < 1) S = 1;
+  if ((long long)S > w.ntiles) S = (int)w.ntiles;
+  w.S = S;
+  w.chunk_part_floats = (size_t)2 * g.nb * S * kWgPartFloats;
+  w.part = (float*)take(w.chunk_part_floats * w.hf * sizeof(float));
+  w.total = off;
+  return w;
+}
+
+cudaError_t tc_mlp_backward_hf(const Geometry& g, const float2* X, float2* G, const float* w1, const float* b1, const float* w2,
+                               const float* b2, float* dw1, float* db1, float* dw2, float* db2, uint8_t* mask1, uint8_t* mask2,
+                               void* ws, cudaStream_t st) {
+  cudaError_t e;
+  if ((e = set_smem(tc_mlp_bwd_hf, kMlpBwdHfSmem)) != cudaSuccess) return e;
+  if ((e = set_smem(tc_wgrad, kWgSmem)) != cudaSuccess) return e;
+  const MlpBwdHfWs w = mlp_bwd_hf_carve(g, (char*)ws);
+  const int hf = w.hf, nW = g.nb * hf * BS * BS;
+  prof_begin("k_tc_prep_weights", st);
+  k_tc_prep_weights_hf<<<(nW + 255) / 256, 256, 0, st>>>(w1, b1, w2, b2, w.wprep, w.bprep, g.nb, hf);
+  prof_end(st);
+  count_launch();
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  int dev = 0, sms = 148;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+  if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+  MlpBwdHfParams mp{};
+  mp.X = X; mp.G = G; mp.wprep = (const uint8_t*)w.wprep; mp.bprep = w.bprep;
+  mp.Xh = w.Xh; mp.G2 = w.G2; mp.O1 = w.O1; mp.G1 = w.G1; mp.mask1 = mask1; mp.mask2 = mask2;
+  mp.rows = g.rows(); mp.ntiles = w.ntiles; mp.C = g.C; mp.nb = g.nb; mp.H = g.H; mp.Kw = g.Kw; mp.Wh = g.Wh; mp.Kh = g.Kh;
+  mp.hf = hf; mp.lambda = g.lambda;
+  int S = sms / g.nb;
+  if (S < 1) S = 1;
+  if ((long long)S > w.ntiles) S = (int)w.ntiles;
+  prof_begin("tc_mlp_bwd_hf", st);
+  e = launch_k(tc_mlp_bwd_hf, g.nb * S, kMlpThreads, kMlpBwdHfSmem, st, true, mp, S);
+  prof_end(st);
+  count_launch();
+  if (e != cudaSuccess || (e = cudaGetLastError()) != cudaSuccess) return e;
+  const size_t img = (size_t)w.ntiles * g.nb * kTileBytes;
+  for (int hc = 0; hc < hf; ++hc) {
+    // chunk hc: layer 2 = (O1_c, G2) -> dW2[c rows]; layer 1 = (Xh, G1_c) -> dW1[:, c columns]
+    prof_begin("tc_wgrad", st);
+    e = launch_k(tc_wgrad, 2 * g.nb * w.S, 128, kWgSmem, st, true, (const __nv_bfloat16*)((const char*)w.O1 + hc * img), w.G2, w.Xh,
+                 (const __nv_bfloat16*)((const char*)w.G1 + hc * img), w.part + hc * w.chunk_part_floats, (int)w.ntiles, HP, g.nb,
+                 w.S, 0);
+    prof_end(st);
+    count_launch();
+    if (e != cudaSuccess || (e = cudaGetLastError()) != cudaSuccess) return e;
+  }
+  const int nred = nW + g.nb * g.hid;
+  prof_begin("k_tc_wgrad_reduce", st);
+  e = launch_k(k_tc_wgrad_reduce_hf, dim3((nred + 255) / 256, 2), 256, 0, st, true, w.part, (float2*)dw2, (float2*)db2,
+               (float2*)dw1, (float2*)db1, g.nb, w.S, hf, g.accum ? 1 : 0);
+  prof_end(st);
+  count_launch();
+  return e != cudaSuccess ? e : cudaGetLastError();
+}
+} // namespace
+size_t tc_mlp_bwd_workspace_bytes(const Geometry& g) {
+  return g.hid != g.bs ? mlp_bwd_hf_carve(g, nullptr).total : mlp_bwd_carve(g, nullptr).total;
+}
 
 cudaError_t tc_mlp_backward(const Geometry& g, const float2* X, float2* G, const float* w1, const float* b1, const float* w2,
                             const float* b2, float* dw1, float* db1, float* dw2, float* db2, uint8_t* mask1, uint8_t* mask2,
                             void* ws, cudaStream_t st) {
+  if (g.hid != g.bs) return tc_mlp_backward_hf(g, X, G, w1, b1, w2, b2, dw1, db1, dw2, db2, mask1, mask2, ws, st);
   cudaError_t e;
   if ((e = set_smem(tc_mlp_bwd, kMlpBwdSmem)) != cudaSuccess) return e;
   if ((e = set_smem(tc_wgrad, kWgSmem)) != cudaSuccess) return e;

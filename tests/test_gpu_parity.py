@@ -359,6 +359,39 @@ def test_bf16_backward_beyond_the_fused_chain(oracle, B, H, W, C, nb, f):
         assert np.allclose(t.cpu().numpy(), 1.0 + g[k], rtol=0, atol=2e-6 * max(1.0, np.abs(g[k]).max())), k
 
 
+@pytest.mark.parametrize("B,H,W,C,nb,hf,f", [
+    (2, 16, 32, 192, 2, 2, 1.0),     # hidden = 192 per block, small grid, ragged last tile
+    (1, 100, 40, 96, 1, 3, 0.5),     # hidden = 288, H past the fused chain's limit, truncated
+    (1, 90, 180, 768, 8, 2, 1.0),    # the headline grid with hidden factor 2
+])
+def test_bf16_hidden_factor_backward(oracle, B, H, W, C, nb, hf, f):
+    """hidden factor > 1, BACKWARD on the hybrid path (tc_mlp_bwd_hf: two passes over the 96-wide
+    hidden chunks, P2 and GX accumulated over the chunks in tensor memory, one tc_wgrad launch per chunk), mask-consistently
+    against the oracle per tile and per block; ACCUM_GRADS on top."""
+    import torch
+    wl = inputs.Workload(5, f"{H}x{W}x{C} nb={nb} hf={hf} bf16 B={B} bwd", B, H, W, C, nb, hf, 0.01, f, "bf16", True, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert desc.hidden_factor == hf and binding.afno_spectral_path(desc) == "hybrid-fft32-tcgen05"
+    g = _check_backward(oracle, desc, data, label=wl.name)
+    args = (data["x"], data["dy"], data["w1"], data["b1"], data["w2"], data["b2"])
+    d32 = parity.desc_for(wl, flags=binding.FLAG_FORCE_FP32_MATH)
+    g32 = parity.GpuLayer(d32).backward(*args)
+    assert parity.rel_l2(g["dx"], g32["dx"]) <= 5e-3
+    layer = parity.GpuLayer(desc)
+    d_acc = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_ACCUM_GRADS})
+    ws = torch.empty(binding.afno_spectral_workspace_bytes(d_acc, True), dtype=torch.uint8, device="cuda")
+    tx, tdy = parity.to_device_act(data["x"], True), parity.to_device_act(data["dy"], True)
+    p = layer.params(data["w1"], data["b1"], data["w2"], data["b2"])
+    acc = [torch.ones_like(t) for t in p]
+    tdx = torch.empty_like(tx)
+    binding.afno_spectral_bwd(d_acc, tx, tdy, *p, tdx, *acc, ws)
+    torch.cuda.synchronize()
+    assert np.array_equal(parity.from_device_act(tdx), g["dx"])
+    for t, k in zip(acc, ("dw1", "db1", "dw2", "db2")):
+        assert np.allclose(t.cpu().numpy(), 1.0 + g[k], rtol=0, atol=2e-6 * max(1.0, np.abs(g[k]).max())), k
+
+
 def test_bf16_paper_shape_backward(oracle):
     """the paper's own layer shape (180 x 360 tokens, 1,024 channels in 32 blocks of 32), backward on
     the hybrid path, mask-consistently against the oracle per tile and per block."""

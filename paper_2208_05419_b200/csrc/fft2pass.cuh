@@ -1,0 +1,280 @@
+// Part of generic.cu (included inside namespace afno { namespace { after the radix butterflies): two-pass FFT kernels
+// for the grid sizes of BASELINE.json and of the paper (90, 180, 360 points per axis).
+//
+// The generic kernels above run one radix-2/3/4/5 stage per pass over shared memory; ncu shows them bound by the
+// instruction issue rate (index arithmetic, twiddle loads, one butterfly per warp iteration: 27 k warp instructions per
+// 180-point x 32-channel tile where the arithmetic needs ~6 k).  Here N = N1 x N2 and each of the two passes is a
+// complete length-N1 (length-N2) transform held in REGISTERS by one thread (lane = channel), fully unrolled, every
+// inner twiddle a compile-time constant:
+//   n = N2 n1 + n2, k = k1 + N1 k2:
+//   pass A (per n2): y[k1] = w_N^(n2 k1) sum_n1 x[N2 n1 + n2] w_N1^(n1 k1)       -> shared memory row k1 N2 + n2
+//   pass B (per k1): X[k1 + N1 k2] = sum_n2 y[k1 N2 + n2] w_N2^(n2 k2)           -> natural order, straight to global memory
+// Two shared-memory passes instead of four or five, no output permutation.  Same arithmetic (fp32), same results to
+// rounding; used when the size is in the table below and C is a multiple of 64, the generic kernels otherwise.
+constexpr double cx_pi = 3.14159265358979323846264338327950288;
+constexpr double cx_sin(double x) {   // |x| <= pi
+  double x2 = x * x, term = x, sum = x;
+  for (int i = 1; i <= 16; ++i) {
+    term *= -x2 / (double)((2 * i) * (2 * i + 1));
+    sum += term;
+  }
+  return sum;
+}
+constexpr double cx_cos(double x) {
+  double x2 = x * x, term = 1.0, sum = 1.0;
+  for (int i = 1; i <= 16; ++i) {
+    term *= -x2 / (double)((2 * i - 1) * (2 * i));
+    sum += term;
+  }
+  return sum;
+}
+
+template <int N>
+struct FirstRadix {
+  static constexpr int value = (N <= 5) ? N : (N % 4 == 0) ? 4 : (N % 2 == 0) ? 2 : (N % 3 == 0) ? 3 : 5;
+};
+
+// natural-order in, natural-order out; SG = -1 forward (exp(-i..)), +1 inverse
+template <int N, int SG>
+struct RegFFT {
+  static constexpr int R = FirstRadix<N>::value, M = N / R;
+  template <int E>
+  static __device__ __forceinline__ float2 twiddle(float2 t) {
+    constexpr int e = E % N;
+    if constexpr (e == 0) {
+      return t;
+    } else {
+      constexpr double ang = 2.0 * cx_pi * (double)(e > N / 2 ? e - N : e) / (double)N;
+      constexpr float c = (float)cx_cos(ang), s = (float)((double)SG * cx_sin(ang));
+      return make_float2(fmaf(t.x, c, -t.y * s), fmaf(t.x, s, t.y * c));
+    }
+  }
+  template <int J, int... P>
+  static __device__ __forceinline__ void column(const float2 (&v)[N], float2 (&y)[R][M], std::integer_sequence<int, P...>) {
+    float2 t[R];
+    ((t[P] = v[P * M + J]), ...);
+    small_dft<R>(t, (float)SG);
+    ((y[P][J] = twiddle<J * P>(t[P])), ...);
+  }
+  template <int... J>
+  static __device__ __forceinline__ void columns(const float2 (&v)[N], float2 (&y)[R][M], std::integer_sequence<int, J...>) {
+    (column<J>(v, y, std::make_integer_sequence<int, R>{}), ...);
+  }
+  static __device__ __forceinline__ void run(float2 (&v)[N]) {
+    if constexpr (N <= 5) {
+      small_dft<N>(v, (float)SG);
+    } else {
+      float2 y[R][M];
+      columns(v, y, std::make_integer_sequence<int, M>{});
+#pragma unroll
+      for (int p = 0; p < R; ++p) RegFFT<M, SG>::run(y[p]);
+#pragma unroll
+      for (int p = 0; p < R; ++p)
+#pragma unroll
+        for (int k = 0; k < M; ++k) v[R * k + p] = y[p][k];
+    }
+  }
+};
+
+// pass A of one (n2, lane): rows n1 N2 + n2 -> rows k1 N2 + n2, in place.  tw[k] = exp(-2 pi i k / N).
+template <int N1, int N2, int SG>
+__device__ __forceinline__ void pass_a(float2* s, int lw, int l, int n2, const float2* __restrict__ tw) {
+  float2 v[N1];
+#pragma unroll
+  for (int n1 = 0; n1 < N1; ++n1) v[n1] = s[(n1 * N2 + n2) * lw + l];
+  RegFFT<N1, SG>::run(v);
+  s[n2 * lw + l] = v[0];
+#pragma unroll
+  for (int k1 = 1; k1 < N1; ++k1) {
+    float2 o = v[k1];
+    if (n2 != 0) {
+      float2 t = __ldg(tw + n2 * k1);   // uniform across the warp
+      if (SG > 0) t.y = -t.y;
+      o = cmul(o, t);
+    }
+    s[(k1 * N2 + n2) * lw + l] = o;
+  }
+}
+// pass B of one (k1, lane): rows k1 N2 + n2 -> v[k2] = X[k1 + N1 k2]
+template <int N1, int N2, int SG>
+__device__ __forceinline__ void pass_b(const float2* s, int lw, int l, int k1, float2 (&v)[N2]) {
+#pragma unroll
+  for (int n2 = 0; n2 < N2; ++n2) v[n2] = s[(k1 * N2 + n2) * lw + l];
+  RegFFT<N2, SG>::run(v);
+}
+
+constexpr int kF2Warps = 8;
+
+// ---- F2 / F7: H-direction complex FFT, in place on S[B][H][Kw][C]; tile = 64 channels of one (b, kw) column ----------
+// grid (C / 64, Kw, B), block 256; smem H * 64 float2
+template <int N1, int N2, int SG>
+__global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(float2* __restrict__ S, const float2* __restrict__ tw, int Kw, int C) {
+  constexpr int H = N1 * N2;
+  extern __shared__ float2 smem[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int kw = blockIdx.y, b = blockIdx.z;
+  float2* base = S + ((size_t)b * H * Kw + kw) * C + (size_t)blockIdx.x * 64;
+  const size_t hstride = (size_t)Kw * C;
+  // a row of the tile is 512 contiguous bytes: one float4 per lane
+  for (int h0 = warp; h0 < H; h0 += kF2Warps * kLoadBatch) {
+    float4 v[kLoadBatch];
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int h = h0 + u * kF2Warps;
+      if (h < H) v[u] = *(const float4*)(base + (size_t)h * hstride + 2 * lane);
+    }
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int h = h0 + u * kF2Warps;
+      if (h < H) *(float4*)(smem + h * 64 + 2 * lane) = v[u];
+    }
+  }
+  __syncthreads();
+  for (int task = warp; task < 2 * N2; task += kF2Warps) {
+    const int g = task / N2, n2 = task - g * N2;
+    pass_a<N1, N2, SG>(smem, 64, g * 32 + lane, n2, tw);
+  }
+  __syncthreads();
+  for (int task = warp; task < 2 * N1; task += kF2Warps) {
+    const int g = task / N1, k1 = task - g * N1;
+    float2 v[N2];
+    pass_b<N1, N2, SG>(smem, 64, g * 32 + lane, k1, v);
+    float2* dst = base + g * 32 + lane;
+#pragma unroll
+    for (int k2 = 0; k2 < N2; ++k2) dst[(size_t)(k1 + N1 * k2) * hstride] = v[k2];
+  }
+}
+
+// ---- F1 / B2: W-direction real FFT, two real channels packed into one complex transform ---------------------------------
+// grid (C / 64, H, B), block 256; smem W * 32 float2.  Pass B runs the tasks k1 and N1 - k1 together: the Hermitian
+// split of bin k needs Z[k] and Z[W - k], which live in exactly those two tasks, so the half-spectrum leaves from
+// registers.
+template <typename T, int N1, int N2>
+__global__ void __launch_bounds__(32 * kF2Warps)
+k_wfft_fwd2(const T* __restrict__ x, float2* __restrict__ S, const float2* __restrict__ tw, int H, int C, int Kw, float scale,
+            int alpha_weight) {
+  constexpr int W = N1 * N2;
+  extern __shared__ float2 smem[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int h = blockIdx.y, b = blockIdx.z;
+  const int c = blockIdx.x * 64 + 2 * lane;
+  const T* xrow = x + ((size_t)(b * H + h) * W) * C + c;
+  for (int w0 = warp; w0 < W; w0 += kF2Warps * kLoadBatch) {
+    float2 v[kLoadBatch];
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int w = w0 + u * kF2Warps;
+      if (w < W) v[u] = ActIO<T>::ld2(xrow + (size_t)w * C);
+    }
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int w = w0 + u * kF2Warps;
+      if (w < W) smem[w * 32 + lane] = v[u];   // channel c in the real part, channel c + 1 in the imaginary part
+    }
+  }
+  __syncthreads();
+  for (int n2 = warp; n2 < N2; n2 += kF2Warps) pass_a<N1, N2, -1>(smem, 32, lane, n2, tw);
+  __syncthreads();
+  float2* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
+  // bin k from Z[k] = zk and Z[W - k] = zn (both channels of the pair)
+  auto emit = [&](int k, float2 zk, float2 zn) {
+    if (k >= Kw) return;
+    float sc = 0.5f * scale;
+    if (alpha_weight && k != 0 && 2 * k != W) sc *= 2.f;
+    *(float4*)(Srow + (size_t)k * C) = make_float4(sc * (zk.x + zn.x), sc * (zk.y - zn.y), sc * (zk.y + zn.y), -sc * (zk.x - zn.x));
+  };
+  // work items: k1 = 0 alone, k1 = N1 / 2 alone (N1 even), pairs (k1, N1 - k1)
+  constexpr int kItems = N1 / 2 + 1;
+  for (int item = warp; item < kItems; item += kF2Warps) {
+    const int ka = item, kb = (N1 - item) % N1;
+    float2 va[N2];
+    pass_b<N1, N2, -1>(smem, 32, lane, ka, va);
+    if (ka == kb) {
+      if (ka == 0) {
+        // k = N1 k2, W - k = N1 (N2 - k2)
+#pragma unroll
+        for (int k2 = 0; k2 < N2; ++k2) emit(N1 * k2, va[k2], va[(N2 - k2) % N2]);
+      } else {
+        // k1 = N1 / 2: W - k = k1 + N1 (N2 - 1 - k2)
+#pragma unroll
+        for (int k2 = 0; k2 < N2; ++k2) emit(ka + N1 * k2, va[k2], va[N2 - 1 - k2]);
+      }
+    } else {
+      float2 vb[N2];
+      pass_b<N1, N2, -1>(smem, 32, lane, kb, vb);
+#pragma unroll
+      for (int k2 = 0; k2 < N2; ++k2) {
+        emit(ka + N1 * k2, va[k2], vb[N2 - 1 - k2]);
+        emit(kb + N1 * k2, vb[k2], va[N2 - 1 - k2]);
+      }
+    }
+  }
+}
+
+// ---- F8 + F9 / B8: W-direction complex-to-real inverse FFT, residual, store ------------------------------------------
+// grid (C / 64, H, B), block 256; smem W * 32 float2
+template <typename T, int N1, int N2>
+__global__ void __launch_bounds__(32 * kF2Warps)
+k_wfft_inv2(const float2* __restrict__ S, const T* __restrict__ res, T* __restrict__ out, const float2* __restrict__ tw, int H,
+            int C, int Kw, float scale, int half_interior) {
+  constexpr int W = N1 * N2;
+  extern __shared__ float2 smem[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int h = blockIdx.y, b = blockIdx.z;
+  const int c = blockIdx.x * 64 + 2 * lane;
+  const float2* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
+  for (int k0 = warp; k0 < W; k0 += kF2Warps * kLoadBatch) {
+    float4 t[kLoadBatch];
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int k = k0 + u * kF2Warps;
+      const int kk = 2 * k > W ? W - k : k;
+      t[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (k < W && kk < Kw) t[u] = __ldg((const float4*)(Srow + (size_t)kk * C));
+    }
+#pragma unroll
+    for (int u = 0; u < kLoadBatch; ++u) {
+      const int k = k0 + u * kF2Warps;
+      if (k >= W) continue;
+      const bool mirrored = 2 * k > W;
+      const int kk = mirrored ? W - k : k;
+      float2 z = make_float2(0.f, 0.f);
+      if (kk < Kw) {
+        float2 ta = make_float2(t[u].x, t[u].y), tb = make_float2(t[u].z, t[u].w);
+        if (kk == 0 || 2 * kk == W) {
+          ta.y = 0.f;   // reading A4: imaginary parts of the c = 0 and c = W/2 columns are discarded
+          tb.y = 0.f;
+        } else {
+          if (half_interior) { ta.x *= 0.5f; ta.y *= 0.5f; tb.x *= 0.5f; tb.y *= 0.5f; }
+          if (mirrored) { ta.y = -ta.y; tb.y = -tb.y; }   // Hermitian extension
+        }
+        z = make_float2(ta.x - tb.y, ta.y + tb.x);   // Ta + i Tb: channel c -> Re, channel c + 1 -> Im
+      }
+      smem[k * 32 + lane] = z;
+    }
+  }
+  __syncthreads();
+  for (int n2 = warp; n2 < N2; n2 += kF2Warps) pass_a<N1, N2, +1>(smem, 32, lane, n2, tw);
+  __syncthreads();
+  const size_t rowoff = ((size_t)(b * H + h) * W) * C + c;
+  for (int k1 = warp; k1 < N1; k1 += kF2Warps) {
+    float2 r[N2];
+#pragma unroll
+    for (int k2 = 0; k2 < N2; ++k2)
+      r[k2] = res ? ActIO<T>::ld2(res + rowoff + (size_t)(k1 + N1 * k2) * C) : make_float2(0.f, 0.f);
+    float2 v[N2];
+    pass_b<N1, N2, +1>(smem, 32, lane, k1, v);
+#pragma unroll
+    for (int k2 = 0; k2 < N2; ++k2)
+      ActIO<T>::st2(out + rowoff + (size_t)(k1 + N1 * k2) * C, scale * v[k2].x + r[k2].x, scale * v[k2].y + r[k2].y);
+  }
+}
+
+// size table: N -> (N1, N2)
+template <typename F>
+bool fft2_dispatch(int n, F&& f) {
+  if (n == 90) { f(std::integral_constant<int, 9>{}, std::integral_constant<int, 10>{}); return true; }
+  if (n == 180) { f(std::integral_constant<int, 12>{}, std::integral_constant<int, 15>{}); return true; }
+  if (n == 360) { f(std::integral_constant<int, 18>{}, std::integral_constant<int, 20>{}); return true; }
+  return false;
+}

@@ -17,6 +17,9 @@
 // butterfly is conflict-free and needs no shuffles; warps split the butterflies of a stage.
 #include <cuda_bf16.h>
 
+#include <type_traits>
+#include <utility>
+
 #include "afno_internal.h"
 
 namespace afno {
@@ -317,6 +320,8 @@ k_wfft_inv(const float2* __restrict__ S, const T* __restrict__ res, T* __restric
   }
 }
 
+#include "fft2pass.cuh"
+
 // ---- F3-F6 / B5 / B7: block-diagonal complex GEMM over modes ----------------------------
 enum { EPI_RELU = 0, EPI_SHRINK = 1, EPI_MASK = 2, EPI_NONE = 3 };
 constexpr int kGemmTM = 64, kGemmRM = 8, kGemmThreads = 256;
@@ -538,6 +543,17 @@ cudaError_t set_smem(K kernel, size_t bytes) {
 template <typename T>
 void launch_wfft_fwd(Launcher& L, const Geometry& g, const Plan& p, const T* x, float2* S, bool alpha) {
   if (L.err != cudaSuccess) return;
+  if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2) {
+        constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value;
+        const size_t smem2 = (size_t)g.W * 32 * sizeof(float2);
+        L.err = set_smem(k_wfft_fwd2<T, N1, N2>, smem2);
+        if (L.err != cudaSuccess) return;
+        L.begin("k_wfft_fwd");
+        k_wfft_fwd2<T, N1, N2><<<dim3(g.C / 64, g.H, g.B), 32 * kF2Warps, smem2, L.st>>>(x, S, p.fw.tw, g.H, g.C, g.Kw, g.scale,
+                                                                                          alpha ? 1 : 0);
+        L.check();
+      }))
+    return;
   const size_t smem = (size_t)g.W * kLanes * sizeof(float2);
   L.err = set_smem(k_wfft_fwd<T>, smem);
   if (L.err != cudaSuccess) return;
@@ -549,6 +565,17 @@ void launch_wfft_fwd(Launcher& L, const Geometry& g, const Plan& p, const T* x, 
 
 void launch_hfft(Launcher& L, const Geometry& g, const Plan& p, float2* S, int C, bool inverse) {
   if (L.err != cudaSuccess) return;
+  if (C % 64 == 0 && fft2_dispatch(g.H, [&](auto n1, auto n2) {
+        constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value;
+        const size_t smem2 = (size_t)g.H * 64 * sizeof(float2);
+        L.err = inverse ? set_smem(k_hfft2<N1, N2, +1>, smem2) : set_smem(k_hfft2<N1, N2, -1>, smem2);
+        if (L.err != cudaSuccess) return;
+        L.begin("k_hfft");
+        if (inverse) k_hfft2<N1, N2, +1><<<dim3(C / 64, g.Kw, g.B), 32 * kF2Warps, smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
+        else k_hfft2<N1, N2, -1><<<dim3(C / 64, g.Kw, g.B), 32 * kF2Warps, smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
+        L.check();
+      }))
+    return;
   const size_t smem = (size_t)g.H * kLanes * sizeof(float2);
   L.err = set_smem(k_hfft, smem);
   if (L.err != cudaSuccess) return;
@@ -562,6 +589,17 @@ template <typename T>
 void launch_wfft_inv(Launcher& L, const Geometry& g, const Plan& p, const float2* S, const T* res, T* out,
                      bool half_interior) {
   if (L.err != cudaSuccess) return;
+  if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2) {
+        constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value;
+        const size_t smem2 = (size_t)g.W * 32 * sizeof(float2);
+        L.err = set_smem(k_wfft_inv2<T, N1, N2>, smem2);
+        if (L.err != cudaSuccess) return;
+        L.begin("k_wfft_inv");
+        k_wfft_inv2<T, N1, N2><<<dim3(g.C / 64, g.H, g.B), 32 * kF2Warps, smem2, L.st>>>(S, res, out, p.fw.tw, g.H, g.C, g.Kw, g.scale,
+                                                                                          half_interior ? 1 : 0);
+        L.check();
+      }))
+    return;
   const size_t smem = (size_t)g.W * kLanes * sizeof(float2);
   L.err = set_smem(k_wfft_inv<T>, smem);
   if (L.err != cudaSuccess) return;

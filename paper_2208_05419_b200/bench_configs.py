@@ -43,6 +43,8 @@ CONFIGS = {
     "paper shape 180x360x1024 nb=32 fwd B=2 (hybrid)": (2, 180, 360, 1024, 32, 1, 1.0, False, False),
     "paper shape 180x360x1024 nb=32 fwd+bwd B=1 (hybrid)": (1, 180, 360, 1024, 32, 1, 1.0, True, False),
     "hidden factor 2, 90x180x768 fwd B=4 (hybrid)": (4, 90, 180, 768, 8, 2, 1.0, False, False),
+    "hidden factor 2, 90x180x768 fwd+bwd B=4 (hybrid)": (4, 90, 180, 768, 8, 2, 1.0, True, False),
+    "fp32 activations 90x180x768 fwd+bwd B=2 (generic)": (2, 90, 180, 768, 8, 1, 1.0, True, False),
 }
 
 
@@ -61,20 +63,22 @@ def run(name, cfg, calls, reps):
 
     B, H, W, C, nb, hf, f, backward, ctx = cfg
     hbm, tensor, src = _peaks()
-    desc = binding.Desc(B, H, W, C, nb, hf, 0.01, f, binding.AFNO_BF16, 0)
+    f32 = name.startswith("fp32")
+    adt = torch.float32 if f32 else torch.bfloat16
+    desc = binding.Desc(B, H, W, C, nb, hf, 0.01, f, binding.AFNO_F32 if f32 else binding.AFNO_BF16, 0)
     binding.afno_plan_warmup(desc)
     dev = torch.device("cuda")
     g = torch.Generator(device="cuda").manual_seed(1)
     act = B * H * W * C
-    nsets = max(2, int(np.ceil(300e6 / (act * 2 * (4 if backward else 2)))))
+    nsets = max(2, int(np.ceil(300e6 / (act * (4 if name.startswith("fp32") else 2) * (4 if backward else 2)))))
     nsets = min(nsets, 8)
     bs = C // nb
     hid = bs * hf
     sets = []
     for _ in range(nsets):
-        s = dict(x=torch.randn((B, H, W, C), device=dev, generator=g).to(torch.bfloat16), y=torch.empty((B, H, W, C), device=dev, dtype=torch.bfloat16))
+        s = dict(x=torch.randn((B, H, W, C), device=dev, generator=g).to(adt), y=torch.empty((B, H, W, C), device=dev, dtype=adt))
         if backward:
-            s["dy"] = torch.randn((B, H, W, C), device=dev, generator=g).to(torch.bfloat16)
+            s["dy"] = torch.randn((B, H, W, C), device=dev, generator=g).to(adt)
             s["dx"] = torch.empty_like(s["x"])
         sets.append(s)
     params = [0.02 * torch.randn(shape, device=dev, generator=g) for shape in
@@ -114,7 +118,7 @@ def run(name, cfg, calls, reps):
         call(i)
     prof = binding.afno_profile_stop()
     # 2-term layer roofline: compulsory bytes and model MLP FLOPs
-    a_bytes = act * 2
+    a_bytes = act * (4 if f32 else 2)
     pbytes = 2 * (nb * bs * hid * 2 + (hid + bs) * nb) * 4
     nbytes = (2 * a_bytes + pbytes) + ((3 * a_bytes + 2 * pbytes) if backward else 0)
     gemm = 2 * (2 * bs) * (2 * hid) * nb * kept_modes(H, W, f) * B

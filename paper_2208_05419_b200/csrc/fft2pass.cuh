@@ -223,34 +223,29 @@ k_wfft_inv2(const float2* __restrict__ S, const T* __restrict__ res, T* __restri
   const int h = blockIdx.y, b = blockIdx.z;
   const int c = blockIdx.x * 64 + 2 * lane;
   const float2* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
-  for (int k0 = warp; k0 < W; k0 += kF2Warps * kLoadBatch) {
+  // every stored bin kk <= W/2 feeds the transform twice: as z[kk] and, conjugated (Hermitian extension), as z[W - kk]
+  for (int k0 = warp; k0 <= W / 2; k0 += kF2Warps * kLoadBatch) {
     float4 t[kLoadBatch];
 #pragma unroll
     for (int u = 0; u < kLoadBatch; ++u) {
-      const int k = k0 + u * kF2Warps;
-      const int kk = 2 * k > W ? W - k : k;
+      const int kk = k0 + u * kF2Warps;
       t[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (k < W && kk < Kw) t[u] = __ldg((const float4*)(Srow + (size_t)kk * C));
+      if (kk < Kw) t[u] = __ldg((const float4*)(Srow + (size_t)kk * C));
     }
 #pragma unroll
     for (int u = 0; u < kLoadBatch; ++u) {
-      const int k = k0 + u * kF2Warps;
-      if (k >= W) continue;
-      const bool mirrored = 2 * k > W;
-      const int kk = mirrored ? W - k : k;
-      float2 z = make_float2(0.f, 0.f);
-      if (kk < Kw) {
-        float2 ta = make_float2(t[u].x, t[u].y), tb = make_float2(t[u].z, t[u].w);
-        if (kk == 0 || 2 * kk == W) {
-          ta.y = 0.f;   // reading A4: imaginary parts of the c = 0 and c = W/2 columns are discarded
-          tb.y = 0.f;
-        } else {
-          if (half_interior) { ta.x *= 0.5f; ta.y *= 0.5f; tb.x *= 0.5f; tb.y *= 0.5f; }
-          if (mirrored) { ta.y = -ta.y; tb.y = -tb.y; }   // Hermitian extension
-        }
-        z = make_float2(ta.x - tb.y, ta.y + tb.x);   // Ta + i Tb: channel c -> Re, channel c + 1 -> Im
+      const int kk = k0 + u * kF2Warps;
+      if (kk > W / 2) continue;
+      float2 ta = make_float2(t[u].x, t[u].y), tb = make_float2(t[u].z, t[u].w);
+      if (kk == 0 || 2 * kk == W) {
+        ta.y = 0.f;   // reading A4: imaginary parts of the c = 0 and c = W/2 columns are discarded
+        tb.y = 0.f;
+      } else if (half_interior) {
+        ta.x *= 0.5f; ta.y *= 0.5f; tb.x *= 0.5f; tb.y *= 0.5f;
       }
-      smem[k * 32 + lane] = z;
+      // Ta + i Tb: channel c -> Re, channel c + 1 -> Im
+      smem[kk * 32 + lane] = make_float2(ta.x - tb.y, ta.y + tb.x);
+      if (kk != 0 && 2 * kk != W) smem[(W - kk) * 32 + lane] = make_float2(ta.x + tb.y, -ta.y + tb.x);   // conj(Ta) + i conj(Tb)
     }
   }
   __syncthreads();

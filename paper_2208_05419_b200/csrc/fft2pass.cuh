@@ -116,16 +116,18 @@ __global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(float2* __restrict__ S,
   float2* base = S + ((size_t)b * H * Kw + kw) * C + (size_t)blockIdx.x * 64;
   const size_t hstride = (size_t)Kw * C;
   // a row of the tile is 512 contiguous bytes: one float4 per lane
-  for (int h0 = warp; h0 < H; h0 += kF2Warps * kLoadBatch) {
-    float4 v[kLoadBatch];
+  // (every row of the warp is in flight before the first shared-memory store: one latency period per tile)
+  {
+    constexpr int LB = (H + kF2Warps - 1) / kF2Warps;
+    float4 v[LB];
 #pragma unroll
-    for (int u = 0; u < kLoadBatch; ++u) {
-      const int h = h0 + u * kF2Warps;
+    for (int u = 0; u < LB; ++u) {
+      const int h = warp + u * kF2Warps;
       if (h < H) v[u] = *(const float4*)(base + (size_t)h * hstride + 2 * lane);
     }
 #pragma unroll
-    for (int u = 0; u < kLoadBatch; ++u) {
-      const int h = h0 + u * kF2Warps;
+    for (int u = 0; u < LB; ++u) {
+      const int h = warp + u * kF2Warps;
       if (h < H) *(float4*)(smem + h * 64 + 2 * lane) = v[u];
     }
   }
@@ -149,8 +151,8 @@ __global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(float2* __restrict__ S,
 // grid (C / 64, H, B), block 256; smem W * 32 float2.  Pass B runs the tasks k1 and N1 - k1 together: the Hermitian
 // split of bin k needs Z[k] and Z[W - k], which live in exactly those two tasks, so the half-spectrum leaves from
 // registers.
-template <typename T, int N1, int N2>
-__global__ void __launch_bounds__(32 * kF2Warps)
+template <typename T, int N1, int N2, int NW>
+__global__ void __launch_bounds__(32 * NW, 2)
 k_wfft_fwd2(const T* __restrict__ x, float2* __restrict__ S, const float2* __restrict__ tw, int H, int C, int Kw, float scale,
             int alpha_weight) {
   constexpr int W = N1 * N2;
@@ -159,21 +161,23 @@ k_wfft_fwd2(const T* __restrict__ x, float2* __restrict__ S, const float2* __res
   const int h = blockIdx.y, b = blockIdx.z;
   const int c = blockIdx.x * 64 + 2 * lane;
   const T* xrow = x + ((size_t)(b * H + h) * W) * C + c;
-  for (int w0 = warp; w0 < W; w0 += kF2Warps * kLoadBatch) {
-    float2 v[kLoadBatch];
+  {
+    // all rows of the warp in flight at once, kept in the storage type (bf16 pairs: one register each)
+    constexpr int LB = (W + NW - 1) / NW;
+    typename ActIO<T>::raw2 v[LB];
 #pragma unroll
-    for (int u = 0; u < kLoadBatch; ++u) {
-      const int w = w0 + u * kF2Warps;
-      if (w < W) v[u] = ActIO<T>::ld2(xrow + (size_t)w * C);
+    for (int u = 0; u < LB; ++u) {
+      const int w = warp + u * NW;
+      if (w < W) v[u] = ActIO<T>::ldraw2(xrow + (size_t)w * C);
     }
 #pragma unroll
-    for (int u = 0; u < kLoadBatch; ++u) {
-      const int w = w0 + u * kF2Warps;
-      if (w < W) smem[w * 32 + lane] = v[u];   // channel c in the real part, channel c + 1 in the imaginary part
+    for (int u = 0; u < LB; ++u) {
+      const int w = warp + u * NW;
+      if (w < W) smem[w * 32 + lane] = ActIO<T>::unraw2(v[u]);   // channel c in the real part, channel c + 1 in the imaginary part
     }
   }
   __syncthreads();
-  for (int n2 = warp; n2 < N2; n2 += kF2Warps) pass_a<N1, N2, -1>(smem, 32, lane, n2, tw);
+  for (int n2 = warp; n2 < N2; n2 += NW) pass_a<N1, N2, -1>(smem, 32, lane, n2, tw);
   __syncthreads();
   float2* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
   // bin k from Z[k] = zk and Z[W - k] = zn (both channels of the pair)
@@ -185,7 +189,7 @@ k_wfft_fwd2(const T* __restrict__ x, float2* __restrict__ S, const float2* __res
   };
   // work items: k1 = 0 alone, k1 = N1 / 2 alone (N1 even), pairs (k1, N1 - k1)
   constexpr int kItems = N1 / 2 + 1;
-  for (int item = warp; item < kItems; item += kF2Warps) {
+  for (int item = warp; item < kItems; item += NW) {
     const int ka = item, kb = (N1 - item) % N1;
     float2 va[N2];
     pass_b<N1, N2, -1>(smem, 32, lane, ka, va);
@@ -213,8 +217,8 @@ k_wfft_fwd2(const T* __restrict__ x, float2* __restrict__ S, const float2* __res
 
 // ---- F8 + F9 / B8: W-direction complex-to-real inverse FFT, residual, store ------------------------------------------
 // grid (C / 64, H, B), block 256; smem W * 32 float2
-template <typename T, int N1, int N2>
-__global__ void __launch_bounds__(32 * kF2Warps)
+template <typename T, int N1, int N2, int NW>
+__global__ void __launch_bounds__(32 * NW, 2)
 k_wfft_inv2(const float2* __restrict__ S, const T* __restrict__ res, T* __restrict__ out, const float2* __restrict__ tw, int H,
             int C, int Kw, float scale, int half_interior) {
   constexpr int W = N1 * N2;
@@ -224,17 +228,18 @@ k_wfft_inv2(const float2* __restrict__ S, const T* __restrict__ res, T* __restri
   const int c = blockIdx.x * 64 + 2 * lane;
   const float2* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
   // every stored bin kk <= W/2 feeds the transform twice: as z[kk] and, conjugated (Hermitian extension), as z[W - kk]
-  for (int k0 = warp; k0 <= W / 2; k0 += kF2Warps * kLoadBatch) {
-    float4 t[kLoadBatch];
+  {
+    constexpr int LB = (W / 2 + NW) / NW;
+    float4 t[LB];
 #pragma unroll
-    for (int u = 0; u < kLoadBatch; ++u) {
-      const int kk = k0 + u * kF2Warps;
+    for (int u = 0; u < LB; ++u) {
+      const int kk = warp + u * NW;
       t[u] = make_float4(0.f, 0.f, 0.f, 0.f);
       if (kk < Kw) t[u] = __ldg((const float4*)(Srow + (size_t)kk * C));
     }
 #pragma unroll
-    for (int u = 0; u < kLoadBatch; ++u) {
-      const int kk = k0 + u * kF2Warps;
+    for (int u = 0; u < LB; ++u) {
+      const int kk = warp + u * NW;
       if (kk > W / 2) continue;
       float2 ta = make_float2(t[u].x, t[u].y), tb = make_float2(t[u].z, t[u].w);
       if (kk == 0 || 2 * kk == W) {
@@ -249,10 +254,10 @@ k_wfft_inv2(const float2* __restrict__ S, const T* __restrict__ res, T* __restri
     }
   }
   __syncthreads();
-  for (int n2 = warp; n2 < N2; n2 += kF2Warps) pass_a<N1, N2, +1>(smem, 32, lane, n2, tw);
+  for (int n2 = warp; n2 < N2; n2 += NW) pass_a<N1, N2, +1>(smem, 32, lane, n2, tw);
   __syncthreads();
   const size_t rowoff = ((size_t)(b * H + h) * W) * C + c;
-  for (int k1 = warp; k1 < N1; k1 += kF2Warps) {
+  for (int k1 = warp; k1 < N1; k1 += NW) {
     float2 r[N2];
 #pragma unroll
     for (int k2 = 0; k2 < N2; ++k2)
@@ -265,11 +270,12 @@ k_wfft_inv2(const float2* __restrict__ S, const T* __restrict__ res, T* __restri
   }
 }
 
-// size table: N -> (N1, N2)
+// size table: N -> (N1, N2) and the warps per block of the W-direction kernels (pass A has N2 tasks, pass B N1 / 2 + 1
+// paired items forward, N1 tasks inverse)
 template <typename F>
 bool fft2_dispatch(int n, F&& f) {
-  if (n == 90) { f(std::integral_constant<int, 9>{}, std::integral_constant<int, 10>{}); return true; }
-  if (n == 180) { f(std::integral_constant<int, 12>{}, std::integral_constant<int, 15>{}); return true; }
-  if (n == 360) { f(std::integral_constant<int, 18>{}, std::integral_constant<int, 20>{}); return true; }
+  if (n == 90) { f(std::integral_constant<int, 9>{}, std::integral_constant<int, 10>{}, std::integral_constant<int, 5>{}); return true; }
+  if (n == 180) { f(std::integral_constant<int, 12>{}, std::integral_constant<int, 15>{}, std::integral_constant<int, 8>{}); return true; }
+  if (n == 360) { f(std::integral_constant<int, 18>{}, std::integral_constant<int, 20>{}, std::integral_constant<int, 10>{}); return true; }
   return false;
 }

@@ -139,6 +139,9 @@ template <typename T>
 struct ActIO;
 template <>
 struct ActIO<float> {
+  typedef float2 raw2;
+  static __device__ __forceinline__ raw2 ldraw2(const float* p) { return __ldg((const float2*)p); }
+  static __device__ __forceinline__ float2 unraw2(raw2 v) { return v; }
   static __device__ __forceinline__ float ld(const float* p) { return __ldg(p); }
   static __device__ __forceinline__ float2 ld2(const float* p) { return __ldg((const float2*)p); }
   static __device__ __forceinline__ void st(float* p, float v) { *p = v; }
@@ -146,6 +149,9 @@ struct ActIO<float> {
 };
 template <>
 struct ActIO<__nv_bfloat16> {
+  typedef uint32_t raw2;
+  static __device__ __forceinline__ raw2 ldraw2(const __nv_bfloat16* p) { return __ldg((const uint32_t*)p); }
+  static __device__ __forceinline__ float2 unraw2(raw2 v) { return make_float2(__uint_as_float(v << 16), __uint_as_float(v & 0xFFFF0000u)); }
   static __device__ __forceinline__ float ld(const __nv_bfloat16* p) { return __bfloat162float(*p); }
   static __device__ __forceinline__ float2 ld2(const __nv_bfloat16* p) {
     return __bfloat1622float2(*(const __nv_bfloat162*)p);
@@ -543,13 +549,13 @@ cudaError_t set_smem(K kernel, size_t bytes) {
 template <typename T>
 void launch_wfft_fwd(Launcher& L, const Geometry& g, const Plan& p, const T* x, float2* S, bool alpha) {
   if (L.err != cudaSuccess) return;
-  if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2) {
-        constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value;
+  if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2, auto nw) {
+        constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value, NW = decltype(nw)::value;
         const size_t smem2 = (size_t)g.W * 32 * sizeof(float2);
-        L.err = set_smem(k_wfft_fwd2<T, N1, N2>, smem2);
+        L.err = set_smem(k_wfft_fwd2<T, N1, N2, NW>, smem2);
         if (L.err != cudaSuccess) return;
         L.begin("k_wfft_fwd");
-        k_wfft_fwd2<T, N1, N2><<<dim3(g.C / 64, g.H, g.B), 32 * kF2Warps, smem2, L.st>>>(x, S, p.fw.tw, g.H, g.C, g.Kw, g.scale,
+        k_wfft_fwd2<T, N1, N2, NW><<<dim3(g.C / 64, g.H, g.B), 32 * NW, smem2, L.st>>>(x, S, p.fw.tw, g.H, g.C, g.Kw, g.scale,
                                                                                           alpha ? 1 : 0);
         L.check();
       }))
@@ -565,7 +571,7 @@ void launch_wfft_fwd(Launcher& L, const Geometry& g, const Plan& p, const T* x, 
 
 void launch_hfft(Launcher& L, const Geometry& g, const Plan& p, float2* S, int C, bool inverse) {
   if (L.err != cudaSuccess) return;
-  if (C % 64 == 0 && fft2_dispatch(g.H, [&](auto n1, auto n2) {
+  if (C % 64 == 0 && fft2_dispatch(g.H, [&](auto n1, auto n2, auto) {
         constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value;
         const size_t smem2 = (size_t)g.H * 64 * sizeof(float2);
         L.err = inverse ? set_smem(k_hfft2<N1, N2, +1>, smem2) : set_smem(k_hfft2<N1, N2, -1>, smem2);
@@ -589,13 +595,13 @@ template <typename T>
 void launch_wfft_inv(Launcher& L, const Geometry& g, const Plan& p, const float2* S, const T* res, T* out,
                      bool half_interior) {
   if (L.err != cudaSuccess) return;
-  if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2) {
-        constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value;
+  if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2, auto nw) {
+        constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value, NW = decltype(nw)::value;
         const size_t smem2 = (size_t)g.W * 32 * sizeof(float2);
-        L.err = set_smem(k_wfft_inv2<T, N1, N2>, smem2);
+        L.err = set_smem(k_wfft_inv2<T, N1, N2, NW>, smem2);
         if (L.err != cudaSuccess) return;
         L.begin("k_wfft_inv");
-        k_wfft_inv2<T, N1, N2><<<dim3(g.C / 64, g.H, g.B), 32 * kF2Warps, smem2, L.st>>>(S, res, out, p.fw.tw, g.H, g.C, g.Kw, g.scale,
+        k_wfft_inv2<T, N1, N2, NW><<<dim3(g.C / 64, g.H, g.B), 32 * NW, smem2, L.st>>>(S, res, out, p.fw.tw, g.H, g.C, g.Kw, g.scale,
                                                                                           half_interior ? 1 : 0);
         L.check();
       }))

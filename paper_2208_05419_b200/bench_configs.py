@@ -45,6 +45,8 @@ CONFIGS = {
     "hidden factor 2, 90x180x768 fwd B=4 (hybrid)": (4, 90, 180, 768, 8, 2, 1.0, False, False),
     "hidden factor 2, 90x180x768 fwd+bwd B=4 (hybrid)": (4, 90, 180, 768, 8, 2, 1.0, True, False),
     "fp32 activations 90x180x768 fwd+bwd B=2 (generic)": (2, 90, 180, 768, 8, 1, 1.0, True, False),
+    "p->1 token grid 720x1440x768 fwd B=1 (hybrid)": (1, 720, 1440, 768, 8, 1, 1.0, False, False),
+    "p->1 token grid 720x1440x768 fwd+bwd B=1 (hybrid)": (1, 720, 1440, 768, 8, 1, 1.0, True, False),
 }
 
 

@@ -104,43 +104,45 @@ __device__ __forceinline__ void pass_b(const float2* s, int lw, int l, int k1, f
 }
 
 constexpr int kF2Warps = 8;
+constexpr int kF2MaxBatch = 24;   // rows a thread keeps in flight before its first shared-memory store
 
-// ---- F2 / F7: H-direction complex FFT, in place on S[B][H][Kw][C]; tile = 64 channels of one (b, kw) column ----------
-// grid (C / 64, Kw, B), block 256; smem H * 64 float2
-template <int N1, int N2, int SG>
+// ---- F2 / F7: H-direction complex FFT, in place on S[B][H][Kw][C]; tile = 32 G channels of one (b, kw) column ---------
+// grid (C / (32 G), Kw, B), block 256; smem H * 32 G float2 (G = 2 up to 360 points, 1 beyond: 184 KB at 720)
+template <int N1, int N2, int SG, int G>
 __global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(float2* __restrict__ S, const float2* __restrict__ tw, int Kw, int C) {
-  constexpr int H = N1 * N2;
+  constexpr int H = N1 * N2, LW = 32 * G;
   extern __shared__ float2 smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int kw = blockIdx.y, b = blockIdx.z;
-  float2* base = S + ((size_t)b * H * Kw + kw) * C + (size_t)blockIdx.x * 64;
+  float2* base = S + ((size_t)b * H * Kw + kw) * C + (size_t)blockIdx.x * LW;
   const size_t hstride = (size_t)Kw * C;
-  // a row of the tile is 512 contiguous bytes: one float4 per lane
-  // (every row of the warp is in flight before the first shared-memory store: one latency period per tile)
-  {
-    constexpr int LB = (H + kF2Warps - 1) / kF2Warps;
-    float4 v[LB];
+  // a row of the tile is 256 G contiguous bytes: one float2 (G = 1) or float4 (G = 2) per lane; up to kF2MaxBatch
+  // rows of the warp are in flight before the first shared-memory store
+  typedef typename std::conditional<G == 2, float4, float2>::type vec_t;
+  constexpr int PER = (H + kF2Warps - 1) / kF2Warps, LB = PER < kF2MaxBatch ? PER : kF2MaxBatch;
+  for (int h0 = warp; h0 < H; h0 += kF2Warps * LB) {
+    vec_t v[LB];
 #pragma unroll
     for (int u = 0; u < LB; ++u) {
-      const int h = warp + u * kF2Warps;
-      if (h < H) v[u] = *(const float4*)(base + (size_t)h * hstride + 2 * lane);
+      const int h = h0 + u * kF2Warps;
+      if (h < H) v[u] = *(const vec_t*)(base + (size_t)h * hstride + G * lane);
     }
 #pragma unroll
     for (int u = 0; u < LB; ++u) {
-      const int h = warp + u * kF2Warps;
-      if (h < H) *(float4*)(smem + h * 64 + 2 * lane) = v[u];
+      const int h = h0 + u * kF2Warps;
+      if (h < H) *(vec_t*)(smem + h * LW + G * lane) = v[u];
     }
   }
   __syncthreads();
-  for (int task = warp; task < 2 * N2; task += kF2Warps) {
+  for (int task = warp; task < G * N2; task += kF2Warps) {
     const int g = task / N2, n2 = task - g * N2;
-    pass_a<N1, N2, SG>(smem, 64, g * 32 + lane, n2, tw);
+    pass_a<N1, N2, SG>(smem, LW, g * 32 + lane, n2, tw);
   }
   __syncthreads();
-  for (int task = warp; task < 2 * N1; task += kF2Warps) {
+  for (int task = warp; task < G * N1; task += kF2Warps) {
     const int g = task / N1, k1 = task - g * N1;
     float2 v[N2];
-    pass_b<N1, N2, SG>(smem, 64, g * 32 + lane, k1, v);
+    pass_b<N1, N2, SG>(smem, LW, g * 32 + lane, k1, v);
     float2* dst = base + g * 32 + lane;
 #pragma unroll
     for (int k2 = 0; k2 < N2; ++k2) dst[(size_t)(k1 + N1 * k2) * hstride] = v[k2];
@@ -148,36 +150,40 @@ __global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(float2* __restrict__ S,
 }
 
 // ---- F1 / B2: W-direction real FFT, two real channels packed into one complex transform ---------------------------------
-// grid (C / 64, H, B), block 256; smem W * 32 float2.  Pass B runs the tasks k1 and N1 - k1 together: the Hermitian
-// split of bin k needs Z[k] and Z[W - k], which live in exactly those two tasks, so the half-spectrum leaves from
-// registers.
-template <typename T, int N1, int N2, int NW>
-__global__ void __launch_bounds__(32 * NW, 2)
+// grid (C / (2 LW), H, B), block 32 NW; smem W * LW float2.  LW = 32 packed channels per row (one task per warp
+// iteration) up to 360 points; LW = 16 beyond (184 KB at 1,440 points): a warp then runs two tasks side by side, one
+// per half-warp.  Pass B runs the tasks k1 and N1 - k1 together: the Hermitian split of bin k needs Z[k] and Z[W - k],
+// which live in exactly those two tasks, so the half-spectrum leaves from registers.
+template <typename T, int N1, int N2, int NW, int LW>
+__global__ void __launch_bounds__(32 * NW, LW == 32 ? 2 : 1)
 k_wfft_fwd2(const T* __restrict__ x, float2* __restrict__ S, const float2* __restrict__ tw, int H, int C, int Kw, float scale,
             int alpha_weight) {
-  constexpr int W = N1 * N2;
+  constexpr int W = N1 * N2, TPW = 32 / LW, NSLOT = NW * TPW;
   extern __shared__ float2 smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int l = lane % LW, slot = warp * TPW + lane / LW;
   const int h = blockIdx.y, b = blockIdx.z;
-  const int c = blockIdx.x * 64 + 2 * lane;
+  const int c = blockIdx.x * (2 * LW) + 2 * l;
   const T* xrow = x + ((size_t)(b * H + h) * W) * C + c;
   {
-    // all rows of the warp in flight at once, kept in the storage type (bf16 pairs: one register each)
-    constexpr int LB = (W + NW - 1) / NW;
-    typename ActIO<T>::raw2 v[LB];
+    // rows in flight kept in the storage type (bf16 pairs: one register each)
+    constexpr int PER = (W + NSLOT - 1) / NSLOT, LB = PER < 2 * kF2MaxBatch ? PER : 2 * kF2MaxBatch;
+    for (int w0 = slot; w0 < W; w0 += NSLOT * LB) {
+      typename ActIO<T>::raw2 v[LB];
 #pragma unroll
-    for (int u = 0; u < LB; ++u) {
-      const int w = warp + u * NW;
-      if (w < W) v[u] = ActIO<T>::ldraw2(xrow + (size_t)w * C);
-    }
+      for (int u = 0; u < LB; ++u) {
+        const int w = w0 + u * NSLOT;
+        if (w < W) v[u] = ActIO<T>::ldraw2(xrow + (size_t)w * C);
+      }
 #pragma unroll
-    for (int u = 0; u < LB; ++u) {
-      const int w = warp + u * NW;
-      if (w < W) smem[w * 32 + lane] = ActIO<T>::unraw2(v[u]);   // channel c in the real part, channel c + 1 in the imaginary part
+      for (int u = 0; u < LB; ++u) {
+        const int w = w0 + u * NSLOT;
+        if (w < W) smem[w * LW + l] = ActIO<T>::unraw2(v[u]);   // channel c in the real part, channel c + 1 in the imaginary part
+      }
     }
   }
   __syncthreads();
-  for (int n2 = warp; n2 < N2; n2 += NW) pass_a<N1, N2, -1>(smem, 32, lane, n2, tw);
+  for (int n2 = slot; n2 < N2; n2 += NSLOT) pass_a<N1, N2, -1>(smem, LW, l, n2, tw);
   __syncthreads();
   float2* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
   // bin k from Z[k] = zk and Z[W - k] = zn (both channels of the pair)
@@ -189,10 +195,10 @@ k_wfft_fwd2(const T* __restrict__ x, float2* __restrict__ S, const float2* __res
   };
   // work items: k1 = 0 alone, k1 = N1 / 2 alone (N1 even), pairs (k1, N1 - k1)
   constexpr int kItems = N1 / 2 + 1;
-  for (int item = warp; item < kItems; item += NW) {
+  for (int item = slot; item < kItems; item += NSLOT) {
     const int ka = item, kb = (N1 - item) % N1;
     float2 va[N2];
-    pass_b<N1, N2, -1>(smem, 32, lane, ka, va);
+    pass_b<N1, N2, -1>(smem, LW, l, ka, va);
     if (ka == kb) {
       if (ka == 0) {
         // k = N1 k2, W - k = N1 (N2 - k2)
@@ -205,7 +211,7 @@ k_wfft_fwd2(const T* __restrict__ x, float2* __restrict__ S, const float2* __res
       }
     } else {
       float2 vb[N2];
-      pass_b<N1, N2, -1>(smem, 32, lane, kb, vb);
+      pass_b<N1, N2, -1>(smem, LW, l, kb, vb);
 #pragma unroll
       for (int k2 = 0; k2 < N2; ++k2) {
         emit(ka + N1 * k2, va[k2], vb[N2 - 1 - k2]);
@@ -216,66 +222,76 @@ k_wfft_fwd2(const T* __restrict__ x, float2* __restrict__ S, const float2* __res
 }
 
 // ---- F8 + F9 / B8: W-direction complex-to-real inverse FFT, residual, store ------------------------------------------
-// grid (C / 64, H, B), block 256; smem W * 32 float2
-template <typename T, int N1, int N2, int NW>
-__global__ void __launch_bounds__(32 * NW, 2)
+// grid (C / (2 LW), H, B), block 32 NW; smem W * LW float2
+template <typename T, int N1, int N2, int NW, int LW>
+__global__ void __launch_bounds__(32 * NW, LW == 32 ? 2 : 1)
 k_wfft_inv2(const float2* __restrict__ S, const T* __restrict__ res, T* __restrict__ out, const float2* __restrict__ tw, int H,
             int C, int Kw, float scale, int half_interior) {
-  constexpr int W = N1 * N2;
+  constexpr int W = N1 * N2, TPW = 32 / LW, NSLOT = NW * TPW;
   extern __shared__ float2 smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int l = lane % LW, slot = warp * TPW + lane / LW;
   const int h = blockIdx.y, b = blockIdx.z;
-  const int c = blockIdx.x * 64 + 2 * lane;
+  const int c = blockIdx.x * (2 * LW) + 2 * l;
   const float2* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
   // every stored bin kk <= W/2 feeds the transform twice: as z[kk] and, conjugated (Hermitian extension), as z[W - kk]
   {
-    constexpr int LB = (W / 2 + NW) / NW;
-    float4 t[LB];
+    constexpr int PER = (W / 2 + NSLOT) / NSLOT, LB = PER < kF2MaxBatch ? PER : kF2MaxBatch;
+    for (int k0 = slot; k0 <= W / 2; k0 += NSLOT * LB) {
+      float4 t[LB];
 #pragma unroll
-    for (int u = 0; u < LB; ++u) {
-      const int kk = warp + u * NW;
-      t[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (kk < Kw) t[u] = __ldg((const float4*)(Srow + (size_t)kk * C));
-    }
-#pragma unroll
-    for (int u = 0; u < LB; ++u) {
-      const int kk = warp + u * NW;
-      if (kk > W / 2) continue;
-      float2 ta = make_float2(t[u].x, t[u].y), tb = make_float2(t[u].z, t[u].w);
-      if (kk == 0 || 2 * kk == W) {
-        ta.y = 0.f;   // reading A4: imaginary parts of the c = 0 and c = W/2 columns are discarded
-        tb.y = 0.f;
-      } else if (half_interior) {
-        ta.x *= 0.5f; ta.y *= 0.5f; tb.x *= 0.5f; tb.y *= 0.5f;
+      for (int u = 0; u < LB; ++u) {
+        const int kk = k0 + u * NSLOT;
+        t[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (kk < Kw) t[u] = __ldg((const float4*)(Srow + (size_t)kk * C));
       }
-      // Ta + i Tb: channel c -> Re, channel c + 1 -> Im
-      smem[kk * 32 + lane] = make_float2(ta.x - tb.y, ta.y + tb.x);
-      if (kk != 0 && 2 * kk != W) smem[(W - kk) * 32 + lane] = make_float2(ta.x + tb.y, -ta.y + tb.x);   // conj(Ta) + i conj(Tb)
+#pragma unroll
+      for (int u = 0; u < LB; ++u) {
+        const int kk = k0 + u * NSLOT;
+        if (kk > W / 2) continue;
+        float2 ta = make_float2(t[u].x, t[u].y), tb = make_float2(t[u].z, t[u].w);
+        if (kk == 0 || 2 * kk == W) {
+          ta.y = 0.f;   // reading A4: imaginary parts of the c = 0 and c = W/2 columns are discarded
+          tb.y = 0.f;
+        } else if (half_interior) {
+          ta.x *= 0.5f; ta.y *= 0.5f; tb.x *= 0.5f; tb.y *= 0.5f;
+        }
+        // Ta + i Tb: channel c -> Re, channel c + 1 -> Im
+        smem[kk * LW + l] = make_float2(ta.x - tb.y, ta.y + tb.x);
+        if (kk != 0 && 2 * kk != W) smem[(W - kk) * LW + l] = make_float2(ta.x + tb.y, -ta.y + tb.x);   // conj(Ta) + i conj(Tb)
+      }
     }
   }
   __syncthreads();
-  for (int n2 = warp; n2 < N2; n2 += NW) pass_a<N1, N2, +1>(smem, 32, lane, n2, tw);
+  for (int n2 = slot; n2 < N2; n2 += NSLOT) pass_a<N1, N2, +1>(smem, LW, l, n2, tw);
   __syncthreads();
   const size_t rowoff = ((size_t)(b * H + h) * W) * C + c;
-  for (int k1 = warp; k1 < N1; k1 += NW) {
-    float2 r[N2];
+  for (int k1 = slot; k1 < N1; k1 += NSLOT) {
+    typename ActIO<T>::raw2 r[N2];
 #pragma unroll
     for (int k2 = 0; k2 < N2; ++k2)
-      r[k2] = res ? ActIO<T>::ld2(res + rowoff + (size_t)(k1 + N1 * k2) * C) : make_float2(0.f, 0.f);
+      if (res) r[k2] = ActIO<T>::ldraw2(res + rowoff + (size_t)(k1 + N1 * k2) * C);
     float2 v[N2];
-    pass_b<N1, N2, +1>(smem, 32, lane, k1, v);
+    pass_b<N1, N2, +1>(smem, LW, l, k1, v);
 #pragma unroll
-    for (int k2 = 0; k2 < N2; ++k2)
-      ActIO<T>::st2(out + rowoff + (size_t)(k1 + N1 * k2) * C, scale * v[k2].x + r[k2].x, scale * v[k2].y + r[k2].y);
+    for (int k2 = 0; k2 < N2; ++k2) {
+      const float2 rr = res ? ActIO<T>::unraw2(r[k2]) : make_float2(0.f, 0.f);
+      ActIO<T>::st2(out + rowoff + (size_t)(k1 + N1 * k2) * C, scale * v[k2].x + rr.x, scale * v[k2].y + rr.y);
+    }
   }
 }
 
-// size table: N -> (N1, N2) and the warps per block of the W-direction kernels (pass A has N2 tasks, pass B N1 / 2 + 1
-// paired items forward, N1 tasks inverse)
+// size table: N -> (N1, N2), the warps per block of the W-direction kernels (pass A has N2 tasks, pass B N1 / 2 + 1 paired
+// items forward, N1 tasks inverse) and whether the tile is narrow (720 / 1,440 points: 32 channels per H tile, 16 packed
+// lanes per W tile, so that one row or column still fits shared memory)
 template <typename F>
 bool fft2_dispatch(int n, F&& f) {
-  if (n == 90) { f(std::integral_constant<int, 9>{}, std::integral_constant<int, 10>{}, std::integral_constant<int, 5>{}); return true; }
-  if (n == 180) { f(std::integral_constant<int, 12>{}, std::integral_constant<int, 15>{}, std::integral_constant<int, 8>{}); return true; }
-  if (n == 360) { f(std::integral_constant<int, 18>{}, std::integral_constant<int, 20>{}, std::integral_constant<int, 10>{}); return true; }
+  using std::integral_constant;
+  if (n == 90) { f(integral_constant<int, 9>{}, integral_constant<int, 10>{}, integral_constant<int, 5>{}, integral_constant<int, 0>{}); return true; }
+  if (n == 180) { f(integral_constant<int, 12>{}, integral_constant<int, 15>{}, integral_constant<int, 8>{}, integral_constant<int, 0>{}); return true; }
+  if (n == 360) { f(integral_constant<int, 18>{}, integral_constant<int, 20>{}, integral_constant<int, 10>{}, integral_constant<int, 0>{}); return true; }
+  if (n == 720) { f(integral_constant<int, 24>{}, integral_constant<int, 30>{}, integral_constant<int, 8>{}, integral_constant<int, 1>{}); return true; }
+  if (n == 1440) { f(integral_constant<int, 36>{}, integral_constant<int, 40>{}, integral_constant<int, 10>{}, integral_constant<int, 1>{}); return true; }
   return false;
 }
+inline bool fft2_has(int n) { return n == 90 || n == 180 || n == 360 || n == 720 || n == 1440; }

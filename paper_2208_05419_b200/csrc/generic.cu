@@ -549,14 +549,15 @@ cudaError_t set_smem(K kernel, size_t bytes) {
 template <typename T>
 void launch_wfft_fwd(Launcher& L, const Geometry& g, const Plan& p, const T* x, float2* S, bool alpha) {
   if (L.err != cudaSuccess) return;
-  if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2, auto nw) {
+  if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2, auto nw, auto narrow) {
         constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value, NW = decltype(nw)::value;
-        const size_t smem2 = (size_t)g.W * 32 * sizeof(float2);
-        L.err = set_smem(k_wfft_fwd2<T, N1, N2, NW>, smem2);
+        constexpr int LW = decltype(narrow)::value ? 16 : 32;
+        const size_t smem2 = (size_t)g.W * LW * sizeof(float2);
+        L.err = set_smem(k_wfft_fwd2<T, N1, N2, NW, LW>, smem2);
         if (L.err != cudaSuccess) return;
         L.begin("k_wfft_fwd");
-        k_wfft_fwd2<T, N1, N2, NW><<<dim3(g.C / 64, g.H, g.B), 32 * NW, smem2, L.st>>>(x, S, p.fw.tw, g.H, g.C, g.Kw, g.scale,
-                                                                                          alpha ? 1 : 0);
+        k_wfft_fwd2<T, N1, N2, NW, LW><<<dim3(g.C / (2 * LW), g.H, g.B), 32 * NW, smem2, L.st>>>(x, S, p.fw.tw, g.H, g.C, g.Kw,
+                                                                                                g.scale, alpha ? 1 : 0);
         L.check();
       }))
     return;
@@ -571,14 +572,15 @@ void launch_wfft_fwd(Launcher& L, const Geometry& g, const Plan& p, const T* x, 
 
 void launch_hfft(Launcher& L, const Geometry& g, const Plan& p, float2* S, int C, bool inverse) {
   if (L.err != cudaSuccess) return;
-  if (C % 64 == 0 && fft2_dispatch(g.H, [&](auto n1, auto n2, auto) {
-        constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value;
-        const size_t smem2 = (size_t)g.H * 64 * sizeof(float2);
-        L.err = inverse ? set_smem(k_hfft2<N1, N2, +1>, smem2) : set_smem(k_hfft2<N1, N2, -1>, smem2);
+  if (C % 64 == 0 && fft2_dispatch(g.H, [&](auto n1, auto n2, auto, auto narrow) {
+        constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value, G = decltype(narrow)::value ? 1 : 2;
+        const size_t smem2 = (size_t)g.H * 32 * G * sizeof(float2);
+        L.err = inverse ? set_smem(k_hfft2<N1, N2, +1, G>, smem2) : set_smem(k_hfft2<N1, N2, -1, G>, smem2);
         if (L.err != cudaSuccess) return;
         L.begin("k_hfft");
-        if (inverse) k_hfft2<N1, N2, +1><<<dim3(C / 64, g.Kw, g.B), 32 * kF2Warps, smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
-        else k_hfft2<N1, N2, -1><<<dim3(C / 64, g.Kw, g.B), 32 * kF2Warps, smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
+        const dim3 grid(C / (32 * G), g.Kw, g.B);
+        if (inverse) k_hfft2<N1, N2, +1, G><<<grid, 32 * kF2Warps, smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
+        else k_hfft2<N1, N2, -1, G><<<grid, 32 * kF2Warps, smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
         L.check();
       }))
     return;
@@ -595,14 +597,15 @@ template <typename T>
 void launch_wfft_inv(Launcher& L, const Geometry& g, const Plan& p, const float2* S, const T* res, T* out,
                      bool half_interior) {
   if (L.err != cudaSuccess) return;
-  if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2, auto nw) {
+  if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2, auto nw, auto narrow) {
         constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value, NW = decltype(nw)::value;
-        const size_t smem2 = (size_t)g.W * 32 * sizeof(float2);
-        L.err = set_smem(k_wfft_inv2<T, N1, N2, NW>, smem2);
+        constexpr int LW = decltype(narrow)::value ? 16 : 32;
+        const size_t smem2 = (size_t)g.W * LW * sizeof(float2);
+        L.err = set_smem(k_wfft_inv2<T, N1, N2, NW, LW>, smem2);
         if (L.err != cudaSuccess) return;
         L.begin("k_wfft_inv");
-        k_wfft_inv2<T, N1, N2, NW><<<dim3(g.C / 64, g.H, g.B), 32 * NW, smem2, L.st>>>(S, res, out, p.fw.tw, g.H, g.C, g.Kw, g.scale,
-                                                                                          half_interior ? 1 : 0);
+        k_wfft_inv2<T, N1, N2, NW, LW><<<dim3(g.C / (2 * LW), g.H, g.B), 32 * NW, smem2, L.st>>>(S, res, out, p.fw.tw, g.H, g.C, g.Kw,
+                                                                                                g.scale, half_interior ? 1 : 0);
         L.check();
       }))
     return;
@@ -811,8 +814,10 @@ cudaError_t backward_t(const Geometry& g, const Plan& p, const T* x, const T* dy
 
 bool generic_supported(const Geometry& g, const char** why) {
   const size_t lim = 227 * 1024;
-  if ((size_t)g.W * kLanes * sizeof(float2) > lim || (size_t)g.H * kLanes * sizeof(float2) > lim) {
-    *why = "H or W too large for the single-pass shared-memory FFT (max 908)";
+  const bool w_ok = (size_t)g.W * kLanes * sizeof(float2) <= lim || (fft2_has(g.W) && g.C % 64 == 0);
+  const bool h_ok = (size_t)g.H * kLanes * sizeof(float2) <= lim || (fft2_has(g.H) && g.C % 64 == 0);
+  if (!w_ok || !h_ok) {
+    *why = "H or W too large for the shared-memory FFT kernels (max 908; 1,440 with C a multiple of 64)";
     return false;
   }
   const int kmax = g.hid > g.bs ? g.hid : g.bs;

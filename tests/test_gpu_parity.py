@@ -824,3 +824,29 @@ def test_data_parallel_step_with_gradient_bucket(oracle):
     assert np.array_equal(parity.from_device_act(ty), ref["y"]) and np.array_equal(parity.from_device_act(tdx), ref["dx"])
     for v, k in zip(bucket.views, ("dw1", "db1", "dw2", "db2")):
         assert np.array_equal(v.cpu().numpy(), ref[k]), k
+
+
+def test_p1_token_grid_fp32_forward(oracle):
+    """SURVEY.md S8(f) item 1, last clause: the p -> 1 token grid (720 x 1,440 tokens).  One row of 1,440 points
+    no longer fits shared memory at 32 packed channels; the two-pass register FFT kernels run it with 16 packed lanes per
+    W tile and 32 channels per H tile (fft2pass.cuh).  fp32 path, forward, against the oracle per tile."""
+    rng = np.random.default_rng(1440)
+    B, H, W, C, nb = 1, 720, 1440, 64, 2
+    bs = C // nb
+    data = dict(x=rng.standard_normal((B, H, W, C)).astype(np.float32))
+    data["w1"], data["b1"], data["w2"], data["b2"] = [
+        (0.2 * rng.standard_normal(s)).astype(np.float32) for s in [(nb, bs, bs, 2), (nb, bs, 2), (nb, bs, bs, 2), (nb, bs, 2)]]
+    desc = binding.Desc(B, H, W, C, nb, 1, 0.01, 1.0, binding.AFNO_F32)
+    assert binding.afno_spectral_path(desc) == "generic-fp32"
+    _check_forward(oracle, desc, data, label="720x1440x64 fp32")
+
+
+def test_p1_token_grid_bf16_hybrid(oracle):
+    """The same grid with bf16 activations on the hybrid path (32-wide blocks, partly filled last group), forward and
+    backward, mask-consistently against the oracle."""
+    wl = inputs.Workload(5, "720x1440x128 nb=4 bf16 B=1", 1, 720, 1440, 128, 4, 1, 0.01, 1.0, "bf16", True, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert binding.afno_spectral_path(desc) == "hybrid-fft32-tcgen05"
+    _check_forward(oracle, desc, data, label=wl.name)
+    _check_backward(oracle, desc, data, label=wl.name)

@@ -394,16 +394,15 @@ def run_ours(args):
         hp = [pin(p) for p in params]
         hy, hdx = torch.empty_like(hx).pin_memory(), torch.empty_like(hx).pin_memory()
         hg = [torch.empty_like(p).pin_memory() for p in hp]
-        arena = torch.empty(max(binding.afno_spectral_host_arena_bytes(desc, False),
-                                binding.afno_spectral_host_arena_bytes(desc, True)), dtype=torch.uint8, device=dev)
+        arena = torch.empty(binding.afno_spectral_host_arena_bytes(desc, 2), dtype=torch.uint8, device=dev)
         act = hx.numel() * 2
         pbytes = sum(p.numel() * 4 for p in hp)
         E2E_STEPS = max(1, min(args.steps, 5))
 
         def host_step():
-            binding.afno_spectral_fwd_host(desc, hx, *hp, hy, arena, stream)
-            # x is already in the arena (left there by fwd_host): the step uploads it once
-            binding.afno_spectral_bwd_host(desc, None, hdy, *hp, hdx, *hg, arena, stream)
+            # one call per training step: x and dy in, y, dx and the parameter gradients out, the two directions of the
+            # link busy across the forward / backward boundary (x is uploaded once)
+            binding.afno_spectral_step_host(desc, hx, hdy, *hp, hy, hdx, *hg, arena, stream)
 
         host_step()
         barrier()
@@ -414,7 +413,7 @@ def run_ours(args):
         dt = max_over_ranks(time.perf_counter() - t0, dist, dev)
         e2e = {"value": whole_job_value(world, B, E2E_STEPS, dt * 1e3), "unit": UNIT,
                "h2d_bytes_per_step": 2 * act + 2 * pbytes, "d2h_bytes_per_step": 2 * act + pbytes,
-               "steps": E2E_STEPS, "note": "afno_spectral_fwd_host + afno_spectral_bwd_host (x uploaded once), pinned host buffers, wall clock"}
+               "steps": E2E_STEPS, "note": "afno_spectral_step_host (one C-ABI call per step: fwd + bwd from pinned host buffers, x uploaded once, results back on the host), wall clock"}
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.timed_only:

@@ -145,7 +145,7 @@ int afno_spectral_bwd(const afno_desc_t* d, const void* x, const void* dy, const
  * afno_spectral_fwd_host call that preceded it on the SAME arena and descriptor left it (a
  * training step uploads x once).  On an error the calls first wait for the copies and
  * kernels they have already enqueued, so the caller may free its buffers at once. */
-size_t afno_spectral_host_arena_bytes(const afno_desc_t* d, int for_backward);
+size_t afno_spectral_host_arena_bytes(const afno_desc_t* d, int for_backward); /* 0 fwd_host, 1 bwd_host, 2 step_host */
 int afno_spectral_fwd_host(const afno_desc_t* d, const void* x_host, const float* w1_host,
                            const float* b1_host, const float* w2_host, const float* b2_host,
                            void* y_host, void* arena, size_t arena_bytes, void* cuda_stream);
@@ -154,6 +154,17 @@ int afno_spectral_bwd_host(const afno_desc_t* d, const void* x_host, const void*
                            const float* b2_host, void* dx_host, float* dw1_host,
                            float* db1_host, float* dw2_host, float* db2_host, void* arena,
                            size_t arena_bytes, void* cuda_stream);
+
+/* A whole training step from HOST buffers in one call: y = fwd(x); dx, dw*, db* = bwd(x, dy) (rows F1-F9, B1-B8).
+ * Per sample x and dy travel host->device back to back, the forward (which saves its context) and the backward
+ * (which uses it) run as soon as their input has landed, y and dx travel device->host meanwhile: both directions of
+ * the link stay busy across the forward / backward boundary.  Results equal afno_spectral_fwd_host followed by
+ * afno_spectral_bwd_host bit for bit.  `arena`: at least afno_spectral_host_arena_bytes(d, 2) bytes. */
+int afno_spectral_step_host(const afno_desc_t* d, const void* x_host, const void* dy_host,
+                            const float* w1_host, const float* b1_host, const float* w2_host,
+                            const float* b2_host, void* y_host, void* dx_host, float* dw1_host,
+                            float* db1_host, float* dw2_host, float* db2_host, void* arena,
+                            size_t arena_bytes, void* cuda_stream);
 
 /* Number of kernel launches the last fwd / bwd call of this thread enqueued (bench.py's
  * "gpu_launches" is counted from this, not guessed). */

@@ -23,7 +23,7 @@ EXPORTS = [
     "afno_version", "afno_status_string", "afno_last_error", "afno_spectral_path",
     "afno_spectral_workspace_bytes", "afno_spectral_mask_bytes", "afno_plan_warmup",
     "afno_spectral_fwd", "afno_spectral_bwd", "afno_spectral_host_arena_bytes",
-    "afno_spectral_fwd_host", "afno_spectral_bwd_host", "afno_last_launch_count",
+    "afno_spectral_fwd_host", "afno_spectral_bwd_host", "afno_spectral_step_host", "afno_last_launch_count",
     "afno_profile_start", "afno_profile_stop", "afno_plan_destroy_all",
 ]
 
@@ -78,6 +78,8 @@ def lib():
         L.afno_spectral_fwd_host.argtypes = [dp] + [vp] * 7 + [sz, vp]
         L.afno_spectral_bwd_host.restype = ctypes.c_int
         L.afno_spectral_bwd_host.argtypes = [dp] + [vp] * 12 + [sz, vp]
+        L.afno_spectral_step_host.restype = ctypes.c_int
+        L.afno_spectral_step_host.argtypes = [dp] + [vp] * 13 + [sz, vp]
         L.afno_last_launch_count.restype = ctypes.c_int
         L.afno_plan_destroy_all.restype = ctypes.c_int
         L.afno_profile_start.restype = ctypes.c_int
@@ -157,7 +159,7 @@ def afno_spectral_workspace_bytes(d: Desc, for_backward: bool) -> int:
     return int(lib().afno_spectral_workspace_bytes(ctypes.byref(cd), int(for_backward)))
 
 
-def afno_spectral_host_arena_bytes(d: Desc, for_backward: bool) -> int:
+def afno_spectral_host_arena_bytes(d: Desc, for_backward) -> int:
     cd = d.c()
     return int(lib().afno_spectral_host_arena_bytes(ctypes.byref(cd), int(for_backward)))
 
@@ -227,3 +229,12 @@ def afno_spectral_bwd_host(d: Desc, x, dy, w1, b1, w2, b2, dx, dw1, db1, dw2, db
     _check(lib().afno_spectral_bwd_host(ctypes.byref(cd), _ptr(x), _ptr(dy), _ptr(w1), _ptr(b1), _ptr(w2),
                                         _ptr(b2), _ptr(dx), _ptr(dw1), _ptr(db1), _ptr(dw2), _ptr(db2),
                                         _ptr(arena), _ws_bytes(arena), _stream_handle(stream)))
+
+
+def afno_spectral_step_host(d: Desc, x, dy, w1, b1, w2, b2, y, dx, dw1, db1, dw2, db2, arena, stream=None):
+    """One training step from HOST tensors/arrays (pinned recommended); arena: device tensor of
+    afno_spectral_host_arena_bytes(d, 2) bytes."""
+    cd = d.c()
+    _check(lib().afno_spectral_step_host(ctypes.byref(cd), _ptr(x), _ptr(dy), _ptr(w1), _ptr(b1), _ptr(w2), _ptr(b2),
+                                         _ptr(y), _ptr(dx), _ptr(dw1), _ptr(db1), _ptr(dw2), _ptr(db2),
+                                         _ptr(arena), _ws_bytes(arena), _stream_handle(stream)))

@@ -398,7 +398,8 @@ struct HostLayout {
   void* ws;
   size_t ws_bytes, total, act, nw, nb1, nb2;
 };
-HostLayout host_layout(const afno_desc_t* d, const Geometry& g, bool backward, char* base) {
+HostLayout host_layout(const afno_desc_t* d, const Geometry& g, int mode, char* base) {
+  const bool backward = mode != 0;
   HostLayout h{};
   Arena a{base};
   h.act = act_bytes(g);
@@ -417,9 +418,8 @@ HostLayout host_layout(const afno_desc_t* d, const Geometry& g, bool backward, c
     h.db1 = (float*)a.take(h.nb1);
     h.dw2 = (float*)a.take(h.nw);
     h.db2 = (float*)a.take(h.nb2);
-  } else {
-    h.y = a.take(h.act);
   }
+  if (mode != 1) h.y = a.take(h.act);
   h.ws_bytes = afno_spectral_workspace_bytes(d, backward ? 1 : 0);
   h.ws = a.take(h.ws_bytes);
   h.total = a.off;
@@ -430,7 +430,7 @@ HostLayout host_layout(const afno_desc_t* d, const Geometry& g, bool backward, c
 size_t afno_spectral_host_arena_bytes(const afno_desc_t* d, int for_backward) {
   Geometry g;
   if (resolve(d, &g) != AFNO_OK) return 0;
-  return host_layout(d, g, for_backward != 0, nullptr).total;
+  return host_layout(d, g, for_backward == 2 ? 2 : (for_backward != 0 ? 1 : 0), nullptr).total;
 }
 
 #define AFNO_CUDA_TRY(expr)                                                                     \
@@ -517,7 +517,7 @@ int afno_spectral_fwd_host(const afno_desc_t* d, const void* x_host, const float
   if (!x_host || !w1_host || !b1_host || !w2_host || !b2_host || !y_host || !arena)
     return fail(AFNO_ERR_INVALID_ARG, "NULL pointer argument");
   if (!aligned16(arena)) return fail(AFNO_ERR_INVALID_ARG, "arena must be 16-byte aligned");
-  HostLayout h = host_layout(d, g, false, (char*)arena);
+  HostLayout h = host_layout(d, g, 0, (char*)arena);
   if (arena_bytes < h.total) return fail(AFNO_ERR_WORKSPACE, "arena smaller than afno_spectral_host_arena_bytes(d, 0)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   HostPipe* hp = nullptr;
@@ -566,7 +566,7 @@ int afno_spectral_bwd_host(const afno_desc_t* d, const void* x_host, const void*
   if (d->flags & AFNO_FLAG_EXPORT_MASKS)
     return fail(AFNO_ERR_INVALID_ARG, "AFNO_FLAG_EXPORT_MASKS is not meaningful for the host variant");
   if (!aligned16(arena)) return fail(AFNO_ERR_INVALID_ARG, "arena must be 16-byte aligned");
-  HostLayout h = host_layout(d, g, true, (char*)arena);
+  HostLayout h = host_layout(d, g, 1, (char*)arena);
   if (arena_bytes < h.total) return fail(AFNO_ERR_WORKSPACE, "arena smaller than afno_spectral_host_arena_bytes(d, 1)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
   HostPipe* hp = nullptr;
@@ -588,6 +588,71 @@ int afno_spectral_bwd_host(const afno_desc_t* d, const void* x_host, const void*
     AFNO_PIPE_TRY(hp->mark(hp->h2d, st));
     d1.flags = b == 0 ? (d1.flags & ~(uint32_t)AFNO_FLAG_ACCUM_GRADS) : (d1.flags | AFNO_FLAG_ACCUM_GRADS);
     rc = afno_spectral_bwd(&d1, (char*)h.x + off, (char*)h.dy + off, h.w1, h.b1, h.w2, h.b2, (char*)h.dx + off, h.dw1, h.db1,
+                           h.dw2, h.db2, h.ws, h.ws_bytes, cuda_stream);
+    if (rc != AFNO_OK) {
+      hp->drain(st);
+      return rc;
+    }
+    AFNO_PIPE_TRY(hp->mark(st, hp->d2h));
+    AFNO_PIPE_TRY(cudaMemcpyAsync((char*)dx_host + off, (char*)h.dx + off, sample, cudaMemcpyDeviceToHost, hp->d2h));
+  }
+  AFNO_PIPE_TRY(cudaMemcpyAsync(dw1_host, h.dw1, h.nw, cudaMemcpyDeviceToHost, hp->d2h));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(db1_host, h.db1, h.nb1, cudaMemcpyDeviceToHost, hp->d2h));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(dw2_host, h.dw2, h.nw, cudaMemcpyDeviceToHost, hp->d2h));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(db2_host, h.db2, h.nb2, cudaMemcpyDeviceToHost, hp->d2h));
+  AFNO_PIPE_TRY(cudaStreamSynchronize(hp->d2h));
+  AFNO_PIPE_TRY(cudaStreamSynchronize(st));
+  return AFNO_OK;
+}
+
+// One training step from host buffers: per sample x and dy travel host->device back to back on one copy stream, the
+// forward (saving its context) and the backward (using it) run on the caller's stream as soon as their input has
+// landed, y and dx travel device->host on the second copy stream: the two directions of the link stay busy across
+// the forward / backward boundary, which the two separate calls cannot do (each synchronises before it returns).
+int afno_spectral_step_host(const afno_desc_t* d, const void* x_host, const void* dy_host, const float* w1_host,
+                            const float* b1_host, const float* w2_host, const float* b2_host, void* y_host,
+                            void* dx_host, float* dw1_host, float* db1_host, float* dw2_host, float* db2_host,
+                            void* arena, size_t arena_bytes, void* cuda_stream) {
+  Geometry g;
+  int rc = resolve(d, &g);
+  if (rc != AFNO_OK) return rc;
+  if (!x_host || !dy_host || !w1_host || !b1_host || !w2_host || !b2_host || !y_host || !dx_host || !dw1_host ||
+      !db1_host || !dw2_host || !db2_host || !arena)
+    return fail(AFNO_ERR_INVALID_ARG, "NULL pointer argument");
+  if (d->flags & (AFNO_FLAG_ACCUM_GRADS | AFNO_FLAG_EXPORT_MASKS))
+    return fail(AFNO_ERR_INVALID_ARG, "AFNO_FLAG_ACCUM_GRADS / AFNO_FLAG_EXPORT_MASKS are not meaningful for the host variant");
+  if (!aligned16(arena)) return fail(AFNO_ERR_INVALID_ARG, "arena must be 16-byte aligned");
+  afno_desc_t d1 = *d;
+  d1.B = 1;
+  d1.flags &= ~(uint32_t)(AFNO_FLAG_SAVE_CONTEXT | AFNO_FLAG_USE_CONTEXT);
+  HostLayout h = host_layout(d, g, 2, (char*)arena);
+  if (arena_bytes < h.total) return fail(AFNO_ERR_WORKSPACE, "arena smaller than afno_spectral_host_arena_bytes(d, 2)");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  HostPipe* hp = nullptr;
+  AFNO_CUDA_TRY(host_pipe(&hp));
+  afno_desc_t df = d1, db = d1;
+  df.flags |= AFNO_FLAG_SAVE_CONTEXT;
+  const size_t sample = h.act / (size_t)g.B;
+  AFNO_PIPE_TRY(hp->mark(st, hp->h2d));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.w1, w1_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.b1, b1_host, h.nb1, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.w2, w2_host, h.nw, cudaMemcpyHostToDevice, hp->h2d));
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.b2, b2_host, h.nb2, cudaMemcpyHostToDevice, hp->h2d));
+  for (int b = 0; b < g.B; ++b) {
+    const size_t off = (size_t)b * sample;
+    AFNO_PIPE_TRY(cudaMemcpyAsync((char*)h.x + off, (const char*)x_host + off, sample, cudaMemcpyHostToDevice, hp->h2d));
+    AFNO_PIPE_TRY(hp->mark(hp->h2d, st));
+    rc = afno_spectral_fwd(&df, (char*)h.x + off, h.w1, h.b1, h.w2, h.b2, (char*)h.y + off, h.ws, h.ws_bytes, cuda_stream);
+    if (rc != AFNO_OK) {
+      hp->drain(st);
+      return rc;
+    }
+    AFNO_PIPE_TRY(hp->mark(st, hp->d2h));
+    AFNO_PIPE_TRY(cudaMemcpyAsync((char*)y_host + off, (char*)h.y + off, sample, cudaMemcpyDeviceToHost, hp->d2h));
+    AFNO_PIPE_TRY(cudaMemcpyAsync((char*)h.dy + off, (const char*)dy_host + off, sample, cudaMemcpyHostToDevice, hp->h2d));
+    AFNO_PIPE_TRY(hp->mark(hp->h2d, st));
+    db.flags = (d1.flags | AFNO_FLAG_USE_CONTEXT) | (b == 0 ? 0u : (uint32_t)AFNO_FLAG_ACCUM_GRADS);
+    rc = afno_spectral_bwd(&db, (char*)h.x + off, (char*)h.dy + off, h.w1, h.b1, h.w2, h.b2, (char*)h.dx + off, h.dw1, h.db1,
                            h.dw2, h.db2, h.ws, h.ws_bytes, cuda_stream);
     if (rc != AFNO_OK) {
       hp->drain(st);

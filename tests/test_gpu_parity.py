@@ -850,3 +850,38 @@ def test_p1_token_grid_bf16_hybrid(oracle):
     assert binding.afno_spectral_path(desc) == "hybrid-fft32-tcgen05"
     _check_forward(oracle, desc, data, label=wl.name)
     _check_backward(oracle, desc, data, label=wl.name)
+
+
+def test_step_host_equals_fwd_host_then_bwd_host(oracle):
+    """afno_spectral_step_host (one call per training step, both link directions busy across the forward / backward boundary)
+    returns bit for bit what afno_spectral_fwd_host followed by afno_spectral_bwd_host return, on the tcgen05 path and on the
+    fp32 path; y is checked against the oracle."""
+    import torch
+    for wl in (inputs.Workload(4, "30x60x192 bf16 B=3 step_host", 3, 30, 60, 192, 2, 1, 0.01, 1.0, "bf16", True, False),
+               inputs.WORKLOADS["sub_bwd_nb2"]):
+        data = inputs.make_inputs(wl)
+        desc = parity.desc_for(wl)
+        bf16 = wl.dtype == "bf16"
+        hx, hdy = (parity.to_device_act(data[k], bf16).cpu().pin_memory() for k in ("x", "dy"))
+        hp = [torch.from_numpy(np.ascontiguousarray(data[k], dtype=np.float32)).pin_memory() for k in ("w1", "b1", "w2", "b2")]
+        out = {}
+        for mode in ("two", "one"):
+            hy, hdx = torch.empty_like(hx).pin_memory(), torch.empty_like(hx).pin_memory()
+            hg = [torch.empty_like(t).pin_memory() for t in hp]
+            if mode == "two":
+                arena = torch.empty(max(binding.afno_spectral_host_arena_bytes(desc, 0), binding.afno_spectral_host_arena_bytes(desc, 1)),
+                                    dtype=torch.uint8, device="cuda")
+                binding.afno_spectral_fwd_host(desc, hx, *hp, hy, arena)
+                binding.afno_spectral_bwd_host(desc, None, hdy, *hp, hdx, *hg, arena)
+            else:
+                arena = torch.empty(binding.afno_spectral_host_arena_bytes(desc, 2), dtype=torch.uint8, device="cuda")
+                binding.afno_spectral_step_host(desc, hx, hdy, *hp, hy, hdx, *hg, arena)
+            out[mode] = [hy.clone(), hdx.clone()] + [t.clone() for t in hg]
+        for a, b in zip(out["two"], out["one"]):
+            assert torch.equal(a, b)
+        y = parity.from_device_act(out["one"][0].cuda()) if bf16 else out["one"][0].numpy()
+        y_ref = oracle.forward(parity.oracle_cfg(oracle, desc), data["x"], data["w1"], data["b1"], data["w2"], data["b2"])
+        assert parity.rel_l2(y, y_ref) <= _tol(desc)
+        with pytest.raises(binding.AfnoError) as e:
+            binding.afno_spectral_step_host(desc, hx, hdy, *hp, hy, hdx, *hg, arena[:1024])
+        assert e.value.status == binding.AFNO_ERR_WORKSPACE

@@ -885,3 +885,40 @@ def test_step_host_equals_fwd_host_then_bwd_host(oracle):
         with pytest.raises(binding.AfnoError) as e:
             binding.afno_spectral_step_host(desc, hx, hdy, *hp, hy, hdx, *hg, arena[:1024])
         assert e.value.status == binding.AFNO_ERR_WORKSPACE
+
+
+def test_hybrid_backward_context_flags_and_graph_replay(oracle):
+    """The hybrid path keeps no context: SAVE_CONTEXT / USE_CONTEXT are accepted and the backward recomputes (include/afno.h),
+    so the context step equals the plain calls bit for bit; and a forward + backward pair captured in a CUDA graph
+     replays bit-identically (tc_mlp_bwd, tc_wgrad and the FFT kernels inside the capture)."""
+    import torch
+    wl = inputs.Workload(4, "100x40x192 bf16 B=2 hybrid ctx", 2, 100, 40, 192, 2, 1, 0.01, 1.0, "bf16", True, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert binding.afno_spectral_path(desc) == "hybrid-fft32-tcgen05"
+    layer = parity.GpuLayer(desc)
+    args = (data["x"], data["dy"], data["w1"], data["b1"], data["w2"], data["b2"])
+    plain = layer.backward(*args, export_masks=False)
+    y_plain = layer.forward(data["x"], *args[2:])
+    got = _ctx_step(desc, data)
+    assert np.array_equal(got["y"], y_plain) and np.array_equal(got["dx"], plain["dx"])
+    for k in ("dw1", "db1", "dw2", "db2"):
+        assert np.array_equal(got[k], plain[k]), k
+    # capture + replay
+    tx, tdy = parity.to_device_act(data["x"], True), parity.to_device_act(data["dy"], True)
+    ty, tdx = torch.zeros_like(tx), torch.zeros_like(tx)
+    p = layer.params(data["w1"], data["b1"], data["w2"], data["b2"])
+    g = [torch.zeros_like(t) for t in p]
+    ws = torch.empty(binding.afno_spectral_workspace_bytes(desc, True), dtype=torch.uint8, device="cuda")
+    s = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(graph, stream=s):
+            binding.afno_spectral_fwd(desc, tx, *p, ty, ws, stream=s)
+            binding.afno_spectral_bwd(desc, tx, tdy, *p, tdx, *g, ws, stream=s)
+    for _ in range(2):
+        graph.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(parity.from_device_act(ty), y_plain) and np.array_equal(parity.from_device_act(tdx), plain["dx"])
+    for t, k in zip(g, ("dw1", "db1", "dw2", "db2")):
+        assert np.array_equal(t.cpu().numpy(), plain[k]), k

@@ -419,6 +419,135 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd_hf(const MlpParams 
   if (warp == 0) tmem_dealloc<512>(tmem);
 }
 
+// ---- pieces shared by the hybrid backward kernels (tc_mlp_bwd, tc_mlp_bwd_hf) -------------------------------------------
+// T (+)= A W (transposed = false) or A W^H (true) as real GEMMs on the (re | im) halves; A = bf16 K-major
+// [96 rows][re 96 | im 96] in shared memory (chunk of 8 columns = kTileSbo bytes), W = the images of one 96 x 96 block
+// (read as MN-major operands with the negate bit for the conjugate transpose); acc0 = 1 keeps what D holds.
+__device__ __forceinline__ void mlp_issue_gemm(uint32_t D, uint32_t aA, uint32_t wr, uint32_t wi, bool transposed, uint32_t acc0,
+                                               uint64_t* bar) {
+  const uint32_t id = idesc_bf16(128, BS, transposed ? kIdescBMn : 0u);
+  const uint32_t lbo = transposed ? kWSbo : kWLbo, sbo = transposed ? kWLbo : kWSbo;
+#pragma unroll
+  for (int ks = 0; ks < BS / 16; ++ks) {
+    const uint64_t ad = smem_desc(aA + ks * 2 * kTileSbo, kTileSbo, kTileLbo);
+    mma_ss(D, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, acc0 | (uint32_t)(ks != 0));
+    mma_ss(D + BS, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? (id | kIdescNegB) : id, acc0 | (uint32_t)(ks != 0));
+  }
+#pragma unroll
+  for (int ks = 0; ks < BS / 16; ++ks) {
+    const uint64_t ad = smem_desc(aA + (BS / 8 + ks * 2) * kTileSbo, kTileSbo, kTileLbo);
+    mma_ss(D, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? id : (id | kIdescNegB), 1u);
+    mma_ss(D + BS, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, 1u);
+  }
+  mma_commit(bar);
+}
+// 96 fp32 complex rows of one channel group -> bf16 operand buffer; lanes run over the 8-channel chunks of a row (768
+// contiguous bytes).  Rows past `rows` and channels past `nch` become zero.  mask2 != nullptr: the softshrink mask of
+// the row ({re bits 0..31, re 32..47, im 0..31, im 32..47} per row and 48-channel half) is applied on the way.
+__device__ __forceinline__ void mlp_load_operand(const float2* __restrict__ src_rows, long long r0, long long rows, int C, int ch0,
+                                                 int nch, uint8_t* dstbuf, const uint4 (*mask2)[2], int tid) {
+  for (uint32_t u = tid; u < HP * (BS / 8); u += kMlpThreads) {
+    const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
+    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, d = a;
+    if (r0 + rr < rows && 8 * c8 < nch) {
+      const float4* src = (const float4*)(src_rows + (size_t)(r0 + rr) * C + ch0 + 8 * c8);
+      a = __ldg(src); b = __ldg(src + 1); c = __ldg(src + 2); d = __ldg(src + 3);
+    }
+    uint4 re = make_uint4(pack_bf16(a.x, a.z), pack_bf16(b.x, b.z), pack_bf16(c.x, c.z), pack_bf16(d.x, d.z));
+    uint4 im = make_uint4(pack_bf16(a.y, a.w), pack_bf16(b.y, b.w), pack_bf16(c.y, c.w), pack_bf16(d.y, d.w));
+    if (mask2 != nullptr) {
+      const uint4 mk = mask2[rr][c8 / 6];
+      const int sh = (c8 % 6) * 8;
+      const uint32_t mre = (uint32_t)((((uint64_t)mk.y << 32) | mk.x) >> sh) & 0xFFu;
+      const uint32_t mim = (uint32_t)((((uint64_t)mk.w << 32) | mk.z) >> sh) & 0xFFu;
+      auto sel = [](uint32_t v, uint32_t bits) {   // bits: bit 0 -> low half, bit 1 -> high half
+        return v & ((bits & 1u ? 0x0000FFFFu : 0u) | (bits & 2u ? 0xFFFF0000u : 0u));
+      };
+      re = make_uint4(sel(re.x, mre), sel(re.y, mre >> 2), sel(re.z, mre >> 4), sel(re.w, mre >> 6));
+      im = make_uint4(sel(im.x, mim), sel(im.y, mim >> 2), sel(im.z, mim >> 4), sel(im.w, mim >> 6));
+    }
+    uint8_t* dst = dstbuf + (size_t)rr * 16;
+    *(uint4*)(dst + (size_t)c8 * kTileSbo) = re;
+    *(uint4*)(dst + (size_t)(BS / 8 + c8) * kTileSbo) = im;
+  }
+}
+// 48 accumulator columns of this thread's row (the caller waits with tmem_wait_ld)
+__device__ __forceinline__ void mlp_ld48(uint32_t taddr, uint32_t (&v)[48]) {
+  tmem_ld16<0>(taddr, v);
+  tmem_ld16<16>(taddr + 16, v);
+  tmem_ld16<32>(taddr + 32, v);
+}
+// O1 = relu(v + bias) of 48 columns -> six 16-byte pieces of the operand buffer; returns the ReLU mask bits
+__device__ __forceinline__ uint64_t mlp_relu_store(const uint32_t (&v)[48], const float* bias, uint8_t* dst) {
+  uint64_t m = 0;
+#pragma unroll
+  for (int g = 0; g < 6; ++g) {
+    uint32_t pk[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const float lo = __uint_as_float(v[8 * g + 2 * e]) + bias[8 * g + 2 * e];
+      const float hi = __uint_as_float(v[8 * g + 2 * e + 1]) + bias[8 * g + 2 * e + 1];
+      m |= (uint64_t)(lo > 0.f) << (8 * g + 2 * e);
+      m |= (uint64_t)(hi > 0.f) << (8 * g + 2 * e + 1);
+      pk[e] = pack_relu_bf16(lo, hi);
+    }
+    *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+  }
+  return m;
+}
+// G1 = mask (.) v of 48 columns -> operand buffer
+__device__ __forceinline__ void mlp_masked_store(const uint32_t (&v)[48], uint64_t m, uint8_t* dst) {
+#pragma unroll
+  for (int g = 0; g < 6; ++g) {
+    uint32_t pk[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const int c = 8 * g + 2 * e;
+      const float lo = ((m >> c) & 1u) ? __uint_as_float(v[c]) : 0.f;
+      const float hi = ((m >> (c + 1)) & 1u) ? __uint_as_float(v[c + 1]) : 0.f;
+      pk[e] = pack_bf16(lo, hi);
+    }
+    *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+  }
+}
+// softshrink mask bits of 48 columns: |v + bias| > lambda on kept rows
+__device__ __forceinline__ uint64_t mlp_shrink_mask(const uint32_t (&v)[48], const float* bias, float lam, bool kept) {
+  uint64_t m = 0;
+#pragma unroll
+  for (int c = 0; c < 48; ++c) m |= (uint64_t)(kept && fabsf(__uint_as_float(v[c]) + bias[c]) > lam) << c;
+  return m;
+}
+// GX (re in vr, im in vi: 48 channels of this thread's row) -> fp32 complex rows of G: each warp transposes its 32 rows
+// through a private slice of an idle operand buffer (16 channels per pass, row pitch 144 B) and stores 128
+// contiguous bytes per row
+__device__ __forceinline__ void mlp_store_rows(const uint32_t (&vr)[48], const uint32_t (&vi)[48], uint8_t* scratch, float2* G,
+                                               long long wrow0, long long rows, int C, int chg, int nch, int lane) {
+  constexpr uint32_t kPitch = 16 * 8 + 16;
+#pragma unroll
+  for (int pass = 0; pass < 3; ++pass) {
+#pragma unroll
+    for (int c = 0; c < 16; c += 2) {
+      const int cc = pass * 16 + c;
+      *(float4*)(scratch + lane * kPitch + c * 8) = make_float4(__uint_as_float(vr[cc]), __uint_as_float(vi[cc]),
+                                                               __uint_as_float(vr[cc + 1]), __uint_as_float(vi[cc + 1]));
+    }
+    __syncwarp();
+    const int chp = pass * 16;   // first channel of this pass within the thread's 48
+#pragma unroll
+    for (int it = 0; it < 8; ++it) {
+      const int id = it * 32 + lane, rr = id >> 3, piece = id & 7;
+      const float4 o = *(const float4*)(scratch + rr * kPitch + piece * 16);
+      if (wrow0 + rr < rows && chg + chp + 2 * piece < nch) *(float4*)(G + (size_t)(wrow0 + rr) * C + chg + chp + 2 * piece) = o;
+    }
+    __syncwarp();
+  }
+}
+// activation masks of this thread's 48 channels -> [..][C'][2] bytes (parity tests)
+__device__ __forceinline__ void mlp_export_mask(uint8_t* dst, uint64_t mre, uint64_t mim, int nvalid) {
+  for (int c = 0; c < 48; ++c)
+    if (c < nvalid) *(uchar2*)(dst + 2 * c) = make_uchar2((unsigned char)((mre >> c) & 1u), (unsigned char)((mim >> c) & 1u));
+}
+
 // ---- hybrid BACKWARD (rows B1 second half, B3-B7) on the tensor cores, hidden factor 1 ---------------------------------
 // For grids the fused chain does not reach the backward call runs the transforms as fp32 FFTs (generic.cu) and this
 // kernel in between: per tile of 96 spectrum rows x one group of 96 channels
@@ -486,28 +615,11 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
   const int q = warp & 3, chalf = warp >> 2;    // TMEM lane quarter (rows 32 q ..), 48-channel half of the group
   const int r = q * 32 + lane;                  // row of the tile (quarter 3 holds no rows: HP = 96)
   const bool epi = q < 3;
-  const uint32_t lane_sel = (uint32_t)(q * 32) << 16;
+  const uint32_t acc = D + ((uint32_t)(q * 32) << 16) + chalf * 48;   // this thread's re columns; im at + BS
   const bool storer = tid == 3 * 32;            // lane 0 of an otherwise idle warp issues the image copies
   const uint64_t pol_img = l2_evict_normal();
+  const size_t chunk_off = (size_t)chalf * 6 * kTileSbo, im_off = (size_t)(BS / 8) * kTileSbo;
   uint32_t ph = 0;
-  // T = A W (TRANSPOSED = false) or A W^H (true); A = bf16 K-major [96 rows][re 96 | im 96] in shared memory
-  auto issue = [&](uint32_t aA, uint32_t wr, uint32_t wi, bool transposed) {
-    const uint32_t id = idesc_bf16(128, BS, transposed ? kIdescBMn : 0u);
-    const uint32_t lbo = transposed ? kWSbo : kWLbo, sbo = transposed ? kWLbo : kWSbo;
-#pragma unroll
-    for (int ks = 0; ks < BS / 16; ++ks) {
-      const uint64_t ad = smem_desc(aA + ks * 2 * kTileSbo, kTileSbo, kTileLbo);
-      mma_ss(D, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, ks != 0);
-      mma_ss(D + BS, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? (id | kIdescNegB) : id, ks != 0);
-    }
-#pragma unroll
-    for (int ks = 0; ks < BS / 16; ++ks) {
-      const uint64_t ad = smem_desc(aA + (BS / 8 + ks * 2) * kTileSbo, kTileSbo, kTileLbo);
-      mma_ss(D, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? id : (id | kIdescNegB), 1u);
-      mma_ss(D + BS, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, 1u);
-    }
-    mma_commit(&done);
-  };
   // every thread has written its part of operand `buf`: hand it to the tensor core (and to the copy engine as an image)
   auto run_gemm = [&](const uint8_t* buf, uint32_t wr, uint32_t wi, bool transposed, __nv_bfloat16* img, size_t img_off) {
     fence_async_smem();
@@ -515,46 +627,13 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
     __syncthreads();
     if (warp == 0 && elect_one()) {
       tc_fence_after();
-      issue(smem_u32(buf), wr, wi, transposed);
+      mlp_issue_gemm(D, smem_u32(buf), wr, wi, transposed, 0u, &done);
     }
     if (storer) bulk_store((uint8_t*)img + img_off, smem_u32(buf), kTileBytes, pol_img);
     __syncwarp();
     mbar_wait(&done, ph);
     tc_fence_after();
     ph ^= 1u;
-  };
-  // fp32 complex rows of the group -> bf16 operand, lanes run over the 8-channel chunks of a row (768 contiguous
-  // bytes); MASKED: the softshrink mask of the row (sMask2) is applied on the way
-  auto load_operand = [&](const float2* src_rows, long long r0, uint8_t* dstbuf, bool masked) {
-    for (uint32_t u = tid; u < HP * (BS / 8); u += kMlpThreads) {
-      const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
-      float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, d = a;
-      if (r0 + rr < p.rows && 8 * c8 < nch) {
-        const float4* src = (const float4*)(src_rows + (size_t)(r0 + rr) * p.C + ch0 + 8 * c8);
-        a = __ldg(src); b = __ldg(src + 1); c = __ldg(src + 2); d = __ldg(src + 3);
-      }
-      uint4 re = make_uint4(pack_bf16(a.x, a.z), pack_bf16(b.x, b.z), pack_bf16(c.x, c.z), pack_bf16(d.x, d.z));
-      uint4 im = make_uint4(pack_bf16(a.y, a.w), pack_bf16(b.y, b.w), pack_bf16(c.y, c.w), pack_bf16(d.y, d.w));
-      if (masked) {
-        const uint4 mk = sMask2[rr][c8 / 6];
-        const int sh = (c8 % 6) * 8;
-        const uint32_t mre = (uint32_t)((((uint64_t)mk.y << 32) | mk.x) >> sh) & 0xFFu;
-        const uint32_t mim = (uint32_t)((((uint64_t)mk.w << 32) | mk.z) >> sh) & 0xFFu;
-        auto sel = [](uint32_t v, uint32_t bits) {   // bits: bit 0 -> low half, bit 1 -> high half
-          return v & ((bits & 1u ? 0x0000FFFFu : 0u) | (bits & 2u ? 0xFFFF0000u : 0u));
-        };
-        re = make_uint4(sel(re.x, mre), sel(re.y, mre >> 2), sel(re.z, mre >> 4), sel(re.w, mre >> 6));
-        im = make_uint4(sel(im.x, mim), sel(im.y, mim >> 2), sel(im.z, mim >> 4), sel(im.w, mim >> 6));
-      }
-      uint8_t* dst = dstbuf + (size_t)rr * 16;
-      *(uint4*)(dst + (size_t)c8 * kTileSbo) = re;
-      *(uint4*)(dst + (size_t)(BS / 8 + c8) * kTileSbo) = im;
-    }
-  };
-  auto ld48x = [&](uint32_t col, uint32_t (&v)[48]) {
-    tmem_ld16<0>(D + lane_sel + col, v);
-    tmem_ld16<16>(D + lane_sel + col + 16, v);
-    tmem_ld16<32>(D + lane_sel + col + 32, v);
   };
   for (long long t = s0; t < ntiles; t += S) {
     const long long r0 = t * HP;
@@ -565,44 +644,27 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
     const bool kept = row_valid && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
     uint64_t m1[2] = {0, 0}, m2[2] = {0, 0};   // [re, im] bits of this thread's 48 channels
     // ---- X -> bf16 operand; P1 = X W1 ----
-    load_operand(p.X, r0, bX, false);
+    mlp_load_operand(p.X, r0, p.rows, p.C, ch0, nch, bX, nullptr, tid);
     run_gemm(bX, w1r, w1i, false, p.Xh, img_off);
     // ---- O1 = relu(P1 + b1), mask1 ----
     if (epi) {
 #pragma unroll
       for (int half = 0; half < 2; ++half) {
         uint32_t v[48];
-        ld48x(half * BS + chalf * 48, v);
+        mlp_ld48(acc + half * BS, v);
         tmem_wait_ld();
-        const float* bias = sBias + half * BS + chalf * 48;
-        uint8_t* dst = bO + (size_t)r * 16 + (size_t)(half * (BS / 8) + chalf * 6) * kTileSbo;
-#pragma unroll
-        for (int g = 0; g < 6; ++g) {
-          uint32_t pk[4];
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const float lo = __uint_as_float(v[8 * g + 2 * e]) + bias[8 * g + 2 * e];
-            const float hi = __uint_as_float(v[8 * g + 2 * e + 1]) + bias[8 * g + 2 * e + 1];
-            m1[half] |= (uint64_t)(lo > 0.f) << (8 * g + 2 * e);
-            m1[half] |= (uint64_t)(hi > 0.f) << (8 * g + 2 * e + 1);
-            pk[e] = pack_relu_bf16(lo, hi);
-          }
-          *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-        }
+        m1[half] = mlp_relu_store(v, sBias + half * BS + chalf * 48, bO + (size_t)r * 16 + half * im_off + chunk_off);
       }
     }
     run_gemm(bO, w2r, w2i, false, p.O1, img_off);
     // ---- mask2 = (|P2 + b2| > lambda) on kept rows ----
     if (epi) {
-      const float lam = p.lambda;
 #pragma unroll
       for (int half = 0; half < 2; ++half) {
         uint32_t v[48];
-        ld48x(half * BS + chalf * 48, v);
+        mlp_ld48(acc + half * BS, v);
         tmem_wait_ld();
-        const float* bias = sBias + NT + half * BS + chalf * 48;
-#pragma unroll
-        for (int c = 0; c < 48; ++c) m2[half] |= (uint64_t)(kept && fabsf(__uint_as_float(v[c]) + bias[c]) > lam) << c;
+        m2[half] = mlp_shrink_mask(v, sBias + NT + half * BS + chalf * 48, p.lambda, kept);
       }
       sMask2[r][chalf] = make_uint4((uint32_t)m2[0], (uint32_t)(m2[0] >> 32), (uint32_t)m2[1], (uint32_t)(m2[1] >> 32));
     }
@@ -611,71 +673,33 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
     __syncthreads();
     tc_fence_after();
     // ---- G2 = mask2 (.) G -> bf16 operand; G1pre = G2 W2^H ----
-    load_operand(p.G, r0, bG2, true);
+    mlp_load_operand(p.G, r0, p.rows, p.C, ch0, nch, bG2, sMask2, tid);
     run_gemm(bG2, w2r, w2i, true, p.G2, img_off);
     // ---- G1 = mask1 (.) G1pre ----
     if (epi) {
 #pragma unroll
       for (int half = 0; half < 2; ++half) {
         uint32_t v[48];
-        ld48x(half * BS + chalf * 48, v);
+        mlp_ld48(acc + half * BS, v);
         tmem_wait_ld();
-        uint8_t* dst = bG1 + (size_t)r * 16 + (size_t)(half * (BS / 8) + chalf * 6) * kTileSbo;
-#pragma unroll
-        for (int g = 0; g < 6; ++g) {
-          uint32_t pk[4];
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const int c = 8 * g + 2 * e;
-            const float lo = ((m1[half] >> c) & 1u) ? __uint_as_float(v[c]) : 0.f;
-            const float hi = ((m1[half] >> (c + 1)) & 1u) ? __uint_as_float(v[c + 1]) : 0.f;
-            pk[e] = pack_bf16(lo, hi);
-          }
-          *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-        }
+        mlp_masked_store(v, m1[half], bG1 + (size_t)r * 16 + half * im_off + chunk_off);
       }
     }
     run_gemm(bG1, w1r, w1i, true, p.G1, img_off);
-    // ---- GX -> fp32 complex, in place over G: each warp transposes its 32 rows through a private slice of bX
-    //      (16 channels per pass, row pitch 144 B) and stores 128 contiguous bytes per row ----
+    // ---- GX -> fp32 complex, in place over G ----
     if (epi) {
       uint32_t vr[48], vi[48];
-      ld48x(chalf * 48, vr);
-      ld48x(BS + chalf * 48, vi);
+      mlp_ld48(acc, vr);
+      mlp_ld48(acc + BS, vi);
       tmem_wait_ld();
-      constexpr uint32_t kPitch = 16 * 8 + 16;
-      uint8_t* scratch = bX + (size_t)warp * (kTileBytes / 8 / 16 * 16);
-      const long long wrow0 = r0 + q * 32;
-#pragma unroll
-      for (int pass = 0; pass < 3; ++pass) {
-#pragma unroll
-        for (int c = 0; c < 16; c += 2) {
-          const int cc = pass * 16 + c;
-          *(float4*)(scratch + lane * kPitch + c * 8) = make_float4(__uint_as_float(vr[cc]), __uint_as_float(vi[cc]),
-                                                                   __uint_as_float(vr[cc + 1]), __uint_as_float(vi[cc + 1]));
-        }
-        __syncwarp();
-        const int chp = chalf * 48 + pass * 16;
-#pragma unroll
-        for (int it = 0; it < 8; ++it) {
-          const int id = it * 32 + lane, rr = id >> 3, piece = id & 7;
-          const float4 o = *(const float4*)(scratch + rr * kPitch + piece * 16);
-          if (wrow0 + rr < p.rows && chp + 2 * piece < nch)
-            *(float4*)(p.G + (size_t)(wrow0 + rr) * p.C + ch0 + chp + 2 * piece) = o;
-        }
-        __syncwarp();
-      }
+      mlp_store_rows(vr, vi, bX + (size_t)warp * (kTileBytes / 8 / 16 * 16), p.G + ch0, r0 + q * 32, p.rows, p.C, chalf * 48, nch, lane);
       if (p.mask1 != nullptr && row_valid) {
         // export for the mask-consistent parity tests: [B][H][Wh][C][2] bytes, this thread's 48 channels
         const long long bh = row / p.Kw;
         const int kw = (int)(row - bh * p.Kw);
         const size_t base = ((size_t)(bh * p.Wh + kw) * p.C + ch0 + chalf * 48) * 2;
-        for (int c = 0; c < 48; ++c) {
-          if (chalf * 48 + c < nch) {
-            *(uchar2*)(p.mask1 + base + 2 * c) = make_uchar2((unsigned char)((m1[0] >> c) & 1u), (unsigned char)((m1[1] >> c) & 1u));
-            *(uchar2*)(p.mask2 + base + 2 * c) = make_uchar2((unsigned char)((m2[0] >> c) & 1u), (unsigned char)((m2[1] >> c) & 1u));
-          }
-        }
+        mlp_export_mask(p.mask1 + base, m1[0], m1[1], nch - chalf * 48);
+        mlp_export_mask(p.mask2 + base, m2[0], m2[1], nch - chalf * 48);
       }
     }
     if (storer) bulk_wait_read<0>();   // every image of this tile has left its buffer
@@ -747,27 +771,11 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
   const int q = warp & 3, chalf = warp >> 2;
   const int r = q * 32 + lane;
   const bool epi = q < 3;
-  const uint32_t lane_sel = (uint32_t)(q * 32) << 16;
+  const uint32_t lane_col = ((uint32_t)(q * 32) << 16) + chalf * 48;   // this thread's re columns of an accumulator; im at + BS
   const bool storer = tid == 3 * 32;
   const uint64_t pol_img = l2_evict_normal();
+  const size_t chunk_off = (size_t)chalf * 6 * kTileSbo, im_off = (size_t)(BS / 8) * kTileSbo;
   uint32_t ph = 0;
-  auto issue = [&](uint32_t D, uint32_t aA, uint32_t wr, uint32_t wi, bool transposed, uint32_t acc0) {
-    const uint32_t id = idesc_bf16(128, BS, transposed ? kIdescBMn : 0u);
-    const uint32_t lbo = transposed ? kWSbo : kWLbo, sbo = transposed ? kWLbo : kWSbo;
-#pragma unroll
-    for (int ks = 0; ks < BS / 16; ++ks) {
-      const uint64_t ad = smem_desc(aA + ks * 2 * kTileSbo, kTileSbo, kTileLbo);
-      mma_ss(D, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, acc0 | (uint32_t)(ks != 0));
-      mma_ss(D + BS, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? (id | kIdescNegB) : id, acc0 | (uint32_t)(ks != 0));
-    }
-#pragma unroll
-    for (int ks = 0; ks < BS / 16; ++ks) {
-      const uint64_t ad = smem_desc(aA + (BS / 8 + ks * 2) * kTileSbo, kTileSbo, kTileLbo);
-      mma_ss(D, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? id : (id | kIdescNegB), 1u);
-      mma_ss(D + BS, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, 1u);
-    }
-    mma_commit(&done);
-  };
   // operand `buf` is complete: GEMM into D (and the image copy); returns when the GEMM has completed
   auto run_gemm = [&](uint32_t D, const uint8_t* buf, uint32_t wr, uint32_t wi, bool transposed, uint32_t acc0,
                       __nv_bfloat16* img, size_t img_off) {
@@ -776,7 +784,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
     __syncthreads();
     if (warp == 0 && elect_one()) {
       tc_fence_after();
-      issue(D, smem_u32(buf), wr, wi, transposed, acc0);
+      mlp_issue_gemm(D, smem_u32(buf), wr, wi, transposed, acc0, &done);
     }
     if (storer && img != nullptr) bulk_store((uint8_t*)img + img_off, smem_u32(buf), kTileBytes, pol_img);
     __syncwarp();
@@ -790,36 +798,12 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
     for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMlpThreads) cp_async16(aW + i * 16, wsrc + (size_t)i * 16);
     cp_async_wait_all();
   };
-  auto load_operand = [&](const float2* src_rows, long long r0, uint8_t* dstbuf, bool masked) {
-    for (uint32_t u = tid; u < HP * (BS / 8); u += kMlpThreads) {
-      const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
-      float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, d = a;
-      if (r0 + rr < p.rows) {
-        const float4* src = (const float4*)(src_rows + (size_t)(r0 + rr) * p.C + ch0 + 8 * c8);
-        a = __ldg(src); b = __ldg(src + 1); c = __ldg(src + 2); d = __ldg(src + 3);
-      }
-      uint4 re = make_uint4(pack_bf16(a.x, a.z), pack_bf16(b.x, b.z), pack_bf16(c.x, c.z), pack_bf16(d.x, d.z));
-      uint4 im = make_uint4(pack_bf16(a.y, a.w), pack_bf16(b.y, b.w), pack_bf16(c.y, c.w), pack_bf16(d.y, d.w));
-      if (masked) {
-        const uint4 mk = sMask2[rr][c8 / 6];
-        const int sh = (c8 % 6) * 8;
-        const uint32_t mre = (uint32_t)((((uint64_t)mk.y << 32) | mk.x) >> sh) & 0xFFu;
-        const uint32_t mim = (uint32_t)((((uint64_t)mk.w << 32) | mk.z) >> sh) & 0xFFu;
-        auto sel = [](uint32_t v, uint32_t bits) {
-          return v & ((bits & 1u ? 0x0000FFFFu : 0u) | (bits & 2u ? 0xFFFF0000u : 0u));
-        };
-        re = make_uint4(sel(re.x, mre), sel(re.y, mre >> 2), sel(re.z, mre >> 4), sel(re.w, mre >> 6));
-        im = make_uint4(sel(im.x, mim), sel(im.y, mim >> 2), sel(im.z, mim >> 4), sel(im.w, mim >> 6));
-      }
-      uint8_t* dst = dstbuf + (size_t)rr * 16;
-      *(uint4*)(dst + (size_t)c8 * kTileSbo) = re;
-      *(uint4*)(dst + (size_t)(BS / 8 + c8) * kTileSbo) = im;
-    }
-  };
-  auto ld48x = [&](uint32_t D, uint32_t col, uint32_t (&v)[48]) {
-    tmem_ld16<0>(D + lane_sel + col, v);
-    tmem_ld16<16>(D + lane_sel + col + 16, v);
-    tmem_ld16<32>(D + lane_sel + col + 32, v);
+  // the previous image copy has left the buffer the next epilogue overwrites
+  auto buffers_free = [&]() {
+    if (storer) bulk_wait_read<0>();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
   };
   const size_t chunk_imgs = (size_t)p.ntiles * p.nb * kTileBytes;   // bytes of one chunk's image tensor
   for (long long t = s0; t < p.ntiles; t += S) {
@@ -831,136 +815,70 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
     const bool kept = row_valid && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
     const long long bh = row / p.Kw;
     const int kw = (int)(row - bh * p.Kw);
-    load_operand(p.X, r0, bX, false);
+    mlp_load_operand(p.X, r0, p.rows, p.C, ch0, BS, bX, nullptr, tid);
     // ---- pass 1 ----
     for (int hc = 0; hc < hf; ++hc) {
       load_weights(hc);
       run_gemm(D1, bX, wAr, wAi, false, 0u, hc == 0 ? p.Xh : nullptr, img_off);
-      if (storer) bulk_wait_read<0>();   // the previous chunk's O1 image (and Xh) have left their buffers
-      tc_fence_before();
-      __syncthreads();
-      tc_fence_after();
+      buffers_free();   // the previous chunk's O1 image has left bH
       if (epi) {
-        uint64_t m1[2] = {0, 0};
+        uint64_t m1[2];
 #pragma unroll
         for (int half = 0; half < 2; ++half) {
           uint32_t v[48];
-          ld48x(D1, half * BS + chalf * 48, v);
+          mlp_ld48(D1 + lane_col + half * BS, v);
           tmem_wait_ld();
-          const float* bias = sBias + (size_t)hc * NT + half * BS + chalf * 48;
-          uint8_t* dst = bH + (size_t)r * 16 + (size_t)(half * (BS / 8) + chalf * 6) * kTileSbo;
-#pragma unroll
-          for (int g = 0; g < 6; ++g) {
-            uint32_t pk[4];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const float lo = __uint_as_float(v[8 * g + 2 * e]) + bias[8 * g + 2 * e];
-              const float hi = __uint_as_float(v[8 * g + 2 * e + 1]) + bias[8 * g + 2 * e + 1];
-              m1[half] |= (uint64_t)(lo > 0.f) << (8 * g + 2 * e);
-              m1[half] |= (uint64_t)(hi > 0.f) << (8 * g + 2 * e + 1);
-              pk[e] = pack_relu_bf16(lo, hi);
-            }
-            *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-          }
+          m1[half] = mlp_relu_store(v, sBias + (size_t)hc * NT + half * BS + chalf * 48, bH + (size_t)r * 16 + half * im_off + chunk_off);
         }
         sMask1[((size_t)hc * HP + r) * 2 + chalf] = make_uint4((uint32_t)m1[0], (uint32_t)(m1[0] >> 32), (uint32_t)m1[1], (uint32_t)(m1[1] >> 32));
-        if (p.mask1 != nullptr && row_valid) {
-          const size_t base = ((size_t)(bh * p.Wh + kw) * ((size_t)p.nb * hid) + (size_t)j * hid + hc * BS + chalf * 48) * 2;
-          for (int c = 0; c < 48; ++c)
-            *(uchar2*)(p.mask1 + base + 2 * c) = make_uchar2((unsigned char)((m1[0] >> c) & 1u), (unsigned char)((m1[1] >> c) & 1u));
-        }
+        if (p.mask1 != nullptr && row_valid)
+          mlp_export_mask(p.mask1 + ((size_t)(bh * p.Wh + kw) * ((size_t)p.nb * hid) + (size_t)j * hid + hc * BS + chalf * 48) * 2, m1[0],
+                          m1[1], 48);
       }
       run_gemm(D2, bH, wBr, wBi, false, hc > 0 ? 1u : 0u, p.O1, (size_t)hc * chunk_imgs + img_off);
     }
     // ---- mask2 = (|P2 + b2| > lambda) on kept rows ----
     if (epi) {
-      const float lam = p.lambda;
-      uint64_t m2[2] = {0, 0};
+      uint64_t m2[2];
 #pragma unroll
       for (int half = 0; half < 2; ++half) {
         uint32_t v[48];
-        ld48x(D2, half * BS + chalf * 48, v);
+        mlp_ld48(D2 + lane_col + half * BS, v);
         tmem_wait_ld();
-        const float* bias = sBias + (size_t)hf * NT + half * BS + chalf * 48;
-#pragma unroll
-        for (int c = 0; c < 48; ++c) m2[half] |= (uint64_t)(kept && fabsf(__uint_as_float(v[c]) + bias[c]) > lam) << c;
+        m2[half] = mlp_shrink_mask(v, sBias + (size_t)hf * NT + half * BS + chalf * 48, p.lambda, kept);
       }
       sMask2[r][chalf] = make_uint4((uint32_t)m2[0], (uint32_t)(m2[0] >> 32), (uint32_t)m2[1], (uint32_t)(m2[1] >> 32));
-      if (p.mask2 != nullptr && row_valid) {
-        const size_t base = ((size_t)(bh * p.Wh + kw) * p.C + ch0 + chalf * 48) * 2;
-        for (int c = 0; c < 48; ++c)
-          *(uchar2*)(p.mask2 + base + 2 * c) = make_uchar2((unsigned char)((m2[0] >> c) & 1u), (unsigned char)((m2[1] >> c) & 1u));
-      }
+      if (p.mask2 != nullptr && row_valid)
+        mlp_export_mask(p.mask2 + ((size_t)(bh * p.Wh + kw) * p.C + ch0 + chalf * 48) * 2, m2[0], m2[1], 48);
     }
-    if (storer) bulk_wait_read<0>();
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
+    buffers_free();
     // ---- pass 2 ----
-    load_operand(p.G, r0, bG2, true);
+    mlp_load_operand(p.G, r0, p.rows, p.C, ch0, BS, bG2, sMask2, tid);
     for (int hc = 0; hc < hf; ++hc) {
       load_weights(hc);
       run_gemm(D1, bG2, wBr, wBi, true, 0u, hc == 0 ? p.G2 : nullptr, img_off);   // G2 W2[c, :]^H
-      if (storer) bulk_wait_read<0>();
-      tc_fence_before();
-      __syncthreads();
-      tc_fence_after();
+      buffers_free();
       if (epi) {
         const uint4 mk = sMask1[((size_t)hc * HP + r) * 2 + chalf];
         const uint64_t m1[2] = {((uint64_t)mk.y << 32) | mk.x, ((uint64_t)mk.w << 32) | mk.z};
 #pragma unroll
         for (int half = 0; half < 2; ++half) {
           uint32_t v[48];
-          ld48x(D1, half * BS + chalf * 48, v);
+          mlp_ld48(D1 + lane_col + half * BS, v);
           tmem_wait_ld();
-          uint8_t* dst = bH + (size_t)r * 16 + (size_t)(half * (BS / 8) + chalf * 6) * kTileSbo;
-#pragma unroll
-          for (int g = 0; g < 6; ++g) {
-            uint32_t pk[4];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const int c = 8 * g + 2 * e;
-              const float lo = ((m1[half] >> c) & 1u) ? __uint_as_float(v[c]) : 0.f;
-              const float hi = ((m1[half] >> (c + 1)) & 1u) ? __uint_as_float(v[c + 1]) : 0.f;
-              pk[e] = pack_bf16(lo, hi);
-            }
-            *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-          }
+          mlp_masked_store(v, m1[half], bH + (size_t)r * 16 + half * im_off + chunk_off);
         }
       }
       run_gemm(D2, bH, wAr, wAi, true, hc > 0 ? 1u : 0u, p.G1, (size_t)hc * chunk_imgs + img_off);   // GX += G1_c W1[:, c]^H
     }
-    if (storer) bulk_wait_read<0>();   // bX is the scratch area of the store below
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
+    buffers_free();   // bX is the scratch area of the store below
     // ---- GX -> fp32 complex, in place over G ----
     if (epi) {
       uint32_t vr[48], vi[48];
-      ld48x(D2, chalf * 48, vr);
-      ld48x(D2, BS + chalf * 48, vi);
+      mlp_ld48(D2 + lane_col, vr);
+      mlp_ld48(D2 + lane_col + BS, vi);
       tmem_wait_ld();
-      constexpr uint32_t kPitch = 16 * 8 + 16;
-      uint8_t* scratch = bX + (size_t)warp * (kTileBytes / 8 / 16 * 16);
-      const long long wrow0 = r0 + q * 32;
-#pragma unroll
-      for (int pass = 0; pass < 3; ++pass) {
-#pragma unroll
-        for (int c = 0; c < 16; c += 2) {
-          const int cc = pass * 16 + c;
-          *(float4*)(scratch + lane * kPitch + c * 8) = make_float4(__uint_as_float(vr[cc]), __uint_as_float(vi[cc]),
-                                                                   __uint_as_float(vr[cc + 1]), __uint_as_float(vi[cc + 1]));
-        }
-        __syncwarp();
-        const int chp = chalf * 48 + pass * 16;
-#pragma unroll
-        for (int it = 0; it < 8; ++it) {
-          const int id = it * 32 + lane, rr = id >> 3, piece = id & 7;
-          const float4 o = *(const float4*)(scratch + rr * kPitch + piece * 16);
-          if (wrow0 + rr < p.rows) *(float4*)(p.G + (size_t)(wrow0 + rr) * p.C + ch0 + chp + 2 * piece) = o;
-        }
-        __syncwarp();
-      }
+      mlp_store_rows(vr, vi, bX + (size_t)warp * (kTileBytes / 8 / 16 * 16), p.G + ch0, r0 + q * 32, p.rows, p.C, chalf * 48, BS, lane);
     }
     tc_fence_before();
     __syncthreads();

@@ -1,6 +1,7 @@
 // Internal declarations shared by the translation units of libafno_b200.so.
 // Nothing here is part of the C ABI (include/afno.h) and nothing here is shared with oracle/.
 #pragma once
+#include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <stddef.h>
 #include <stdint.h>
@@ -83,16 +84,46 @@ cudaError_t tc_backward(const Geometry& g, const Plan& p, const void* x, const v
 // hybrid path (bf16 activations on grids beyond the fused chain): generic fp32 FFTs + tensor-core block MLP, forward
 bool tc_mlp_supported(const Geometry& g);
 size_t tc_mlp_workspace_bytes(const Geometry& g);
-cudaError_t tc_mlp_forward(const Geometry& g, float2* X, const float* w1, const float* b1, const float* w2,
+// X (and G below): the spectrum in the generic path's [row][C] layout, fp32 complex or (spec16) bf16 complex
+cudaError_t tc_mlp_forward(const Geometry& g, void* X, bool spec16, const float* w1, const float* b1, const float* w2,
                            const float* b2, void* ws, cudaStream_t st);
 
 // hybrid backward, hidden factor 1: block MLP gradient stages and parameter gradients on the tensor cores
 bool tc_mlp_bwd_supported(const Geometry& g);
 size_t tc_mlp_bwd_workspace_bytes(const Geometry& g);
-cudaError_t tc_mlp_backward(const Geometry& g, const float2* X, float2* G, const float* w1, const float* b1, const float* w2,
-                            const float* b2, float* dw1, float* db1, float* dw2, float* db2, uint8_t* mask1, uint8_t* mask2,
-                            void* ws, cudaStream_t st);
+cudaError_t tc_mlp_backward(const Geometry& g, const void* X, void* G, bool spec16, const float* w1, const float* b1,
+                            const float* w2, const float* b2, float* dw1, float* db1, float* dw2, float* db2, uint8_t* mask1,
+                            uint8_t* mask2, void* ws, cudaStream_t st);
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+#ifdef __CUDACC__
+// Storage type of the half-spectra between the kernels of the generic / hybrid paths: fp32 complex (float2) or, on the
+// hybrid path when every transform runs through the two-pass kernels, bf16 complex (SpecBf16: re in the low half).
+// The arithmetic is fp32 either way; pairs = two adjacent channels.
+struct SpecBf16 { uint32_t v; };
+template <typename ST> struct SpecIO;
+template <> struct SpecIO<float2> {
+  typedef float4 pair_t;
+  static __device__ __forceinline__ pair_t ldpair(const float2* p) { return __ldg((const float4*)p); }
+  static __device__ __forceinline__ void unpair(pair_t v, float2& a, float2& b) { a = make_float2(v.x, v.y); b = make_float2(v.z, v.w); }
+  static __device__ __forceinline__ void stpair(float2* p, float2 a, float2 b) { *(float4*)p = make_float4(a.x, a.y, b.x, b.y); }
+  static __device__ __forceinline__ float2 ld(const float2* p) { return *p; }
+  static __device__ __forceinline__ void st(float2* p, float2 v) { *p = v; }
+};
+template <> struct SpecIO<SpecBf16> {
+  typedef uint2 pair_t;
+  static __device__ __forceinline__ float2 up(uint32_t u) { return make_float2(__uint_as_float(u << 16), __uint_as_float(u & 0xFFFF0000u)); }
+  static __device__ __forceinline__ uint32_t down(float2 v) {
+    __nv_bfloat162 t = __floats2bfloat162_rn(v.x, v.y);
+    return *reinterpret_cast<uint32_t*>(&t);
+  }
+  static __device__ __forceinline__ pair_t ldpair(const SpecBf16* p) { return __ldg((const uint2*)p); }
+  static __device__ __forceinline__ void unpair(pair_t v, float2& a, float2& b) { a = up(v.x); b = up(v.y); }
+  static __device__ __forceinline__ void stpair(SpecBf16* p, float2 a, float2 b) { *(uint2*)p = make_uint2(down(a), down(b)); }
+  static __device__ __forceinline__ float2 ld(const SpecBf16* p) { return up(p->v); }
+  static __device__ __forceinline__ void st(SpecBf16* p, float2 v) { p->v = down(v); }
+};
+#endif
 
 } // namespace afno

@@ -108,17 +108,17 @@ constexpr int kF2MaxBatch = 24;   // rows a thread keeps in flight before its fi
 
 // ---- F2 / F7: H-direction complex FFT, in place on S[B][H][Kw][C]; tile = 32 G channels of one (b, kw) column ---------
 // grid (C / (32 G), Kw, B), block 256; smem H * 32 G float2 (G = 2 up to 360 points, 1 beyond: 184 KB at 720)
-template <int N1, int N2, int SG, int G>
-__global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(float2* __restrict__ S, const float2* __restrict__ tw, int Kw, int C) {
+template <int N1, int N2, int SG, int G, typename ST>
+__global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(ST* __restrict__ S, const float2* __restrict__ tw, int Kw, int C) {
   constexpr int H = N1 * N2, LW = 32 * G;
   extern __shared__ float2 smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int kw = blockIdx.y, b = blockIdx.z;
-  float2* base = S + ((size_t)b * H * Kw + kw) * C + (size_t)blockIdx.x * LW;
+  ST* base = S + ((size_t)b * H * Kw + kw) * C + (size_t)blockIdx.x * LW;
   const size_t hstride = (size_t)Kw * C;
   // a row of the tile is 256 G contiguous bytes: one float2 (G = 1) or float4 (G = 2) per lane; up to kF2MaxBatch
   // rows of the warp are in flight before the first shared-memory store
-  typedef typename std::conditional<G == 2, float4, float2>::type vec_t;
+  typedef typename std::conditional<G == 2, typename SpecIO<ST>::pair_t, ST>::type vec_t;
   constexpr int PER = (H + kF2Warps - 1) / kF2Warps, LB = PER < kF2MaxBatch ? PER : kF2MaxBatch;
   for (int h0 = warp; h0 < H; h0 += kF2Warps * LB) {
     vec_t v[LB];
@@ -130,7 +130,15 @@ __global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(float2* __restrict__ S,
 #pragma unroll
     for (int u = 0; u < LB; ++u) {
       const int h = h0 + u * kF2Warps;
-      if (h < H) *(vec_t*)(smem + h * LW + G * lane) = v[u];
+      if (h < H) {
+        if constexpr (G == 2) {
+          float2 a, b2;
+          SpecIO<ST>::unpair(v[u], a, b2);
+          *(float4*)(smem + h * LW + 2 * lane) = make_float4(a.x, a.y, b2.x, b2.y);
+        } else {
+          smem[h * LW + lane] = SpecIO<ST>::ld(&v[u]);
+        }
+      }
     }
   }
   __syncthreads();
@@ -143,9 +151,9 @@ __global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(float2* __restrict__ S,
     const int g = task / N1, k1 = task - g * N1;
     float2 v[N2];
     pass_b<N1, N2, SG>(smem, LW, g * 32 + lane, k1, v);
-    float2* dst = base + g * 32 + lane;
+    ST* dst = base + g * 32 + lane;
 #pragma unroll
-    for (int k2 = 0; k2 < N2; ++k2) dst[(size_t)(k1 + N1 * k2) * hstride] = v[k2];
+    for (int k2 = 0; k2 < N2; ++k2) SpecIO<ST>::st(dst + (size_t)(k1 + N1 * k2) * hstride, v[k2]);
   }
 }
 
@@ -154,9 +162,9 @@ __global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(float2* __restrict__ S,
 // iteration) up to 360 points; LW = 16 beyond (184 KB at 1,440 points): a warp then runs two tasks side by side, one
 // per half-warp.  Pass B runs the tasks k1 and N1 - k1 together: the Hermitian split of bin k needs Z[k] and Z[W - k],
 // which live in exactly those two tasks, so the half-spectrum leaves from registers.
-template <typename T, int N1, int N2, int NW, int LW>
+template <typename T, int N1, int N2, int NW, int LW, typename ST>
 __global__ void __launch_bounds__(32 * NW, LW == 32 ? 2 : 1)
-k_wfft_fwd2(const T* __restrict__ x, float2* __restrict__ S, const float2* __restrict__ tw, int H, int C, int Kw, float scale,
+k_wfft_fwd2(const T* __restrict__ x, ST* __restrict__ S, const float2* __restrict__ tw, int H, int C, int Kw, float scale,
             int alpha_weight) {
   constexpr int W = N1 * N2, TPW = 32 / LW, NSLOT = NW * TPW;
   extern __shared__ float2 smem[];
@@ -185,13 +193,14 @@ k_wfft_fwd2(const T* __restrict__ x, float2* __restrict__ S, const float2* __res
   __syncthreads();
   for (int n2 = slot; n2 < N2; n2 += NSLOT) pass_a<N1, N2, -1>(smem, LW, l, n2, tw);
   __syncthreads();
-  float2* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
+  ST* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
   // bin k from Z[k] = zk and Z[W - k] = zn (both channels of the pair)
   auto emit = [&](int k, float2 zk, float2 zn) {
     if (k >= Kw) return;
     float sc = 0.5f * scale;
     if (alpha_weight && k != 0 && 2 * k != W) sc *= 2.f;
-    *(float4*)(Srow + (size_t)k * C) = make_float4(sc * (zk.x + zn.x), sc * (zk.y - zn.y), sc * (zk.y + zn.y), -sc * (zk.x - zn.x));
+    SpecIO<ST>::stpair(Srow + (size_t)k * C, make_float2(sc * (zk.x + zn.x), sc * (zk.y - zn.y)),
+                       make_float2(sc * (zk.y + zn.y), -sc * (zk.x - zn.x)));
   };
   // work items: k1 = 0 alone, k1 = N1 / 2 alone (N1 even), pairs (k1, N1 - k1)
   constexpr int kItems = N1 / 2 + 1;
@@ -223,9 +232,9 @@ k_wfft_fwd2(const T* __restrict__ x, float2* __restrict__ S, const float2* __res
 
 // ---- F8 + F9 / B8: W-direction complex-to-real inverse FFT, residual, store ------------------------------------------
 // grid (C / (2 LW), H, B), block 32 NW; smem W * LW float2
-template <typename T, int N1, int N2, int NW, int LW>
+template <typename T, int N1, int N2, int NW, int LW, typename ST>
 __global__ void __launch_bounds__(32 * NW, LW == 32 ? 2 : 1)
-k_wfft_inv2(const float2* __restrict__ S, const T* __restrict__ res, T* __restrict__ out, const float2* __restrict__ tw, int H,
+k_wfft_inv2(const ST* __restrict__ S, const T* __restrict__ res, T* __restrict__ out, const float2* __restrict__ tw, int H,
             int C, int Kw, float scale, int half_interior) {
   constexpr int W = N1 * N2, TPW = 32 / LW, NSLOT = NW * TPW;
   extern __shared__ float2 smem[];
@@ -233,23 +242,24 @@ k_wfft_inv2(const float2* __restrict__ S, const T* __restrict__ res, T* __restri
   const int l = lane % LW, slot = warp * TPW + lane / LW;
   const int h = blockIdx.y, b = blockIdx.z;
   const int c = blockIdx.x * (2 * LW) + 2 * l;
-  const float2* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
+  const ST* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
   // every stored bin kk <= W/2 feeds the transform twice: as z[kk] and, conjugated (Hermitian extension), as z[W - kk]
   {
     constexpr int PER = (W / 2 + NSLOT) / NSLOT, LB = PER < kF2MaxBatch ? PER : kF2MaxBatch;
     for (int k0 = slot; k0 <= W / 2; k0 += NSLOT * LB) {
-      float4 t[LB];
+      typename SpecIO<ST>::pair_t t[LB];
 #pragma unroll
       for (int u = 0; u < LB; ++u) {
         const int kk = k0 + u * NSLOT;
-        t[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (kk < Kw) t[u] = __ldg((const float4*)(Srow + (size_t)kk * C));
+        t[u] = typename SpecIO<ST>::pair_t{};
+        if (kk < Kw) t[u] = SpecIO<ST>::ldpair(Srow + (size_t)kk * C);
       }
 #pragma unroll
       for (int u = 0; u < LB; ++u) {
         const int kk = k0 + u * NSLOT;
         if (kk > W / 2) continue;
-        float2 ta = make_float2(t[u].x, t[u].y), tb = make_float2(t[u].z, t[u].w);
+        float2 ta, tb;
+        SpecIO<ST>::unpair(t[u], ta, tb);
         if (kk == 0 || 2 * kk == W) {
           ta.y = 0.f;   // reading A4: imaginary parts of the c = 0 and c = W/2 columns are discarded
           tb.y = 0.f;

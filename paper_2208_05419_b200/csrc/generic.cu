@@ -546,77 +546,90 @@ cudaError_t set_smem(K kernel, size_t bytes) {
   return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
-template <typename T>
-void launch_wfft_fwd(Launcher& L, const Geometry& g, const Plan& p, const T* x, float2* S, bool alpha) {
+template <typename T, typename ST = float2>
+void launch_wfft_fwd(Launcher& L, const Geometry& g, const Plan& p, const T* x, ST* S, bool alpha) {
   if (L.err != cudaSuccess) return;
   if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2, auto nw, auto narrow) {
         constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value, NW = decltype(nw)::value;
         constexpr int LW = decltype(narrow)::value ? 16 : 32;
         const size_t smem2 = (size_t)g.W * LW * sizeof(float2);
-        L.err = set_smem(k_wfft_fwd2<T, N1, N2, NW, LW>, smem2);
+        L.err = set_smem(k_wfft_fwd2<T, N1, N2, NW, LW, ST>, smem2);
         if (L.err != cudaSuccess) return;
         L.begin("k_wfft_fwd");
-        k_wfft_fwd2<T, N1, N2, NW, LW><<<dim3(g.C / (2 * LW), g.H, g.B), 32 * NW, smem2, L.st>>>(x, S, p.fw.tw, g.H, g.C, g.Kw,
+        k_wfft_fwd2<T, N1, N2, NW, LW, ST><<<dim3(g.C / (2 * LW), g.H, g.B), 32 * NW, smem2, L.st>>>(x, S, p.fw.tw, g.H, g.C, g.Kw,
                                                                                                 g.scale, alpha ? 1 : 0);
         L.check();
       }))
     return;
-  const size_t smem = (size_t)g.W * kLanes * sizeof(float2);
-  L.err = set_smem(k_wfft_fwd<T>, smem);
-  if (L.err != cudaSuccess) return;
-  dim3 grid((g.C + 63) / 64, g.H, g.B), block(kLanes, kWfftWarps);
-  L.begin("k_wfft_fwd");
-  k_wfft_fwd<T><<<grid, block, smem, L.st>>>(x, S, p.fw, g.H, g.W, g.C, g.Kw, g.scale, alpha ? 1 : 0);
-  L.check();
+  if constexpr (std::is_same<ST, float2>::value) {
+    const size_t smem = (size_t)g.W * kLanes * sizeof(float2);
+    L.err = set_smem(k_wfft_fwd<T>, smem);
+    if (L.err != cudaSuccess) return;
+    dim3 grid((g.C + 63) / 64, g.H, g.B), block(kLanes, kWfftWarps);
+    L.begin("k_wfft_fwd");
+    k_wfft_fwd<T><<<grid, block, smem, L.st>>>(x, S, p.fw, g.H, g.W, g.C, g.Kw, g.scale, alpha ? 1 : 0);
+    L.check();
+  } else {
+    L.err = cudaErrorInvalidValue;   // the bf16 spectrum exists on the two-pass kernels only (spec16() guarantees them)
+  }
 }
 
-void launch_hfft(Launcher& L, const Geometry& g, const Plan& p, float2* S, int C, bool inverse) {
+template <typename ST = float2>
+void launch_hfft(Launcher& L, const Geometry& g, const Plan& p, ST* S, int C, bool inverse) {
   if (L.err != cudaSuccess) return;
   if (C % 64 == 0 && fft2_dispatch(g.H, [&](auto n1, auto n2, auto, auto narrow) {
         constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value, G = decltype(narrow)::value ? 1 : 2;
         const size_t smem2 = (size_t)g.H * 32 * G * sizeof(float2);
-        L.err = inverse ? set_smem(k_hfft2<N1, N2, +1, G>, smem2) : set_smem(k_hfft2<N1, N2, -1, G>, smem2);
+        L.err = inverse ? set_smem(k_hfft2<N1, N2, +1, G, ST>, smem2) : set_smem(k_hfft2<N1, N2, -1, G, ST>, smem2);
         if (L.err != cudaSuccess) return;
         L.begin("k_hfft");
         const dim3 grid(C / (32 * G), g.Kw, g.B);
-        if (inverse) k_hfft2<N1, N2, +1, G><<<grid, 32 * kF2Warps, smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
-        else k_hfft2<N1, N2, -1, G><<<grid, 32 * kF2Warps, smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
+        if (inverse) k_hfft2<N1, N2, +1, G, ST><<<grid, 32 * kF2Warps, smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
+        else k_hfft2<N1, N2, -1, G, ST><<<grid, 32 * kF2Warps, smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
         L.check();
       }))
     return;
-  const size_t smem = (size_t)g.H * kLanes * sizeof(float2);
-  L.err = set_smem(k_hfft, smem);
-  if (L.err != cudaSuccess) return;
-  dim3 grid((C + kLanes - 1) / kLanes, g.Kw, g.B), block(kLanes, kFftWarps);
-  L.begin("k_hfft");
-  k_hfft<<<grid, block, smem, L.st>>>(S, p.fh, g.H, g.Kw, C, inverse ? +1.f : -1.f);
-  L.check();
+  if constexpr (std::is_same<ST, float2>::value) {
+    const size_t smem = (size_t)g.H * kLanes * sizeof(float2);
+    L.err = set_smem(k_hfft, smem);
+    if (L.err != cudaSuccess) return;
+    dim3 grid((C + kLanes - 1) / kLanes, g.Kw, g.B), block(kLanes, kFftWarps);
+    L.begin("k_hfft");
+    k_hfft<<<grid, block, smem, L.st>>>(S, p.fh, g.H, g.Kw, C, inverse ? +1.f : -1.f);
+    L.check();
+  } else {
+    L.err = cudaErrorInvalidValue;
+  }
 }
 
-template <typename T>
-void launch_wfft_inv(Launcher& L, const Geometry& g, const Plan& p, const float2* S, const T* res, T* out,
+template <typename T, typename ST = float2>
+void launch_wfft_inv(Launcher& L, const Geometry& g, const Plan& p, const ST* S, const T* res, T* out,
                      bool half_interior) {
   if (L.err != cudaSuccess) return;
   if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2, auto nw, auto narrow) {
         constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value, NW = decltype(nw)::value;
         constexpr int LW = decltype(narrow)::value ? 16 : 32;
         const size_t smem2 = (size_t)g.W * LW * sizeof(float2);
-        L.err = set_smem(k_wfft_inv2<T, N1, N2, NW, LW>, smem2);
+        L.err = set_smem(k_wfft_inv2<T, N1, N2, NW, LW, ST>, smem2);
         if (L.err != cudaSuccess) return;
         L.begin("k_wfft_inv");
-        k_wfft_inv2<T, N1, N2, NW, LW><<<dim3(g.C / (2 * LW), g.H, g.B), 32 * NW, smem2, L.st>>>(S, res, out, p.fw.tw, g.H, g.C, g.Kw,
+        k_wfft_inv2<T, N1, N2, NW, LW, ST><<<dim3(g.C / (2 * LW), g.H, g.B), 32 * NW, smem2, L.st>>>(S, res, out, p.fw.tw, g.H, g.C, g.Kw,
                                                                                                 g.scale, half_interior ? 1 : 0);
         L.check();
       }))
     return;
-  const size_t smem = (size_t)g.W * kLanes * sizeof(float2);
-  L.err = set_smem(k_wfft_inv<T>, smem);
-  if (L.err != cudaSuccess) return;
-  dim3 grid((g.C + 63) / 64, g.H, g.B), block(kLanes, kWfftWarps);
-  L.begin("k_wfft_inv");
-  k_wfft_inv<T><<<grid, block, smem, L.st>>>(S, res, out, p.fw, g.H, g.W, g.C, g.Kw, g.scale,
-                                           half_interior ? 1 : 0);
-  L.check();
+  if constexpr (std::is_same<ST, float2>::value) {
+    const size_t smem = (size_t)g.W * kLanes * sizeof(float2);
+    L.err = set_smem(k_wfft_inv<T>, smem);
+    if (L.err != cudaSuccess) return;
+    dim3 grid((g.C + 63) / 64, g.H, g.B), block(kLanes, kWfftWarps);
+    L.begin("k_wfft_inv");
+    k_wfft_inv<T><<<grid, block, smem, L.st>>>(S, res, out, p.fw, g.H, g.W, g.C, g.Kw, g.scale,
+                                             half_interior ? 1 : 0);
+    L.check();
+  } else {
+    L.err = cudaErrorInvalidValue;
+  }
 }
 
 template <int EPI>
@@ -673,6 +686,12 @@ struct GenericWs {
   size_t total;
 };
 
+// Hybrid path with every transform on the two-pass kernels: the spectra between the kernels are stored as bf16 complex
+// (half the HBM traffic of the path's five round trips; the arithmetic stays fp32, the MLP operands are bf16 anyway).
+bool spec16(const Geometry& g) {
+  return tc_mlp_supported(g) && fft2_has(g.H) && fft2_has(g.W) && g.C % 64 == 0;
+}
+
 GenericWs carve(const Geometry& g, bool backward, char* base, size_t mask_region) {
   GenericWs w{};
   size_t off = mask_region;
@@ -682,10 +701,11 @@ GenericWs carve(const Geometry& g, bool backward, char* base, size_t mask_region
     return p;
   };
   const size_t rows = (size_t)g.rows();
-  w.Xh = take(rows * g.C);
+  const size_t spec_elems = spec16(g) ? (rows * g.C + 1) / 2 : rows * g.C;   // in units of float2
+  w.Xh = take(spec_elems);
   if (backward && tc_mlp_bwd_supported(g)) {
     // hybrid backward: the two spectra and the tensor-core MLP's own region (weight images, operand images, partial sums)
-    w.G = take(rows * g.C);
+    w.G = take(spec_elems);
     w.mlp = take((tc_mlp_bwd_workspace_bytes(g) + sizeof(float2) - 1) / sizeof(float2));
     w.total = off;
     return w;
@@ -718,11 +738,21 @@ cudaError_t forward_t(const Geometry& g, const Plan& p, const T* x, const float*
                       const float* w2, const float* b2, T* y, void* ws, cudaStream_t st) {
   GenericWs w = carve(g, false, (char*)ws, 0);
   Launcher L{st};
+  if (spec16(g)) {
+    // hybrid path, bf16 spectra: F1, F2 (two-pass fp32 FFTs), F3-F6 on the tensor cores in place, F7, F8 + F9
+    SpecBf16* S = (SpecBf16*)w.Xh;
+    launch_wfft_fwd<T, SpecBf16>(L, g, p, x, S, false);
+    launch_hfft<SpecBf16>(L, g, p, S, g.C, false);
+    if (L.err == cudaSuccess) L.err = tc_mlp_forward(g, S, true, w1, b1, w2, b2, w.mlp, L.st);
+    launch_hfft<SpecBf16>(L, g, p, S, g.C, true);
+    launch_wfft_inv<T, SpecBf16>(L, g, p, S, g.no_residual ? nullptr : x, y, false);
+    return L.err;
+  }
   launch_wfft_fwd<T>(L, g, p, x, w.Xh, false);                                      // F1
   launch_hfft(L, g, p, w.Xh, g.C, false);                                           // F2
   if (w.mlp != nullptr) {
     // hybrid path (bf16 activations): F3-F6 on the tensor cores, in place on the spectrum
-    if (L.err == cudaSuccess) L.err = tc_mlp_forward(g, w.Xh, w1, b1, w2, b2, w.mlp, L.st);
+    if (L.err == cudaSuccess) L.err = tc_mlp_forward(g, w.Xh, false, w1, b1, w2, b2, w.mlp, L.st);
   } else {
     launch_gemm<EPI_RELU>(L, g, w.Xh, g.C, (const float2*)w1, (const float2*)b1, w.O1, g.CH, nullptr, 0,
                           g.bs, g.hid);                                             // F3, F4
@@ -749,14 +779,26 @@ cudaError_t backward_t(const Geometry& g, const Plan& p, const T* x, const T* dy
   if (tc_mlp_bwd_supported(g)) {
     // hybrid path (bf16 activations, hidden factor 1): transforms as fp32 FFTs, rows B1 (second half) and B3-B7 on
     // the tensor cores (tc_mlp_bwd, tc_wgrad), GX replaces G in place
+    uint8_t* mk1 = g.export_masks ? (uint8_t*)ws : nullptr;
+    uint8_t* mk2 = g.export_masks ? (uint8_t*)ws + m2off : nullptr;
+    if (spec16(g)) {
+      SpecBf16 *SX = (SpecBf16*)w.Xh, *SG = (SpecBf16*)w.G;
+      launch_wfft_fwd<T, SpecBf16>(L, g, p, x, SX, false);
+      launch_hfft<SpecBf16>(L, g, p, SX, g.C, false);
+      launch_wfft_fwd<T, SpecBf16>(L, g, p, dy, SG, true);
+      launch_hfft<SpecBf16>(L, g, p, SG, g.C, false);
+      if (L.err == cudaSuccess && g.export_masks) L.err = cudaMemsetAsync(ws, 0, mask_region, st);
+      if (L.err == cudaSuccess) L.err = tc_mlp_backward(g, SX, SG, true, w1, b1, w2, b2, dw1, db1, dw2, db2, mk1, mk2, w.mlp, st);
+      launch_hfft<SpecBf16>(L, g, p, SG, g.C, true);
+      launch_wfft_inv<T, SpecBf16>(L, g, p, SG, g.no_residual ? nullptr : dy, dx, true);
+      return L.err;
+    }
     launch_wfft_fwd<T>(L, g, p, x, w.Xh, false);
     launch_hfft(L, g, p, w.Xh, g.C, false);
     launch_wfft_fwd<T>(L, g, p, dy, w.G, true);
     launch_hfft(L, g, p, w.G, g.C, false);
     if (L.err == cudaSuccess && g.export_masks) L.err = cudaMemsetAsync(ws, 0, mask_region, st);
-    if (L.err == cudaSuccess)
-      L.err = tc_mlp_backward(g, w.Xh, w.G, w1, b1, w2, b2, dw1, db1, dw2, db2, g.export_masks ? (uint8_t*)ws : nullptr,
-                              g.export_masks ? (uint8_t*)ws + m2off : nullptr, w.mlp, st);
+    if (L.err == cudaSuccess) L.err = tc_mlp_backward(g, w.Xh, w.G, false, w1, b1, w2, b2, dw1, db1, dw2, db2, mk1, mk2, w.mlp, st);
     launch_hfft(L, g, p, w.G, g.C, true);
     launch_wfft_inv<T>(L, g, p, w.G, g.no_residual ? nullptr : dy, dx, true);
     return L.err;

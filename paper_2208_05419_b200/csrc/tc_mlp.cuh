@@ -15,11 +15,13 @@ constexpr int kMlpThreads = 256;
 constexpr int kMlpRows = 128;
 constexpr uint32_t kMlpALbo = kMlpRows * 16 + 16, kMlpASbo = 128;   // K-major A [128 x 192]: k-chunk stride padded by 16 B
 constexpr uint32_t kMlpABytes = (NT / 8) * kMlpALbo;                // 49,536
-constexpr uint32_t kMlpStageBytes = kMlpRows * BS * 8;              // 98,304: [128 rows][96 float2]
-constexpr uint32_t kMlpSmem = 4 * kWBytes + kMlpABytes + kMlpStageBytes;   // 221,568
+template <typename ST>
+constexpr uint32_t mlp_stage_bytes() { return kMlpRows * BS * (uint32_t)sizeof(ST); }   // 98,304 (fp32) / 49,152 (bf16): [128 rows][96 complex]
+template <typename ST>
+constexpr uint32_t mlp_fwd_smem() { return 4 * kWBytes + kMlpABytes + mlp_stage_bytes<ST>(); }   // 221,568 / 172,416
 
 struct MlpParams {
-  float2* X;                 // [rows][C] fp32 complex, transformed in place
+  void* X;                   // [rows][C] complex (fp32 or bf16: the kernel's ST), transformed in place
   const uint8_t* wprep;      // per group 4 x kWBytes: W1r, W1i, W2r, W2i
   const float* bprep;        // per group [2 layers][192]
   long long rows;
@@ -27,8 +29,168 @@ struct MlpParams {
   float lambda;
 };
 
+// ---- pieces shared by the kernels of the hybrid path -------------------------------------------------------------------------
+// ST = storage type of the spectrum (afno_internal.h): float2 (fp32 complex) or SpecBf16 (bf16 complex, used when every
+// transform of the call runs through the two-pass FFT kernels).
+
+// 8 adjacent complex channels (at `src`, global or shared memory) -> bf16 (re x 8, im x 8)
+template <typename ST>
+__device__ __forceinline__ void mlp_pack8(const ST* src, uint4& re, uint4& im);
+template <>
+__device__ __forceinline__ void mlp_pack8<float2>(const float2* src, uint4& re, uint4& im) {
+  const float4* s4 = (const float4*)src;
+  const float4 a = s4[0], b = s4[1], c = s4[2], d = s4[3];
+  re = make_uint4(pack_bf16(a.x, a.z), pack_bf16(b.x, b.z), pack_bf16(c.x, c.z), pack_bf16(d.x, d.z));
+  im = make_uint4(pack_bf16(a.y, a.w), pack_bf16(b.y, b.w), pack_bf16(c.y, c.w), pack_bf16(d.y, d.w));
+}
+template <>
+__device__ __forceinline__ void mlp_pack8<SpecBf16>(const SpecBf16* src, uint4& re, uint4& im) {
+  const uint4* s4 = (const uint4*)src;   // a word = (re, im) of one channel: de-interleave by byte permutes
+  const uint4 a = s4[0], b = s4[1];
+  re = make_uint4(__byte_perm(a.x, a.y, 0x5410), __byte_perm(a.z, a.w, 0x5410), __byte_perm(b.x, b.y, 0x5410), __byte_perm(b.z, b.w, 0x5410));
+  im = make_uint4(__byte_perm(a.x, a.y, 0x7632), __byte_perm(a.z, a.w, 0x7632), __byte_perm(b.x, b.y, 0x7632), __byte_perm(b.z, b.w, 0x7632));
+}
+
+// T (+)= A W (transposed = false) or A W^H (true) as real GEMMs on the (re | im) halves; A = bf16 K-major
+// [96 rows][re 96 | im 96] in shared memory (chunk of 8 columns = kTileSbo bytes), W = the images of one 96 x 96 block
+// (read as MN-major operands with the negate bit for the conjugate transpose); acc0 = 1 keeps what D holds.
+__device__ __forceinline__ void mlp_issue_gemm(uint32_t D, uint32_t aA, uint32_t wr, uint32_t wi, bool transposed, uint32_t acc0,
+                                               uint64_t* bar) {
+  const uint32_t id = idesc_bf16(128, BS, transposed ? kIdescBMn : 0u);
+  const uint32_t lbo = transposed ? kWSbo : kWLbo, sbo = transposed ? kWLbo : kWSbo;
+#pragma unroll
+  for (int ks = 0; ks < BS / 16; ++ks) {
+    const uint64_t ad = smem_desc(aA + ks * 2 * kTileSbo, kTileSbo, kTileLbo);
+    mma_ss(D, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, acc0 | (uint32_t)(ks != 0));
+    mma_ss(D + BS, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? (id | kIdescNegB) : id, acc0 | (uint32_t)(ks != 0));
+  }
+#pragma unroll
+  for (int ks = 0; ks < BS / 16; ++ks) {
+    const uint64_t ad = smem_desc(aA + (BS / 8 + ks * 2) * kTileSbo, kTileSbo, kTileLbo);
+    mma_ss(D, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? id : (id | kIdescNegB), 1u);
+    mma_ss(D + BS, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, 1u);
+  }
+  mma_commit(bar);
+}
+// ROWS complex rows of one channel group -> bf16 K-major operand buffer (chunk of 8 columns = STRIDE bytes); lanes run
+// over the 8-channel chunks of a row.  Rows past `rows` and channels past `nch` become zero.  mask2 != nullptr: the
+// softshrink mask of the row ({re bits 0..31, re 32..47, im 0..31, im 32..47} per row and 48-channel half) is applied.
+template <int ROWS, uint32_t STRIDE, typename ST>
+__device__ __forceinline__ void mlp_load_operand(const ST* __restrict__ src_rows, long long r0, long long rows, int C, int ch0, int nch,
+                                                 uint8_t* dstbuf, const uint4 (*mask2)[2], int tid) {
+  for (uint32_t u = tid; u < ROWS * (BS / 8); u += kMlpThreads) {
+    const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
+    uint4 re = make_uint4(0, 0, 0, 0), im = re;
+    if (r0 + rr < rows && 8 * c8 < nch) mlp_pack8<ST>(src_rows + (size_t)(r0 + rr) * C + ch0 + 8 * c8, re, im);
+    if (mask2 != nullptr) {
+      const uint4 mk = mask2[rr][c8 / 6];
+      const int sh = (c8 % 6) * 8;
+      const uint32_t mre = (uint32_t)((((uint64_t)mk.y << 32) | mk.x) >> sh) & 0xFFu;
+      const uint32_t mim = (uint32_t)((((uint64_t)mk.w << 32) | mk.z) >> sh) & 0xFFu;
+      auto sel = [](uint32_t v, uint32_t bits) {   // bits: bit 0 -> low half, bit 1 -> high half
+        return v & ((bits & 1u ? 0x0000FFFFu : 0u) | (bits & 2u ? 0xFFFF0000u : 0u));
+      };
+      re = make_uint4(sel(re.x, mre), sel(re.y, mre >> 2), sel(re.z, mre >> 4), sel(re.w, mre >> 6));
+      im = make_uint4(sel(im.x, mim), sel(im.y, mim >> 2), sel(im.z, mim >> 4), sel(im.w, mim >> 6));
+    }
+    uint8_t* dst = dstbuf + (size_t)rr * 16;
+    *(uint4*)(dst + (size_t)c8 * STRIDE) = re;
+    *(uint4*)(dst + (size_t)(BS / 8 + c8) * STRIDE) = im;
+  }
+}
+// 48 accumulator columns of this thread's row (the caller waits with tmem_wait_ld)
+__device__ __forceinline__ void mlp_ld48(uint32_t taddr, uint32_t (&v)[48]) {
+  tmem_ld16<0>(taddr, v);
+  tmem_ld16<16>(taddr + 16, v);
+  tmem_ld16<32>(taddr + 32, v);
+}
+// O1 = relu(v + bias) of 48 columns -> six 16-byte pieces of the operand buffer; returns the ReLU mask bits
+__device__ __forceinline__ uint64_t mlp_relu_store(const uint32_t (&v)[48], const float* bias, uint8_t* dst) {
+  uint64_t m = 0;
+#pragma unroll
+  for (int g = 0; g < 6; ++g) {
+    uint32_t pk[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const float lo = __uint_as_float(v[8 * g + 2 * e]) + bias[8 * g + 2 * e];
+      const float hi = __uint_as_float(v[8 * g + 2 * e + 1]) + bias[8 * g + 2 * e + 1];
+      m |= (uint64_t)(lo > 0.f) << (8 * g + 2 * e);
+      m |= (uint64_t)(hi > 0.f) << (8 * g + 2 * e + 1);
+      pk[e] = pack_relu_bf16(lo, hi);
+    }
+    *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+  }
+  return m;
+}
+// G1 = mask (.) v of 48 columns -> operand buffer
+__device__ __forceinline__ void mlp_masked_store(const uint32_t (&v)[48], uint64_t m, uint8_t* dst) {
+#pragma unroll
+  for (int g = 0; g < 6; ++g) {
+    uint32_t pk[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const int c = 8 * g + 2 * e;
+      const float lo = ((m >> c) & 1u) ? __uint_as_float(v[c]) : 0.f;
+      const float hi = ((m >> (c + 1)) & 1u) ? __uint_as_float(v[c + 1]) : 0.f;
+      pk[e] = pack_bf16(lo, hi);
+    }
+    *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+  }
+}
+// softshrink mask bits of 48 columns: |v + bias| > lambda on kept rows
+__device__ __forceinline__ uint64_t mlp_shrink_mask(const uint32_t (&v)[48], const float* bias, float lam, bool kept) {
+  uint64_t m = 0;
+#pragma unroll
+  for (int c = 0; c < 48; ++c) m |= (uint64_t)(kept && fabsf(__uint_as_float(v[c]) + bias[c]) > lam) << c;
+  return m;
+}
+// complex values (re in vr, im in vi: 48 channels of this thread's row, fp32 bits) -> rows of the spectrum G: each warp
+// transposes its 32 rows through a private slice of an idle operand buffer (16 channels per pass, padded row pitch) and
+// stores 128 (fp32) / 64 (bf16) contiguous bytes per row
+template <typename ST>
+__device__ __forceinline__ void mlp_store_rows(const uint32_t (&vr)[48], const uint32_t (&vi)[48], uint8_t* scratch, ST* G,
+                                               long long wrow0, long long rows, int C, int chg, int nch, int lane) {
+  constexpr uint32_t kRow = 16 * sizeof(ST), kPitch = kRow + 16, kPieces = kRow / 16, kCpp = 16 / sizeof(ST);   // channels per 16-byte piece
+#pragma unroll
+  for (int pass = 0; pass < 3; ++pass) {
+#pragma unroll
+    for (int c = 0; c < 16; c += 2) {
+      const int cc = pass * 16 + c;
+      SpecIO<ST>::stpair((ST*)(scratch + lane * kPitch) + c, make_float2(__uint_as_float(vr[cc]), __uint_as_float(vi[cc])),
+                         make_float2(__uint_as_float(vr[cc + 1]), __uint_as_float(vi[cc + 1])));
+    }
+    __syncwarp();
+    const int chp = pass * 16;   // first channel of this pass within the thread's 48
+#pragma unroll
+    for (int it = 0; it < (int)kPieces; ++it) {
+      const int id = it * 32 + lane, rr = id / (int)kPieces, piece = id % (int)kPieces;
+      const uint4 o = *(const uint4*)(scratch + rr * kPitch + piece * 16);
+      if (wrow0 + rr < rows && chg + chp + (int)kCpp * piece < nch)
+        *(uint4*)(G + (size_t)(wrow0 + rr) * C + chg + chp + kCpp * piece) = o;
+    }
+    __syncwarp();
+  }
+}
+// Z = softshrink(P2 + b2) on the fp32 sum (reading A15), zero on truncated rows, in place in the accumulator registers
+__device__ __forceinline__ void mlp_shrink48(uint32_t (&vr)[48], uint32_t (&vi)[48], const float* bre, const float* bim, float lam,
+                                             bool kept) {
+#pragma unroll
+  for (int c = 0; c < 48; ++c) {
+    const float t0 = __uint_as_float(vr[c]) + bre[c], t1 = __uint_as_float(vi[c]) + bim[c];
+    vr[c] = __float_as_uint(kept ? t0 - fminf(fmaxf(t0, -lam), lam) : 0.f);
+    vi[c] = __float_as_uint(kept ? t1 - fminf(fmaxf(t1, -lam), lam) : 0.f);
+  }
+}
+// activation masks of this thread's 48 channels -> [..][C'][2] bytes (parity tests)
+__device__ __forceinline__ void mlp_export_mask(uint8_t* dst, uint64_t mre, uint64_t mim, int nvalid) {
+  for (int c = 0; c < 48; ++c)
+    if (c < nvalid) *(uchar2*)(dst + 2 * c) = make_uchar2((unsigned char)((mre >> c) & 1u), (unsigned char)((mim >> c) & 1u));
+}
+
+template <typename ST>
 __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd(const MlpParams p, int S) {
   extern __shared__ __align__(1024) uint8_t smem[];
+  ST* const X = (ST*)p.X;
   __shared__ __align__(8) uint64_t done[2];
   __shared__ uint32_t tmem_slot;
   __shared__ __align__(16) float sBias[2 * NT];
@@ -54,14 +216,15 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd(const MlpParams p, 
     for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMlpThreads) cp_async16(smem_u32(sW) + i * 16, wsrc + (size_t)i * 16);
   }
   for (int i = tid; i < 2 * NT; i += kMlpThreads) sBias[i] = p.bprep[(size_t)j * 2 * NT + i];
-  // staging loads of one tile: 16-byte pieces, a row of the group is nch * 8 contiguous bytes; pieces past the last
-  // row or the last channel are zero-filled (cp.async with src-size 0)
+  // staging loads of one tile: 16-byte pieces, a row of the group is nch * sizeof(ST) contiguous bytes; pieces past the
+  // last row or the last channel are zero-filled (cp.async with src-size 0)
+  constexpr int kCpp = 16 / sizeof(ST), kPpr = BS / kCpp;   // channels per piece, pieces per row
   auto stage_tile = [&](long long t) {
     const long long r0 = t * kMlpRows;
-    for (uint32_t i = tid; i < kMlpStageBytes / 16; i += kMlpThreads) {
-      const int r = i / (BS / 2), c2 = i - r * (BS / 2);       // piece = 2 channels
-      const bool ok = (r0 + r < p.rows) && (2 * c2 < nch);
-      const float2* src = p.X + (size_t)(ok ? r0 + r : 0) * p.C + ch0 + (ok ? 2 * c2 : 0);
+    for (uint32_t i = tid; i < mlp_stage_bytes<ST>() / 16; i += kMlpThreads) {
+      const int r = i / kPpr, c2 = i - r * kPpr;
+      const bool ok = (r0 + r < p.rows) && (kCpp * c2 < nch);
+      const ST* src = X + (size_t)(ok ? r0 + r : 0) * p.C + ch0 + (ok ? kCpp * c2 : 0);
       asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(sStage) + i * 16), "l"(src), "r"(ok ? 16 : 0)
                    : "memory");
     }
@@ -100,14 +263,12 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd(const MlpParams p, 
   };
   for (long long t = s0; t < ntiles; t += S) {
     const long long r0 = t * kMlpRows;
-    // ---- staging (fp32 complex) -> bf16 A operand: unit = (row, 8 channels); lanes run over the channel chunks ----
+    // ---- staging -> bf16 A operand: unit = (row, 8 channels); lanes run over the channel chunks ----
     for (uint32_t u = tid; u < kMlpRows * (BS / 8); u += kMlpThreads) {
       const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
-      const float4* src = (const float4*)(sStage + (size_t)rr * (BS * 8) + c8 * 64);
-      const float4 a = src[0], b = src[1], c = src[2], d = src[3];
-      const uint4 re = make_uint4(pack_bf16(a.x, a.z), pack_bf16(b.x, b.z), pack_bf16(c.x, c.z), pack_bf16(d.x, d.z));
-      const uint4 im = make_uint4(pack_bf16(a.y, a.w), pack_bf16(b.y, b.w), pack_bf16(c.y, c.w), pack_bf16(d.y, d.w));
-      uint8_t* dst = sA + (size_t)(rr >> 3) * kMlpASbo + (rr & 7) * 16;
+      uint4 re, im;
+      mlp_pack8<ST>((const ST*)sStage + (size_t)rr * BS + 8 * c8, re, im);
+      uint8_t* dst = sA + (size_t)rr * 16;
       *(uint4*)(dst + (size_t)c8 * kMlpALbo) = re;
       *(uint4*)(dst + (size_t)(BS / 8 + c8) * kMlpALbo) = im;
     }
@@ -153,53 +314,20 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd(const MlpParams p, 
     __syncwarp();
     mbar_wait(&done[1], ph);
     tc_fence_after();
-    // ---- Z = softshrink(P2 + b2) on the fp32 sum, zero on truncated rows -> fp32 complex, in place ----
+    // ---- Z = softshrink(P2 + b2) on the fp32 sum, zero on truncated rows -> spectrum rows, in place ----
     {
       uint32_t vr[48], vi[48];
-      tmem_ld16<0>(D2 + lane_sel + chalf * 48, vr);
-      tmem_ld16<16>(D2 + lane_sel + chalf * 48 + 16, vr);
-      tmem_ld16<32>(D2 + lane_sel + chalf * 48 + 32, vr);
-      tmem_ld16<0>(D2 + lane_sel + BS + chalf * 48, vi);
-      tmem_ld16<16>(D2 + lane_sel + BS + chalf * 48 + 16, vi);
-      tmem_ld16<32>(D2 + lane_sel + BS + chalf * 48 + 32, vi);
+      mlp_ld48(D2 + lane_sel + chalf * 48, vr);
+      mlp_ld48(D2 + lane_sel + BS + chalf * 48, vi);
       tmem_wait_ld();
       const long long row = r0 + r;
       const int h = (int)((row / p.Kw) % p.H);
       const bool kept = row < p.rows && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
-      const float lam = p.lambda;
       const float* bre = sBias + NT + chalf * 48;
-      const float* bim = bre + BS;
-      // A thread holds one ROW (48 channels); written straight to global memory a warp instruction would touch 32
-      // rows with 16 bytes each.  The warp transposes through its private slice of the (now idle) A buffer
-      // instead, 16 channels per pass (row pitch 144 B: conflict-free), and stores 128 contiguous bytes per row.
-      constexpr uint32_t kPitch = 16 * 8 + 16;
-      uint8_t* scratch = sA + (size_t)warp * (kMlpABytes / 8 / 16 * 16);
-      const long long wrow0 = r0 + q * 32;       // first row of this warp
-#pragma unroll
-      for (int pass = 0; pass < 3; ++pass) {
-#pragma unroll
-        for (int c = 0; c < 16; c += 2) {
-          const int cc = pass * 16 + c;
-          float4 o;
-          const float t0 = __uint_as_float(vr[cc]) + bre[cc], t1 = __uint_as_float(vi[cc]) + bim[cc];
-          const float t2 = __uint_as_float(vr[cc + 1]) + bre[cc + 1], t3 = __uint_as_float(vi[cc + 1]) + bim[cc + 1];
-          o.x = kept ? t0 - fminf(fmaxf(t0, -lam), lam) : 0.f;
-          o.y = kept ? t1 - fminf(fmaxf(t1, -lam), lam) : 0.f;
-          o.z = kept ? t2 - fminf(fmaxf(t2, -lam), lam) : 0.f;
-          o.w = kept ? t3 - fminf(fmaxf(t3, -lam), lam) : 0.f;
-          *(float4*)(scratch + lane * kPitch + c * 8) = o;
-        }
-        __syncwarp();
-        const int chp = chalf * 48 + pass * 16;   // first channel (within the group) of this pass
-#pragma unroll
-        for (int it = 0; it < 8; ++it) {
-          const int id = it * 32 + lane, rr = id >> 3, piece = id & 7;
-          const float4 o = *(const float4*)(scratch + rr * kPitch + piece * 16);
-          if (wrow0 + rr < p.rows && chp + 2 * piece < nch)
-            *(float4*)(p.X + (size_t)(wrow0 + rr) * p.C + ch0 + chp + 2 * piece) = o;
-        }
-        __syncwarp();
-      }
+      mlp_shrink48(vr, vi, bre, bre + BS, p.lambda, kept);
+      // a thread holds one ROW (48 channels): the warp transposes through its private slice of the (now idle) operand
+      // buffer and stores contiguous row segments (mlp_store_rows)
+      mlp_store_rows<ST>(vr, vi, sA + (size_t)warp * (kMlpABytes / 8 / 16 * 16), X + ch0, r0 + q * 32, p.rows, p.C, chalf * 48, nch, lane);
     }
     ph ^= 1u;
     cp_async_wait_all();   // the next tile has landed in the staging buffer
@@ -254,8 +382,10 @@ __global__ void k_tc_prep_weights_hf(const float* __restrict__ w1, const float* 
   base[3 * m + f] = __float2bfloat16_rn(b.y);
 }
 
+template <typename ST>
 __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd_hf(const MlpParams p, int S, int hf) {
   extern __shared__ __align__(1024) uint8_t smem[];
+  ST* const X = (ST*)p.X;
   __shared__ __align__(8) uint64_t done[2];
   __shared__ uint32_t tmem_slot;
   __shared__ __align__(16) float sBias[(kMlpMaxHf + 1) * NT];
@@ -304,20 +434,8 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd_hf(const MlpParams 
   };
   for (long long t = s0; t < ntiles; t += S) {
     const long long r0 = t * kMlpRows;
-    // ---- fp32 complex rows -> bf16 A operand (lanes run over the 8-channel chunks of a row: 768 contiguous bytes) ----
-    for (uint32_t u = tid; u < kMlpRows * (BS / 8); u += kMlpThreads) {
-      const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
-      float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, d = a;
-      if (r0 + rr < p.rows) {
-        const float4* src = (const float4*)(p.X + (size_t)(r0 + rr) * p.C + ch0 + 8 * c8);
-        a = __ldg(src); b = __ldg(src + 1); c = __ldg(src + 2); d = __ldg(src + 3);
-      }
-      const uint4 re = make_uint4(pack_bf16(a.x, a.z), pack_bf16(b.x, b.z), pack_bf16(c.x, c.z), pack_bf16(d.x, d.z));
-      const uint4 im = make_uint4(pack_bf16(a.y, a.w), pack_bf16(b.y, b.w), pack_bf16(c.y, c.w), pack_bf16(d.y, d.w));
-      uint8_t* dst = sAX + (size_t)(rr >> 3) * kMlpASbo + (rr & 7) * 16;
-      *(uint4*)(dst + (size_t)c8 * kMlpALbo) = re;
-      *(uint4*)(dst + (size_t)(BS / 8 + c8) * kMlpALbo) = im;
-    }
+    // ---- spectrum rows -> bf16 A operand (lanes run over the 8-channel chunks of a row) ----
+    mlp_load_operand<kMlpRows, kMlpALbo, ST>(X, r0, p.rows, p.C, ch0, BS, sAX, nullptr, tid);
     for (int hc = 0; hc < hf; ++hc) {
       // the chunk's weight images (the previous chunk's GEMMs have completed: done[1] was awaited)
       const uint8_t* wsrc = p.wprep + ((size_t)j * hf + hc) * 4 * kWBytes;
@@ -366,49 +484,20 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd_hf(const MlpParams 
       tc_fence_after();
       ph ^= 1u;
     }
-    // ---- Z = softshrink(P2 + b2) on the fp32 sum, zero on truncated rows -> fp32 complex, in place ----
+    // ---- Z = softshrink(P2 + b2) on the fp32 sum, zero on truncated rows -> spectrum rows, in place ----
     {
       uint32_t vr[48], vi[48];
-      tmem_ld16<0>(D2 + lane_sel + chalf * 48, vr);
-      tmem_ld16<16>(D2 + lane_sel + chalf * 48 + 16, vr);
-      tmem_ld16<32>(D2 + lane_sel + chalf * 48 + 32, vr);
-      tmem_ld16<0>(D2 + lane_sel + BS + chalf * 48, vi);
-      tmem_ld16<16>(D2 + lane_sel + BS + chalf * 48 + 16, vi);
-      tmem_ld16<32>(D2 + lane_sel + BS + chalf * 48 + 32, vi);
+      mlp_ld48(D2 + lane_sel + chalf * 48, vr);
+      mlp_ld48(D2 + lane_sel + BS + chalf * 48, vi);
       tmem_wait_ld();
       const long long row = r0 + r;
       const int h = (int)((row / p.Kw) % p.H);
       const bool kept = row < p.rows && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
-      const float lam = p.lambda;
       const float* bre = sBias + (size_t)hf * NT + chalf * 48;
-      const float* bim = bre + BS;
-      constexpr uint32_t kPitch = 16 * 8 + 16;
-      uint8_t* scratch = sAO + (size_t)warp * (kMlpABytes / 8 / 16 * 16);   // layer 2 of the last chunk has completed
-      const long long wrow0 = r0 + q * 32;
-#pragma unroll
-      for (int pass = 0; pass < 3; ++pass) {
-#pragma unroll
-        for (int c = 0; c < 16; c += 2) {
-          const int cc = pass * 16 + c;
-          float4 o;
-          const float t0 = __uint_as_float(vr[cc]) + bre[cc], t1 = __uint_as_float(vi[cc]) + bim[cc];
-          const float t2 = __uint_as_float(vr[cc + 1]) + bre[cc + 1], t3 = __uint_as_float(vi[cc + 1]) + bim[cc + 1];
-          o.x = kept ? t0 - fminf(fmaxf(t0, -lam), lam) : 0.f;
-          o.y = kept ? t1 - fminf(fmaxf(t1, -lam), lam) : 0.f;
-          o.z = kept ? t2 - fminf(fmaxf(t2, -lam), lam) : 0.f;
-          o.w = kept ? t3 - fminf(fmaxf(t3, -lam), lam) : 0.f;
-          *(float4*)(scratch + lane * kPitch + c * 8) = o;
-        }
-        __syncwarp();
-        const int chp = chalf * 48 + pass * 16;
-#pragma unroll
-        for (int it = 0; it < 8; ++it) {
-          const int id = it * 32 + lane, rr = id >> 3, piece = id & 7;
-          const float4 o = *(const float4*)(scratch + rr * kPitch + piece * 16);
-          if (wrow0 + rr < p.rows) *(float4*)(p.X + (size_t)(wrow0 + rr) * p.C + ch0 + chp + 2 * piece) = o;
-        }
-        __syncwarp();
-      }
+      mlp_shrink48(vr, vi, bre, bre + BS, p.lambda, kept);
+      // a thread holds one ROW (48 channels): the warp transposes through its private slice of the (now idle) operand
+      // buffer and stores contiguous row segments (mlp_store_rows)
+      mlp_store_rows<ST>(vr, vi, sAO + (size_t)warp * (kMlpABytes / 8 / 16 * 16), X + ch0, r0 + q * 32, p.rows, p.C, chalf * 48, BS, lane);
     }
     tc_fence_before();
     __syncthreads();   // every warp has read its accumulators and left the scratch area: next tile
@@ -417,135 +506,6 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd_hf(const MlpParams 
   tc_fence_before();
   __syncthreads();
   if (warp == 0) tmem_dealloc<512>(tmem);
-}
-
-// ---- pieces shared by the hybrid backward kernels (tc_mlp_bwd, tc_mlp_bwd_hf) -------------------------------------------
-// T (+)= A W (transposed = false) or A W^H (true) as real GEMMs on the (re | im) halves; A = bf16 K-major
-// [96 rows][re 96 | im 96] in shared memory (chunk of 8 columns = kTileSbo bytes), W = the images of one 96 x 96 block
-// (read as MN-major operands with the negate bit for the conjugate transpose); acc0 = 1 keeps what D holds.
-__device__ __forceinline__ void mlp_issue_gemm(uint32_t D, uint32_t aA, uint32_t wr, uint32_t wi, bool transposed, uint32_t acc0,
-                                               uint64_t* bar) {
-  const uint32_t id = idesc_bf16(128, BS, transposed ? kIdescBMn : 0u);
-  const uint32_t lbo = transposed ? kWSbo : kWLbo, sbo = transposed ? kWLbo : kWSbo;
-#pragma unroll
-  for (int ks = 0; ks < BS / 16; ++ks) {
-    const uint64_t ad = smem_desc(aA + ks * 2 * kTileSbo, kTileSbo, kTileLbo);
-    mma_ss(D, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, acc0 | (uint32_t)(ks != 0));
-    mma_ss(D + BS, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? (id | kIdescNegB) : id, acc0 | (uint32_t)(ks != 0));
-  }
-#pragma unroll
-  for (int ks = 0; ks < BS / 16; ++ks) {
-    const uint64_t ad = smem_desc(aA + (BS / 8 + ks * 2) * kTileSbo, kTileSbo, kTileLbo);
-    mma_ss(D, ad, smem_desc(wi + ks * 2 * lbo, lbo, sbo), transposed ? id : (id | kIdescNegB), 1u);
-    mma_ss(D + BS, ad, smem_desc(wr + ks * 2 * lbo, lbo, sbo), id, 1u);
-  }
-  mma_commit(bar);
-}
-// 96 fp32 complex rows of one channel group -> bf16 operand buffer; lanes run over the 8-channel chunks of a row (768
-// contiguous bytes).  Rows past `rows` and channels past `nch` become zero.  mask2 != nullptr: the softshrink mask of
-// the row ({re bits 0..31, re 32..47, im 0..31, im 32..47} per row and 48-channel half) is applied on the way.
-__device__ __forceinline__ void mlp_load_operand(const float2* __restrict__ src_rows, long long r0, long long rows, int C, int ch0,
-                                                 int nch, uint8_t* dstbuf, const uint4 (*mask2)[2], int tid) {
-  for (uint32_t u = tid; u < HP * (BS / 8); u += kMlpThreads) {
-    const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
-    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, d = a;
-    if (r0 + rr < rows && 8 * c8 < nch) {
-      const float4* src = (const float4*)(src_rows + (size_t)(r0 + rr) * C + ch0 + 8 * c8);
-      a = __ldg(src); b = __ldg(src + 1); c = __ldg(src + 2); d = __ldg(src + 3);
-    }
-    uint4 re = make_uint4(pack_bf16(a.x, a.z), pack_bf16(b.x, b.z), pack_bf16(c.x, c.z), pack_bf16(d.x, d.z));
-    uint4 im = make_uint4(pack_bf16(a.y, a.w), pack_bf16(b.y, b.w), pack_bf16(c.y, c.w), pack_bf16(d.y, d.w));
-    if (mask2 != nullptr) {
-      const uint4 mk = mask2[rr][c8 / 6];
-      const int sh = (c8 % 6) * 8;
-      const uint32_t mre = (uint32_t)((((uint64_t)mk.y << 32) | mk.x) >> sh) & 0xFFu;
-      const uint32_t mim = (uint32_t)((((uint64_t)mk.w << 32) | mk.z) >> sh) & 0xFFu;
-      auto sel = [](uint32_t v, uint32_t bits) {   // bits: bit 0 -> low half, bit 1 -> high half
-        return v & ((bits & 1u ? 0x0000FFFFu : 0u) | (bits & 2u ? 0xFFFF0000u : 0u));
-      };
-      re = make_uint4(sel(re.x, mre), sel(re.y, mre >> 2), sel(re.z, mre >> 4), sel(re.w, mre >> 6));
-      im = make_uint4(sel(im.x, mim), sel(im.y, mim >> 2), sel(im.z, mim >> 4), sel(im.w, mim >> 6));
-    }
-    uint8_t* dst = dstbuf + (size_t)rr * 16;
-    *(uint4*)(dst + (size_t)c8 * kTileSbo) = re;
-    *(uint4*)(dst + (size_t)(BS / 8 + c8) * kTileSbo) = im;
-  }
-}
-// 48 accumulator columns of this thread's row (the caller waits with tmem_wait_ld)
-__device__ __forceinline__ void mlp_ld48(uint32_t taddr, uint32_t (&v)[48]) {
-  tmem_ld16<0>(taddr, v);
-  tmem_ld16<16>(taddr + 16, v);
-  tmem_ld16<32>(taddr + 32, v);
-}
-// O1 = relu(v + bias) of 48 columns -> six 16-byte pieces of the operand buffer; returns the ReLU mask bits
-__device__ __forceinline__ uint64_t mlp_relu_store(const uint32_t (&v)[48], const float* bias, uint8_t* dst) {
-  uint64_t m = 0;
-#pragma unroll
-  for (int g = 0; g < 6; ++g) {
-    uint32_t pk[4];
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      const float lo = __uint_as_float(v[8 * g + 2 * e]) + bias[8 * g + 2 * e];
-      const float hi = __uint_as_float(v[8 * g + 2 * e + 1]) + bias[8 * g + 2 * e + 1];
-      m |= (uint64_t)(lo > 0.f) << (8 * g + 2 * e);
-      m |= (uint64_t)(hi > 0.f) << (8 * g + 2 * e + 1);
-      pk[e] = pack_relu_bf16(lo, hi);
-    }
-    *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-  }
-  return m;
-}
-// G1 = mask (.) v of 48 columns -> operand buffer
-__device__ __forceinline__ void mlp_masked_store(const uint32_t (&v)[48], uint64_t m, uint8_t* dst) {
-#pragma unroll
-  for (int g = 0; g < 6; ++g) {
-    uint32_t pk[4];
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      const int c = 8 * g + 2 * e;
-      const float lo = ((m >> c) & 1u) ? __uint_as_float(v[c]) : 0.f;
-      const float hi = ((m >> (c + 1)) & 1u) ? __uint_as_float(v[c + 1]) : 0.f;
-      pk[e] = pack_bf16(lo, hi);
-    }
-    *(uint4*)(dst + (size_t)g * kTileSbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-  }
-}
-// softshrink mask bits of 48 columns: |v + bias| > lambda on kept rows
-__device__ __forceinline__ uint64_t mlp_shrink_mask(const uint32_t (&v)[48], const float* bias, float lam, bool kept) {
-  uint64_t m = 0;
-#pragma unroll
-  for (int c = 0; c < 48; ++c) m |= (uint64_t)(kept && fabsf(__uint_as_float(v[c]) + bias[c]) > lam) << c;
-  return m;
-}
-// GX (re in vr, im in vi: 48 channels of this thread's row) -> fp32 complex rows of G: each warp transposes its 32 rows
-// through a private slice of an idle operand buffer (16 channels per pass, row pitch 144 B) and stores 128
-// contiguous bytes per row
-__device__ __forceinline__ void mlp_store_rows(const uint32_t (&vr)[48], const uint32_t (&vi)[48], uint8_t* scratch, float2* G,
-                                               long long wrow0, long long rows, int C, int chg, int nch, int lane) {
-  constexpr uint32_t kPitch = 16 * 8 + 16;
-#pragma unroll
-  for (int pass = 0; pass < 3; ++pass) {
-#pragma unroll
-    for (int c = 0; c < 16; c += 2) {
-      const int cc = pass * 16 + c;
-      *(float4*)(scratch + lane * kPitch + c * 8) = make_float4(__uint_as_float(vr[cc]), __uint_as_float(vi[cc]),
-                                                               __uint_as_float(vr[cc + 1]), __uint_as_float(vi[cc + 1]));
-    }
-    __syncwarp();
-    const int chp = pass * 16;   // first channel of this pass within the thread's 48
-#pragma unroll
-    for (int it = 0; it < 8; ++it) {
-      const int id = it * 32 + lane, rr = id >> 3, piece = id & 7;
-      const float4 o = *(const float4*)(scratch + rr * kPitch + piece * 16);
-      if (wrow0 + rr < rows && chg + chp + 2 * piece < nch) *(float4*)(G + (size_t)(wrow0 + rr) * C + chg + chp + 2 * piece) = o;
-    }
-    __syncwarp();
-  }
-}
-// activation masks of this thread's 48 channels -> [..][C'][2] bytes (parity tests)
-__device__ __forceinline__ void mlp_export_mask(uint8_t* dst, uint64_t mre, uint64_t mim, int nvalid) {
-  for (int c = 0; c < 48; ++c)
-    if (c < nvalid) *(uchar2*)(dst + 2 * c) = make_uchar2((unsigned char)((mre >> c) & 1u), (unsigned char)((mim >> c) & 1u));
 }
 
 // ---- hybrid BACKWARD (rows B1 second half, B3-B7) on the tensor cores, hidden factor 1 ---------------------------------
@@ -564,8 +524,8 @@ __device__ __forceinline__ void mlp_export_mask(uint8_t* dst, uint64_t mre, uint
 constexpr uint32_t kMlpBwdSmem = 4 * kWBytes + 4 * kTileBytes + 512;   // 223,232 (+512: rows 96..127 of the last chunk alias past the buffer)
 
 struct MlpBwdParams {
-  const float2* X;           // [rows][C] spectrum of x, read only
-  float2* G;                 // [rows][C] alpha-weighted spectrum of dY, replaced by GX
+  const void* X;             // [rows][C] spectrum of x (the kernel's ST), read only
+  void* G;                   // [rows][C] alpha-weighted spectrum of dY, replaced by GX
   const uint8_t* wprep;      // per group 4 x kWBytes: W1r, W1i, W2r, W2i
   const float* bprep;        // per group [2 layers][192]
   __nv_bfloat16 *Xh, *O1, *G2, *G1;   // operand images for tc_wgrad: [tile][group][kTileBytes]
@@ -575,8 +535,11 @@ struct MlpBwdParams {
   float lambda;
 };
 
+template <typename ST>
 __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams p, int S) {
   extern __shared__ __align__(1024) uint8_t smem[];
+  const ST* const X = (const ST*)p.X;
+  ST* const G = (ST*)p.G;
   __shared__ __align__(8) uint64_t done;
   __shared__ uint32_t tmem_slot;
   __shared__ __align__(16) float sBias[2 * NT];
@@ -644,7 +607,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
     const bool kept = row_valid && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
     uint64_t m1[2] = {0, 0}, m2[2] = {0, 0};   // [re, im] bits of this thread's 48 channels
     // ---- X -> bf16 operand; P1 = X W1 ----
-    mlp_load_operand(p.X, r0, p.rows, p.C, ch0, nch, bX, nullptr, tid);
+    mlp_load_operand<HP, kTileSbo, ST>(X, r0, p.rows, p.C, ch0, nch, bX, nullptr, tid);
     run_gemm(bX, w1r, w1i, false, p.Xh, img_off);
     // ---- O1 = relu(P1 + b1), mask1 ----
     if (epi) {
@@ -673,7 +636,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
     __syncthreads();
     tc_fence_after();
     // ---- G2 = mask2 (.) G -> bf16 operand; G1pre = G2 W2^H ----
-    mlp_load_operand(p.G, r0, p.rows, p.C, ch0, nch, bG2, sMask2, tid);
+    mlp_load_operand<HP, kTileSbo, ST>((const ST*)G, r0, p.rows, p.C, ch0, nch, bG2, sMask2, tid);
     run_gemm(bG2, w2r, w2i, true, p.G2, img_off);
     // ---- G1 = mask1 (.) G1pre ----
     if (epi) {
@@ -692,7 +655,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
       mlp_ld48(acc, vr);
       mlp_ld48(acc + BS, vi);
       tmem_wait_ld();
-      mlp_store_rows(vr, vi, bX + (size_t)warp * (kTileBytes / 8 / 16 * 16), p.G + ch0, r0 + q * 32, p.rows, p.C, chalf * 48, nch, lane);
+      mlp_store_rows<ST>(vr, vi, bX + (size_t)warp * (kTileBytes / 8 / 16 * 16), G + ch0, r0 + q * 32, p.rows, p.C, chalf * 48, nch, lane);
       if (p.mask1 != nullptr && row_valid) {
         // export for the mask-consistent parity tests: [B][H][Wh][C][2] bytes, this thread's 48 channels
         const long long bh = row / p.Kw;
@@ -726,8 +689,8 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
 constexpr uint32_t kMlpBwdHfSmem = 4 * kWBytes + 3 * kTileBytes + 512 + kMlpMaxHf * HP * 2 * 16;   // 210,560
 
 struct MlpBwdHfParams {
-  const float2* X;
-  float2* G;
+  const void* X;
+  void* G;
   const uint8_t* wprep;      // per (block, chunk) 4 x kWBytes (k_tc_prep_weights_hf)
   const float* bprep;        // per block: b1 [hf][192], then b2 [192]
   __nv_bfloat16 *Xh, *G2;    // images [tile][block]
@@ -738,8 +701,11 @@ struct MlpBwdHfParams {
   float lambda;
 };
 
+template <typename ST>
 __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfParams p, int S) {
   extern __shared__ __align__(1024) uint8_t smem[];
+  const ST* const X = (const ST*)p.X;
+  ST* const G = (ST*)p.G;
   __shared__ __align__(8) uint64_t done;
   __shared__ uint32_t tmem_slot;
   __shared__ __align__(16) float sBias[(kMlpMaxHf + 1) * NT];
@@ -815,7 +781,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
     const bool kept = row_valid && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
     const long long bh = row / p.Kw;
     const int kw = (int)(row - bh * p.Kw);
-    mlp_load_operand(p.X, r0, p.rows, p.C, ch0, BS, bX, nullptr, tid);
+    mlp_load_operand<HP, kTileSbo, ST>(X, r0, p.rows, p.C, ch0, BS, bX, nullptr, tid);
     // ---- pass 1 ----
     for (int hc = 0; hc < hf; ++hc) {
       load_weights(hc);
@@ -853,7 +819,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
     }
     buffers_free();
     // ---- pass 2 ----
-    mlp_load_operand(p.G, r0, p.rows, p.C, ch0, BS, bG2, sMask2, tid);
+    mlp_load_operand<HP, kTileSbo, ST>((const ST*)G, r0, p.rows, p.C, ch0, BS, bG2, sMask2, tid);
     for (int hc = 0; hc < hf; ++hc) {
       load_weights(hc);
       run_gemm(D1, bG2, wBr, wBi, true, 0u, hc == 0 ? p.G2 : nullptr, img_off);   // G2 W2[c, :]^H
@@ -878,7 +844,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
       mlp_ld48(D2 + lane_col, vr);
       mlp_ld48(D2 + lane_col + BS, vi);
       tmem_wait_ld();
-      mlp_store_rows(vr, vi, bX + (size_t)warp * (kTileBytes / 8 / 16 * 16), p.G + ch0, r0 + q * 32, p.rows, p.C, chalf * 48, BS, lane);
+      mlp_store_rows<ST>(vr, vi, bX + (size_t)warp * (kTileBytes / 8 / 16 * 16), G + ch0, r0 + q * 32, p.rows, p.C, chalf * 48, BS, lane);
     }
     tc_fence_before();
     __syncthreads();

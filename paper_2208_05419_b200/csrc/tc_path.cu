@@ -342,13 +342,21 @@ size_t tc_mlp_workspace_bytes(const Geometry& g) {
   const size_t groups = (size_t)(g.C + BS - 1) / BS;
   return align_up(groups * 4 * kWBytes, 256) + align_up(groups * 2 * NT * sizeof(float), 256);
 }
-cudaError_t tc_mlp_forward(const Geometry& g, float2* X, const float* w1, const float* b1, const float* w2, const float* b2,
-                           void* ws, cudaStream_t st) {
+namespace {
+template <typename ST>
+cudaError_t mlp_forward_launch(bool multi, int grid, cudaStream_t st, const MlpParams& mp, int S, int hf) {
+  // per device and cheap: the attribute is set on every call rather than cached in a static that another device or thread would miss
+  cudaError_t e = multi ? set_smem(tc_mlp_fwd_hf<ST>, kMlpHfSmem) : set_smem(tc_mlp_fwd<ST>, mlp_fwd_smem<ST>());
+  if (e != cudaSuccess) return e;
+  return multi ? launch_k(tc_mlp_fwd_hf<ST>, grid, kMlpThreads, kMlpHfSmem, st, true, mp, S, hf)
+               : launch_k(tc_mlp_fwd<ST>, grid, kMlpThreads, mlp_fwd_smem<ST>(), st, true, mp, S);
+}
+} // namespace
+cudaError_t tc_mlp_forward(const Geometry& g, void* X, bool spec16, const float* w1, const float* b1, const float* w2,
+                           const float* b2, void* ws, cudaStream_t st) {
   cudaError_t e;
   const bool multi = g.hid != g.bs;
   const int hf = multi ? g.hid / BS : 1;
-  // per device and cheap: set on every call rather than cached in a static that another device or thread would miss
-  if ((e = multi ? set_smem(tc_mlp_fwd_hf, kMlpHfSmem) : set_smem(tc_mlp_fwd, kMlpSmem)) != cudaSuccess) return e;
   const int groups = multi ? g.nb : (g.C + BS - 1) / BS;
   __nv_bfloat16* wprep = (__nv_bfloat16*)ws;
   float* bprep = (float*)((char*)ws + align_up((size_t)groups * hf * 4 * kWBytes, 256));
@@ -373,8 +381,7 @@ cudaError_t tc_mlp_forward(const Geometry& g, float2* X, const float* w1, const 
   if (S < 1) S = 1;
   if ((long long)S > ntiles) S = (int)ntiles;
   prof_begin(multi ? "tc_mlp_fwd_hf" : "tc_mlp_fwd", st);
-  e = multi ? launch_k(tc_mlp_fwd_hf, groups * S, kMlpThreads, kMlpHfSmem, st, true, mp, S, hf)
-            : launch_k(tc_mlp_fwd, groups * S, kMlpThreads, kMlpSmem, st, true, mp, S);
+  e = spec16 ? mlp_forward_launch<SpecBf16>(multi, groups * S, st, mp, S, hf) : mlp_forward_launch<float2>(multi, groups * S, st, mp, S, hf);
   prof_end(st);
   count_launch();
   return e != cudaSuccess ? e : cudaGetLastError();
@@ -454,11 +461,12 @@ MlpBwdHfWs mlp_bwd_hf_carve(const Geometry& g, char* base) {
   return w;
 }
 
-cudaError_t tc_mlp_backward_hf(const Geometry& g, const float2* X, float2* G, const float* w1, const float* b1, const float* w2,
-                               const float* b2, float* dw1, float* db1, float* dw2, float* db2, uint8_t* mask1, uint8_t* mask2,
-                               void* ws, cudaStream_t st) {
+cudaError_t tc_mlp_backward_hf(const Geometry& g, const void* X, void* G, bool spec16, const float* w1, const float* b1,
+                               const float* w2, const float* b2, float* dw1, float* db1, float* dw2, float* db2, uint8_t* mask1,
+                               uint8_t* mask2, void* ws, cudaStream_t st) {
   cudaError_t e;
-  if ((e = set_smem(tc_mlp_bwd_hf, kMlpBwdHfSmem)) != cudaSuccess) return e;
+  if ((e = spec16 ? set_smem(tc_mlp_bwd_hf<SpecBf16>, kMlpBwdHfSmem) : set_smem(tc_mlp_bwd_hf<float2>, kMlpBwdHfSmem)) != cudaSuccess)
+    return e;
   if ((e = set_smem(tc_wgrad, kWgSmem)) != cudaSuccess) return e;
   const MlpBwdHfWs w = mlp_bwd_hf_carve(g, (char*)ws);
   const int hf = w.hf, nW = g.nb * hf * BS * BS;
@@ -479,7 +487,8 @@ cudaError_t tc_mlp_backward_hf(const Geometry& g, const float2* X, float2* G, co
   if (S < 1) S = 1;
   if ((long long)S > w.ntiles) S = (int)w.ntiles;
   prof_begin("tc_mlp_bwd_hf", st);
-  e = launch_k(tc_mlp_bwd_hf, g.nb * S, kMlpThreads, kMlpBwdHfSmem, st, true, mp, S);
+  e = spec16 ? launch_k(tc_mlp_bwd_hf<SpecBf16>, g.nb * S, kMlpThreads, kMlpBwdHfSmem, st, true, mp, S)
+             : launch_k(tc_mlp_bwd_hf<float2>, g.nb * S, kMlpThreads, kMlpBwdHfSmem, st, true, mp, S);
   prof_end(st);
   count_launch();
   if (e != cudaSuccess || (e = cudaGetLastError()) != cudaSuccess) return e;
@@ -507,12 +516,12 @@ size_t tc_mlp_bwd_workspace_bytes(const Geometry& g) {
   return g.hid != g.bs ? mlp_bwd_hf_carve(g, nullptr).total : mlp_bwd_carve(g, nullptr).total;
 }
 
-cudaError_t tc_mlp_backward(const Geometry& g, const float2* X, float2* G, const float* w1, const float* b1, const float* w2,
-                            const float* b2, float* dw1, float* db1, float* dw2, float* db2, uint8_t* mask1, uint8_t* mask2,
-                            void* ws, cudaStream_t st) {
-  if (g.hid != g.bs) return tc_mlp_backward_hf(g, X, G, w1, b1, w2, b2, dw1, db1, dw2, db2, mask1, mask2, ws, st);
+cudaError_t tc_mlp_backward(const Geometry& g, const void* X, void* G, bool spec16, const float* w1, const float* b1,
+                            const float* w2, const float* b2, float* dw1, float* db1, float* dw2, float* db2, uint8_t* mask1,
+                            uint8_t* mask2, void* ws, cudaStream_t st) {
+  if (g.hid != g.bs) return tc_mlp_backward_hf(g, X, G, spec16, w1, b1, w2, b2, dw1, db1, dw2, db2, mask1, mask2, ws, st);
   cudaError_t e;
-  if ((e = set_smem(tc_mlp_bwd, kMlpBwdSmem)) != cudaSuccess) return e;
+  if ((e = spec16 ? set_smem(tc_mlp_bwd<SpecBf16>, kMlpBwdSmem) : set_smem(tc_mlp_bwd<float2>, kMlpBwdSmem)) != cudaSuccess) return e;
   if ((e = set_smem(tc_wgrad, kWgSmem)) != cudaSuccess) return e;
   const MlpBwdWs w = mlp_bwd_carve(g, (char*)ws);
   const int nW = w.groups * BS * BS;
@@ -535,7 +544,8 @@ cudaError_t tc_mlp_backward(const Geometry& g, const float2* X, float2* G, const
   if (S < 1) S = 1;
   if ((long long)S > w.ntiles) S = (int)w.ntiles;
   prof_begin("tc_mlp_bwd", st);
-  e = launch_k(tc_mlp_bwd, w.groups * S, kMlpThreads, kMlpBwdSmem, st, true, mp, S);
+  e = spec16 ? launch_k(tc_mlp_bwd<SpecBf16>, w.groups * S, kMlpThreads, kMlpBwdSmem, st, true, mp, S)
+             : launch_k(tc_mlp_bwd<float2>, w.groups * S, kMlpThreads, kMlpBwdSmem, st, true, mp, S);
   prof_end(st);
   count_launch();
   if (e != cudaSuccess || (e = cudaGetLastError()) != cudaSuccess) return e;

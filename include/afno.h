@@ -92,7 +92,8 @@ const char* afno_last_error(void); /* thread-local, valid until the thread's nex
 /* Name of the kernel family the descriptor dispatches to: "tcgen05-bf16" (every transform and MLP layer a
  * tensor-core GEMM: bf16, blocks dividing 96, hidden factor 1, H <= 96, W/2+1 <= 96), "hybrid-fft32-tcgen05"
  * (bf16 activations beyond those limits: fp32 FFTs on the CUDA cores, the block MLP, its gradient stages and the
- * parameter gradients on the tensor cores; hidden factor > 1: forward only, its backward runs the fp32 kernels)
+ * parameter gradients on the tensor cores, hidden factors 1..8; the spectra between its kernels are stored as bf16
+ * complex when H and W are among 90 / 180 / 360 / 720 / 1,440 and C % 64 == 0, as fp32 complex otherwise)
  * or "generic-fp32".  Returns NULL for an invalid / unsupported descriptor. */
 const char* afno_spectral_path(const afno_desc_t* d);
 

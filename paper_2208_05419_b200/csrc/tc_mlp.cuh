@@ -98,6 +98,47 @@ __device__ __forceinline__ void mlp_load_operand(const ST* __restrict__ src_rows
     *(uint4*)(dst + (size_t)(BS / 8 + c8) * STRIDE) = im;
   }
 }
+// The same in two halves, for the bf16 spectrum (32 bytes per unit): fetch keeps a thread's units in registers, so that
+// the loads of the NEXT operand are in flight under a GEMM and its epilogue; commit de-interleaves, masks and stores.
+constexpr int kMlpFetchUnits = (HP * (BS / 8) + kMlpThreads - 1) / kMlpThreads;   // 5
+struct MlpFetch { uint4 a[kMlpFetchUnits], b[kMlpFetchUnits]; };
+__device__ __forceinline__ void mlp_fetch_operand(const SpecBf16* __restrict__ src_rows, long long r0, long long rows, int C, int ch0,
+                                                  int nch, int tid, MlpFetch& f) {
+#pragma unroll
+  for (int k = 0; k < kMlpFetchUnits; ++k) {
+    const uint32_t u = tid + k * kMlpThreads;
+    const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
+    f.a[k] = f.b[k] = make_uint4(0, 0, 0, 0);
+    if (u < HP * (BS / 8) && r0 + rr < rows && 8 * c8 < nch) {
+      const uint4* src = (const uint4*)(src_rows + (size_t)(r0 + rr) * C + ch0 + 8 * c8);
+      f.a[k] = __ldg(src);
+      f.b[k] = __ldg(src + 1);
+    }
+  }
+}
+__device__ __forceinline__ void mlp_commit_operand(const MlpFetch& f, uint8_t* dstbuf, const uint4 (*mask2)[2], int tid) {
+#pragma unroll
+  for (int k = 0; k < kMlpFetchUnits; ++k) {
+    const uint32_t u = tid + k * kMlpThreads;
+    if (u >= HP * (BS / 8)) continue;
+    const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
+    const uint4 a = f.a[k], b = f.b[k];
+    uint4 re = make_uint4(__byte_perm(a.x, a.y, 0x5410), __byte_perm(a.z, a.w, 0x5410), __byte_perm(b.x, b.y, 0x5410), __byte_perm(b.z, b.w, 0x5410));
+    uint4 im = make_uint4(__byte_perm(a.x, a.y, 0x7632), __byte_perm(a.z, a.w, 0x7632), __byte_perm(b.x, b.y, 0x7632), __byte_perm(b.z, b.w, 0x7632));
+    if (mask2 != nullptr) {
+      const uint4 mk = mask2[rr][c8 / 6];
+      const int sh = (c8 % 6) * 8;
+      const uint32_t mre = (uint32_t)((((uint64_t)mk.y << 32) | mk.x) >> sh) & 0xFFu;
+      const uint32_t mim = (uint32_t)((((uint64_t)mk.w << 32) | mk.z) >> sh) & 0xFFu;
+      auto sel = [](uint32_t v, uint32_t bits) { return v & ((bits & 1u ? 0x0000FFFFu : 0u) | (bits & 2u ? 0xFFFF0000u : 0u)); };
+      re = make_uint4(sel(re.x, mre), sel(re.y, mre >> 2), sel(re.z, mre >> 4), sel(re.w, mre >> 6));
+      im = make_uint4(sel(im.x, mim), sel(im.y, mim >> 2), sel(im.z, mim >> 4), sel(im.w, mim >> 6));
+    }
+    uint8_t* dst = dstbuf + (size_t)rr * 16;
+    *(uint4*)(dst + (size_t)c8 * kTileSbo) = re;
+    *(uint4*)(dst + (size_t)(BS / 8 + c8) * kTileSbo) = im;
+  }
+}
 // 48 accumulator columns of this thread's row (the caller waits with tmem_wait_ld)
 __device__ __forceinline__ void mlp_ld48(uint32_t taddr, uint32_t (&v)[48]) {
   tmem_ld16<0>(taddr, v);
@@ -584,7 +625,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
   const size_t chunk_off = (size_t)chalf * 6 * kTileSbo, im_off = (size_t)(BS / 8) * kTileSbo;
   uint32_t ph = 0;
   // every thread has written its part of operand `buf`: hand it to the tensor core (and to the copy engine as an image)
-  auto run_gemm = [&](const uint8_t* buf, uint32_t wr, uint32_t wi, bool transposed, __nv_bfloat16* img, size_t img_off) {
+  auto start_gemm = [&](const uint8_t* buf, uint32_t wr, uint32_t wi, bool transposed, __nv_bfloat16* img, size_t img_off) {
     fence_async_smem();
     tc_fence_before();
     __syncthreads();
@@ -594,10 +635,19 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
     }
     if (storer) bulk_store((uint8_t*)img + img_off, smem_u32(buf), kTileBytes, pol_img);
     __syncwarp();
+  };
+  auto finish_gemm = [&]() {
     mbar_wait(&done, ph);
     tc_fence_after();
     ph ^= 1u;
   };
+  // bf16 spectrum: the next operand's rows travel global -> registers under the GEMM before it (G under layer 2 and
+  // its epilogue, the next tile's X under GX and its store); fp32 spectrum: loaded where it is needed
+  constexpr bool kPrefetch = std::is_same<ST, SpecBf16>::value;
+  MlpFetch fx, fg;
+  if constexpr (kPrefetch) {
+    if (s0 < ntiles) mlp_fetch_operand((const SpecBf16*)X, s0 * HP, p.rows, p.C, ch0, nch, tid, fx);
+  }
   for (long long t = s0; t < ntiles; t += S) {
     const long long r0 = t * HP;
     const size_t img_off = ((size_t)t * p.ngroups + j) * kTileBytes;
@@ -607,8 +657,10 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
     const bool kept = row_valid && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
     uint64_t m1[2] = {0, 0}, m2[2] = {0, 0};   // [re, im] bits of this thread's 48 channels
     // ---- X -> bf16 operand; P1 = X W1 ----
-    mlp_load_operand<HP, kTileSbo, ST>(X, r0, p.rows, p.C, ch0, nch, bX, nullptr, tid);
-    run_gemm(bX, w1r, w1i, false, p.Xh, img_off);
+    if constexpr (kPrefetch) mlp_commit_operand(fx, bX, nullptr, tid);
+    else mlp_load_operand<HP, kTileSbo, ST>(X, r0, p.rows, p.C, ch0, nch, bX, nullptr, tid);
+    start_gemm(bX, w1r, w1i, false, p.Xh, img_off);
+    finish_gemm();
     // ---- O1 = relu(P1 + b1), mask1 ----
     if (epi) {
 #pragma unroll
@@ -619,7 +671,9 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
         m1[half] = mlp_relu_store(v, sBias + half * BS + chalf * 48, bO + (size_t)r * 16 + half * im_off + chunk_off);
       }
     }
-    run_gemm(bO, w2r, w2i, false, p.O1, img_off);
+    start_gemm(bO, w2r, w2i, false, p.O1, img_off);
+    if constexpr (kPrefetch) mlp_fetch_operand((const SpecBf16*)G, r0, p.rows, p.C, ch0, nch, tid, fg);
+    finish_gemm();
     // ---- mask2 = (|P2 + b2| > lambda) on kept rows ----
     if (epi) {
 #pragma unroll
@@ -636,8 +690,10 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
     __syncthreads();
     tc_fence_after();
     // ---- G2 = mask2 (.) G -> bf16 operand; G1pre = G2 W2^H ----
-    mlp_load_operand<HP, kTileSbo, ST>((const ST*)G, r0, p.rows, p.C, ch0, nch, bG2, sMask2, tid);
-    run_gemm(bG2, w2r, w2i, true, p.G2, img_off);
+    if constexpr (kPrefetch) mlp_commit_operand(fg, bG2, sMask2, tid);
+    else mlp_load_operand<HP, kTileSbo, ST>((const ST*)G, r0, p.rows, p.C, ch0, nch, bG2, sMask2, tid);
+    start_gemm(bG2, w2r, w2i, true, p.G2, img_off);
+    finish_gemm();
     // ---- G1 = mask1 (.) G1pre ----
     if (epi) {
 #pragma unroll
@@ -648,7 +704,11 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd(const MlpBwdParams 
         mlp_masked_store(v, m1[half], bG1 + (size_t)r * 16 + half * im_off + chunk_off);
       }
     }
-    run_gemm(bG1, w1r, w1i, true, p.G1, img_off);
+    start_gemm(bG1, w1r, w1i, true, p.G1, img_off);
+    if constexpr (kPrefetch) {
+      if (t + S < ntiles) mlp_fetch_operand((const SpecBf16*)X, (t + S) * HP, p.rows, p.C, ch0, nch, tid, fx);
+    }
+    finish_gemm();
     // ---- GX -> fp32 complex, in place over G ----
     if (epi) {
       uint32_t vr[48], vi[48];

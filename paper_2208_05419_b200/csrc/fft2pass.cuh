@@ -108,9 +108,11 @@ constexpr int kF2MaxBatch = 24;   // rows a thread keeps in flight before its fi
 
 // ---- F2 / F7: H-direction complex FFT, in place on S[B][H][Kw][C]; tile = 32 G channels of one (b, kw) column ---------
 // grid (C / (32 G), Kw, B), block 256; smem H * 32 G float2 (G = 2 up to 360 points, 1 beyond: 184 KB at 720)
+// warps per block of the H kernel: the narrow tile (G = 1: one block per SM) runs 16 warps to keep the SM busy
+constexpr int hfft2_warps(int G) { return G == 1 ? 16 : kF2Warps; }
 template <int N1, int N2, int SG, int G, typename ST>
-__global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(ST* __restrict__ S, const float2* __restrict__ tw, int Kw, int C) {
-  constexpr int H = N1 * N2, LW = 32 * G;
+__global__ void __launch_bounds__(32 * hfft2_warps(G)) k_hfft2(ST* __restrict__ S, const float2* __restrict__ tw, int Kw, int C) {
+  constexpr int H = N1 * N2, LW = 32 * G, NW = hfft2_warps(G);
   extern __shared__ float2 smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int kw = blockIdx.y, b = blockIdx.z;
@@ -119,17 +121,17 @@ __global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(ST* __restrict__ S, con
   // a row of the tile is 256 G contiguous bytes: one float2 (G = 1) or float4 (G = 2) per lane; up to kF2MaxBatch
   // rows of the warp are in flight before the first shared-memory store
   typedef typename std::conditional<G == 2, typename SpecIO<ST>::pair_t, ST>::type vec_t;
-  constexpr int PER = (H + kF2Warps - 1) / kF2Warps, LB = PER < kF2MaxBatch ? PER : kF2MaxBatch;
-  for (int h0 = warp; h0 < H; h0 += kF2Warps * LB) {
+  constexpr int PER = (H + NW - 1) / NW, LB = PER < kF2MaxBatch ? PER : kF2MaxBatch;
+  for (int h0 = warp; h0 < H; h0 += NW * LB) {
     vec_t v[LB];
 #pragma unroll
     for (int u = 0; u < LB; ++u) {
-      const int h = h0 + u * kF2Warps;
+      const int h = h0 + u * NW;
       if (h < H) v[u] = *(const vec_t*)(base + (size_t)h * hstride + G * lane);
     }
 #pragma unroll
     for (int u = 0; u < LB; ++u) {
-      const int h = h0 + u * kF2Warps;
+      const int h = h0 + u * NW;
       if (h < H) {
         if constexpr (G == 2) {
           float2 a, b2;
@@ -142,12 +144,12 @@ __global__ void __launch_bounds__(32 * kF2Warps) k_hfft2(ST* __restrict__ S, con
     }
   }
   __syncthreads();
-  for (int task = warp; task < G * N2; task += kF2Warps) {
+  for (int task = warp; task < G * N2; task += NW) {
     const int g = task / N2, n2 = task - g * N2;
     pass_a<N1, N2, SG>(smem, LW, g * 32 + lane, n2, tw);
   }
   __syncthreads();
-  for (int task = warp; task < G * N1; task += kF2Warps) {
+  for (int task = warp; task < G * N1; task += NW) {
     const int g = task / N1, k1 = task - g * N1;
     float2 v[N2];
     pass_b<N1, N2, SG>(smem, LW, g * 32 + lane, k1, v);

@@ -584,8 +584,8 @@ void launch_hfft(Launcher& L, const Geometry& g, const Plan& p, ST* S, int C, bo
         if (L.err != cudaSuccess) return;
         L.begin("k_hfft");
         const dim3 grid(C / (32 * G), g.Kw, g.B);
-        if (inverse) k_hfft2<N1, N2, +1, G, ST><<<grid, 32 * kF2Warps, smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
-        else k_hfft2<N1, N2, -1, G, ST><<<grid, 32 * kF2Warps, smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
+        if (inverse) k_hfft2<N1, N2, +1, G, ST><<<grid, 32 * hfft2_warps(G), smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
+        else k_hfft2<N1, N2, -1, G, ST><<<grid, 32 * hfft2_warps(G), smem2, L.st>>>(S, p.fh.tw, g.Kw, C);
         L.check();
       }))
     return;

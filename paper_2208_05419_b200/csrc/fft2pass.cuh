@@ -77,8 +77,9 @@ struct RegFFT {
 };
 
 // pass A of one (n2, lane): rows n1 N2 + n2 -> rows k1 N2 + n2, in place.  tw[k] = exp(-2 pi i k / N).
+// (tws: stride of the twiddle table, for a sub-transform of length N / tws inside a three-pass transform)
 template <int N1, int N2, int SG>
-__device__ __forceinline__ void pass_a(float2* s, int lw, int l, int n2, const float2* __restrict__ tw) {
+__device__ __forceinline__ void pass_a(float2* s, int lw, int l, int n2, const float2* __restrict__ tw, int tws = 1) {
   float2 v[N1];
 #pragma unroll
   for (int n1 = 0; n1 < N1; ++n1) v[n1] = s[(n1 * N2 + n2) * lw + l];
@@ -88,7 +89,7 @@ __device__ __forceinline__ void pass_a(float2* s, int lw, int l, int n2, const f
   for (int k1 = 1; k1 < N1; ++k1) {
     float2 o = v[k1];
     if (n2 != 0) {
-      float2 t = __ldg(tw + n2 * k1);   // uniform across the warp
+      float2 t = __ldg(tw + tws * n2 * k1);   // uniform across the warp
       if (SG > 0) t.y = -t.y;
       o = cmul(o, t);
     }
@@ -156,6 +157,50 @@ __global__ void __launch_bounds__(32 * hfft2_warps(G)) k_hfft2(ST* __restrict__ 
     ST* dst = base + g * 32 + lane;
 #pragma unroll
     for (int k2 = 0; k2 < N2; ++k2) SpecIO<ST>::st(dst + (size_t)(k1 + N1 * k2) * hstride, v[k2]);
+  }
+}
+
+// ---- the same for the long axis of the p -> 1 grid (720 = 8 x 9 x 10): three passes with short codelets -----------------
+// N = N1 x Q, Q = N2 x N3: pass 1 is pass A of (N1, Q); every block k1 of Q rows then is a two-pass transform of length Q
+// (twiddle table read with stride N1), whose result X[k1 + N1 (k2 + N2 k3)] leaves from registers.  The 24- and 30-point
+// codelets of the two-pass split need ~190 registers (one 8-warp block per SM with a 184 KB tile); 8- to 10-point
+// codelets fit 64, so one block runs 32 warps.  grid (C / 32, Kw, B), block 1024; smem H * 32 float2.
+template <int N1, int N2, int N3, int SG, typename ST>
+__global__ void __launch_bounds__(1024) k_hfft3(ST* __restrict__ S, const float2* __restrict__ tw, int Kw, int C) {
+  constexpr int Q = N2 * N3, H = N1 * Q, NW = 32;
+  extern __shared__ float2 smem[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int kw = blockIdx.y, b = blockIdx.z;
+  ST* base = S + ((size_t)b * H * Kw + kw) * C + (size_t)blockIdx.x * 32 + lane;
+  const size_t hstride = (size_t)Kw * C;
+  constexpr int PER = (H + NW - 1) / NW, LB = PER < 12 ? PER : 12;
+  for (int h0 = warp; h0 < H; h0 += NW * LB) {
+    ST v[LB];
+#pragma unroll
+    for (int u = 0; u < LB; ++u) {
+      const int h = h0 + u * NW;
+      if (h < H) v[u] = base[(size_t)h * hstride];
+    }
+#pragma unroll
+    for (int u = 0; u < LB; ++u) {
+      const int h = h0 + u * NW;
+      if (h < H) smem[h * 32 + lane] = SpecIO<ST>::ld(&v[u]);
+    }
+  }
+  __syncthreads();
+  for (int m = warp; m < Q; m += NW) pass_a<N1, Q, SG>(smem, 32, lane, m, tw);
+  __syncthreads();
+  for (int t = warp; t < N1 * N3; t += NW) {
+    const int k1 = t / N3, n3 = t - k1 * N3;
+    pass_a<N2, N3, SG>(smem + k1 * Q * 32, 32, lane, n3, tw, N1);
+  }
+  __syncthreads();
+  for (int t = warp; t < N1 * N2; t += NW) {
+    const int k1 = t / N2, k2 = t - k1 * N2;
+    float2 v[N3];
+    pass_b<N2, N3, SG>(smem + k1 * Q * 32, 32, lane, k2, v);
+#pragma unroll
+    for (int k3 = 0; k3 < N3; ++k3) SpecIO<ST>::st(base + (size_t)(k1 + N1 * (k2 + N2 * k3)) * hstride, v[k3]);
   }
 }
 

@@ -577,6 +577,18 @@ void launch_wfft_fwd(Launcher& L, const Geometry& g, const Plan& p, const T* x, 
 template <typename ST = float2>
 void launch_hfft(Launcher& L, const Geometry& g, const Plan& p, ST* S, int C, bool inverse) {
   if (L.err != cudaSuccess) return;
+  if (C % 64 == 0 && g.H == 720) {
+    // the long axis of the p -> 1 grid: three passes (8 x 9 x 10), 32 channels per tile
+    const size_t smem3 = (size_t)g.H * 32 * sizeof(float2);
+    L.err = inverse ? set_smem(k_hfft3<8, 9, 10, +1, ST>, smem3) : set_smem(k_hfft3<8, 9, 10, -1, ST>, smem3);
+    if (L.err != cudaSuccess) return;
+    L.begin("k_hfft");
+    const dim3 grid(C / 32, g.Kw, g.B);
+    if (inverse) k_hfft3<8, 9, 10, +1, ST><<<grid, 1024, smem3, L.st>>>(S, p.fh.tw, g.Kw, C);
+    else k_hfft3<8, 9, 10, -1, ST><<<grid, 1024, smem3, L.st>>>(S, p.fh.tw, g.Kw, C);
+    L.check();
+    return;
+  }
   if (C % 64 == 0 && fft2_dispatch(g.H, [&](auto n1, auto n2, auto, auto narrow) {
         constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value, G = decltype(narrow)::value ? 1 : 2;
         const size_t smem2 = (size_t)g.H * 32 * G * sizeof(float2);
@@ -857,7 +869,7 @@ cudaError_t backward_t(const Geometry& g, const Plan& p, const T* x, const T* dy
 bool generic_supported(const Geometry& g, const char** why) {
   const size_t lim = 227 * 1024;
   const bool w_ok = (size_t)g.W * kLanes * sizeof(float2) <= lim || (fft2_has(g.W) && g.C % 64 == 0);
-  const bool h_ok = (size_t)g.H * kLanes * sizeof(float2) <= lim || (fft2_has(g.H) && g.C % 64 == 0);
+  const bool h_ok = (size_t)g.H * kLanes * sizeof(float2) <= lim;   // (720 points: 184 KB; a column of 1,440 does not fit)
   if (!w_ok || !h_ok) {
     *why = "H or W too large for the shared-memory FFT kernels (max 908; 1,440 with C a multiple of 64)";
     return false;

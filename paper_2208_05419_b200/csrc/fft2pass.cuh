@@ -338,6 +338,142 @@ k_wfft_inv2(const ST* __restrict__ S, const T* __restrict__ res, T* __restrict__
   }
 }
 
+// ---- the W-direction transforms of the p -> 1 grid (1,440 = 16 x 9 x 10 points): three passes, 16 packed lanes per row ----
+// (see k_hfft3; grid (C / 32, H, B), block 1024 = 64 half-warp task slots; smem W * 16 float2 = 184 KB)
+template <int N1, int N2, int N3, int SG>
+__device__ __forceinline__ void three_pass_ab(float2* smem, int l, int slot, const float2* __restrict__ tw) {
+  constexpr int Q = N2 * N3, NSLOT = 64;
+  for (int m = slot; m < Q; m += NSLOT) pass_a<N1, Q, SG>(smem, 16, l, m, tw);
+  __syncthreads();
+  for (int t = slot; t < N1 * N3; t += NSLOT) {
+    const int k1 = t / N3, n3 = t - k1 * N3;
+    pass_a<N2, N3, SG>(smem + k1 * Q * 16, 16, l, n3, tw, N1);
+  }
+  __syncthreads();
+}
+
+template <typename T, int N1, int N2, int N3, typename ST>
+__global__ void __launch_bounds__(1024)
+k_wfft_fwd3(const T* __restrict__ x, ST* __restrict__ S, const float2* __restrict__ tw, int H, int C, int Kw, float scale,
+            int alpha_weight) {
+  constexpr int Q = N2 * N3, W = N1 * Q, NSLOT = 64;
+  extern __shared__ float2 smem[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int l = lane & 15, slot = warp * 2 + (lane >> 4);
+  const int h = blockIdx.y, b = blockIdx.z;
+  const int c = blockIdx.x * 32 + 2 * l;
+  const T* xrow = x + ((size_t)(b * H + h) * W) * C + c;
+  {
+    constexpr int PER = (W + NSLOT - 1) / NSLOT, LB = PER < 12 ? PER : 12;
+    for (int w0 = slot; w0 < W; w0 += NSLOT * LB) {
+      typename ActIO<T>::raw2 v[LB];
+#pragma unroll
+      for (int u = 0; u < LB; ++u) {
+        const int w = w0 + u * NSLOT;
+        if (w < W) v[u] = ActIO<T>::ldraw2(xrow + (size_t)w * C);
+      }
+#pragma unroll
+      for (int u = 0; u < LB; ++u) {
+        const int w = w0 + u * NSLOT;
+        if (w < W) smem[w * 16 + l] = ActIO<T>::unraw2(v[u]);
+      }
+    }
+  }
+  __syncthreads();
+  three_pass_ab<N1, N2, N3, -1>(smem, l, slot, tw);
+  ST* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
+  auto emit = [&](int k, float2 zk, float2 zn) {   // bin k from Z[k] and Z[W - k]
+    if (k >= Kw) return;
+    float sc = 0.5f * scale;
+    if (alpha_weight && k != 0 && 2 * k != W) sc *= 2.f;
+    SpecIO<ST>::stpair(Srow + (size_t)k * C, make_float2(sc * (zk.x + zn.x), sc * (zk.y - zn.y)),
+                       make_float2(sc * (zk.y + zn.y), -sc * (zk.x - zn.x)));
+  };
+  // last pass: task (k1, k2) yields Z[k1 + N1 (k2 + N2 k3)], k3 < N3.  Z[W - k] lives in the partner task
+  //   k1 >= 1:        (N1 - k1, N2 - 1 - k2), element N3 - 1 - k3
+  //   k1 = 0, k2 >= 1: (0, N2 - k2),           element N3 - 1 - k3
+  //   k1 = k2 = 0:     itself,                 element (N3 - k3) mod N3
+  // a slot runs a task together with its partner (the one with the smaller index takes the pair)
+  for (int ti = slot; ti < N1 * N2; ti += NSLOT) {
+    const int k1 = ti / N2, k2 = ti - k1 * N2;
+    const int p1 = (N1 - k1) % N1, p2 = k1 ? N2 - 1 - k2 : (N2 - k2) % N2;
+    const int pti = p1 * N2 + p2;
+    if (ti > pti) continue;
+    float2 va[N3];
+    pass_b<N2, N3, -1>(smem + k1 * Q * 16, 16, l, k2, va);
+    if (ti == pti) {
+      const bool origin = (k1 | k2) == 0;
+#pragma unroll
+      for (int k3 = 0; k3 < N3; ++k3) emit(k1 + N1 * (k2 + N2 * k3), va[k3], origin ? va[(N3 - k3) % N3] : va[N3 - 1 - k3]);
+    } else {
+      float2 vb[N3];
+      pass_b<N2, N3, -1>(smem + p1 * Q * 16, 16, l, p2, vb);
+#pragma unroll
+      for (int k3 = 0; k3 < N3; ++k3) {
+        emit(k1 + N1 * (k2 + N2 * k3), va[k3], vb[N3 - 1 - k3]);
+        emit(p1 + N1 * (p2 + N2 * k3), vb[k3], va[N3 - 1 - k3]);
+      }
+    }
+  }
+}
+
+template <typename T, int N1, int N2, int N3, typename ST>
+__global__ void __launch_bounds__(1024)
+k_wfft_inv3(const ST* __restrict__ S, const T* __restrict__ res, T* __restrict__ out, const float2* __restrict__ tw, int H, int C,
+            int Kw, float scale, int half_interior) {
+  constexpr int Q = N2 * N3, W = N1 * Q, NSLOT = 64;
+  extern __shared__ float2 smem[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int l = lane & 15, slot = warp * 2 + (lane >> 4);
+  const int h = blockIdx.y, b = blockIdx.z;
+  const int c = blockIdx.x * 32 + 2 * l;
+  const ST* Srow = S + ((size_t)(b * H + h) * Kw) * C + c;
+  {
+    constexpr int PER = (W / 2 + NSLOT) / NSLOT, LB = PER < 8 ? PER : 8;
+    for (int k0 = slot; k0 <= W / 2; k0 += NSLOT * LB) {
+      typename SpecIO<ST>::pair_t t[LB];
+#pragma unroll
+      for (int u = 0; u < LB; ++u) {
+        const int kk = k0 + u * NSLOT;
+        t[u] = typename SpecIO<ST>::pair_t{};
+        if (kk < Kw) t[u] = SpecIO<ST>::ldpair(Srow + (size_t)kk * C);
+      }
+#pragma unroll
+      for (int u = 0; u < LB; ++u) {
+        const int kk = k0 + u * NSLOT;
+        if (kk > W / 2) continue;
+        float2 ta, tb;
+        SpecIO<ST>::unpair(t[u], ta, tb);
+        if (kk == 0 || 2 * kk == W) {
+          ta.y = 0.f;   // reading A4
+          tb.y = 0.f;
+        } else if (half_interior) {
+          ta.x *= 0.5f; ta.y *= 0.5f; tb.x *= 0.5f; tb.y *= 0.5f;
+        }
+        smem[kk * 16 + l] = make_float2(ta.x - tb.y, ta.y + tb.x);
+        if (kk != 0 && 2 * kk != W) smem[(W - kk) * 16 + l] = make_float2(ta.x + tb.y, -ta.y + tb.x);
+      }
+    }
+  }
+  __syncthreads();
+  three_pass_ab<N1, N2, N3, +1>(smem, l, slot, tw);
+  const size_t rowoff = ((size_t)(b * H + h) * W) * C + c;
+  for (int t = slot; t < N1 * N2; t += NSLOT) {
+    const int k1 = t / N2, k2 = t - k1 * N2;
+    typename ActIO<T>::raw2 r[N3];
+#pragma unroll
+    for (int k3 = 0; k3 < N3; ++k3)
+      if (res) r[k3] = ActIO<T>::ldraw2(res + rowoff + (size_t)(k1 + N1 * (k2 + N2 * k3)) * C);
+    float2 v[N3];
+    pass_b<N2, N3, +1>(smem + k1 * Q * 16, 16, l, k2, v);
+#pragma unroll
+    for (int k3 = 0; k3 < N3; ++k3) {
+      const float2 rr = res ? ActIO<T>::unraw2(r[k3]) : make_float2(0.f, 0.f);
+      ActIO<T>::st2(out + rowoff + (size_t)(k1 + N1 * (k2 + N2 * k3)) * C, scale * v[k3].x + rr.x, scale * v[k3].y + rr.y);
+    }
+  }
+}
+
 // size table: N -> (N1, N2), the warps per block of the W-direction kernels (pass A has N2 tasks, pass B N1 / 2 + 1 paired
 // items forward, N1 tasks inverse) and whether the tile is narrow (720 / 1,440 points: 32 channels per H tile, 16 packed
 // lanes per W tile, so that one row or column still fits shared memory)

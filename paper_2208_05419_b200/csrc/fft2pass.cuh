@@ -474,9 +474,10 @@ k_wfft_inv3(const ST* __restrict__ S, const T* __restrict__ res, T* __restrict__
   }
 }
 
-// size table: N -> (N1, N2), the warps per block of the W-direction kernels (pass A has N2 tasks, pass B N1 / 2 + 1 paired
-// items forward, N1 tasks inverse) and whether the tile is narrow (720 / 1,440 points: 32 channels per H tile, 16 packed
-// lanes per W tile, so that one row or column still fits shared memory)
+// size table of the two-pass kernels: N -> (N1, N2), the warps per block of the W-direction kernels (pass A has N2 tasks,
+// pass B N1 / 2 + 1 paired items forward, N1 tasks inverse) and whether the tile is narrow (720 points: 32 channels per H
+// tile, 16 packed lanes per W tile).  The launchers send H = 720 and W = 1,440 to the three-pass kernels before they
+// consult this table (fft2_has() lists every size one of the register kernels serves).
 template <typename F>
 bool fft2_dispatch(int n, F&& f) {
   using std::integral_constant;
@@ -484,7 +485,6 @@ bool fft2_dispatch(int n, F&& f) {
   if (n == 180) { f(integral_constant<int, 12>{}, integral_constant<int, 15>{}, integral_constant<int, 8>{}, integral_constant<int, 0>{}); return true; }
   if (n == 360) { f(integral_constant<int, 18>{}, integral_constant<int, 20>{}, integral_constant<int, 10>{}, integral_constant<int, 0>{}); return true; }
   if (n == 720) { f(integral_constant<int, 24>{}, integral_constant<int, 30>{}, integral_constant<int, 8>{}, integral_constant<int, 1>{}); return true; }
-  if (n == 1440) { f(integral_constant<int, 36>{}, integral_constant<int, 40>{}, integral_constant<int, 10>{}, integral_constant<int, 1>{}); return true; }
   return false;
 }
 inline bool fft2_has(int n) { return n == 90 || n == 180 || n == 360 || n == 720 || n == 1440; }

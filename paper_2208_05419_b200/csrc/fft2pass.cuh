@@ -109,8 +109,7 @@ constexpr int kF2MaxBatch = 24;   // rows a thread keeps in flight before its fi
 
 // ---- F2 / F7: H-direction complex FFT, in place on S[B][H][Kw][C]; tile = 32 G channels of one (b, kw) column ---------
 // grid (C / (32 G), Kw, B), block 256; smem H * 32 G float2 (G = 2 up to 360 points, 1 beyond: 184 KB at 720)
-// warps per block of the H kernel: the narrow tile (G = 1: one block per SM) runs 16 warps to keep the SM busy
-constexpr int hfft2_warps(int G) { return G == 1 ? 16 : kF2Warps; }
+constexpr int hfft2_warps(int) { return kF2Warps; }
 template <int N1, int N2, int SG, int G, typename ST>
 __global__ void __launch_bounds__(32 * hfft2_warps(G)) k_hfft2(ST* __restrict__ S, const float2* __restrict__ tw, int Kw, int C) {
   constexpr int H = N1 * N2, LW = 32 * G, NW = hfft2_warps(G);
@@ -475,16 +474,23 @@ k_wfft_inv3(const ST* __restrict__ S, const T* __restrict__ res, T* __restrict__
 }
 
 // size table of the two-pass kernels: N -> (N1, N2), the warps per block of the W-direction kernels (pass A has N2 tasks,
-// pass B N1 / 2 + 1 paired items forward, N1 tasks inverse) and whether the tile is narrow (720 points: 32 channels per H
-// tile, 16 packed lanes per W tile).  The launchers send H = 720 and W = 1,440 to the three-pass kernels before they
-// consult this table (fft2_has() lists every size one of the register kernels serves).
+// pass B N1 / 2 + 1 paired items forward, N1 tasks inverse); `narrow` stays 0 (64 channels per H tile, 32 packed lanes per
+// W tile).  720 and 1,440 points go to the three-pass kernels (fft3_dispatch); fft2_has() lists every size one of the
+// register kernels serves.
 template <typename F>
 bool fft2_dispatch(int n, F&& f) {
   using std::integral_constant;
   if (n == 90) { f(integral_constant<int, 9>{}, integral_constant<int, 10>{}, integral_constant<int, 5>{}, integral_constant<int, 0>{}); return true; }
   if (n == 180) { f(integral_constant<int, 12>{}, integral_constant<int, 15>{}, integral_constant<int, 8>{}, integral_constant<int, 0>{}); return true; }
   if (n == 360) { f(integral_constant<int, 18>{}, integral_constant<int, 20>{}, integral_constant<int, 10>{}, integral_constant<int, 0>{}); return true; }
-  if (n == 720) { f(integral_constant<int, 24>{}, integral_constant<int, 30>{}, integral_constant<int, 8>{}, integral_constant<int, 1>{}); return true; }
+  return false;
+}
+// three-pass sizes: N -> N1 (N = N1 x 9 x 10)
+template <typename F>
+bool fft3_dispatch(int n, F&& f) {
+  using std::integral_constant;
+  if (n == 720) { f(integral_constant<int, 8>{}); return true; }
+  if (n == 1440) { f(integral_constant<int, 16>{}); return true; }
   return false;
 }
 inline bool fft2_has(int n) { return n == 90 || n == 180 || n == 360 || n == 720 || n == 1440; }

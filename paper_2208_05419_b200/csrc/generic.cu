@@ -549,16 +549,18 @@ cudaError_t set_smem(K kernel, size_t bytes) {
 template <typename T, typename ST = float2>
 void launch_wfft_fwd(Launcher& L, const Geometry& g, const Plan& p, const T* x, ST* S, bool alpha) {
   if (L.err != cudaSuccess) return;
-  if (g.C % 64 == 0 && g.W == 1440) {
-    // the long axis of the p -> 1 grid: three passes (16 x 9 x 10), 16 packed lanes per row
-    const size_t smem3 = (size_t)g.W * 16 * sizeof(float2);
-    L.err = set_smem(k_wfft_fwd3<T, 16, 9, 10, ST>, smem3);
-    if (L.err != cudaSuccess) return;
-    L.begin("k_wfft_fwd");
-    k_wfft_fwd3<T, 16, 9, 10, ST><<<dim3(g.C / 32, g.H, g.B), 1024, smem3, L.st>>>(x, S, p.fw.tw, g.H, g.C, g.Kw, g.scale, alpha ? 1 : 0);
-    L.check();
+  // the long axes (720, 1,440 points; the p -> 1 grid): three passes (N1 x 9 x 10), 16 packed lanes per row
+  if (g.C % 64 == 0 && fft3_dispatch(g.W, [&](auto n1) {
+        constexpr int N1 = decltype(n1)::value;
+        const size_t smem3 = (size_t)g.W * 16 * sizeof(float2);
+        L.err = set_smem(k_wfft_fwd3<T, N1, 9, 10, ST>, smem3);
+        if (L.err != cudaSuccess) return;
+        L.begin("k_wfft_fwd");
+        k_wfft_fwd3<T, N1, 9, 10, ST><<<dim3(g.C / 32, g.H, g.B), 1024, smem3, L.st>>>(x, S, p.fw.tw, g.H, g.C, g.Kw, g.scale,
+                                                                                      alpha ? 1 : 0);
+        L.check();
+      }))
     return;
-  }
   if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2, auto nw, auto narrow) {
         constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value, NW = decltype(nw)::value;
         constexpr int LW = decltype(narrow)::value ? 16 : 32;
@@ -628,16 +630,17 @@ template <typename T, typename ST = float2>
 void launch_wfft_inv(Launcher& L, const Geometry& g, const Plan& p, const ST* S, const T* res, T* out,
                      bool half_interior) {
   if (L.err != cudaSuccess) return;
-  if (g.C % 64 == 0 && g.W == 1440) {
-    const size_t smem3 = (size_t)g.W * 16 * sizeof(float2);
-    L.err = set_smem(k_wfft_inv3<T, 16, 9, 10, ST>, smem3);
-    if (L.err != cudaSuccess) return;
-    L.begin("k_wfft_inv");
-    k_wfft_inv3<T, 16, 9, 10, ST><<<dim3(g.C / 32, g.H, g.B), 1024, smem3, L.st>>>(S, res, out, p.fw.tw, g.H, g.C, g.Kw, g.scale,
-                                                                              half_interior ? 1 : 0);
-    L.check();
+  if (g.C % 64 == 0 && fft3_dispatch(g.W, [&](auto n1) {
+        constexpr int N1 = decltype(n1)::value;
+        const size_t smem3 = (size_t)g.W * 16 * sizeof(float2);
+        L.err = set_smem(k_wfft_inv3<T, N1, 9, 10, ST>, smem3);
+        if (L.err != cudaSuccess) return;
+        L.begin("k_wfft_inv");
+        k_wfft_inv3<T, N1, 9, 10, ST><<<dim3(g.C / 32, g.H, g.B), 1024, smem3, L.st>>>(S, res, out, p.fw.tw, g.H, g.C, g.Kw, g.scale,
+                                                                                      half_interior ? 1 : 0);
+        L.check();
+      }))
     return;
-  }
   if (g.C % 64 == 0 && fft2_dispatch(g.W, [&](auto n1, auto n2, auto nw, auto narrow) {
         constexpr int N1 = decltype(n1)::value, N2 = decltype(n2)::value, NW = decltype(nw)::value;
         constexpr int LW = decltype(narrow)::value ? 16 : 32;

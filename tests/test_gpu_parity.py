@@ -924,3 +924,18 @@ def test_hybrid_backward_context_flags_and_graph_replay(oracle):
     assert np.array_equal(parity.from_device_act(ty), y_plain) and np.array_equal(parity.from_device_act(tdx), plain["dx"])
     for t, k in zip(g, ("dw1", "db1", "dw2", "db2")):
         assert np.array_equal(t.cpu().numpy(), plain[k]), k
+
+
+@pytest.mark.parametrize("H,W", [(90, 720), (720, 20), (36, 1440)])
+def test_three_pass_fft_long_axes(oracle, H, W):
+    """The three-pass register FFT kernels (fft2pass.cuh: 720 = 8 x 9 x 10, 1,440 = 16 x 9 x 10 points) on their own, each
+    combined with another kernel family on the other axis: fp32 path, forward and backward against the oracle per tile."""
+    rng = np.random.default_rng(H * 7 + W)
+    B, C, nb = 1, 64, 2
+    bs = C // nb
+    data = dict(x=rng.standard_normal((B, H, W, C)).astype(np.float32), dy=rng.standard_normal((B, H, W, C)).astype(np.float32))
+    data["w1"], data["b1"], data["w2"], data["b2"] = [
+        (0.2 * rng.standard_normal(s)).astype(np.float32) for s in [(nb, bs, bs, 2), (nb, bs, 2), (nb, bs, bs, 2), (nb, bs, 2)]]
+    desc = binding.Desc(B, H, W, C, nb, 1, 0.05, 1.0, binding.AFNO_F32)
+    _check_forward(oracle, desc, data, label=f"{H}x{W}x{C} fp32 three-pass")
+    _check_backward(oracle, desc, data, label=f"{H}x{W}x{C} fp32 three-pass")

@@ -802,6 +802,13 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
   const uint64_t pol_img = l2_evict_normal();
   const size_t chunk_off = (size_t)chalf * 6 * kTileSbo, im_off = (size_t)(BS / 8) * kTileSbo;
   uint32_t ph = 0;
+  constexpr bool kPrefetch = std::is_same<ST, SpecBf16>::value;
+  MlpFetch fq;
+  const SpecBf16* fetch_src = nullptr;   // set before a run_gemm call: what to fetch under that GEMM
+  long long fetch_r0 = 0;
+  if constexpr (kPrefetch) {
+    if (s0 < p.ntiles) mlp_fetch_operand((const SpecBf16*)X, s0 * HP, p.rows, p.C, ch0, BS, tid, fq);
+  }
   // operand `buf` is complete: GEMM into D (and the image copy); returns when the GEMM has completed
   auto run_gemm = [&](uint32_t D, const uint8_t* buf, uint32_t wr, uint32_t wi, bool transposed, uint32_t acc0,
                       __nv_bfloat16* img, size_t img_off) {
@@ -814,6 +821,12 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
     }
     if (storer && img != nullptr) bulk_store((uint8_t*)img + img_off, smem_u32(buf), kTileBytes, pol_img);
     __syncwarp();
+    // bf16 spectrum: the next operand's rows travel global -> registers under this GEMM (G under the last layer-2 GEMM of
+    // pass 1, the next tile's X under the last GEMM of pass 2)
+    if constexpr (kPrefetch) {
+      if (fetch_src != nullptr) mlp_fetch_operand(fetch_src, fetch_r0, p.rows, p.C, ch0, BS, tid, fq);
+      fetch_src = nullptr;
+    }
     mbar_wait(&done, ph);
     tc_fence_after();
     ph ^= 1u;
@@ -841,7 +854,8 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
     const bool kept = row_valid && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
     const long long bh = row / p.Kw;
     const int kw = (int)(row - bh * p.Kw);
-    mlp_load_operand<HP, kTileSbo, ST>(X, r0, p.rows, p.C, ch0, BS, bX, nullptr, tid);
+    if constexpr (kPrefetch) mlp_commit_operand(fq, bX, nullptr, tid);
+    else mlp_load_operand<HP, kTileSbo, ST>(X, r0, p.rows, p.C, ch0, BS, bX, nullptr, tid);
     // ---- pass 1 ----
     for (int hc = 0; hc < hf; ++hc) {
       load_weights(hc);
@@ -861,6 +875,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
           mlp_export_mask(p.mask1 + ((size_t)(bh * p.Wh + kw) * ((size_t)p.nb * hid) + (size_t)j * hid + hc * BS + chalf * 48) * 2, m1[0],
                           m1[1], 48);
       }
+      if (kPrefetch && hc == hf - 1) { fetch_src = (const SpecBf16*)G; fetch_r0 = r0; }
       run_gemm(D2, bH, wBr, wBi, false, hc > 0 ? 1u : 0u, p.O1, (size_t)hc * chunk_imgs + img_off);
     }
     // ---- mask2 = (|P2 + b2| > lambda) on kept rows ----
@@ -879,7 +894,8 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
     }
     buffers_free();
     // ---- pass 2 ----
-    mlp_load_operand<HP, kTileSbo, ST>((const ST*)G, r0, p.rows, p.C, ch0, BS, bG2, sMask2, tid);
+    if constexpr (kPrefetch) mlp_commit_operand(fq, bG2, sMask2, tid);
+    else mlp_load_operand<HP, kTileSbo, ST>((const ST*)G, r0, p.rows, p.C, ch0, BS, bG2, sMask2, tid);
     for (int hc = 0; hc < hf; ++hc) {
       load_weights(hc);
       run_gemm(D1, bG2, wBr, wBi, true, 0u, hc == 0 ? p.G2 : nullptr, img_off);   // G2 W2[c, :]^H
@@ -895,6 +911,7 @@ __global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_bwd_hf(const MlpBwdHfPa
           mlp_masked_store(v, m1[half], bH + (size_t)r * 16 + half * im_off + chunk_off);
         }
       }
+      if (kPrefetch && hc == hf - 1 && t + S < p.ntiles) { fetch_src = (const SpecBf16*)X; fetch_r0 = (t + S) * HP; }
       run_gemm(D2, bH, wAr, wAi, true, hc > 0 ? 1u : 0u, p.G1, (size_t)hc * chunk_imgs + img_off);   // GX += G1_c W1[:, c]^H
     }
     buffers_free();   // bX is the scratch area of the store below

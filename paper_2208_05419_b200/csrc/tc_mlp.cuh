@@ -973,3 +973,177 @@ __global__ void k_tc_wgrad_reduce_hf(const float* __restrict__ part, float2* __r
     *dst = acc;
   }
 }
+
+// ---- hybrid forward, bf16 spectrum, hidden factor 1: software-pipelined over two tiles ------------------------------------
+// tc_mlp_fwd runs load | GEMM | epilogue | GEMM | epilogue + store in sequence; both GEMM latencies are exposed.  With a
+// bf16 spectrum the staging buffer is 48 KB, which leaves room for TWO operand buffers, and two accumulators fit
+// tensor memory (2 x 192 columns): layer 2 of tile t runs under the conversion of tile t + 1, layer 1 of tile t + 1
+// under the softshrink epilogue and store of tile t.  Same arithmetic and layouts as tc_mlp_fwd.
+constexpr uint32_t kMlpPipeSmem = 4 * kWBytes + 2 * kMlpABytes + kMlpRows * BS * 4;   // 221,952
+
+__global__ void __launch_bounds__(kMlpThreads, 1) tc_mlp_fwd_pipe(const MlpParams p, int S) {
+  typedef SpecBf16 ST;
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t done[2];
+  __shared__ uint32_t tmem_slot;
+  __shared__ __align__(16) float sBias[2 * NT];
+  ST* const X = (ST*)p.X;
+  uint8_t* sW = smem;
+  uint8_t* sA0 = smem + 4 * kWBytes;
+  uint8_t* sStage = sA0 + 2 * kMlpABytes;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int j = blockIdx.x / S, s0 = blockIdx.x - j * S;
+  const long long ntiles = (p.rows + kMlpRows - 1) / kMlpRows;
+  const int ch0 = j * BS;
+  const int nch = min(BS, p.C - ch0);
+  pdl_launch_dependents();
+  for (uint32_t i = tid; i < 2 * kMlpABytes / 16; i += kMlpThreads) ((uint4*)sA0)[i] = make_uint4(0, 0, 0, 0);
+  if (tid == 0) {
+    mbar_init(&done[0], 1);
+    mbar_init(&done[1], 1);
+    mbar_init_fence();
+  }
+  if (warp == 0) tmem_alloc<512>(&tmem_slot);
+  pdl_wait();
+  {
+    const uint8_t* wsrc = p.wprep + (size_t)j * 4 * kWBytes;
+    for (uint32_t i = tid; i < 4 * kWBytes / 16; i += kMlpThreads) cp_async16(smem_u32(sW) + i * 16, wsrc + (size_t)i * 16);
+  }
+  for (int i = tid; i < 2 * NT; i += kMlpThreads) sBias[i] = p.bprep[(size_t)j * 2 * NT + i];
+  // staging loads of one tile: 16-byte pieces (4 channels); pieces past the last row or channel are zero-filled
+  auto stage_tile = [&](long long t) {
+    const long long r0 = t * kMlpRows;
+    for (uint32_t i = tid; i < kMlpRows * BS * 4 / 16; i += kMlpThreads) {
+      const int rr = i / (BS / 4), c4 = i - rr * (BS / 4);
+      const bool ok = (r0 + rr < p.rows) && (4 * c4 < nch);
+      const ST* src = X + (size_t)(ok ? r0 + rr : 0) * p.C + ch0 + (ok ? 4 * c4 : 0);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(sStage) + i * 16), "l"(src), "r"(ok ? 16 : 0) : "memory");
+    }
+  };
+  // staging -> bf16 K-major operand buffer: unit = (row, 8 channels)
+  auto convert = [&](uint8_t* sA) {
+    for (uint32_t u = tid; u < kMlpRows * (BS / 8); u += kMlpThreads) {
+      const int rr = u / (BS / 8), c8 = u - rr * (BS / 8);
+      uint4 re, im;
+      mlp_pack8<ST>((const ST*)sStage + (size_t)rr * BS + 8 * c8, re, im);
+      uint8_t* dst = sA + (size_t)rr * 16;
+      *(uint4*)(dst + (size_t)c8 * kMlpALbo) = re;
+      *(uint4*)(dst + (size_t)(BS / 8 + c8) * kMlpALbo) = im;
+    }
+  };
+  if (s0 < ntiles) stage_tile(s0);
+  cp_async_wait_all();
+  fence_async_smem();
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_slot;
+  const uint32_t aW = smem_u32(sW);
+  const uint32_t w1r = aW, w1i = aW + kWBytes, w2r = aW + 2 * kWBytes, w2i = aW + 3 * kWBytes;
+  const int q = warp & 3, chalf = warp >> 2;
+  const int r = q * 32 + lane;
+  const uint32_t lane_sel = (uint32_t)(q * 32) << 16;
+  uint32_t ph[2] = {0, 0};
+  auto issue_layer = [&](uint32_t D, uint32_t aA, uint32_t wr, uint32_t wi, uint64_t* bar) {
+    const uint32_t id = idesc_bf16(128, BS, 0u);
+#pragma unroll
+    for (int ks = 0; ks < BS / 16; ++ks) {
+      const uint64_t ad = smem_desc(aA + ks * 2 * kMlpALbo, kMlpALbo, kMlpASbo);
+      mma_ss(D, ad, smem_desc(wr + ks * 2 * kWLbo, kWLbo, kWSbo), id, ks != 0);
+      mma_ss(D + BS, ad, smem_desc(wi + ks * 2 * kWLbo, kWLbo, kWSbo), id, ks != 0);
+    }
+#pragma unroll
+    for (int ks = 0; ks < BS / 16; ++ks) {
+      const uint64_t ad = smem_desc(aA + (BS / 8 + ks * 2) * kMlpALbo, kMlpALbo, kMlpASbo);
+      mma_ss(D, ad, smem_desc(wi + ks * 2 * kWLbo, kWLbo, kWSbo), id | kIdescNegB, 1u);
+      mma_ss(D + BS, ad, smem_desc(wr + ks * 2 * kWLbo, kWLbo, kWSbo), id, 1u);
+    }
+    mma_commit(bar);
+  };
+  // prime the pipeline: tile s0 -> buffer 0, layer 1 issued
+  if (s0 < ntiles) {
+    convert(sA0);
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (s0 + S < ntiles) stage_tile(s0 + S);
+    if (warp == 0 && elect_one()) {
+      tc_fence_after();
+      issue_layer(tmem, smem_u32(sA0), w1r, w1i, &done[0]);
+    }
+    __syncwarp();
+  }
+  int cur = 0;
+  for (long long t = s0; t < ntiles; t += S, cur ^= 1) {
+    const long long r0 = t * kMlpRows;
+    const int nxt = cur ^ 1;
+    uint8_t* sA = sA0 + (size_t)cur * kMlpABytes;
+    uint8_t* sAn = sA0 + (size_t)nxt * kMlpABytes;
+    const uint32_t D = tmem + (uint32_t)cur * NT, Dn = tmem + (uint32_t)nxt * NT;
+    const bool has_next = t + S < ntiles;
+    // ---- layer 1 of this tile has been issued: O1 = relu(P1 + b1) -> operand of layer 2, over X ----
+    mbar_wait(&done[cur], ph[cur]);
+    ph[cur] ^= 1u;
+    tc_fence_after();
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+      uint32_t v[48];
+      mlp_ld48(D + lane_sel + half * BS + chalf * 48, v);
+      tmem_wait_ld();
+      const float* bias = sBias + half * BS + chalf * 48;
+      uint8_t* dst = sA + (size_t)r * 16 + (size_t)(half * (BS / 8) + chalf * 6) * kMlpALbo;
+#pragma unroll
+      for (int g = 0; g < 6; ++g) {
+        uint32_t pk[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+          pk[e] = pack_relu_bf16(__uint_as_float(v[8 * g + 2 * e]) + bias[8 * g + 2 * e], __uint_as_float(v[8 * g + 2 * e + 1]) + bias[8 * g + 2 * e + 1]);
+        *(uint4*)(dst + (size_t)g * kMlpALbo) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+      }
+    }
+    cp_async_wait_all();   // (the next tile, requested an iteration ago, has landed in the staging buffer)
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0 && elect_one()) {
+      tc_fence_after();
+      issue_layer(D, smem_u32(sA), w2r, w2i, &done[cur]);
+    }
+    __syncwarp();
+    // ---- under layer 2: the next tile staging -> other buffer, its layer 1 queued behind ----
+    if (has_next) {
+      convert(sAn);
+      fence_async_smem();
+      tc_fence_before();
+      __syncthreads();
+      if (t + 2LL * S < ntiles) stage_tile(t + 2LL * S);
+      if (warp == 0 && elect_one()) {
+        tc_fence_after();
+        issue_layer(Dn, smem_u32(sAn), w1r, w1i, &done[nxt]);
+      }
+      __syncwarp();
+    }
+    // ---- Z = softshrink(P2 + b2), zero on truncated rows -> spectrum rows, in place (under the next tile's layer 1) ----
+    mbar_wait(&done[cur], ph[cur]);
+    ph[cur] ^= 1u;
+    tc_fence_after();
+    {
+      uint32_t vr[48], vi[48];
+      mlp_ld48(D + lane_sel + chalf * 48, vr);
+      mlp_ld48(D + lane_sel + BS + chalf * 48, vi);
+      tmem_wait_ld();
+      const long long row = r0 + r;
+      const int h = (int)((row / p.Kw) % p.H);
+      const bool kept = row < p.rows && ((h <= p.H / 2) ? h : p.H - h) < p.Kh;
+      const float* bre = sBias + NT + chalf * 48;
+      mlp_shrink48(vr, vi, bre, bre + BS, p.lambda, kept);
+      mlp_store_rows<ST>(vr, vi, sA + (size_t)warp * (kMlpABytes / 8 / 16 * 16), X + ch0, r0 + q * 32, p.rows, p.C, chalf * 48, nch, lane);
+    }
+    tc_fence_before();
+    __syncthreads();   // buffer `cur` (scratch) and its accumulator are free for the tile after next
+    tc_fence_after();
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc<512>(tmem);
+}

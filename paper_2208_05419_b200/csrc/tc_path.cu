@@ -381,7 +381,13 @@ cudaError_t tc_mlp_forward(const Geometry& g, void* X, bool spec16, const float*
   if (S < 1) S = 1;
   if ((long long)S > ntiles) S = (int)ntiles;
   prof_begin(multi ? "tc_mlp_fwd_hf" : "tc_mlp_fwd", st);
-  e = spec16 ? mlp_forward_launch<SpecBf16>(multi, groups * S, st, mp, S, hf) : mlp_forward_launch<float2>(multi, groups * S, st, mp, S, hf);
+  if (spec16 && !multi) {
+    // bf16 spectrum, hidden factor 1: the software-pipelined kernel (two operand buffers, two accumulators)
+    if ((e = set_smem(tc_mlp_fwd_pipe, kMlpPipeSmem)) != cudaSuccess) return e;
+    e = launch_k(tc_mlp_fwd_pipe, groups * S, kMlpThreads, kMlpPipeSmem, st, true, mp, S);
+  } else {
+    e = spec16 ? mlp_forward_launch<SpecBf16>(multi, groups * S, st, mp, S, hf) : mlp_forward_launch<float2>(multi, groups * S, st, mp, S, hf);
+  }
   prof_end(st);
   count_launch();
   return e != cudaSuccess ? e : cudaGetLastError();

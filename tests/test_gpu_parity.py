@@ -939,3 +939,14 @@ def test_three_pass_fft_long_axes(oracle, H, W):
     desc = binding.Desc(B, H, W, C, nb, 1, 0.05, 1.0, binding.AFNO_F32)
     _check_forward(oracle, desc, data, label=f"{H}x{W}x{C} fp32 three-pass")
     _check_backward(oracle, desc, data, label=f"{H}x{W}x{C} fp32 three-pass")
+
+
+def test_three_pass_fft_bf16_spectrum_w720(oracle):
+    """The 720-point three-pass W kernels with the bf16 spectrum of the hybrid path (90 x 720 tokens, 32-wide blocks),
+    forward and backward against the oracle."""
+    wl = inputs.Workload(5, "90x720x64 nb=2 bf16 B=1", 1, 90, 720, 64, 2, 1, 0.01, 1.0, "bf16", True, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    assert binding.afno_spectral_path(desc) == "hybrid-fft32-tcgen05"
+    _check_forward(oracle, desc, data, label=wl.name)
+    _check_backward(oracle, desc, data, label=wl.name)

@@ -167,6 +167,53 @@ int afno_spectral_step_host(const afno_desc_t* d, const void* x_host, const void
                             float* db1_host, float* dw2_host, float* db2_host, void* arena,
                             size_t arena_bytes, void* cuda_stream);
 
+/* Parameter gradients of one block-diagonal complex linear layer for callers that must not allocate device memory.
+ *
+ * Who needs this: code that runs where cudaMalloc / cudaFree are off limits and that has no spare device buffer to
+ * hand over as a workspace either.  Typical cases are an operator plugged into a framework or serving engine that
+ * owns all device memory through its own pool (a raw allocation there escapes the pool's accounting and can fail
+ * although the pool has room), a latency-critical loop (cudaMalloc and cudaFree may synchronise the whole device and
+ * stall every other stream), and a process confined to a fixed memory reservation that is already handed out.
+ * afno_spectral_bwd cannot serve them: it needs a caller workspace of afno_spectral_workspace_bytes() and plan
+ * tables that the library allocates on first use.
+ *
+ * What it computes (rows B4 and B6 of SURVEY.md S8(a); the convention of afno_spectral_bwd above; the layer is
+ * PAPER.md:115-121, the gradient reduction PAPER.md:134): for every block j < num_blocks
+ *     dw[j][i][o] = sum_{m < M} conj(a[m][j*K + i]) * g[m][j*N + o]      i < K, o < N
+ *     db[j][o]    = sum_{m < M} g[m][j*N + o]
+ * with a = the layer's input rows (the spectrum Xh for layer 1, the hidden activations O1 for layer 2) and g = the
+ * gradient at its output (G1, G2), one row per (sample, mode).  It runs the fp32 kernels the generic-fp32 path of
+ * afno_spectral_bwd runs for these rows; sums are taken in a fixed order, so repeated calls agree bit for bit.
+ *
+ *   a   device, [M][lda] complex fp32 (re, im adjacent), lda >= num_blocks*K complex elements per row
+ *   g   device, [M][ldg] complex fp32, ldg >= num_blocks*N
+ *   dw  device, [num_blocks][K][N][2] fp32;  db  device, [num_blocks][N][2] fp32; neither may overlap a or g
+ *   flags  0 or AFNO_FLAG_ACCUM_GRADS (dw, db += instead of =)
+ *   All four pointers 8-byte aligned and owned by the caller.  M == 0 is allowed (a, g are then not read; dw, db
+ *   become zero, or stay as they are with ACCUM_GRADS).
+ *
+ * Scratch memory: the row range is split over thread blocks and each split's partial sums go to a static array of
+ * AFNO_STATIC_SCRATCH_BYTES that is part of the library's device code.  Every GPU onto which the library's code gets
+ * loaded holds these bytes from then until the process exits, whether or not this function is ever called.  The
+ * call itself issues no cudaMalloc, cudaFree or other allocating routine, on the first call or later.
+ *   - Limit: one split's partial sums, num_blocks * (K + 1) * N * 8 bytes, must fit the array (8 blocks of 96 x 96: 0.6 MB;
+ *     one block of 1,024 x 1,024: 8.4 MB).  Larger shapes return AFNO_ERR_UNSUPPORTED, the message names both sizes;
+ *     nothing is launched.  Within the limit the library uses as many splits as fit, up to two per SM per block.
+ *   - First call on a device: the function looks up the array's address on the current device once per device
+ *     (cudaGetSymbolAddress; the CUDA runtime may load the library's device code at that moment).  Make that first
+ *     call with the device current that the stream belongs to, and before any stream capture begins.
+ *   - The array is shared by every call on that device and keeps the previous call's partial sums.  That is
+ *     harmless for calls that follow each other on one stream: every entry is rewritten before it is read, nothing
+ *     needs clearing.  Two calls that can overlap on the GPU (issued to different streams, from one host thread or
+ *     several) race on the array and return garbage: serialise them, e.g. keep all calls of a device on one stream
+ *     or chain them with events.  Separate processes have separate copies and do not disturb each other.
+ * Errors: AFNO_ERR_INVALID_ARG (NULL / misaligned pointer, non-positive num_blocks / K / N, negative M, row stride too
+ * small, unknown flag), AFNO_ERR_UNSUPPORTED (beyond the limit above, or num_blocks / tile count beyond the launch grid's 65,535),
+ * AFNO_ERR_CUDA (address lookup or launch failed). */
+#define AFNO_STATIC_SCRATCH_BYTES (16u << 20)
+int afno_block_wgrad_static(const float* a, int32_t lda, const float* g, int32_t ldg, int64_t M, int32_t num_blocks,
+                            int32_t K, int32_t N, float* dw, float* db, uint32_t flags, void* cuda_stream);
+
 /* Number of kernel launches the last fwd / bwd call of this thread enqueued (bench.py's
  * "gpu_launches" is counted from this, not guessed). */
 int afno_last_launch_count(void);

@@ -24,8 +24,9 @@ EXPORTS = [
     "afno_spectral_workspace_bytes", "afno_spectral_mask_bytes", "afno_plan_warmup",
     "afno_spectral_fwd", "afno_spectral_bwd", "afno_spectral_host_arena_bytes",
     "afno_spectral_fwd_host", "afno_spectral_bwd_host", "afno_spectral_step_host", "afno_last_launch_count",
-    "afno_profile_start", "afno_profile_stop", "afno_plan_destroy_all",
+    "afno_profile_start", "afno_profile_stop", "afno_plan_destroy_all", "afno_block_wgrad_static",
 ]
+STATIC_SCRATCH_BYTES = 16 << 20   # AFNO_STATIC_SCRATCH_BYTES
 
 
 class AfnoDesc(ctypes.Structure):
@@ -85,6 +86,9 @@ def lib():
         L.afno_profile_start.restype = ctypes.c_int
         L.afno_profile_stop.restype = ctypes.c_int
         L.afno_profile_stop.argtypes = [ctypes.c_char_p, sz]
+        L.afno_block_wgrad_static.restype = ctypes.c_int
+        L.afno_block_wgrad_static.argtypes = [vp, ctypes.c_int32, vp, ctypes.c_int32, ctypes.c_int64, ctypes.c_int32,
+                                              ctypes.c_int32, ctypes.c_int32, vp, vp, ctypes.c_uint32, vp]
         _lib = L
     return _lib
 
@@ -238,3 +242,14 @@ def afno_spectral_step_host(d: Desc, x, dy, w1, b1, w2, b2, y, dx, dw1, db1, dw2
     _check(lib().afno_spectral_step_host(ctypes.byref(cd), _ptr(x), _ptr(dy), _ptr(w1), _ptr(b1), _ptr(w2), _ptr(b2),
                                          _ptr(y), _ptr(dx), _ptr(dw1), _ptr(db1), _ptr(dw2), _ptr(db2),
                                          _ptr(arena), _ws_bytes(arena), _stream_handle(stream)))
+
+
+def afno_block_wgrad_static(a, g, M: int, num_blocks: int, K: int, N: int, dw, db, flags: int = 0, stream=None,
+                            lda: int | None = None, ldg: int | None = None):
+    """dw[j][i][o] = sum_m conj(a[m][j*K+i]) g[m][j*N+o], db[j][o] = sum_m g[m][j*N+o] for callers that may not allocate
+    device memory: the kernels' scratch is the library's static device array (include/afno.h has the contract: size
+    limit, first-call set-up, no overlapping calls).  a, g: device tensors of complex fp32 rows ([M][lda] / [M][ldg],
+    strides in complex elements, default num_blocks*K / num_blocks*N); dw, db: fp32 device tensors."""
+    _check(lib().afno_block_wgrad_static(_ptr(a), num_blocks * K if lda is None else lda, _ptr(g),
+                                         num_blocks * N if ldg is None else ldg, M, num_blocks, K, N, _ptr(dw), _ptr(db),
+                                         flags, _stream_handle(stream)))

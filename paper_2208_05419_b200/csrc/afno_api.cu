@@ -672,6 +672,37 @@ int afno_spectral_step_host(const afno_desc_t* d, const void* x_host, const void
 
 // Frees every plan of the calling process (constant tables on all devices).  No call of this library may
 // be in flight; the next fwd / bwd / afno_plan_warmup rebuilds what it needs.
+// Rows B4 / B6 on caller-supplied operands with the split partial sums in the library's static device array: see
+// include/afno.h.  Nothing on this path allocates: argument checks here, then the address lookup and three launches
+// in generic.cu.  (The per-kernel profiler creates CUDA events; it is off unless afno_profile_start was called.)
+int afno_block_wgrad_static(const float* a, int32_t lda, const float* g, int32_t ldg, int64_t M, int32_t num_blocks,
+                            int32_t K, int32_t N, float* dw, float* db, uint32_t flags, void* cuda_stream) {
+  t_launches = 0;
+  if (num_blocks <= 0 || K <= 0 || N <= 0) return fail(AFNO_ERR_INVALID_ARG, "num_blocks, K and N must be positive");
+  if (M < 0) return fail(AFNO_ERR_INVALID_ARG, "M must be >= 0");
+  if (flags & ~(uint32_t)AFNO_FLAG_ACCUM_GRADS)
+    return fail(AFNO_ERR_INVALID_ARG, "afno_block_wgrad_static takes no flag other than AFNO_FLAG_ACCUM_GRADS");
+  if ((long long)num_blocks * K > lda || (long long)num_blocks * N > ldg)
+    return fail(AFNO_ERR_INVALID_ARG, "row stride smaller than num_blocks*K (lda) or num_blocks*N (ldg) complex elements");
+  if (!dw || !db || (M > 0 && (!a || !g))) return fail(AFNO_ERR_INVALID_ARG, "NULL pointer argument");
+  const void* ptrs[] = {a, g, dw, db};
+  for (const void* p : ptrs)
+    if (((uintptr_t)p & 7u) != 0) return fail(AFNO_ERR_INVALID_ARG, "pointers must be 8-byte aligned (complex fp32)");
+  const long long tiles = (long long)((K + 95) / 96) * ((N + 95) / 96);
+  if (num_blocks > 65535 || tiles > 65535)
+    return fail(AFNO_ERR_UNSUPPORTED, "num_blocks or ceil(K/96)*ceil(N/96) exceeds 65,535 (launch grid)");
+  const size_t need = wgrad_static_split_bytes(num_blocks, K, N);
+  if (need > kStaticScratchBytes)
+    return fail(AFNO_ERR_UNSUPPORTED,
+                "afno_block_wgrad_static: num_blocks*(K+1)*N*8 = " + std::to_string(need) +
+                    " bytes of partial sums exceed the static scratch array of " + std::to_string(kStaticScratchBytes) +
+                    " bytes (AFNO_STATIC_SCRATCH_BYTES); use afno_spectral_bwd with a caller workspace for this shape");
+  cudaError_t e = generic_wgrad_static((const float2*)a, lda, (const float2*)g, ldg, (long long)M, num_blocks, K, N, dw, db,
+                                       (flags & AFNO_FLAG_ACCUM_GRADS) != 0, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) return fail(AFNO_ERR_CUDA, std::string("afno_block_wgrad_static: ") + cudaGetErrorString(e));
+  return AFNO_OK;
+}
+
 int afno_plan_destroy_all(void) {
   std::lock_guard<std::mutex> lock(g_plan_mutex);
   int dev = 0;

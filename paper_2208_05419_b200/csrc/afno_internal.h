@@ -95,6 +95,13 @@ cudaError_t tc_mlp_backward(const Geometry& g, const void* X, void* G, bool spec
                             const float* w2, const float* b2, float* dw1, float* db1, float* dw2, float* db2, uint8_t* mask1,
                             uint8_t* mask2, void* ws, cudaStream_t st);
 
+// afno_block_wgrad_static (generic.cu): rows B4 / B6 on caller-supplied operands, the split partial sums kept in the
+// library's static device array instead of a workspace.  wgrad_static_split_bytes: bytes one split occupies there.
+constexpr size_t kStaticScratchBytes = AFNO_STATIC_SCRATCH_BYTES;
+size_t wgrad_static_split_bytes(int nb, int K, int N);
+cudaError_t generic_wgrad_static(const float2* A, int lda, const float2* G, int ldg, long long M, int nb, int K, int N,
+                                 float* dW, float* dB, bool accum, cudaStream_t st);
+
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 #ifdef __CUDACC__

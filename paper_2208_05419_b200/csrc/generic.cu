@@ -17,6 +17,7 @@
 // butterfly is conflict-free and needs no shuffles; warps split the butterflies of a stage.
 #include <cuda_bf16.h>
 
+#include <mutex>
 #include <type_traits>
 #include <utility>
 
@@ -930,6 +931,77 @@ cudaError_t generic_backward(const Geometry& g, const Plan& p, const void* x, co
                                      (__nv_bfloat16*)dx, dw1, db1, dw2, db2, ws, mask1_bytes, mask2_offset, st);
   return backward_t<float>(g, p, (const float*)x, (const float*)dy, w1, b1, w2, b2, (float*)dx, dw1, db1, dw2,
                            db2, ws, mask1_bytes, mask2_offset, st);
+}
+
+// ---- afno_block_wgrad_static: rows B4 / B6 without a workspace -------------------------------------------------
+// The same two kernels as launch_wgrad above (k_block_wgrad, then k_reduce_parts in ascending split order); the only
+// difference is where the split partial sums live.  They sit in the array below, which is part of the library's
+// device image: the driver places it when the module is loaded onto a device and releases it when the process ends,
+// so a call needs no cudaMalloc and no caller workspace.  Every call on a device uses the same bytes.  Nothing in
+// it has to start at zero: k_block_wgrad writes every (split, block, i < K, o < N) entry it owns, also for a split
+// whose row range is empty, before k_reduce_parts reads any of them, so what an earlier call left there is dead.
+static __device__ __align__(256) unsigned char s_wgrad_scratch[AFNO_STATIC_SCRATCH_BYTES];
+
+namespace {
+// In host code `s_wgrad_scratch` is only a handle for the runtime, not an address a kernel may be given.  The device
+// address differs per device and is looked up once per device, with that device current, by cudaGetSymbolAddress
+// (which also makes the runtime load this module onto the device if nothing of it has run there yet).
+constexpr int kMaxDevices = 64;
+std::mutex s_scratch_mutex;
+float2* s_scratch_addr[kMaxDevices] = {};
+
+cudaError_t static_scratch(float2** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(s_scratch_mutex);
+  if (s_scratch_addr[dev] == nullptr) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, s_wgrad_scratch);
+    if (e != cudaSuccess) return e;
+    s_scratch_addr[dev] = (float2*)p;
+  }
+  *out = s_scratch_addr[dev];
+  return cudaSuccess;
+}
+} // namespace
+
+size_t wgrad_static_split_bytes(int nb, int K, int N) {
+  return (size_t)nb * ((size_t)K * N + (size_t)N) * sizeof(float2);
+}
+
+// The caller (afno_api.cu) has checked the arguments and that one split fits the array.
+cudaError_t generic_wgrad_static(const float2* A, int lda, const float2* G, int ldg, long long M, int nb, int K, int N,
+                                 float* dW, float* dB, bool accum, cudaStream_t st) {
+  float2* part = nullptr;
+  cudaError_t e = static_scratch(&part);
+  if (e != cudaSuccess) return e;
+  // splits: two waves of CTAs over the SMs like wgrad_splits(), at least 16 rows each, and no more than fit the array
+  long long S = (2 * 148 + nb - 1) / nb;
+  const long long maxS = (M + kWgTR - 1) / kWgTR;
+  const long long fit = (long long)(kStaticScratchBytes / wgrad_static_split_bytes(nb, K, N));
+  if (S > maxS) S = maxS;
+  if (S > fit) S = fit;
+  if (S < 1) S = 1;
+  long long rps = (M + S - 1) / S;
+  rps = (rps + kWgTR - 1) / kWgTR * kWgTR;
+  const int ntK = (K + kWgTile - 1) / kWgTile, ntN = (N + kWgTile - 1) / kWgTile;
+  float2* partW = part;
+  float2* partB = part + (size_t)S * nb * K * N;
+  Launcher L{st};
+  L.begin("k_block_wgrad");
+  k_block_wgrad<<<dim3((unsigned)S, nb, ntK * ntN), 256, 0, L.st>>>(A, lda, G, ldg, partW, partB, M, K, N, rps, ntN);
+  L.check();
+  if (L.err != cudaSuccess) return L.err;
+  const size_t nW = (size_t)nb * K * N, nB = (size_t)nb * N;
+  L.begin("k_reduce_parts");
+  k_reduce_parts<<<(unsigned)((nW + 255) / 256), 256, 0, L.st>>>(partW, (float2*)dW, nW, (int)S, accum ? 1 : 0);
+  L.check();
+  L.begin("k_reduce_parts");
+  k_reduce_parts<<<(unsigned)((nB + 255) / 256), 256, 0, L.st>>>(partB, (float2*)dB, nB, (int)S, accum ? 1 : 0);
+  L.check();
+  return L.err;
 }
 
 } // namespace afno

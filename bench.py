@@ -16,6 +16,7 @@ parallelism needs on top: ONE all-reduce(SUM) of the 1.19 MB of parameter gradie
 from __future__ import annotations
 
 import argparse
+import re
 import json
 import os
 import sys
@@ -71,8 +72,10 @@ def executed_tensor_flops(B, wl, Kw, ctx=True):
     """Tensor FLOPs the tcgen05 path EXECUTES per step, counted from the UMMA instructions the kernels issue
     (S5.3): every transform is a dense DFT GEMM and M is padded to 128."""
     umma96, umma192 = 2.0 * 128 * 96 * 16, 2.0 * 128 * 192 * 16
-    t_mode = B * Kw * wl.num_blocks                          # (b, kw, block) tiles of tc_mix2 / tc_wgrad
-    t_row = B * wl.H * wl.num_blocks                         # (b, h, block) tiles of the W-direction kernels
+    groups = (wl.C + 95) // 96                               # the kernels tile over GROUPS of 96 channels (a group holds
+                                                             # 96 / bs blocks when the blocks are narrower: 32 blocks of 32 = 11 groups)
+    t_mode = B * Kw * groups                                 # (b, kw, group) tiles of tc_mix2 / tc_wgrad
+    t_row = B * wl.H * groups                                # (b, h, group) tiles of the W-direction kernels
     mix_fwd = 96 * umma96 * t_mode                           # H-DFT 24 + layer 1 24 + layer 2 24 + inverse H-DFT 24
     mix_bwd = (96 if ctx else 168) * umma96 * t_mode
     wdft = 24 * umma96 * t_row                               # one launch; fwd has 2 (x -> A, A -> y), bwd 2 (+1 stateless)
@@ -268,7 +271,7 @@ def run_ours(args):
         binding.afno_spectral_bwd(desc_b, s["x"], s["dy"], *params, s["dx"], *grads, ws_b, st)
         launches[0] = n + binding.afno_last_launch_count()
         if args.parallel == "dp":
-            bucket.all_reduce(dist)      # PAPER.md:134; NCCL, on the current stream (no-op at world size 1)
+            bucket.all_reduce(dist, stream=st)   # PAPER.md:134; NCCL, on the step's stream (no-op at world size 1)
 
     def barrier():
         torch.cuda.synchronize()
@@ -443,32 +446,60 @@ def run_ours(args):
     return 0
 
 
-class TrafficTable:
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture of this build
-    (profiles/r2_dram_traffic.csv: '# git <hash>' header, then kernel,bytes_per_launch).  A stored capture, not a
-    live measurement: `source` names the file and the commit it was taken on."""
+TRAFFIC_CSV = os.path.join("profiles", "r3_dram_traffic.csv")
 
-    def __init__(self):
+
+def kernel_source_hash():
+    """sha256 (first 16 hex digits) over the names and contents of every file under paper_2208_05419_b200/csrc/: what a
+    stored ncu capture must have been taken on to describe this tree's kernels."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2208_05419_b200", "csrc")
+    for name in sorted(os.listdir(csrc)):
+        if name.endswith((".cu", ".cuh", ".h")):
+            h.update(name.encode() + b"\0")
+            h.update(open(os.path.join(csrc, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+class TrafficTable:
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture (profiles/r3_dram_traffic.csv,
+    written by `bench.py --write-traffic`: '# src <hash of csrc/>' and '# git <commit>' header lines, then
+    kernel,bytes_per_launch).  A stored capture, not a live measurement, so it only counts for the kernels it was taken
+    on: when the hash of this tree's kernel sources differs from the header's, every figure is None and `source` says
+    why (a stale capture is never quoted)."""
+
+    def __init__(self, path=None, src_hash=None):
         self.rows, self.source = {}, None
-        path = os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")
+        rel = TRAFFIC_CSV if path is None else path
+        path = rel if os.path.isabs(rel) else os.path.join(ROOT, rel)
         try:
-            git = "unknown"
+            git, src, rows = "unknown", None, {}
             for line in open(path).read().splitlines():
                 if line.startswith("#"):
-                    if "git" in line:
-                        git = line.split("git", 1)[1].strip()
+                    w = line[1:].split()
+                    if len(w) >= 2 and w[0] == "git":
+                        git = w[1]
+                    if len(w) >= 2 and w[0] == "src":
+                        src = w[1]
                     continue
                 k, v = line.split(",")[:2]
                 if k != "kernel":
-                    self.rows[k] = int(float(v))
-            self.source = f"profiles/r2_dram_traffic.csv (ncu capture of commit {git}; stored, not measured by this run)"
+                    rows[k] = int(float(v))
+            have = kernel_source_hash() if src_hash is None else src_hash
+            if src != have:
+                self.source = (f"null: {rel} was captured on kernel sources {src} (commit {git}), this tree's are {have}; "
+                               f"re-capture with the command in {os.path.splitext(rel)[0]}.md")
+            else:
+                self.rows = rows
+                self.source = f"{rel} (ncu capture of kernel sources {src}, commit {git}; stored, not measured by this run)"
         except Exception as ex:
             self.source = f"unavailable: {ex}"
 
     def get(self, name):
         if name not in self.rows:
             if self.rows:
-                sys.stderr.write(f"bench.py: profiles/r2_dram_traffic.csv has no row for kernel {name!r}\n")
+                sys.stderr.write(f"bench.py: {TRAFFIC_CSV} has no row for kernel {name!r}\n")
             return None
         return self.rows[name]
 
@@ -482,6 +513,45 @@ class TrafficTable:
                 continue
             tot += t * n / steps
         return int(tot) if tot else None
+
+
+def write_traffic(raw_csv, out_path):
+    """profiles/r3_dram_traffic.csv from ncu's raw page (`ncu -i X.ncu-rep --page raw --csv > raw.csv`) of a capture of
+    `bench.py --timed-only` that starts on a step boundary: mean dram__bytes_read.sum + dram__bytes_write.sum per launch
+    and kernel.  ncu names both chain launches tc_mix2; within a step the first is the forward's (tc_mix_fwd), the
+    second the backward's (tc_mix_bwd), which is how the library's own profiler names them."""
+    import csv
+    import subprocess
+    rows = list(csv.reader(open(raw_csv)))
+    hdr = next(i for i, r in enumerate(rows) if "Kernel Name" in r)
+    cols = {c: i for i, c in enumerate(rows[hdr])}
+    units = rows[hdr + 1]
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    acc, mix = {}, 0
+    for r in rows[hdr + 2:]:
+        if len(r) <= cols["Kernel Name"]:
+            continue
+        m = re.search(r"(\w+)(?:<[^<>]*>)?\(", r[cols["Kernel Name"]])     # 'void afno::<unnamed>::tc_mix2<2, 0>(...)' -> tc_mix2
+        name = m.group(1) if m else r[cols["Kernel Name"]].strip()
+        if name == "tc_mix2":
+            name = "tc_mix_fwd" if mix % 2 == 0 else "tc_mix_bwd"
+            mix += 1
+        name = {"tc_wdft_fwd2": "tc_wdft_fwd", "tc_wdft_inv2": "tc_wdft_inv"}.get(name, name)
+        tot = 0.0
+        for m in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            tot += float(r[cols[m]].replace(",", "")) * scale[units[cols[m]]]
+        acc.setdefault(name, []).append(tot)
+    try:
+        git = subprocess.run(["git", "-C", ROOT, "rev-parse", "--short", "HEAD"], capture_output=True, text=True).stdout.strip() or "unknown"
+    except Exception:
+        git = "unknown"
+    with open(out_path, "w") as f:
+        f.write(f"# src {kernel_source_hash()}\n# git {git}\n")
+        f.write("# dram__bytes_read.sum + dram__bytes_write.sum per launch (mean over the captured launches), ncu --set full\n")
+        f.write("kernel,bytes_per_launch\n")
+        for k, v in acc.items():
+            f.write(f"{k},{int(sum(v) / len(v))}\n")
+    return acc
 
 
 def kernel_work(name, work, exe):
@@ -538,6 +608,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--write-traffic", metavar="RAW_CSV", default=None,
+                    help="no benchmark: turn ncu's raw page of a --timed-only capture into " + TRAFFIC_CSV)
     ap.add_argument("--timed-only", action="store_true",
                     help="warm-up, the timed steps and the per-kernel event pass only (no CUDA-graph replay, e2e or "
                          "cpu_baseline legs): the command the ncu captures under profiles/ run")
@@ -547,6 +619,10 @@ def main():
     ap.add_argument("--stateless", action="store_true",
                     help="time the stateless afno_spectral_bwd (recomputes F1) instead of the saved-context step")
     args = ap.parse_args()
+    if args.write_traffic:
+        acc = write_traffic(args.write_traffic, os.path.join(ROOT, TRAFFIC_CSV))
+        print(json.dumps({"written": TRAFFIC_CSV, "src": kernel_source_hash(), "launches": {k: len(v) for k, v in acc.items()}}))
+        return 0
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     if args.impl == "reference":

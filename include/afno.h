@@ -144,7 +144,10 @@ int afno_spectral_bwd(const afno_desc_t* d, const void* x, const void* dy, const
  * from one batched call).  The context flags and EXPORT_MASKS have no meaning here.
  * afno_spectral_bwd_host accepts x_host == NULL: x is then taken from the arena, where the
  * afno_spectral_fwd_host call that preceded it on the SAME arena and descriptor left it (a
- * training step uploads x once).  On an error the calls first wait for the copies and
+ * training step uploads x once).  Every host call that completes stamps the arena with the
+ * B, H, W, C and dtype of the x it leaves there; with x_host == NULL the stamp must match the
+ * descriptor, otherwise (fresh or foreign arena, other shape) the call returns
+ * AFNO_ERR_INVALID_ARG and computes nothing.  On an error the calls first wait for the copies and
  * kernels they have already enqueued, so the caller may free its buffers at once. */
 size_t afno_spectral_host_arena_bytes(const afno_desc_t* d, int for_backward); /* 0 fwd_host, 1 bwd_host, 2 step_host */
 int afno_spectral_fwd_host(const afno_desc_t* d, const void* x_host, const float* w1_host,

@@ -287,7 +287,7 @@ int afno_profile_stop(char* out, size_t cap) {
 const char* afno_spectral_path(const afno_desc_t* d) {
   Geometry g;
   if (resolve(d, &g) != AFNO_OK) return nullptr;
-  // "hybrid": fp32 FFTs on the CUDA cores + the block MLP (forward, and for hidden factor 1 also the gradient stages and
+  // "hybrid": fp32 FFTs on the CUDA cores + the block MLP (forward, and, for hidden factors 1..8, also the gradient stages and
   // the parameter gradients) on the tensor cores
   return use_tc_fwd(g) ? "tcgen05-bf16" : (tc_mlp_supported(g) ? "hybrid-fft32-tcgen05" : "generic-fp32");
 }
@@ -392,7 +392,18 @@ struct Arena {
     return p;
   }
 };
+// What the x at the head of an arena belongs to: written by every host call that leaves a complete x there, checked by
+// afno_spectral_bwd_host when it is asked to reuse that x (x_host == NULL).
+struct ArenaStamp {
+  uint32_t magic;
+  int32_t B, H, W, C, dtype;
+  uint32_t pad[2];
+};
+constexpr uint32_t kArenaMagic = 0x41464E4Fu;   // "AFNO"
+ArenaStamp stamp_of(const Geometry& g) { return ArenaStamp{kArenaMagic, g.B, g.H, g.W, g.C, g.bf16 ? 1 : 0, {0u, 0u}}; }
+
 struct HostLayout {
+  void* stamp;   // ArenaStamp, same offset in the three layouts (x and the parameters come first in all of them)
   void *x, *dy, *y, *dx;
   float *w1, *b1, *w2, *b2, *dw1, *db1, *dw2, *db2;
   void* ws;
@@ -411,6 +422,7 @@ HostLayout host_layout(const afno_desc_t* d, const Geometry& g, int mode, char* 
   h.b1 = (float*)a.take(h.nb1);
   h.w2 = (float*)a.take(h.nw);
   h.b2 = (float*)a.take(h.nb2);
+  h.stamp = a.take(sizeof(ArenaStamp));
   if (backward) {
     h.dy = a.take(h.act);
     h.dx = a.take(h.act);
@@ -475,12 +487,24 @@ struct HostPipe {
     cudaStreamSynchronize(d2h);
   }
 };
-thread_local std::vector<HostPipe*> t_pipes;
+// one set per (thread, device); released when the thread ends (errors ignored: at process exit the runtime may be gone)
+struct HostPipes {
+  std::vector<HostPipe*> v;
+  ~HostPipes() {
+    for (HostPipe* p : v) {
+      for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
+      if (p->h2d) cudaStreamDestroy(p->h2d);
+      if (p->d2h) cudaStreamDestroy(p->d2h);
+      delete p;
+    }
+  }
+};
+thread_local HostPipes t_pipes;
 cudaError_t host_pipe(HostPipe** out) {
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
-  for (HostPipe* p : t_pipes)
+  for (HostPipe* p : t_pipes.v)
     if (p->device == dev) {
       *out = p;
       return cudaSuccess;
@@ -493,7 +517,7 @@ cudaError_t host_pipe(HostPipe** out) {
     return e;
   }
   p->device = dev;
-  t_pipes.push_back(p);
+  t_pipes.v.push_back(p);
   *out = p;
   return cudaSuccess;
 }
@@ -544,6 +568,8 @@ int afno_spectral_fwd_host(const afno_desc_t* d, const void* x_host, const float
     AFNO_PIPE_TRY(cudaMemcpyAsync((char*)y_host + off, (char*)h.y + off, sample, cudaMemcpyDeviceToHost, hp->d2h));
   }
   AFNO_PIPE_TRY(cudaStreamSynchronize(hp->d2h));
+  const ArenaStamp stamp = stamp_of(g);   // x of this descriptor now sits complete at the head of the arena
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.stamp, &stamp, sizeof(stamp), cudaMemcpyHostToDevice, st));
   AFNO_PIPE_TRY(cudaStreamSynchronize(st));
   return AFNO_OK;
 }
@@ -569,6 +595,18 @@ int afno_spectral_bwd_host(const afno_desc_t* d, const void* x_host, const void*
   HostLayout h = host_layout(d, g, 1, (char*)arena);
   if (arena_bytes < h.total) return fail(AFNO_ERR_WORKSPACE, "arena smaller than afno_spectral_host_arena_bytes(d, 1)");
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (!x_host) {
+    // the arena must say that a host call left x of exactly this shape and dtype there: a fresh or foreign arena would
+    // otherwise yield plausible-looking dx and gradients of whatever bytes it holds
+    ArenaStamp got{};
+    AFNO_CUDA_TRY(cudaMemcpyAsync(&got, h.stamp, sizeof(got), cudaMemcpyDeviceToHost, st));
+    AFNO_CUDA_TRY(cudaStreamSynchronize(st));
+    const ArenaStamp want = stamp_of(g);
+    if (memcmp(&got, &want, sizeof(want)) != 0)
+      return fail(AFNO_ERR_INVALID_ARG,
+                  "x_host is NULL, but no afno_spectral_fwd_host / _step_host / _bwd_host call with the same B, H, W, C "
+                  "and dtype has left x in this arena");
+  }
   HostPipe* hp = nullptr;
   AFNO_CUDA_TRY(host_pipe(&hp));
   afno_desc_t d1 = *d;
@@ -601,6 +639,8 @@ int afno_spectral_bwd_host(const afno_desc_t* d, const void* x_host, const void*
   AFNO_PIPE_TRY(cudaMemcpyAsync(dw2_host, h.dw2, h.nw, cudaMemcpyDeviceToHost, hp->d2h));
   AFNO_PIPE_TRY(cudaMemcpyAsync(db2_host, h.db2, h.nb2, cudaMemcpyDeviceToHost, hp->d2h));
   AFNO_PIPE_TRY(cudaStreamSynchronize(hp->d2h));
+  const ArenaStamp stamp = stamp_of(g);   // x of this descriptor now sits complete at the head of the arena
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.stamp, &stamp, sizeof(stamp), cudaMemcpyHostToDevice, st));
   AFNO_PIPE_TRY(cudaStreamSynchronize(st));
   return AFNO_OK;
 }
@@ -666,12 +706,12 @@ int afno_spectral_step_host(const afno_desc_t* d, const void* x_host, const void
   AFNO_PIPE_TRY(cudaMemcpyAsync(dw2_host, h.dw2, h.nw, cudaMemcpyDeviceToHost, hp->d2h));
   AFNO_PIPE_TRY(cudaMemcpyAsync(db2_host, h.db2, h.nb2, cudaMemcpyDeviceToHost, hp->d2h));
   AFNO_PIPE_TRY(cudaStreamSynchronize(hp->d2h));
+  const ArenaStamp stamp = stamp_of(g);   // x of this descriptor now sits complete at the head of the arena
+  AFNO_PIPE_TRY(cudaMemcpyAsync(h.stamp, &stamp, sizeof(stamp), cudaMemcpyHostToDevice, st));
   AFNO_PIPE_TRY(cudaStreamSynchronize(st));
   return AFNO_OK;
 }
 
-// Frees every plan of the calling process (constant tables on all devices).  No call of this library may
-// be in flight; the next fwd / bwd / afno_plan_warmup rebuilds what it needs.
 // Rows B4 / B6 on caller-supplied operands with the split partial sums in the library's static device array: see
 // include/afno.h.  Nothing on this path allocates: argument checks here, then the address lookup and three launches
 // in generic.cu.  (The per-kernel profiler creates CUDA events; it is off unless afno_profile_start was called.)
@@ -703,6 +743,8 @@ int afno_block_wgrad_static(const float* a, int32_t lda, const float* g, int32_t
   return AFNO_OK;
 }
 
+// Frees every plan of the calling process (constant tables on all devices).  No call of this library may
+// be in flight; the next fwd / bwd / afno_plan_warmup rebuilds what it needs.
 int afno_plan_destroy_all(void) {
   std::lock_guard<std::mutex> lock(g_plan_mutex);
   int dev = 0;

@@ -88,7 +88,8 @@ size_t tc_mlp_workspace_bytes(const Geometry& g);
 cudaError_t tc_mlp_forward(const Geometry& g, void* X, bool spec16, const float* w1, const float* b1, const float* w2,
                            const float* b2, void* ws, cudaStream_t st);
 
-// hybrid backward, hidden factor 1: block MLP gradient stages and parameter gradients on the tensor cores
+// hybrid backward, hidden factors 1..8 (blocks of 96 for hf > 1; tc_mlp_backward dispatches hf > 1 to tc_mlp_backward_hf):
+// block MLP gradient stages and parameter gradients on the tensor cores
 bool tc_mlp_bwd_supported(const Geometry& g);
 size_t tc_mlp_bwd_workspace_bytes(const Geometry& g);
 cudaError_t tc_mlp_backward(const Geometry& g, const void* X, void* G, bool spec16, const float* w1, const float* b1,

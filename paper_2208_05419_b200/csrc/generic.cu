@@ -813,7 +813,7 @@ cudaError_t backward_t(const Geometry& g, const Plan& p, const T* x, const T* dy
   Launcher L{st};
   const size_t rows = (size_t)g.rows();
   if (tc_mlp_bwd_supported(g)) {
-    // hybrid path (bf16 activations, hidden factor 1): transforms as fp32 FFTs, rows B1 (second half) and B3-B7 on
+    // hybrid path (bf16 activations, hidden factors 1..8): transforms as fp32 FFTs, rows B1 (second half) and B3-B7 on
     // the tensor cores (tc_mlp_bwd, tc_wgrad), GX replaces G in place
     uint8_t* mk1 = g.export_masks ? (uint8_t*)ws : nullptr;
     uint8_t* mk2 = g.export_masks ? (uint8_t*)ws + m2off : nullptr;

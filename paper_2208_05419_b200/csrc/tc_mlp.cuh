@@ -394,6 +394,7 @@ constexpr uint32_t kMlpHfSmem = 4 * kWBytes + 2 * kMlpABytes;   // 172,800
 __global__ void k_tc_prep_weights_hf(const float* __restrict__ w1, const float* __restrict__ b1, const float* __restrict__ w2,
                                      const float* __restrict__ b2, __nv_bfloat16* __restrict__ out, float* __restrict__ bout,
                                      int nb, int hf) {
+  pdl_launch_dependents();   // the MLP kernel behind it sets itself up meanwhile; it waits (pdl_wait) before it reads the images
   const int hid = hf * BS;
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx < nb * hid) {           // b1 is [nb][hid][2]

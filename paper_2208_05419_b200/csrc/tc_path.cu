@@ -393,7 +393,8 @@ cudaError_t tc_mlp_forward(const Geometry& g, void* X, bool spec16, const float*
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
-// hybrid backward (hidden factor 1): rows B1 (second half), B3-B7 between the fp32 FFT kernels of generic.cu.
+// hybrid backward (hidden factor 1 here; 2..8, with blocks of 96, through tc_mlp_backward_hf below): rows B1 (second half),
+// B3-B7 between the fp32 FFT kernels of generic.cu.
 // X = spectrum of x, G = alpha-weighted spectrum of dY (replaced by GX); the parameter gradients go through the same
 // tc_wgrad + k_tc_wgrad_reduce launches as the fused path, over tiles of 96 consecutive spectrum rows.
 bool tc_mlp_bwd_supported(const Geometry& g) { return tc_mlp_supported(g); }

@@ -154,7 +154,7 @@ tc_wgrad(const __nv_bfloat16* __restrict__ A_l2, const __nv_bfloat16* __restrict
 // USE_CONTEXT (`guard`): the last kernel of the call also checks the context header the forward call left against
 // this call's descriptor; on a mismatch (context never saved, other geometry / flag set) the gradients become NaN
 // here and the grid overwrites dx with NaN (a foreign context must not return plausible numbers).
-__global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __restrict__ dW2, float2* __restrict__ dB2,
+__global__ void k_tc_wgrad_reduce(const float* part, float2* __restrict__ dW2, float2* __restrict__ dB2,
                                   float2* __restrict__ dW1, float2* __restrict__ dB1, int ngroups, int S, int bs, int C,
                                   int accumulate, int guard, const CtxHeader* __restrict__ got, const CtxHeader want,
                                   uint16_t* __restrict__ dx, size_t n_act, int wait_first) {
@@ -162,6 +162,10 @@ __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __rest
   // wait_first = 0 (fused path): the kernel before this one in the stream is tc_wdft_inv2, which lets its dependents
   // start only after ITS prerequisites (tc_wgrad among them) have completed: the partial sums are final, and the
   // sums below run under the inverse transform; only the guard's overwrite of dx has to wait for it.
+  // PTX promises visibility of a prerequisite grid's writes only to the grid that executes griddepcontrol.wait, and
+  // this grid reads `part` BEFORE its own wait: the reads therefore go to L2 (ld.global.cg, __ldcg below), where
+  // tc_wgrad's bulk stores / bulk reductions land, never through the non-coherent path or a stale L1 line, and
+  // `part` is not declared __restrict__ (S5.3 states the reliance).
   if (wait_first) pdl_wait();
   bool ok = true;
   if (guard) {
@@ -185,8 +189,8 @@ __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __rest
       const float* P = lpart + (size_t)(j * S + s) * kWgPartFloats;
       const float* Pre = P + (size_t)i * kWgPitch;
       const float* Pim = P + (size_t)(kWgRowsRe + i) * kWgPitch;
-      acc.x += Pre[o] + Pim[BS + o];
-      acc.y += Pre[BS + o] - Pim[o];
+      acc.x += __ldcg(Pre + o) + __ldcg(Pim + BS + o);
+      acc.y += __ldcg(Pre + BS + o) - __ldcg(Pim + o);
     }
     dW[idx] = ok ? acc : make_float2(poison, poison);
   } else if (idx < nW + C) {
@@ -194,8 +198,8 @@ __global__ void k_tc_wgrad_reduce(const float* __restrict__ part, float2* __rest
     float2 acc = accumulate ? dB[k] : make_float2(0.f, 0.f);
     for (int s = 0; s < S; ++s) {
       const float* P = lpart + (size_t)(j * S + s) * kWgPartFloats + (size_t)BS * kWgPitch;
-      acc.x += P[o];
-      acc.y += P[BS + o];
+      acc.x += __ldcg(P + o);
+      acc.y += __ldcg(P + BS + o);
     }
     dB[k] = ok ? acc : make_float2(poison, poison);
   }

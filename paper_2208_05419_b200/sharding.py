@@ -74,10 +74,21 @@ class GradBucket:
         flat = torch.zeros(total, dtype=torch.float32, device=device)
         return cls(flat, [flat[o:o + n].view(s) for (o, n), s in zip(offs, shapes)])
 
-    def all_reduce(self, dist, group=None):
-        """Sum over the data-parallel ranks; enqueued on the current stream (NCCL) / blocking (gloo)."""
+    def all_reduce(self, dist, group=None, stream=None):
+        """Sum over the data-parallel ranks: NCCL enqueues it, gloo blocks.
+
+        `stream`: the stream the gradients were written on (torch.cuda.Stream or a raw handle).  torch.distributed orders
+        an NCCL collective only against torch's CURRENT stream, so the collective is issued with `stream` made current:
+        it then runs behind the backward kernels that fill the bucket, whichever stream the caller has current.  None =
+        the caller's current stream (right only when the backward was enqueued there)."""
         if dist is not None and dist.get_world_size(group) > 1:
-            dist.all_reduce(self.flat, op=dist.ReduceOp.SUM, group=group)
+            if stream is not None and getattr(self.flat, "is_cuda", False):
+                import torch
+                s = torch.cuda.ExternalStream(stream) if isinstance(stream, int) else stream
+                with torch.cuda.stream(s):
+                    dist.all_reduce(self.flat, op=dist.ReduceOp.SUM, group=group)
+            else:
+                dist.all_reduce(self.flat, op=dist.ReduceOp.SUM, group=group)
         return self.views
 
 
@@ -90,12 +101,13 @@ def data_parallel_step(binding, desc_local, x, dy, params, y, dx, bucket: GradBu
     """One training step of the layer on this rank's samples, then ONE all-reduce of the parameter gradients.
 
     desc_local: descriptor with B = this rank's sample count.  The forward saves its context in `ws`, the backward
-    reads it (S1).  Returns the launch count of the two calls."""
+    reads it (S1).  `stream` (None = the current stream) carries all three: forward, backward and the
+    collective.  Returns the launch count of the two calls."""
     d_f = binding.Desc(**{**desc_local.__dict__, "flags": desc_local.flags | binding.FLAG_SAVE_CONTEXT})
     d_b = binding.Desc(**{**desc_local.__dict__, "flags": desc_local.flags | binding.FLAG_USE_CONTEXT})
     binding.afno_spectral_fwd(d_f, x, *params, y, ws, stream)
     n = binding.afno_last_launch_count()
     binding.afno_spectral_bwd(d_b, x, dy, *params, dx, *bucket.views, ws, stream)
     n += binding.afno_last_launch_count()
-    bucket.all_reduce(dist, group)
+    bucket.all_reduce(dist, group, stream)     # on `stream`, behind the backward, not on whatever stream is current
     return n

@@ -120,11 +120,17 @@ def preactivation_scales(cfg, dump, w1, b1, w2, b2, bf16=True):
         ~ u * rms_r |Xh[:,kw,c]| (the H transform against a rounded matrix spreads column kw's energy over
         its rows: a DFT is normwise, not componentwise, accurate), a part ~ u * rms_kw |Xh[r,:,c]| (the same
         for the W transform: its error is a random combination of the field's rows, so after the H transform
-        it sits in the rows r where the field has energy, at every kw) and a plane-wide floor:
-            var_X = u^2 (|Xh|^2 + 2 colms[kw,c] + 2 rowms[r,c] + planems[c])
-      * P1[o] = sum_i Xh[i] W1[i,o] + b1:  var_1[o] = sum_i |W1[i,o]|^2 (var_X[i] + u^2 |Xh[i]|^2)
-      * O1 = relu(P1) rounded:             var_O[i] = var_1[i] + u^2 |O1[i]|^2
-      * P2[o] = sum_i O1[i] W2[i,o] + b2:  var_2[o] = sum_i |W2[i,o]|^2 (var_O[i] + u^2 |O1[i]|^2)
+        it sits in the rows r where the field has energy, at every kw), a plane-wide floor, and a leak term: the
+        rounding errors of a DFT matrix are not random, a strong line leaks coherently into the bins harmonically
+        related to it, so LEAK times the largest line of the column and of the row enters whole.  With the second
+        rounding of Xh (as the bf16 operand of layer 1) folded in, the code below uses
+            var_X = u^2 (2 |Xh|^2 + 2 colms[kw,c] + 2 rowms[r,c] + planems[c] + LEAK (colmax[kw,c] + rowmax[r,c]))
+      * P1[o] = sum_i Xh[i] W1[i,o] + b1:  var_1[o] = sum_i |W1[i,o]|^2 var_X[i]
+      * O1 = relu(P1), rounded once when stored and once as the operand of layer 2:
+                                           var_O[i] = var_1[i] + 2 u^2 |O1[i]|^2
+      * P2[o] = sum_i O1[i] W2[i,o] + b2:  var_2[o] = sum_i |W2[i,o]|^2 var_O[i]
+    The constants are hand-set, not fitted: TAU_K = 6 sigma, LEAK = 0.1, and for the fp32 path u = 16 ulp (U_F32, the
+    depth of the FFT); the worst flip observed on the bf16 path sits at 0.81 of the allowed distance.
     Returns sigma1 [B,H,Wh,nb*hid], sigma2 [B,H,Wh,C] (per real component: half the complex variance); a
     flipped mask is justified when the oracle's pre-activation lies within TAU_K sigma of its threshold."""
     nb, bs, hid = cfg.num_blocks, cfg.bs, cfg.hid

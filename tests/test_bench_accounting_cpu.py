@@ -52,3 +52,32 @@ def test_kernel_work_counts_compulsory_bytes_only():
 def test_whole_job_value_and_reference_line_shape():
     assert bench.whole_job_value(2, 4, 10, 5.0) == 2 * 4 * 10 / 5e-3
     assert np.isclose(bench.whole_job_value(1, 4, 20, 20 * 0.4568), 4 / 0.4568e-3)
+
+
+def test_executed_flops_count_groups_of_96_channels_not_blocks():
+    """32 blocks of 32 channels are 11 groups of 96 (the kernels' tile), not 32: the executed-FLOP figure of the paper's
+    channel structure follows the groups."""
+    wl = inputs.WORKLOADS["paper_ch_b2"]
+    assert (wl.C, wl.num_blocks) == (1024, 32)
+    _, Kw, _ = bench.kept_counts(wl)
+    exe = bench.executed_tensor_flops(wl.B, wl, Kw)
+    umma96 = 2.0 * 128 * 96 * 16
+    assert exe["tc_mix_fwd"] == 96 * umma96 * wl.B * Kw * 11
+    assert exe["tc_wdft_per_launch"] == 24 * umma96 * wl.B * wl.H * 11
+
+
+def test_stale_traffic_capture_is_never_quoted(tmp_path):
+    """The stored ncu DRAM-traffic table carries the hash of the kernel sources it was captured on; with another hash
+    in the tree every figure is None and the source string says so."""
+    p = tmp_path / "t.csv"
+    p.write_text("# src 0123456789abcdef\n# git abc1234\nkernel,bytes_per_launch\ntc_wdft_fwd,1000\ntc_mix_fwd,2000\n")
+    fresh = bench.TrafficTable(str(p), src_hash="0123456789abcdef")
+    assert fresh.get("tc_wdft_fwd") == 1000 and "stored" in fresh.source
+    assert fresh.step_total({"tc_wdft_fwd": (4, 0.1), "tc_mix_fwd": (2, 0.1)}, 2) == 2 * 1000 + 2000
+    stale = bench.TrafficTable(str(p), src_hash="ffffffffffffffff")
+    assert stale.rows == {} and stale.source.startswith("null:") and "ffffffffffffffff" in stale.source
+    assert stale.step_total({"tc_wdft_fwd": (4, 0.1)}, 2) is None
+    assert len(bench.kernel_source_hash()) == 16
+    # the committed table, whatever its state, never raises
+    t = bench.TrafficTable()
+    assert t.source is not None

@@ -721,6 +721,50 @@ def test_saved_context_step_is_bitwise_repeatable():
                 assert torch.equal(a, b), (it, k)
 
 
+def test_step_gradients_bitwise_under_concurrent_load():
+    """k_tc_wgrad_reduce sums tc_wgrad's partial sums before its own griddepcontrol.wait (it overlaps the inverse
+    transform; S5.3 states what it relies on).  40 saved-context steps enqueued back to back with no host
+    synchronisation, while a second stream keeps the SMs and the L2 busy with copies, must return the same bits as a
+    quiet step; every step writes its gradients to its own buffers."""
+    import torch
+    wl = inputs.WORKLOADS["fcn_b4_bwd"]
+    desc = parity.desc_for(wl, B=2)
+    d_save = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_SAVE_CONTEXT})
+    d_use = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_USE_CONTEXT})
+    binding.afno_plan_warmup(desc)
+    data = inputs.make_inputs(wl, B=2)
+    tx, tdy = parity.to_device_act(data["x"], True), parity.to_device_act(data["dy"], True)
+    p = parity.GpuLayer(desc).params(data["w1"], data["b1"], data["w2"], data["b2"])
+    ws = torch.empty(binding.afno_spectral_workspace_bytes(desc, True), dtype=torch.uint8, device="cuda")
+    ty, tdx = torch.empty_like(tx), torch.empty_like(tx)
+
+    def step(g):
+        binding.afno_spectral_fwd(d_save, tx, *p, ty, ws)
+        binding.afno_spectral_bwd(d_use, tx, tdy, *p, tdx, *g, ws)
+
+    quiet = [torch.empty_like(t) for t in p]
+    step(quiet)
+    torch.cuda.synchronize()
+    N = 40
+    outs = [[torch.full_like(t, float("nan")) for t in p] for _ in range(N)]
+    src = torch.empty(256 << 20, dtype=torch.uint8, device="cuda").fill_(3)
+    dst = torch.empty_like(src)
+    side = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        for _ in range(60):
+            dst.copy_(src)
+            src.add_(1)
+    for it in range(N):
+        step(outs[it])
+    busy = not side.query()      # the load should still be running when the last step has been enqueued
+    torch.cuda.synchronize()
+    print(f"[load] side stream still busy after enqueueing {N} steps: {busy}")
+    for it in range(N):
+        for k, (a, b) in enumerate(zip(quiet, outs[it])):
+            assert torch.equal(a, b), (it, k)
+
+
 def test_host_variants_match_device(oracle):
     import torch
     wl = inputs.WORKLOADS["sub_bwd_nb8"]
@@ -785,6 +829,63 @@ def test_host_variants_tcgen05(oracle):
     assert np.array_equal(hy.float().numpy(), y_dev)
 
 
+def test_bwd_host_without_x_needs_an_arena_that_holds_it():
+    """afno_spectral_bwd_host(x_host = NULL) reuses the x a host call left in the arena.  An arena no host call has
+    written, or one that holds x of another shape, is refused (AFNO_ERR_INVALID_ARG) instead of yielding dx and gradients
+    of whatever bytes sit there; after a fwd_host with the same descriptor the call goes through.  The host calls of
+    a short-lived thread work too (its copy streams and events are released with the thread)."""
+    import threading
+    import torch
+    wl = inputs.Workload(4, "30x60x192 bf16 B=2", 2, 30, 60, 192, 2, 1, 0.01, 1.0, "bf16", True, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    desc1 = parity.desc_for(wl, B=1)
+    pin_act = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(torch.bfloat16).pin_memory()
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
+    hx, hdy = pin_act(data["x"]), pin_act(data["dy"])
+    hp = [pin(data[k]) for k in ("w1", "b1", "w2", "b2")]
+    hy, hdx = torch.empty_like(hx).pin_memory(), torch.empty_like(hx).pin_memory()
+    hg = [torch.empty_like(t).pin_memory() for t in hp]
+    nbytes = max(binding.afno_spectral_host_arena_bytes(desc, m) for m in (0, 1, 2))
+    for fill in (0, 0x4F):      # a zeroed arena and one full of bytes that occur in the stamp's magic
+        arena = torch.full((nbytes,), fill, dtype=torch.uint8, device="cuda")
+        with pytest.raises(binding.AfnoError) as ei:
+            binding.afno_spectral_bwd_host(desc, None, hdy, *hp, hdx, *hg, arena)
+        assert ei.value.status == binding.AFNO_ERR_INVALID_ARG and "x_host is NULL" in str(ei.value)
+    binding.afno_spectral_fwd_host(desc, hx, *hp, hy, arena)
+    binding.afno_spectral_bwd_host(desc, None, hdy, *hp, hdx, *hg, arena)
+    ref_dx = hdx.clone()
+    # x of two samples is there; a call that expects one sample's x must not take it
+    with pytest.raises(binding.AfnoError) as ei:
+        binding.afno_spectral_bwd_host(desc1, None, hdy[:1], *hp, hdx[:1], *hg, arena)
+    assert ei.value.status == binding.AFNO_ERR_INVALID_ARG
+    # bwd_host with an x of its own leaves that x behind, step_host too
+    binding.afno_spectral_bwd_host(desc1, hx[:1], hdy[:1], *hp, hdx[:1], *hg, arena)
+    binding.afno_spectral_bwd_host(desc1, None, hdy[:1], *hp, hdx[:1], *hg, arena)
+    assert torch.equal(hdx[:1], ref_dx[:1])
+    binding.afno_spectral_step_host(desc, hx, hdy, *hp, hy, hdx, *hg, arena)
+    binding.afno_spectral_bwd_host(desc, None, hdy, *hp, hdx, *hg, arena)
+    assert torch.equal(hdx, ref_dx)
+
+    errs = []
+
+    def worker():
+        try:
+            torch.cuda.set_device(0)
+            out = torch.empty_like(hx).pin_memory()
+            binding.afno_spectral_fwd_host(desc, hx, *hp, out, arena, stream=torch.cuda.current_stream())
+            assert torch.equal(out, hy)
+        except Exception as ex:      # surfaced below: an exception in a thread does not fail the test by itself
+            errs.append(ex)
+
+    for _ in range(8):
+        t = threading.Thread(target=worker)
+        t.start()
+        t.join()
+    assert not errs, errs
+    torch.cuda.synchronize()
+
+
 def test_w192_runs_on_the_generic_path(oracle):
     """W = 192 has W/2+1 = 97 bins: one more than the tcgen05 path's constant images hold.  The plan must be
     built without touching them (round-1 advisor finding: heap overflow in tc_build_plan) and the
@@ -826,6 +927,51 @@ def test_data_parallel_step_with_gradient_bucket(oracle):
     assert np.array_equal(parity.from_device_act(ty), ref["y"]) and np.array_equal(parity.from_device_act(tdx), ref["dx"])
     for v, k in zip(bucket.views, ("dw1", "db1", "dw2", "db2")):
         assert np.array_equal(v.cpu().numpy(), ref[k]), k
+
+
+def test_data_parallel_step_on_a_side_stream_orders_the_collective_behind_the_backward():
+    """The all-reduce must ride on the stream the backward wrote the bucket on, not on torch's current stream (NCCL orders
+    against the current stream only).  One GPU cannot run a 2-rank NCCL group, so the process group is a stand-in that
+    reports two ranks and 'reduces' by doubling the bucket on whatever stream is current when it is called: issued on
+    the wrong stream it would both trip the assertion and race with k_tc_wgrad_reduce."""
+    import torch
+    from paper_2208_05419_b200 import sharding
+    wl = inputs.Workload(4, "30x60x192 bf16 B=2 dp", 2, 30, 60, 192, 2, 1, 0.01, 1.0, "bf16", True, False)
+    data = inputs.make_inputs(wl)
+    desc = parity.desc_for(wl)
+    ref = _ctx_step(desc, data)
+    layer = parity.GpuLayer(desc)
+    tx, tdy = parity.to_device_act(data["x"], True), parity.to_device_act(data["dy"], True)
+    ty, tdx = torch.empty_like(tx), torch.empty_like(tx)
+    p = layer.params(data["w1"], data["b1"], data["w2"], data["b2"])
+    ws = torch.empty(binding.afno_spectral_workspace_bytes(desc, True), dtype=torch.uint8, device="cuda")
+    side = torch.cuda.Stream()
+
+    class TwoRanks:
+        class ReduceOp:
+            SUM = "sum"
+        seen = []
+
+        @staticmethod
+        def get_world_size(group=None):
+            return 2
+
+        @classmethod
+        def all_reduce(cls, t, op=None, group=None):
+            cls.seen.append(torch.cuda.current_stream().cuda_stream)
+            t.mul_(2.0)      # two ranks holding the same gradients
+
+    for handle in (side, side.cuda_stream):     # a torch stream and the raw handle the C ABI takes
+        bucket = sharding.GradBucket.allocate(wl.num_blocks, wl.C // wl.num_blocks, 1, device="cuda")
+        torch.cuda.synchronize()
+        assert torch.cuda.current_stream().cuda_stream != side.cuda_stream
+        sharding.data_parallel_step(binding, desc, tx, tdy, p, ty, tdx, bucket, ws, handle, dist=TwoRanks)
+        assert TwoRanks.seen[-1] == side.cuda_stream      # raw handles: torch stream objects do not compare reliably
+        assert torch.cuda.current_stream().cuda_stream != side.cuda_stream
+        torch.cuda.synchronize()
+        assert np.array_equal(parity.from_device_act(tdx), ref["dx"])
+        for v, k in zip(bucket.views, ("dw1", "db1", "dw2", "db2")):
+            assert np.array_equal(v.cpu().numpy(), 2.0 * ref[k]), k
 
 
 def test_p1_token_grid_fp32_forward(oracle):

@@ -601,6 +601,151 @@ def kernel_roofline(name, n_launch, total_ms, steps, work, exe, peaks, traffic, 
     return out
 
 
+# ---- the other configurations of BASELINE.json and SURVEY.md S8(f): `bench.py --workload NAME` -----------------------
+# name -> (what it is, B, H, W, C, num_blocks, hidden_factor, kept_fraction, dtype, backward, saved context)
+WORKLOAD_TABLE = {
+    "fcn_b1": ("BASELINE.json configs[1]: 90x180x768 bf16 fwd B=1", 1, 90, 180, 768, 8, 1, 1.0, "bf16", False, False),
+    "fcn_b8": ("BASELINE.json configs[2]: 90x180x768 bf16 fwd B=8, kept 1.0", 8, 90, 180, 768, 8, 1, 1.0, "bf16", False, False),
+    "fcn_b8_half": ("BASELINE.json configs[2]: 90x180x768 bf16 fwd B=8, kept 0.5", 8, 90, 180, 768, 8, 1, 0.5, "bf16", False, False),
+    "hires_b2": ("BASELINE.json configs[3]: 180x360x768 bf16 fwd B=2 (hybrid path)", 2, 180, 360, 768, 8, 1, 1.0, "bf16", False, False),
+    "fcn_b4_fwd": ("90x180x768 bf16 fwd B=4", 4, 90, 180, 768, 8, 1, 1.0, "bf16", False, False),
+    "fcn_b4_bwd_stateless": ("BASELINE.json configs[4] with the stateless backward (recomputes the spectrum of x)", 4, 90, 180, 768, 8, 1, 1.0, "bf16", True, False),
+    "fcn_b8_bwd": ("90x180x768 bf16 fwd+bwd B=8, saved context", 8, 90, 180, 768, 8, 1, 1.0, "bf16", True, True),
+    "paper_ch_b4": ("paper channel structure 90x180x1024, 32 blocks of 32, fwd B=4", 4, 90, 180, 1024, 32, 1, 1.0, "bf16", False, False),
+    "paper_ch_b4_bwd": ("paper channel structure 90x180x1024, 32 blocks of 32, fwd+bwd B=4, saved context", 4, 90, 180, 1024, 32, 1, 1.0, "bf16", True, True),
+    "hires_b2_bwd": ("180x360x768 bf16 fwd+bwd B=2 (hybrid path)", 2, 180, 360, 768, 8, 1, 1.0, "bf16", True, False),
+    "paper_shape_b2": ("paper layer shape 180x360x1024, 32 blocks of 32, fwd B=2 (hybrid path)", 2, 180, 360, 1024, 32, 1, 1.0, "bf16", False, False),
+    "paper_shape_b1_bwd": ("paper layer shape 180x360x1024, 32 blocks of 32, fwd+bwd B=1 (hybrid path)", 1, 180, 360, 1024, 32, 1, 1.0, "bf16", True, False),
+    "hf2_b4": ("hidden factor 2, 90x180x768 bf16 fwd B=4 (hybrid path)", 4, 90, 180, 768, 8, 2, 1.0, "bf16", False, False),
+    "hf2_b4_bwd": ("hidden factor 2, 90x180x768 bf16 fwd+bwd B=4 (hybrid path)", 4, 90, 180, 768, 8, 2, 1.0, "bf16", True, False),
+    "fp32_b2_bwd": ("fp32 activations 90x180x768 fwd+bwd B=2 (generic fp32 path)", 2, 90, 180, 768, 8, 1, 1.0, "f32", True, False),
+    "p1_b1": ("p -> 1 token grid 720x1440x768 bf16 fwd B=1 (hybrid path)", 1, 720, 1440, 768, 8, 1, 1.0, "bf16", False, False),
+    "p1_b1_bwd": ("p -> 1 token grid 720x1440x768 bf16 fwd+bwd B=1 (hybrid path)", 1, 720, 1440, 768, 8, 1, 1.0, "bf16", True, False),
+}
+
+
+def workload_roofline(B, H, W, C, nb, hf, f, f32, backward):
+    """2-term layer roofline of any configuration (SURVEY.md S8(d)): compulsory bytes (x in, y out; x, dy in, dx out;
+    parameters in, gradients out) and the model FLOPs of the block MLP (2 GEMMs forward, 4 more backward)."""
+    bs = C // nb
+    hid = bs * hf
+    a_bytes = B * H * W * C * (4 if f32 else 2)
+    pbytes = 2 * (nb * bs * hid * 2 + (hid + bs) * nb) * 4
+    nbytes = (2 * a_bytes + pbytes) + ((3 * a_bytes + 2 * pbytes) if backward else 0)
+    Kh = max(1, min(H // 2 + 1, int(np.floor(float(np.float32(f)) * (H // 2 + 1)))))
+    Kw = max(1, min(W // 2 + 1, int(np.floor(float(np.float32(f)) * (W // 2 + 1)))))
+    kept = (2 * Kh - 1 if Kh <= H // 2 else H) * Kw
+    gemm = 2 * (2 * bs) * (2 * hid) * nb * kept * B
+    return nbytes, 2 * gemm + (4 * gemm if backward else 0)
+
+
+def run_workload(args):
+    """One of the other configurations through the C ABI, same JSON line as the headline (single GPU; inputs resident in
+    HBM and rotated over buffer sets larger than the L2; EXACTLY --steps steps between two CUDA events after --warmup
+    warm-up steps).  No e2e / cpu_baseline legs: they belong to the headline run."""
+    import torch
+
+    from paper_2208_05419_b200 import binding
+
+    if int(os.environ.get("WORLD_SIZE", "1")) != 1 or args.gpus != 1:
+        raise SystemExit("bench.py --workload other than the headline runs on one GPU")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the AFNO path has no CPU fallback")
+    what, B, H, W, C, nb, hf, f, dtype, backward, ctx = WORKLOAD_TABLE[args.workload]
+    f32 = dtype == "f32"
+    peaks = _peaks()
+    adt = torch.float32 if f32 else torch.bfloat16
+    desc = binding.Desc(B, H, W, C, nb, hf, 0.01, f, binding.AFNO_F32 if f32 else binding.AFNO_BF16, 0)
+    binding.afno_plan_warmup(desc)
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    g = torch.Generator(device="cuda").manual_seed(220805419)
+    act = B * H * W * C
+    nsets = int(np.ceil(300e6 / (act * (4 if f32 else 2) * (4 if backward else 2))))
+    nsets = min(max(2, nsets), 8)
+    bs, hid = C // nb, (C // nb) * hf
+    sets = []
+    for _ in range(nsets):
+        s = dict(x=torch.randn((B, H, W, C), device=dev, generator=g).to(adt), y=torch.empty((B, H, W, C), device=dev, dtype=adt))
+        if backward:
+            s["dy"] = torch.randn((B, H, W, C), device=dev, generator=g).to(adt)
+            s["dx"] = torch.empty_like(s["x"])
+        sets.append(s)
+    params = [0.02 * torch.randn(shape, device=dev, generator=g) for shape in
+              [(nb, bs, hid, 2), (nb, hid, 2), (nb, hid, bs, 2), (nb, bs, 2)]]
+    grads = [torch.empty_like(p) for p in params]
+    desc_f = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_SAVE_CONTEXT if ctx else 0})
+    desc_b = binding.Desc(**{**desc.__dict__, "flags": binding.FLAG_USE_CONTEXT if ctx else 0})
+    ws = torch.empty(max(16, binding.afno_spectral_workspace_bytes(desc_f, backward)), dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    launches = [0]
+
+    def step(i):
+        s = sets[i % nsets]
+        binding.afno_spectral_fwd(desc_f, s["x"], *params, s["y"], ws, stream)
+        launches[0] = binding.afno_last_launch_count()
+        if backward:
+            binding.afno_spectral_bwd(desc_b, s["x"], s["dy"], *params, s["dx"], *grads, ws, stream)
+            launches[0] += binding.afno_last_launch_count()
+
+    for i in range(args.warmup):
+        step(i)
+    torch.cuda.synchronize()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    with ClockSampler(0) as clocks:
+        evs[0].record(stream)
+        for i in range(args.steps):
+            step(i)
+            evs[i + 1].record(stream)
+        torch.cuda.synchronize()
+    ms = evs[0].elapsed_time(evs[-1])
+    per_step = np.array([evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)])
+    ms_per_step = ms / args.steps
+    binding.afno_profile_start()
+    PROF_STEPS = max(2, min(args.steps, 3))
+    for i in range(PROF_STEPS):
+        step(i)
+    prof = binding.afno_profile_stop()
+    nbytes, flops = workload_roofline(B, H, W, C, nb, hf, f, f32, backward)
+    t_step = ms_per_step * 1e-3
+    t_hbm, t_tensor = nbytes / (peaks["hbm_gbs"] * 1e9), flops / (peaks["tensor_tflops"] * 1e12)
+    hbm_bound = t_hbm >= t_tensor
+    dom = max(prof, key=lambda k: prof[k][1])
+    line = {
+        "metric": f"afno_spectral_{'fwd_bwd' if backward else 'fwd'}_samples_per_s_{H}x{W}x{C}_{dtype}",
+        "value": B * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if f32 else "bf16", "data": "synthetic N(0,1) activations and 0.02 N(0,1) parameters drawn on the device (seeded)",
+        "ms_per_step_median": float(np.median(per_step)), "ms_per_step_best": float(per_step.min()),
+        "config": {"workload": f"{args.workload}: {what}", "B_per_gpu": B, "H": H, "W": W, "C": C, "num_blocks": nb,
+                   "hidden_factor": hf, "lambda": 0.01, "kept_fraction": f, "path": binding.afno_spectral_path(desc),
+                   "backward": ("saved context" if ctx else "stateless") if backward else "none (forward only)",
+                   "parallelism": "single GPU",
+                   "l2": f"{nsets} rotating buffer sets of {(4 if backward else 2) * act * (4 if f32 else 2) / 1e6:.0f} MB "
+                         "(together > 126 MB L2), no explicit flush"},
+        "clocks": clocks.summary(),
+        "e2e": None, "e2e_note": "the host-buffer leg is measured on the headline workload (python bench.py)",
+        "gpu_launches": launches[0] * args.steps,
+        "roofline": {
+            "scope": "layer: all launches of one step (SURVEY.md S8(d) 2-term roofline of this shape)",
+            "bound": "hbm" if hbm_bound else "tensor",
+            "achieved": (nbytes / t_step / 1e9) if hbm_bound else (flops / t_step / 1e12),
+            "peak": peaks["hbm_gbs"] if hbm_bound else peaks["tensor_tflops"], "unit": "GB/s" if hbm_bound else "TFLOP/s",
+            "frac": max(t_hbm, t_tensor) / t_step, "traffic": None,
+            "traffic_source": "null: no ncu DRAM capture is stored for this workload",
+            "algorithmic_bytes_per_step": nbytes, "mlp_flops_model_per_step": flops,
+            "t_roof_us_per_step": 1e6 * max(t_hbm, t_tensor),
+            "peaks": f"{peaks['hbm_gbs']} GB/s copy, {peaks['tensor_tflops']} TFLOP/s bf16 burst ({peaks['source']}, MEASURED_PEAKS.json)",
+            "dominant_kernel": {"kernel": dom, "ms_per_step": prof[dom][1] / PROF_STEPS, "launches_per_step": prof[dom][0] / PROF_STEPS},
+            "kernels_ms_per_step": {k: round(v[1] / PROF_STEPS, 4) for k, v in sorted(prof.items())},
+        },
+        "cuda_graph": None,
+        "cpu_baseline": None, "cpu_baseline_note": "skipped: the oracle leg is timed on the headline workload (python bench.py)",
+    }
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -610,6 +755,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--write-traffic", metavar="RAW_CSV", default=None,
                     help="no benchmark: turn ncu's raw page of a --timed-only capture into " + TRAFFIC_CSV)
+    ap.add_argument("--workload", default=WL_NAME, choices=[WL_NAME] + sorted(WORKLOAD_TABLE),
+                    help="default: the BASELINE.json headline (configs[4], fwd+bwd B=4 at 90x180x768 bf16); the other names "
+                         "time the remaining BASELINE.json configs and the SURVEY.md S8(f) shapes (single GPU, same JSON line)")
     ap.add_argument("--timed-only", action="store_true",
                     help="warm-up, the timed steps and the per-kernel event pass only (no CUDA-graph replay, e2e or "
                          "cpu_baseline legs): the command the ncu captures under profiles/ run")
@@ -627,6 +775,8 @@ def main():
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload != WL_NAME:
+        return run_workload(args)
     return run_ours(args)
 
 

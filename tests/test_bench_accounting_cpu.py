@@ -81,3 +81,23 @@ def test_stale_traffic_capture_is_never_quoted(tmp_path):
     # the committed table, whatever its state, never raises
     t = bench.TrafficTable()
     assert t.source is not None
+
+
+def test_workload_table_is_valid_and_its_roofline_agrees_with_the_headline_accounting():
+    """Every `bench.py --workload` entry is a descriptor the C ABI accepts (host-side check, no GPU), and the generic
+    roofline formula reproduces the headline's hand-derived figures."""
+    from paper_2208_05419_b200 import binding
+    for name, (what, B, H, W, C, nb, hf, f, dtype, backward, ctx) in bench.WORKLOAD_TABLE.items():
+        d = binding.Desc(B, H, W, C, nb, hf, 0.01, f, binding.AFNO_F32 if dtype == "f32" else binding.AFNO_BF16, 0)
+        path = binding.afno_spectral_path(d)
+        assert path is not None, name
+        assert ("hybrid" in what) == (path == "hybrid-fft32-tcgen05"), (name, path)
+        assert not ctx or backward, name
+    wl = inputs.WORKLOADS[bench.WL_NAME]
+    _, _, kept = bench.kept_counts(wl)
+    work = bench.layer_work(wl.B, wl.H, wl.W, wl.C, wl.num_blocks, kept)
+    assert bench.workload_roofline(wl.B, wl.H, wl.W, wl.C, wl.num_blocks, 1, wl.kept_fraction, False, True) == (
+        work["bytes"], work["flops_model"])
+    # forward only: x in, y out, parameters in; two block GEMMs
+    nbytes, flops = bench.workload_roofline(1, 90, 180, 768, 8, 1, 1.0, False, False)
+    assert nbytes == 2 * 90 * 180 * 768 * 2 + work["params"] and flops == 2 * work["gemm"] // 4
